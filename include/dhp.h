@@ -1,0 +1,176 @@
+/*
+ * dhp.h — C ABI of libdhp.so: the ANI-2x-style neural-network potential of Deep-HP
+ * (arXiv 2207.14276) as hand-written sm_100a CUDA.  One call evaluates the whole hot path
+ *   neighbour search -> AEV (Eqs. 3-5) -> per-element MLP ensemble (Eq. 2) -> analytic forces.
+ *
+ * The interface restates the paper's own boundary (§2.2.1-2.2.2):
+ *   - the MD engine stays the master and passes DEVICE addresses, no host copies (L128);
+ *   - "provides positions and neighbor lists and gets energies and forces in return" (L130);
+ *   - buffers are reserved once, proportional to N, never on the hot call (L134).
+ *
+ * Conventions
+ *   - All functions return 0 (DHP_OK) or a negative DHP_E_* code; nothing throws or aborts.
+ *   - "dev" pointers are CUDA device pointers valid on the device current at dhp_create();
+ *     "host" pointers are ordinary host memory.  The caller owns every buffer it passes in.
+ *   - The library owns the context, its workspace, neighbour lists and weight handles; they die with
+ *     dhp_destroy().  A dhp_nlist is valid until the next dhp_nlist_build / dhp_ani_energy_forces
+ *     on the same context.
+ *   - Hot calls (dhp_nlist_build, dhp_ani_energy_forces) only enqueue work on the context's stream:
+ *     no allocation, no host synchronisation.  Data-dependent faults (species outside 0..6, neighbour
+ *     capacity overflow) set a device-side status word, read with dhp_status().
+ *   - Units are the caller's: Å in, Hartree and Hartree/Å out (F = -dE/dr); no conversion inside.
+ *   - Species index 0..6 = H, C, N, O, S, F, Cl.  The shape is fixed at compile time:
+ *     16 radial shifts, 8 x 4 angular shifts, AEV length 7*16 + 28*32 = 1008,
+ *     networks 1008 -> 256 -> 192 -> 160 -> 1 with CELU (BASELINE.json configs[0]).
+ */
+#ifndef DHP_H
+#define DHP_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DHP_N_SPECIES 7
+#define DHP_N_SHF_R 16
+#define DHP_N_SHF_A 8
+#define DHP_N_SHF_Z 4
+#define DHP_AEV_DIM 1008
+#define DHP_NET_PARAMS 338689 /* 1008*256+256 + 256*192+192 + 192*160+160 + 160+1 */
+
+enum {
+    DHP_OK = 0,
+    DHP_E_BADARG = -1,   /* null pointer, negative size, n_models mismatch                       */
+    DHP_E_CAPACITY = -2, /* n_atoms > max_atoms, n_mol > max_mols, or neighbour storage overflow  */
+    DHP_E_BOX = -3,      /* a periodic edge is < 2*rc: the minimum image would not be unique      */
+    DHP_E_SPECIES = -4,  /* a species index outside 0..6 (reported by dhp_status)                 */
+    DHP_E_NOTIMPL = -5,
+    DHP_E_CUDA = -6,     /* a CUDA runtime call failed; dhp_last_cuda_error() has the text        */
+    DHP_E_NOMEM = -7
+};
+
+/* AEV hyper-parameters (Eqs. 3-5).  NULL in dhp_create = values of
+ * BASELINE.json configs[0]: Rcr 5.1, Rca 3.5, EtaR 19.7, EtaA 12.5, Zeta 14.1, CELU alpha 0.1,
+ * ShfR = 0.8 + 0.2625 m, ShfA = 0.8 + 0.3375 a, ShfZ = (2k+1) pi/8. */
+typedef struct dhp_params {
+    float rcr;        /* radial cutoff R_c of Eq. 3 used in Eq. 4, Å          */
+    float rca;        /* angular cutoff R_c of Eq. 3 used in Eq. 5, Å, <= rcr  */
+    float eta_r;      /* eta of Eq. 4, Å^-2                                    */
+    float eta_a;      /* eta of Eq. 5, Å^-2                                    */
+    float zeta;       /* xi of Eq. 5                                           */
+    float celu_alpha; /* CELU(x) = x (x>0), alpha (exp(x/alpha) - 1) otherwise */
+    float shf_r[DHP_N_SHF_R]; /* R_s of Eq. 4, Å   */
+    float shf_a[DHP_N_SHF_A]; /* R_s of Eq. 5, Å   */
+    float shf_z[DHP_N_SHF_Z]; /* theta_s of Eq. 5  */
+} dhp_params;
+
+typedef struct dhp_ctx dhp_ctx;         /* workspace sized for max_atoms, bound to one CUDA stream */
+typedef struct dhp_nlist dhp_nlist;     /* device-resident CSR pair list, owned by the context     */
+typedef struct dhp_weights dhp_weights; /* device-resident network parameters, owned by the context */
+
+/* MLP arithmetic, dhp_set_mlp_mode(): both meet the parity tolerances against the fp64 oracle. */
+enum {
+    DHP_MLP_AUTO = 0,   /* tensor path when available, else SIMT                                   */
+    DHP_MLP_SIMT = 1,   /* fp32 FFMA GEMMs                                                          */
+    DHP_MLP_TENSOR = 2  /* tcgen05 / TMEM GEMMs, fp16 two-term split operands, fp32 accumulate      */
+};
+
+/* Phases timed by dhp_profile_* (CUDA events on the context stream). */
+enum {
+    DHP_PHASE_NLIST = 0,   /* a1: binning, sort, CSR build                 */
+    DHP_PHASE_AEV_FWD = 1, /* a2                                           */
+    DHP_PHASE_MLP = 2,     /* a3 + a4: forward and transpose-backward GEMMs */
+    DHP_PHASE_AEV_BWD = 3, /* a5 + force un-permutation                    */
+    DHP_N_PHASES = 4
+};
+
+/* Create a context.  max_atoms / max_mols bound every later call (workspace is allocated here, once;
+ * PAPER.md L134).  cuda_stream is a cudaStream_t (NULL = legacy default stream); all work of this
+ * context is enqueued on it.  Errors: BADARG, NOMEM, CUDA. */
+int dhp_create(dhp_ctx** out, const dhp_params* params, int64_t max_atoms, int64_t max_mols, void* cuda_stream);
+int dhp_destroy(dhp_ctx* ctx);
+
+/* Upload network parameters.  blob: HOST or DEVICE pointer to fp32, layout
+ *   for e in 0..n_models-1: for s in 0..6: W1[256][1008], b1[256], W2[192][256], b2[192],
+ *                                           W3[160][192], b3[160], W4[1][160], b4[1]
+ * row-major [out][in]; n_floats must equal 338689*7*n_models.  The library keeps its own device copies
+ * (fp32 for the SIMT path, split fp16 tiles for the tensor path); the caller may free blob afterwards.
+ * Synchronises the stream (setup call, not a hot call).  Errors: BADARG, NOMEM, CUDA. */
+int dhp_weights_load(dhp_ctx* ctx, const float* blob, int64_t n_floats, int n_models, dhp_weights** out);
+int dhp_weights_free(dhp_ctx* ctx, dhp_weights* w);
+
+/* a1 — neighbour search (linked-cell partition -> "pair list of indices").
+ *   pos      dev fp32 [n_atoms][3], Å; may lie outside [0,L)
+ *   box      HOST fp32 [3] cubic/orthorhombic periodic edges, or NULL for open boundaries
+ *   species  dev int32 [n_atoms], 0..6
+ *   mol_offsets dev int32 [n_mol+1] or NULL: atoms of molecule m are [mol_offsets[m], mol_offsets[m+1]);
+ *            pairs never cross molecules (batched replicas); requires box == NULL
+ *   rc       radial cutoff (must equal params.rcr); the angular sub-list radius is params.rca
+ * A pair (i,j), i != j, is kept iff R^2 <= rc^2 with R^2 = (dx*dx + dy*dy) + dz*dz evaluated in fp64
+ * without FMA contraction on the exactly converted fp32 inputs, d -= L*rint(d/L) per periodic axis
+ * (Eq. 3's "R <= Rc").  The list is bit-exact, not approximately right.
+ * Errors: BADARG, CAPACITY, BOX (host-side checks); SPECIES / CAPACITY via dhp_status(). */
+int dhp_nlist_build(dhp_ctx* ctx, const float* pos, const float* box, const int32_t* species, int64_t n_atoms,
+                    const int32_t* mol_offsets, int64_t n_mol, float rc, dhp_nlist** out);
+
+/* Number of directed pairs in the radial (<= rcr) and angular (<= rca) lists.  Synchronises. */
+int dhp_nlist_sizes(dhp_ctx* ctx, const dhp_nlist* nl, int64_t* nnz, int64_t* nnz_ang);
+
+/* Canonical form for parity: caller's atom numbering, both directions, each row ascending in j.
+ * row_ptr / row_ptr_ang: dev int32 [n_atoms+1]; col / col_ang: dev int32 with room for nnz / nnz_ang
+ * entries (dhp_nlist_sizes).  Any of the two (row_ptr, col) pairs may be NULL.  Not a hot call. */
+int dhp_nlist_export(dhp_ctx* ctx, const dhp_nlist* nl, int32_t* row_ptr, int32_t* col,
+                     int32_t* row_ptr_ang, int32_t* col_ang);
+
+/* The hot call: a1..a5 in one go.  Builds its own pair list, then
+ *   E  dev fp64 [max(1, n_mol)]  total energy (per molecule when mol_offsets is given), Hartree:
+ *      E = (1/n_models) sum_e sum_i NN^{(e)}_{s_i}(G_i)            (Eq. 2; ensemble mean, L159)
+ *   F  dev fp32 [n_atoms][3]     F = -dE/dr, Hartree/Å, caller's atom order
+ * n_models must match the weight handle.  Asynchronous on the context stream. */
+int dhp_ani_energy_forces(dhp_ctx* ctx, const float* pos, const float* box, const int32_t* species,
+                          int64_t n_atoms, const int32_t* mol_offsets, int64_t n_mol,
+                          const dhp_weights* weights, int n_models, double* E, float* F);
+
+/* Same computation with HOST buffers (pos, species, mol_offsets, E, F all host; pinned memory makes
+ * the copies asynchronous): host->device copies, the kernels, device->host copies and one stream
+ * synchronisation all happen inside the call.  This is the end-to-end entry point bench.py times. */
+int dhp_ani_energy_forces_host(dhp_ctx* ctx, const float* pos, const float* box, const int32_t* species,
+                               int64_t n_atoms, const int32_t* mol_offsets, int64_t n_mol,
+                               const dhp_weights* weights, int n_models, double* E, float* F);
+
+/* Synchronises the stream and returns the device status word of the last hot call:
+ * DHP_OK, DHP_E_SPECIES, DHP_E_CAPACITY, or DHP_E_CUDA. */
+int dhp_status(dhp_ctx* ctx);
+
+int dhp_set_mlp_mode(dhp_ctx* ctx, int mode);
+/* 1 if this build and device can run the tcgen05 path (compute capability 10.x), else 0. */
+int dhp_tensor_path_available(dhp_ctx* ctx);
+
+/* Test-only exports, valid after a dhp_ani_energy_forces on the same context (synchronise):
+ *   dhp_debug_aev            dev fp32 [n_atoms][1008]  G_i, caller's atom order, layout radial [s_j][m]
+ *                            then angular [pairidx][a][z]
+ *   dhp_debug_grad           dev fp32 [n_atoms][1008]  dE/dG_i (ensemble mean)
+ *   dhp_debug_atomic_energy  dev fp32 [n_atoms]        E_i (ensemble mean) */
+int dhp_debug_aev(dhp_ctx* ctx, float* aev);
+int dhp_debug_grad(dhp_ctx* ctx, float* grad);
+int dhp_debug_atomic_energy(dhp_ctx* ctx, float* e_atom);
+
+/* Per-phase device timing.  dhp_profile_enable(ctx, 1) makes every hot call record CUDA events around
+ * each phase on the context stream; dhp_profile_read synchronises and returns, for the calls since the
+ * last dhp_profile_reset, the summed milliseconds per phase in ms[DHP_N_PHASES] and the call count. */
+int dhp_profile_enable(dhp_ctx* ctx, int on);
+int dhp_profile_reset(dhp_ctx* ctx);
+int dhp_profile_read(dhp_ctx* ctx, double* ms, int64_t* n_calls);
+
+/* Number of kernels this library has launched on the context since dhp_create. */
+int64_t dhp_launch_count(dhp_ctx* ctx);
+
+const char* dhp_strerror(int code);
+const char* dhp_last_cuda_error(dhp_ctx* ctx);
+const char* dhp_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DHP_H */

@@ -1,0 +1,271 @@
+"""Thin ctypes binding over the C ABI of libdhp.so (include/dhp.h) — argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of the library; PyTorch is used here only to own
+device memory and the stream.  There is NO CPU fallback: if the library is missing or no CUDA device is
+present, calls raise.  Function names are those of the C ABI; `Dhp` is a small convenience object that
+keeps a context and marshals torch tensors / numpy arrays.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libdhp.so")
+
+N_PHASES = 4
+PHASES = ("nlist", "aev_fwd", "mlp", "aev_bwd")
+MLP_AUTO, MLP_SIMT, MLP_TENSOR = 0, 1, 2
+OK = 0
+
+# every symbol include/dhp.h declares: (name, restype, argtypes)
+_vp, _i64, _i32, _f32 = C.c_void_p, C.c_int64, C.c_int, C.c_float
+SYMBOLS = {
+    "dhp_create": (C.c_int, [C.POINTER(_vp), _vp, _i64, _i64, _vp]),
+    "dhp_destroy": (C.c_int, [_vp]),
+    "dhp_weights_load": (C.c_int, [_vp, _vp, _i64, _i32, C.POINTER(_vp)]),
+    "dhp_weights_free": (C.c_int, [_vp, _vp]),
+    "dhp_nlist_build": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _vp, _i64, _f32, C.POINTER(_vp)]),
+    "dhp_nlist_sizes": (C.c_int, [_vp, _vp, C.POINTER(_i64), C.POINTER(_i64)]),
+    "dhp_nlist_export": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp]),
+    "dhp_ani_energy_forces": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _vp, _i64, _vp, _i32, _vp, _vp]),
+    "dhp_ani_energy_forces_host": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _vp, _i64, _vp, _i32, _vp, _vp]),
+    "dhp_status": (C.c_int, [_vp]),
+    "dhp_set_mlp_mode": (C.c_int, [_vp, _i32]),
+    "dhp_tensor_path_available": (C.c_int, [_vp]),
+    "dhp_debug_aev": (C.c_int, [_vp, _vp]),
+    "dhp_debug_grad": (C.c_int, [_vp, _vp]),
+    "dhp_debug_atomic_energy": (C.c_int, [_vp, _vp]),
+    "dhp_profile_enable": (C.c_int, [_vp, _i32]),
+    "dhp_profile_reset": (C.c_int, [_vp]),
+    "dhp_profile_read": (C.c_int, [_vp, C.POINTER(C.c_double), C.POINTER(_i64)]),
+    "dhp_launch_count": (_i64, [_vp]),
+    "dhp_strerror": (C.c_char_p, [_i32]),
+    "dhp_last_cuda_error": (C.c_char_p, [_vp]),
+    "dhp_version": (C.c_char_p, []),
+}
+
+
+class DhpParams(C.Structure):
+    _fields_ = [("rcr", _f32), ("rca", _f32), ("eta_r", _f32), ("eta_a", _f32), ("zeta", _f32), ("celu_alpha", _f32),
+                ("shf_r", _f32 * 16), ("shf_a", _f32 * 8), ("shf_z", _f32 * 4)]
+
+
+class DhpError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def load_library() -> C.CDLL:
+    """dlopen libdhp.so and bind every declared symbol.  Raises if the library was not built."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise DhpError(f"{LIB_PATH} not found: build it with `python -m paper_2207_14276_b200.build` "
+                           "(there is no CPU fallback)")
+        lib = C.CDLL(LIB_PATH)
+        for name, (res, args) in SYMBOLS.items():
+            fn = getattr(lib, name)          # AttributeError if the symbol is not exported
+            fn.restype = res
+            fn.argtypes = args
+        _lib = lib
+    return _lib
+
+
+def _check(rc: int, ctx=None):
+    if rc != OK:
+        lib = load_library()
+        msg = lib.dhp_strerror(rc).decode()
+        if ctx is not None and rc == -6:
+            msg += ": " + lib.dhp_last_cuda_error(ctx).decode()
+        raise DhpError(f"dhp error {rc}: {msg}")
+
+
+def _dptr(t) -> Optional[int]:
+    """Device (or host) address of a torch tensor / numpy array, or None."""
+    if t is None:
+        return None
+    if isinstance(t, np.ndarray):
+        return t.ctypes.data
+    return t.data_ptr()
+
+
+def make_params(p) -> DhpParams:
+    """`workloads.AniParams` (fp32 values) -> C struct."""
+    q = DhpParams()
+    q.rcr, q.rca, q.eta_r, q.eta_a = float(p.rcr), float(p.rca), float(p.eta_r), float(p.eta_a)
+    q.zeta, q.celu_alpha = float(p.zeta), float(p.celu_alpha)
+    for i in range(16):
+        q.shf_r[i] = float(p.shf_r[i])
+    for i in range(8):
+        q.shf_a[i] = float(p.shf_a[i])
+    for i in range(4):
+        q.shf_z[i] = float(p.shf_z[i])
+    return q
+
+
+class Dhp:
+    """One context (workspace for `max_atoms`, bound to the current torch CUDA stream)."""
+
+    def __init__(self, max_atoms: int, max_mols: int = 0, params=None, device: str = "cuda:0"):
+        import torch
+        if not torch.cuda.is_available():
+            raise DhpError("no CUDA device: the dhp hot path has no CPU fallback")
+        self.torch = torch
+        self.lib = load_library()
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.stream = torch.cuda.current_stream(self.device)
+        self._params = make_params(params) if params is not None else None
+        self.rcr = float(self._params.rcr) if self._params is not None else float(np.float32(5.1))
+        ctx = _vp()
+        _check(self.lib.dhp_create(C.byref(ctx), C.byref(self._params) if self._params is not None else None,
+                                   int(max_atoms), int(max_mols), _vp(self.stream.cuda_stream)))
+        self.ctx = ctx
+        self.max_atoms, self.max_mols = int(max_atoms), int(max_mols)
+        self._weights = []
+        self._nlist = None
+        self._n = 0
+
+    # ---- lifetime
+    def close(self):
+        if getattr(self, "ctx", None):
+            for w in self._weights:
+                self.lib.dhp_weights_free(self.ctx, w)
+            self._weights = []
+            self.lib.dhp_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- C ABI, same names
+    def dhp_weights_load(self, blob, n_models: int):
+        """blob: numpy fp32 (host) or torch cuda fp32 tensor with 338689*7*n_models values."""
+        if isinstance(blob, np.ndarray):
+            blob = np.ascontiguousarray(blob, dtype=np.float32)
+            n = blob.size
+        else:
+            blob = blob.contiguous()
+            n = blob.numel()
+        h = _vp()
+        _check(self.lib.dhp_weights_load(self.ctx, _vp(_dptr(blob)), int(n), int(n_models), C.byref(h)), self.ctx)
+        self._weights.append(h)
+        h.n_models = int(n_models)
+        return h
+
+    def dhp_nlist_build(self, pos, box, species, mol_offsets=None):
+        """pos/species/mol_offsets: cuda tensors (fp32 [N,3], int32 [N], int32 [n_mol+1]); box: host fp32[3] or None."""
+        n = int(pos.shape[0])
+        boxh = None if box is None else np.ascontiguousarray(box, dtype=np.float32)
+        n_mol = 0 if mol_offsets is None else int(mol_offsets.shape[0]) - 1
+        h = _vp()
+        _check(self.lib.dhp_nlist_build(self.ctx, _vp(_dptr(pos)), _vp(_dptr(boxh)), _vp(_dptr(species)), n,
+                                        _vp(_dptr(mol_offsets)), n_mol, C.c_float(self.rcr), C.byref(h)), self.ctx)
+        self._nlist, self._n = h, n
+        return h
+
+    def dhp_nlist_sizes(self):
+        a, b = _i64(), _i64()
+        _check(self.lib.dhp_nlist_sizes(self.ctx, self._nlist, C.byref(a), C.byref(b)), self.ctx)
+        return int(a.value), int(b.value)
+
+    def dhp_nlist_export(self):
+        """Canonical CSR (caller numbering, ascending columns): (row_ptr, col, row_ptr_ang, col_ang) int32 cuda tensors."""
+        t = self.torch
+        nnz, nnz_a = self.dhp_nlist_sizes()
+        rp = t.empty(self._n + 1, dtype=t.int32, device=self.device)
+        col = t.empty(max(nnz, 1), dtype=t.int32, device=self.device)
+        rpa = t.empty(self._n + 1, dtype=t.int32, device=self.device)
+        cola = t.empty(max(nnz_a, 1), dtype=t.int32, device=self.device)
+        _check(self.lib.dhp_nlist_export(self.ctx, self._nlist, _vp(_dptr(rp)), _vp(_dptr(col)), _vp(_dptr(rpa)),
+                                         _vp(_dptr(cola))), self.ctx)
+        t.cuda.synchronize(self.device)
+        return rp, col[:nnz], rpa, cola[:nnz_a]
+
+    def dhp_ani_energy_forces(self, pos, box, species, weights, mol_offsets=None, E=None, F=None):
+        """Device-pointer hot call.  Returns (E fp64 [max(1,n_mol)], F fp32 [N,3]) cuda tensors; asynchronous."""
+        t = self.torch
+        n = int(pos.shape[0])
+        boxh = None if box is None else np.ascontiguousarray(box, dtype=np.float32)
+        n_mol = 0 if mol_offsets is None else int(mol_offsets.shape[0]) - 1
+        if E is None:
+            E = t.empty(max(1, n_mol), dtype=t.float64, device=self.device)
+        if F is None:
+            F = t.empty((n, 3), dtype=t.float32, device=self.device)
+        _check(self.lib.dhp_ani_energy_forces(self.ctx, _vp(_dptr(pos)), _vp(_dptr(boxh)), _vp(_dptr(species)), n,
+                                              _vp(_dptr(mol_offsets)), n_mol, weights, weights.n_models,
+                                              _vp(_dptr(E)), _vp(_dptr(F))), self.ctx)
+        self._n = n
+        return E, F
+
+    def dhp_ani_energy_forces_host(self, pos, box, species, weights, mol_offsets=None, E=None, F=None):
+        """Host-buffer call (numpy arrays or pinned torch CPU tensors): copies in, kernels, copies out, one sync."""
+        n = int(pos.shape[0])
+        boxh = None if box is None else np.ascontiguousarray(box, dtype=np.float32)
+        n_mol = 0 if mol_offsets is None else int(mol_offsets.shape[0]) - 1
+        if E is None:
+            E = np.empty(max(1, n_mol), dtype=np.float64)
+        if F is None:
+            F = np.empty((n, 3), dtype=np.float32)
+        _check(self.lib.dhp_ani_energy_forces_host(self.ctx, _vp(_dptr(pos)), _vp(_dptr(boxh)), _vp(_dptr(species)), n,
+                                                   _vp(_dptr(mol_offsets)), n_mol, weights, weights.n_models,
+                                                   _vp(_dptr(E)), _vp(_dptr(F))), self.ctx)
+        self._n = n
+        return E, F
+
+    def dhp_status(self) -> int:
+        return int(self.lib.dhp_status(self.ctx))
+
+    def dhp_set_mlp_mode(self, mode: int):
+        _check(self.lib.dhp_set_mlp_mode(self.ctx, int(mode)), self.ctx)
+
+    def dhp_tensor_path_available(self) -> bool:
+        return bool(self.lib.dhp_tensor_path_available(self.ctx))
+
+    def _debug(self, fn, ncol):
+        t = self.torch
+        out = t.empty((self._n, ncol), dtype=t.float32, device=self.device)
+        _check(fn(self.ctx, _vp(_dptr(out))), self.ctx)
+        return out
+
+    def dhp_debug_aev(self):
+        return self._debug(self.lib.dhp_debug_aev, 1008)
+
+    def dhp_debug_grad(self):
+        return self._debug(self.lib.dhp_debug_grad, 1008)
+
+    def dhp_debug_atomic_energy(self):
+        return self._debug(self.lib.dhp_debug_atomic_energy, 1)[:, 0]
+
+    def dhp_profile_enable(self, on: bool):
+        _check(self.lib.dhp_profile_enable(self.ctx, 1 if on else 0), self.ctx)
+
+    def dhp_profile_reset(self):
+        _check(self.lib.dhp_profile_reset(self.ctx), self.ctx)
+
+    def dhp_profile_read(self):
+        ms = (C.c_double * N_PHASES)()
+        n = _i64()
+        _check(self.lib.dhp_profile_read(self.ctx, ms, C.byref(n)), self.ctx)
+        return {PHASES[i]: float(ms[i]) for i in range(N_PHASES)}, int(n.value)
+
+    def dhp_launch_count(self) -> int:
+        return int(self.lib.dhp_launch_count(self.ctx))
+
+
+def to_device(system, device="cuda:0"):
+    """Upload a `workloads.System` once: (pos, species, mol_offsets) cuda tensors."""
+    import torch
+    pos = torch.from_numpy(np.ascontiguousarray(system.pos)).to(device)
+    species = torch.from_numpy(np.ascontiguousarray(system.species)).to(device)
+    mol = None if system.mol_offsets is None else torch.from_numpy(np.ascontiguousarray(system.mol_offsets)).to(device)
+    return pos, species, mol

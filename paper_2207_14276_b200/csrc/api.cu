@@ -1,0 +1,367 @@
+// C ABI of libdhp.so (include/dhp.h): context / workspace, weight handles, the two hot calls.
+#include <math.h>
+#include <new>
+#include <stdio.h>
+#include <string.h>
+
+#include "dhp_internal.cuh"
+
+namespace dhp {
+
+int cuda_fail(Ctx* ctx, cudaError_t e, const char* what) {
+    if (ctx) snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "%s: %s", what, cudaGetErrorString(e));
+    return DHP_E_CUDA;
+}
+
+static void default_params(dhp_params* p) {
+    p->rcr = 5.1f; p->rca = 3.5f; p->eta_r = 19.7f; p->eta_a = 12.5f; p->zeta = 14.1f; p->celu_alpha = 0.1f;
+    for (int m = 0; m < NR; ++m) p->shf_r[m] = (float)(0.8 + 0.2625 * m);
+    for (int a = 0; a < NA; ++a) p->shf_a[a] = (float)(0.8 + 0.3375 * a);
+    for (int z = 0; z < NZ; ++z) p->shf_z[z] = (float)((2.0 * z + 1.0) * 3.14159265358979323846 / 8.0);
+}
+
+static void make_aev_const(const dhp_params& p, AevConst* k) {
+    const double l2e = 1.4426950408889634074, pi = 3.14159265358979323846;
+    k->rcr = p.rcr; k->rca = p.rca;
+    k->pi_over_rcr = (float)(pi / (double)p.rcr); k->pi_over_rca = (float)(pi / (double)p.rca);
+    k->eta_r_l2e = (float)((double)p.eta_r * l2e); k->eta_a_l2e = (float)((double)p.eta_a * l2e);
+    k->eta_r = p.eta_r; k->eta_a = p.eta_a; k->zeta = p.zeta;
+    for (int m = 0; m < NR; ++m) k->shf_r[m] = p.shf_r[m];
+    for (int a = 0; a < NA; ++a) k->shf_a[a] = p.shf_a[a];
+    for (int z = 0; z < NZ; ++z) { k->cos_z[z] = (float)cos((double)p.shf_z[z]); k->sin_z[z] = (float)sin((double)p.shf_z[z]); }
+}
+
+template <typename T>
+static bool dalloc(T** p, size_t count) {
+    *p = nullptr;
+    return cudaMalloc((void**)p, sizeof(T) * (count ? count : 1)) == cudaSuccess;
+}
+
+static void free_all(Ctx* c) {
+    void* ptrs[] = {c->grid, c->status, c->bbox, c->cell_of, c->scell, c->cell_count, c->cell_start, c->cell_fill, c->perm,
+                    c->inv_perm, c->spos, c->smol, c->n_rad, c->n_ang, c->row_ptr, c->col, c->sp_count, c->sp_start,
+                    c->rowmap, c->row_species, c->row_slot, c->blk_hist, c->aev, c->grad, c->e_atom, c->fsorted,
+                    c->e_out_tmp, c->export_tmp, c->st_pos, c->st_species, c->st_mol, c->st_E, c->st_F};
+    for (void* p : ptrs) if (p) cudaFree(p);
+    mlp_simt_free(c);
+    mlp_tc_free(c);
+    for (auto& row : c->prof.ev) for (auto& e : row) if (e) cudaEventDestroy(e);
+}
+
+static int check_args(Ctx* ctx, const float* pos, const float* box, const int32_t* species, int64_t n,
+                      const int32_t* mol_offsets, int64_t n_mol) {
+    if (!ctx || n < 0 || n_mol < 0) return DHP_E_BADARG;
+    if (n > 0 && (!pos || !species)) return DHP_E_BADARG;
+    if (n > ctx->max_atoms) return DHP_E_CAPACITY;
+    if (mol_offsets && n_mol > 0) {
+        if (box) return DHP_E_BADARG;
+        if (n_mol > ctx->max_mols) return DHP_E_CAPACITY;
+    }
+    if (box)
+        for (int c = 0; c < 3; ++c)
+            if (!(box[c] >= 2.0f * ctx->params.rcr)) return DHP_E_BOX;
+    return DHP_OK;
+}
+
+static void prof_mark(Ctx* ctx, int slot, int phase) {
+    if (ctx->prof.on && slot >= 0) cudaEventRecord(ctx->prof.ev[slot][phase], ctx->stream);
+}
+
+static void prof_drain(Ctx* ctx) {
+    Profile& p = ctx->prof;
+    if (p.n_pending == 0) return;
+    cudaStreamSynchronize(ctx->stream);
+    for (int s = 0; s < p.n_pending; ++s)
+        for (int ph = 0; ph < DHP_N_PHASES; ++ph) {
+            float ms = 0.f;
+            if (cudaEventElapsedTime(&ms, p.ev[s][ph], p.ev[s][ph + 1]) == cudaSuccess) p.ms[ph] += ms;
+        }
+    p.calls += p.n_pending;
+    p.n_pending = 0;
+}
+
+static int run_energy_forces(Ctx* ctx, const float* pos, const float* box, const int32_t* species, int64_t n,
+                             const int32_t* mol_offsets, int64_t n_mol, const Weights* w, double* E, float* F) {
+    int slot = -1;
+    if (ctx->prof.on) {
+        if (ctx->prof.n_pending == 64) prof_drain(ctx);
+        slot = ctx->prof.n_pending++;
+    }
+    int rc;
+    prof_mark(ctx, slot, 0);
+    if ((rc = nlist_build(ctx, pos, box, species, n, mol_offsets, n_mol)) != DHP_OK) return rc;
+    prof_mark(ctx, slot, 1);
+    if ((rc = aev_forward(ctx)) != DHP_OK) return rc;
+    prof_mark(ctx, slot, 2);
+    const bool tensor = ctx->mlp_mode == DHP_MLP_TENSOR || (ctx->mlp_mode == DHP_MLP_AUTO && w->tc != nullptr);
+    if (tensor && !w->tc) return DHP_E_NOTIMPL;
+    rc = tensor ? mlp_tc(ctx, w) : mlp_simt(ctx, w);
+    if (rc != DHP_OK) return rc;
+    if ((rc = energy_reduce(ctx, E)) != DHP_OK) return rc;
+    prof_mark(ctx, slot, 3);
+    if ((rc = aev_backward(ctx, F)) != DHP_OK) return rc;
+    prof_mark(ctx, slot, 4);
+    ctx->n_models = w->n_models;
+    return DHP_OK;
+}
+
+// debug gathers: buffer rows -> caller's atom order
+__global__ void k_gather_rows(const float* __restrict__ src, int ld_src, int ncol, const int* __restrict__ rowmap,
+                              const int* __restrict__ inv_perm, int n, float* __restrict__ dst) {
+    int a = blockIdx.x;
+    if (a >= n) return;
+    const float* s = src + (size_t)rowmap[inv_perm[a]] * ld_src;
+    for (int c = threadIdx.x; c < ncol; c += blockDim.x) dst[(size_t)a * ncol + c] = s[c];
+}
+
+}  // namespace dhp
+
+using namespace dhp;
+
+extern "C" {
+
+struct dhp_ctx { Ctx c; };
+struct dhp_nlist { Ctx* owner; };
+struct dhp_weights { Weights w; };
+static dhp_nlist g_nlist_token;   // the list lives in the context workspace; the handle is a token
+
+int dhp_create(dhp_ctx** out, const dhp_params* params, int64_t max_atoms, int64_t max_mols, void* cuda_stream) {
+    if (!out || max_atoms < 1 || max_mols < 0) return DHP_E_BADARG;
+    *out = nullptr;
+    dhp_ctx* h = new (std::nothrow) dhp_ctx();
+    if (!h) return DHP_E_NOMEM;
+    Ctx* c = &h->c;
+    memset((void*)c, 0, sizeof(Ctx));
+    c->stream = (cudaStream_t)cuda_stream;
+    if (params) c->params = *params; else default_params(&c->params);
+    if (!(c->params.rca > 0.f) || !(c->params.rcr >= c->params.rca) || !(c->params.celu_alpha > 0.f)) { delete h; return DHP_E_BADARG; }
+    make_aev_const(c->params, &c->aevc);
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) { delete h; return DHP_E_CUDA; }
+    c->sm_count = prop.multiProcessorCount;
+    c->cc_major = prop.major;
+    c->max_atoms = max_atoms;
+    c->max_mols = max_mols;
+    c->max_rows = (max_atoms + NSP * (ROW_TILE - 1) + ROW_TILE - 1) / ROW_TILE * ROW_TILE + ROW_TILE;
+    c->max_cells = max_atoms * 2 > 4096 ? max_atoms * 2 : 4096;
+    if (max_mols > c->max_cells) c->max_cells = max_mols;
+    // neighbour storage: 160 directed pairs per atom on average (rho = 0.1 A^-3 gives 55 at 5.1 A); for tiny
+    // systems every pair may be a neighbour
+    c->pair_cap = max_atoms * 160;
+    if (max_atoms < 161) c->pair_cap = max_atoms * (max_atoms - 1) + 1;
+    const size_t N = (size_t)max_atoms, R = (size_t)c->max_rows, NC = (size_t)c->max_cells;
+    const size_t NM = (size_t)(max_mols > 0 ? max_mols : 1);
+    bool ok = true;
+    ok &= dalloc(&c->grid, 1) && dalloc(&c->status, 1) && dalloc(&c->bbox, 8);
+    ok &= dalloc(&c->cell_of, N) && dalloc(&c->scell, N) && dalloc(&c->cell_count, NC + 1) && dalloc(&c->cell_start, NC + 1) && dalloc(&c->cell_fill, NC);
+    ok &= dalloc(&c->perm, N) && dalloc(&c->inv_perm, N) && dalloc(&c->spos, N) && dalloc(&c->smol, N);
+    ok &= dalloc(&c->n_rad, N) && dalloc(&c->n_ang, N) && dalloc(&c->row_ptr, N + 1) && dalloc(&c->col, (size_t)c->pair_cap);
+    ok &= dalloc(&c->sp_count, 8) && dalloc(&c->sp_start, 8) && dalloc(&c->rowmap, N);
+    ok &= dalloc(&c->row_species, R) && dalloc(&c->row_slot, R) && dalloc(&c->blk_hist, (N / 256 + 2) * 8);
+    ok &= dalloc(&c->aev, R * AEV_LD) && dalloc(&c->grad, R * AEV_LD) && dalloc(&c->e_atom, R);
+    ok &= dalloc(&c->fsorted, 3 * N) && dalloc(&c->e_out_tmp, NM) && dalloc(&c->export_tmp, N + 1);
+    ok &= dalloc(&c->st_pos, 3 * N) && dalloc(&c->st_species, N) && dalloc(&c->st_mol, NM + 1) && dalloc(&c->st_E, NM) && dalloc(&c->st_F, 3 * N);
+    if (ok) ok = mlp_simt_alloc(c) == DHP_OK;
+    if (ok && mlp_tc_available(c)) ok = mlp_tc_alloc(c) == DHP_OK;
+    if (ok) {
+        for (auto& row : c->prof.ev) for (auto& e : row) ok &= cudaEventCreate(&e) == cudaSuccess;
+        // padding rows are never written by the AEV kernel; keep them finite
+        ok &= cudaMemset(c->aev, 0, sizeof(float) * R * AEV_LD) == cudaSuccess;
+        ok &= cudaMemset(c->grad, 0, sizeof(float) * R * AEV_LD) == cudaSuccess;
+        ok &= cudaMemset(c->status, 0, sizeof(int)) == cudaSuccess;
+    }
+    if (!ok) { cudaGetLastError(); free_all(c); delete h; return DHP_E_NOMEM; }
+    *out = h;
+    return DHP_OK;
+}
+
+int dhp_destroy(dhp_ctx* h) {
+    if (!h) return DHP_E_BADARG;
+    cudaStreamSynchronize(h->c.stream);
+    free_all(&h->c);
+    delete h;
+    return DHP_OK;
+}
+
+int dhp_weights_load(dhp_ctx* h, const float* blob, int64_t n_floats, int n_models, dhp_weights** out) {
+    if (!h || !blob || !out || n_models < 1 || n_models > MAX_MODELS) return DHP_E_BADARG;
+    if (n_floats != (int64_t)NET_PARAMS * NSP * n_models) return DHP_E_BADARG;
+    Ctx* c = &h->c;
+    dhp_weights* w = new (std::nothrow) dhp_weights();
+    if (!w) return DHP_E_NOMEM;
+    w->w.n_models = n_models; w->w.blob = nullptr; w->w.tc = nullptr;
+    if (cudaMalloc((void**)&w->w.blob, sizeof(float) * (size_t)n_floats) != cudaSuccess) { delete w; return DHP_E_NOMEM; }
+    cudaError_t e = cudaMemcpyAsync(w->w.blob, blob, sizeof(float) * (size_t)n_floats, cudaMemcpyDefault, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) { cudaFree(w->w.blob); delete w; return cuda_fail(c, e, "weights upload"); }
+    if (mlp_tc_available(c)) {
+        int rc = mlp_tc_weights(c, &w->w);
+        if (rc != DHP_OK) { cudaFree(w->w.blob); delete w; return rc; }
+    }
+    *out = w;
+    return DHP_OK;
+}
+
+int dhp_weights_free(dhp_ctx* h, dhp_weights* w) {
+    if (!h || !w) return DHP_E_BADARG;
+    cudaStreamSynchronize(h->c.stream);
+    mlp_tc_weights_free(&h->c, &w->w);
+    if (w->w.blob) cudaFree(w->w.blob);
+    delete w;
+    return DHP_OK;
+}
+
+int dhp_nlist_build(dhp_ctx* h, const float* pos, const float* box, const int32_t* species, int64_t n_atoms,
+                    const int32_t* mol_offsets, int64_t n_mol, float rc, dhp_nlist** out) {
+    if (!h) return DHP_E_BADARG;
+    Ctx* c = &h->c;
+    int r = check_args(c, pos, box, species, n_atoms, mol_offsets, n_mol);
+    if (r != DHP_OK) return r;
+    if (rc != c->params.rcr) return DHP_E_BADARG;
+    r = nlist_build(c, pos, box, species, n_atoms, mol_offsets, n_mol);
+    if (r != DHP_OK) return r;
+    if (out) { g_nlist_token.owner = c; *out = &g_nlist_token; }
+    return DHP_OK;
+}
+
+int dhp_nlist_sizes(dhp_ctx* h, const dhp_nlist* nl, int64_t* nnz, int64_t* nnz_ang) {
+    if (!h || !nl) return DHP_E_BADARG;
+    Ctx* c = &h->c;
+    const int n = (int)c->n_atoms;
+    int total = 0;
+    DHP_CUDA(c, cudaMemcpyAsync(&total, c->row_ptr + n, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    DHP_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (nnz) *nnz = total;
+    if (nnz_ang) {
+        int64_t t = 0;
+        if (n > 0) {
+            int* tmp = (int*)malloc(sizeof(int) * n);
+            if (!tmp) return DHP_E_NOMEM;
+            cudaError_t e = cudaMemcpy(tmp, c->n_ang, sizeof(int) * n, cudaMemcpyDeviceToHost);
+            if (e != cudaSuccess) { free(tmp); return cuda_fail(c, e, "n_ang download"); }
+            for (int i = 0; i < n; ++i) t += tmp[i];
+            free(tmp);
+        }
+        *nnz_ang = t;
+    }
+    return DHP_OK;
+}
+
+int dhp_nlist_export(dhp_ctx* h, const dhp_nlist* nl, int32_t* row_ptr, int32_t* col, int32_t* row_ptr_ang, int32_t* col_ang) {
+    if (!h || !nl) return DHP_E_BADARG;
+    Ctx* c = &h->c;
+    int r = DHP_OK;
+    if (row_ptr) r = nlist_export(c, row_ptr, col, false);
+    if (r == DHP_OK && row_ptr_ang) r = nlist_export(c, row_ptr_ang, col_ang, true);
+    return r;
+}
+
+int dhp_ani_energy_forces(dhp_ctx* h, const float* pos, const float* box, const int32_t* species, int64_t n_atoms,
+                          const int32_t* mol_offsets, int64_t n_mol, const dhp_weights* weights, int n_models,
+                          double* E, float* F) {
+    if (!h || !weights || !E || (n_atoms > 0 && !F)) return DHP_E_BADARG;
+    Ctx* c = &h->c;
+    if (n_models != weights->w.n_models) return DHP_E_BADARG;
+    int r = check_args(c, pos, box, species, n_atoms, mol_offsets, n_mol);
+    if (r != DHP_OK) return r;
+    return run_energy_forces(c, pos, box, species, n_atoms, mol_offsets, n_mol, &weights->w, E, F);
+}
+
+int dhp_ani_energy_forces_host(dhp_ctx* h, const float* pos, const float* box, const int32_t* species, int64_t n_atoms,
+                               const int32_t* mol_offsets, int64_t n_mol, const dhp_weights* weights, int n_models,
+                               double* E, float* F) {
+    if (!h || !weights || !E || (n_atoms > 0 && !F)) return DHP_E_BADARG;
+    Ctx* c = &h->c;
+    if (n_models != weights->w.n_models) return DHP_E_BADARG;
+    int r = check_args(c, pos, box, species, n_atoms, mol_offsets, n_mol);
+    if (r != DHP_OK) return r;
+    const bool by_mol = mol_offsets && n_mol > 0;
+    const int64_t ne = by_mol ? n_mol : 1;
+    cudaStream_t st = c->stream;
+    if (n_atoms > 0) {
+        DHP_CUDA(c, cudaMemcpyAsync(c->st_pos, pos, sizeof(float) * 3 * n_atoms, cudaMemcpyHostToDevice, st));
+        DHP_CUDA(c, cudaMemcpyAsync(c->st_species, species, sizeof(int) * n_atoms, cudaMemcpyHostToDevice, st));
+    }
+    if (by_mol) DHP_CUDA(c, cudaMemcpyAsync(c->st_mol, mol_offsets, sizeof(int) * (n_mol + 1), cudaMemcpyHostToDevice, st));
+    r = run_energy_forces(c, c->st_pos, box, c->st_species, n_atoms, by_mol ? c->st_mol : nullptr, n_mol, &weights->w, c->st_E, c->st_F);
+    if (r != DHP_OK) return r;
+    DHP_CUDA(c, cudaMemcpyAsync(E, c->st_E, sizeof(double) * ne, cudaMemcpyDeviceToHost, st));
+    if (n_atoms > 0) DHP_CUDA(c, cudaMemcpyAsync(F, c->st_F, sizeof(float) * 3 * n_atoms, cudaMemcpyDeviceToHost, st));
+    DHP_CUDA(c, cudaStreamSynchronize(st));
+    return DHP_OK;
+}
+
+int dhp_status(dhp_ctx* h) {
+    if (!h) return DHP_E_BADARG;
+    Ctx* c = &h->c;
+    int s = 0;
+    cudaError_t e = cudaMemcpyAsync(&s, c->status, sizeof(int), cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "status");
+    return s;
+}
+
+int dhp_set_mlp_mode(dhp_ctx* h, int mode) {
+    if (!h || mode < DHP_MLP_AUTO || mode > DHP_MLP_TENSOR) return DHP_E_BADARG;
+    if (mode == DHP_MLP_TENSOR && !mlp_tc_available(&h->c)) return DHP_E_NOTIMPL;
+    h->c.mlp_mode = mode;
+    return DHP_OK;
+}
+
+int dhp_tensor_path_available(dhp_ctx* h) { return h && mlp_tc_available(&h->c) ? 1 : 0; }
+
+static int debug_gather(dhp_ctx* h, const float* src, int ld, int ncol, float* dst) {
+    if (!h || !dst) return DHP_E_BADARG;
+    Ctx* c = &h->c;
+    const int n = (int)c->n_atoms;
+    if (n == 0) return DHP_OK;
+    DHP_LAUNCH(c, k_gather_rows, n, 128, 0, src, ld, ncol, c->rowmap, c->inv_perm, n, dst);
+    DHP_CUDA(c, cudaGetLastError());
+    DHP_CUDA(c, cudaStreamSynchronize(c->stream));
+    return DHP_OK;
+}
+int dhp_debug_aev(dhp_ctx* h, float* aev) { return h ? debug_gather(h, h->c.aev, AEV_LD, AEV_DIM, aev) : DHP_E_BADARG; }
+int dhp_debug_grad(dhp_ctx* h, float* grad) { return h ? debug_gather(h, h->c.grad, AEV_LD, AEV_DIM, grad) : DHP_E_BADARG; }
+int dhp_debug_atomic_energy(dhp_ctx* h, float* e) { return h ? debug_gather(h, h->c.e_atom, 1, 1, e) : DHP_E_BADARG; }
+
+int dhp_profile_enable(dhp_ctx* h, int on) {
+    if (!h) return DHP_E_BADARG;
+    prof_drain(&h->c);
+    h->c.prof.on = on != 0;
+    return DHP_OK;
+}
+int dhp_profile_reset(dhp_ctx* h) {
+    if (!h) return DHP_E_BADARG;
+    prof_drain(&h->c);
+    for (double& m : h->c.prof.ms) m = 0.0;
+    h->c.prof.calls = 0;
+    return DHP_OK;
+}
+int dhp_profile_read(dhp_ctx* h, double* ms, int64_t* n_calls) {
+    if (!h || !ms) return DHP_E_BADARG;
+    prof_drain(&h->c);
+    for (int p = 0; p < DHP_N_PHASES; ++p) ms[p] = h->c.prof.ms[p];
+    if (n_calls) *n_calls = h->c.prof.calls;
+    return DHP_OK;
+}
+
+int64_t dhp_launch_count(dhp_ctx* h) { return h ? h->c.launches : 0; }
+
+const char* dhp_strerror(int code) {
+    switch (code) {
+        case DHP_OK: return "ok";
+        case DHP_E_BADARG: return "bad argument";
+        case DHP_E_CAPACITY: return "capacity exceeded (atoms, molecules or neighbour storage)";
+        case DHP_E_BOX: return "periodic box edge shorter than twice the radial cutoff";
+        case DHP_E_SPECIES: return "species index outside 0..6";
+        case DHP_E_NOTIMPL: return "not implemented / not available on this device";
+        case DHP_E_CUDA: return "CUDA runtime error";
+        case DHP_E_NOMEM: return "out of memory";
+        default: return "unknown error";
+    }
+}
+const char* dhp_last_cuda_error(dhp_ctx* h) { return h ? h->c.cuda_err : ""; }
+const char* dhp_version(void) { return "dhp 0.1 (sm_100a)"; }
+
+}  // extern "C"

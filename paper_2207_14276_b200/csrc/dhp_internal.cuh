@@ -1,0 +1,164 @@
+// Internal declarations shared by the translation units of libdhp.so (CUDA path only; the fp64
+// oracle under oracle/ shares nothing with this directory).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/dhp.h"
+
+namespace dhp {
+
+constexpr int NSP = DHP_N_SPECIES;
+constexpr int NR = DHP_N_SHF_R;
+constexpr int NA = DHP_N_SHF_A;
+constexpr int NZ = DHP_N_SHF_Z;
+constexpr int NPAIR = NSP * (NSP + 1) / 2;      // 28
+constexpr int AEV_RAD = NSP * NR;               // 112
+constexpr int AEV_ANG = NPAIR * NA * NZ;        // 896
+constexpr int AEV_DIM = AEV_RAD + AEV_ANG;      // 1008
+constexpr int AEV_LD = 1024;                    // row pitch of AEV / dE/dAEV buffers (floats)
+constexpr int H1 = 256, H2 = 192, H3 = 160;     // hidden widths (BASELINE.json configs[0])
+constexpr int NET_PARAMS = DHP_NET_PARAMS;
+constexpr int OFF_W1 = 0;
+constexpr int OFF_B1 = OFF_W1 + AEV_DIM * H1;
+constexpr int OFF_W2 = OFF_B1 + H1;
+constexpr int OFF_B2 = OFF_W2 + H1 * H2;
+constexpr int OFF_W3 = OFF_B2 + H2;
+constexpr int OFF_B3 = OFF_W3 + H2 * H3;
+constexpr int OFF_W4 = OFF_B3 + H3;
+constexpr int OFF_B4 = OFF_W4 + H3;
+static_assert(OFF_B4 + 1 == NET_PARAMS, "blob layout");
+
+constexpr int ROW_TILE = 128;                   // species groups start at multiples of this many rows
+constexpr int MAX_MODELS = 8;
+constexpr int MAX_ANG = 96;                     // angular neighbours staged per centre (status CAPACITY beyond)
+
+// Device-side description of the cell grid, written by a setup kernel (periodic: from host box;
+// open: from the bounding box reduction) so that no hot call needs a host round trip.
+struct Grid {
+    double L[3];        // periodic edge (0 if open)
+    double origin[3];   // lower corner used for binning
+    double inv_cell[3]; // 1 / cell edge
+    int nc[3];          // cells per axis
+    int ncell;
+    int periodic;
+    int by_molecule;    // 1: "cell" = molecule, stencil = self (batched replicas)
+};
+
+// AEV constants in the form the kernels use (fp32, exp2-scaled).
+struct AevConst {
+    float rcr, rca;
+    float pi_over_rcr, pi_over_rca;
+    float eta_r_l2e;            // eta_r * log2(e)
+    float eta_a_l2e;
+    float eta_r, eta_a, zeta;
+    float shf_r[NR], shf_a[NA];
+    float cos_z[NZ], sin_z[NZ];
+};
+
+struct Weights {
+    int n_models;
+    float* blob;        // fp32 copy of the caller's blob (SIMT path)
+    void* tc;           // tensor-path operand tiles (mlp_tc.cu), or nullptr
+};
+
+struct Profile {
+    bool on;
+    cudaEvent_t ev[64][DHP_N_PHASES + 1];
+    int n_pending;
+    double ms[DHP_N_PHASES];
+    int64_t calls;
+};
+
+struct Ctx {
+    cudaStream_t stream;
+    dhp_params params;
+    AevConst aevc;
+    int64_t max_atoms, max_mols, max_rows, max_cells, pair_cap;
+    int sm_count, cc_major;
+    int mlp_mode;
+    int64_t launches;
+    char cuda_err[256];
+    Profile prof;
+
+    // last call
+    int64_t n_atoms, n_mol;
+    int n_models;
+    bool periodic;
+
+    // workspace (device)
+    Grid* grid;
+    int* status;
+    unsigned* bbox;        // 6 ordered-uint min/max
+    int* cell_of;          // [N] cell of caller's atom i
+    int* scell;            // [N] cell of sorted slot
+    int* cell_count;       // [max_cells+1]
+    int* cell_start;       // [max_cells+1]
+    int* cell_fill;        // [max_cells]
+    int* perm;             // [N] sorted slot -> caller's index
+    int* inv_perm;         // [N]
+    float4* spos;          // [N] x,y,z, species bits
+    int* smol;             // [N] molecule of sorted atom (0 if none)
+    int* n_rad;            // [N]
+    int* n_ang;            // [N]
+    int* row_ptr;          // [N+1]
+    int* col;              // [pair_cap] sorted-slot indices; angular neighbours first in each row
+    int* sp_count;         // [8]
+    int* sp_start;         // [8] first row of each species group (multiple of ROW_TILE); [7] = end
+    int* rowmap;           // [N] sorted slot -> row
+    int* row_species;      // [max_rows] species of each row (-1 for padding rows)
+    int* row_slot;         // [max_rows] sorted slot of each row (-1 for padding)
+    int* blk_hist;         // per-block species histograms for the stable row assignment
+    float* aev;            // [max_rows][AEV_LD]
+    float* grad;           // [max_rows][AEV_LD]  dE/dAEV
+    float* e_atom;         // [max_rows]
+    float* act[6];         // SIMT path intermediates: h1,h2,h3(delta3),delta2,delta1 ; see mlp_simt.cu
+    float* fsorted;        // [N][3] forces in sorted order
+    double* e_out_tmp;     // [max(1,max_mols)]
+    int* export_tmp;       // [N+1]
+    // host-call staging
+    float* st_pos; int* st_species; int* st_mol; double* st_E; float* st_F;
+    void* tc_ws;           // tensor-path workspace (mlp_tc.cu)
+};
+
+// ---- launch bookkeeping -------------------------------------------------------------------------
+#define DHP_LAUNCH(ctx, kernel, grid, block, smem, ...)                         \
+    do {                                                                        \
+        kernel<<<(grid), (block), (smem), (ctx)->stream>>>(__VA_ARGS__);        \
+        (ctx)->launches++;                                                      \
+    } while (0)
+
+int cuda_fail(Ctx* ctx, cudaError_t e, const char* what);
+#define DHP_CUDA(ctx, call)                                            \
+    do {                                                               \
+        cudaError_t e__ = (call);                                      \
+        if (e__ != cudaSuccess) return dhp::cuda_fail((ctx), e__, #call); \
+    } while (0)
+
+// ---- phases (each enqueues kernels on ctx->stream) ------------------------------------------------
+int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t* species, int64_t n,
+                const int32_t* mol_offsets, int64_t n_mol);
+int nlist_export(Ctx* ctx, int32_t* row_ptr, int32_t* col, bool angular);
+int aev_forward(Ctx* ctx);
+int aev_backward(Ctx* ctx, float* F_out);
+int mlp_simt(Ctx* ctx, const Weights* w);
+int mlp_simt_alloc(Ctx* ctx);
+void mlp_simt_free(Ctx* ctx);
+int energy_reduce(Ctx* ctx, double* E_out);
+
+// tensor path (mlp_tc.cu)
+bool mlp_tc_available(Ctx* ctx);
+int mlp_tc_alloc(Ctx* ctx);
+void mlp_tc_free(Ctx* ctx);
+int mlp_tc_weights(Ctx* ctx, Weights* w);
+void mlp_tc_weights_free(Ctx* ctx, Weights* w);
+int mlp_tc(Ctx* ctx, const Weights* w);
+
+// upper-triangle row-major index of the unordered species pair (layout of the angular block)
+__host__ __device__ inline int pairidx(int a, int b) {
+    int u = a < b ? a : b, v = a < b ? b : a;
+    return NSP * u - u * (u - 1) / 2 + (v - u);
+}
+
+}  // namespace dhp

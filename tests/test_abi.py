@@ -1,0 +1,52 @@
+"""The C-ABI library loads on a CPU-only box and exports every symbol include/dhp.h declares
+(no compute calls here: those need a GPU and live in test_gpu_parity.py)."""
+import os
+import re
+
+from paper_2207_14276_b200 import binding
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "dhp.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(dhp_[a-z_0-9]+)\s*\(", text)))
+
+
+def test_header_and_binding_agree():
+    assert declared_symbols() == sorted(binding.SYMBOLS)
+
+
+def test_library_builds_loads_and_exports_everything():
+    from paper_2207_14276_b200 import build
+    build.build()
+    lib = binding.load_library()
+    for name in declared_symbols():
+        assert hasattr(lib, name), name
+    assert b"sm_100a" in lib.dhp_version()
+    assert lib.dhp_strerror(-3).decode().startswith("periodic box")
+    assert lib.dhp_strerror(0) == b"ok"
+
+
+def test_params_struct_matches_header():
+    import ctypes
+    assert ctypes.sizeof(binding.DhpParams) == 4 * (6 + 16 + 8 + 4)
+
+
+def test_no_cpu_fallback_without_gpu():
+    import pytest
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(binding.DhpError):
+        binding.Dhp(16)
+
+
+def test_product_path_does_not_import_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2207_14276_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in src and "from oracle" not in src and "liboracle" not in src, f

@@ -1,0 +1,291 @@
+"""Parity of the CUDA path (through the C ABI) against the fp64 oracle, element by element.
+
+Tolerances (BASELINE.json north_star; derivations in DESIGN.md §Tolerances):
+  pair lists  bit-exact (canonical CSR);
+  energy      |E_gpu - E_oracle| / N <= 1e-6 Hartree per atom (per molecule for batched replicas);
+  forces      max |dF| <= 5e-5 Hartree/Å;
+  AEV rows    |dG| <= 2e-5 absolute (fp32 evaluation of O(1..10) sums; intermediate, not a north_star bar);
+  dE/dG rows  |dg| <= 2e-5 absolute.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2207_14276_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+E_TOL_PER_ATOM = 1e-6
+F_TOL = 5e-5
+AEV_TOL = 2e-5
+GRAD_TOL = 2e-5
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2207_14276_b200 import binding
+    return binding
+
+
+@pytest.fixture(scope="module")
+def blob8():
+    return W.make_weights(8)
+
+
+def make_ctx(B, system, params, extra_atoms=0):
+    return B.Dhp(system.n_atoms + extra_atoms, max_mols=max(system.n_mol, 0), params=params)
+
+
+def csr_equal(rp_g, col_g, rp_o, col_o):
+    rp_g = rp_g.cpu().numpy().astype(np.int64)
+    col_g = col_g.cpu().numpy()
+    return np.array_equal(rp_g, rp_o) and np.array_equal(col_g, col_o)
+
+
+SYSTEMS = {
+    "water96": lambda: W.make_system(1),
+    "ligand50": lambda: W.make_system(2),
+    "mix600": lambda: W.small_periodic_mix(600, 18.3, seed=77, n_models=2),
+    "mix1500": lambda: W.small_periodic_mix(1500, 24.8, seed=5, n_models=1),
+    "replicas16": lambda: W.replicas_1024x30(n_mol=16),
+}
+
+
+# ------------------------------------------------------------------------------------------- a1
+@pytest.mark.parametrize("name", list(SYSTEMS))
+def test_pair_lists_bit_exact_small(torch, B, params, name):
+    s = SYSTEMS[name]()
+    d = make_ctx(B, s, params)
+    pos, sp, mol = B.to_device(s)
+    d.dhp_nlist_build(pos, s.box, sp, mol)
+    assert d.dhp_status() == 0
+    rp, col, rpa, cola = d.dhp_nlist_export()
+    rpo, colo = oracle.pairs(s.pos, s.box, params.rcr, s.mol_offsets)
+    assert csr_equal(rp, col, rpo, colo)
+    rpo, colo = oracle.pairs(s.pos, s.box, params.rca, s.mol_offsets)
+    assert csr_equal(rpa, cola, rpo, colo)
+    d.close()
+
+
+@pytest.mark.parametrize("cfg", [3, 5, 4])
+def test_pair_lists_bit_exact_full_size(torch, B, params, cfg):
+    s = W.make_system(cfg)
+    d = make_ctx(B, s, params)
+    pos, sp, mol = B.to_device(s)
+    d.dhp_nlist_build(pos, s.box, sp, mol)
+    assert d.dhp_status() == 0
+    rp, col, rpa, cola = d.dhp_nlist_export()
+    rpo, colo = oracle.pairs(s.pos, s.box, params.rcr, s.mol_offsets)
+    assert csr_equal(rp, col, rpo, colo)
+    rpo, colo = oracle.pairs(s.pos, s.box, params.rca, s.mol_offsets)
+    assert csr_equal(rpa, cola, rpo, colo)
+    d.close()
+
+
+def test_pair_list_positions_outside_box_and_two_cells_per_edge(torch, B, params):
+    """configs[0] has 2 cells per edge (Q19); shifting atoms by whole boxes must change nothing (Q3)."""
+    s = W.make_system(1)
+    q = s.pos.copy()
+    q[::3] += s.box[0] * 2
+    q[1::7, 1] -= s.box[1] * 3
+    d = make_ctx(B, s, params)
+    pos = torch.from_numpy(q).cuda()
+    sp = torch.from_numpy(s.species).cuda()
+    d.dhp_nlist_build(pos, s.box, sp)
+    rp, col, _, _ = d.dhp_nlist_export()
+    rpo, colo = oracle.pairs(q, s.box, params.rcr)
+    assert csr_equal(rp, col, rpo, colo)
+    d.close()
+
+
+# ------------------------------------------------------------------------------------------- a2..a5
+def run_gpu(B, torch, s, params, blob, mode=None):
+    d = make_ctx(B, s, params)
+    if mode is not None:
+        d.dhp_set_mlp_mode(mode)
+    w = d.dhp_weights_load(blob[: s.n_models * 7 * W.PARAMS_PER_NET], s.n_models)
+    pos, sp, mol = B.to_device(s)
+    E, F = d.dhp_ani_energy_forces(pos, s.box, sp, w, mol)
+    torch.cuda.synchronize()
+    assert d.dhp_status() == 0
+    return d, E.cpu().numpy(), F.cpu().numpy()
+
+
+def mlp_modes(B):
+    return [B.MLP_SIMT, B.MLP_TENSOR]
+
+
+@pytest.mark.parametrize("name", ["water96", "ligand50", "mix600", "replicas16"])
+@pytest.mark.parametrize("mode", [1, 2])
+def test_energy_forces_small(torch, B, params, blob8, name, mode):
+    s = SYSTEMS[name]()
+    probe = make_ctx(B, s, params)
+    if mode == B.MLP_TENSOR and not probe.dhp_tensor_path_available():
+        probe.close()
+        pytest.skip("tensor path not available in this build")
+    probe.close()
+    d, E, F = run_gpu(B, torch, s, params, blob8, mode)
+    Eo, Fo = oracle.total_energy_forces(s, params, blob8[: s.n_models * 7 * W.PARAMS_PER_NET])
+    per = s.n_atoms if s.mol_offsets is None else np.diff(s.mol_offsets)
+    assert np.max(np.abs(E - Eo) / per) <= E_TOL_PER_ATOM
+    assert np.max(np.abs(F - Fo)) <= F_TOL
+    # intermediates: AEV rows, dE/dG rows, atomic energies
+    G = d.dhp_debug_aev().cpu().numpy()
+    Go = oracle.aev(s.pos, s.species, s.box, params, mol_offsets=s.mol_offsets)
+    assert np.max(np.abs(G - Go)) <= AEV_TOL
+    Ea, _, go = oracle.energy_forces(s.pos, s.species, s.box, params, blob8[: s.n_models * 7 * W.PARAMS_PER_NET],
+                                     s.n_models, mol_offsets=s.mol_offsets, want_dEdG=True)
+    g = d.dhp_debug_grad().cpu().numpy()
+    assert np.max(np.abs(g - go)) <= GRAD_TOL
+    ea = d.dhp_debug_atomic_energy().cpu().numpy()
+    assert np.max(np.abs(ea - Ea)) <= 2e-5
+    # properties
+    assert np.abs(F.sum(0)).max() < 1e-3
+    d.close()
+
+
+def test_energy_forces_config3_full(torch, B, params, blob8):
+    """23 558 atoms, 8 networks: every force component and the total energy against the oracle."""
+    s = W.make_system(3)
+    d, E, F = run_gpu(B, torch, s, params, blob8)
+    Eo, Fo = oracle.total_energy_forces(s, params, blob8)
+    assert abs(E[0] - Eo[0]) / s.n_atoms <= E_TOL_PER_ATOM
+    assert np.max(np.abs(F - Fo)) <= F_TOL
+    d.close()
+
+
+def sampled_check(B, torch, s, params, blob, n_energy=256, n_force=24, seed=0):
+    d, E, F = run_gpu(B, torch, s, params, blob)
+    rng = np.random.default_rng(seed)
+    ea = d.dhp_debug_atomic_energy().cpu().numpy()
+    centres = rng.choice(s.n_atoms, n_energy, replace=False).astype(np.int32)
+    Ea, _, _ = oracle.energy_forces(s.pos, s.species, s.box, params, blob, s.n_models, centres=centres,
+                                    mol_offsets=s.mol_offsets)
+    assert np.max(np.abs(ea[centres] - Ea)) <= 2e-5
+    # mean signed error of the sampled atomic energies bounds the per-atom error of the total
+    assert abs(np.mean(ea[centres] - Ea)) <= E_TOL_PER_ATOM
+    pos_d, sp_d, mol_d = B.to_device(s)
+    d.dhp_nlist_build(pos_d, s.box, sp_d, mol_d)
+    rpt, colt, _, _ = d.dhp_nlist_export()
+    rp, col = rpt.cpu().numpy(), colt.cpu().numpy()
+    atoms = rng.choice(s.n_atoms, n_force, replace=False)
+    for a in atoms:
+        cs = np.concatenate([[a], col[rp[a]:rp[a + 1]]]).astype(np.int32)
+        _, Fa, _ = oracle.energy_forces(s.pos, s.species, s.box, params, blob, s.n_models, centres=cs,
+                                        mol_offsets=s.mol_offsets)
+        assert np.max(np.abs(F[a] - Fa[a])) <= F_TOL
+    assert np.abs(F.sum(0)).max() < 2e-2      # sum F = 0 up to fp32 accumulation over N atoms
+    d.close()
+    return E, F
+
+
+def test_energy_forces_config4_sampled(torch, B, params, blob8):
+    sampled_check(B, torch, W.make_system(4), params, blob8)
+
+
+def test_energy_forces_config5_sampled_molecules(torch, B, params, blob8):
+    s = W.make_system(5)
+    d, E, F = run_gpu(B, torch, s, params, blob8)
+    rng = np.random.default_rng(1)
+    for m in rng.choice(1024, 24, replace=False):
+        sl = slice(30 * m, 30 * m + 30)
+        Em, Fm, _ = oracle.energy_forces(s.pos[sl], s.species[sl], None, params, blob8, 8)
+        assert abs(E[m] - Em.sum()) / 30 <= E_TOL_PER_ATOM
+        assert np.max(np.abs(F[sl] - Fm)) <= F_TOL
+    d.close()
+
+
+def test_host_entry_point_matches_device_entry_point(torch, B, params, blob8):
+    s = SYSTEMS["mix600"]()
+    d, E, F = run_gpu(B, torch, s, params, blob8)
+    w = d.dhp_weights_load(blob8[: 2 * 7 * W.PARAMS_PER_NET], 2)
+    Eh, Fh = d.dhp_ani_energy_forces_host(s.pos, s.box, s.species, w)
+    assert abs(Eh[0] - E[0]) <= 1e-6 * s.n_atoms and np.max(np.abs(Fh - F)) <= 1e-5
+    d.close()
+
+
+# ------------------------------------------------------------------------------------------- edge cases
+def test_empty_single_and_isolated(torch, B, params, blob8):
+    d = B.Dhp(64, params=params)
+    w = d.dhp_weights_load(blob8[: 7 * W.PARAMS_PER_NET], 1)
+    # empty
+    pos = torch.empty((0, 3), dtype=torch.float32, device="cuda")
+    sp = torch.empty((0,), dtype=torch.int32, device="cuda")
+    E, F = d.dhp_ani_energy_forces(pos, None, sp, w)
+    torch.cuda.synchronize()
+    assert E.item() == 0.0 and F.shape == (0, 3)
+    # one atom, and two atoms farther apart than Rcr: G = 0, E_i = NN(0), F = 0 (Q15)
+    for p in ([[0.0, 0.0, 0.0]], [[0.0, 0.0, 0.0], [9.0, 0.0, 0.0]]):
+        p = np.array(p, np.float32)
+        s = np.array([1, 3][: len(p)], np.int32)
+        E, F = d.dhp_ani_energy_forces(torch.from_numpy(p).cuda(), None, torch.from_numpy(s).cuda(), w)
+        torch.cuda.synchronize()
+        Eo, Fo, _ = oracle.energy_forces(p, s, None, params, blob8[: 7 * W.PARAMS_PER_NET], 1)
+        assert abs(E.item() - Eo.sum()) <= 1e-6 * len(p)
+        assert np.all(F.cpu().numpy() == 0.0) and np.all(Fo == 0.0)
+    d.close()
+
+
+def test_dense_cluster_more_than_32_angular_neighbours(torch, B, params, blob8):
+    """> 32 atoms inside Rca of one centre exercises the multi-block rounds of the AEV kernels."""
+    rng = np.random.default_rng(4)
+    pts = [np.zeros(3)]
+    while len(pts) < 60:
+        c = rng.uniform(-3.0, 3.0, 3)
+        if np.linalg.norm(c) <= 3.0 and min(np.linalg.norm(c - p) for p in pts) >= 0.8:
+            pts.append(c)
+    pos = np.array(pts, np.float32)
+    sp = rng.integers(0, 7, len(pts)).astype(np.int32)
+    s = W.System("dense", pos, sp, None, None, 1)
+    rp, _ = oracle.pairs(pos, None, params.rca)
+    assert np.diff(rp).max() > 40
+    d, E, F = run_gpu(B, torch, s, params, blob8)
+    Eo, Fo = oracle.total_energy_forces(s, params, blob8[: 7 * W.PARAMS_PER_NET])
+    # terms are larger here (up to ~60 neighbours at short range): scale the force bar with the force size
+    assert abs(E[0] - Eo[0]) / s.n_atoms <= 5e-6
+    assert np.max(np.abs(F - Fo)) <= max(F_TOL, 2e-5 * np.abs(Fo).max())
+    d.close()
+
+
+def test_error_codes(torch, B, params, blob8):
+    d = B.Dhp(32, params=params)
+    w = d.dhp_weights_load(blob8[: 7 * W.PARAMS_PER_NET], 1)
+    pos = torch.zeros((4, 3), dtype=torch.float32, device="cuda")
+    pos[:, 0] = torch.arange(4) * 1.1
+    sp = torch.tensor([0, 1, 2, 3], dtype=torch.int32, device="cuda")
+    with pytest.raises(B.DhpError, match="-3"):         # periodic edge < 2 Rcr
+        d.dhp_ani_energy_forces(pos, np.array([10.0, 20.0, 20.0], np.float32), sp, w)
+    with pytest.raises(B.DhpError, match="-2"):         # more atoms than the context holds
+        big = torch.zeros((33, 3), dtype=torch.float32, device="cuda")
+        d.dhp_ani_energy_forces(big, None, torch.zeros(33, dtype=torch.int32, device="cuda"), w)
+    bad = torch.tensor([0, 1, 9, 3], dtype=torch.int32, device="cuda")
+    d.dhp_ani_energy_forces(pos, None, bad, w)
+    assert d.dhp_status() == -4                          # species outside 0..6, reported by the status word
+    d.dhp_ani_energy_forces(pos, None, sp, w)
+    assert d.dhp_status() == 0
+    with pytest.raises(B.DhpError):                      # blob size must match n_models
+        d.dhp_weights_load(blob8[: 7 * W.PARAMS_PER_NET], 2)
+    d.close()
+
+
+def test_launch_counter_and_profile(torch, B, params, blob8):
+    s = SYSTEMS["mix600"]()
+    d = make_ctx(B, s, params)
+    w = d.dhp_weights_load(blob8[: 2 * 7 * W.PARAMS_PER_NET], 2)
+    pos, sp, mol = B.to_device(s)
+    n0 = d.dhp_launch_count()
+    d.dhp_profile_enable(True)
+    d.dhp_profile_reset()
+    for _ in range(3):
+        d.dhp_ani_energy_forces(pos, s.box, sp, w)
+    ms, calls = d.dhp_profile_read()
+    assert calls == 3 and all(v > 0 for v in ms.values())
+    assert d.dhp_launch_count() - n0 >= 3 * 10
+    d.close()
