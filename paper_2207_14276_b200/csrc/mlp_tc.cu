@@ -1,12 +1,590 @@
-// a3 + a4 on the 5th-generation tensor cores (tcgen05 / TMEM / TMA).  Placeholder until the kernels land:
-// reports "not available" so that DHP_MLP_AUTO uses the SIMT path.
+// a3 + a4 on the 5th-generation tensor cores: tcgen05.mma with TMEM accumulators, operands staged by TMA
+// (Eq. 2, L159 ensemble, L161 "back-propagation" = the dominant cost).
+//
+// Arithmetic.  Single-pass fp16/bf16/tf32 misses the force tolerance by an order of magnitude,
+// so every operand x is kept as a two-term fp16 split  x = hi + lo  (hi = fp16(x), lo = fp16(x - hi)) and every
+// product is three MMAs into the same fp32 accumulator:  hi*hi + hi*lo + lo*hi  (the dropped lo*lo term is
+// 2^-22 relative).  Weights are pre-scaled by 2^6 and back-propagated deltas by 2^10 so that the lo terms stay in
+// the fp16 normal range; the power-of-two scales are removed exactly in the epilogues.
+//
+// One persistent, warp-specialised kernel template does all six GEMMs of the path:
+//   warp 0      TMA producer   (cp.async.bulk.tensor.2d, SWIZZLE_128B, 64-wide K blocks, mbarrier ring)
+//   warp 1      MMA issuer     (one elected lane: 3 x tcgen05.mma.cta_group::1.kind::f16 per 16-wide K step)
+//   warps 2..5  epilogue       (tcgen05.ld 32x32b -> bias / CELU / CELU' / split -> global), overlapped with the
+//                               next tile's MMAs through two TMEM accumulator stages (2 x 256 columns)
+// Tile = 128 rows (atoms of ONE species: row groups start at multiples of 128) x BN columns; tiles of the same
+// row block are adjacent in the schedule so that concurrently running CTAs share the A tile through L2.
+//
+//   G1  H1 = CELU(G W1^T + b1)          K = 1024 (1008 padded)  BN = 256  n-tiles = models
+//   G2  H2 = CELU(H1 W2^T + b2)         K = 256                 BN = 192
+//   G3  H3 = CELU(H2 W3^T + b3);  E_i += (w4.H3 + b4)/M;  D3 = w4 * CELU'(z3) / M      K = 192, BN = 160
+//   B3  D2 = (D3 W3) * CELU'(z2)        K = 160                 BN = 192
+//   B2  D1 = (D2 W2) * CELU'(z1)        K = 192                 BN = 256
+//   B1  dE/dG = sum_e D1_e W1_e         K = models*256          BN = 256  n-tiles = 4
+#include <cuda.h>
+#include <cuda_fp16.h>
+#include <new>
+#include <stdio.h>
+#include <string.h>
+
 #include "dhp_internal.cuh"
 
 namespace dhp {
-bool mlp_tc_available(Ctx*) { return false; }
-int mlp_tc_alloc(Ctx*) { return DHP_OK; }
-void mlp_tc_free(Ctx*) {}
-int mlp_tc_weights(Ctx*, Weights*) { return DHP_OK; }
-void mlp_tc_weights_free(Ctx*, Weights*) {}
-int mlp_tc(Ctx*, const Weights*) { return DHP_E_NOTIMPL; }
+
+namespace {
+
+constexpr int BM = 128;            // rows per tile (UMMA M)
+constexpr int BK = 64;             // K elements per stage (128 bytes of fp16: one SWIZZLE_128B row)
+constexpr int STAGES = 2;
+constexpr int A_PLANE_BYTES = BM * BK * 2;       // 16 KB
+constexpr int B_SLOT_BYTES = 256 * BK * 2;       // 32 KB (BN <= 256)
+constexpr int STAGE_BYTES = 2 * A_PLANE_BYTES + 2 * B_SLOT_BYTES;   // 96 KB
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
+constexpr int TMEM_COLS = 512;
+constexpr int ACC_STRIDE = 256;    // TMEM columns per accumulator stage
+constexpr int TC_THREADS = 192;
+constexpr float W_SCALE = 64.0f;       // 2^6 on every weight matrix
+constexpr float D_SCALE = 1024.0f;     // 2^10 on the back-propagated deltas
+
+enum { EPI_CELU = 0, EPI_OUT = 1, EPI_DCELU = 2, EPI_GRAD = 3 };
+
+struct TcArgs {
+    int K;                    // reduction length in elements (multiple of 16)
+    int BN;                   // tile width (multiple of 16, <= 256)
+    int n_tiles;              // column tiles per row block
+    int a_k_off_per_tile;     // A column offset per column tile (per-model activations), else 0
+    int a_plane_rows;         // rows of one A plane (lo plane starts there)
+    int b_rows_per_species;   // rows of one B plane of one species
+    int b_rows_per_tile;      // B row offset per column tile
+    float acc_scale;          // removes the power-of-two operand scales
+    const int* row_species;
+    const int* sp_start;
+    const float* bias;        // [species][n_tiles*BN]  (EPI_CELU, EPI_OUT)
+    const float* w4;          // [species][models*160]  (EPI_OUT)
+    const float* b4;          // [species][models]
+    float inv_models;
+    float alpha;
+    __half* out_planes;       // [2][out_plane_rows][out_ld]  hi plane then lo plane
+    int out_ld;
+    int out_plane_rows;
+    const __half* h_planes;   // saved activations for CELU' (EPI_DCELU), same geometry as out
+    float* out_f32;           // EPI_GRAD: [rows][out_ld]
+    float* e_atom;            // EPI_OUT
+};
+
+// ---- PTX wrappers ------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.b32 %0, 1, 0, P;\n\t}" : "=r"(pred));
+    return pred != 0;
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n\t.reg .pred P;\n"
+        "WAIT_LOOP:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 P, [%0], %1;\n\t"
+        "@P bra DONE;\n\t"
+        "bra WAIT_LOOP;\n"
+        "DONE:\n\t}" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                 ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void prefetch_tmap(const CUtensorMap* map) {
+    asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t cols) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(cols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t cols) {
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(cols) : "memory");
+}
+__device__ __forceinline__ void umma_f16(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+        ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+          "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+          "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr) : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
+// K-major, SWIZZLE_128B shared-memory matrix descriptor (sm_100 format): start address >> 4 in bits [0,14),
+// stride byte offset (8 rows x 128 B = 1024) >> 4 in bits [32,46), version 1 in bits [46,48), layout type 2
+// (SWIZZLE_128B) in bits [61,64).  The leading byte offset is unused for swizzled K-major operands.
+__device__ __forceinline__ uint64_t make_smem_desc(uint32_t saddr) {
+    uint64_t d = 0;
+    d |= (uint64_t)((saddr & 0x3FFFF) >> 4);
+    d |= (uint64_t)(1024 >> 4) << 32;
+    d |= (uint64_t)1 << 46;
+    d |= (uint64_t)2 << 61;
+    return d;
+}
+// instruction descriptor: D = f32, A = B = f16, both K-major, M = 128, N = bn
+__device__ __forceinline__ uint32_t make_idesc(int bn) {
+    return (1u << 4) | ((uint32_t)(bn >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+}
+
+__device__ __forceinline__ float celu_f(float v, float alpha) { return v > 0.f ? v : alpha * expm1f(v / alpha); }
+__device__ __forceinline__ float dcelu_from_h(float h, float alpha) { return h > 0.f ? 1.0f : h / alpha + 1.0f; }
+
+__device__ __forceinline__ void split_half(float x, __half& hi, __half& lo) {
+    x = fminf(fmaxf(x, -65000.f), 65000.f);
+    hi = __float2half_rn(x);
+    lo = __float2half_rn(x - __half2float(hi));
+}
+
+__device__ __forceinline__ uint32_t pack_half2(__half a, __half b) {
+    __half2 h = __halves2half2(a, b);
+    return *reinterpret_cast<uint32_t*>(&h);
+}
+// 32 consecutive values of one row -> hi and lo planes (4 x 16-byte stores each)
+__device__ __forceinline__ void store_split32(const float (&x)[32], __half* hi_dst, __half* lo_dst) {
+    uint32_t ph[16], pl[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        __half h0, l0, h1, l1;
+        split_half(x[2 * i], h0, l0);
+        split_half(x[2 * i + 1], h1, l1);
+        ph[i] = pack_half2(h0, h1);
+        pl[i] = pack_half2(l0, l1);
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        reinterpret_cast<uint4*>(hi_dst)[i] = make_uint4(ph[4 * i], ph[4 * i + 1], ph[4 * i + 2], ph[4 * i + 3]);
+        reinterpret_cast<uint4*>(lo_dst)[i] = make_uint4(pl[4 * i], pl[4 * i + 1], pl[4 * i + 2], pl[4 * i + 3]);
+    }
+}
+__device__ __forceinline__ void unpack_add(uint32_t h, uint32_t l, float& a, float& b) {
+    const float2 fh = __half22float2(*reinterpret_cast<__half2*>(&h));
+    const float2 fl = __half22float2(*reinterpret_cast<__half2*>(&l));
+    a = fh.x + fl.x;
+    b = fh.y + fl.y;
+}
+__device__ __forceinline__ void load_joined32(const __half* hi_src, const __half* lo_src, float (&x)[32]) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const uint4 h = reinterpret_cast<const uint4*>(hi_src)[i];
+        const uint4 l = reinterpret_cast<const uint4*>(lo_src)[i];
+        unpack_add(h.x, l.x, x[8 * i + 0], x[8 * i + 1]);
+        unpack_add(h.y, l.y, x[8 * i + 2], x[8 * i + 3]);
+        unpack_add(h.z, l.z, x[8 * i + 4], x[8 * i + 5]);
+        unpack_add(h.w, l.w, x[8 * i + 6], x[8 * i + 7]);
+    }
+}
+
+template <int EPI>
+__global__ void __launch_bounds__(TC_THREADS, 1)
+k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const TcArgs p) {
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t raw = smem_u32(smem_raw);
+    const uint32_t base = (raw + 1023u) & ~1023u;                      // SWIZZLE_128B tiles need 1024-byte alignment
+    uint8_t* base_ptr = smem_raw + (base - raw);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(base_ptr + STAGES * STAGE_BYTES);
+    const uint32_t bar0 = base + STAGES * STAGE_BYTES;
+    // barrier layout: full[STAGES], empty[STAGES], tfull[2], tempty[2], then the TMEM base address word
+    auto full_bar = [&](int s) { return bar0 + 8u * s; };
+    auto empty_bar = [&](int s) { return bar0 + 8u * (STAGES + s); };
+    auto tfull_bar = [&](int s) { return bar0 + 8u * (2 * STAGES + s); };
+    auto tempty_bar = [&](int s) { return bar0 + 8u * (2 * STAGES + 2 + s); };
+    volatile uint32_t* tmem_word = reinterpret_cast<volatile uint32_t*>(bars + 2 * STAGES + 4);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n_row_tiles = p.sp_start[NSP] / BM;
+    const int total_tiles = n_row_tiles * p.n_tiles;
+    const int KB = (p.K + BK - 1) / BK;
+
+    if (warp == 0 && lane == 0) {
+        for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+        for (int s = 0; s < 2; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), 4); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        prefetch_tmap(&tmA);
+        prefetch_tmap(&tmB);
+    }
+    if (warp == 1) tmem_alloc(smem_u32((const void*)tmem_word), TMEM_COLS);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_word;
+
+    if (warp == 0) {
+        // ===== TMA producer =====
+        if (elect_one()) {
+            int stage = 0; uint32_t phase = 0;
+            const uint32_t tx = 2u * A_PLANE_BYTES + 2u * (uint32_t)p.BN * BK * 2u;
+            for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+                const int rt = tile / p.n_tiles, nt = tile - rt * p.n_tiles;
+                const int row0 = rt * BM;
+                const int s = max(p.row_species[row0], 0);
+                const int brow = (2 * s) * p.b_rows_per_species + nt * p.b_rows_per_tile;
+                for (int kb = 0; kb < KB; ++kb) {
+                    mbar_wait(empty_bar(stage), phase ^ 1u);
+                    const uint32_t sa = base + stage * STAGE_BYTES;
+                    mbar_expect_tx(full_bar(stage), tx);
+                    const int ka = p.a_k_off_per_tile * nt + kb * BK;
+                    tma_load_2d(sa, &tmA, ka, row0, full_bar(stage));
+                    tma_load_2d(sa + A_PLANE_BYTES, &tmA, ka, p.a_plane_rows + row0, full_bar(stage));
+                    tma_load_2d(sa + 2 * A_PLANE_BYTES, &tmB, kb * BK, brow, full_bar(stage));
+                    tma_load_2d(sa + 2 * A_PLANE_BYTES + B_SLOT_BYTES, &tmB, kb * BK, brow + p.b_rows_per_species, full_bar(stage));
+                    if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer =====
+        if (elect_one()) {
+            int stage = 0; uint32_t phase = 0;
+            int acc = 0; uint32_t acc_phase = 0;
+            const uint32_t idesc = make_idesc(p.BN);
+            for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+                mbar_wait(tempty_bar(acc), acc_phase ^ 1u);
+                tc_fence_after();
+                const uint32_t d_tmem = tmem_base + (uint32_t)(acc * ACC_STRIDE);
+                for (int kb = 0; kb < KB; ++kb) {
+                    mbar_wait(full_bar(stage), phase);
+                    tc_fence_after();
+                    const uint32_t sa = base + stage * STAGE_BYTES;
+                    const uint64_t a_hi = make_smem_desc(sa), a_lo = make_smem_desc(sa + A_PLANE_BYTES);
+                    const uint64_t b_hi = make_smem_desc(sa + 2 * A_PLANE_BYTES);
+                    const uint64_t b_lo = make_smem_desc(sa + 2 * A_PLANE_BYTES + B_SLOT_BYTES);
+                    const int ksteps = min(BK / 16, (p.K - kb * BK) / 16);
+                    for (int k = 0; k < ksteps; ++k) {
+                        const uint64_t adv = (uint64_t)(k * 2);          // 16 fp16 = 32 bytes = 2 x 16-byte units
+                        umma_f16(d_tmem, a_hi + adv, b_hi + adv, idesc, (kb | k) ? 1u : 0u);
+                        umma_f16(d_tmem, a_hi + adv, b_lo + adv, idesc, 1u);
+                        umma_f16(d_tmem, a_lo + adv, b_hi + adv, idesc, 1u);
+                    }
+                    umma_commit(empty_bar(stage));                     // frees the smem stage when the MMAs retire
+                    if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                }
+                umma_commit(tfull_bar(acc));                           // accumulator complete -> epilogue
+                if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+            }
+        }
+    } else {
+        // ===== epilogue (warps 2..5; a warp may touch only TMEM lanes 32*(warp%4) .. +31) =====
+        const int q = warp & 3;
+        int acc = 0; uint32_t acc_phase = 0;
+        for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+            const int rt = tile / p.n_tiles, nt = tile - rt * p.n_tiles;
+            const int row = rt * BM + q * 32 + lane;
+            const int s = max(p.row_species[rt * BM], 0);
+            mbar_wait(tfull_bar(acc), acc_phase);
+            tc_fence_after();
+            const uint32_t t_row = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * ACC_STRIDE);
+            const int ncols = p.n_tiles * p.BN;
+            float e_acc = 0.f;
+            for (int c0 = 0; c0 < p.BN; c0 += 32) {
+                uint32_t v[32];
+                tmem_ld32(t_row + (uint32_t)c0, v);
+                float x[32];
+                const int col = nt * p.BN + c0;
+                if (EPI == EPI_CELU || EPI == EPI_OUT) {
+                    const float* bias = p.bias + (size_t)s * ncols + col;
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) x[i] = celu_f(__uint_as_float(v[i]) * p.acc_scale + bias[i], p.alpha);
+                }
+                if (EPI == EPI_CELU) {
+                    __half* hi = p.out_planes + (size_t)row * p.out_ld + col;
+                    store_split32(x, hi, hi + (size_t)p.out_plane_rows * p.out_ld);
+                } else if (EPI == EPI_OUT) {
+                    const float* w4 = p.w4 + (size_t)s * ncols + col;
+                    const float dsc = p.inv_models * D_SCALE;
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) {
+                        const float wv = w4[i];
+                        e_acc = fmaf(wv, x[i], e_acc);
+                        x[i] = wv * dcelu_from_h(x[i], p.alpha) * dsc;
+                    }
+                    __half* hi = p.out_planes + (size_t)row * p.out_ld + col;
+                    store_split32(x, hi, hi + (size_t)p.out_plane_rows * p.out_ld);
+                } else if (EPI == EPI_DCELU) {
+                    float h[32];
+                    const __half* hh = p.h_planes + (size_t)row * p.out_ld + col;
+                    load_joined32(hh, hh + (size_t)p.out_plane_rows * p.out_ld, h);
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) x[i] = __uint_as_float(v[i]) * p.acc_scale * dcelu_from_h(h[i], p.alpha);
+                    __half* hi = p.out_planes + (size_t)row * p.out_ld + col;
+                    store_split32(x, hi, hi + (size_t)p.out_plane_rows * p.out_ld);
+                } else {   // EPI_GRAD
+                    float4* dst = reinterpret_cast<float4*>(p.out_f32 + (size_t)row * p.out_ld + col);
+#pragma unroll
+                    for (int i = 0; i < 8; ++i)
+                        dst[i] = make_float4(__uint_as_float(v[4 * i]) * p.acc_scale, __uint_as_float(v[4 * i + 1]) * p.acc_scale,
+                                             __uint_as_float(v[4 * i + 2]) * p.acc_scale, __uint_as_float(v[4 * i + 3]) * p.acc_scale);
+                }
+            }
+            if (EPI == EPI_OUT) atomicAdd(&p.e_atom[row], (e_acc + p.b4[s * p.n_tiles + nt]) * p.inv_models);
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(tempty_bar(acc));
+            if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) tmem_dealloc(tmem_base, TMEM_COLS);
+}
+
+// ---- operand preparation -------------------------------------------------------------------------------
+// fp32 rows -> hi / lo fp16 planes (AEV rows for G1)
+__global__ void k_split_rows(const float* __restrict__ src, int ld_src, const int* __restrict__ sp_start, int ncol,
+                             __half* __restrict__ dst, int plane_rows) {
+    const int rows = sp_start[NSP];
+    const size_t total = (size_t)rows * (ncol / 4);
+    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
+        const int r = (int)(idx / (ncol / 4)), c = (int)(idx % (ncol / 4)) * 4;
+        const float4 v = *reinterpret_cast<const float4*>(src + (size_t)r * ld_src + c);
+        __half h[4], l[4];
+        split_half(v.x, h[0], l[0]); split_half(v.y, h[1], l[1]); split_half(v.z, h[2], l[2]); split_half(v.w, h[3], l[3]);
+        *reinterpret_cast<uint2*>(dst + (size_t)r * ncol + c) = *reinterpret_cast<uint2*>(h);
+        *reinterpret_cast<uint2*>(dst + ((size_t)plane_rows + r) * ncol + c) = *reinterpret_cast<uint2*>(l);
+    }
+}
+
+// weight tiles: dst[(2*s + plane)*rows + r][c] = split(W_SCALE * src(r, c)); see the modes below
+enum { WP_W1F = 0, WP_W2F, WP_W3F, WP_W3B, WP_W2B, WP_W1B };
+__global__ void k_prep_weights(const float* __restrict__ blob, int n_models, int mode, int rows, int cols, __half* __restrict__ dst) {
+    const int s = blockIdx.y;
+    const size_t total = (size_t)rows * cols;
+    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
+        const int r = (int)(idx / cols), c = (int)(idx % cols);
+        float v = 0.f;
+        int e, n, k;
+        switch (mode) {
+            case WP_W1F: e = r / H1; n = r % H1; k = c;
+                if (k < AEV_DIM) v = blob[(size_t)(e * NSP + s) * NET_PARAMS + OFF_W1 + (size_t)n * AEV_DIM + k]; break;
+            case WP_W2F: e = r / H2; n = r % H2; k = c;
+                v = blob[(size_t)(e * NSP + s) * NET_PARAMS + OFF_W2 + n * H1 + k]; break;
+            case WP_W3F: e = r / H3; n = r % H3; k = c;
+                v = blob[(size_t)(e * NSP + s) * NET_PARAMS + OFF_W3 + n * H2 + k]; break;
+            case WP_W3B: e = r / H2; n = r % H2; k = c;          // B(n,k) = W3[k][n]
+                v = blob[(size_t)(e * NSP + s) * NET_PARAMS + OFF_W3 + k * H2 + n]; break;
+            case WP_W2B: e = r / H1; n = r % H1; k = c;          // B(n,k) = W2[k][n]
+                v = blob[(size_t)(e * NSP + s) * NET_PARAMS + OFF_W2 + k * H1 + n]; break;
+            default: n = r; e = c / H1; k = c % H1;              // WP_W1B: B(n, e*256+j) = W1_e[j][n]
+                if (n < AEV_DIM) v = blob[(size_t)(e * NSP + s) * NET_PARAMS + OFF_W1 + (size_t)k * AEV_DIM + n]; break;
+        }
+        __half hi, lo;
+        split_half(v * W_SCALE, hi, lo);
+        dst[((size_t)(2 * s) * rows + r) * cols + c] = hi;
+        dst[((size_t)(2 * s + 1) * rows + r) * cols + c] = lo;
+    }
+}
+__global__ void k_prep_small(const float* __restrict__ blob, int n_models, float* __restrict__ b1, float* __restrict__ b2,
+                             float* __restrict__ b3, float* __restrict__ w4, float* __restrict__ b4) {
+    const int s = blockIdx.x;
+    for (int e = 0; e < n_models; ++e) {
+        const float* net = blob + (size_t)(e * NSP + s) * NET_PARAMS;
+        for (int i = threadIdx.x; i < H1; i += blockDim.x) b1[(size_t)s * n_models * H1 + e * H1 + i] = net[OFF_B1 + i];
+        for (int i = threadIdx.x; i < H2; i += blockDim.x) b2[(size_t)s * n_models * H2 + e * H2 + i] = net[OFF_B2 + i];
+        for (int i = threadIdx.x; i < H3; i += blockDim.x) {
+            b3[(size_t)s * n_models * H3 + e * H3 + i] = net[OFF_B3 + i];
+            w4[(size_t)s * n_models * H3 + e * H3 + i] = net[OFF_W4 + i];
+        }
+        if (threadIdx.x == 0) b4[s * n_models + e] = net[OFF_B4];
+    }
+}
+
+// ---- host ------------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode() {
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+        else
+            cudaGetLastError();
+    }
+    return fn;
+}
+
+// 2-D fp16 tensor [rows][cols] row-major, box = 64 columns x box_rows rows, 128-byte swizzle
+bool make_map(CUtensorMap* m, const void* ptr, uint64_t rows, uint64_t cols, uint32_t box_rows) {
+    EncodeTiledFn enc = get_encode();
+    if (!enc) return false;
+    cuuint64_t dims[2] = {cols, rows};
+    cuuint64_t strides[1] = {cols * 2};
+    cuuint32_t box[2] = {BK, box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, const_cast<void*>(ptr), dims, strides, box, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+struct TcWorkspace {                  // activations, per context
+    __half *aev, *h1, *h2, *d3, *d2, *d1;          // [2][max_rows][width]
+    CUtensorMap m_aev, m_h1, m_h2, m_d3, m_d2, m_d1;
+    int models;
+};
+struct TcWeights {                    // per weight handle
+    __half *w1f, *w2f, *w3f, *w3b, *w2b, *w1b;
+    float *b1, *b2, *b3, *w4, *b4;
+    CUtensorMap m_w1f, m_w2f, m_w3f, m_w3b, m_w2b, m_w1b;
+};
+
+template <int EPI>
+int launch_gemm(Ctx* ctx, const CUtensorMap& a, const CUtensorMap& b, const TcArgs& args) {
+    static bool attr = false;
+    if (!attr) {
+        DHP_CUDA(ctx, cudaFuncSetAttribute(k_gemm_tc<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
+        attr = true;
+    }
+    DHP_LAUNCH(ctx, k_gemm_tc<EPI>, ctx->sm_count, TC_THREADS, SMEM_BYTES, a, b, args);
+    return DHP_OK;
+}
+
+}  // namespace
+
+bool mlp_tc_available(Ctx* ctx) { return ctx->cc_major == 10 && get_encode() != nullptr; }
+
+int mlp_tc_alloc(Ctx* ctx) {
+    TcWorkspace* w = new (std::nothrow) TcWorkspace();
+    if (!w) return DHP_E_NOMEM;
+    memset((void*)w, 0, sizeof(*w));
+    ctx->tc_ws = w;
+    const size_t R = (size_t)ctx->max_rows, M = MAX_MODELS;
+    struct { __half** p; size_t width; CUtensorMap* m; } bufs[] = {
+        {&w->aev, (size_t)AEV_LD, &w->m_aev}, {&w->h1, M * H1, &w->m_h1}, {&w->h2, M * H2, &w->m_h2},
+        {&w->d3, M * H3, &w->m_d3},           {&w->d2, M * H2, &w->m_d2}, {&w->d1, M * H1, &w->m_d1}};
+    for (auto& b : bufs) {
+        if (cudaMalloc((void**)b.p, 2 * R * b.width * sizeof(__half)) != cudaSuccess) return DHP_E_NOMEM;
+        if (cudaMemset(*b.p, 0, 2 * R * b.width * sizeof(__half)) != cudaSuccess) return DHP_E_CUDA;
+        if (!make_map(b.m, *b.p, 2 * R, b.width, BM)) return DHP_E_CUDA;
+    }
+    w->models = MAX_MODELS;
+    return DHP_OK;
+}
+
+void mlp_tc_free(Ctx* ctx) {
+    TcWorkspace* w = (TcWorkspace*)ctx->tc_ws;
+    if (!w) return;
+    __half* ptrs[] = {w->aev, w->h1, w->h2, w->d3, w->d2, w->d1};
+    for (__half* p : ptrs) if (p) cudaFree(p);
+    delete w;
+    ctx->tc_ws = nullptr;
+}
+
+int mlp_tc_weights(Ctx* ctx, Weights* wt) {
+    TcWeights* t = new (std::nothrow) TcWeights();
+    if (!t) return DHP_E_NOMEM;
+    memset((void*)t, 0, sizeof(*t));
+    wt->tc = t;
+    const int M = wt->n_models;
+    struct { __half** p; int mode, rows, cols; CUtensorMap* m; uint32_t box_rows; } mats[] = {
+        {&t->w1f, WP_W1F, M * H1, AEV_LD, &t->m_w1f, (uint32_t)H1}, {&t->w2f, WP_W2F, M * H2, H1, &t->m_w2f, (uint32_t)H2},
+        {&t->w3f, WP_W3F, M * H3, H2, &t->m_w3f, (uint32_t)H3},     {&t->w3b, WP_W3B, M * H2, H3, &t->m_w3b, (uint32_t)H2},
+        {&t->w2b, WP_W2B, M * H1, H2, &t->m_w2b, (uint32_t)H1},     {&t->w1b, WP_W1B, AEV_LD, M * H1, &t->m_w1b, 256u}};
+    for (auto& m : mats) {
+        const size_t n = (size_t)2 * NSP * m.rows * m.cols;
+        if (cudaMalloc((void**)m.p, n * sizeof(__half)) != cudaSuccess) return DHP_E_NOMEM;
+        DHP_LAUNCH(ctx, k_prep_weights, dim3(256, NSP), 256, 0, wt->blob, M, m.mode, m.rows, m.cols, *m.p);
+        if (!make_map(m.m, *m.p, (uint64_t)2 * NSP * m.rows, m.cols, m.box_rows)) return DHP_E_CUDA;
+    }
+    float** smalls[] = {&t->b1, &t->b2, &t->b3, &t->w4, &t->b4};
+    const size_t sizes[] = {(size_t)NSP * M * H1, (size_t)NSP * M * H2, (size_t)NSP * M * H3, (size_t)NSP * M * H3, (size_t)NSP * M};
+    for (int i = 0; i < 5; ++i)
+        if (cudaMalloc((void**)smalls[i], sizes[i] * sizeof(float)) != cudaSuccess) return DHP_E_NOMEM;
+    DHP_LAUNCH(ctx, k_prep_small, NSP, 256, 0, wt->blob, M, t->b1, t->b2, t->b3, t->w4, t->b4);
+    DHP_CUDA(ctx, cudaGetLastError());
+    DHP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return DHP_OK;
+}
+
+void mlp_tc_weights_free(Ctx*, Weights* wt) {
+    TcWeights* t = (TcWeights*)wt->tc;
+    if (!t) return;
+    void* ptrs[] = {t->w1f, t->w2f, t->w3f, t->w3b, t->w2b, t->w1b, t->b1, t->b2, t->b3, t->w4, t->b4};
+    for (void* p : ptrs) if (p) cudaFree(p);
+    delete t;
+    wt->tc = nullptr;
+}
+
+int mlp_tc(Ctx* ctx, const Weights* wt) {
+    if (ctx->n_atoms == 0) return DHP_OK;
+    TcWorkspace* ws = (TcWorkspace*)ctx->tc_ws;
+    const TcWeights* t = (const TcWeights*)wt->tc;
+    if (!ws || !t) return DHP_E_NOTIMPL;
+    const int M = wt->n_models;
+    const int R = (int)ctx->max_rows;
+    int rc;
+    // activation maps depend on the ensemble size through the row pitch
+    if (ws->models != M) {
+        struct { __half* p; size_t width; CUtensorMap* m; } bufs[] = {
+            {ws->h1, (size_t)M * H1, &ws->m_h1}, {ws->h2, (size_t)M * H2, &ws->m_h2}, {ws->d3, (size_t)M * H3, &ws->m_d3},
+            {ws->d2, (size_t)M * H2, &ws->m_d2}, {ws->d1, (size_t)M * H1, &ws->m_d1}};
+        for (auto& b : bufs) if (!make_map(b.m, b.p, (uint64_t)2 * R, b.width, BM)) return DHP_E_CUDA;
+        ws->models = M;
+    }
+    DHP_CUDA(ctx, cudaMemsetAsync(ctx->e_atom, 0, sizeof(float) * ctx->max_rows, ctx->stream));
+    DHP_LAUNCH(ctx, k_split_rows, 4 * ctx->sm_count, 256, 0, ctx->aev, AEV_LD, ctx->sp_start, AEV_LD, ws->aev, R);
+
+    TcArgs a{};
+    a.row_species = ctx->row_species; a.sp_start = ctx->sp_start; a.alpha = ctx->params.celu_alpha;
+    a.inv_models = 1.0f / (float)M; a.a_plane_rows = R; a.out_plane_rows = R; a.e_atom = ctx->e_atom;
+    a.w4 = t->w4; a.b4 = t->b4;
+    // G1
+    a.K = AEV_LD; a.BN = H1; a.n_tiles = M; a.a_k_off_per_tile = 0; a.b_rows_per_species = M * H1; a.b_rows_per_tile = H1;
+    a.acc_scale = 1.0f / W_SCALE; a.bias = t->b1; a.out_planes = ws->h1; a.out_ld = M * H1;
+    if ((rc = launch_gemm<EPI_CELU>(ctx, ws->m_aev, t->m_w1f, a)) != DHP_OK) return rc;
+    // G2
+    a.K = H1; a.BN = H2; a.a_k_off_per_tile = H1; a.b_rows_per_species = M * H2; a.b_rows_per_tile = H2;
+    a.bias = t->b2; a.out_planes = ws->h2; a.out_ld = M * H2;
+    if ((rc = launch_gemm<EPI_CELU>(ctx, ws->m_h1, t->m_w2f, a)) != DHP_OK) return rc;
+    // G3 + output layer + seed of the backward pass
+    a.K = H2; a.BN = H3; a.a_k_off_per_tile = H2; a.b_rows_per_species = M * H3; a.b_rows_per_tile = H3;
+    a.bias = t->b3; a.out_planes = ws->d3; a.out_ld = M * H3;
+    if ((rc = launch_gemm<EPI_OUT>(ctx, ws->m_h2, t->m_w3f, a)) != DHP_OK) return rc;
+    // B3
+    a.K = H3; a.BN = H2; a.a_k_off_per_tile = H3; a.b_rows_per_species = M * H2; a.b_rows_per_tile = H2;
+    a.h_planes = ws->h2; a.out_planes = ws->d2; a.out_ld = M * H2;
+    if ((rc = launch_gemm<EPI_DCELU>(ctx, ws->m_d3, t->m_w3b, a)) != DHP_OK) return rc;
+    // B2
+    a.K = H2; a.BN = H1; a.a_k_off_per_tile = H2; a.b_rows_per_species = M * H1; a.b_rows_per_tile = H1;
+    a.h_planes = ws->h1; a.out_planes = ws->d1; a.out_ld = M * H1;
+    if ((rc = launch_gemm<EPI_DCELU>(ctx, ws->m_d2, t->m_w2b, a)) != DHP_OK) return rc;
+    // B1
+    a.K = M * H1; a.BN = 256; a.n_tiles = AEV_LD / 256; a.a_k_off_per_tile = 0; a.b_rows_per_species = AEV_LD; a.b_rows_per_tile = 256;
+    a.acc_scale = 1.0f / (W_SCALE * D_SCALE); a.out_f32 = ctx->grad; a.out_ld = AEV_LD;
+    if ((rc = launch_gemm<EPI_GRAD>(ctx, ws->m_d1, t->m_w1b, a)) != DHP_OK) return rc;
+    DHP_CUDA(ctx, cudaGetLastError());
+    return DHP_OK;
+}
+
 }  // namespace dhp
