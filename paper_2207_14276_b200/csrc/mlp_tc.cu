@@ -42,7 +42,8 @@ constexpr int STAGE_BYTES = 2 * A_PLANE_BYTES + 2 * B_SLOT_BYTES;   // 96 KB
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
 constexpr int TMEM_COLS = 512;
 constexpr int ACC_STRIDE = 256;    // TMEM columns per accumulator stage
-constexpr int TC_THREADS = 192;
+constexpr int EPI_WARPS = 8;         // two per TMEM lane quadrant, splitting the column chunks
+constexpr int TC_THREADS = 64 + 32 * EPI_WARPS;
 constexpr float W_SCALE = 64.0f;       // 2^6 on every weight matrix
 constexpr float D_SCALE = 1024.0f;     // 2^10 on the back-propagated deltas
 
@@ -124,7 +125,7 @@ __device__ __forceinline__ void umma_f16(uint32_t d_tmem, uint64_t a_desc, uint6
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
+__device__ __forceinline__ void tmem_ld32_issue(uint32_t taddr, uint32_t (&v)[32]) {
     asm volatile(
         "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
         "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
@@ -134,8 +135,8 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
           "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
           "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
         : "r"(taddr) : "memory");
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 // K-major, SWIZZLE_128B shared-memory matrix descriptor (sm_100 format): start address >> 4 in bits [0,14),
 // stride byte offset (8 rows x 128 B = 1024) >> 4 in bits [32,46), version 1 in bits [46,48), layout type 2
@@ -153,9 +154,31 @@ __device__ __forceinline__ uint32_t make_idesc(int bn) {
     return (1u << 4) | ((uint32_t)(bn >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
 }
 
-__device__ __forceinline__ float celu_f(float v, float alpha) { return v > 0.f ? v : alpha * expm1f(v / alpha); }
-__device__ __forceinline__ float dcelu_from_h(float h, float alpha) { return h > 0.f ? 1.0f : h / alpha + 1.0f; }
+// CELU(v) = v (v > 0), alpha (exp(v/alpha) - 1) otherwise; k = log2(e)/alpha.  ex2.approx has 2^-22 relative error,
+// so the absolute error of the negative branch is <= alpha 2^-22 (2.4e-8 at alpha = 0.1), below fp32 eps of O(1) values.
+__device__ __forceinline__ float fast_ex2(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float celu_f(float v, float alpha, float k) {
+    const float e = fmaf(alpha, fast_ex2(v * k), -alpha);
+    return v > 0.f ? v : e;
+}
+__device__ __forceinline__ float dcelu_from_h(float h, float inv_alpha) { return h > 0.f ? 1.0f : fmaf(h, inv_alpha, 1.0f); }
 
+// two floats -> packed fp16 pair, round-to-nearest, saturating to the largest finite fp16 (first argument -> low half)
+__device__ __forceinline__ uint32_t cvt_pack(float lo_half, float hi_half) {
+    uint32_t r;
+    asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi_half), "f"(lo_half));
+    return r;
+}
+// x = hi + lo for two values at once: hi = fp16(x), lo = fp16(x - hi)
+__device__ __forceinline__ void split_pair(float x0, float x1, uint32_t& hi, uint32_t& lo) {
+    hi = cvt_pack(x0, x1);
+    const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&hi));
+    lo = cvt_pack(x0 - f.x, x1 - f.y);
+}
 __device__ __forceinline__ void split_half(float x, __half& hi, __half& lo) {
     x = fminf(fmaxf(x, -65000.f), 65000.f);
     hi = __float2half_rn(x);
@@ -170,17 +193,18 @@ __device__ __forceinline__ uint32_t pack_half2(__half a, __half b) {
 __device__ __forceinline__ void store_split32(const float (&x)[32], __half* hi_dst, __half* lo_dst) {
     uint32_t ph[16], pl[16];
 #pragma unroll
-    for (int i = 0; i < 16; ++i) {
-        __half h0, l0, h1, l1;
-        split_half(x[2 * i], h0, l0);
-        split_half(x[2 * i + 1], h1, l1);
-        ph[i] = pack_half2(h0, h1);
-        pl[i] = pack_half2(l0, l1);
-    }
+    for (int i = 0; i < 16; ++i) split_pair(x[2 * i], x[2 * i + 1], ph[i], pl[i]);
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         reinterpret_cast<uint4*>(hi_dst)[i] = make_uint4(ph[4 * i], ph[4 * i + 1], ph[4 * i + 2], ph[4 * i + 3]);
         reinterpret_cast<uint4*>(lo_dst)[i] = make_uint4(pl[4 * i], pl[4 * i + 1], pl[4 * i + 2], pl[4 * i + 3]);
+    }
+}
+__device__ __forceinline__ void load32(const float* __restrict__ src, float (&x)[32]) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const float4 v = __ldg(reinterpret_cast<const float4*>(src) + i);
+        x[4 * i] = v.x; x[4 * i + 1] = v.y; x[4 * i + 2] = v.z; x[4 * i + 3] = v.w;
     }
 }
 __device__ __forceinline__ void unpack_add(uint32_t h, uint32_t l, float& a, float& b) {
@@ -224,7 +248,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
 
     if (warp == 0 && lane == 0) {
         for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-        for (int s = 0; s < 2; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), 4); }
+        for (int s = 0; s < 2; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), EPI_WARPS); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         prefetch_tmap(&tmA);
         prefetch_tmap(&tmB);
@@ -290,50 +314,54 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
             }
         }
     } else {
-        // ===== epilogue (warps 2..5; a warp may touch only TMEM lanes 32*(warp%4) .. +31) =====
-        const int q = warp & 3;
+        // ===== epilogue (warps 2..9; a warp may touch only TMEM lanes 32*(warp%4) .. +31; the two warps of a
+        //       lane quadrant take alternate 32-column chunks) =====
+        const int q = warp & 3, half = (warp - 2) >> 2;
         int acc = 0; uint32_t acc_phase = 0;
+        const float kexp = 1.4426950408889634f / p.alpha, inv_alpha = 1.0f / p.alpha;
         for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
             const int rt = tile / p.n_tiles, nt = tile - rt * p.n_tiles;
             const int row = rt * BM + q * 32 + lane;
             const int s = max(p.row_species[rt * BM], 0);
+            const int ncols = p.n_tiles * p.BN;
+            const size_t plane = (size_t)p.out_plane_rows * p.out_ld;
             mbar_wait(tfull_bar(acc), acc_phase);
             tc_fence_after();
             const uint32_t t_row = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * ACC_STRIDE);
-            const int ncols = p.n_tiles * p.BN;
             float e_acc = 0.f;
-            for (int c0 = 0; c0 < p.BN; c0 += 32) {
-                uint32_t v[32];
-                tmem_ld32(t_row + (uint32_t)c0, v);
-                float x[32];
+            for (int c0 = half * 32; c0 < p.BN; c0 += 64) {
                 const int col = nt * p.BN + c0;
+                uint32_t v[32];
+                float x[32], aux[32];
+                tmem_ld32_issue(t_row + (uint32_t)c0, v);
+                if (EPI == EPI_CELU || EPI == EPI_OUT) load32(p.bias + (size_t)s * ncols + col, aux);
+                if (EPI == EPI_DCELU) {
+                    const __half* hh = p.h_planes + (size_t)row * p.out_ld + col;
+                    load_joined32(hh, hh + plane, aux);
+                }
+                tmem_ld_wait();
                 if (EPI == EPI_CELU || EPI == EPI_OUT) {
-                    const float* bias = p.bias + (size_t)s * ncols + col;
 #pragma unroll
-                    for (int i = 0; i < 32; ++i) x[i] = celu_f(__uint_as_float(v[i]) * p.acc_scale + bias[i], p.alpha);
+                    for (int i = 0; i < 32; ++i) x[i] = celu_f(fmaf(__uint_as_float(v[i]), p.acc_scale, aux[i]), p.alpha, kexp);
                 }
                 if (EPI == EPI_CELU) {
                     __half* hi = p.out_planes + (size_t)row * p.out_ld + col;
-                    store_split32(x, hi, hi + (size_t)p.out_plane_rows * p.out_ld);
+                    store_split32(x, hi, hi + plane);
                 } else if (EPI == EPI_OUT) {
-                    const float* w4 = p.w4 + (size_t)s * ncols + col;
+                    load32(p.w4 + (size_t)s * ncols + col, aux);
                     const float dsc = p.inv_models * D_SCALE;
 #pragma unroll
                     for (int i = 0; i < 32; ++i) {
-                        const float wv = w4[i];
-                        e_acc = fmaf(wv, x[i], e_acc);
-                        x[i] = wv * dcelu_from_h(x[i], p.alpha) * dsc;
+                        e_acc = fmaf(aux[i], x[i], e_acc);
+                        x[i] = aux[i] * dsc * dcelu_from_h(x[i], inv_alpha);
                     }
                     __half* hi = p.out_planes + (size_t)row * p.out_ld + col;
-                    store_split32(x, hi, hi + (size_t)p.out_plane_rows * p.out_ld);
+                    store_split32(x, hi, hi + plane);
                 } else if (EPI == EPI_DCELU) {
-                    float h[32];
-                    const __half* hh = p.h_planes + (size_t)row * p.out_ld + col;
-                    load_joined32(hh, hh + (size_t)p.out_plane_rows * p.out_ld, h);
 #pragma unroll
-                    for (int i = 0; i < 32; ++i) x[i] = __uint_as_float(v[i]) * p.acc_scale * dcelu_from_h(h[i], p.alpha);
+                    for (int i = 0; i < 32; ++i) x[i] = __uint_as_float(v[i]) * p.acc_scale * dcelu_from_h(aux[i], inv_alpha);
                     __half* hi = p.out_planes + (size_t)row * p.out_ld + col;
-                    store_split32(x, hi, hi + (size_t)p.out_plane_rows * p.out_ld);
+                    store_split32(x, hi, hi + plane);
                 } else {   // EPI_GRAD
                     float4* dst = reinterpret_cast<float4*>(p.out_f32 + (size_t)row * p.out_ld + col);
 #pragma unroll
@@ -342,7 +370,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                                              __uint_as_float(v[4 * i + 2]) * p.acc_scale, __uint_as_float(v[4 * i + 3]) * p.acc_scale);
                 }
             }
-            if (EPI == EPI_OUT) atomicAdd(&p.e_atom[row], (e_acc + p.b4[s * p.n_tiles + nt]) * p.inv_models);
+            if (EPI == EPI_OUT) atomicAdd(&p.e_atom[row], (e_acc + (half == 0 ? p.b4[s * p.n_tiles + nt] : 0.f)) * p.inv_models);
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(tempty_bar(acc));
