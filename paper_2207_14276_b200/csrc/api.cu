@@ -38,10 +38,10 @@ static bool dalloc(T** p, size_t count) {
 }
 
 static void free_all(Ctx* c) {
-    void* ptrs[] = {c->grid, c->status, c->bbox, c->cell_of, c->scell, c->cell_count, c->cell_start, c->cell_fill, c->perm,
+    void* ptrs[] = {c->grid, c->status, c->bbox, c->cell_of, c->perm_tmp, c->cell_count, c->cell_start, c->cell_fill, c->perm,
                     c->inv_perm, c->spos, c->smol, c->n_rad, c->n_ang, c->row_ptr, c->col, c->sp_count, c->sp_start,
                     c->rowmap, c->row_species, c->row_slot, c->blk_hist, c->aev, c->grad, c->e_atom, c->fsorted,
-                    c->e_out_tmp, c->export_tmp, c->st_pos, c->st_species, c->st_mol, c->st_E, c->st_F};
+                    c->e_out_tmp, c->export_tmp, c->tmp_col, c->blk_sum, c->blk_off, c->seg_cnt, c->st_pos, c->st_species, c->st_mol, c->st_E, c->st_F};
     for (void* p : ptrs) if (p) cudaFree(p);
     mlp_simt_free(c);
     mlp_tc_free(c);
@@ -144,19 +144,22 @@ int dhp_create(dhp_ctx** out, const dhp_params* params, int64_t max_atoms, int64
     c->max_atoms = max_atoms;
     c->max_mols = max_mols;
     c->max_rows = (max_atoms + NSP * (ROW_TILE - 1) + ROW_TILE - 1) / ROW_TILE * ROW_TILE + ROW_TILE;
-    c->max_cells = max_atoms * 2 > 4096 ? max_atoms * 2 : 4096;
+    c->max_cells = max_atoms * 2 > 256 ? max_atoms * 2 : 256;
     if (max_mols > c->max_cells) c->max_cells = max_mols;
     // neighbour storage: 160 directed pairs per atom on average (rho = 0.1 A^-3 gives 55 at 5.1 A); for tiny
     // systems every pair may be a neighbour
     c->pair_cap = max_atoms * 160;
     if (max_atoms < 161) c->pair_cap = max_atoms * (max_atoms - 1) + 1;
+    // per-atom capacity of the pass-1 temporary rows (rho = 0.1 A^-3 gives 55 neighbours at 5.1 A)
+    c->tmp_stride = (int)(max_atoms - 1 < 192 ? (max_atoms > 1 ? max_atoms - 1 : 1) : 192);
     const size_t N = (size_t)max_atoms, R = (size_t)c->max_rows, NC = (size_t)c->max_cells;
     const size_t NM = (size_t)(max_mols > 0 ? max_mols : 1);
     bool ok = true;
     ok &= dalloc(&c->grid, 1) && dalloc(&c->status, 1) && dalloc(&c->bbox, 8);
-    ok &= dalloc(&c->cell_of, N) && dalloc(&c->scell, N) && dalloc(&c->cell_count, NC + 1) && dalloc(&c->cell_start, NC + 1) && dalloc(&c->cell_fill, NC);
+    ok &= dalloc(&c->cell_of, N) && dalloc(&c->perm_tmp, N) && dalloc(&c->cell_count, NC + 1) && dalloc(&c->cell_start, NC + 1) && dalloc(&c->cell_fill, NC);
     ok &= dalloc(&c->perm, N) && dalloc(&c->inv_perm, N) && dalloc(&c->spos, N) && dalloc(&c->smol, N);
     ok &= dalloc(&c->n_rad, N) && dalloc(&c->n_ang, N) && dalloc(&c->row_ptr, N + 1) && dalloc(&c->col, (size_t)c->pair_cap);
+    ok &= dalloc(&c->tmp_col, N * c->tmp_stride) && dalloc(&c->blk_sum, N / 256 + 3) && dalloc(&c->blk_off, N / 256 + 3) && dalloc(&c->seg_cnt, N * 16);
     ok &= dalloc(&c->sp_count, 8) && dalloc(&c->sp_start, 8) && dalloc(&c->rowmap, N);
     ok &= dalloc(&c->row_species, R) && dalloc(&c->row_slot, R) && dalloc(&c->blk_hist, (N / 256 + 2) * 8);
     ok &= dalloc(&c->aev, R * AEV_LD) && dalloc(&c->grad, R * AEV_LD) && dalloc(&c->e_atom, R);

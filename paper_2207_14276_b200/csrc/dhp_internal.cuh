@@ -44,6 +44,10 @@ struct Grid {
     int ncell;
     int periodic;
     int by_molecule;    // 1: "cell" = molecule, stencil = self (batched replicas)
+    double edge[3];     // cell edge
+    double inv_L[3];    // 1 / L (0 if open)
+    int wrap[3];        // periodic axis with < 3 cells: per-pair minimum image also in the fp32 prefilter
+    float Lf[3], inv_Lf[3];
 };
 
 // AEV constants in the form the kernels use (fp32, exp2-scaled).
@@ -92,7 +96,7 @@ struct Ctx {
     int* status;
     unsigned* bbox;        // 6 ordered-uint min/max
     int* cell_of;          // [N] cell of caller's atom i
-    int* scell;            // [N] cell of sorted slot
+    int* perm_tmp;         // [N] cell-bucketed caller indices before the in-cell ordering
     int* cell_count;       // [max_cells+1]
     int* cell_start;       // [max_cells+1]
     int* cell_fill;        // [max_cells]
@@ -103,7 +107,12 @@ struct Ctx {
     int* n_rad;            // [N]
     int* n_ang;            // [N]
     int* row_ptr;          // [N+1]
-    int* col;              // [pair_cap] sorted-slot indices; angular neighbours first in each row
+    int* col;              // [pair_cap] sorted-slot indices; each row ordered by (angular, radial-only) x species
+    unsigned* tmp_col;     // [N][tmp_stride] unordered kept pairs of pass 1
+    int tmp_stride;
+    int* blk_sum;          // [N/256 + 2] pairs per 256-atom block
+    int* blk_off;          // [N/256 + 2] exclusive scan, then total, then overflow flag
+    unsigned short* seg_cnt; // [N][16] per row: angular count per species (0..6), n_ang (7), radial-only per species (8..14), (15)
     int* sp_count;         // [8]
     int* sp_start;         // [8] first row of each species group (multiple of ROW_TILE); [7] = end
     int* rowmap;           // [N] sorted slot -> row

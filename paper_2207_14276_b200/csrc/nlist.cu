@@ -1,10 +1,12 @@
 // a1 — neighbour search: periodic / open cell list -> CSR pair list (§2.2.2).
 //
-// Atoms are binned into cells of edge >= rc(1+2^-20), counting-sorted by cell (ties broken by the
-// caller's index, so the internal order is deterministic), and each atom's stencil of <= 27 cells is
-// scanned twice (count, then fill).  The keep/drop decision is ONLY the canonical fp64 predicate of
-// include/dhp.h: binning is conservative, never decisive.  Rows hold sorted-slot
-// indices with the angular neighbours (R <= rca) as a prefix.  Rows of the AEV / MLP buffers are
+// Atoms are binned into cells of edge >= rc(1+2^-20) and counting-sorted by cell (ties broken by the
+// caller's index, so the internal order is deterministic).  One block per cell stages its <= 27 stencil
+// cells in shared memory as centre-relative fp32 coordinates and tests every (centre, candidate) pair
+// in fp32; pairs within the fp32 error margin of a cutoff are decided by the canonical fp64 predicate of
+// include/dhp.h, so the list is bit-exact.  Kept pairs go to a fixed-stride
+// temporary row; a second pass assigns CSR offsets and orders each row by (angular first, then
+// radial-only) x neighbour species.  Rows hold sorted-slot indices.  Rows of the AEV / MLP buffers are
 // grouped by the central atom's species (stable in sorted order), each group starting at a multiple
 // of ROW_TILE rows so that one MLP tile never mixes networks.
 #include <algorithm>
@@ -93,7 +95,10 @@ __global__ void k_setup_grid(Grid* g, int periodic, double Lx, double Ly, double
     g->periodic = periodic;
     g->by_molecule = by_molecule;
     if (by_molecule) {
-        for (int c = 0; c < 3; ++c) { g->L[c] = 0; g->origin[c] = 0; g->inv_cell[c] = 0; g->nc[c] = 1; }
+        for (int c = 0; c < 3; ++c) {
+            g->L[c] = 0; g->origin[c] = 0; g->inv_cell[c] = 0; g->nc[c] = 1;
+            g->edge[c] = 0; g->inv_L[c] = 0; g->wrap[c] = 0; g->Lf[c] = 0.f; g->inv_Lf[c] = 0.f;
+        }
         g->nc[0] = n_mol;
         g->ncell = n_mol;
         return;
@@ -120,7 +125,14 @@ __global__ void k_setup_grid(Grid* g, int periodic, double Lx, double Ly, double
         if (g->nc[2] > g->nc[big]) big = 2;
         g->nc[big] = max(1, g->nc[big] / 2);
     }
-    for (int c = 0; c < 3; ++c) g->inv_cell[c] = (double)g->nc[c] / ext[c];
+    for (int c = 0; c < 3; ++c) {
+        g->inv_cell[c] = (double)g->nc[c] / ext[c];
+        g->edge[c] = ext[c] / (double)g->nc[c];
+        g->inv_L[c] = periodic ? 1.0 / L[c] : 0.0;
+        g->wrap[c] = (periodic && g->nc[c] < 3) ? 1 : 0;
+        g->Lf[c] = (float)L[c];
+        g->inv_Lf[c] = periodic ? (float)(1.0 / L[c]) : 0.f;
+    }
     g->ncell = g->nc[0] * g->nc[1] * g->nc[2];
 }
 
@@ -174,27 +186,25 @@ __global__ void k_scatter(const int* __restrict__ cell_of, int n, const int* __r
     perm[cell_start[c] + atomicAdd(&cell_fill[c], 1)] = i;
 }
 
-// one thread per cell: order its atoms by caller index (deterministic internal order), then gather
+// one warp per cell: order its atoms by caller index (deterministic internal order), then gather
 __global__ void k_sort_gather(const float* __restrict__ pos, const int* __restrict__ species,
-                              const Grid* __restrict__ g, const int* __restrict__ cell_start, int* __restrict__ perm,
-                              int* __restrict__ inv_perm, float4* __restrict__ spos, int* __restrict__ smol,
-                              int* __restrict__ scell) {
-    int c = blockIdx.x * blockDim.x + threadIdx.x;
+                              const Grid* __restrict__ g, const int* __restrict__ cell_start, const int* __restrict__ perm_in,
+                              int* __restrict__ perm, int* __restrict__ inv_perm, float4* __restrict__ spos,
+                              int* __restrict__ smol) {
+    const int c = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (c >= g->ncell) return;
-    int b = cell_start[c], e = cell_start[c + 1];
-    for (int a = b + 1; a < e; ++a) {
-        int v = perm[a], q = a - 1;
-        while (q >= b && perm[q] > v) { perm[q + 1] = perm[q]; --q; }
-        perm[q + 1] = v;
-    }
-    for (int a = b; a < e; ++a) {
-        int i = perm[a];
-        inv_perm[i] = a;
-        int s = species[i];
+    const int b = cell_start[c], e = cell_start[c + 1];
+    for (int a = b + lane; a < e; a += 32) {
+        const int v = perm_in[a];
+        int rank = 0;
+        for (int q = b; q < e; ++q) rank += perm_in[q] < v;     // caller indices are distinct
+        const int dst = b + rank;
+        perm[dst] = v;
+        inv_perm[v] = dst;
+        int s = species[v];
         s = min(max(s, 0), NSP - 1);
-        spos[a] = make_float4(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], __int_as_float(s));
-        smol[a] = g->by_molecule ? c : 0;
-        scell[a] = c;
+        spos[dst] = make_float4(pos[3 * v], pos[3 * v + 1], pos[3 * v + 2], __int_as_float(s));
+        smol[dst] = g->by_molecule ? c : 0;
     }
 }
 
@@ -217,21 +227,28 @@ __global__ void k_species_hist(const float4* __restrict__ spos, int n, int* __re
     if (threadIdx.x < NSP) blk_hist[blockIdx.x * 8 + threadIdx.x] = h[threadIdx.x];
 }
 
-// single block: per species exclusive scan over blocks; group starts aligned to ROW_TILE
+// single block, one warp per species: exclusive scan over blocks; group starts aligned to ROW_TILE
 __global__ void k_species_scan(int* __restrict__ blk_hist, int nblk, int* __restrict__ sp_count, int* __restrict__ sp_start) {
     __shared__ int tot[NSP + 1];
-    int t = threadIdx.x;
-    if (t < NSP) {
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (w < NSP) {
         int run = 0;
-        for (int b = 0; b < nblk; ++b) {
-            int v = blk_hist[b * 8 + t];
-            blk_hist[b * 8 + t] = run;
-            run += v;
+        for (int base = 0; base < nblk; base += 32) {
+            const int b = base + lane;
+            const int v = b < nblk ? blk_hist[b * 8 + w] : 0;
+            int x = v;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                int y = __shfl_up_sync(0xffffffffu, x, o);
+                if (lane >= o) x += y;
+            }
+            if (b < nblk) blk_hist[b * 8 + w] = run + x - v;
+            run += __shfl_sync(0xffffffffu, x, 31);
         }
-        tot[t] = run;
+        if (lane == 0) tot[w] = run;
     }
     __syncthreads();
-    if (t == 0) {
+    if (threadIdx.x == 0) {
         int start = 0;
         for (int s = 0; s < NSP; ++s) {
             sp_count[s] = tot[s];
@@ -267,7 +284,11 @@ __global__ void k_species_rank(const float4* __restrict__ spos, int n, const int
 }
 
 // ---------------------------------------------------------------------------------------------
-// stencil traversal (count + fill share it)
+// pass 1: one block per cell; the <= 27 stencil cells are staged in shared memory as fp32 coordinates
+// relative to the centre cell (minimum image applied in fp64 at staging), so the inner loop is plain
+// fp32.  A pair whose fp32 R^2 lies within a proven margin of rcr^2 or rca^2 is decided by the
+// canonical fp64 predicate on the ORIGINAL coordinates; every other pair is decided by fp32 alone
+// (its fp32 error is smaller than its distance to the threshold), so the list is still bit-exact.
 // ---------------------------------------------------------------------------------------------
 struct Stencil {
     int n[3];
@@ -309,77 +330,227 @@ __device__ __forceinline__ double pair_r2(const float4& pi, const float4& pj, co
     return __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
 }
 
-template <bool FILL>
-__global__ void __launch_bounds__(256) k_neighbours(const float4* __restrict__ spos, const int* __restrict__ scell, int n,
-                                                   const Grid* __restrict__ gp, const int* __restrict__ cell_start,
-                                                   double rcr2, double rca2, int* __restrict__ n_rad,
-                                                   int* __restrict__ n_ang, const int* __restrict__ row_ptr,
-                                                   int* __restrict__ col) {
+constexpr int P1_THREADS = 128;
+constexpr int CAND_TILE = 1024;        // candidates staged per tile (16 KB)
+constexpr unsigned ENT_RADIAL_ONLY = 0x80000000u;   // temp-row entry: bit 31 = beyond rca, bits 28..30 = species, low 28 = slot
+
+__global__ void __launch_bounds__(P1_THREADS)
+k_pairs(const float4* __restrict__ spos, const Grid* __restrict__ gp, const int* __restrict__ cell_start, double rcr2,
+        double rca2, int stride, int* __restrict__ cnt, unsigned* __restrict__ tmp, int* __restrict__ blk_sum,
+        int* __restrict__ status) {
     __shared__ Grid g;
+    __shared__ float4 cand[CAND_TILE];
+    __shared__ int seg_cell_b[28], seg_off[28], nseg_s;
+    __shared__ float bmax_s[P1_THREADS / 32];
     if (threadIdx.x == 0) g = *gp;
     __syncthreads();
-    const int lane = threadIdx.x & 31;
-    const int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    if (i >= n) return;
-    const float4 pi = spos[i];
-    Stencil st;
-    make_stencil(g, scell[i], st);
-    int cnt_r = 0, cnt_a = 0;
-    int base_a = 0, base_r = 0;
-    if (FILL) {
-        base_a = row_ptr[i];
-        base_r = base_a + n_ang[i];
-        if (row_ptr[i + 1] - base_a != n_rad[i]) return;   // overflowed list was emptied by the scan
+    const int cell = blockIdx.x;
+    if (cell >= g.ncell) return;
+    const int cb = cell_start[cell], ce = cell_start[cell + 1];
+    if (ce == cb) return;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+
+    // candidate segments: one per stencil cell
+    if (threadIdx.x == 0) {
+        Stencil st;
+        make_stencil(g, cell, st);
+        int ns = 0, off = 0;
+        for (int iz = 0; iz < st.n[2]; ++iz)
+            for (int iy = 0; iy < st.n[1]; ++iy)
+                for (int ix = 0; ix < st.n[0]; ++ix) {
+                    int c = g.by_molecule ? st.c[0][0] : st.c[0][ix] + g.nc[0] * (st.c[1][iy] + g.nc[1] * st.c[2][iz]);
+                    int b = cell_start[c], e = cell_start[c + 1];
+                    if (e > b) { seg_cell_b[ns] = b; seg_off[ns] = off; off += e - b; ++ns; }
+                }
+        seg_cell_b[ns] = 0; seg_off[ns] = off;     // sentinel: total
+        nseg_s = ns;
     }
+    __syncthreads();
+    const int nseg = nseg_s;
+    const int ncand = seg_off[nseg];
+
+    // centre of the block's cell (reference point of the relative coordinates)
+    double ctr[3];
+    if (g.by_molecule) {
+        const float4 p0 = spos[cb];
+        ctr[0] = p0.x; ctr[1] = p0.y; ctr[2] = p0.z;
+    } else {
+        int cc[3] = {cell % g.nc[0], (cell / g.nc[0]) % g.nc[1], cell / (g.nc[0] * g.nc[1])};
+#pragma unroll
+        for (int d = 0; d < 3; ++d) ctr[d] = g.origin[d] + ((double)cc[d] + 0.5) * g.edge[d];
+    }
+    const bool wrapx = g.wrap[0], wrapy = g.wrap[1], wrapz = g.wrap[2];
+    const float Lx = g.Lf[0], Ly = g.Lf[1], Lz = g.Lf[2];
+    const float iLx = g.inv_Lf[0], iLy = g.inv_Lf[1], iLz = g.inv_Lf[2];
+    const float rcr2f = (float)rcr2, rca2f = (float)rca2;
+    const float rcr = sqrtf(rcr2f), rca = sqrtf(rca2f);
     const unsigned lt = (1u << lane) - 1u;
-    for (int iz = 0; iz < st.n[2]; ++iz)
-        for (int iy = 0; iy < st.n[1]; ++iy)
-            for (int ix = 0; ix < st.n[0]; ++ix) {
-                int c = g.by_molecule ? st.c[0][0] : st.c[0][ix] + g.nc[0] * (st.c[1][iy] + g.nc[1] * st.c[2][iz]);
-                int b = cell_start[c], e = cell_start[c + 1];
-                for (int j0 = b; j0 < e; j0 += 32) {
-                    int j = j0 + lane;
-                    bool in_r = false, in_a = false;
-                    if (j < e && j != i) {
-                        double r2 = pair_r2(pi, spos[j], g);
-                        in_r = r2 <= rcr2;
-                        in_a = r2 <= rca2;
-                    }
-                    if (FILL) {
-                        unsigned ma = __ballot_sync(0xffffffffu, in_a);
-                        unsigned mr = __ballot_sync(0xffffffffu, in_r && !in_a);
-                        if (in_a) col[base_a + __popc(ma & lt)] = j;
-                        else if (in_r) col[base_r + __popc(mr & lt)] = j;
-                        base_a += __popc(ma);
-                        base_r += __popc(mr);
-                    } else {
-                        cnt_r += in_r;
-                        cnt_a += in_a;
+
+    for (int t0 = 0; t0 < ncand; t0 += CAND_TILE) {
+        const int tn = min(CAND_TILE, ncand - t0);
+        // ---- stage the tile -------------------------------------------------------------------
+        float bmax = 0.f;
+        for (int t = threadIdx.x; t < tn; t += P1_THREADS) {
+            const int f = t0 + t;
+            int sg = 0;
+            while (sg + 1 < nseg && seg_off[sg + 1] <= f) ++sg;
+            const int j = seg_cell_b[sg] + (f - seg_off[sg]);
+            const float4 pj = spos[j];
+            double r[3] = {(double)pj.x - ctr[0], (double)pj.y - ctr[1], (double)pj.z - ctr[2]};
+            if (g.periodic) {
+#pragma unroll
+                for (int d = 0; d < 3; ++d) r[d] -= g.L[d] * rint(r[d] * g.inv_L[d]);
+            }
+            const float x = (float)r[0], y = (float)r[1], z = (float)r[2];
+            bmax = fmaxf(bmax, fmaxf(fabsf(x), fmaxf(fabsf(y), fabsf(z))));
+            cand[t] = make_float4(x, y, z, __int_as_float(j | (__float_as_int(pj.w) << 28)));
+        }
+        for (int o = 16; o; o >>= 1) bmax = fmaxf(bmax, __shfl_xor_sync(0xffffffffu, bmax, o));
+        if (lane == 0) bmax_s[warp] = bmax;
+        __syncthreads();
+        float B = 0.f;
+#pragma unroll
+        for (int q = 0; q < P1_THREADS / 32; ++q) B = fmaxf(B, bmax_s[q]);
+        // fp32 error bound of R^2 near a cutoff rc: |err| <= rc B 2^-19 + rc^2 2^-22; doubled
+        const float mr = rcr * B * 3.8146973e-06f + rcr2f * 4.7683716e-07f;
+        const float ma = rca * B * 3.8146973e-06f + rca2f * 4.7683716e-07f;
+
+        // ---- centre atoms of this cell, one warp each ----------------------------------------
+        for (int i = cb + warp; i < ce; i += P1_THREADS / 32) {
+            // the centre's own relative coordinates: same arithmetic as the staged copy
+            const float4 pio = spos[i];
+            double ri[3] = {(double)pio.x - ctr[0], (double)pio.y - ctr[1], (double)pio.z - ctr[2]};
+            if (g.periodic) {
+#pragma unroll
+                for (int d = 0; d < 3; ++d) ri[d] -= g.L[d] * rint(ri[d] * g.inv_L[d]);
+            }
+            const float pix = (float)ri[0], piy = (float)ri[1], piz = (float)ri[2];
+            int base = t0 ? cnt[i] : 0;
+            for (int c0 = 0; c0 < tn; c0 += 32) {
+                const int t = c0 + lane;
+                bool in_r = false, in_a = false, amb = false;
+                int jj = 0;
+                if (t < tn) {
+                    const float4 c = cand[t];
+                    jj = __float_as_int(c.w);
+                    float dx = c.x - pix, dy = c.y - piy, dz = c.z - piz;
+                    if (wrapx) dx -= Lx * rintf(dx * iLx);
+                    if (wrapy) dy -= Ly * rintf(dy * iLy);
+                    if (wrapz) dz -= Lz * rintf(dz * iLz);
+                    const float r2 = dx * dx + dy * dy + dz * dz;
+                    const bool other = (jj & 0x0fffffff) != i;
+                    in_r = other && r2 <= rcr2f;
+                    in_a = other && r2 <= rca2f;
+                    amb = other && (fabsf(r2 - rcr2f) <= mr || fabsf(r2 - rca2f) <= ma);
+                }
+                if (__any_sync(0xffffffffu, amb)) {
+                    if (amb) {
+                        const double r2d = pair_r2(pio, spos[jj & 0x0fffffff], g);
+                        in_r = r2d <= rcr2;
+                        in_a = r2d <= rca2;
                     }
                 }
+                const unsigned m = __ballot_sync(0xffffffffu, in_r);
+                if (in_r) {
+                    const int pos = base + __popc(m & lt);
+                    if (pos < stride) tmp[(size_t)i * stride + pos] = (unsigned)jj | (in_a ? 0u : ENT_RADIAL_ONLY);
+                }
+                base += __popc(m);
             }
-    if (!FILL) {
-        for (int o = 16; o; o >>= 1) {
-            cnt_r += __shfl_xor_sync(0xffffffffu, cnt_r, o);
-            cnt_a += __shfl_xor_sync(0xffffffffu, cnt_a, o);
+            if (lane == 0) {
+                if (base > stride) { atomicExch(status, DHP_E_CAPACITY); base = stride; }
+                cnt[i] = base;
+                if (t0 + CAND_TILE >= ncand) atomicAdd(&blk_sum[i >> 8], base);
+            }
         }
-        if (lane == 0) { n_rad[i] = cnt_r; n_ang[i] = cnt_a; }
+        __syncthreads();
     }
 }
 
-__global__ void k_scan_rows(const int* __restrict__ n_rad, int* __restrict__ row_ptr, int n, int64_t pair_cap,
-                            int* __restrict__ status) {
-    __shared__ int overflow;
-    block_scan_excl(n_rad, row_ptr, n);
+// exclusive scan of the per-256-atom block sums; total > pair_cap empties the list (status CAPACITY)
+__global__ void k_scan_blocks(const int* __restrict__ blk_sum, int* __restrict__ blk_off, int nblk, int64_t pair_cap,
+                              int* __restrict__ status) {
+    block_scan_excl(blk_sum, blk_off, nblk);
     __syncthreads();
     if (threadIdx.x == 0) {
-        // int32 wrap-around shows up as a negative or non-monotone total; both count as overflow
-        overflow = (row_ptr[n] < 0 || (int64_t)row_ptr[n] > pair_cap) ? 1 : 0;
-        if (overflow) atomicExch(status, DHP_E_CAPACITY);
+        const int ovf = (blk_off[nblk] < 0 || (int64_t)blk_off[nblk] > pair_cap) ? 1 : 0;
+        if (ovf) atomicExch(status, DHP_E_CAPACITY);
+        blk_off[nblk + 1] = ovf;
     }
+}
+
+// pass 2: 256 atoms per block; rows get their CSR offsets, entries are ordered by (angular first, then
+// radial-only) x neighbour species, and the 14 segment sizes of every row are stored for the AEV kernels.
+__global__ void __launch_bounds__(256)
+k_rows(const unsigned* __restrict__ tmp, int stride, const int* __restrict__ cnt, const int* __restrict__ blk_off, int nblk,
+       int n, int* __restrict__ row_ptr, int* __restrict__ col, int* __restrict__ n_rad, int* __restrict__ n_ang,
+       unsigned short* __restrict__ seg_cnt) {
+    __shared__ int wsum[8];
+    __shared__ int rstart[256];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int i0 = blockIdx.x * 256;
+    const bool ovf = blk_off[nblk + 1] != 0;
+    const int a = i0 + tid;
+    const int c = (a < n && !ovf) ? cnt[a] : 0;
+    int x = c;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int y = __shfl_up_sync(0xffffffffu, x, o);
+        if (lane >= o) x += y;
+    }
+    if (lane == 31) wsum[warp] = x;
     __syncthreads();
-    if (overflow)
-        for (int i = threadIdx.x; i <= n; i += blockDim.x) row_ptr[i] = 0;
+    int before = ovf ? 0 : blk_off[blockIdx.x];
+    for (int q = 0; q < warp; ++q) before += wsum[q];
+    const int start = before + x - c;
+    rstart[tid] = start;
+    if (a < n) { row_ptr[a] = start; n_rad[a] = c; }
+    if (a == n - 1) row_ptr[n] = start + c;
+    __syncthreads();
+
+    const unsigned lt = (1u << lane) - 1u;
+    for (int q = 0; q < 32; ++q) {
+        const int i = i0 + warp * 32 + q;
+        if (i >= n) break;
+        const int ni = ovf ? 0 : cnt[i];
+        const unsigned* src = tmp + (size_t)i * stride;
+        int segc[14];
+#pragma unroll
+        for (int k = 0; k < 14; ++k) segc[k] = 0;
+        for (int t0 = 0; t0 < ni; t0 += 32) {
+            const int t = t0 + lane;
+            int key = -1;
+            if (t < ni) { const unsigned e = src[t]; key = (int)((e >> 28) & 7u) + ((e & ENT_RADIAL_ONLY) ? 7 : 0); }
+#pragma unroll
+            for (int k = 0; k < 14; ++k) segc[k] += __popc(__ballot_sync(0xffffffffu, key == k));
+        }
+        int segs[14];
+        int run = rstart[warp * 32 + q];
+        int na = 0;
+#pragma unroll
+        for (int k = 0; k < 14; ++k) { segs[k] = run; run += segc[k]; if (k < 7) na += segc[k]; }
+        for (int t0 = 0; t0 < ni; t0 += 32) {
+            const int t = t0 + lane;
+            int key = -1;
+            unsigned e = 0;
+            if (t < ni) { e = src[t]; key = (int)((e >> 28) & 7u) + ((e & ENT_RADIAL_ONLY) ? 7 : 0); }
+#pragma unroll
+            for (int k = 0; k < 14; ++k) {
+                const unsigned m = __ballot_sync(0xffffffffu, key == k);
+                if (key == k) col[segs[k] + __popc(m & lt)] = (int)(e & 0x0fffffffu);
+                segs[k] += __popc(m);
+            }
+        }
+        if (lane == 0) n_ang[i] = na;
+        if (lane < 16) {
+            int v = 0;
+#pragma unroll
+            for (int k = 0; k < 14; ++k) if (lane == (k < 7 ? k : k + 1)) v = segc[k];
+            if (lane == 7) v = na;
+            if (lane == 15) v = ni - na;
+            seg_cnt[(size_t)i * 16 + lane] = (unsigned short)v;
+        }
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -395,6 +566,7 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
     ctx->n_mol = by_mol ? n_mol : 0;
     ctx->periodic = periodic;
     cudaStream_t st = ctx->stream;
+    const int nblk = (n + 255) / 256;
 
     DHP_CUDA(ctx, cudaMemsetAsync(ctx->status, 0, sizeof(int), st));
     DHP_CUDA(ctx, cudaMemsetAsync(ctx->cell_count, 0, sizeof(int) * (ctx->max_cells + 1), st));
@@ -407,6 +579,7 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
         DHP_CUDA(ctx, cudaMemsetAsync(ctx->sp_start, 0, sizeof(int) * 8, st));
         return DHP_OK;
     }
+    DHP_CUDA(ctx, cudaMemsetAsync(ctx->blk_sum, 0, sizeof(int) * (nblk + 2), st));
     double L[3] = {0, 0, 0};
     if (periodic) for (int c = 0; c < 3; ++c) L[c] = (double)box_host[c];
     if (!periodic && !by_mol) {
@@ -421,30 +594,29 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
     DHP_LAUNCH(ctx, k_assign_cells, nb, 256, 0, pos, species, n, mol_offsets, n_mol, ctx->grid, ctx->cell_of,
                ctx->cell_count, ctx->status);
     DHP_LAUNCH(ctx, k_scan_cells, 1, 1024, 0, ctx->cell_count, ctx->cell_start, ctx->grid);
-    DHP_LAUNCH(ctx, k_scatter, nb, 256, 0, ctx->cell_of, n, ctx->cell_start, ctx->cell_fill, ctx->perm);
-    // the cell count lives on the device; launch for the bound and let surplus threads exit
+    DHP_LAUNCH(ctx, k_scatter, nb, 256, 0, ctx->cell_of, n, ctx->cell_start, ctx->cell_fill, ctx->perm_tmp);
+    // the cell count lives on the device; launch for the bound and let surplus blocks exit
     int64_t cell_bound = by_mol ? n_mol : ctx->max_cells;
     if (periodic) {
         int64_t t = 1;
         for (int c = 0; c < 3; ++c) t *= (int64_t)fmax(1.0, floor(L[c] / rcr));
         cell_bound = t < cell_bound ? t : cell_bound;
     }
-    DHP_LAUNCH(ctx, k_sort_gather, (int)((cell_bound + 127) / 128), 128, 0, pos, species, ctx->grid, ctx->cell_start,
-               ctx->perm, ctx->inv_perm, ctx->spos, ctx->smol, ctx->scell);
+    DHP_LAUNCH(ctx, k_sort_gather, (int)((cell_bound + 3) / 4), 128, 0, pos, species, ctx->grid, ctx->cell_start,
+               ctx->perm_tmp, ctx->perm, ctx->inv_perm, ctx->spos, ctx->smol);
     // rows grouped by species
     const int nrb = (n + RB - 1) / RB;
     DHP_LAUNCH(ctx, k_species_hist, nrb, RB, 0, ctx->spos, n, ctx->blk_hist);
-    DHP_LAUNCH(ctx, k_species_scan, 1, 32, 0, ctx->blk_hist, nrb, ctx->sp_count, ctx->sp_start);
+    DHP_LAUNCH(ctx, k_species_scan, 1, 32 * NSP, 0, ctx->blk_hist, nrb, ctx->sp_count, ctx->sp_start);
     DHP_LAUNCH(ctx, k_species_rank, nrb, RB, 0, ctx->spos, n, ctx->blk_hist, ctx->sp_start, ctx->rowmap,
                ctx->row_species, ctx->row_slot);
-    // CSR
-    const int nwb = (n + 7) / 8;   // 8 warps per block, one warp per atom
+    // pair list
     const double rcr2 = rcr * rcr, rca2 = rca * rca;
-    DHP_LAUNCH(ctx, k_neighbours<false>, nwb, 256, 0, ctx->spos, ctx->scell, n, ctx->grid, ctx->cell_start, rcr2,
-               rca2, ctx->n_rad, ctx->n_ang, ctx->row_ptr, ctx->col);
-    DHP_LAUNCH(ctx, k_scan_rows, 1, 1024, 0, ctx->n_rad, ctx->row_ptr, n, ctx->pair_cap, ctx->status);
-    DHP_LAUNCH(ctx, k_neighbours<true>, nwb, 256, 0, ctx->spos, ctx->scell, n, ctx->grid, ctx->cell_start, rcr2,
-               rca2, ctx->n_rad, ctx->n_ang, ctx->row_ptr, ctx->col);
+    DHP_LAUNCH(ctx, k_pairs, (int)cell_bound, P1_THREADS, 0, ctx->spos, ctx->grid, ctx->cell_start, rcr2, rca2,
+               ctx->tmp_stride, ctx->n_rad, ctx->tmp_col, ctx->blk_sum, ctx->status);
+    DHP_LAUNCH(ctx, k_scan_blocks, 1, 1024, 0, ctx->blk_sum, ctx->blk_off, nblk, ctx->pair_cap, ctx->status);
+    DHP_LAUNCH(ctx, k_rows, nblk, 256, 0, ctx->tmp_col, ctx->tmp_stride, ctx->n_rad, ctx->blk_off, nblk, n, ctx->row_ptr,
+               ctx->col, ctx->n_rad, ctx->n_ang, ctx->seg_cnt);
     DHP_CUDA(ctx, cudaGetLastError());
     return DHP_OK;
 }
