@@ -159,7 +159,7 @@ int dhp_create(dhp_ctx** out, const dhp_params* params, int64_t max_atoms, int64
     ok &= dalloc(&c->cell_of, N) && dalloc(&c->perm_tmp, N) && dalloc(&c->cell_count, NC + 1) && dalloc(&c->cell_start, NC + 1) && dalloc(&c->cell_fill, NC);
     ok &= dalloc(&c->perm, N) && dalloc(&c->inv_perm, N) && dalloc(&c->spos, N) && dalloc(&c->smol, N);
     ok &= dalloc(&c->n_rad, N) && dalloc(&c->n_ang, N) && dalloc(&c->row_ptr, N + 1) && dalloc(&c->col, (size_t)c->pair_cap);
-    ok &= dalloc(&c->tmp_col, N * c->tmp_stride) && dalloc(&c->blk_sum, N / 256 + 3) && dalloc(&c->blk_off, N / 256 + 3) && dalloc(&c->seg_cnt, N * 16);
+    ok &= dalloc(&c->tmp_col, N * c->tmp_stride) && dalloc(&c->blk_sum, N / 64 + 3) && dalloc(&c->blk_off, N / 64 + 3) && dalloc(&c->seg_cnt, N * 16);
     ok &= dalloc(&c->sp_count, 8) && dalloc(&c->sp_start, 8) && dalloc(&c->rowmap, N);
     ok &= dalloc(&c->row_species, R) && dalloc(&c->row_slot, R) && dalloc(&c->blk_hist, (N / 256 + 2) * 8);
     ok &= dalloc(&c->aev, R * AEV_LD) && dalloc(&c->grad, R * AEV_LD) && dalloc(&c->e_atom, R);

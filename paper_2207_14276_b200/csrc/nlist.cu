@@ -331,15 +331,17 @@ __device__ __forceinline__ double pair_r2(const float4& pi, const float4& pj, co
 }
 
 constexpr int P1_THREADS = 128;
+constexpr int ROWS_PER_BLK = 64;        // granularity of the block-sum scan that yields the CSR offsets
 constexpr int CAND_TILE = 1024;        // candidates staged per tile (16 KB)
 constexpr unsigned ENT_RADIAL_ONLY = 0x80000000u;   // temp-row entry: bit 31 = beyond rca, bits 28..30 = species, low 28 = slot
 
-__global__ void __launch_bounds__(P1_THREADS)
+template <bool WRAP>
+__global__ void __launch_bounds__(P1_THREADS, 8)
 k_pairs(const float4* __restrict__ spos, const Grid* __restrict__ gp, const int* __restrict__ cell_start, double rcr2,
         double rca2, int stride, int* __restrict__ cnt, unsigned* __restrict__ tmp, int* __restrict__ blk_sum,
         int* __restrict__ status) {
     __shared__ Grid g;
-    __shared__ float4 cand[CAND_TILE];
+    __shared__ float4 cand[CAND_TILE + 32];
     __shared__ int seg_cell_b[28], seg_off[28], nseg_s;
     __shared__ float bmax_s[P1_THREADS / 32];
     if (threadIdx.x == 0) g = *gp;
@@ -350,20 +352,28 @@ k_pairs(const float4* __restrict__ spos, const Grid* __restrict__ gp, const int*
     if (ce == cb) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 
-    // candidate segments: one per stencil cell
-    if (threadIdx.x == 0) {
+    // candidate segments: one per non-empty stencil cell (warp 0: lane <-> stencil cell, ballot-compacted)
+    if (warp == 0) {
         Stencil st;
         make_stencil(g, cell, st);
-        int ns = 0, off = 0;
-        for (int iz = 0; iz < st.n[2]; ++iz)
-            for (int iy = 0; iy < st.n[1]; ++iy)
-                for (int ix = 0; ix < st.n[0]; ++ix) {
-                    int c = g.by_molecule ? st.c[0][0] : st.c[0][ix] + g.nc[0] * (st.c[1][iy] + g.nc[1] * st.c[2][iz]);
-                    int b = cell_start[c], e = cell_start[c + 1];
-                    if (e > b) { seg_cell_b[ns] = b; seg_off[ns] = off; off += e - b; ++ns; }
-                }
-        seg_cell_b[ns] = 0; seg_off[ns] = off;     // sentinel: total
-        nseg_s = ns;
+        const int nst = st.n[0] * st.n[1] * st.n[2];
+        int b = 0, cntc = 0;
+        if (lane < nst) {
+            const int ix = lane % st.n[0], iy = (lane / st.n[0]) % st.n[1], iz = lane / (st.n[0] * st.n[1]);
+            const int c = g.by_molecule ? st.c[0][0] : st.c[0][ix] + g.nc[0] * (st.c[1][iy] + g.nc[1] * st.c[2][iz]);
+            b = cell_start[c];
+            cntc = cell_start[c + 1] - b;
+        }
+        int x = cntc;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, cntc > 0);
+        const int slot = __popc(m & ((1u << lane) - 1u));
+        if (cntc > 0) { seg_cell_b[slot] = b; seg_off[slot] = x - cntc; }
+        if (lane == 31) { const int ns = __popc(m); seg_cell_b[ns] = 0; seg_off[ns] = x; nseg_s = ns; }
     }
     __syncthreads();
     const int nseg = nseg_s;
@@ -405,6 +415,7 @@ k_pairs(const float4* __restrict__ spos, const Grid* __restrict__ gp, const int*
             bmax = fmaxf(bmax, fmaxf(fabsf(x), fmaxf(fabsf(y), fabsf(z))));
             cand[t] = make_float4(x, y, z, __int_as_float(j | (__float_as_int(pj.w) << 28)));
         }
+        if (threadIdx.x < 32) cand[tn + threadIdx.x] = make_float4(1.0e15f, 1.0e15f, 1.0e15f, __int_as_float(0x0fffffff));
         for (int o = 16; o; o >>= 1) bmax = fmaxf(bmax, __shfl_xor_sync(0xffffffffu, bmax, o));
         if (lane == 0) bmax_s[warp] = bmax;
         __syncthreads();
@@ -427,22 +438,19 @@ k_pairs(const float4* __restrict__ spos, const Grid* __restrict__ gp, const int*
             const float pix = (float)ri[0], piy = (float)ri[1], piz = (float)ri[2];
             int base = t0 ? cnt[i] : 0;
             for (int c0 = 0; c0 < tn; c0 += 32) {
-                const int t = c0 + lane;
-                bool in_r = false, in_a = false, amb = false;
-                int jj = 0;
-                if (t < tn) {
-                    const float4 c = cand[t];
-                    jj = __float_as_int(c.w);
-                    float dx = c.x - pix, dy = c.y - piy, dz = c.z - piz;
+                const float4 c = cand[c0 + lane];          // the tile is padded with far-away dummies
+                const int jj = __float_as_int(c.w);
+                float dx = c.x - pix, dy = c.y - piy, dz = c.z - piz;
+                if (WRAP) {
                     if (wrapx) dx -= Lx * rintf(dx * iLx);
                     if (wrapy) dy -= Ly * rintf(dy * iLy);
                     if (wrapz) dz -= Lz * rintf(dz * iLz);
-                    const float r2 = dx * dx + dy * dy + dz * dz;
-                    const bool other = (jj & 0x0fffffff) != i;
-                    in_r = other && r2 <= rcr2f;
-                    in_a = other && r2 <= rca2f;
-                    amb = other && (fabsf(r2 - rcr2f) <= mr || fabsf(r2 - rca2f) <= ma);
                 }
+                const float r2 = dx * dx + dy * dy + dz * dz;
+                const bool other = (jj & 0x0fffffff) != i && (!WRAP || c0 + lane < tn);
+                bool in_r = other && r2 <= rcr2f;
+                bool in_a = other && r2 <= rca2f;
+                const bool amb = other && (fabsf(r2 - rcr2f) <= mr || fabsf(r2 - rca2f) <= ma);
                 if (__any_sync(0xffffffffu, amb)) {
                     if (amb) {
                         const double r2d = pair_r2(pio, spos[jj & 0x0fffffff], g);
@@ -460,7 +468,7 @@ k_pairs(const float4* __restrict__ spos, const Grid* __restrict__ gp, const int*
             if (lane == 0) {
                 if (base > stride) { atomicExch(status, DHP_E_CAPACITY); base = stride; }
                 cnt[i] = base;
-                if (t0 + CAND_TILE >= ncand) atomicAdd(&blk_sum[i >> 8], base);
+                if (t0 + CAND_TILE >= ncand) atomicAdd(&blk_sum[i / ROWS_PER_BLK], base);
             }
         }
         __syncthreads();
@@ -479,76 +487,99 @@ __global__ void k_scan_blocks(const int* __restrict__ blk_sum, int* __restrict__
     }
 }
 
-// pass 2: 256 atoms per block; rows get their CSR offsets, entries are ordered by (angular first, then
+// pass 2: ROWS_PER_BLK atoms per block; rows get their CSR offsets, entries are ordered by (angular first, then
 // radial-only) x neighbour species, and the 14 segment sizes of every row are stored for the AEV kernels.
-__global__ void __launch_bounds__(256)
+constexpr int P2_THREADS = 256;
+constexpr int MAX_STRIDE_CHUNKS = 6;    // tmp_stride <= 192
+
+__global__ void __launch_bounds__(P2_THREADS)
 k_rows(const unsigned* __restrict__ tmp, int stride, const int* __restrict__ cnt, const int* __restrict__ blk_off, int nblk,
        int n, int* __restrict__ row_ptr, int* __restrict__ col, int* __restrict__ n_rad, int* __restrict__ n_ang,
        unsigned short* __restrict__ seg_cnt) {
-    __shared__ int wsum[8];
-    __shared__ int rstart[256];
+    __shared__ int wsum[ROWS_PER_BLK / 32];
+    __shared__ int rstart[ROWS_PER_BLK];
+    __shared__ int segs[P2_THREADS / 32][16];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int i0 = blockIdx.x * 256;
+    const int i0 = blockIdx.x * ROWS_PER_BLK;
     const bool ovf = blk_off[nblk + 1] != 0;
-    const int a = i0 + tid;
-    const int c = (a < n && !ovf) ? cnt[a] : 0;
-    int x = c;
+    if (tid < ROWS_PER_BLK) {
+        const int a = i0 + tid;
+        const int c = (a < n && !ovf) ? cnt[a] : 0;
+        int x = c;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        int y = __shfl_up_sync(0xffffffffu, x, o);
-        if (lane >= o) x += y;
+        for (int o = 1; o < 32; o <<= 1) {
+            int y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
+        }
+        if (lane == 31) wsum[warp] = x;
+        rstart[tid] = x - c;
     }
-    if (lane == 31) wsum[warp] = x;
     __syncthreads();
-    int before = ovf ? 0 : blk_off[blockIdx.x];
-    for (int q = 0; q < warp; ++q) before += wsum[q];
-    const int start = before + x - c;
-    rstart[tid] = start;
-    if (a < n) { row_ptr[a] = start; n_rad[a] = c; }
-    if (a == n - 1) row_ptr[n] = start + c;
+    if (tid < ROWS_PER_BLK) {
+        const int a = i0 + tid;
+        int before = ovf ? 0 : blk_off[blockIdx.x];
+        for (int q = 0; q < warp; ++q) before += wsum[q];
+        const int start = before + rstart[tid];
+        const int c = (a < n && !ovf) ? cnt[a] : 0;
+        if (a < n) { row_ptr[a] = start; n_rad[a] = c; }
+        if (a == n - 1) row_ptr[n] = start + c;
+        rstart[tid] = start;
+    }
     __syncthreads();
 
     const unsigned lt = (1u << lane) - 1u;
-    for (int q = 0; q < 32; ++q) {
-        const int i = i0 + warp * 32 + q;
+    int* sg = segs[warp];
+    for (int q = warp; q < ROWS_PER_BLK; q += P2_THREADS / 32) {
+        const int i = i0 + q;
         if (i >= n) break;
-        const int ni = ovf ? 0 : cnt[i];
+        const int ni = ovf ? 0 : n_rad[i];
         const unsigned* src = tmp + (size_t)i * stride;
-        int segc[14];
+        unsigned e[MAX_STRIDE_CHUNKS];
 #pragma unroll
-        for (int k = 0; k < 14; ++k) segc[k] = 0;
-        for (int t0 = 0; t0 < ni; t0 += 32) {
-            const int t = t0 + lane;
-            int key = -1;
-            if (t < ni) { const unsigned e = src[t]; key = (int)((e >> 28) & 7u) + ((e & ENT_RADIAL_ONLY) ? 7 : 0); }
+        for (int k = 0; k < MAX_STRIDE_CHUNKS; ++k) e[k] = (k * 32 + lane < ni) ? src[k * 32 + lane] : 0xffffffffu;
+        if (lane < 16) sg[lane] = 0;
+        __syncwarp();
+        // counts per key = class * 8 + species (class 0: angular, 1: radial-only); 15 = no entry
 #pragma unroll
-            for (int k = 0; k < 14; ++k) segc[k] += __popc(__ballot_sync(0xffffffffu, key == k));
-        }
-        int segs[14];
-        int run = rstart[warp * 32 + q];
-        int na = 0;
-#pragma unroll
-        for (int k = 0; k < 14; ++k) { segs[k] = run; run += segc[k]; if (k < 7) na += segc[k]; }
-        for (int t0 = 0; t0 < ni; t0 += 32) {
-            const int t = t0 + lane;
-            int key = -1;
-            unsigned e = 0;
-            if (t < ni) { e = src[t]; key = (int)((e >> 28) & 7u) + ((e & ENT_RADIAL_ONLY) ? 7 : 0); }
-#pragma unroll
-            for (int k = 0; k < 14; ++k) {
-                const unsigned m = __ballot_sync(0xffffffffu, key == k);
-                if (key == k) col[segs[k] + __popc(m & lt)] = (int)(e & 0x0fffffffu);
-                segs[k] += __popc(m);
+        for (int k = 0; k < MAX_STRIDE_CHUNKS; ++k) {
+            if (k * 32 < ni) {
+                const int key = (e[k] == 0xffffffffu) ? 15 : (int)((e[k] >> 28) & 15u);
+                const unsigned m = __match_any_sync(0xffffffffu, key);
+                if ((m & lt) == 0) sg[key] += __popc(m);      // group leader; keys are distinct across leaders
+                __syncwarp();
             }
         }
-        if (lane == 0) n_ang[i] = na;
-        if (lane < 16) {
-            int v = 0;
+        // lane k < 16 owns key k: exclusive prefix over keys -> segment starts
+        int cnt_k = lane < 16 ? sg[lane] : 0;
+        if (lane == 15 || lane == 7) cnt_k = 0;
+        int x = cnt_k;
 #pragma unroll
-            for (int k = 0; k < 14; ++k) if (lane == (k < 7 ? k : k + 1)) v = segc[k];
+        for (int o = 1; o < 16; o <<= 1) {
+            int y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
+        }
+        const int na = __shfl_sync(0xffffffffu, x, 7);
+        if (lane < 16) {
+            int v = cnt_k;
             if (lane == 7) v = na;
             if (lane == 15) v = ni - na;
             seg_cnt[(size_t)i * 16 + lane] = (unsigned short)v;
+        }
+        if (lane == 0) n_ang[i] = na;
+        __syncwarp();
+        if (lane < 16) sg[lane] = rstart[q] + x - cnt_k;
+        __syncwarp();
+#pragma unroll
+        for (int k = 0; k < MAX_STRIDE_CHUNKS; ++k) {
+            if (k * 32 < ni) {
+                const int key = (e[k] == 0xffffffffu) ? 15 : (int)((e[k] >> 28) & 15u);
+                const unsigned m = __match_any_sync(0xffffffffu, key);
+                const int base = sg[key];
+                if (key != 15) col[base + __popc(m & lt)] = (int)(e[k] & 0x0fffffffu);
+                __syncwarp();
+                if ((m & lt) == 0) sg[key] = base + __popc(m);
+                __syncwarp();
+            }
         }
     }
 }
@@ -566,7 +597,7 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
     ctx->n_mol = by_mol ? n_mol : 0;
     ctx->periodic = periodic;
     cudaStream_t st = ctx->stream;
-    const int nblk = (n + 255) / 256;
+    const int nblk = (n + ROWS_PER_BLK - 1) / ROWS_PER_BLK;
 
     DHP_CUDA(ctx, cudaMemsetAsync(ctx->status, 0, sizeof(int), st));
     DHP_CUDA(ctx, cudaMemsetAsync(ctx->cell_count, 0, sizeof(int) * (ctx->max_cells + 1), st));
@@ -612,10 +643,21 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
                ctx->row_species, ctx->row_slot);
     // pair list
     const double rcr2 = rcr * rcr, rca2 = rca * rca;
-    DHP_LAUNCH(ctx, k_pairs, (int)cell_bound, P1_THREADS, 0, ctx->spos, ctx->grid, ctx->cell_start, rcr2, rca2,
-               ctx->tmp_stride, ctx->n_rad, ctx->tmp_col, ctx->blk_sum, ctx->status);
+    bool wrap = false;     // same rule as k_setup_grid: a periodic axis with fewer than 3 cells
+    if (periodic) {
+        const double edge = rcr * (1.0 + 9.5367431640625e-07);
+        for (int c = 0; c < 3; ++c) wrap |= floor(L[c] / edge) < 3.0;
+        // k_setup_grid may coarsen the grid when it exceeds max_cells; be conservative then
+        if ((double)floor(L[0] / edge) * floor(L[1] / edge) * floor(L[2] / edge) > (double)ctx->max_cells) wrap = true;
+    }
+    if (wrap)
+        DHP_LAUNCH(ctx, k_pairs<true>, (int)cell_bound, P1_THREADS, 0, ctx->spos, ctx->grid, ctx->cell_start, rcr2, rca2,
+                   ctx->tmp_stride, ctx->n_rad, ctx->tmp_col, ctx->blk_sum, ctx->status);
+    else
+        DHP_LAUNCH(ctx, k_pairs<false>, (int)cell_bound, P1_THREADS, 0, ctx->spos, ctx->grid, ctx->cell_start, rcr2, rca2,
+                   ctx->tmp_stride, ctx->n_rad, ctx->tmp_col, ctx->blk_sum, ctx->status);
     DHP_LAUNCH(ctx, k_scan_blocks, 1, 1024, 0, ctx->blk_sum, ctx->blk_off, nblk, ctx->pair_cap, ctx->status);
-    DHP_LAUNCH(ctx, k_rows, nblk, 256, 0, ctx->tmp_col, ctx->tmp_stride, ctx->n_rad, ctx->blk_off, nblk, n, ctx->row_ptr,
+    DHP_LAUNCH(ctx, k_rows, nblk, P2_THREADS, 0, ctx->tmp_col, ctx->tmp_stride, ctx->n_rad, ctx->blk_off, nblk, n, ctx->row_ptr,
                ctx->col, ctx->n_rad, ctx->n_ang, ctx->seg_cnt);
     DHP_CUDA(ctx, cudaGetLastError());
     return DHP_OK;
