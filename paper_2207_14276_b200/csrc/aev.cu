@@ -149,7 +149,7 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
             S.tA[lane] = make_float4(A[0], A[1], A[2], A[3]);
             S.tB[lane][0] = make_float4(B[0], B[1], B[2], B[3]);
             S.tB[lane][1] = make_float4(B[4], B[5], B[6], B[7]);
-            S.tp[lane] = pairidx(S.sp[j], S.sp[k]);
+            S.tp[lane] = ipair(S.sp[j], S.sp[k]);
         }
         __syncwarp();
         const int cnt = min(32, npairs - T0);
@@ -164,8 +164,9 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
 
     // ---- write the row (species-grouped row order) -------------------------------------------------
     float* out = aev + (size_t)rowmap[i] * AEV_LD;
-    for (int c = lane; c < AEV_RAD; c += 32) out[c] = S.rad[0][c] + S.rad[1][c];
-    for (int c = lane; c < AEV_ANG; c += 32) out[AEV_RAD + c] = S.ang[c];
+    // internal column order (dhp_internal.cuh): angular blocks by ipair(), radial blocks by species priority, zeros
+    for (int c = lane; c < AEV_ANG; c += 32) out[c] = S.ang[c];
+    for (int c = lane; c < AEV_RAD; c += 32) out[rad_col(c >> 4) + (c & 15)] = S.rad[0][c] + S.rad[1][c];
     if (lane < AEV_LD - AEV_DIM) out[AEV_DIM + lane] = 0.f;
 }
 
@@ -194,8 +195,8 @@ k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
     WarpSmemBwd& S = reinterpret_cast<WarpSmemBwd*>(smem_raw)[w];
 
     const float* grow = grad + (size_t)rowmap[i] * AEV_LD;
-    for (int c = lane; c < AEV_RAD; c += 32) S.grad_rad[c] = grow[c];
-    for (int c = lane; c < AEV_ANG; c += 32) S.grad_ang[(c >> 5) * GP + (c & 31)] = grow[AEV_RAD + c];
+    for (int c = lane; c < AEV_RAD; c += 32) S.grad_rad[c] = grow[rad_col(c >> 4) + (c & 15)];
+    for (int c = lane; c < AEV_ANG; c += 32) S.grad_ang[(c >> 5) * GP + (c & 31)] = grow[c];
 
     const float4 pi = spos[i];
     const int rb = row_ptr[i], re = row_ptr[i + 1];
@@ -231,7 +232,7 @@ k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
                 const float s = sqrtf(cx * cx + cy * cy + cz * cz);
                 const float fj = S.fc[j], fk = S.fc[k], dfj = S.dfc[j], dfk = S.dfc[k];
                 const float Rm = 0.5f * (Rj + Rk);
-                const float* gb = &S.grad_ang[GP * pairidx(S.sp[j], S.sp[k])];
+                const float* gb = &S.grad_ang[GP * ipair(S.sp[j], S.sp[k])];
                 float Az[NZ], dAz[NZ];
 #pragma unroll
                 for (int z = 0; z < NZ; ++z) {

@@ -40,7 +40,7 @@ static bool dalloc(T** p, size_t count) {
 static void free_all(Ctx* c) {
     void* ptrs[] = {c->grid, c->status, c->bbox, c->cell_of, c->perm_tmp, c->cell_count, c->cell_start, c->cell_fill, c->perm,
                     c->inv_perm, c->spos, c->smol, c->n_rad, c->n_ang, c->row_ptr, c->col, c->sp_count, c->sp_start,
-                    c->rowmap, c->row_species, c->row_slot, c->blk_hist, c->aev, c->grad, c->e_atom, c->fsorted,
+                    c->rowmap, c->row_species, c->row_slot, c->blk_hist, c->tile_mask, c->tc_sched, c->col2feat, c->aev, c->grad, c->e_atom, c->fsorted,
                     c->e_out_tmp, c->export_tmp, c->tmp_col, c->blk_sum, c->blk_off, c->seg_cnt, c->st_pos, c->st_species, c->st_mol, c->st_E, c->st_F};
     for (void* p : ptrs) if (p) cudaFree(p);
     mlp_simt_free(c);
@@ -106,12 +106,22 @@ static int run_energy_forces(Ctx* ctx, const float* pos, const float* box, const
 }
 
 // debug gathers: buffer rows -> caller's atom order
+// With a column map the source is in the internal column order; feature blocks that are inactive for the row's
+// tile were never computed (they are identically zero in the AEV and unused in dE/dAEV) and read as 0.
 __global__ void k_gather_rows(const float* __restrict__ src, int ld_src, int ncol, const int* __restrict__ rowmap,
-                              const int* __restrict__ inv_perm, int n, float* __restrict__ dst) {
+                              const int* __restrict__ inv_perm, int n, const int* __restrict__ col2feat,
+                              const unsigned* __restrict__ tile_mask, float* __restrict__ dst) {
     int a = blockIdx.x;
     if (a >= n) return;
-    const float* s = src + (size_t)rowmap[inv_perm[a]] * ld_src;
-    for (int c = threadIdx.x; c < ncol; c += blockDim.x) dst[(size_t)a * ncol + c] = s[c];
+    const int row = rowmap[inv_perm[a]];
+    const float* s = src + (size_t)row * ld_src;
+    if (!col2feat) {
+        for (int c = threadIdx.x; c < ncol; c += blockDim.x) dst[(size_t)a * ncol + c] = s[c];
+        return;
+    }
+    const unsigned mask = tile_mask[row / ROW_TILE];
+    for (int c = threadIdx.x; c < AEV_DIM; c += blockDim.x)
+        dst[(size_t)a * ncol + col2feat[c]] = ((mask >> (c / KBLK)) & 1u) ? s[c] : 0.f;
 }
 
 }  // namespace dhp
@@ -163,6 +173,7 @@ int dhp_create(dhp_ctx** out, const dhp_params* params, int64_t max_atoms, int64
     ok &= dalloc(&c->sp_count, 8) && dalloc(&c->sp_start, 8) && dalloc(&c->rowmap, N);
     ok &= dalloc(&c->row_species, R) && dalloc(&c->row_slot, R) && dalloc(&c->blk_hist, (N / 256 + 2) * 8);
     ok &= dalloc(&c->aev, R * AEV_LD) && dalloc(&c->grad, R * AEV_LD) && dalloc(&c->e_atom, R);
+    ok &= dalloc(&c->tile_mask, R / ROW_TILE) && dalloc(&c->tc_sched, 8) && dalloc(&c->col2feat, AEV_LD);
     ok &= dalloc(&c->fsorted, 3 * N) && dalloc(&c->e_out_tmp, NM) && dalloc(&c->export_tmp, N + 1);
     ok &= dalloc(&c->st_pos, 3 * N) && dalloc(&c->st_species, N) && dalloc(&c->st_mol, NM + 1) && dalloc(&c->st_E, NM) && dalloc(&c->st_F, 3 * N);
     if (ok) ok = mlp_simt_alloc(c) == DHP_OK;
@@ -173,6 +184,9 @@ int dhp_create(dhp_ctx** out, const dhp_params* params, int64_t max_atoms, int64
         ok &= cudaMemset(c->aev, 0, sizeof(float) * R * AEV_LD) == cudaSuccess;
         ok &= cudaMemset(c->grad, 0, sizeof(float) * R * AEV_LD) == cudaSuccess;
         ok &= cudaMemset(c->status, 0, sizeof(int)) == cudaSuccess;
+        int map[AEV_LD];
+        for (int col = 0; col < AEV_LD; ++col) map[col] = col2feat(col);
+        ok &= cudaMemcpy(c->col2feat, map, sizeof(map), cudaMemcpyHostToDevice) == cudaSuccess;
     }
     if (!ok) { cudaGetLastError(); free_all(c); delete h; return DHP_E_NOMEM; }
     *out = h;
@@ -314,19 +328,20 @@ int dhp_set_mlp_mode(dhp_ctx* h, int mode) {
 
 int dhp_tensor_path_available(dhp_ctx* h) { return h && mlp_tc_available(&h->c) ? 1 : 0; }
 
-static int debug_gather(dhp_ctx* h, const float* src, int ld, int ncol, float* dst) {
+static int debug_gather(dhp_ctx* h, const float* src, int ld, int ncol, float* dst, bool feature_rows) {
     if (!h || !dst) return DHP_E_BADARG;
     Ctx* c = &h->c;
     const int n = (int)c->n_atoms;
     if (n == 0) return DHP_OK;
-    DHP_LAUNCH(c, k_gather_rows, n, 128, 0, src, ld, ncol, c->rowmap, c->inv_perm, n, dst);
+    DHP_LAUNCH(c, k_gather_rows, n, 128, 0, src, ld, ncol, c->rowmap, c->inv_perm, n,
+               feature_rows ? c->col2feat : (const int*)nullptr, c->tile_mask, dst);
     DHP_CUDA(c, cudaGetLastError());
     DHP_CUDA(c, cudaStreamSynchronize(c->stream));
     return DHP_OK;
 }
-int dhp_debug_aev(dhp_ctx* h, float* aev) { return h ? debug_gather(h, h->c.aev, AEV_LD, AEV_DIM, aev) : DHP_E_BADARG; }
-int dhp_debug_grad(dhp_ctx* h, float* grad) { return h ? debug_gather(h, h->c.grad, AEV_LD, AEV_DIM, grad) : DHP_E_BADARG; }
-int dhp_debug_atomic_energy(dhp_ctx* h, float* e) { return h ? debug_gather(h, h->c.e_atom, 1, 1, e) : DHP_E_BADARG; }
+int dhp_debug_aev(dhp_ctx* h, float* aev) { return h ? debug_gather(h, h->c.aev, AEV_LD, AEV_DIM, aev, true) : DHP_E_BADARG; }
+int dhp_debug_grad(dhp_ctx* h, float* grad) { return h ? debug_gather(h, h->c.grad, AEV_LD, AEV_DIM, grad, true) : DHP_E_BADARG; }
+int dhp_debug_atomic_energy(dhp_ctx* h, float* e) { return h ? debug_gather(h, h->c.e_atom, 1, 1, e, false) : DHP_E_BADARG; }
 
 int dhp_profile_enable(dhp_ctx* h, int on) {
     if (!h) return DHP_E_BADARG;

@@ -31,6 +31,8 @@ constexpr int OFF_B4 = OFF_W4 + H3;
 static_assert(OFF_B4 + 1 == NET_PARAMS, "blob layout");
 
 constexpr int ROW_TILE = 128;                   // species groups start at multiples of this many rows
+constexpr int KBLK = 64;                        // feature-block width: the unit in which zero columns are skipped
+constexpr int N_KBLK = AEV_LD / KBLK;           // 16 blocks: 14 angular (2 species pairs each) + 2 radial
 constexpr int MAX_MODELS = 8;
 constexpr int MAX_ANG = 96;                     // angular neighbours staged per centre (status CAPACITY beyond)
 
@@ -119,7 +121,10 @@ struct Ctx {
     int* row_species;      // [max_rows] species of each row (-1 for padding rows)
     int* row_slot;         // [max_rows] sorted slot of each row (-1 for padding)
     int* blk_hist;         // per-block species histograms for the stable row assignment
-    float* aev;            // [max_rows][AEV_LD]
+    unsigned* tile_mask;   // [max_rows / ROW_TILE] bit b: feature block b is non-zero for some row of the tile
+    int* tc_sched;         // [8] dynamic tile counters of the tensor-path GEMMs
+    int* col2feat;         // [AEV_LD] internal column -> canonical feature (-1: padding)
+    float* aev;            // [max_rows][AEV_LD]  internal column order, see col2feat()
     float* grad;           // [max_rows][AEV_LD]  dE/dAEV
     float* e_atom;         // [max_rows]
     float* act[6];         // SIMT path intermediates: h1,h2,h3(delta3),delta2,delta1 ; see mlp_simt.cu
@@ -164,10 +169,39 @@ int mlp_tc_weights(Ctx* ctx, Weights* w);
 void mlp_tc_weights_free(Ctx* ctx, Weights* w);
 int mlp_tc(Ctx* ctx, const Weights* w);
 
-// upper-triangle row-major index of the unordered species pair (layout of the angular block)
+// upper-triangle row-major index of the unordered species pair (canonical layout of the angular block, Q9)
 __host__ __device__ inline int pairidx(int a, int b) {
     int u = a < b ? a : b, v = a < b ? b : a;
     return NSP * u - u * (u - 1) / 2 + (v - u);
+}
+
+// ---- internal column order of the AEV / dE/dAEV rows -------------------------------------------------
+// The buffers are private to the library, so their column order is free.  Columns are arranged so that the
+// 64-wide blocks a GEMM can skip are identically zero as often as possible for solvated biomolecules: species
+// are ranked H, O, C, N, S, F, Cl ("priority" q), the angular blocks come first, ordered by (max q, min q) of
+// the species pair - HH, HO, OO, HC, OC, CC, ... - then the radial blocks in priority order, then 16 zeros.
+// A water-only tile touches 3 of the 16 blocks.  Debug exports and the weight preparation translate with
+// col2feat(); the oracle and the tests only ever see the canonical order.
+constexpr unsigned SP_PRIO_PACKED = 0x6541320u;   // nibble s: priority position of species s
+constexpr unsigned PRIO_SP_PACKED = 0x6542130u;   // nibble q: species at priority position q
+__host__ __device__ inline int sp_prio(int s) { return (int)((SP_PRIO_PACKED >> (4 * s)) & 7u); }
+__host__ __device__ inline int prio_sp(int q) { return (int)((PRIO_SP_PACKED >> (4 * q)) & 7u); }
+__host__ __device__ inline int ipair(int sa, int sb) {
+    const int a = sp_prio(sa), b = sp_prio(sb);
+    const int lo = a < b ? a : b, hi = a < b ? b : a;
+    return hi * (hi + 1) / 2 + lo;
+}
+__host__ __device__ inline int rad_col(int s) { return AEV_ANG + NR * sp_prio(s); }
+__host__ __device__ inline int col2feat(int c) {
+    if (c < AEV_ANG) {
+        const int ip = c >> 5, rem = c & 31;
+        int hi = 0;
+        while ((hi + 1) * (hi + 2) / 2 <= ip) ++hi;
+        const int lo = ip - hi * (hi + 1) / 2;
+        return AEV_RAD + 32 * pairidx(prio_sp(lo), prio_sp(hi)) + rem;
+    }
+    if (c < AEV_DIM) return NR * prio_sp((c - AEV_ANG) >> 4) + (c & 15);
+    return -1;
 }
 
 }  // namespace dhp

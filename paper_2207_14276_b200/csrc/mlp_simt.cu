@@ -27,6 +27,8 @@ struct GemmArgs {
     int N, K;
     int n_models;                                   // EPI_SUM: models folded into the K loop
     float alpha;
+    const int* kmap;                                // internal AEV column -> canonical feature for the k index (layer 1), or null
+    const int* nmap;                                // the same for the n index (dE/dAEV), or null
 };
 
 template <int EPI, bool B_KMAJOR>
@@ -58,14 +60,16 @@ __global__ void __launch_bounds__(256) k_sgemm(const GemmArgs a, const int* __re
                 for (int q = 0; q < 4; ++q) {
                     int nn = (tid >> 4) + 16 * q, kk = tid & 15;
                     int ng = n0 + nn;
-                    Bs[kk][nn] = ng < a.N ? Bp[(size_t)ng * a.sbn + (size_t)(k0 + kk) * a.sbk] : 0.f;
+                    const int kf = a.kmap ? a.kmap[k0 + kk] : k0 + kk;
+                    Bs[kk][nn] = ng < a.N ? Bp[(size_t)ng * a.sbn + (size_t)kf * a.sbk] : 0.f;
                 }
             } else {
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
                     int nn = tid & 63, kk = (tid >> 6) + 4 * q;
                     int ng = n0 + nn;
-                    Bs[kk][nn] = ng < a.N ? Bp[(size_t)ng * a.sbn + (size_t)(k0 + kk) * a.sbk] : 0.f;
+                    const int nf = (a.nmap && ng < a.N) ? a.nmap[ng] : ng;
+                    Bs[kk][nn] = ng < a.N ? Bp[(size_t)nf * a.sbn + (size_t)(k0 + kk) * a.sbk] : 0.f;
                 }
             }
             __syncthreads();
@@ -151,8 +155,10 @@ int mlp_simt(Ctx* ctx, const Weights* w) {
     g.W = w->blob; g.alpha = alpha; g.n_models = M;
     // forward
     g.A = ctx->aev; g.lda = AEV_LD; g.a_model_stride = 0; g.w_off = OFF_W1; g.sbn = AEV_DIM; g.sbk = 1; g.bias_off = OFF_B1;
+    g.kmap = ctx->col2feat;
     g.C = h1; g.ldc = M * H1; g.c_model_stride = H1; g.N = H1; g.K = AEV_DIM;
     DHP_LAUNCH(ctx, (k_sgemm<EPI_CELU, true>), dim3(row_tiles, H1 / TN, M), 256, 0, g, ctx->row_species, ctx->sp_start);
+    g.kmap = nullptr;
     g.A = h1; g.lda = M * H1; g.a_model_stride = H1; g.w_off = OFF_W2; g.sbn = H1; g.bias_off = OFF_B2;
     g.C = h2; g.ldc = M * H2; g.c_model_stride = H2; g.N = H2; g.K = H1;
     DHP_LAUNCH(ctx, (k_sgemm<EPI_CELU, true>), dim3(row_tiles, H2 / TN, M), 256, 0, g, ctx->row_species, ctx->sp_start);
@@ -170,7 +176,7 @@ int mlp_simt(Ctx* ctx, const Weights* w) {
     g.Hs = h1; g.ldh = M * H1; g.h_model_stride = H1; g.C = d1; g.ldc = M * H1; g.c_model_stride = H1; g.N = H1; g.K = H2;
     DHP_LAUNCH(ctx, (k_sgemm<EPI_DCELU, false>), dim3(row_tiles, H1 / TN, M), 256, 0, g, ctx->row_species, ctx->sp_start);
     g.A = d1; g.lda = M * H1; g.a_model_stride = H1; g.w_off = OFF_W1; g.sbn = 1; g.sbk = AEV_DIM;
-    g.C = ctx->grad; g.ldc = AEV_LD; g.c_model_stride = 0; g.N = AEV_DIM; g.K = H1;
+    g.C = ctx->grad; g.ldc = AEV_LD; g.c_model_stride = 0; g.N = AEV_DIM; g.K = H1; g.nmap = ctx->col2feat;
     DHP_LAUNCH(ctx, (k_sgemm<EPI_SUM, false>), dim3(row_tiles, (AEV_DIM + TN - 1) / TN, 1), 256, 0, g, ctx->row_species, ctx->sp_start);
     DHP_CUDA(ctx, cudaGetLastError());
     return DHP_OK;

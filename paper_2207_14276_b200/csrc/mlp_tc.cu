@@ -7,6 +7,15 @@
 // 2^-22 relative).  Weights are pre-scaled by 2^6 and back-propagated deltas by 2^10 so that the lo terms stay in
 // the fp16 normal range; the power-of-two scales are removed exactly in the epilogues.
 //
+// Activation layout.  An epilogue thread owns one row (one TMEM lane), so row-major activations make every
+// 16-byte store of a warp land in a different 128-byte line.  The activation planes (h1, h2, d3, d2, d1) are
+// therefore stored as the image of the no-swizzle K-major UMMA operand tile:
+//     [plane hi/lo][row tile][64-column block][8-column group (8)][row in tile (128)][8 halves = 16 B]
+// so that the 32 lanes of a warp write (and, for CELU', read back) 512 contiguous bytes per instruction, and the
+// next GEMM fetches its A operand as one contiguous 16 KB cp.async.bulk per plane and K block (descriptor:
+// SWIZZLE_NONE, leading byte offset 2048 = next 8-column group, stride byte offset 128 = next 8 rows).
+// AEV rows (A of G1) and all weights (B) stay row-major and come in through TMA tensor maps with SWIZZLE_128B.
+//
 // One persistent, warp-specialised kernel template does all six GEMMs of the path:
 //   warp 0      TMA producer   (cp.async.bulk.tensor.2d, SWIZZLE_128B, 64-wide K blocks, mbarrier ring)
 //   warp 1      MMA issuer     (one elected lane: 3 x tcgen05.mma.cta_group::1.kind::f16 per 16-wide K step)
@@ -39,10 +48,12 @@ constexpr int STAGES = 2;
 constexpr int A_PLANE_BYTES = BM * BK * 2;       // 16 KB
 constexpr int B_SLOT_BYTES = 256 * BK * 2;       // 32 KB (BN <= 256)
 constexpr int STAGE_BYTES = 2 * A_PLANE_BYTES + 2 * B_SLOT_BYTES;   // 96 KB
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align*/ + 256 /*barriers, TMEM word, tile ring*/;
 constexpr int TMEM_COLS = 512;
 constexpr int ACC_STRIDE = 256;    // TMEM columns per accumulator stage
 constexpr int EPI_WARPS = 8;         // two per TMEM lane quadrant, splitting the column chunks
+constexpr int RING = 4;              // depth of the tile-id ring between the scheduler (TMA warp) and the other roles
+constexpr int NB_BLOCK_BYTES = KBLK * BK * 2;   // one 64-row block of a B tile (8 KB)
 constexpr int TC_THREADS = 64 + 32 * EPI_WARPS;
 constexpr float W_SCALE = 64.0f;       // 2^6 on every weight matrix
 constexpr float D_SCALE = 1024.0f;     // 2^10 on the back-propagated deltas
@@ -65,13 +76,23 @@ struct TcArgs {
     const float* b4;          // [species][models]
     float inv_models;
     float alpha;
-    __half* out_planes;       // [2][out_plane_rows][out_ld]  hi plane then lo plane
-    int out_ld;
-    int out_plane_rows;
+    __half* out_planes;       // tiled activation planes (hi plane then lo plane)
+    int out_ld;               // EPI_GRAD: row pitch of out_f32
     const __half* h_planes;   // saved activations for CELU' (EPI_DCELU), same geometry as out
     float* out_f32;           // EPI_GRAD: [rows][out_ld]
     float* e_atom;            // EPI_OUT
+    const __half* a_tiled;    // A in the tiled activation layout (null: A comes through tmA, row-major AEV planes)
+    int a_kblocks;            // 64-column blocks per row tile of the A buffer
+    int a_kb_per_tile;        // A block offset per column tile (per-model activations), else 0
+    int plane_tiles;          // row tiles per plane of every activation buffer (max_rows / 128)
+    int out_kblocks;          // 64-column blocks per row tile of the output buffer (and of h_planes)
+    int out_cols_per_tile;    // output column pitch per column tile (BN, or 192 for the 160-wide d3)
+    const unsigned* tile_mask;  // [row tiles] active 64-wide feature blocks (G1: K blocks to visit, B1: N blocks to produce)
+    int* sched;               // dynamic tile counter of this launch (zeroed by the host)
 };
+
+// how the feature-block mask of a row tile is used
+enum { CMP_NONE = 0, CMP_K = 1, CMP_N = 2 };
 
 // ---- PTX wrappers ------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -102,6 +123,10 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar) {
     asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
                  ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
 __device__ __forceinline__ void prefetch_tmap(const CUtensorMap* map) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
@@ -149,6 +174,16 @@ __device__ __forceinline__ uint64_t make_smem_desc(uint32_t saddr) {
     d |= (uint64_t)2 << 61;
     return d;
 }
+// K-major operand without swizzle, [8-column group][row][16 B]: leading byte offset (next core matrix along K) 2048,
+// stride byte offset (next 8 rows) 128
+__device__ __forceinline__ uint64_t make_smem_desc_tiled(uint32_t saddr) {
+    uint64_t d = 0;
+    d |= (uint64_t)((saddr & 0x3FFFF) >> 4);
+    d |= (uint64_t)(2048 >> 4) << 16;
+    d |= (uint64_t)(128 >> 4) << 32;
+    d |= (uint64_t)1 << 46;
+    return d;
+}
 // instruction descriptor: D = f32, A = B = f16, both K-major, M = 128, N = bn
 __device__ __forceinline__ uint32_t make_idesc(int bn) {
     return (1u << 4) | ((uint32_t)(bn >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
@@ -189,15 +224,36 @@ __device__ __forceinline__ uint32_t pack_half2(__half a, __half b) {
     __half2 h = __halves2half2(a, b);
     return *reinterpret_cast<uint32_t*>(&h);
 }
-// 32 consecutive values of one row -> hi and lo planes (4 x 16-byte stores each)
-__device__ __forceinline__ void store_split32(const float (&x)[32], __half* hi_dst, __half* lo_dst) {
+__device__ __forceinline__ void unpack_add(uint32_t h, uint32_t l, float& a, float& b) {
+    const float2 fh = __half22float2(*reinterpret_cast<__half2*>(&h));
+    const float2 fl = __half22float2(*reinterpret_cast<__half2*>(&l));
+    a = fh.x + fl.x;
+    b = fh.y + fl.y;
+}
+// tiled activation layout: element offset of (row tile rt, 64-column block kb) and, inside it, of (8-column group g, row r)
+__device__ __forceinline__ size_t tile_off(int plane_tiles, int kblocks, int plane, int rt, int kb) {
+    return ((size_t)(plane * plane_tiles + rt) * kblocks + kb) * (size_t)(BM * BK);
+}
+// 32 consecutive columns (4 groups) of one row -> hi and lo planes; tile pointers already include group and row
+__device__ __forceinline__ void store_split32_tiled(const float (&x)[32], __half* hi_dst, __half* lo_dst) {
     uint32_t ph[16], pl[16];
 #pragma unroll
     for (int i = 0; i < 16; ++i) split_pair(x[2 * i], x[2 * i + 1], ph[i], pl[i]);
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-        reinterpret_cast<uint4*>(hi_dst)[i] = make_uint4(ph[4 * i], ph[4 * i + 1], ph[4 * i + 2], ph[4 * i + 3]);
-        reinterpret_cast<uint4*>(lo_dst)[i] = make_uint4(pl[4 * i], pl[4 * i + 1], pl[4 * i + 2], pl[4 * i + 3]);
+        *reinterpret_cast<uint4*>(hi_dst + i * (BM * 8)) = make_uint4(ph[4 * i], ph[4 * i + 1], ph[4 * i + 2], ph[4 * i + 3]);
+        *reinterpret_cast<uint4*>(lo_dst + i * (BM * 8)) = make_uint4(pl[4 * i], pl[4 * i + 1], pl[4 * i + 2], pl[4 * i + 3]);
+    }
+}
+__device__ __forceinline__ void load_joined32_tiled(const __half* hi_src, const __half* lo_src, float (&x)[32]) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const uint4 h = *reinterpret_cast<const uint4*>(hi_src + i * (BM * 8));
+        const uint4 l = *reinterpret_cast<const uint4*>(lo_src + i * (BM * 8));
+        unpack_add(h.x, l.x, x[8 * i + 0], x[8 * i + 1]);
+        unpack_add(h.y, l.y, x[8 * i + 2], x[8 * i + 3]);
+        unpack_add(h.z, l.z, x[8 * i + 4], x[8 * i + 5]);
+        unpack_add(h.w, l.w, x[8 * i + 6], x[8 * i + 7]);
     }
 }
 __device__ __forceinline__ void load32(const float* __restrict__ src, float (&x)[32]) {
@@ -207,25 +263,20 @@ __device__ __forceinline__ void load32(const float* __restrict__ src, float (&x)
         x[4 * i] = v.x; x[4 * i + 1] = v.y; x[4 * i + 2] = v.z; x[4 * i + 3] = v.w;
     }
 }
-__device__ __forceinline__ void unpack_add(uint32_t h, uint32_t l, float& a, float& b) {
-    const float2 fh = __half22float2(*reinterpret_cast<__half2*>(&h));
-    const float2 fl = __half22float2(*reinterpret_cast<__half2*>(&l));
-    a = fh.x + fl.x;
-    b = fh.y + fl.y;
-}
-__device__ __forceinline__ void load_joined32(const __half* hi_src, const __half* lo_src, float (&x)[32]) {
+
+// the (up to 4) feature blocks that column tile nt of a row tile produces: set bits 4 nt .. 4 nt + 3 of the mask
+__device__ __forceinline__ int select_blocks(unsigned mask, int nt, int (&sel)[4]) {
+    for (int i = 0; i < 4 * nt; ++i) mask &= mask - 1u;
+    int n = 0;
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-        const uint4 h = reinterpret_cast<const uint4*>(hi_src)[i];
-        const uint4 l = reinterpret_cast<const uint4*>(lo_src)[i];
-        unpack_add(h.x, l.x, x[8 * i + 0], x[8 * i + 1]);
-        unpack_add(h.y, l.y, x[8 * i + 2], x[8 * i + 3]);
-        unpack_add(h.z, l.z, x[8 * i + 4], x[8 * i + 5]);
-        unpack_add(h.w, l.w, x[8 * i + 6], x[8 * i + 7]);
+        sel[i] = 0;
+        if (mask) { sel[i] = __ffs(mask) - 1; mask &= mask - 1u; n = i + 1; }
     }
+    return n;
 }
 
-template <int EPI>
+template <int EPI, int CMP>
 __global__ void __launch_bounds__(TC_THREADS, 1)
 k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const TcArgs p) {
     extern __shared__ uint8_t smem_raw[];
@@ -234,21 +285,28 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     uint8_t* base_ptr = smem_raw + (base - raw);
     uint64_t* bars = reinterpret_cast<uint64_t*>(base_ptr + STAGES * STAGE_BYTES);
     const uint32_t bar0 = base + STAGES * STAGE_BYTES;
-    // barrier layout: full[STAGES], empty[STAGES], tfull[2], tempty[2], then the TMEM base address word
+    // barrier layout: full[STAGES], empty[STAGES], tfull[2], tempty[2], sfull[RING], sempty[RING], then the TMEM base
+    // address word and the tile-id ring
+    constexpr int NBARS = 2 * STAGES + 4 + 2 * RING;
     auto full_bar = [&](int s) { return bar0 + 8u * s; };
     auto empty_bar = [&](int s) { return bar0 + 8u * (STAGES + s); };
     auto tfull_bar = [&](int s) { return bar0 + 8u * (2 * STAGES + s); };
     auto tempty_bar = [&](int s) { return bar0 + 8u * (2 * STAGES + 2 + s); };
-    volatile uint32_t* tmem_word = reinterpret_cast<volatile uint32_t*>(bars + 2 * STAGES + 4);
+    auto sfull_bar = [&](int s) { return bar0 + 8u * (2 * STAGES + 4 + s); };
+    auto sempty_bar = [&](int s) { return bar0 + 8u * (2 * STAGES + 4 + RING + s); };
+    volatile uint32_t* tmem_word = reinterpret_cast<volatile uint32_t*>(bars + NBARS);
+    volatile int* ring = reinterpret_cast<volatile int*>(bars + NBARS + 1);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n_row_tiles = p.sp_start[NSP] / BM;
     const int total_tiles = n_row_tiles * p.n_tiles;
     const int KB = (p.K + BK - 1) / BK;
+    const unsigned all_k = KB >= 32 ? 0xffffffffu : ((1u << KB) - 1u);
 
     if (warp == 0 && lane == 0) {
         for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
         for (int s = 0; s < 2; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), EPI_WARPS); }
+        for (int s = 0; s < RING; ++s) { mbar_init(sfull_bar(s), 1); mbar_init(sempty_bar(s), 1 + EPI_WARPS); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         prefetch_tmap(&tmA);
         prefetch_tmap(&tmB);
@@ -259,25 +317,73 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     tc_fence_after();
     const uint32_t tmem_base = *tmem_word;
 
+    // G1 visits only the K blocks that are non-zero for the row tile (an all-zero tile - isolated atoms - still
+    // runs one block of zeros so that the accumulator is defined); everything else visits all of K.
+    auto k_mask = [&](int rt) -> unsigned {
+        if (CMP != CMP_K) return all_k;
+        const unsigned m = p.tile_mask[rt];
+        return m ? m : (1u << 14);
+    };
+
     if (warp == 0) {
-        // ===== TMA producer =====
+        // ===== tile scheduler + TMA producer =====
         if (elect_one()) {
             int stage = 0; uint32_t phase = 0;
-            const uint32_t tx = 2u * A_PLANE_BYTES + 2u * (uint32_t)p.BN * BK * 2u;
-            for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-                const int rt = tile / p.n_tiles, nt = tile - rt * p.n_tiles;
+            int slot = 0; uint32_t sphase = 0;
+            for (;;) {
+                int tile, rt = 0, nt = 0;
+                for (;;) {
+                    tile = atomicAdd(p.sched, 1);
+                    if (tile >= total_tiles) { tile = -1; break; }
+                    rt = tile / p.n_tiles; nt = tile - rt * p.n_tiles;
+                    if (CMP != CMP_N || 4 * nt < __popc(p.tile_mask[rt])) break;      // B1: nothing to produce
+                }
+                mbar_wait(sempty_bar(slot), sphase ^ 1u);
+                ring[slot] = tile;
+                mbar_arrive(sfull_bar(slot));
+                if (++slot == RING) { slot = 0; sphase ^= 1u; }
+                if (tile < 0) break;
                 const int row0 = rt * BM;
                 const int s = max(p.row_species[row0], 0);
-                const int brow = (2 * s) * p.b_rows_per_species + nt * p.b_rows_per_tile;
-                for (int kb = 0; kb < KB; ++kb) {
+                int brow = (2 * s) * p.b_rows_per_species;
+                int sel[4] = {0, 0, 0, 0};
+                int nb = 0;
+                uint32_t tx;
+                if (CMP == CMP_N) {
+                    nb = select_blocks(p.tile_mask[rt], nt, sel);
+                    tx = 2u * A_PLANE_BYTES + 2u * (uint32_t)nb * NB_BLOCK_BYTES;
+                } else {
+                    brow += nt * p.b_rows_per_tile;
+                    tx = 2u * A_PLANE_BYTES + 2u * (uint32_t)p.BN * BK * 2u;
+                }
+                for (unsigned km = k_mask(rt); km; km &= km - 1u) {
+                    const int kb = __ffs(km) - 1;
                     mbar_wait(empty_bar(stage), phase ^ 1u);
                     const uint32_t sa = base + stage * STAGE_BYTES;
                     mbar_expect_tx(full_bar(stage), tx);
-                    const int ka = p.a_k_off_per_tile * nt + kb * BK;
-                    tma_load_2d(sa, &tmA, ka, row0, full_bar(stage));
-                    tma_load_2d(sa + A_PLANE_BYTES, &tmA, ka, p.a_plane_rows + row0, full_bar(stage));
-                    tma_load_2d(sa + 2 * A_PLANE_BYTES, &tmB, kb * BK, brow, full_bar(stage));
-                    tma_load_2d(sa + 2 * A_PLANE_BYTES + B_SLOT_BYTES, &tmB, kb * BK, brow + p.b_rows_per_species, full_bar(stage));
+                    if (p.a_tiled) {
+                        const int kba = p.a_kb_per_tile * nt + kb;
+                        bulk_load(sa, p.a_tiled + tile_off(p.plane_tiles, p.a_kblocks, 0, rt, kba), A_PLANE_BYTES, full_bar(stage));
+                        bulk_load(sa + A_PLANE_BYTES, p.a_tiled + tile_off(p.plane_tiles, p.a_kblocks, 1, rt, kba), A_PLANE_BYTES,
+                                  full_bar(stage));
+                    } else {
+                        const int ka = p.a_k_off_per_tile * nt + kb * BK;
+                        tma_load_2d(sa, &tmA, ka, row0, full_bar(stage));
+                        tma_load_2d(sa + A_PLANE_BYTES, &tmA, ka, p.a_plane_rows + row0, full_bar(stage));
+                    }
+                    const uint32_t sb = sa + 2 * A_PLANE_BYTES;
+                    if (CMP == CMP_N) {
+#pragma unroll
+                        for (int j = 0; j < 4; ++j)
+                            if (j < nb) {
+                                tma_load_2d(sb + j * NB_BLOCK_BYTES, &tmB, kb * BK, brow + sel[j] * KBLK, full_bar(stage));
+                                tma_load_2d(sb + B_SLOT_BYTES + j * NB_BLOCK_BYTES, &tmB, kb * BK,
+                                            brow + p.b_rows_per_species + sel[j] * KBLK, full_bar(stage));
+                            }
+                    } else {
+                        tma_load_2d(sb, &tmB, kb * BK, brow, full_bar(stage));
+                        tma_load_2d(sb + B_SLOT_BYTES, &tmB, kb * BK, brow + p.b_rows_per_species, full_bar(stage));
+                    }
                     if (++stage == STAGES) { stage = 0; phase ^= 1u; }
                 }
             }
@@ -287,24 +393,40 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         if (elect_one()) {
             int stage = 0; uint32_t phase = 0;
             int acc = 0; uint32_t acc_phase = 0;
-            const uint32_t idesc = make_idesc(p.BN);
-            for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+            int slot = 0; uint32_t sphase = 0;
+            for (;;) {
+                mbar_wait(sfull_bar(slot), sphase);
+                const int tile = ring[slot];
+                mbar_arrive(sempty_bar(slot));
+                if (++slot == RING) { slot = 0; sphase ^= 1u; }
+                if (tile < 0) break;
+                const int rt = tile / p.n_tiles, nt = tile - rt * p.n_tiles;
+                int bn = p.BN;
+                if (CMP == CMP_N) bn = KBLK * min(4, __popc(p.tile_mask[rt]) - 4 * nt);
+                const uint32_t idesc = make_idesc(bn);
                 mbar_wait(tempty_bar(acc), acc_phase ^ 1u);
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + (uint32_t)(acc * ACC_STRIDE);
-                for (int kb = 0; kb < KB; ++kb) {
+                uint32_t accumulate = 0u;
+                for (unsigned km = k_mask(rt); km; km &= km - 1u) {
+                    const int kb = __ffs(km) - 1;
                     mbar_wait(full_bar(stage), phase);
                     tc_fence_after();
                     const uint32_t sa = base + stage * STAGE_BYTES;
-                    const uint64_t a_hi = make_smem_desc(sa), a_lo = make_smem_desc(sa + A_PLANE_BYTES);
+                    const bool tiled = p.a_tiled != nullptr;
+                    const uint64_t a_hi = tiled ? make_smem_desc_tiled(sa) : make_smem_desc(sa);
+                    const uint64_t a_lo = tiled ? make_smem_desc_tiled(sa + A_PLANE_BYTES) : make_smem_desc(sa + A_PLANE_BYTES);
                     const uint64_t b_hi = make_smem_desc(sa + 2 * A_PLANE_BYTES);
                     const uint64_t b_lo = make_smem_desc(sa + 2 * A_PLANE_BYTES + B_SLOT_BYTES);
+                    // one K step = 16 fp16: 32 bytes inside a swizzled 128-byte row, or two 8-column groups (4096 bytes) when tiled
+                    const uint64_t a_step = tiled ? (uint64_t)(4096 >> 4) : 2u;
                     const int ksteps = min(BK / 16, (p.K - kb * BK) / 16);
                     for (int k = 0; k < ksteps; ++k) {
-                        const uint64_t adv = (uint64_t)(k * 2);          // 16 fp16 = 32 bytes = 2 x 16-byte units
-                        umma_f16(d_tmem, a_hi + adv, b_hi + adv, idesc, (kb | k) ? 1u : 0u);
-                        umma_f16(d_tmem, a_hi + adv, b_lo + adv, idesc, 1u);
-                        umma_f16(d_tmem, a_lo + adv, b_hi + adv, idesc, 1u);
+                        const uint64_t adv = (uint64_t)(k * 2), a_adv = (uint64_t)k * a_step;
+                        umma_f16(d_tmem, a_hi + a_adv, b_hi + adv, idesc, accumulate);
+                        umma_f16(d_tmem, a_hi + a_adv, b_lo + adv, idesc, 1u);
+                        umma_f16(d_tmem, a_lo + a_adv, b_hi + adv, idesc, 1u);
+                        accumulate = 1u;
                     }
                     umma_commit(empty_bar(stage));                     // frees the smem stage when the MMAs retire
                     if (++stage == STAGES) { stage = 0; phase ^= 1u; }
@@ -318,35 +440,46 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         //       lane quadrant take alternate 32-column chunks) =====
         const int q = warp & 3, half = (warp - 2) >> 2;
         int acc = 0; uint32_t acc_phase = 0;
+        int slot = 0; uint32_t sphase = 0;
         const float kexp = 1.4426950408889634f / p.alpha, inv_alpha = 1.0f / p.alpha;
-        for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+        for (;;) {
+            mbar_wait(sfull_bar(slot), sphase);
+            const int tile = ring[slot];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(sempty_bar(slot));
+            if (++slot == RING) { slot = 0; sphase ^= 1u; }
+            if (tile < 0) break;
             const int rt = tile / p.n_tiles, nt = tile - rt * p.n_tiles;
             const int row = rt * BM + q * 32 + lane;
             const int s = max(p.row_species[rt * BM], 0);
             const int ncols = p.n_tiles * p.BN;
-            const size_t plane = (size_t)p.out_plane_rows * p.out_ld;
+            const int r_in = q * 32 + lane;
+            int sel[4] = {0, 0, 0, 0};
+            int bn = p.BN;
+            if (CMP == CMP_N) bn = KBLK * select_blocks(p.tile_mask[rt], nt, sel);
             mbar_wait(tfull_bar(acc), acc_phase);
             tc_fence_after();
             const uint32_t t_row = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * ACC_STRIDE);
             float e_acc = 0.f;
-            for (int c0 = half * 32; c0 < p.BN; c0 += 64) {
+            for (int c0 = half * 32; c0 < bn; c0 += 64) {
                 const int col = nt * p.BN + c0;
                 uint32_t v[32];
                 float x[32], aux[32];
                 tmem_ld32_issue(t_row + (uint32_t)c0, v);
                 if (EPI == EPI_CELU || EPI == EPI_OUT) load32(p.bias + (size_t)s * ncols + col, aux);
-                if (EPI == EPI_DCELU) {
-                    const __half* hh = p.h_planes + (size_t)row * p.out_ld + col;
-                    load_joined32(hh, hh + plane, aux);
-                }
+                // tiled output (and saved-activation) position of this thread's 32 columns
+                const int ocol = nt * p.out_cols_per_tile + c0;
+                const size_t in_tile = (size_t)(((ocol & 63) >> 3) * BM + r_in) * 8;
+                const size_t o_hi = tile_off(p.plane_tiles, p.out_kblocks, 0, rt, ocol >> 6) + in_tile;
+                const size_t o_lo = tile_off(p.plane_tiles, p.out_kblocks, 1, rt, ocol >> 6) + in_tile;
+                if (EPI == EPI_DCELU) load_joined32_tiled(p.h_planes + o_hi, p.h_planes + o_lo, aux);
                 tmem_ld_wait();
                 if (EPI == EPI_CELU || EPI == EPI_OUT) {
 #pragma unroll
                     for (int i = 0; i < 32; ++i) x[i] = celu_f(fmaf(__uint_as_float(v[i]), p.acc_scale, aux[i]), p.alpha, kexp);
                 }
                 if (EPI == EPI_CELU) {
-                    __half* hi = p.out_planes + (size_t)row * p.out_ld + col;
-                    store_split32(x, hi, hi + plane);
+                    store_split32_tiled(x, p.out_planes + o_hi, p.out_planes + o_lo);
                 } else if (EPI == EPI_OUT) {
                     load32(p.w4 + (size_t)s * ncols + col, aux);
                     const float dsc = p.inv_models * D_SCALE;
@@ -355,15 +488,19 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                         e_acc = fmaf(aux[i], x[i], e_acc);
                         x[i] = aux[i] * dsc * dcelu_from_h(x[i], inv_alpha);
                     }
-                    __half* hi = p.out_planes + (size_t)row * p.out_ld + col;
-                    store_split32(x, hi, hi + plane);
+                    store_split32_tiled(x, p.out_planes + o_hi, p.out_planes + o_lo);
                 } else if (EPI == EPI_DCELU) {
 #pragma unroll
                     for (int i = 0; i < 32; ++i) x[i] = __uint_as_float(v[i]) * p.acc_scale * dcelu_from_h(aux[i], inv_alpha);
-                    __half* hi = p.out_planes + (size_t)row * p.out_ld + col;
-                    store_split32(x, hi, hi + plane);
+                    store_split32_tiled(x, p.out_planes + o_hi, p.out_planes + o_lo);
                 } else {   // EPI_GRAD
-                    float4* dst = reinterpret_cast<float4*>(p.out_f32 + (size_t)row * p.out_ld + col);
+                    int gcol = col;
+                    if (CMP == CMP_N) {                                  // chunk c0 belongs to the (c0/64)-th selected block
+                        const int j = c0 >> 6;
+                        const int blk = j == 0 ? sel[0] : j == 1 ? sel[1] : j == 2 ? sel[2] : sel[3];
+                        gcol = blk * KBLK + (c0 & 63);
+                    }
+                    float4* dst = reinterpret_cast<float4*>(p.out_f32 + (size_t)row * p.out_ld + gcol);
 #pragma unroll
                     for (int i = 0; i < 8; ++i)
                         dst[i] = make_float4(__uint_as_float(v[4 * i]) * p.acc_scale, __uint_as_float(v[4 * i + 1]) * p.acc_scale,
@@ -408,8 +545,8 @@ __global__ void k_prep_weights(const float* __restrict__ blob, int n_models, int
         float v = 0.f;
         int e, n, k;
         switch (mode) {
-            case WP_W1F: e = r / H1; n = r % H1; k = c;
-                if (k < AEV_DIM) v = blob[(size_t)(e * NSP + s) * NET_PARAMS + OFF_W1 + (size_t)n * AEV_DIM + k]; break;
+            case WP_W1F: e = r / H1; n = r % H1; k = col2feat(c);       // columns in the internal AEV order
+                if (k >= 0) v = blob[(size_t)(e * NSP + s) * NET_PARAMS + OFF_W1 + (size_t)n * AEV_DIM + k]; break;
             case WP_W2F: e = r / H2; n = r % H2; k = c;
                 v = blob[(size_t)(e * NSP + s) * NET_PARAMS + OFF_W2 + n * H1 + k]; break;
             case WP_W3F: e = r / H3; n = r % H3; k = c;
@@ -418,8 +555,8 @@ __global__ void k_prep_weights(const float* __restrict__ blob, int n_models, int
                 v = blob[(size_t)(e * NSP + s) * NET_PARAMS + OFF_W3 + k * H2 + n]; break;
             case WP_W2B: e = r / H1; n = r % H1; k = c;          // B(n,k) = W2[k][n]
                 v = blob[(size_t)(e * NSP + s) * NET_PARAMS + OFF_W2 + k * H1 + n]; break;
-            default: n = r; e = c / H1; k = c % H1;              // WP_W1B: B(n, e*256+j) = W1_e[j][n]
-                if (n < AEV_DIM) v = blob[(size_t)(e * NSP + s) * NET_PARAMS + OFF_W1 + (size_t)k * AEV_DIM + n]; break;
+            default: n = col2feat(r); e = c / H1; k = c % H1;    // WP_W1B: B(n, e*256+j) = W1_e[j][feature of column n]
+                if (n >= 0) v = blob[(size_t)(e * NSP + s) * NET_PARAMS + OFF_W1 + (size_t)k * AEV_DIM + n]; break;
         }
         __half hi, lo;
         split_half(v * W_SCALE, hi, lo);
@@ -476,10 +613,10 @@ bool make_map(CUtensorMap* m, const void* ptr, uint64_t rows, uint64_t cols, uin
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-struct TcWorkspace {                  // activations, per context
-    __half *aev, *h1, *h2, *d3, *d2, *d1;          // [2][max_rows][width]
-    CUtensorMap m_aev, m_h1, m_h2, m_d3, m_d2, m_d1;
-    int models;
+struct TcWorkspace {                  // per context
+    __half* aev;                                   // [2][max_rows][AEV_LD] row-major hi / lo planes (A of G1, via TMA)
+    __half *h1, *h2, *d3, *d2, *d1;                // tiled activation planes (see the header); d3 is padded to 192 per model
+    CUtensorMap m_aev;
 };
 struct TcWeights {                    // per weight handle
     __half *w1f, *w2f, *w3f, *w3b, *w2b, *w1b;
@@ -487,14 +624,14 @@ struct TcWeights {                    // per weight handle
     CUtensorMap m_w1f, m_w2f, m_w3f, m_w3b, m_w2b, m_w1b;
 };
 
-template <int EPI>
+template <int EPI, int CMP>
 int launch_gemm(Ctx* ctx, const CUtensorMap& a, const CUtensorMap& b, const TcArgs& args) {
     static bool attr = false;
     if (!attr) {
-        DHP_CUDA(ctx, cudaFuncSetAttribute(k_gemm_tc<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
+        DHP_CUDA(ctx, cudaFuncSetAttribute((k_gemm_tc<EPI, CMP>), cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
         attr = true;
     }
-    DHP_LAUNCH(ctx, k_gemm_tc<EPI>, ctx->sm_count, TC_THREADS, SMEM_BYTES, a, b, args);
+    DHP_LAUNCH(ctx, (k_gemm_tc<EPI, CMP>), ctx->sm_count, TC_THREADS, SMEM_BYTES, a, b, args);
     return DHP_OK;
 }
 
@@ -508,15 +645,13 @@ int mlp_tc_alloc(Ctx* ctx) {
     memset((void*)w, 0, sizeof(*w));
     ctx->tc_ws = w;
     const size_t R = (size_t)ctx->max_rows, M = MAX_MODELS;
-    struct { __half** p; size_t width; CUtensorMap* m; } bufs[] = {
-        {&w->aev, (size_t)AEV_LD, &w->m_aev}, {&w->h1, M * H1, &w->m_h1}, {&w->h2, M * H2, &w->m_h2},
-        {&w->d3, M * H3, &w->m_d3},           {&w->d2, M * H2, &w->m_d2}, {&w->d1, M * H1, &w->m_d1}};
+    struct { __half** p; size_t width; } bufs[] = {{&w->aev, (size_t)AEV_LD}, {&w->h1, M * H1}, {&w->h2, M * H2},
+                                                    {&w->d3, M * H2},          {&w->d2, M * H2}, {&w->d1, M * H1}};
     for (auto& b : bufs) {
         if (cudaMalloc((void**)b.p, 2 * R * b.width * sizeof(__half)) != cudaSuccess) return DHP_E_NOMEM;
         if (cudaMemset(*b.p, 0, 2 * R * b.width * sizeof(__half)) != cudaSuccess) return DHP_E_CUDA;
-        if (!make_map(b.m, *b.p, 2 * R, b.width, BM)) return DHP_E_CUDA;
     }
-    w->models = MAX_MODELS;
+    if (!make_map(&w->m_aev, w->aev, 2 * R, AEV_LD, BM)) return DHP_E_CUDA;
     return DHP_OK;
 }
 
@@ -538,7 +673,7 @@ int mlp_tc_weights(Ctx* ctx, Weights* wt) {
     struct { __half** p; int mode, rows, cols; CUtensorMap* m; uint32_t box_rows; } mats[] = {
         {&t->w1f, WP_W1F, M * H1, AEV_LD, &t->m_w1f, (uint32_t)H1}, {&t->w2f, WP_W2F, M * H2, H1, &t->m_w2f, (uint32_t)H2},
         {&t->w3f, WP_W3F, M * H3, H2, &t->m_w3f, (uint32_t)H3},     {&t->w3b, WP_W3B, M * H2, H3, &t->m_w3b, (uint32_t)H2},
-        {&t->w2b, WP_W2B, M * H1, H2, &t->m_w2b, (uint32_t)H1},     {&t->w1b, WP_W1B, AEV_LD, M * H1, &t->m_w1b, 256u}};
+        {&t->w2b, WP_W2B, M * H1, H2, &t->m_w2b, (uint32_t)H1},     {&t->w1b, WP_W1B, AEV_LD, M * H1, &t->m_w1b, (uint32_t)KBLK}};
     for (auto& m : mats) {
         const size_t n = (size_t)2 * NSP * m.rows * m.cols;
         if (cudaMalloc((void**)m.p, n * sizeof(__half)) != cudaSuccess) return DHP_E_NOMEM;
@@ -572,45 +707,51 @@ int mlp_tc(Ctx* ctx, const Weights* wt) {
     const int M = wt->n_models;
     const int R = (int)ctx->max_rows;
     int rc;
-    // activation maps depend on the ensemble size through the row pitch
-    if (ws->models != M) {
-        struct { __half* p; size_t width; CUtensorMap* m; } bufs[] = {
-            {ws->h1, (size_t)M * H1, &ws->m_h1}, {ws->h2, (size_t)M * H2, &ws->m_h2}, {ws->d3, (size_t)M * H3, &ws->m_d3},
-            {ws->d2, (size_t)M * H2, &ws->m_d2}, {ws->d1, (size_t)M * H1, &ws->m_d1}};
-        for (auto& b : bufs) if (!make_map(b.m, b.p, (uint64_t)2 * R, b.width, BM)) return DHP_E_CUDA;
-        ws->models = M;
-    }
     DHP_CUDA(ctx, cudaMemsetAsync(ctx->e_atom, 0, sizeof(float) * ctx->max_rows, ctx->stream));
+    DHP_CUDA(ctx, cudaMemsetAsync(ctx->tc_sched, 0, sizeof(int) * 8, ctx->stream));
     DHP_LAUNCH(ctx, k_split_rows, 4 * ctx->sm_count, 256, 0, ctx->aev, AEV_LD, ctx->sp_start, AEV_LD, ws->aev, R);
 
     TcArgs a{};
     a.row_species = ctx->row_species; a.sp_start = ctx->sp_start; a.alpha = ctx->params.celu_alpha;
-    a.inv_models = 1.0f / (float)M; a.a_plane_rows = R; a.out_plane_rows = R; a.e_atom = ctx->e_atom;
-    a.w4 = t->w4; a.b4 = t->b4;
-    // G1
+    a.inv_models = 1.0f / (float)M; a.a_plane_rows = R; a.plane_tiles = R / BM; a.e_atom = ctx->e_atom;
+    a.w4 = t->w4; a.b4 = t->b4; a.tile_mask = ctx->tile_mask;
+    const int KB1 = H1 / BK, KB2 = H2 / BK;         // 64-column blocks per model: 4 (h1, d1), 3 (h2, d2, and d3 padded to 192)
+    // G1: AEV rows (row-major, TMA) -> h1
     a.K = AEV_LD; a.BN = H1; a.n_tiles = M; a.a_k_off_per_tile = 0; a.b_rows_per_species = M * H1; a.b_rows_per_tile = H1;
-    a.acc_scale = 1.0f / W_SCALE; a.bias = t->b1; a.out_planes = ws->h1; a.out_ld = M * H1;
-    if ((rc = launch_gemm<EPI_CELU>(ctx, ws->m_aev, t->m_w1f, a)) != DHP_OK) return rc;
-    // G2
-    a.K = H1; a.BN = H2; a.a_k_off_per_tile = H1; a.b_rows_per_species = M * H2; a.b_rows_per_tile = H2;
-    a.bias = t->b2; a.out_planes = ws->h2; a.out_ld = M * H2;
-    if ((rc = launch_gemm<EPI_CELU>(ctx, ws->m_h1, t->m_w2f, a)) != DHP_OK) return rc;
-    // G3 + output layer + seed of the backward pass
-    a.K = H2; a.BN = H3; a.a_k_off_per_tile = H2; a.b_rows_per_species = M * H3; a.b_rows_per_tile = H3;
-    a.bias = t->b3; a.out_planes = ws->d3; a.out_ld = M * H3;
-    if ((rc = launch_gemm<EPI_OUT>(ctx, ws->m_h2, t->m_w3f, a)) != DHP_OK) return rc;
-    // B3
-    a.K = H3; a.BN = H2; a.a_k_off_per_tile = H3; a.b_rows_per_species = M * H2; a.b_rows_per_tile = H2;
-    a.h_planes = ws->h2; a.out_planes = ws->d2; a.out_ld = M * H2;
-    if ((rc = launch_gemm<EPI_DCELU>(ctx, ws->m_d3, t->m_w3b, a)) != DHP_OK) return rc;
-    // B2
-    a.K = H2; a.BN = H1; a.a_k_off_per_tile = H2; a.b_rows_per_species = M * H1; a.b_rows_per_tile = H1;
-    a.h_planes = ws->h1; a.out_planes = ws->d1; a.out_ld = M * H1;
-    if ((rc = launch_gemm<EPI_DCELU>(ctx, ws->m_d2, t->m_w2b, a)) != DHP_OK) return rc;
-    // B1
-    a.K = M * H1; a.BN = 256; a.n_tiles = AEV_LD / 256; a.a_k_off_per_tile = 0; a.b_rows_per_species = AEV_LD; a.b_rows_per_tile = 256;
+    a.acc_scale = 1.0f / W_SCALE; a.bias = t->b1;
+    a.a_tiled = nullptr; a.out_planes = ws->h1; a.out_kblocks = M * KB1; a.out_cols_per_tile = H1;
+    a.sched = ctx->tc_sched + 0;
+    if ((rc = launch_gemm<EPI_CELU, CMP_K>(ctx, ws->m_aev, t->m_w1f, a)) != DHP_OK) return rc;
+    // G2: h1 -> h2
+    a.K = H1; a.BN = H2; a.b_rows_per_species = M * H2; a.b_rows_per_tile = H2; a.bias = t->b2;
+    a.a_tiled = ws->h1; a.a_kblocks = M * KB1; a.a_kb_per_tile = KB1;
+    a.out_planes = ws->h2; a.out_kblocks = M * KB2; a.out_cols_per_tile = H2;
+    a.sched = ctx->tc_sched + 1;
+    if ((rc = launch_gemm<EPI_CELU, CMP_NONE>(ctx, ws->m_aev, t->m_w2f, a)) != DHP_OK) return rc;
+    // G3 + output layer + seed of the backward pass: h2 -> d3
+    a.K = H2; a.BN = H3; a.b_rows_per_species = M * H3; a.b_rows_per_tile = H3; a.bias = t->b3;
+    a.a_tiled = ws->h2; a.a_kblocks = M * KB2; a.a_kb_per_tile = KB2;
+    a.out_planes = ws->d3; a.out_kblocks = M * KB2; a.out_cols_per_tile = H2;
+    a.sched = ctx->tc_sched + 2;
+    if ((rc = launch_gemm<EPI_OUT, CMP_NONE>(ctx, ws->m_aev, t->m_w3f, a)) != DHP_OK) return rc;
+    // B3: d3 -> d2
+    a.K = H3; a.BN = H2; a.b_rows_per_species = M * H2; a.b_rows_per_tile = H2;
+    a.a_tiled = ws->d3; a.a_kblocks = M * KB2; a.a_kb_per_tile = KB2;
+    a.h_planes = ws->h2; a.out_planes = ws->d2; a.out_kblocks = M * KB2; a.out_cols_per_tile = H2;
+    a.sched = ctx->tc_sched + 3;
+    if ((rc = launch_gemm<EPI_DCELU, CMP_NONE>(ctx, ws->m_aev, t->m_w3b, a)) != DHP_OK) return rc;
+    // B2: d2 -> d1
+    a.K = H2; a.BN = H1; a.b_rows_per_species = M * H1; a.b_rows_per_tile = H1;
+    a.a_tiled = ws->d2; a.a_kblocks = M * KB2; a.a_kb_per_tile = KB2;
+    a.h_planes = ws->h1; a.out_planes = ws->d1; a.out_kblocks = M * KB1; a.out_cols_per_tile = H1;
+    a.sched = ctx->tc_sched + 4;
+    if ((rc = launch_gemm<EPI_DCELU, CMP_NONE>(ctx, ws->m_aev, t->m_w2b, a)) != DHP_OK) return rc;
+    // B1: d1 (all models along K) -> dE/dAEV, only the feature blocks that are active for the row tile
+    a.K = M * H1; a.BN = 256; a.n_tiles = AEV_LD / 256; a.b_rows_per_species = AEV_LD; a.b_rows_per_tile = 256;
+    a.a_tiled = ws->d1; a.a_kblocks = M * KB1; a.a_kb_per_tile = 0;
     a.acc_scale = 1.0f / (W_SCALE * D_SCALE); a.out_f32 = ctx->grad; a.out_ld = AEV_LD;
-    if ((rc = launch_gemm<EPI_GRAD>(ctx, ws->m_d1, t->m_w1b, a)) != DHP_OK) return rc;
+    a.sched = ctx->tc_sched + 5;
+    if ((rc = launch_gemm<EPI_GRAD, CMP_N>(ctx, ws->m_aev, t->m_w1b, a)) != DHP_OK) return rc;
     DHP_CUDA(ctx, cudaGetLastError());
     return DHP_OK;
 }

@@ -495,7 +495,7 @@ constexpr int MAX_STRIDE_CHUNKS = 6;    // tmp_stride <= 192
 __global__ void __launch_bounds__(P2_THREADS)
 k_rows(const unsigned* __restrict__ tmp, int stride, const int* __restrict__ cnt, const int* __restrict__ blk_off, int nblk,
        int n, int* __restrict__ row_ptr, int* __restrict__ col, int* __restrict__ n_rad, int* __restrict__ n_ang,
-       unsigned short* __restrict__ seg_cnt) {
+       unsigned short* __restrict__ seg_cnt, const int* __restrict__ rowmap, unsigned* __restrict__ tile_mask) {
     __shared__ int wsum[ROWS_PER_BLK / 32];
     __shared__ int rstart[ROWS_PER_BLK];
     __shared__ int segs[P2_THREADS / 32][16];
@@ -552,6 +552,21 @@ k_rows(const unsigned* __restrict__ tmp, int stride, const int* __restrict__ cnt
         // lane k < 16 owns key k: exclusive prefix over keys -> segment starts
         int cnt_k = lane < 16 ? sg[lane] : 0;
         if (lane == 15 || lane == 7) cnt_k = 0;
+        {   // which 64-wide feature blocks of this row's AEV can be non-zero (internal column order, dhp_internal.cuh)
+            const unsigned has1 = __ballot_sync(0xffffffffu, cnt_k > 0), has2 = __ballot_sync(0xffffffffu, cnt_k > 1);
+            const unsigned am = has1 & 0x7fu, am2 = has2 & 0x7fu, rm = (am | (has1 >> 8)) & 0x7fu;
+            bool pp = false;
+            if (lane < NPAIR) {                                   // lane = internal pair index
+                int hi = 0;
+                while ((hi + 1) * (hi + 2) / 2 <= lane) ++hi;
+                const int sa = prio_sp(lane - hi * (hi + 1) / 2), sb = prio_sp(hi);
+                pp = (sa == sb) ? ((am2 >> sa) & 1u) != 0 : (((am >> sa) & (am >> sb)) & 1u) != 0;
+            }
+            const unsigned pm = __ballot_sync(0xffffffffu, pp);
+            const bool bb = lane < 14 ? ((pm >> (2 * lane)) & 3u) != 0 : lane == 14 ? (rm & 0x0fu) != 0 : lane == 15 ? (rm & 0x70u) != 0 : false;
+            const unsigned bmask = __ballot_sync(0xffffffffu, bb);
+            if (lane == 0 && bmask) atomicOr(&tile_mask[rowmap[i] / ROW_TILE], bmask);
+        }
         int x = cnt_k;
 #pragma unroll
         for (int o = 1; o < 16; o <<= 1) {
@@ -604,6 +619,7 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
     DHP_CUDA(ctx, cudaMemsetAsync(ctx->cell_fill, 0, sizeof(int) * ctx->max_cells, st));
     DHP_CUDA(ctx, cudaMemsetAsync(ctx->row_slot, 0xFF, sizeof(int) * ctx->max_rows, st));
     DHP_CUDA(ctx, cudaMemsetAsync(ctx->row_species, 0xFF, sizeof(int) * ctx->max_rows, st));
+    DHP_CUDA(ctx, cudaMemsetAsync(ctx->tile_mask, 0, sizeof(unsigned) * (ctx->max_rows / ROW_TILE), st));
     if (n == 0) {
         DHP_CUDA(ctx, cudaMemsetAsync(ctx->row_ptr, 0, sizeof(int), st));
         DHP_CUDA(ctx, cudaMemsetAsync(ctx->sp_count, 0, sizeof(int) * 8, st));
@@ -658,7 +674,7 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
                    ctx->tmp_stride, ctx->n_rad, ctx->tmp_col, ctx->blk_sum, ctx->status);
     DHP_LAUNCH(ctx, k_scan_blocks, 1, 1024, 0, ctx->blk_sum, ctx->blk_off, nblk, ctx->pair_cap, ctx->status);
     DHP_LAUNCH(ctx, k_rows, nblk, P2_THREADS, 0, ctx->tmp_col, ctx->tmp_stride, ctx->n_rad, ctx->blk_off, nblk, n, ctx->row_ptr,
-               ctx->col, ctx->n_rad, ctx->n_ang, ctx->seg_cnt);
+               ctx->col, ctx->n_rad, ctx->n_ang, ctx->seg_cnt, ctx->rowmap, ctx->tile_mask);
     DHP_CUDA(ctx, cudaGetLastError());
     return DHP_OK;
 }

@@ -142,8 +142,12 @@ def test_energy_forces_small(torch, B, params, blob8, name, mode):
     assert np.max(np.abs(G - Go)) <= AEV_TOL
     Ea, _, go = oracle.energy_forces(s.pos, s.species, s.box, params, blob8[: s.n_models * 7 * W.PARAMS_PER_NET],
                                      s.n_models, mol_offsets=s.mol_offsets, want_dEdG=True)
+    # dE/dG is produced only for the 64-wide feature blocks that are non-zero somewhere in the atom's 128-row tile
+    # (the others multiply identically-zero dG/dr and are skipped; the export reads them as 0)
     g = d.dhp_debug_grad().cpu().numpy()
-    assert np.max(np.abs(g - go)) <= GRAD_TOL
+    close = np.abs(g - go) <= GRAD_TOL
+    assert np.all(close | ((g == 0) & (Go == 0)))
+    assert np.all(close[Go != 0])
     ea = d.dhp_debug_atomic_energy().cpu().numpy()
     assert np.max(np.abs(ea - Ea)) <= 2e-5
     # properties
