@@ -19,7 +19,7 @@
 
 namespace dhp {
 
-constexpr int AEV_WARPS = 4;
+constexpr int BWD_WARPS = 4;
 constexpr int GP = 36;   // pitch of one 32-float angular block of the staged gradient row (bank spread, 16 B aligned)
 
 __device__ __forceinline__ float fast_exp2(float x) { return exp2f(x); }     // ex2.approx under -use_fast_math
@@ -35,7 +35,7 @@ __device__ __forceinline__ NbrGeom neighbour_geom(const float4& pi, const float4
     double d[3] = {(double)pj.x - (double)pi.x, (double)pj.y - (double)pi.y, (double)pj.z - (double)pi.z};
     if (g.periodic) {
 #pragma unroll
-        for (int c = 0; c < 3; ++c) d[c] -= g.L[c] * rint(d[c] / g.L[c]);
+        for (int c = 0; c < 3; ++c) d[c] -= g.L[c] * rint(d[c] * g.inv_L[c]);   // listed pairs are far from the half-box tie
     }
     float x = (float)d[0], y = (float)d[1], z = (float)d[2];
     float r2 = x * x + y * y + z * z;
@@ -52,20 +52,48 @@ __device__ __forceinline__ NbrGeom neighbour_geom(const float4& pi, const float4
 __device__ __forceinline__ float fcut(float R, float inv_rc) { return 0.5f * cospif(R * inv_rc) + 0.5f; }
 __device__ __forceinline__ float dfcut(float R, float inv_rc, float pi_over_rc) { return -0.5f * pi_over_rc * sinpif(R * inv_rc); }
 
-struct WarpSmemFwd {
-    float rad[2][AEV_RAD];
-    float ang[AEV_ANG];
-    float ux[MAX_ANG], uy[MAX_ANG], uz[MAX_ANG], R[MAX_ANG], fc[MAX_ANG];
-    int sp[MAX_ANG];
-    float4 tA[32];
-    float4 tB[32][2];
-    int tp[32];
+// ---- forward ---------------------------------------------------------------------------------------
+// Row i of the pair list is ordered [angular, species 0..6][radial-only, species 0..6] (nlist.cu), seg_cnt holds
+// the 14 run lengths.  The kernel uses that order twice:
+//   radial   lane = (shift m, parity h): a register sum over the two runs of each neighbour species;
+//   angular  triplets are enumerated species pair by species pair (internal pair index p = angular block p of
+//            the row), each pair padded to a multiple of 4 slots.  A round of 32 slots:
+//              phase 1  lane <-> slot: geometry, 4 angular factors, 8 radial Gaussians -> staged [factor][slot];
+//              phase 2  lane <-> feature (a,z): sum over the slots of each pair present in the round with
+//                       16-byte broadcast reads (2 per 4 triplets), the sum carried in a register until the
+//                       pair ends, then stored once to the row buffer (no read-modify-write, no atomics).
+// Output: PLANES = false, full fp32 rows (SIMT MLP path); PLANES = true, the two-term fp16 split of the
+// feature blocks that are active for the row's tile (what G1 reads), written straight into the tensor path's planes.
+constexpr int AEV_WARPS = 8;
+constexpr int MAX_RAD = 192;    // radial neighbours staged per centre (= the pair list's per-row capacity)
+
+__constant__ unsigned char c_pair_sp[NPAIR];    // internal pair p -> species a | species b << 4
+
+constexpr int TP = 36;          // pitch of the staged factor rows: 16-byte aligned, rows 4 banks apart (conflict-free float4 reads)
+
+struct __align__(16) WarpSmemFwd {
+    float4 nb[MAX_ANG];          // ux, uy, uz, R of the angular neighbours
+    float fca[MAX_ANG];          // f_c(R; Rca)
+    float2 rr[MAX_RAD];          // all neighbours: R, f_c(R; Rcr)
+    float tA[NZ][TP];
+    float tB[NA][TP];
+    int4 tab[NPAIR + 1];         // non-empty species pairs in slot order: first slot, j0 | k0 << 8 | nk << 16 | same << 24,
+                                 // triplets, angular block; terminated by {total slots, ...}
+    float row[AEV_LD];           // the finished row in the internal column order
 };
 
+__device__ __forceinline__ uint32_t cvt_pack_h2(float lo_half, float hi_half) {
+    uint32_t r;
+    asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi_half), "f"(lo_half));
+    return r;
+}
+
+template <bool PLANES>
 __global__ void __launch_bounds__(AEV_WARPS * 32)
 k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, const int* __restrict__ col,
-          const int* __restrict__ n_ang, const int* __restrict__ rowmap, const Grid* __restrict__ gp,
-          const __grid_constant__ AevConst K, int n, float* __restrict__ aev, int* __restrict__ status) {
+          const unsigned short* __restrict__ seg_cnt, const int* __restrict__ rowmap, const unsigned* __restrict__ tile_mask,
+          const Grid* __restrict__ gp, const __grid_constant__ AevConst K, int n, float* __restrict__ aev,
+          __half* __restrict__ planes, size_t plane_stride, int* __restrict__ status) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ Grid g;
     if (threadIdx.x == 0) g = *gp;
@@ -74,100 +102,181 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
     const int i = blockIdx.x * AEV_WARPS + w;
     if (i >= n) return;
     WarpSmemFwd& S = reinterpret_cast<WarpSmemFwd*>(smem_raw)[w];
+    const unsigned FULL = 0xffffffffu;
+    const unsigned lt = (1u << lane) - 1u;
 
-    for (int c = lane; c < 2 * AEV_RAD; c += 32) (&S.rad[0][0])[c] = 0.f;
-    for (int c = lane; c < AEV_ANG; c += 32) S.ang[c] = 0.f;
-    __syncwarp();
+    for (int c = lane; c < AEV_LD / 4; c += 32) reinterpret_cast<float4*>(S.row)[c] = make_float4(0.f, 0.f, 0.f, 0.f);
 
+    // run lengths of the row: lane k < 7 angular species k, 8 <= k < 15 radial-only species k - 8
+    int cnt = (lane < 16 && lane != 7 && lane != 15) ? (int)seg_cnt[(size_t)i * 16 + lane] : 0;
+    int start = cnt;                                   // exclusive prefix over lanes = first slot of the run
+#pragma unroll
+    for (int o = 1; o < 16; o <<= 1) {
+        int y = __shfl_up_sync(FULL, start, o);
+        if (lane >= o) start += y;
+    }
+    start -= cnt;
+    const int na = __shfl_sync(FULL, start, 8);        // angular neighbours = first slot of the radial-only class
+    const int ntot = __shfl_sync(FULL, start, 15);
+    if (na > MAX_ANG || ntot > MAX_RAD) {              // capacity: report it and produce a zero row
+        if (lane == 0) atomicExch(status, DHP_E_CAPACITY);
+        cnt = 0;
+    }
+    const int nst = (na > MAX_ANG || ntot > MAX_RAD) ? 0 : ntot;
+    const int rb = row_ptr[i];
     const float4 pi = spos[i];
-    const int rb = row_ptr[i], re = row_ptr[i + 1];
-    int na = n_ang[i];
-    if (na > MAX_ANG) { if (lane == 0) atomicExch(status, DHP_E_CAPACITY); na = MAX_ANG; }
     const float inv_rcr = 1.0f / K.rcr, inv_rca = 1.0f / K.rca;
-    const int m = lane & 15, half = lane >> 4;
-    const float shf = K.shf_r[m];
 
-    // ---- radial (Eq. 4) + staging of the angular neighbours --------------------------------------
-    for (int base = rb; base < re; base += 32) {
-        const int idx = base + lane;
-        NbrGeom q; q.R = 1.f; q.sp = 0; q.ux = q.uy = q.uz = 0.f;
-        float fc = 0.f;
-        if (idx < re) {
-            q = neighbour_geom(pi, spos[col[idx]], g);
-            fc = fcut(q.R, inv_rcr);
-            const int a = idx - rb;
-            if (a < na) {
-                S.ux[a] = q.ux; S.uy[a] = q.uy; S.uz[a] = q.uz; S.R[a] = q.R; S.sp[a] = q.sp;
-                S.fc[a] = fcut(q.R, inv_rca);
-            }
+    // ---- stage all neighbours -------------------------------------------------------------------------
+    for (int a = lane; a < nst; a += 32) {
+        const NbrGeom q = neighbour_geom(pi, spos[col[rb + a]], g);
+        S.rr[a] = make_float2(q.R, fcut(q.R, inv_rcr));
+        if (a < na) {
+            S.nb[a] = make_float4(q.ux, q.uy, q.uz, q.R);
+            S.fca[a] = fcut(q.R, inv_rca);
         }
-        const int cnt = min(32, re - base);
-        for (int t = 0; t < cnt; t += 2) {
-            const int src = t + half;
-            float Rq = __shfl_sync(0xffffffffu, q.R, src & 31);
-            float fq = __shfl_sync(0xffffffffu, fc, src & 31);
-            int sq = __shfl_sync(0xffffffffu, q.sp, src & 31);
-            if (src < cnt) {
-                float dr = Rq - shf;
-                S.rad[half][NR * sq + m] += fast_exp2(-K.eta_r_l2e * dr * dr) * fq;
-            }
+    }
+
+    // ---- table of the non-empty species pairs (lane p < 28: internal pair p = angular block p) -------------
+    int T_pad;
+    {
+        int psa = 0, psb = 0, pcount = 0;
+        if (lane < NPAIR) { const int e = c_pair_sp[lane]; psa = e & 15; psb = e >> 4; }
+        const int ca = __shfl_sync(FULL, cnt, psa), cb = __shfl_sync(FULL, cnt, psb);
+        const int ja0 = __shfl_sync(FULL, start, psa), kb0 = __shfl_sync(FULL, start, psb);
+        if (lane < NPAIR) pcount = (psa == psb) ? ca * (ca - 1) / 2 : ca * cb;
+        const int padded = (pcount + 3) & ~3;          // each pair padded to a multiple of 4 slots
+        int pstart = padded;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int y = __shfl_up_sync(FULL, pstart, o);
+            if (lane >= o) pstart += y;
         }
+        T_pad = __shfl_sync(FULL, pstart, 31);
+        pstart -= padded;
+        const unsigned nz = __ballot_sync(FULL, pcount > 0);
+        if (pcount > 0) S.tab[__popc(nz & lt)] = make_int4(pstart, ja0 | (kb0 << 8) | (cb << 16) | ((psa == psb) << 24), pcount, lane);
+        if (lane == 0) S.tab[__popc(nz)] = make_int4(T_pad, 0, 0, 0);
     }
     __syncwarp();
 
-    // ---- angular (Eq. 5) ---------------------------------------------------------------------------
-    const int npairs = na * (na - 1) / 2;
-    const float inv_na = na > 0 ? 1.0f / (float)na : 0.f;
-    const int za = lane & 3, aa = lane >> 2;
-    for (int T0 = 0; T0 < npairs; T0 += 32) {
-        const int T = T0 + lane;
-        if (T < npairs) {
-            int d = (int)(((float)T + 0.5f) * inv_na);
-            int j = T - d * na;
-            if (j < 0) { --d; j += na; } else if (j >= na) { ++d; j -= na; }
-            int k = j + d + 1;
-            if (k >= na) k -= na;
-            float ujx = S.ux[j], ujy = S.uy[j], ujz = S.uz[j];
-            float ukx = S.ux[k], uky = S.uy[k], ukz = S.uz[k];
-            float c = ujx * ukx + ujy * uky + ujz * ukz;
-            float cx = ujy * ukz - ujz * uky, cy = ujz * ukx - ujx * ukz, cz = ujx * uky - ujy * ukx;
-            float s = sqrtf(cx * cx + cy * cy + cz * cz);
-            float f2 = 2.0f * S.fc[j] * S.fc[k];
-            float Rm = 0.5f * (S.R[j] + S.R[k]);
-            float A[NZ];
-#pragma unroll
-            for (int z = 0; z < NZ; ++z) {
-                float u = fmaxf(0.5f * (1.0f + c * K.cos_z[z] + s * K.sin_z[z]), 0.f);
-                A[z] = f2 * fast_exp2(K.zeta * fast_log2(u));        // 2 ((1+cos(theta-theta_z))/2)^zeta f_j f_k
+    // ---- radial (Eq. 4): lane = (shift m, parity h), one register sum per neighbour species ----------------
+    {
+        const int m = lane & 15, h = lane >> 4;
+        const float shf = K.shf_r[m];
+        for (int s = 0; s < NSP; ++s) {
+            const int ca = __shfl_sync(FULL, cnt, s), sa = __shfl_sync(FULL, start, s);
+            const int cr = __shfl_sync(FULL, cnt, 8 + s), sr = __shfl_sync(FULL, start, 8 + s) - ca;
+            if (ca + cr == 0) continue;
+            float acc = 0.f;
+#pragma unroll 2
+            for (int x = h; x < ca + cr; x += 2) {
+                const float2 q = S.rr[x < ca ? sa + x : sr + x];
+                const float dr = q.x - shf;
+                acc = fmaf(fast_exp2(-K.eta_r_l2e * dr * dr), q.y, acc);
             }
-            float B[NA];
-#pragma unroll
-            for (int a = 0; a < NA; ++a) {
-                float mm = Rm - K.shf_a[a];
-                B[a] = fast_exp2(-K.eta_a_l2e * mm * mm);
-            }
-            S.tA[lane] = make_float4(A[0], A[1], A[2], A[3]);
-            S.tB[lane][0] = make_float4(B[0], B[1], B[2], B[3]);
-            S.tB[lane][1] = make_float4(B[4], B[5], B[6], B[7]);
-            S.tp[lane] = ipair(S.sp[j], S.sp[k]);
+            acc += __shfl_xor_sync(FULL, acc, 16);
+            if (lane < 16) S.row[rad_col(s) + m] = acc;
         }
+    }
+
+    // ---- angular (Eq. 5) ------------------------------------------------------------------------------
+    const int za = lane & 3, aa = lane >> 2;
+    float facc = 0.f;                                    // running sum of feature (aa, za) of the current pair
+    int e = 0;                                           // table entry of this lane's slot (monotonic over the rounds)
+    for (int T0 = 0; T0 < T_pad; T0 += 32) {
+        const int t = T0 + lane;
+        float A[NZ] = {0.f, 0.f, 0.f, 0.f};
+        float B[NA] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        if (t < T_pad) {
+            while (t >= S.tab[e + 1].x) ++e;
+            const int4 E = S.tab[e];
+            const int u = t - E.x;
+            if (u < E.z) {
+                // u -> (x, y) with u = x nk + y.  Different species: j = j0 + x, k = k0 + y.  Same species: distance
+                // enumeration of the unordered pairs of nk items (d = x, j = y, k = y + d + 1 mod nk), each pair once.
+                const int j0 = E.y & 255, k0 = (E.y >> 8) & 255, nk = (E.y >> 16) & 255;
+                int x = (int)(((float)u + 0.5f) * __frcp_rn((float)nk));
+                int y = u - x * nk;
+                if (y < 0) { --x; y += nk; } else if (y >= nk) { ++x; y -= nk; }
+                int j, k;
+                if (!(E.y >> 24)) { j = j0 + x; k = k0 + y; }
+                else { j = j0 + y; k = y + x + 1; if (k >= nk) k -= nk; k += j0; }
+                const float4 qj = S.nb[j], qk = S.nb[k];
+                const float c = qj.x * qk.x + qj.y * qk.y + qj.z * qk.z;
+                const float cx = qj.y * qk.z - qj.z * qk.y, cy = qj.z * qk.x - qj.x * qk.z, cz = qj.x * qk.y - qj.y * qk.x;
+                const float sn = sqrtf(cx * cx + cy * cy + cz * cz);
+                const float f2 = 2.0f * S.fca[j] * S.fca[k];
+                const float Rm = 0.5f * (qj.w + qk.w);
+#pragma unroll
+                for (int z = 0; z < NZ; ++z) {
+                    const float uu = fmaxf(fmaf(0.5f * K.sin_z[z], sn, fmaf(0.5f * K.cos_z[z], c, 0.5f)), 0.f);
+                    A[z] = f2 * fast_exp2(K.zeta * fast_log2(uu));    // 2 ((1+cos(theta-theta_z))/2)^zeta f_j f_k
+                }
+#pragma unroll
+                for (int a = 0; a < NA; ++a) {
+                    const float mm = Rm - K.shf_a[a];
+                    B[a] = fast_exp2(-K.eta_a_l2e * mm * mm);
+                }
+            }
+        }
+#pragma unroll
+        for (int z = 0; z < NZ; ++z) S.tA[z][lane] = A[z];
+#pragma unroll
+        for (int a = 0; a < NA; ++a) S.tB[a][lane] = B[a];
         __syncwarp();
-        const int cnt = min(32, npairs - T0);
-        const float* tA = reinterpret_cast<const float*>(S.tA);
-        const float* tB = reinterpret_cast<const float*>(S.tB);
-        for (int t = 0; t < cnt; ++t) {
-            float v = tA[4 * t + za] * tB[8 * t + aa];
-            S.ang[32 * S.tp[t] + lane] += v;                        // lane == 4*aa + za: layout [a][z]
+        // phase 2: the pairs present in this round, in order
+        const int e_first = __shfl_sync(FULL, e, 0);
+        const int e_last = __shfl_sync(FULL, e, (T0 + 31 < T_pad) ? 31 : (T_pad - 1 - T0));
+        for (int ee = e_first; ee <= e_last; ++ee) {
+            const int s0 = S.tab[ee].x, s1 = S.tab[ee + 1].x;
+            const int lo = max(s0, T0) - T0, hi = min(s1, T0 + 32) - T0;
+#pragma unroll 2
+            for (int q = lo; q < hi; q += 4) {
+                const float4 a4 = *reinterpret_cast<const float4*>(&S.tA[za][q]);
+                const float4 b4 = *reinterpret_cast<const float4*>(&S.tB[aa][q]);
+                facc = fmaf(a4.x, b4.x, facc); facc = fmaf(a4.y, b4.y, facc);
+                facc = fmaf(a4.z, b4.z, facc); facc = fmaf(a4.w, b4.w, facc);
+            }
+            if (s1 <= T0 + 32) { S.row[32 * S.tab[ee].w + lane] = facc; facc = 0.f; }   // pair complete
         }
         __syncwarp();
     }
+    __syncwarp();
 
-    // ---- write the row (species-grouped row order) -------------------------------------------------
-    float* out = aev + (size_t)rowmap[i] * AEV_LD;
-    // internal column order (dhp_internal.cuh): angular blocks by ipair(), radial blocks by species priority, zeros
-    for (int c = lane; c < AEV_ANG; c += 32) out[c] = S.ang[c];
-    for (int c = lane; c < AEV_RAD; c += 32) out[rad_col(c >> 4) + (c & 15)] = S.rad[0][c] + S.rad[1][c];
-    if (lane < AEV_LD - AEV_DIM) out[AEV_DIM + lane] = 0.f;
+    // ---- write the row (species-grouped row order) -----------------------------------------------------
+    const int row = rowmap[i];
+    if (!PLANES) {
+        float4* out = reinterpret_cast<float4*>(aev + (size_t)row * AEV_LD);
+        for (int c = lane; c < AEV_LD / 4; c += 32) out[c] = reinterpret_cast<const float4*>(S.row)[c];
+    } else {
+        unsigned mask = tile_mask[row / ROW_TILE];
+        if (mask == 0) mask = 1u << 14;                  // G1 runs one block of zeros for an all-zero tile
+        const int half16 = lane >> 4, plane = (lane >> 3) & 1, grp = lane & 7;
+        while (mask) {                                   // two blocks per pass: lanes 0-15 / 16-31, hi and lo 8 lanes each
+            const int b0 = __ffs(mask) - 1; mask &= mask - 1u;
+            int b1 = -1;
+            if (mask) { b1 = __ffs(mask) - 1; mask &= mask - 1u; }
+            const int b = half16 ? b1 : b0;
+            if (b >= 0) {
+                const float4 v0 = *reinterpret_cast<const float4*>(&S.row[KBLK * b + 8 * grp]);
+                const float4 v1 = *reinterpret_cast<const float4*>(&S.row[KBLK * b + 8 * grp + 4]);
+                const float x[8] = {v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w};
+                uint32_t o[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const uint32_t hi = cvt_pack_h2(x[2 * q], x[2 * q + 1]);
+                    if (plane == 0) o[q] = hi;
+                    else {
+                        const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&hi));
+                        o[q] = cvt_pack_h2(x[2 * q] - f.x, x[2 * q + 1] - f.y);
+                    }
+                }
+                *reinterpret_cast<uint4*>(planes + (size_t)plane * plane_stride + (size_t)row * AEV_LD + KBLK * b + 8 * grp) =
+                    make_uint4(o[0], o[1], o[2], o[3]);
+            }
+        }
+    }
 }
 
 // -------------------------------------------------------------------------------------------------
@@ -181,7 +290,7 @@ struct WarpSmemBwd {
     int sp[MAX_ANG];
 };
 
-__global__ void __launch_bounds__(AEV_WARPS * 32)
+__global__ void __launch_bounds__(BWD_WARPS * 32)
 k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, const int* __restrict__ col,
           const int* __restrict__ n_ang, const int* __restrict__ rowmap, const Grid* __restrict__ gp,
           const __grid_constant__ AevConst K, int n, const float* __restrict__ grad, float* __restrict__ fsorted) {
@@ -190,7 +299,7 @@ k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
     if (threadIdx.x == 0) g = *gp;
     __syncthreads();
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int i = blockIdx.x * AEV_WARPS + w;
+    const int i = blockIdx.x * BWD_WARPS + w;
     if (i >= n) return;
     WarpSmemBwd& S = reinterpret_cast<WarpSmemBwd*>(smem_raw)[w];
 
@@ -340,17 +449,29 @@ __global__ void k_energy_reduce(const float* __restrict__ e_atom, const int* __r
 }
 
 // -------------------------------------------------------------------------------------------------
-int aev_forward(Ctx* ctx) {
+int aev_forward(Ctx* ctx, bool planes) {
     const int n = (int)ctx->n_atoms;
+    ctx->aev_in_planes = planes;
     if (n == 0) return DHP_OK;
-    static bool attr_set = false;
+    static bool init = false;
     const size_t smem = sizeof(WarpSmemFwd) * AEV_WARPS;
-    if (!attr_set) {
-        DHP_CUDA(ctx, cudaFuncSetAttribute(k_aev_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
+    if (!init) {
+        DHP_CUDA(ctx, cudaFuncSetAttribute(k_aev_fwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        DHP_CUDA(ctx, cudaFuncSetAttribute(k_aev_fwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        unsigned char tab[NPAIR];
+        for (int hi = 0, p = 0; hi < NSP; ++hi)
+            for (int lo = 0; lo <= hi; ++lo, ++p) tab[p] = (unsigned char)(prio_sp(lo) | (prio_sp(hi) << 4));
+        DHP_CUDA(ctx, cudaMemcpyToSymbol(c_pair_sp, tab, sizeof(tab)));
+        init = true;
     }
-    DHP_LAUNCH(ctx, k_aev_fwd, (n + AEV_WARPS - 1) / AEV_WARPS, AEV_WARPS * 32, smem, ctx->spos, ctx->row_ptr, ctx->col,
-               ctx->n_ang, ctx->rowmap, ctx->grid, ctx->aevc, n, ctx->aev, ctx->status);
+    const int blocks = (n + AEV_WARPS - 1) / AEV_WARPS;
+    const size_t plane_stride = (size_t)ctx->max_rows * AEV_LD;
+    if (planes)
+        DHP_LAUNCH(ctx, k_aev_fwd<true>, blocks, AEV_WARPS * 32, smem, ctx->spos, ctx->row_ptr, ctx->col, ctx->seg_cnt, ctx->rowmap,
+                   ctx->tile_mask, ctx->grid, ctx->aevc, n, ctx->aev, ctx->aev_planes, plane_stride, ctx->status);
+    else
+        DHP_LAUNCH(ctx, k_aev_fwd<false>, blocks, AEV_WARPS * 32, smem, ctx->spos, ctx->row_ptr, ctx->col, ctx->seg_cnt, ctx->rowmap,
+                   ctx->tile_mask, ctx->grid, ctx->aevc, n, ctx->aev, ctx->aev_planes, plane_stride, ctx->status);
     DHP_CUDA(ctx, cudaGetLastError());
     return DHP_OK;
 }
@@ -359,13 +480,13 @@ int aev_backward(Ctx* ctx, float* F_out) {
     const int n = (int)ctx->n_atoms;
     if (n == 0) return DHP_OK;
     static bool attr_set = false;
-    const size_t smem = sizeof(WarpSmemBwd) * AEV_WARPS;
+    const size_t smem = sizeof(WarpSmemBwd) * BWD_WARPS;
     if (!attr_set) {
         DHP_CUDA(ctx, cudaFuncSetAttribute(k_aev_bwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
     }
     DHP_CUDA(ctx, cudaMemsetAsync(ctx->fsorted, 0, sizeof(float) * 3 * n, ctx->stream));
-    DHP_LAUNCH(ctx, k_aev_bwd, (n + AEV_WARPS - 1) / AEV_WARPS, AEV_WARPS * 32, smem, ctx->spos, ctx->row_ptr, ctx->col,
+    DHP_LAUNCH(ctx, k_aev_bwd, (n + BWD_WARPS - 1) / BWD_WARPS, BWD_WARPS * 32, smem, ctx->spos, ctx->row_ptr, ctx->col,
                ctx->n_ang, ctx->rowmap, ctx->grid, ctx->aevc, n, ctx->grad, ctx->fsorted);
     DHP_LAUNCH(ctx, k_unsort_forces, (n + 255) / 256, 256, 0, ctx->fsorted, ctx->perm, n, F_out);
     DHP_CUDA(ctx, cudaGetLastError());

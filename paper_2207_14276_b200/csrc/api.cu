@@ -91,10 +91,10 @@ static int run_energy_forces(Ctx* ctx, const float* pos, const float* box, const
     prof_mark(ctx, slot, 0);
     if ((rc = nlist_build(ctx, pos, box, species, n, mol_offsets, n_mol)) != DHP_OK) return rc;
     prof_mark(ctx, slot, 1);
-    if ((rc = aev_forward(ctx)) != DHP_OK) return rc;
-    prof_mark(ctx, slot, 2);
     const bool tensor = ctx->mlp_mode == DHP_MLP_TENSOR || (ctx->mlp_mode == DHP_MLP_AUTO && w->tc != nullptr);
     if (tensor && !w->tc) return DHP_E_NOTIMPL;
+    if ((rc = aev_forward(ctx, tensor && ctx->aev_planes != nullptr)) != DHP_OK) return rc;
+    prof_mark(ctx, slot, 2);
     rc = tensor ? mlp_tc(ctx, w) : mlp_simt(ctx, w);
     if (rc != DHP_OK) return rc;
     if ((rc = energy_reduce(ctx, E)) != DHP_OK) return rc;
@@ -122,6 +122,19 @@ __global__ void k_gather_rows(const float* __restrict__ src, int ld_src, int nco
     const unsigned mask = tile_mask[row / ROW_TILE];
     for (int c = threadIdx.x; c < AEV_DIM; c += blockDim.x)
         dst[(size_t)a * ncol + col2feat[c]] = ((mask >> (c / KBLK)) & 1u) ? s[c] : 0.f;
+}
+// the same from the fp16 hi / lo planes the tensor path's forward pass writes (value = hi + lo)
+__global__ void k_gather_planes(const __half* __restrict__ planes, size_t plane_stride, const int* __restrict__ rowmap,
+                                const int* __restrict__ inv_perm, int n, const int* __restrict__ col2feat,
+                                const unsigned* __restrict__ tile_mask, float* __restrict__ dst) {
+    int a = blockIdx.x;
+    if (a >= n) return;
+    const int row = rowmap[inv_perm[a]];
+    const __half* hi = planes + (size_t)row * AEV_LD;
+    const __half* lo = hi + plane_stride;
+    const unsigned mask = tile_mask[row / ROW_TILE];
+    for (int c = threadIdx.x; c < AEV_DIM; c += blockDim.x)
+        dst[(size_t)a * AEV_DIM + col2feat[c]] = ((mask >> (c / KBLK)) & 1u) ? __half2float(hi[c]) + __half2float(lo[c]) : 0.f;
 }
 
 }  // namespace dhp
@@ -339,7 +352,18 @@ static int debug_gather(dhp_ctx* h, const float* src, int ld, int ncol, float* d
     DHP_CUDA(c, cudaStreamSynchronize(c->stream));
     return DHP_OK;
 }
-int dhp_debug_aev(dhp_ctx* h, float* aev) { return h ? debug_gather(h, h->c.aev, AEV_LD, AEV_DIM, aev, true) : DHP_E_BADARG; }
+int dhp_debug_aev(dhp_ctx* h, float* aev) {
+    if (!h || !aev) return DHP_E_BADARG;
+    Ctx* c = &h->c;
+    if (!c->aev_in_planes) return debug_gather(h, c->aev, AEV_LD, AEV_DIM, aev, true);
+    const int n = (int)c->n_atoms;
+    if (n == 0) return DHP_OK;
+    DHP_LAUNCH(c, k_gather_planes, n, 128, 0, c->aev_planes, (size_t)c->max_rows * AEV_LD, c->rowmap, c->inv_perm, n, c->col2feat,
+               c->tile_mask, aev);
+    DHP_CUDA(c, cudaGetLastError());
+    DHP_CUDA(c, cudaStreamSynchronize(c->stream));
+    return DHP_OK;
+}
 int dhp_debug_grad(dhp_ctx* h, float* grad) { return h ? debug_gather(h, h->c.grad, AEV_LD, AEV_DIM, grad, true) : DHP_E_BADARG; }
 int dhp_debug_atomic_energy(dhp_ctx* h, float* e) { return h ? debug_gather(h, h->c.e_atom, 1, 1, e, false) : DHP_E_BADARG; }
 

@@ -2,6 +2,7 @@
 // oracle under oracle/ shares nothing with this directory).
 #pragma once
 
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -134,6 +135,8 @@ struct Ctx {
     // host-call staging
     float* st_pos; int* st_species; int* st_mol; double* st_E; float* st_F;
     void* tc_ws;           // tensor-path workspace (mlp_tc.cu)
+    __half* aev_planes;    // [2][max_rows][AEV_LD] fp16 hi / lo planes of the AEV rows (owned by tc_ws), or null
+    bool aev_in_planes;    // the last forward pass wrote aev_planes (active blocks only) instead of aev
 };
 
 // ---- launch bookkeeping -------------------------------------------------------------------------
@@ -154,7 +157,7 @@ int cuda_fail(Ctx* ctx, cudaError_t e, const char* what);
 int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t* species, int64_t n,
                 const int32_t* mol_offsets, int64_t n_mol);
 int nlist_export(Ctx* ctx, int32_t* row_ptr, int32_t* col, bool angular);
-int aev_forward(Ctx* ctx);
+int aev_forward(Ctx* ctx, bool planes);   // planes: write the tensor path's fp16 hi/lo planes instead of fp32 rows
 int aev_backward(Ctx* ctx, float* F_out);
 int mlp_simt(Ctx* ctx, const Weights* w);
 int mlp_simt_alloc(Ctx* ctx);

@@ -652,6 +652,7 @@ int mlp_tc_alloc(Ctx* ctx) {
         if (cudaMemset(*b.p, 0, 2 * R * b.width * sizeof(__half)) != cudaSuccess) return DHP_E_CUDA;
     }
     if (!make_map(&w->m_aev, w->aev, 2 * R, AEV_LD, BM)) return DHP_E_CUDA;
+    ctx->aev_planes = w->aev;
     return DHP_OK;
 }
 
@@ -662,6 +663,7 @@ void mlp_tc_free(Ctx* ctx) {
     for (__half* p : ptrs) if (p) cudaFree(p);
     delete w;
     ctx->tc_ws = nullptr;
+    ctx->aev_planes = nullptr;
 }
 
 int mlp_tc_weights(Ctx* ctx, Weights* wt) {
@@ -709,7 +711,8 @@ int mlp_tc(Ctx* ctx, const Weights* wt) {
     int rc;
     DHP_CUDA(ctx, cudaMemsetAsync(ctx->e_atom, 0, sizeof(float) * ctx->max_rows, ctx->stream));
     DHP_CUDA(ctx, cudaMemsetAsync(ctx->tc_sched, 0, sizeof(int) * 8, ctx->stream));
-    DHP_LAUNCH(ctx, k_split_rows, 4 * ctx->sm_count, 256, 0, ctx->aev, AEV_LD, ctx->sp_start, AEV_LD, ws->aev, R);
+    if (!ctx->aev_in_planes)     // rows came from a forward pass in fp32 (debug / mixed use): split them here
+        DHP_LAUNCH(ctx, k_split_rows, 4 * ctx->sm_count, 256, 0, ctx->aev, AEV_LD, ctx->sp_start, AEV_LD, ws->aev, R);
 
     TcArgs a{};
     a.row_species = ctx->row_species; a.sp_start = ctx->sp_start; a.alpha = ctx->params.celu_alpha;
