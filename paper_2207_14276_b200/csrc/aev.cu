@@ -22,8 +22,11 @@ namespace dhp {
 constexpr int BWD_WARPS = 4;
 constexpr int GP = 36;   // pitch of one 32-float angular block of the staged gradient row (bank spread, 16 B aligned)
 
-__device__ __forceinline__ float fast_exp2(float x) { return exp2f(x); }     // ex2.approx under -use_fast_math
-__device__ __forceinline__ float fast_log2(float x) { return __log2f(x); }
+// single-instruction approximations (2^-22 relative error; inputs here are never denormal where it matters)
+__device__ __forceinline__ float fast_exp2(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float fast_log2(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float fast_sqrt(float x) { float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float fast_rcp(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
 struct NbrGeom {
     float ux, uy, uz, R;
@@ -79,13 +82,16 @@ struct __align__(16) WarpSmemFwd {
     float tB[NA][TP];
     int4 tab[NPAIR + 1];         // non-empty species pairs in slot order: first slot, j0 | k0 << 8 | nk << 16 | same << 24,
                                  // triplets, angular block; terminated by {total slots, ...}
-    float row[AEV_LD];           // the finished row in the internal column order
 };
 
-__device__ __forceinline__ uint32_t cvt_pack_h2(float lo_half, float hi_half) {
-    uint32_t r;
-    asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi_half), "f"(lo_half));
-    return r;
+// one feature value of this lane -> the row, either fp32 or as the two-term fp16 split in the hi / lo planes
+template <bool PLANES>
+__device__ __forceinline__ void put_feature(float v, float* __restrict__ row_f32, __half* __restrict__ row_hi,
+                                            size_t plane_stride, int colidx) {
+    if (!PLANES) { row_f32[colidx] = v; return; }
+    const __half hi = __float2half_rn(fminf(fmaxf(v, -65000.f), 65000.f));
+    row_hi[colidx] = hi;
+    row_hi[plane_stride + colidx] = __float2half_rn(v - __half2float(hi));
 }
 
 template <bool PLANES>
@@ -104,8 +110,6 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
     WarpSmemFwd& S = reinterpret_cast<WarpSmemFwd*>(smem_raw)[w];
     const unsigned FULL = 0xffffffffu;
     const unsigned lt = (1u << lane) - 1u;
-
-    for (int c = lane; c < AEV_LD / 4; c += 32) reinterpret_cast<float4*>(S.row)[c] = make_float4(0.f, 0.f, 0.f, 0.f);
 
     // run lengths of the row: lane k < 7 angular species k, 8 <= k < 15 radial-only species k - 8
     int cnt = (lane < 16 && lane != 7 && lane != 15) ? (int)seg_cnt[(size_t)i * 16 + lane] : 0;
@@ -126,6 +130,9 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
     const int rb = row_ptr[i];
     const float4 pi = spos[i];
     const float inv_rcr = 1.0f / K.rcr, inv_rca = 1.0f / K.rca;
+    const int row = rowmap[i];
+    float* row_f32 = aev + (size_t)row * AEV_LD;
+    __half* row_hi = planes + (size_t)row * AEV_LD;
 
     // ---- stage all neighbours -------------------------------------------------------------------------
     for (int a = lane; a < nst; a += 32) {
@@ -139,6 +146,7 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
 
     // ---- table of the non-empty species pairs (lane p < 28: internal pair p = angular block p) -------------
     int T_pad;
+    unsigned nz_pairs;                                   // internal pairs with at least one triplet
     {
         int psa = 0, psb = 0, pcount = 0;
         if (lane < NPAIR) { const int e = c_pair_sp[lane]; psa = e & 15; psb = e >> 4; }
@@ -155,6 +163,7 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
         T_pad = __shfl_sync(FULL, pstart, 31);
         pstart -= padded;
         const unsigned nz = __ballot_sync(FULL, pcount > 0);
+        nz_pairs = nz;
         if (pcount > 0) S.tab[__popc(nz & lt)] = make_int4(pstart, ja0 | (kb0 << 8) | (cb << 16) | ((psa == psb) << 24), pcount, lane);
         if (lane == 0) S.tab[__popc(nz)] = make_int4(T_pad, 0, 0, 0);
     }
@@ -176,7 +185,7 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
                 acc = fmaf(fast_exp2(-K.eta_r_l2e * dr * dr), q.y, acc);
             }
             acc += __shfl_xor_sync(FULL, acc, 16);
-            if (lane < 16) S.row[rad_col(s) + m] = acc;
+            if (lane < 16) put_feature<PLANES>(acc, row_f32, row_hi, plane_stride, rad_col(s) + m);
         }
     }
 
@@ -196,7 +205,7 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
                 // u -> (x, y) with u = x nk + y.  Different species: j = j0 + x, k = k0 + y.  Same species: distance
                 // enumeration of the unordered pairs of nk items (d = x, j = y, k = y + d + 1 mod nk), each pair once.
                 const int j0 = E.y & 255, k0 = (E.y >> 8) & 255, nk = (E.y >> 16) & 255;
-                int x = (int)(((float)u + 0.5f) * __frcp_rn((float)nk));
+                int x = (int)(((float)u + 0.5f) * fast_rcp((float)nk));
                 int y = u - x * nk;
                 if (y < 0) { --x; y += nk; } else if (y >= nk) { ++x; y -= nk; }
                 int j, k;
@@ -205,7 +214,7 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
                 const float4 qj = S.nb[j], qk = S.nb[k];
                 const float c = qj.x * qk.x + qj.y * qk.y + qj.z * qk.z;
                 const float cx = qj.y * qk.z - qj.z * qk.y, cy = qj.z * qk.x - qj.x * qk.z, cz = qj.x * qk.y - qj.y * qk.x;
-                const float sn = sqrtf(cx * cx + cy * cy + cz * cz);
+                const float sn = fast_sqrt(cx * cx + cy * cy + cz * cz);
                 const float f2 = 2.0f * S.fca[j] * S.fca[k];
                 const float Rm = 0.5f * (qj.w + qk.w);
 #pragma unroll
@@ -238,44 +247,28 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
                 facc = fmaf(a4.x, b4.x, facc); facc = fmaf(a4.y, b4.y, facc);
                 facc = fmaf(a4.z, b4.z, facc); facc = fmaf(a4.w, b4.w, facc);
             }
-            if (s1 <= T0 + 32) { S.row[32 * S.tab[ee].w + lane] = facc; facc = 0.f; }   // pair complete
+            if (s1 <= T0 + 32) {                              // pair complete: its 32 features go out, 64 (128) contiguous bytes
+                put_feature<PLANES>(facc, row_f32, row_hi, plane_stride, 32 * S.tab[ee].w + lane);
+                facc = 0.f;
+            }
         }
         __syncwarp();
     }
     __syncwarp();
 
-    // ---- write the row (species-grouped row order) -----------------------------------------------------
-    const int row = rowmap[i];
-    if (!PLANES) {
-        float4* out = reinterpret_cast<float4*>(aev + (size_t)row * AEV_LD);
-        for (int c = lane; c < AEV_LD / 4; c += 32) out[c] = reinterpret_cast<const float4*>(S.row)[c];
-    } else {
-        unsigned mask = tile_mask[row / ROW_TILE];
-        if (mask == 0) mask = 1u << 14;                  // G1 runs one block of zeros for an all-zero tile
-        const int half16 = lane >> 4, plane = (lane >> 3) & 1, grp = lane & 7;
-        while (mask) {                                   // two blocks per pass: lanes 0-15 / 16-31, hi and lo 8 lanes each
-            const int b0 = __ffs(mask) - 1; mask &= mask - 1u;
-            int b1 = -1;
-            if (mask) { b1 = __ffs(mask) - 1; mask &= mask - 1u; }
-            const int b = half16 ? b1 : b0;
-            if (b >= 0) {
-                const float4 v0 = *reinterpret_cast<const float4*>(&S.row[KBLK * b + 8 * grp]);
-                const float4 v1 = *reinterpret_cast<const float4*>(&S.row[KBLK * b + 8 * grp + 4]);
-                const float x[8] = {v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w};
-                uint32_t o[4];
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    const uint32_t hi = cvt_pack_h2(x[2 * q], x[2 * q + 1]);
-                    if (plane == 0) o[q] = hi;
-                    else {
-                        const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&hi));
-                        o[q] = cvt_pack_h2(x[2 * q] - f.x, x[2 * q + 1] - f.y);
-                    }
-                }
-                *reinterpret_cast<uint4*>(planes + (size_t)plane * plane_stride + (size_t)row * AEV_LD + KBLK * b + 8 * grp) =
-                    make_uint4(o[0], o[1], o[2], o[3]);
-            }
+    // ---- zeros for what this atom lacks but a reader will touch -------------------------------------------
+    // (tensor path: the feature blocks that are active for the row's tile; fp32 rows: everything)
+    unsigned mask = 0xffffu;
+    if (PLANES) { mask = tile_mask[row / ROW_TILE]; if (mask == 0) mask = 1u << 14; }   // G1 runs one zero block for an all-zero tile
+    for (int p = 0; p < NPAIR; ++p)
+        if (((mask >> (p >> 1)) & 1u) && !((nz_pairs >> p) & 1u)) put_feature<PLANES>(0.f, row_f32, row_hi, plane_stride, 32 * p + lane);
+    for (int q = 0; q < 8; ++q) {                        // radial slots in priority order; slot 7 is the 16 padding columns
+        bool absent = true;
+        if (q < NSP) {
+            const int s = prio_sp(q);
+            absent = __shfl_sync(FULL, cnt, s) + __shfl_sync(FULL, cnt, 8 + s) == 0;
         }
+        if (((mask >> (14 + (q >> 2))) & 1u) && absent && lane < 16) put_feature<PLANES>(0.f, row_f32, row_hi, plane_stride, AEV_ANG + 16 * q + lane);
     }
 }
 
