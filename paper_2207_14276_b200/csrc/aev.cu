@@ -19,8 +19,6 @@
 
 namespace dhp {
 
-constexpr int BWD_WARPS = 4;
-constexpr int GP = 36;   // pitch of one 32-float angular block of the staged gradient row (bank spread, 16 B aligned)
 
 // single-instruction approximations (2^-22 relative error; inputs here are never denormal where it matters)
 __device__ __forceinline__ float fast_exp2(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
@@ -273,19 +271,33 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
 }
 
 // -------------------------------------------------------------------------------------------------
-// backward
+// backward (a5): F = -sum_i sum_m dE/dG_i[m] dG_i[m]/dr, one warp per central atom i
+//   neighbours   lane <-> neighbour (rounds of 32): geometry once, the whole radial derivative of that neighbour
+//                (16 shifts) in registers; the lane keeps the force of "its" neighbours (slots lane, lane+32, lane+64)
+//                in registers until the end.
+//   angular      triplets in distance order, t = d na + j, k = j + d + 1 (mod na): lane <-> triplet computes the two
+//                gradient vectors (on j and on k) and stages them; then lane <-> neighbour n gathers the (at most
+//                two per distance d present in the round) staged vectors that belong to n - closed-form slot
+//                indices, so there are no atomics and no read-modify-write in shared memory.
+//   scatter      one global atomic triple per neighbour and one for the centre.
 // -------------------------------------------------------------------------------------------------
-struct WarpSmemBwd {
-    float grad_rad[AEV_RAD];
-    float grad_ang[NPAIR * GP];
-    float ux[MAX_ANG], uy[MAX_ANG], uz[MAX_ANG], R[MAX_ANG], fc[MAX_ANG], dfc[MAX_ANG];
-    float fx[MAX_ANG], fy[MAX_ANG], fz[MAX_ANG];
+constexpr int BWD_WARPS = 8;
+constexpr int GP = 36;   // pitch of one 32-float angular block of the staged gradient row (bank spread, 16 B aligned)
+constexpr int OWN = 3;   // neighbour slots per lane that can be angular (MAX_ANG = 96 = 3 x 32)
+static_assert(MAX_ANG <= OWN * 32, "angular neighbours must fit the per-lane force registers");
+
+struct __align__(16) WarpSmemBwd {
+    float g_ang[NPAIR * GP];     // dE/dG angular blocks of the row, [internal pair][32] at pitch GP
+    float g_rad[NSP * NR];       // radial blocks by neighbour species
+    float4 nb[MAX_ANG];          // ux, uy, uz, R of the angular neighbours
+    float2 fd[MAX_ANG];          // f_c(R; Rca), f_c'(R; Rca)
+    float st[6][32];             // staged gradient vectors of one round: on j (x, y, z), on k (x, y, z)
     int sp[MAX_ANG];
 };
 
 __global__ void __launch_bounds__(BWD_WARPS * 32)
 k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, const int* __restrict__ col,
-          const int* __restrict__ n_ang, const int* __restrict__ rowmap, const Grid* __restrict__ gp,
+          const unsigned short* __restrict__ seg_cnt, const int* __restrict__ rowmap, const Grid* __restrict__ gp,
           const __grid_constant__ AevConst K, int n, const float* __restrict__ grad, float* __restrict__ fsorted) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ Grid g;
@@ -295,110 +307,169 @@ k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
     const int i = blockIdx.x * BWD_WARPS + w;
     if (i >= n) return;
     WarpSmemBwd& S = reinterpret_cast<WarpSmemBwd*>(smem_raw)[w];
+    const unsigned FULL = 0xffffffffu;
 
+    // run lengths of the row (as in the forward kernel)
+    int cnt = (lane < 16 && lane != 7 && lane != 15) ? (int)seg_cnt[(size_t)i * 16 + lane] : 0;
+    int start = cnt;
+#pragma unroll
+    for (int o = 1; o < 16; o <<= 1) {
+        int y = __shfl_up_sync(FULL, start, o);
+        if (lane >= o) start += y;
+    }
+    start -= cnt;
+    int na = __shfl_sync(FULL, start, 8);
+    int nst = __shfl_sync(FULL, start, 15);
+    if (na > MAX_ANG || nst > MAX_RAD) { na = 0; nst = 0; cnt = 0; }     // capacity overflow: reported by the forward pass
+
+    // ---- the blocks of dE/dG this atom uses ----------------------------------------------------------------
     const float* grow = grad + (size_t)rowmap[i] * AEV_LD;
-    for (int c = lane; c < AEV_RAD; c += 32) S.grad_rad[c] = grow[rad_col(c >> 4) + (c & 15)];
-    for (int c = lane; c < AEV_ANG; c += 32) S.grad_ang[(c >> 5) * GP + (c & 31)] = grow[c];
-
-    const float4 pi = spos[i];
-    const int rb = row_ptr[i], re = row_ptr[i + 1];
-    const int na = min(n_ang[i], MAX_ANG);
-    const float inv_rcr = 1.0f / K.rcr, inv_rca = 1.0f / K.rca;
-
-    // stage the angular neighbours (the prefix of the row)
-    for (int a = lane; a < na; a += 32) {
-        NbrGeom q = neighbour_geom(pi, spos[col[rb + a]], g);
-        S.ux[a] = q.ux; S.uy[a] = q.uy; S.uz[a] = q.uz; S.R[a] = q.R; S.sp[a] = q.sp;
-        S.fc[a] = fcut(q.R, inv_rca);
-        S.dfc[a] = dfcut(q.R, inv_rca, K.pi_over_rca);
-        S.fx[a] = 0.f; S.fy[a] = 0.f; S.fz[a] = 0.f;
+    {
+        int psa = 0, psb = 0;
+        if (lane < NPAIR) { const int e = c_pair_sp[lane]; psa = e & 15; psb = e >> 4; }
+        const int ca = __shfl_sync(FULL, cnt, psa), cb = __shfl_sync(FULL, cnt, psb);
+        unsigned nz = __ballot_sync(FULL, lane < NPAIR && ((psa == psb) ? ca > 1 : (ca > 0 && cb > 0)));
+        for (; nz; nz &= nz - 1u) {
+            const int p = __ffs(nz) - 1;
+            S.g_ang[p * GP + lane] = grow[32 * p + lane];
+        }
+        for (int s = 0; s < NSP; ++s)
+            if (__shfl_sync(FULL, cnt, s) + __shfl_sync(FULL, cnt, 8 + s) > 0 && lane < NR) S.g_rad[NR * s + lane] = grow[rad_col(s) + lane];
     }
     __syncwarp();
 
-    float fix = 0.f, fiy = 0.f, fiz = 0.f;     // force on the centre, summed over this lane's terms
-
-    // ---- angular: rounds over the index distance d ---------------------------------------------------
-    for (int d = 1; 2 * d <= na; ++d) {
-        const int jmax = (2 * d == na) ? na / 2 : na;     // even n: the last round holds each pair once
-        for (int jb = 0; jb < jmax; jb += 32) {
-            const int j = jb + lane;
-            const bool act = j < jmax;
-            int k = 0;
-            float gjx = 0.f, gjy = 0.f, gjz = 0.f, gkx = 0.f, gky = 0.f, gkz = 0.f;
-            if (act) {
-                k = j + d; if (k >= na) k -= na;
-                const float ujx = S.ux[j], ujy = S.uy[j], ujz = S.uz[j], Rj = S.R[j];
-                const float ukx = S.ux[k], uky = S.uy[k], ukz = S.uz[k], Rk = S.R[k];
-                const float c = ujx * ukx + ujy * uky + ujz * ukz;
-                const float cx = ujy * ukz - ujz * uky, cy = ujz * ukx - ujx * ukz, cz = ujx * uky - ujy * ukx;
-                const float s = sqrtf(cx * cx + cy * cy + cz * cz);
-                const float fj = S.fc[j], fk = S.fc[k], dfj = S.dfc[j], dfk = S.dfc[k];
-                const float Rm = 0.5f * (Rj + Rk);
-                const float* gb = &S.grad_ang[GP * ipair(S.sp[j], S.sp[k])];
-                float Az[NZ], dAz[NZ];
+    const int rb = row_ptr[i];
+    const float4 pi = spos[i];
+    const float inv_rcr = 1.0f / K.rcr, inv_rca = 1.0f / K.rca;
+    float fix = 0.f, fiy = 0.f, fiz = 0.f;              // force on the centre, summed over this lane's terms
+    float Fx[OWN], Fy[OWN], Fz[OWN];                    // forces on the neighbours lane, lane + 32, lane + 64
+    int cj[OWN];
 #pragma unroll
-                for (int z = 0; z < NZ; ++z) {
-                    float u = fmaxf(0.5f * (1.0f + c * K.cos_z[z] + s * K.sin_z[z]), 0.f);
-                    float wz = fast_exp2((K.zeta - 1.0f) * fast_log2(u));      // u^(zeta-1)
-                    Az[z] = 2.0f * u * wz;                                      // A = 2 u^zeta
-                    dAz[z] = -K.zeta * wz * (s * K.cos_z[z] - c * K.sin_z[z]);  // dA/dtheta
-                }
-                float S0 = 0.f, Sm = 0.f, St = 0.f;
-#pragma unroll
-                for (int a = 0; a < NA; ++a) {
-                    const float4 g4 = *reinterpret_cast<const float4*>(gb + 4 * a);
-                    float mm = Rm - K.shf_a[a];
-                    float B = fast_exp2(-K.eta_a_l2e * mm * mm);
-                    float dB = -K.eta_a * mm * B;                               // dB/dR_ij = dB/dR_ik
-                    float ua = g4.x * Az[0] + g4.y * Az[1] + g4.z * Az[2] + g4.w * Az[3];
-                    float va = g4.x * dAz[0] + g4.y * dAz[1] + g4.z * dAz[2] + g4.w * dAz[3];
-                    S0 += B * ua; Sm += dB * ua; St += B * va;
-                }
-                const float dth = St * fj * fk;                                 // sum g dT/dtheta
-                const float dRj = (Sm * fj + S0 * dfj) * fk;                    // sum g dT/dR_ij
-                const float dRk = (Sm * fk + S0 * dfk) * fj;
-                const float inv_s = s > 1e-20f ? 1.0f / s : 0.f;                // collinear: e = 0 (Q7)
-                const float tj = -dth * inv_s / Rj, tk = -dth * inv_s / Rk;     // d theta/d r_j = -e_j / R_ij
-                gjx = tj * (ukx - c * ujx) + dRj * ujx; gjy = tj * (uky - c * ujy) + dRj * ujy; gjz = tj * (ukz - c * ujz) + dRj * ujz;
-                gkx = tk * (ujx - c * ukx) + dRk * ukx; gky = tk * (ujy - c * uky) + dRk * uky; gkz = tk * (ujz - c * ukz) + dRk * ukz;
-                fix += gjx + gkx; fiy += gjy + gky; fiz += gjz + gkz;
-                S.fx[j] -= gjx; S.fy[j] -= gjy; S.fz[j] -= gjz;                 // all j distinct in this step
-            }
-            __syncwarp();
-            if (act) { S.fx[k] -= gkx; S.fy[k] -= gky; S.fz[k] -= gkz; }       // all k distinct in this step
-            __syncwarp();
-        }
-    }
+    for (int q = 0; q < OWN; ++q) { Fx[q] = Fy[q] = Fz[q] = 0.f; cj[q] = 0; }
 
-    // ---- radial + scatter ----------------------------------------------------------------------------
-    for (int base = rb; base < re; base += 32) {
-        const int idx = base + lane;
-        if (idx < re) {
-            const int j = col[idx];
-            NbrGeom q = neighbour_geom(pi, spos[j], g);
-            const float fc = fcut(q.R, inv_rcr), dfc = dfcut(q.R, inv_rcr, K.pi_over_rcr);
-            const float* gr = &S.grad_rad[NR * q.sp];
+    // ---- neighbours: geometry, staging of the angular ones, radial derivative (Eq. 4) -----------------------
+#pragma unroll
+    for (int q = 0; q < MAX_RAD / 32; ++q) {
+        const int a = lane + 32 * q;
+        if (32 * q < nst && a < nst) {
+            const int jg = col[rb + a];
+            const NbrGeom nbq = neighbour_geom(pi, spos[jg], g);
+            const float fc = fcut(nbq.R, inv_rcr), dfc = dfcut(nbq.R, inv_rcr, K.pi_over_rcr);
+            const float c1 = -2.0f * K.eta_r * fc;
+            const float4* gr = reinterpret_cast<const float4*>(&S.g_rad[NR * nbq.sp]);
             float coef = 0.f;
 #pragma unroll
-            for (int mI = 0; mI < NR; ++mI) {
-                float dr = q.R - K.shf_r[mI];
-                float t = fast_exp2(-K.eta_r_l2e * dr * dr);
-                coef += gr[mI] * t * (-2.0f * K.eta_r * dr * fc + dfc);
+            for (int m4 = 0; m4 < NR / 4; ++m4) {
+                const float4 g4 = gr[m4];
+                const float gm[4] = {g4.x, g4.y, g4.z, g4.w};
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const float dr = nbq.R - K.shf_r[4 * m4 + e];
+                    const float t = fast_exp2(-K.eta_r_l2e * dr * dr);
+                    coef = fmaf(gm[e] * t, fmaf(c1, dr, dfc), coef);
+                }
             }
-            float vx = coef * q.ux, vy = coef * q.uy, vz = coef * q.uz;
+            const float vx = coef * nbq.ux, vy = coef * nbq.uy, vz = coef * nbq.uz;
             fix += vx; fiy += vy; fiz += vz;
-            float fjx = -vx, fjy = -vy, fjz = -vz;
-            const int a = idx - rb;
-            if (a < na) { fjx += S.fx[a]; fjy += S.fy[a]; fjz += S.fz[a]; }
-            atomicAdd(&fsorted[3 * j + 0], fjx);
-            atomicAdd(&fsorted[3 * j + 1], fjy);
-            atomicAdd(&fsorted[3 * j + 2], fjz);
+            if (a < na) {
+                S.nb[a] = make_float4(nbq.ux, nbq.uy, nbq.uz, nbq.R);
+                S.fd[a] = make_float2(fcut(nbq.R, inv_rca), dfcut(nbq.R, inv_rca, K.pi_over_rca));
+                S.sp[a] = nbq.sp;
+            }
+            if (q < OWN) { Fx[q] = -vx; Fy[q] = -vy; Fz[q] = -vz; cj[q] = jg; }
+            else {
+                atomicAdd(&fsorted[3 * jg + 0], -vx);
+                atomicAdd(&fsorted[3 * jg + 1], -vy);
+                atomicAdd(&fsorted[3 * jg + 2], -vz);
+            }
+        }
+    }
+    __syncwarp();
+
+    // ---- angular (Eq. 5) -----------------------------------------------------------------------------------
+    const int npairs = na * (na - 1) / 2;
+    const float inv_na = na > 0 ? fast_rcp((float)na) : 0.f;
+    for (int T0 = 0; T0 < npairs; T0 += 32) {
+        const int t = T0 + lane;
+        if (t < npairs) {
+            int d = (int)(((float)t + 0.5f) * inv_na);
+            int j = t - d * na;
+            if (j < 0) { --d; j += na; } else if (j >= na) { ++d; j -= na; }
+            int k = j + d + 1;
+            if (k >= na) k -= na;
+            const float4 qj = S.nb[j], qk = S.nb[k];
+            const float2 fj = S.fd[j], fk = S.fd[k];
+            const float c = qj.x * qk.x + qj.y * qk.y + qj.z * qk.z;
+            const float cx = qj.y * qk.z - qj.z * qk.y, cy = qj.z * qk.x - qj.x * qk.z, cz = qj.x * qk.y - qj.y * qk.x;
+            const float sn = fast_sqrt(cx * cx + cy * cy + cz * cz);
+            const float Rm = 0.5f * (qj.w + qk.w);
+            const float4* gb = reinterpret_cast<const float4*>(&S.g_ang[GP * ipair(S.sp[j], S.sp[k])]);
+            float Az[NZ], dAz[NZ];
+#pragma unroll
+            for (int z = 0; z < NZ; ++z) {
+                const float u = fmaxf(fmaf(0.5f * K.sin_z[z], sn, fmaf(0.5f * K.cos_z[z], c, 0.5f)), 0.f);
+                const float wz = fast_exp2((K.zeta - 1.0f) * fast_log2(u));       // u^(zeta-1)
+                Az[z] = 2.0f * u * wz;                                             // A = 2 u^zeta
+                dAz[z] = -K.zeta * wz * (sn * K.cos_z[z] - c * K.sin_z[z]);        // dA/dtheta
+            }
+            float S0 = 0.f, Sm = 0.f, St = 0.f;
+#pragma unroll
+            for (int a = 0; a < NA; ++a) {
+                const float4 g4 = gb[a];
+                const float mm = Rm - K.shf_a[a];
+                const float B = fast_exp2(-K.eta_a_l2e * mm * mm);
+                const float dB = -K.eta_a * mm * B;                                // dB/dR_ij = dB/dR_ik
+                const float ua = g4.x * Az[0] + g4.y * Az[1] + g4.z * Az[2] + g4.w * Az[3];
+                const float va = g4.x * dAz[0] + g4.y * dAz[1] + g4.z * dAz[2] + g4.w * dAz[3];
+                S0 = fmaf(B, ua, S0); Sm = fmaf(dB, ua, Sm); St = fmaf(B, va, St);
+            }
+            const float dth = St * fj.x * fk.x;                                    // sum g dT/dtheta
+            const float dRj = (Sm * fj.x + S0 * fj.y) * fk.x;                      // sum g dT/dR_ij
+            const float dRk = (Sm * fk.x + S0 * fk.y) * fj.x;
+            const float inv_s = sn > 1e-20f ? fast_rcp(sn) : 0.f;                  // collinear: e = 0 (Q7)
+            const float tj = -dth * inv_s * fast_rcp(qj.w), tk = -dth * inv_s * fast_rcp(qk.w);   // d theta/d r_j = -e_j / R_ij
+            const float gjx = tj * (qk.x - c * qj.x) + dRj * qj.x, gjy = tj * (qk.y - c * qj.y) + dRj * qj.y,
+                        gjz = tj * (qk.z - c * qj.z) + dRj * qj.z;
+            const float gkx = tk * (qj.x - c * qk.x) + dRk * qk.x, gky = tk * (qj.y - c * qk.y) + dRk * qk.y,
+                        gkz = tk * (qj.z - c * qk.z) + dRk * qk.z;
+            fix += gjx + gkx; fiy += gjy + gky; fiz += gjz + gkz;
+            S.st[0][lane] = gjx; S.st[1][lane] = gjy; S.st[2][lane] = gjz;
+            S.st[3][lane] = gkx; S.st[4][lane] = gky; S.st[5][lane] = gkz;
+        }
+        __syncwarp();
+        // gather: neighbour nn is j of slot d na + nn and k of slot d na + (nn - d - 1 mod na), for every d in the round
+        const int cntr = min(32, npairs - T0);
+        const int d_lo = T0 / na, d_hi = (T0 + cntr - 1) / na;
+#pragma unroll
+        for (int q = 0; q < OWN; ++q) {
+            const int nn = lane + 32 * q;
+            if (32 * q < na && nn < na) {
+                for (int d = d_lo; d <= d_hi; ++d) {
+                    const int tj = d * na + nn - T0;
+                    if ((unsigned)tj < (unsigned)cntr) { Fx[q] -= S.st[0][tj]; Fy[q] -= S.st[1][tj]; Fz[q] -= S.st[2][tj]; }
+                    int jj = nn - d - 1;
+                    if (jj < 0) jj += na;
+                    const int tk = d * na + jj - T0;
+                    if ((unsigned)tk < (unsigned)cntr) { Fx[q] -= S.st[3][tk]; Fy[q] -= S.st[4][tk]; Fz[q] -= S.st[5][tk]; }
+                }
+            }
+        }
+        __syncwarp();
+    }
+
+    // ---- scatter ---------------------------------------------------------------------------------------------
+#pragma unroll
+    for (int q = 0; q < OWN; ++q) {
+        if (lane + 32 * q < nst) {
+            atomicAdd(&fsorted[3 * cj[q] + 0], Fx[q]);
+            atomicAdd(&fsorted[3 * cj[q] + 1], Fy[q]);
+            atomicAdd(&fsorted[3 * cj[q] + 2], Fz[q]);
         }
     }
     for (int o = 16; o; o >>= 1) {
-        fix += __shfl_xor_sync(0xffffffffu, fix, o);
-        fiy += __shfl_xor_sync(0xffffffffu, fiy, o);
-        fiz += __shfl_xor_sync(0xffffffffu, fiz, o);
+        fix += __shfl_xor_sync(FULL, fix, o);
+        fiy += __shfl_xor_sync(FULL, fiy, o);
+        fiz += __shfl_xor_sync(FULL, fiz, o);
     }
     if (lane == 0) {
         atomicAdd(&fsorted[3 * i + 0], fix);
@@ -480,7 +551,7 @@ int aev_backward(Ctx* ctx, float* F_out) {
     }
     DHP_CUDA(ctx, cudaMemsetAsync(ctx->fsorted, 0, sizeof(float) * 3 * n, ctx->stream));
     DHP_LAUNCH(ctx, k_aev_bwd, (n + BWD_WARPS - 1) / BWD_WARPS, BWD_WARPS * 32, smem, ctx->spos, ctx->row_ptr, ctx->col,
-               ctx->n_ang, ctx->rowmap, ctx->grid, ctx->aevc, n, ctx->grad, ctx->fsorted);
+               ctx->seg_cnt, ctx->rowmap, ctx->grid, ctx->aevc, n, ctx->grad, ctx->fsorted);
     DHP_LAUNCH(ctx, k_unsort_forces, (n + 255) / 256, 256, 0, ctx->fsorted, ctx->perm, n, F_out);
     DHP_CUDA(ctx, cudaGetLastError());
     return DHP_OK;
