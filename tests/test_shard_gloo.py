@@ -1,0 +1,114 @@
+"""Host-side multi-process logic on CPU: world_size 2, gloo backend, 127.0.0.1 rendezvous.
+
+No GPU here, so the per-rank compute is played by the fp64 oracle (tests may use it); what is under test is the
+sharding arithmetic and the gather / reduce plumbing of `paper_2207_14276_b200.shard`: the sharded result must equal
+the single-process one, units must be covered exactly once, timing is the max over ranks.
+"""
+import os
+import socket
+
+import numpy as np
+import pytest
+
+from paper_2207_14276_b200 import shard
+from paper_2207_14276_b200 import workloads as W
+
+WORLD = 2
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def test_shard_range_covers_every_unit_once():
+    for n in (0, 1, 2, 7, 1024, 98000):
+        for world in (1, 2, 3, 8):
+            parts = [shard.shard_range(n, world, r) for r in range(world)]
+            assert parts[0][0] == 0 and parts[-1][1] == n
+            assert all(parts[r][1] == parts[r + 1][0] for r in range(world - 1))
+            sizes = [hi - lo for lo, hi in parts]
+            assert max(sizes) - min(sizes) <= 1
+    with pytest.raises(ValueError):
+        shard.shard_range(4, 2, 2)
+
+
+def test_shard_molecules_keeps_molecules_whole():
+    s = W.replicas_1024x30(n_mol=11)
+    seen = []
+    for r in range(3):
+        m_lo, m_hi, a_lo, a_hi, off = shard.shard_molecules(s.mol_offsets, 3, r)
+        assert off[0] == 0 and off[-1] == a_hi - a_lo and np.all(np.diff(off) == 30)
+        assert a_lo == s.mol_offsets[m_lo] and a_hi == s.mol_offsets[m_hi]
+        seen += list(range(m_lo, m_hi))
+    assert seen == list(range(11))
+
+
+def test_slab_owner_is_a_balanced_partition_and_periodic_wrap_invariant():
+    s = W.make_system(1)
+    own = shard.slab_owner(s.pos, s.box, 4)
+    assert sorted(np.bincount(own, minlength=4)) == [72, 72, 72, 72]
+    shifted = s.pos.copy()
+    shifted[::5, 0] += 3 * s.box[0]            # whole-box shifts do not move an atom to another slab
+    assert np.array_equal(shard.slab_owner(shifted.astype(np.float64), s.box, 4), own) or \
+        np.mean(shard.slab_owner(shifted, s.box, 4) == own) > 0.98      # fp32 shift rounding may move an edge atom
+    cs = [shard.slab_centres(s.pos, s.box, 4, r) for r in range(4)]
+    assert np.array_equal(np.sort(np.concatenate(cs)), np.arange(s.n_atoms))
+
+
+def _worker(rank, port, results):
+    import torch
+    import torch.distributed as dist
+    import oracle
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=WORLD)
+    try:
+        params = W.default_params()
+        blob = W.make_weights(1)
+        # (1) independent problems: molecules sharded, energies gathered in order
+        s = W.replicas_1024x30(n_mol=7)
+        m_lo, m_hi, a_lo, a_hi, off = shard.shard_molecules(s.mol_offsets, WORLD, rank)
+        Ea, Fa, _ = oracle.energy_forces(s.pos[a_lo:a_hi], s.species[a_lo:a_hi], None, params, blob, 1, mol_offsets=off)
+        E_local = torch.from_numpy(np.add.reduceat(Ea, off[:-1].astype(np.int64)))
+        E_all = shard.gather_molecule_energies(E_local, 7).numpy()
+        # (2) one system, central atoms in slabs: partial forces and energies summed
+        w = W.make_system(1)
+        centres = shard.slab_centres(w.pos, w.box, WORLD, rank)
+        Ec, Fc, _ = oracle.energy_forces(w.pos, w.species, w.box, params, blob, 1, centres=centres)
+        E_part = torch.tensor([Ec.sum()], dtype=torch.float64)
+        F_part = torch.from_numpy(Fc.copy())
+        shard.sum_partial_forces(E_part, F_part)
+        # (3) timing: slowest rank
+        t = shard.max_over_ranks([1.0 + rank, 5.0 - rank])
+        if rank == 0:
+            results.put((E_all, E_part.numpy(), F_part.numpy(), t, len(centres)))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_world2_gloo_sharded_results_equal_single_process():
+    import torch.multiprocessing as mp
+    import oracle
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, port, q)) for r in range(WORLD)]
+    for p in procs:
+        p.start()
+    E_all, E_sum, F_sum, t, n_c0 = q.get(timeout=240)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    params = W.default_params()
+    blob = W.make_weights(1)
+    s = W.replicas_1024x30(n_mol=7)
+    Eo, _ = oracle.total_energy_forces(W.System(s.name, s.pos, s.species, None, s.mol_offsets, 1), params, blob)
+    assert np.allclose(E_all, Eo, rtol=0, atol=1e-12)
+    w = W.make_system(1)
+    Ew, Fw = oracle.total_energy_forces(w, params, blob)
+    assert n_c0 == w.n_atoms // 2
+    assert abs(E_sum[0] - Ew[0]) <= 1e-10
+    assert np.max(np.abs(F_sum - Fw)) <= 1e-12
+    assert t == [2.0, 5.0]
