@@ -155,6 +155,12 @@ int dhp_tensor_path_available(dhp_ctx* ctx);
 int dhp_debug_aev(dhp_ctx* ctx, float* aev);
 int dhp_debug_grad(dhp_ctx* ctx, float* grad);
 int dhp_debug_atomic_energy(dhp_ctx* ctx, float* e_atom);
+/* Work accounting of the last call (host outputs, synchronises): the number of 128-row MLP tiles and the
+ * total number of 64-wide feature blocks that are active over all tiles (at most 16 per tile).  The first
+ * GEMM of the forward pass visits, and the last GEMM of the backward pass produces, only the active blocks
+ * of a tile - the others are identically zero (absent neighbour species) - so the tensor-core work actually
+ * issued for those two GEMMs is n_active_blocks / (16 n_row_tiles) of the dense count. */
+int dhp_debug_tile_blocks(dhp_ctx* ctx, int64_t* n_row_tiles, int64_t* n_active_blocks);
 
 /* Per-phase device timing.  dhp_profile_enable(ctx, 1) makes every hot call record CUDA events around
  * each phase on the context stream; dhp_profile_read synchronises and returns, for the calls since the

@@ -39,6 +39,7 @@ SYMBOLS = {
     "dhp_debug_aev": (C.c_int, [_vp, _vp]),
     "dhp_debug_grad": (C.c_int, [_vp, _vp]),
     "dhp_debug_atomic_energy": (C.c_int, [_vp, _vp]),
+    "dhp_debug_tile_blocks": (C.c_int, [_vp, C.POINTER(_i64), C.POINTER(_i64)]),
     "dhp_profile_enable": (C.c_int, [_vp, _i32]),
     "dhp_profile_reset": (C.c_int, [_vp]),
     "dhp_profile_read": (C.c_int, [_vp, C.POINTER(C.c_double), C.POINTER(_i64)]),
@@ -245,6 +246,12 @@ class Dhp:
 
     def dhp_debug_atomic_energy(self):
         return self._debug(self.lib.dhp_debug_atomic_energy, 1)[:, 0]
+
+    def dhp_debug_tile_blocks(self):
+        """(row tiles, active 64-wide feature blocks summed over tiles) of the last call."""
+        a, b = _i64(), _i64()
+        _check(self.lib.dhp_debug_tile_blocks(self.ctx, C.byref(a), C.byref(b)), self.ctx)
+        return int(a.value), int(b.value)
 
     def dhp_profile_enable(self, on: bool):
         _check(self.lib.dhp_profile_enable(self.ctx, 1 if on else 0), self.ctx)

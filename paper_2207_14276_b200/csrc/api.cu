@@ -2,6 +2,7 @@
 #include <math.h>
 #include <new>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include "dhp_internal.cuh"
@@ -40,7 +41,7 @@ static bool dalloc(T** p, size_t count) {
 static void free_all(Ctx* c) {
     void* ptrs[] = {c->grid, c->status, c->bbox, c->cell_of, c->perm_tmp, c->cell_count, c->cell_start, c->cell_fill, c->perm,
                     c->inv_perm, c->spos, c->smol, c->n_rad, c->n_ang, c->row_ptr, c->col, c->sp_count, c->sp_start,
-                    c->rowmap, c->row_species, c->row_slot, c->blk_hist, c->tile_mask, c->tc_sched, c->col2feat, c->aev, c->grad, c->e_atom, c->fsorted,
+                    c->rowmap, c->row_species, c->row_slot, c->blk_hist, c->key_start, c->amask, c->tile_mask, c->tc_sched, c->col2feat, c->aev, c->grad, c->e_atom, c->fsorted,
                     c->e_out_tmp, c->export_tmp, c->tmp_col, c->blk_sum, c->blk_off, c->seg_cnt, c->st_pos, c->st_species, c->st_mol, c->st_E, c->st_F};
     for (void* p : ptrs) if (p) cudaFree(p);
     mlp_simt_free(c);
@@ -184,7 +185,7 @@ int dhp_create(dhp_ctx** out, const dhp_params* params, int64_t max_atoms, int64
     ok &= dalloc(&c->n_rad, N) && dalloc(&c->n_ang, N) && dalloc(&c->row_ptr, N + 1) && dalloc(&c->col, (size_t)c->pair_cap);
     ok &= dalloc(&c->tmp_col, N * c->tmp_stride) && dalloc(&c->blk_sum, N / 64 + 3) && dalloc(&c->blk_off, N / 64 + 3) && dalloc(&c->seg_cnt, N * 16);
     ok &= dalloc(&c->sp_count, 8) && dalloc(&c->sp_start, 8) && dalloc(&c->rowmap, N);
-    ok &= dalloc(&c->row_species, R) && dalloc(&c->row_slot, R) && dalloc(&c->blk_hist, (N / 256 + 2) * 8);
+    ok &= dalloc(&c->row_species, R) && dalloc(&c->row_slot, R) && dalloc(&c->blk_hist, (N / 256 + 2) * 224) && dalloc(&c->key_start, 224) && dalloc(&c->amask, N);
     ok &= dalloc(&c->aev, R * AEV_LD) && dalloc(&c->grad, R * AEV_LD) && dalloc(&c->e_atom, R);
     ok &= dalloc(&c->tile_mask, R / ROW_TILE) && dalloc(&c->tc_sched, 8) && dalloc(&c->col2feat, AEV_LD);
     ok &= dalloc(&c->fsorted, 3 * N) && dalloc(&c->e_out_tmp, NM) && dalloc(&c->export_tmp, N + 1);
@@ -366,6 +367,26 @@ int dhp_debug_aev(dhp_ctx* h, float* aev) {
 }
 int dhp_debug_grad(dhp_ctx* h, float* grad) { return h ? debug_gather(h, h->c.grad, AEV_LD, AEV_DIM, grad, true) : DHP_E_BADARG; }
 int dhp_debug_atomic_energy(dhp_ctx* h, float* e) { return h ? debug_gather(h, h->c.e_atom, 1, 1, e, false) : DHP_E_BADARG; }
+
+int dhp_debug_tile_blocks(dhp_ctx* h, int64_t* n_row_tiles, int64_t* n_active_blocks) {
+    if (!h || !n_row_tiles || !n_active_blocks) return DHP_E_BADARG;
+    Ctx* c = &h->c;
+    *n_row_tiles = 0; *n_active_blocks = 0;
+    if (c->n_atoms == 0) return DHP_OK;
+    int sp_start[8];
+    DHP_CUDA(c, cudaMemcpyAsync(sp_start, c->sp_start, sizeof(sp_start), cudaMemcpyDeviceToHost, c->stream));
+    DHP_CUDA(c, cudaStreamSynchronize(c->stream));
+    const int nt = sp_start[NSP] / ROW_TILE;
+    unsigned* m = (unsigned*)malloc(sizeof(unsigned) * (nt > 0 ? nt : 1));
+    if (!m) return DHP_E_NOMEM;
+    cudaError_t e = cudaMemcpy(m, c->tile_mask, sizeof(unsigned) * nt, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) { free(m); return cuda_fail(c, e, "tile mask download"); }
+    int64_t blocks = 0;
+    for (int t = 0; t < nt; ++t) blocks += __builtin_popcount(m[t] ? m[t] : (1u << 14));   // an all-zero tile runs one block
+    free(m);
+    *n_row_tiles = nt; *n_active_blocks = blocks;
+    return DHP_OK;
+}
 
 int dhp_profile_enable(dhp_ctx* h, int on) {
     if (!h) return DHP_E_BADARG;

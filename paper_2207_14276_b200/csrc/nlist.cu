@@ -209,78 +209,99 @@ __global__ void k_sort_gather(const float* __restrict__ pos, const int* __restri
 }
 
 // ---------------------------------------------------------------------------------------------
-// species-grouped rows (stable in sorted order)
+// species-grouped rows, ordered inside a species group by the feature blocks the atom can touch
+//
+// One 128-row MLP tile runs one network, so rows are grouped by the central atom's species (groups start at
+// multiples of ROW_TILE).  G1 / B1 skip the 64-wide feature blocks that are zero for a whole tile, so inside a
+// group rows are ordered by a class derived from the atom's own block mask: the highest angular block it can
+// touch (blocks are ordered common species first, dhp_internal.cuh) and whether it sees a rare species radially.
+// Atoms with nested neighbour-species sets (water-only < near the solute < near a sulfur ...) then share tiles
+// and the tile masks stay small.  The order is deterministic (stable in sorted-slot order inside a class).
 // ---------------------------------------------------------------------------------------------
-constexpr int RB = 256;   // slots per block in the row assignment
+constexpr int RB = 256;           // slots per block in the row assignment
+constexpr int NCLS = 32;          // classes per species
+constexpr int NKEY = NSP * NCLS;  // 224 row keys
 
-__global__ void k_species_hist(const float4* __restrict__ spos, int n, int* __restrict__ blk_hist) {
-    __shared__ int h[NSP];
-    if (threadIdx.x < NSP) h[threadIdx.x] = 0;
-    __syncthreads();
-    int a = blockIdx.x * RB + threadIdx.x;
-    int s = a < n ? __float_as_int(spos[a].w) : -1;
-    for (int t = 0; t < NSP; ++t) {
-        unsigned m = __ballot_sync(0xffffffffu, s == t);
-        if ((threadIdx.x & 31) == 0 && m) atomicAdd(&h[t], __popc(m));
-    }
-    __syncthreads();
-    if (threadIdx.x < NSP) blk_hist[blockIdx.x * 8 + threadIdx.x] = h[threadIdx.x];
+__device__ __forceinline__ int row_key(int s, unsigned m) {
+    const unsigned ang = m & 0x3fffu;
+    const int hi = ang ? 32 - __clz(ang) : 0;                 // 0 (no angular block) .. 14
+    return s * NCLS + 2 * hi + (int)((m >> 15) & 1u);
 }
 
-// single block, one warp per species: exclusive scan over blocks; group starts aligned to ROW_TILE
-__global__ void k_species_scan(int* __restrict__ blk_hist, int nblk, int* __restrict__ sp_count, int* __restrict__ sp_start) {
-    __shared__ int tot[NSP + 1];
+// blk_hist is key-major: blk_hist[key * nrb + block]
+__global__ void __launch_bounds__(RB)
+k_rowkey_hist(const float4* __restrict__ spos, const unsigned* __restrict__ amask, int n, int nrb, int* __restrict__ blk_hist) {
+    __shared__ int h[NKEY];
+    for (int k = threadIdx.x; k < NKEY; k += RB) h[k] = 0;
+    __syncthreads();
+    const int a = blockIdx.x * RB + threadIdx.x;
+    if (a < n) atomicAdd(&h[row_key(__float_as_int(spos[a].w), amask[a])], 1);
+    __syncthreads();
+    for (int k = threadIdx.x; k < NKEY; k += RB) blk_hist[(size_t)k * nrb + blockIdx.x] = h[k];
+}
+
+// single block of 1024 threads, warps take keys round-robin: exclusive scan over blocks per key, then the key starts
+// (species groups aligned to ROW_TILE)
+__global__ void __launch_bounds__(1024)
+k_rowkey_scan(int* __restrict__ blk_hist, int nrb, int* __restrict__ sp_count, int* __restrict__ sp_start, int* __restrict__ key_start) {
+    __shared__ int tot[NKEY];
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (w < NSP) {
+    for (int key = w; key < NKEY; key += 32) {
+        int* hk = blk_hist + (size_t)key * nrb;
         int run = 0;
-        for (int base = 0; base < nblk; base += 32) {
+        for (int base = 0; base < nrb; base += 32) {
             const int b = base + lane;
-            const int v = b < nblk ? blk_hist[b * 8 + w] : 0;
+            const int v = b < nrb ? hk[b] : 0;
             int x = v;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
                 int y = __shfl_up_sync(0xffffffffu, x, o);
                 if (lane >= o) x += y;
             }
-            if (b < nblk) blk_hist[b * 8 + w] = run + x - v;
+            if (b < nrb) hk[b] = run + x - v;
             run += __shfl_sync(0xffffffffu, x, 31);
         }
-        if (lane == 0) tot[w] = run;
+        if (lane == 0) tot[key] = run;
     }
     __syncthreads();
     if (threadIdx.x == 0) {
         int start = 0;
         for (int s = 0; s < NSP; ++s) {
-            sp_count[s] = tot[s];
             sp_start[s] = start;
-            start += (tot[s] + ROW_TILE - 1) / ROW_TILE * ROW_TILE;
+            int c = 0;
+            for (int k = 0; k < NCLS; ++k) { key_start[s * NCLS + k] = start + c; c += tot[s * NCLS + k]; }
+            sp_count[s] = c;
+            start += (c + ROW_TILE - 1) / ROW_TILE * ROW_TILE;
         }
         sp_start[NSP] = start;
         sp_count[NSP] = 0;
     }
 }
 
-__global__ void k_species_rank(const float4* __restrict__ spos, int n, const int* __restrict__ blk_hist,
-                               const int* __restrict__ sp_start, int* __restrict__ rowmap,
-                               int* __restrict__ row_species, int* __restrict__ row_slot) {
-    __shared__ int wcnt[RB / 32][NSP];
-    int a = blockIdx.x * RB + threadIdx.x;
-    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    int s = a < n ? __float_as_int(spos[a].w) : -1;
-    int rank_in_warp = 0;
-    for (int t = 0; t < NSP; ++t) {
-        unsigned m = __ballot_sync(0xffffffffu, s == t);
-        if (s == t) rank_in_warp = __popc(m & ((1u << lane) - 1u));
-        if (lane == 0) wcnt[w][t] = __popc(m);
-    }
+__global__ void __launch_bounds__(RB)
+k_rowkey_rank(const float4* __restrict__ spos, const unsigned* __restrict__ amask, int n, int nrb, const int* __restrict__ blk_hist,
+              const int* __restrict__ key_start, int* __restrict__ rowmap, int* __restrict__ row_species,
+              int* __restrict__ row_slot, unsigned* __restrict__ tile_mask) {
+    __shared__ int wcnt[RB / 32][NKEY];
+    for (int k = threadIdx.x; k < (RB / 32) * NKEY; k += RB) (&wcnt[0][0])[k] = 0;
+    __syncthreads();
+    const int a = blockIdx.x * RB + threadIdx.x;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    int s = 0, key = -1;
+    unsigned m = 0;
+    if (a < n) { s = __float_as_int(spos[a].w); m = amask[a]; key = row_key(s, m); }
+    const unsigned grp = __match_any_sync(0xffffffffu, key);
+    const int rank_in_warp = __popc(grp & ((1u << lane) - 1u));
+    if (key >= 0 && rank_in_warp == 0) wcnt[w][key] = __popc(grp);
     __syncthreads();
     if (a >= n) return;
     int before = 0;
-    for (int q = 0; q < w; ++q) before += wcnt[q][s];
-    int row = sp_start[s] + blk_hist[blockIdx.x * 8 + s] + before + rank_in_warp;
+    for (int q = 0; q < w; ++q) before += wcnt[q][key];
+    const int row = key_start[key] + blk_hist[(size_t)key * nrb + blockIdx.x] + before + rank_in_warp;
     rowmap[a] = row;
     row_species[row] = s;
     row_slot[row] = a;
+    if (m) atomicOr(&tile_mask[row / ROW_TILE], m);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -495,7 +516,7 @@ constexpr int MAX_STRIDE_CHUNKS = 6;    // tmp_stride <= 192
 __global__ void __launch_bounds__(P2_THREADS)
 k_rows(const unsigned* __restrict__ tmp, int stride, const int* __restrict__ cnt, const int* __restrict__ blk_off, int nblk,
        int n, int* __restrict__ row_ptr, int* __restrict__ col, int* __restrict__ n_rad, int* __restrict__ n_ang,
-       unsigned short* __restrict__ seg_cnt, const int* __restrict__ rowmap, unsigned* __restrict__ tile_mask) {
+       unsigned short* __restrict__ seg_cnt, unsigned* __restrict__ amask) {
     __shared__ int wsum[ROWS_PER_BLK / 32];
     __shared__ int rstart[ROWS_PER_BLK];
     __shared__ int segs[P2_THREADS / 32][16];
@@ -565,7 +586,7 @@ k_rows(const unsigned* __restrict__ tmp, int stride, const int* __restrict__ cnt
             const unsigned pm = __ballot_sync(0xffffffffu, pp);
             const bool bb = lane < 14 ? ((pm >> (2 * lane)) & 3u) != 0 : lane == 14 ? (rm & 0x0fu) != 0 : lane == 15 ? (rm & 0x70u) != 0 : false;
             const unsigned bmask = __ballot_sync(0xffffffffu, bb);
-            if (lane == 0 && bmask) atomicOr(&tile_mask[rowmap[i] / ROW_TILE], bmask);
+            if (lane == 0) amask[i] = bmask;
         }
         int x = cnt_k;
 #pragma unroll
@@ -651,12 +672,6 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
     }
     DHP_LAUNCH(ctx, k_sort_gather, (int)((cell_bound + 3) / 4), 128, 0, pos, species, ctx->grid, ctx->cell_start,
                ctx->perm_tmp, ctx->perm, ctx->inv_perm, ctx->spos, ctx->smol);
-    // rows grouped by species
-    const int nrb = (n + RB - 1) / RB;
-    DHP_LAUNCH(ctx, k_species_hist, nrb, RB, 0, ctx->spos, n, ctx->blk_hist);
-    DHP_LAUNCH(ctx, k_species_scan, 1, 32 * NSP, 0, ctx->blk_hist, nrb, ctx->sp_count, ctx->sp_start);
-    DHP_LAUNCH(ctx, k_species_rank, nrb, RB, 0, ctx->spos, n, ctx->blk_hist, ctx->sp_start, ctx->rowmap,
-               ctx->row_species, ctx->row_slot);
     // pair list
     const double rcr2 = rcr * rcr, rca2 = rca * rca;
     bool wrap = false;     // same rule as k_setup_grid: a periodic axis with fewer than 3 cells
@@ -674,7 +689,13 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
                    ctx->tmp_stride, ctx->n_rad, ctx->tmp_col, ctx->blk_sum, ctx->status);
     DHP_LAUNCH(ctx, k_scan_blocks, 1, 1024, 0, ctx->blk_sum, ctx->blk_off, nblk, ctx->pair_cap, ctx->status);
     DHP_LAUNCH(ctx, k_rows, nblk, P2_THREADS, 0, ctx->tmp_col, ctx->tmp_stride, ctx->n_rad, ctx->blk_off, nblk, n, ctx->row_ptr,
-               ctx->col, ctx->n_rad, ctx->n_ang, ctx->seg_cnt, ctx->rowmap, ctx->tile_mask);
+               ctx->col, ctx->n_rad, ctx->n_ang, ctx->seg_cnt, ctx->amask);
+    // rows grouped by species, ordered by feature-block class inside a group; tile masks
+    const int nrb = (n + RB - 1) / RB;
+    DHP_LAUNCH(ctx, k_rowkey_hist, nrb, RB, 0, ctx->spos, ctx->amask, n, nrb, ctx->blk_hist);
+    DHP_LAUNCH(ctx, k_rowkey_scan, 1, 1024, 0, ctx->blk_hist, nrb, ctx->sp_count, ctx->sp_start, ctx->key_start);
+    DHP_LAUNCH(ctx, k_rowkey_rank, nrb, RB, 0, ctx->spos, ctx->amask, n, nrb, ctx->blk_hist, ctx->key_start, ctx->rowmap,
+               ctx->row_species, ctx->row_slot, ctx->tile_mask);
     DHP_CUDA(ctx, cudaGetLastError());
     return DHP_OK;
 }

@@ -279,6 +279,22 @@ def test_error_codes(torch, B, params, blob8):
     d.close()
 
 
+def test_rows_are_ordered_by_feature_block_class(torch, B, params, blob8):
+    """Work accounting of the block-skipping GEMMs: a water-only system touches 3 of the 16 feature blocks in every
+    tile (HH+HO, OO+HC, radial); in the mixed box rows are ordered by block class inside a species group, so the mean
+    number of active blocks per tile stays well below the all-species count."""
+    s = W.make_system(1)
+    d, _, _ = run_gpu(B, torch, s, params, blob8)
+    tiles, blocks = d.dhp_debug_tile_blocks()
+    assert tiles == 3 and blocks == 9                      # 192 H -> 2 tiles, 96 O -> 1 tile
+    d.close()
+    s = W.make_system(3)
+    d, _, _ = run_gpu(B, torch, s, params, blob8)
+    tiles, blocks = d.dhp_debug_tile_blocks()
+    assert tiles >= 23558 // 128 and 3.0 <= blocks / tiles <= 8.0
+    d.close()
+
+
 def test_launch_counter_and_profile(torch, B, params, blob8):
     s = SYSTEMS["mix600"]()
     d = make_ctx(B, s, params)
