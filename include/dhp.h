@@ -73,7 +73,9 @@ typedef struct dhp_weights dhp_weights; /* device-resident network parameters, o
 enum {
     DHP_MLP_AUTO = 0,   /* tensor path when available, else SIMT                                   */
     DHP_MLP_SIMT = 1,   /* fp32 FFMA GEMMs                                                          */
-    DHP_MLP_TENSOR = 2  /* tcgen05 / TMEM GEMMs, fp16 two-term split operands, fp32 accumulate      */
+    DHP_MLP_TENSOR = 2, /* tcgen05 / TMEM GEMMs, fp16 two-term split operands, fp32 accumulate; the four
+                           middle GEMMs of the chain fused into one kernel (activations stay on chip)   */
+    DHP_MLP_TENSOR_LAYERWISE = 3 /* same arithmetic, one launch per GEMM (bring-up / comparison path)   */
 };
 
 /* Phases timed by dhp_profile_* (CUDA events on the context stream). */

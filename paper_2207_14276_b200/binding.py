@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(HERE, "libdhp.so")
 
 N_PHASES = 4
 PHASES = ("nlist", "aev_fwd", "mlp", "aev_bwd")
-MLP_AUTO, MLP_SIMT, MLP_TENSOR = 0, 1, 2
+MLP_AUTO, MLP_SIMT, MLP_TENSOR, MLP_TENSOR_LAYERWISE = 0, 1, 2, 3
 OK = 0
 
 # every symbol include/dhp.h declares: (name, restype, argtypes)

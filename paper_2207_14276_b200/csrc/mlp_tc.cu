@@ -519,6 +519,347 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     if (warp == 1) tmem_dealloc(tmem_base, TMEM_COLS);
 }
 
+// ======================================================================================================
+// Fused middle of the chain.  G2, G3, B3 and B2 are small GEMMs whose split-fp16 activations (4 B per element)
+// cost more HBM time than MMA time when every layer is its own launch (profiles/r1c: 66-81 % DRAM).  Here one
+// work item = (row tile, network) runs   h1 -> h2 -> (E_i, d3) -> d2 -> d1   inside one CTA:
+//   * h2, d3 and d2 never leave the SM: the epilogue warps write each of them as the no-swizzle K-major A operand
+//     of the next GEMM into ONE 96 KB shared-memory region X (each is produced only after every MMA that reads its
+//     predecessor has completed);
+//   * CELU'(z2), needed again by B3's epilogue after X has been overwritten, is parked in spare TMEM columns
+//     (tcgen05.st / tcgen05.ld, fp32, 192 columns);
+//   * weights stream from L2 as pre-tiled images (the exact shared-memory image of one 16-wide K step of one GEMM,
+//     hi plane then lo plane, fetched by one plain cp.async.bulk; no tensor map) through a ring of 6 x 20 KB slots;
+//     h1 (tiled activation layout) streams through the same slots.
+// TMEM: RA = columns [0,256): the CELU'(z2) stash, then B2's accumulator; RB = [256,448): accumulator of G2, G3, B3.
+// The next item's G2 MMAs (into RB) overlap this item's B2 epilogue (reading RA).
+// ======================================================================================================
+constexpr int MID_SLOTS = 6;
+constexpr int MID_SLOT_BYTES = 20480;
+constexpr int MID_A_OFF = 12288;                 // G2 slots: W2 image of the K step (12 KB), then h1 hi (4 KB), h1 lo (4 KB)
+constexpr int MID_X_PLANE = BM * H2 * 2;         // 48 KB per plane
+constexpr int MID_X_BYTES = 2 * MID_X_PLANE;
+constexpr int MID_SMEM = MID_X_BYTES + MID_SLOTS * MID_SLOT_BYTES + 1024 /*align*/ + 256 /*barriers, TMEM word, ring*/;
+constexpr uint32_t MID_RA = 0, MID_RB = 256;
+// weight image of one (species, network), in halves: per GEMM [K step][plane][8-column group (2)][n][8]
+constexpr int MID_W_G2 = 0;
+constexpr int MID_W_G3 = MID_W_G2 + (H1 / 16) * 32 * H2;
+constexpr int MID_W_B3 = MID_W_G3 + (H2 / 16) * 32 * H3;
+constexpr int MID_W_B2 = MID_W_B3 + (H3 / 16) * 32 * H2;
+constexpr int MID_W_TOTAL = MID_W_B2 + (H2 / 16) * 32 * H1;
+
+struct MidArgs {
+    const int* row_species;
+    const int* sp_start;
+    int n_models;
+    int plane_tiles;          // row tiles per plane of the activation buffers
+    const __half* h1;         // tiled activation planes, n_models*4 64-column blocks per row tile
+    __half* d1;               // same geometry
+    const __half* wimg;       // [species][network][MID_W_TOTAL]
+    const float *b2, *b3, *w4, *b4;
+    float inv_models, alpha;
+    float* e_atom;
+    int* sched;
+};
+
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
+        "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};"
+        ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]),
+          "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]),
+          "r"(v[16]), "r"(v[17]), "r"(v[18]), "r"(v[19]), "r"(v[20]), "r"(v[21]), "r"(v[22]), "r"(v[23]),
+          "r"(v[24]), "r"(v[25]), "r"(v[26]), "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31])
+        : "memory");
+}
+__device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// K-major operand without swizzle, [8-column group][row][16 B]: leading byte offset = next group (rows * 16), stride
+// byte offset (next 8 rows) 128
+__device__ __forceinline__ uint64_t make_desc_ns(uint32_t saddr, uint32_t lbo_bytes) {
+    uint64_t d = 0;
+    d |= (uint64_t)((saddr & 0x3FFFF) >> 4);
+    d |= (uint64_t)(lbo_bytes >> 4) << 16;
+    d |= (uint64_t)(128 >> 4) << 32;
+    d |= (uint64_t)1 << 46;
+    return d;
+}
+
+// 32 consecutive columns c0.. of row r -> hi / lo planes of X
+__device__ __forceinline__ void store_split32_x(const float (&x)[32], uint8_t* xp, int c0, int r_in) {
+    uint32_t ph[16], pl[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) split_pair(x[2 * i], x[2 * i + 1], ph[i], pl[i]);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        uint8_t* dst = xp + (size_t)(((c0 >> 3) + i) * BM + r_in) * 16;
+        *reinterpret_cast<uint4*>(dst) = make_uint4(ph[4 * i], ph[4 * i + 1], ph[4 * i + 2], ph[4 * i + 3]);
+        *reinterpret_cast<uint4*>(dst + MID_X_PLANE) = make_uint4(pl[4 * i], pl[4 * i + 1], pl[4 * i + 2], pl[4 * i + 3]);
+    }
+}
+
+__global__ void __launch_bounds__(TC_THREADS, 1)
+k_mlp_mid(const MidArgs p) {
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t raw = smem_u32(smem_raw);
+    const uint32_t base = (raw + 1023u) & ~1023u;
+    uint8_t* x_ptr = smem_raw + (base - raw);                         // X region (generic pointer), xs its shared address
+    const uint32_t xs = base;
+    const uint32_t slots = base + MID_X_BYTES;
+    const uint32_t bar0 = slots + MID_SLOTS * MID_SLOT_BYTES;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(x_ptr + MID_X_BYTES + MID_SLOTS * MID_SLOT_BYTES);
+    // barriers: full[SLOTS], empty[SLOTS], acc_b, acc_a, x_ready, sfull[RING], sempty[RING]; then TMEM word and item ring
+    constexpr int NBARS = 2 * MID_SLOTS + 3 + 2 * RING;
+    auto full_bar = [&](int s) { return bar0 + 8u * s; };
+    auto empty_bar = [&](int s) { return bar0 + 8u * (MID_SLOTS + s); };
+    const uint32_t accb_bar = bar0 + 8u * (2 * MID_SLOTS), acca_bar = accb_bar + 8u, xready_bar = accb_bar + 16u;
+    auto sfull_bar = [&](int s) { return bar0 + 8u * (2 * MID_SLOTS + 3 + s); };
+    auto sempty_bar = [&](int s) { return bar0 + 8u * (2 * MID_SLOTS + 3 + RING + s); };
+    volatile uint32_t* tmem_word = reinterpret_cast<volatile uint32_t*>(bars + NBARS);
+    volatile int* ring = reinterpret_cast<volatile int*>(bars + NBARS + 1);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int M = p.n_models;
+    const int total_items = (p.sp_start[NSP] / BM) * M;
+
+    if (warp == 0 && lane == 0) {
+        for (int s = 0; s < MID_SLOTS; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+        mbar_init(accb_bar, 1); mbar_init(acca_bar, 1); mbar_init(xready_bar, EPI_WARPS);
+        for (int s = 0; s < RING; ++s) { mbar_init(sfull_bar(s), 1); mbar_init(sempty_bar(s), 1 + EPI_WARPS); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 1) tmem_alloc(smem_u32((const void*)tmem_word), TMEM_COLS);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_word;
+
+    if (warp == 0) {
+        // ===== item scheduler + producer =====
+        if (elect_one()) {
+            int slot = 0; uint32_t phase = 0;
+            int rs = 0; uint32_t rphase = 0;
+            auto next_slot = [&]() -> uint32_t {
+                mbar_wait(empty_bar(slot), phase ^ 1u);
+                return slots + (uint32_t)slot * MID_SLOT_BYTES;
+            };
+            auto advance = [&]() { if (++slot == MID_SLOTS) { slot = 0; phase ^= 1u; } };
+            for (;;) {
+                int item = atomicAdd(p.sched, 1);
+                if (item >= total_items) item = -1;
+                mbar_wait(sempty_bar(rs), rphase ^ 1u);
+                ring[rs] = item;
+                mbar_arrive(sfull_bar(rs));
+                if (++rs == RING) { rs = 0; rphase ^= 1u; }
+                if (item < 0) break;
+                const int rt = item / M, e = item - rt * M;
+                const int s = max(p.row_species[rt * BM], 0);
+                const __half* w = p.wimg + (size_t)(s * M + e) * MID_W_TOTAL;
+                for (int j = 0; j < H1 / 16; ++j) {                       // G2: W2 K step + the matching 16 columns of h1
+                    const uint32_t sa = next_slot();
+                    mbar_expect_tx(full_bar(slot), 32u * H2 * 2u + 8192u);
+                    bulk_load(sa, w + MID_W_G2 + (size_t)j * 32 * H2, 32u * H2 * 2u, full_bar(slot));
+                    const size_t goff = (size_t)((j & 3) * 2) * BM * 8;
+                    bulk_load(sa + MID_A_OFF, p.h1 + tile_off(p.plane_tiles, M * 4, 0, rt, e * 4 + (j >> 2)) + goff, 4096u, full_bar(slot));
+                    bulk_load(sa + MID_A_OFF + 4096, p.h1 + tile_off(p.plane_tiles, M * 4, 1, rt, e * 4 + (j >> 2)) + goff, 4096u,
+                              full_bar(slot));
+                    advance();
+                }
+                for (int j = 0; j < H2 / 16; ++j) {                       // G3
+                    const uint32_t sa = next_slot();
+                    mbar_expect_tx(full_bar(slot), 32u * H3 * 2u);
+                    bulk_load(sa, w + MID_W_G3 + (size_t)j * 32 * H3, 32u * H3 * 2u, full_bar(slot));
+                    advance();
+                }
+                for (int j = 0; j < H3 / 16; ++j) {                       // B3
+                    const uint32_t sa = next_slot();
+                    mbar_expect_tx(full_bar(slot), 32u * H2 * 2u);
+                    bulk_load(sa, w + MID_W_B3 + (size_t)j * 32 * H2, 32u * H2 * 2u, full_bar(slot));
+                    advance();
+                }
+                for (int j = 0; j < H2 / 16; ++j) {                       // B2
+                    const uint32_t sa = next_slot();
+                    mbar_expect_tx(full_bar(slot), 32u * H1 * 2u);
+                    bulk_load(sa, w + MID_W_B2 + (size_t)j * 32 * H1, 32u * H1 * 2u, full_bar(slot));
+                    advance();
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer =====
+        if (elect_one()) {
+            int slot = 0; uint32_t phase = 0;
+            int rs = 0; uint32_t rphase = 0;
+            uint32_t xphase = 0;
+            // one GEMM: `steps` K steps of 16, B (n x 16, hi plane then lo plane) from the slot, A from the slot (G2) or from X
+            auto run = [&](int n, int steps, bool a_in_slot, uint32_t d_tmem) {
+                const uint32_t idesc = make_idesc(n);
+                const uint32_t lbo_b = (uint32_t)n * 16u;
+                uint32_t accumulate = 0u;
+                for (int j = 0; j < steps; ++j) {
+                    mbar_wait(full_bar(slot), phase);
+                    tc_fence_after();
+                    const uint32_t sa = slots + (uint32_t)slot * MID_SLOT_BYTES;
+                    const uint64_t b_hi = make_desc_ns(sa, lbo_b), b_lo = make_desc_ns(sa + 2u * lbo_b, lbo_b);
+                    const uint32_t a0 = a_in_slot ? sa + MID_A_OFF : xs + (uint32_t)j * 4096u;
+                    const uint64_t a_hi = make_desc_ns(a0, 2048u);
+                    const uint64_t a_lo = make_desc_ns(a0 + (a_in_slot ? 4096u : (uint32_t)MID_X_PLANE), 2048u);
+                    umma_f16(d_tmem, a_hi, b_hi, idesc, accumulate);
+                    umma_f16(d_tmem, a_hi, b_lo, idesc, 1u);
+                    umma_f16(d_tmem, a_lo, b_hi, idesc, 1u);
+                    accumulate = 1u;
+                    umma_commit(empty_bar(slot));
+                    if (++slot == MID_SLOTS) { slot = 0; phase ^= 1u; }
+                }
+            };
+            auto wait_x = [&]() { mbar_wait(xready_bar, xphase); xphase ^= 1u; tc_fence_after(); };
+            for (;;) {
+                mbar_wait(sfull_bar(rs), rphase);
+                const int item = ring[rs];
+                mbar_arrive(sempty_bar(rs));
+                if (++rs == RING) { rs = 0; rphase ^= 1u; }
+                if (item < 0) break;
+                run(H2, H1 / 16, true, tmem_base + MID_RB);  umma_commit(accb_bar);     // G2
+                wait_x();
+                run(H3, H2 / 16, false, tmem_base + MID_RB); umma_commit(accb_bar);     // G3
+                wait_x();
+                run(H2, H3 / 16, false, tmem_base + MID_RB); umma_commit(accb_bar);     // B3
+                wait_x();
+                run(H1, H2 / 16, false, tmem_base + MID_RA); umma_commit(acca_bar);     // B2
+            }
+        }
+    } else {
+        // ===== epilogue warps =====
+        const int q = warp & 3, half = (warp - 2) >> 2;
+        const int r_in = q * 32 + lane;
+        const uint32_t lane_base = tmem_base + ((uint32_t)(q * 32) << 16);
+        int rs = 0; uint32_t rphase = 0;
+        uint32_t bphase = 0, aphase = 0;
+        const float kexp = 1.4426950408889634f / p.alpha, inv_alpha = 1.0f / p.alpha;
+        const float sc = 1.0f / W_SCALE;
+        auto publish_x = [&]() {           // X written by this warp is visible to the tensor core, accumulator reads are done
+            fence_proxy_async_smem();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(xready_bar);
+        };
+        for (;;) {
+            mbar_wait(sfull_bar(rs), rphase);
+            const int item = ring[rs];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(sempty_bar(rs));
+            if (++rs == RING) { rs = 0; rphase ^= 1u; }
+            if (item < 0) break;
+            const int rt = item / M, e = item - rt * M;
+            const int s = max(p.row_species[rt * BM], 0);
+            const int row = rt * BM + r_in;
+            uint32_t v[32];
+            float x[32], aux[32];
+            // ---- G2: h2 = CELU(acc / 64 + b2) -> X; CELU'(z2) -> TMEM stash
+            mbar_wait(accb_bar, bphase); bphase ^= 1u;
+            tc_fence_after();
+            for (int c0 = half * 32; c0 < H2; c0 += 64) {
+                tmem_ld32_issue(lane_base + MID_RB + (uint32_t)c0, v);
+                load32(p.b2 + (size_t)(s * M + e) * H2 + c0, aux);
+                tmem_ld_wait();
+#pragma unroll
+                for (int i = 0; i < 32; ++i) x[i] = celu_f(fmaf(__uint_as_float(v[i]), sc, aux[i]), p.alpha, kexp);
+                store_split32_x(x, x_ptr, c0, r_in);
+#pragma unroll
+                for (int i = 0; i < 32; ++i) v[i] = __float_as_uint(dcelu_from_h(x[i], inv_alpha));
+                tmem_st32(lane_base + MID_RA + (uint32_t)c0, v);
+            }
+            tmem_st_wait();
+            publish_x();
+            // ---- G3: h3 = CELU(acc / 64 + b3); E_i += (w4.h3 + b4)/M; d3 = w4 CELU'(z3) 2^10 / M -> X
+            mbar_wait(accb_bar, bphase); bphase ^= 1u;
+            tc_fence_after();
+            float e_acc = 0.f;
+            const float dsc = p.inv_models * D_SCALE;
+            for (int c0 = half * 32; c0 < H3; c0 += 64) {
+                tmem_ld32_issue(lane_base + MID_RB + (uint32_t)c0, v);
+                load32(p.b3 + (size_t)(s * M + e) * H3 + c0, aux);
+                tmem_ld_wait();
+#pragma unroll
+                for (int i = 0; i < 32; ++i) x[i] = celu_f(fmaf(__uint_as_float(v[i]), sc, aux[i]), p.alpha, kexp);
+                load32(p.w4 + (size_t)(s * M + e) * H3 + c0, aux);
+#pragma unroll
+                for (int i = 0; i < 32; ++i) {
+                    e_acc = fmaf(aux[i], x[i], e_acc);
+                    x[i] = aux[i] * dsc * dcelu_from_h(x[i], inv_alpha);
+                }
+                store_split32_x(x, x_ptr, c0, r_in);
+            }
+            atomicAdd(&p.e_atom[row], (e_acc + (half == 0 ? p.b4[s * M + e] : 0.f)) * p.inv_models);
+            publish_x();
+            // ---- B3: d2 = (acc / 64) CELU'(z2) -> X
+            mbar_wait(accb_bar, bphase); bphase ^= 1u;
+            tc_fence_after();
+            for (int c0 = half * 32; c0 < H2; c0 += 64) {
+                uint32_t st[32];
+                tmem_ld32_issue(lane_base + MID_RB + (uint32_t)c0, v);
+                tmem_ld32_issue(lane_base + MID_RA + (uint32_t)c0, st);
+                tmem_ld_wait();
+#pragma unroll
+                for (int i = 0; i < 32; ++i) x[i] = __uint_as_float(v[i]) * sc * __uint_as_float(st[i]);
+                store_split32_x(x, x_ptr, c0, r_in);
+            }
+            publish_x();
+            // ---- B2: d1 = (acc / 64) CELU'(z1) -> global (tiled planes), CELU' from the saved h1
+            mbar_wait(acca_bar, aphase); aphase ^= 1u;
+            tc_fence_after();
+            for (int c0 = half * 32; c0 < H1; c0 += 64) {
+                tmem_ld32_issue(lane_base + MID_RA + (uint32_t)c0, v);
+                const size_t in_tile = (size_t)(((c0 & 63) >> 3) * BM + r_in) * 8;
+                const size_t o_hi = tile_off(p.plane_tiles, M * 4, 0, rt, e * 4 + (c0 >> 6)) + in_tile;
+                const size_t o_lo = tile_off(p.plane_tiles, M * 4, 1, rt, e * 4 + (c0 >> 6)) + in_tile;
+                load_joined32_tiled(p.h1 + o_hi, p.h1 + o_lo, aux);
+                tmem_ld_wait();
+#pragma unroll
+                for (int i = 0; i < 32; ++i) x[i] = __uint_as_float(v[i]) * sc * dcelu_from_h(aux[i], inv_alpha);
+                store_split32_tiled(x, p.d1 + o_hi, p.d1 + o_lo);
+            }
+            tc_fence_before();
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) tmem_dealloc(tmem_base, TMEM_COLS);
+}
+
+// weight images for k_mlp_mid: img[(s*M + e)][MID_W_TOTAL], see the layout above
+__global__ void k_prep_mid(const float* __restrict__ blob, int n_models, __half* __restrict__ img) {
+    const int se = blockIdx.y;                      // s * n_models + e
+    const int s = se / n_models, e = se - s * n_models;
+    const float* net = blob + (size_t)(e * NSP + s) * NET_PARAMS;
+    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < MID_W_TOTAL; idx += gridDim.x * blockDim.x) {
+        int n_rows, rem, mode;
+        if (idx < MID_W_G3) { mode = 0; n_rows = H2; rem = idx - MID_W_G2; }
+        else if (idx < MID_W_B3) { mode = 1; n_rows = H3; rem = idx - MID_W_G3; }
+        else if (idx < MID_W_B2) { mode = 2; n_rows = H2; rem = idx - MID_W_B3; }
+        else { mode = 3; n_rows = H1; rem = idx - MID_W_B2; }
+        const int step = rem / (32 * n_rows);
+        rem -= step * 32 * n_rows;
+        const int plane = rem / (16 * n_rows);
+        rem -= plane * 16 * n_rows;
+        const int g = rem / (8 * n_rows);
+        rem -= g * 8 * n_rows;
+        const int n = rem >> 3, k = 16 * step + 8 * g + (rem & 7);
+        float v;
+        switch (mode) {
+            case 0: v = net[OFF_W2 + n * H1 + k]; break;       // B(n,k) = W2[n][k]
+            case 1: v = net[OFF_W3 + n * H2 + k]; break;       // W3[n][k]
+            case 2: v = net[OFF_W3 + k * H2 + n]; break;       // W3[k][n]
+            default: v = net[OFF_W2 + k * H1 + n]; break;      // W2[k][n]
+        }
+        __half hi, lo;
+        split_half(v * W_SCALE, hi, lo);
+        img[(size_t)se * MID_W_TOTAL + idx] = plane ? lo : hi;
+    }
+}
+
 // ---- operand preparation -------------------------------------------------------------------------------
 // fp32 rows -> hi / lo fp16 planes (AEV rows for G1)
 __global__ void k_split_rows(const float* __restrict__ src, int ld_src, const int* __restrict__ sp_start, int ncol,
@@ -620,6 +961,7 @@ struct TcWorkspace {                  // per context
 };
 struct TcWeights {                    // per weight handle
     __half *w1f, *w2f, *w3f, *w3b, *w2b, *w1b;
+    __half* wmid;                                   // k_mlp_mid weight images [species][network][MID_W_TOTAL]
     float *b1, *b2, *b3, *w4, *b4;
     CUtensorMap m_w1f, m_w2f, m_w3f, m_w3b, m_w2b, m_w1b;
 };
@@ -682,6 +1024,8 @@ int mlp_tc_weights(Ctx* ctx, Weights* wt) {
         DHP_LAUNCH(ctx, k_prep_weights, dim3(256, NSP), 256, 0, wt->blob, M, m.mode, m.rows, m.cols, *m.p);
         if (!make_map(m.m, *m.p, (uint64_t)2 * NSP * m.rows, m.cols, m.box_rows)) return DHP_E_CUDA;
     }
+    if (cudaMalloc((void**)&t->wmid, (size_t)NSP * M * MID_W_TOTAL * sizeof(__half)) != cudaSuccess) return DHP_E_NOMEM;
+    DHP_LAUNCH(ctx, k_prep_mid, dim3(64, NSP * M), 256, 0, wt->blob, M, t->wmid);
     float** smalls[] = {&t->b1, &t->b2, &t->b3, &t->w4, &t->b4};
     const size_t sizes[] = {(size_t)NSP * M * H1, (size_t)NSP * M * H2, (size_t)NSP * M * H3, (size_t)NSP * M * H3, (size_t)NSP * M};
     for (int i = 0; i < 5; ++i)
@@ -695,7 +1039,7 @@ int mlp_tc_weights(Ctx* ctx, Weights* wt) {
 void mlp_tc_weights_free(Ctx*, Weights* wt) {
     TcWeights* t = (TcWeights*)wt->tc;
     if (!t) return;
-    void* ptrs[] = {t->w1f, t->w2f, t->w3f, t->w3b, t->w2b, t->w1b, t->b1, t->b2, t->b3, t->w4, t->b4};
+    void* ptrs[] = {t->w1f, t->w2f, t->w3f, t->w3b, t->w2b, t->w1b, t->wmid, t->b1, t->b2, t->b3, t->w4, t->b4};
     for (void* p : ptrs) if (p) cudaFree(p);
     delete t;
     wt->tc = nullptr;
@@ -725,30 +1069,44 @@ int mlp_tc(Ctx* ctx, const Weights* wt) {
     a.a_tiled = nullptr; a.out_planes = ws->h1; a.out_kblocks = M * KB1; a.out_cols_per_tile = H1;
     a.sched = ctx->tc_sched + 0;
     if ((rc = launch_gemm<EPI_CELU, CMP_K>(ctx, ws->m_aev, t->m_w1f, a)) != DHP_OK) return rc;
-    // G2: h1 -> h2
-    a.K = H1; a.BN = H2; a.b_rows_per_species = M * H2; a.b_rows_per_tile = H2; a.bias = t->b2;
-    a.a_tiled = ws->h1; a.a_kblocks = M * KB1; a.a_kb_per_tile = KB1;
-    a.out_planes = ws->h2; a.out_kblocks = M * KB2; a.out_cols_per_tile = H2;
-    a.sched = ctx->tc_sched + 1;
-    if ((rc = launch_gemm<EPI_CELU, CMP_NONE>(ctx, ws->m_aev, t->m_w2f, a)) != DHP_OK) return rc;
-    // G3 + output layer + seed of the backward pass: h2 -> d3
-    a.K = H2; a.BN = H3; a.b_rows_per_species = M * H3; a.b_rows_per_tile = H3; a.bias = t->b3;
-    a.a_tiled = ws->h2; a.a_kblocks = M * KB2; a.a_kb_per_tile = KB2;
-    a.out_planes = ws->d3; a.out_kblocks = M * KB2; a.out_cols_per_tile = H2;
-    a.sched = ctx->tc_sched + 2;
-    if ((rc = launch_gemm<EPI_OUT, CMP_NONE>(ctx, ws->m_aev, t->m_w3f, a)) != DHP_OK) return rc;
-    // B3: d3 -> d2
-    a.K = H3; a.BN = H2; a.b_rows_per_species = M * H2; a.b_rows_per_tile = H2;
-    a.a_tiled = ws->d3; a.a_kblocks = M * KB2; a.a_kb_per_tile = KB2;
-    a.h_planes = ws->h2; a.out_planes = ws->d2; a.out_kblocks = M * KB2; a.out_cols_per_tile = H2;
-    a.sched = ctx->tc_sched + 3;
-    if ((rc = launch_gemm<EPI_DCELU, CMP_NONE>(ctx, ws->m_aev, t->m_w3b, a)) != DHP_OK) return rc;
-    // B2: d2 -> d1
-    a.K = H2; a.BN = H1; a.b_rows_per_species = M * H1; a.b_rows_per_tile = H1;
-    a.a_tiled = ws->d2; a.a_kblocks = M * KB2; a.a_kb_per_tile = KB2;
-    a.h_planes = ws->h1; a.out_planes = ws->d1; a.out_kblocks = M * KB1; a.out_cols_per_tile = H1;
-    a.sched = ctx->tc_sched + 4;
-    if ((rc = launch_gemm<EPI_DCELU, CMP_NONE>(ctx, ws->m_aev, t->m_w2b, a)) != DHP_OK) return rc;
+    if (ctx->mlp_mode != DHP_MLP_TENSOR_LAYERWISE) {
+        // G2 .. B2 fused: h1 -> d1 with h2, d3, d2 kept on chip
+        static bool attr = false;
+        if (!attr) {
+            DHP_CUDA(ctx, cudaFuncSetAttribute(k_mlp_mid, cudaFuncAttributeMaxDynamicSharedMemorySize, MID_SMEM));
+            attr = true;
+        }
+        MidArgs m{};
+        m.row_species = ctx->row_species; m.sp_start = ctx->sp_start; m.n_models = M; m.plane_tiles = R / BM;
+        m.h1 = ws->h1; m.d1 = ws->d1; m.wimg = t->wmid; m.b2 = t->b2; m.b3 = t->b3; m.w4 = t->w4; m.b4 = t->b4;
+        m.inv_models = 1.0f / (float)M; m.alpha = ctx->params.celu_alpha; m.e_atom = ctx->e_atom; m.sched = ctx->tc_sched + 1;
+        DHP_LAUNCH(ctx, k_mlp_mid, ctx->sm_count, TC_THREADS, MID_SMEM, m);
+    } else {
+        // G2: h1 -> h2
+        a.K = H1; a.BN = H2; a.b_rows_per_species = M * H2; a.b_rows_per_tile = H2; a.bias = t->b2;
+        a.a_tiled = ws->h1; a.a_kblocks = M * KB1; a.a_kb_per_tile = KB1;
+        a.out_planes = ws->h2; a.out_kblocks = M * KB2; a.out_cols_per_tile = H2;
+        a.sched = ctx->tc_sched + 1;
+        if ((rc = launch_gemm<EPI_CELU, CMP_NONE>(ctx, ws->m_aev, t->m_w2f, a)) != DHP_OK) return rc;
+        // G3 + output layer + seed of the backward pass: h2 -> d3
+        a.K = H2; a.BN = H3; a.b_rows_per_species = M * H3; a.b_rows_per_tile = H3; a.bias = t->b3;
+        a.a_tiled = ws->h2; a.a_kblocks = M * KB2; a.a_kb_per_tile = KB2;
+        a.out_planes = ws->d3; a.out_kblocks = M * KB2; a.out_cols_per_tile = H2;
+        a.sched = ctx->tc_sched + 2;
+        if ((rc = launch_gemm<EPI_OUT, CMP_NONE>(ctx, ws->m_aev, t->m_w3f, a)) != DHP_OK) return rc;
+        // B3: d3 -> d2
+        a.K = H3; a.BN = H2; a.b_rows_per_species = M * H2; a.b_rows_per_tile = H2;
+        a.a_tiled = ws->d3; a.a_kblocks = M * KB2; a.a_kb_per_tile = KB2;
+        a.h_planes = ws->h2; a.out_planes = ws->d2; a.out_kblocks = M * KB2; a.out_cols_per_tile = H2;
+        a.sched = ctx->tc_sched + 3;
+        if ((rc = launch_gemm<EPI_DCELU, CMP_NONE>(ctx, ws->m_aev, t->m_w3b, a)) != DHP_OK) return rc;
+        // B2: d2 -> d1
+        a.K = H2; a.BN = H1; a.b_rows_per_species = M * H1; a.b_rows_per_tile = H1;
+        a.a_tiled = ws->d2; a.a_kblocks = M * KB2; a.a_kb_per_tile = KB2;
+        a.h_planes = ws->h1; a.out_planes = ws->d1; a.out_kblocks = M * KB1; a.out_cols_per_tile = H1;
+        a.sched = ctx->tc_sched + 4;
+        if ((rc = launch_gemm<EPI_DCELU, CMP_NONE>(ctx, ws->m_aev, t->m_w2b, a)) != DHP_OK) return rc;
+    }
     // B1: d1 (all models along K) -> dE/dAEV, only the feature blocks that are active for the row tile
     a.K = M * H1; a.BN = 256; a.n_tiles = AEV_LD / 256; a.b_rows_per_species = AEV_LD; a.b_rows_per_tile = 256;
     a.a_tiled = ws->d1; a.a_kblocks = M * KB1; a.a_kb_per_tile = 0;

@@ -123,11 +123,11 @@ def mlp_modes(B):
 
 
 @pytest.mark.parametrize("name", ["water96", "ligand50", "mix600", "replicas16"])
-@pytest.mark.parametrize("mode", [1, 2])
+@pytest.mark.parametrize("mode", [1, 2, 3])
 def test_energy_forces_small(torch, B, params, blob8, name, mode):
     s = SYSTEMS[name]()
     probe = make_ctx(B, s, params)
-    if mode == B.MLP_TENSOR and not probe.dhp_tensor_path_available():
+    if mode >= B.MLP_TENSOR and not probe.dhp_tensor_path_available():
         probe.close()
         pytest.skip("tensor path not available in this build")
     probe.close()
