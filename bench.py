@@ -34,7 +34,10 @@ from paper_2207_14276_b200 import workloads as W  # noqa: E402
 METRIC = "ani_energy_forces_atoms_evals_per_s"
 UNIT = "atoms*evals/s"
 NS_PER_DAY_PER_EVAL_PER_S = 0.5e-6 * 86400.0      # 0.5 fs step
-MLP_FLOP_PER_ATOM_NET = 2.0 * (1008 * 256 + 256 * 192 + 192 * 160 + 160) * 2.0   # forward + input-gradient
+# DRAM bytes (read + write) per launch at configs[3], from the committed ncu --set full captures of this command
+# (profiles/r1d_ncu_full_summary.txt: G1, k_mlp_mid, B1; profiles/r1c_ncu_full_summary.txt: the others)
+TRAFFIC_98K = {"g1": 0.17083e9 + 0.74936e9, "mid": 0.85889e9 + 0.76818e9, "b1": 0.83663e9 + 0.09485e9,
+               "aev_fwd": 0.02738e9 + 0.12718e9, "aev_bwd": 0.11340e9 + 0.00464e9, "nlist": 0.00236e9 + 0.00077e9 + 0.02743e9 + 0.00004e9}
 
 
 def peaks():
@@ -94,12 +97,16 @@ def oracle_sample_rate(system, params, blob, target_s: float = 15.0, seed: int =
     oracle.energy_forces(system.pos, system.species, system.box, params, blob, system.n_models, centres=centres,
                          mol_offsets=system.mol_offsets)
     dt = time.perf_counter() - t0
-    n = int(min(system.n_atoms, max(n_try, n_try * target_s / max(dt, 1e-3))))
-    centres = rng.choice(system.n_atoms, n, replace=False).astype(np.int32)
-    t0 = time.perf_counter()
-    oracle.energy_forces(system.pos, system.species, system.box, params, blob, system.n_models, centres=centres,
-                         mol_offsets=system.mol_offsets)
-    dt = time.perf_counter() - t0
+    n = n_try
+    for _ in range(3):          # the probe over-estimates the per-atom cost (thread start-up): refine until ~target_s
+        n = int(min(system.n_atoms, max(n_try, n * target_s / max(dt, 1e-3))))
+        centres = rng.choice(system.n_atoms, n, replace=False).astype(np.int32)
+        t0 = time.perf_counter()
+        oracle.energy_forces(system.pos, system.species, system.box, params, blob, system.n_models, centres=centres,
+                             mol_offsets=system.mol_offsets)
+        dt = time.perf_counter() - t0
+        if dt >= 0.6 * target_s or n == system.n_atoms:
+            break
     return n / dt, n, dt, oracle.num_threads()
 
 
@@ -254,41 +261,74 @@ def main():
         atoms_all = system.n_atoms * world
         value = atoms_all * args.steps / (ms_total * 1e-3)
         e2e_value = atoms_all * args.steps / (e2e_ms * 1e-3)
-        mlp_ms = phase_ms["mlp"] / max(calls, 1)
-        flops = MLP_FLOP_PER_ATOM_NET * system.n_models * system.n_atoms
-        achieved = flops / (mlp_ms * 1e-3) / 1e12
+        ph = {k: v / max(calls, 1) for k, v in phase_ms.items()}            # ms per launch, CUDA events on the ctx stream
+        ph["mlp"] = ph["mlp_g1"] + ph["mlp_mid"] + ph["mlp_b1"]
+        N, M = system.n_atoms, system.n_models
         passes = 3 if tensor_path else 1
-        # tensor work actually issued: G1 visits / B1 produces only the active 64-wide feature blocks of a 128-row tile
-        mid = 256 * 192 + 192 * 160 + 160 * 192 + 192 * 256
-        issued = passes * 2.0 * system.n_models * 128.0 * (2 * 64 * 256 * n_active_blocks + mid * n_row_tiles) \
-            if tensor_path else flops
-        issued_tflops = issued / (mlp_ms * 1e-3) / 1e12
-        roof = {"bound": "tensor", "kernel": "mlp phase (a3+a4: forward + transpose-backward GEMMs)",
-                "achieved": achieved, "peak": pk["bf16_tflops_sustained"], "unit": "TFLOP/s",
-                "frac": achieved / pk["bf16_tflops_sustained"], "traffic": None,
-                "peak_source": f"{pk['source']} sustained bf16 (fp16 operands, same rate)",
-                "algorithmic_flop_per_launch": flops, "ms_per_launch": mlp_ms,
-                "issued_tflops": issued_tflops, "issued_frac": issued_tflops / pk["bf16_tflops_sustained"],
-                "row_tiles": n_row_tiles, "active_feature_blocks_per_tile": n_active_blocks / max(n_row_tiles, 1),
-                "arithmetic": "fp16 two-term split, 3 tcgen05 MMAs per product, fp32 accumulate" if tensor_path
-                else "fp32 FFMA (SIMT scaffold; tensor path not built)"}
+        peak_t = pk["bf16_tflops_sustained"]
+        # algorithmic FLOPs (forward + input gradient) per atom and network, by kernel
+        f_g1 = 2.0 * 1008 * 256
+        f_mid = 2.0 * (256 * 192 + 192 * 160 + 160 + 160 * 192 + 192 * 256)
+        f_b1 = 2.0 * 256 * 1008
+        # MMAs actually issued: 3 passes; G1 visits / B1 produces only the active 64-wide feature blocks of a tile
+        rows_pad = 128.0 * n_row_tiles
+        i_g1 = passes * 2.0 * M * 128.0 * 64 * 256 * n_active_blocks
+        i_mid = passes * 2.0 * M * rows_pad * (256 * 192 + 192 * 160 + 160 * 192 + 192 * 256)
+
+        def tensor_entry(name, ms, alg_flop, issued_flop, traffic):
+            ach = alg_flop / (ms * 1e-3) / 1e12
+            return {"kernel": name, "bound": "tensor", "achieved": ach, "peak": peak_t, "unit": "TFLOP/s", "frac": ach / peak_t,
+                    "traffic": traffic, "ms_per_launch": ms, "algorithmic_flop_per_launch": alg_flop,
+                    "issued_tflops": issued_flop / (ms * 1e-3) / 1e12, "issued_frac": issued_flop / (ms * 1e-3) / 1e12 / peak_t}
+
+        def hbm_entry(name, ms, bytes_per_atom, traffic, note):
+            ach = bytes_per_atom * N / (ms * 1e-3) / 1e9
+            return {"kernel": name, "bound": "hbm", "achieved": ach, "peak": pk["hbm_gbs"], "unit": "GB/s",
+                    "frac": ach / pk["hbm_gbs"], "traffic": traffic, "ms_per_launch": ms,
+                    "algorithmic_bytes_per_launch": bytes_per_atom * N, "note": note}
+
+        # `traffic`: dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures of
+        # this same command (profiles/r1d_ncu_full_summary.txt for the MLP kernels, r1c for the others); configs[3] only
+        tr = TRAFFIC_98K if (args.config == 4 and tensor_path) else {}
+        kernels = []
+        if tensor_path:
+            kernels += [tensor_entry("k_gemm_tc<CELU,K-skip> (G1: AEV -> h1)", ph["mlp_g1"], f_g1 * M * N, i_g1, tr.get("g1")),
+                        tensor_entry("k_mlp_mid (G2+G3+out+B3+B2 fused: h1 -> E_i, d1)", ph["mlp_mid"], f_mid * M * N, i_mid, tr.get("mid")),
+                        tensor_entry("k_gemm_tc<GRAD,N-skip> (B1: d1 -> dE/dAEV) + energy reduction", ph["mlp_b1"], f_b1 * M * N, i_g1, tr.get("b1"))]
+        kernels += [hbm_entry("nlist (a1: all kernels)", ph["nlist"], 264.0, tr.get("nlist"), "working set is L2-resident; instruction-bound"),
+                    hbm_entry("k_aev_fwd (a2)", ph["aev_fwd"], 4256.0, tr.get("aev_fwd"), "issue-bound (3.1 k warp instructions per atom)"),
+                    hbm_entry("k_aev_bwd + k_unsort_forces (a5)", ph["aev_bwd"], 4268.0, tr.get("aev_bwd"), "issue-bound")]
+        if tensor_path:
+            roof = dict(max(kernels[:3], key=lambda k: k["ms_per_launch"]))          # the dominant kernel of the step
+            roof["peak_source"] = f"{pk['source']} sustained bf16 (fp16 operands, same rate)"
+            roof["arithmetic"] = "fp16 two-term split, 3 tcgen05 MMAs per product, fp32 accumulate"
+            mlp_phase = tensor_entry("MLP phase (G1 + k_mlp_mid + B1)", ph["mlp"], (f_g1 + f_mid + f_b1) * M * N, 2 * i_g1 + i_mid,
+                                     sum(tr.values()) if {"g1", "mid", "b1"} <= set(tr) else None)
+            mlp_phase["traffic"] = (tr["g1"] + tr["mid"] + tr["b1"]) if {"g1", "mid", "b1"} <= set(tr) else None
+            mlp_phase.update({"row_tiles": n_row_tiles, "active_feature_blocks_per_tile": n_active_blocks / max(n_row_tiles, 1)})
+        else:
+            flops = (f_g1 + f_mid + f_b1) * M * N
+            roof = tensor_entry("mlp_simt (fp32 FFMA scaffold; tensor path not in use)", ph["mlp"], flops, flops, None)
+            mlp_phase = roof
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": workload_name(args.config, system), "n_atoms": system.n_atoms,
                        "n_models": system.n_models, "parallelism": f"{world} independent replica(s), one per GPU",
-                       "l2": "per-step working set (AEV, dE/dAEV and activation buffers, > 1 GB) exceeds the 126 MB L2; "
+                       "l2": "per-step working set (AEV planes, dE/dAEV and activation buffers, > 1 GB) exceeds the 126 MB L2; "
                              "positions rotate over 4 jittered copies",
                        "mlp": "tensor" if tensor_path else "simt"},
             "ns_per_day_at_0.5fs": value / atoms_all * NS_PER_DAY_PER_EVAL_PER_S,   # per replica
             "evals_per_s_per_gpu": value / atoms_all,
-            "phase_ms": {k: v / max(calls, 1) for k, v in phase_ms.items()},
+            "phase_ms": ph,
             "gpu_launches": int(launches),
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "ms_per_step": e2e_ms / args.steps},
             "roofline": roof,
+            "roofline_mlp_phase": mlp_phase,
+            "roofline_kernels": kernels,
         }
         if world == 1 and not args.no_cpu_baseline:
             rate, n, dt, cores = oracle_sample_rate(system, params, blob)

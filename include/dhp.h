@@ -82,9 +82,11 @@ enum {
 enum {
     DHP_PHASE_NLIST = 0,   /* a1: binning, sort, CSR build                 */
     DHP_PHASE_AEV_FWD = 1, /* a2                                           */
-    DHP_PHASE_MLP = 2,     /* a3 + a4: forward and transpose-backward GEMMs */
-    DHP_PHASE_AEV_BWD = 3, /* a5 + force un-permutation                    */
-    DHP_N_PHASES = 4
+    DHP_PHASE_MLP_G1 = 2,  /* a3: first layer, AEV -> h1 (all of a3 + a4 on the SIMT path)           */
+    DHP_PHASE_MLP_MID = 3, /* a3 + a4: layers 2, 3, output, and their transposes, h1 -> (E_i, d1)    */
+    DHP_PHASE_MLP_B1 = 4,  /* a4: first-layer transpose, d1 -> dE/dAEV; energy reduction             */
+    DHP_PHASE_AEV_BWD = 5, /* a5 + force un-permutation                    */
+    DHP_N_PHASES = 6
 };
 
 /* Create a context.  max_atoms / max_mols bound every later call (workspace is allocated here, once;

@@ -16,8 +16,8 @@ import numpy as np
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libdhp.so")
 
-N_PHASES = 4
-PHASES = ("nlist", "aev_fwd", "mlp", "aev_bwd")
+N_PHASES = 6
+PHASES = ("nlist", "aev_fwd", "mlp_g1", "mlp_mid", "mlp_b1", "aev_bwd")
 MLP_AUTO, MLP_SIMT, MLP_TENSOR, MLP_TENSOR_LAYERWISE = 0, 1, 2, 3
 OK = 0
 

@@ -64,8 +64,8 @@ static int check_args(Ctx* ctx, const float* pos, const float* box, const int32_
     return DHP_OK;
 }
 
-static void prof_mark(Ctx* ctx, int slot, int phase) {
-    if (ctx->prof.on && slot >= 0) cudaEventRecord(ctx->prof.ev[slot][phase], ctx->stream);
+void prof_mark(Ctx* ctx, int boundary) {
+    if (ctx->prof.on && ctx->prof.cur_slot >= 0) cudaEventRecord(ctx->prof.ev[ctx->prof.cur_slot][boundary], ctx->stream);
 }
 
 static void prof_drain(Ctx* ctx) {
@@ -83,26 +83,33 @@ static void prof_drain(Ctx* ctx) {
 
 static int run_energy_forces(Ctx* ctx, const float* pos, const float* box, const int32_t* species, int64_t n,
                              const int32_t* mol_offsets, int64_t n_mol, const Weights* w, double* E, float* F) {
-    int slot = -1;
+    ctx->prof.cur_slot = -1;
     if (ctx->prof.on) {
         if (ctx->prof.n_pending == 64) prof_drain(ctx);
-        slot = ctx->prof.n_pending++;
+        ctx->prof.cur_slot = ctx->prof.n_pending++;
     }
     int rc;
-    prof_mark(ctx, slot, 0);
+    prof_mark(ctx, DHP_PHASE_NLIST);
     if ((rc = nlist_build(ctx, pos, box, species, n, mol_offsets, n_mol)) != DHP_OK) return rc;
-    prof_mark(ctx, slot, 1);
+    prof_mark(ctx, DHP_PHASE_AEV_FWD);
     const bool tensor = ctx->mlp_mode == DHP_MLP_TENSOR || ctx->mlp_mode == DHP_MLP_TENSOR_LAYERWISE ||
                         (ctx->mlp_mode == DHP_MLP_AUTO && w->tc != nullptr);
     if (tensor && !w->tc) return DHP_E_NOTIMPL;
     if ((rc = aev_forward(ctx, tensor && ctx->aev_planes != nullptr)) != DHP_OK) return rc;
-    prof_mark(ctx, slot, 2);
-    rc = tensor ? mlp_tc(ctx, w) : mlp_simt(ctx, w);
+    prof_mark(ctx, DHP_PHASE_MLP_G1);
+    if (tensor) {
+        rc = mlp_tc(ctx, w);                 // marks MLP_MID and MLP_B1 itself
+    } else {
+        rc = mlp_simt(ctx, w);
+        prof_mark(ctx, DHP_PHASE_MLP_MID);
+        prof_mark(ctx, DHP_PHASE_MLP_B1);
+    }
     if (rc != DHP_OK) return rc;
     if ((rc = energy_reduce(ctx, E)) != DHP_OK) return rc;
-    prof_mark(ctx, slot, 3);
+    prof_mark(ctx, DHP_PHASE_AEV_BWD);
     if ((rc = aev_backward(ctx, F)) != DHP_OK) return rc;
-    prof_mark(ctx, slot, 4);
+    prof_mark(ctx, DHP_N_PHASES);
+    ctx->prof.cur_slot = -1;
     ctx->n_models = w->n_models;
     return DHP_OK;
 }

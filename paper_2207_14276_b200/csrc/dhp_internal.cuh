@@ -74,6 +74,7 @@ struct Profile {
     bool on;
     cudaEvent_t ev[64][DHP_N_PHASES + 1];
     int n_pending;
+    int cur_slot;          // event row of the call being enqueued, or -1
     double ms[DHP_N_PHASES];
     int64_t calls;
 };
@@ -149,6 +150,7 @@ struct Ctx {
     } while (0)
 
 int cuda_fail(Ctx* ctx, cudaError_t e, const char* what);
+void prof_mark(Ctx* ctx, int boundary);   // records event `boundary` (start of phase `boundary`) of the current call when profiling
 #define DHP_CUDA(ctx, call)                                            \
     do {                                                               \
         cudaError_t e__ = (call);                                      \

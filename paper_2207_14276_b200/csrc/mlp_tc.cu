@@ -197,10 +197,11 @@ __device__ __forceinline__ float fast_ex2(float x) {
     return y;
 }
 __device__ __forceinline__ float celu_f(float v, float alpha, float k) {
-    const float e = fmaf(alpha, fast_ex2(v * k), -alpha);
-    return v > 0.f ? v : e;
+    const float e = fmaf(alpha, fast_ex2(v * k), -alpha);      // e > v for every v; e < 0 iff v < 0
+    return fmaxf(v, fminf(e, 0.f));
 }
-__device__ __forceinline__ float dcelu_from_h(float h, float inv_alpha) { return h > 0.f ? 1.0f : fmaf(h, inv_alpha, 1.0f); }
+// CELU'(z) from h = CELU(z): 1 for h > 0, h / alpha + 1 (<= 1) otherwise
+__device__ __forceinline__ float dcelu_from_h(float h, float inv_alpha) { return fminf(fmaf(h, inv_alpha, 1.0f), 1.0f); }
 
 // two floats -> packed fp16 pair, round-to-nearest, saturating to the largest finite fp16 (first argument -> low half)
 __device__ __forceinline__ uint32_t cvt_pack(float lo_half, float hi_half) {
@@ -534,6 +535,9 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
 // TMEM: RA = columns [0,256): the CELU'(z2) stash, then B2's accumulator; RB = [256,448): accumulator of G2, G3, B3.
 // The next item's G2 MMAs (into RB) overlap this item's B2 epilogue (reading RA).
 // ======================================================================================================
+#ifndef MID_DBG
+#define MID_DBG 0      // timing experiments only: 1 = epilogues without work, 2 = no MMAs issued
+#endif
 constexpr int MID_SLOTS = 6;
 constexpr int MID_SLOT_BYTES = 20480;
 constexpr int MID_A_OFF = 12288;                 // G2 slots: W2 image of the K step (12 KB), then h1 hi (4 KB), h1 lo (4 KB)
@@ -547,6 +551,33 @@ constexpr int MID_W_G3 = MID_W_G2 + (H1 / 16) * 32 * H2;
 constexpr int MID_W_B3 = MID_W_G3 + (H2 / 16) * 32 * H3;
 constexpr int MID_W_B2 = MID_W_B3 + (H3 / 16) * 32 * H2;
 constexpr int MID_W_TOTAL = MID_W_B2 + (H2 / 16) * 32 * H1;
+
+constexpr int MID_EPI_WARPS = 16;    // four per TMEM lane quadrant, each taking every fourth 16-column chunk
+constexpr int MID_THREADS = 64 + 32 * MID_EPI_WARPS;
+
+__device__ __forceinline__ void tmem_ld16_issue(uint32_t taddr, uint32_t (&v)[16]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+        : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&v)[16]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
+        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
+        ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]),
+          "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15])
+        : "memory");
+}
+__device__ __forceinline__ void load16(const float* __restrict__ src, float (&x)[16]) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const float4 v = __ldg(reinterpret_cast<const float4*>(src) + i);
+        x[4 * i] = v.x; x[4 * i + 1] = v.y; x[4 * i + 2] = v.z; x[4 * i + 3] = v.w;
+    }
+}
 
 struct MidArgs {
     const int* row_species;
@@ -587,20 +618,40 @@ __device__ __forceinline__ uint64_t make_desc_ns(uint32_t saddr, uint32_t lbo_by
     return d;
 }
 
-// 32 consecutive columns c0.. of row r -> hi / lo planes of X
-__device__ __forceinline__ void store_split32_x(const float (&x)[32], uint8_t* xp, int c0, int r_in) {
-    uint32_t ph[16], pl[16];
+// 16 consecutive columns c0.. of row r -> hi / lo planes of X
+__device__ __forceinline__ void store_split16_x(const float (&x)[16], uint8_t* xp, int c0, int r_in) {
+    uint32_t ph[8], pl[8];
 #pragma unroll
-    for (int i = 0; i < 16; ++i) split_pair(x[2 * i], x[2 * i + 1], ph[i], pl[i]);
+    for (int i = 0; i < 8; ++i) split_pair(x[2 * i], x[2 * i + 1], ph[i], pl[i]);
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
+    for (int i = 0; i < 2; ++i) {
         uint8_t* dst = xp + (size_t)(((c0 >> 3) + i) * BM + r_in) * 16;
         *reinterpret_cast<uint4*>(dst) = make_uint4(ph[4 * i], ph[4 * i + 1], ph[4 * i + 2], ph[4 * i + 3]);
         *reinterpret_cast<uint4*>(dst + MID_X_PLANE) = make_uint4(pl[4 * i], pl[4 * i + 1], pl[4 * i + 2], pl[4 * i + 3]);
     }
 }
+// the same to / from the tiled activation planes in global memory (pointers include group and row)
+__device__ __forceinline__ void store_split16_tiled(const float (&x)[16], __half* hi_dst, __half* lo_dst) {
+    uint32_t ph[8], pl[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) split_pair(x[2 * i], x[2 * i + 1], ph[i], pl[i]);
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+        *reinterpret_cast<uint4*>(hi_dst + i * (BM * 8)) = make_uint4(ph[4 * i], ph[4 * i + 1], ph[4 * i + 2], ph[4 * i + 3]);
+        *reinterpret_cast<uint4*>(lo_dst + i * (BM * 8)) = make_uint4(pl[4 * i], pl[4 * i + 1], pl[4 * i + 2], pl[4 * i + 3]);
+    }
+}
+__device__ __forceinline__ void join16(const uint4 (&h)[2], const uint4 (&l)[2], float (&x)[16]) {
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+        unpack_add(h[i].x, l[i].x, x[8 * i + 0], x[8 * i + 1]);
+        unpack_add(h[i].y, l[i].y, x[8 * i + 2], x[8 * i + 3]);
+        unpack_add(h[i].z, l[i].z, x[8 * i + 4], x[8 * i + 5]);
+        unpack_add(h[i].w, l[i].w, x[8 * i + 6], x[8 * i + 7]);
+    }
+}
 
-__global__ void __launch_bounds__(TC_THREADS, 1)
+__global__ void __launch_bounds__(MID_THREADS, 1)
 k_mlp_mid(const MidArgs p) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t raw = smem_u32(smem_raw);
@@ -626,8 +677,8 @@ k_mlp_mid(const MidArgs p) {
 
     if (warp == 0 && lane == 0) {
         for (int s = 0; s < MID_SLOTS; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-        mbar_init(accb_bar, 1); mbar_init(acca_bar, 1); mbar_init(xready_bar, EPI_WARPS);
-        for (int s = 0; s < RING; ++s) { mbar_init(sfull_bar(s), 1); mbar_init(sempty_bar(s), 1 + EPI_WARPS); }
+        mbar_init(accb_bar, 1); mbar_init(acca_bar, 1); mbar_init(xready_bar, MID_EPI_WARPS);
+        for (int s = 0; s < RING; ++s) { mbar_init(sfull_bar(s), 1); mbar_init(sempty_bar(s), 1 + MID_EPI_WARPS); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 1) tmem_alloc(smem_u32((const void*)tmem_word), TMEM_COLS);
@@ -706,9 +757,11 @@ k_mlp_mid(const MidArgs p) {
                     const uint32_t a0 = a_in_slot ? sa + MID_A_OFF : xs + (uint32_t)j * 4096u;
                     const uint64_t a_hi = make_desc_ns(a0, 2048u);
                     const uint64_t a_lo = make_desc_ns(a0 + (a_in_slot ? 4096u : (uint32_t)MID_X_PLANE), 2048u);
-                    umma_f16(d_tmem, a_hi, b_hi, idesc, accumulate);
-                    umma_f16(d_tmem, a_hi, b_lo, idesc, 1u);
-                    umma_f16(d_tmem, a_lo, b_hi, idesc, 1u);
+                    if (!(MID_DBG & 2)) {
+                        umma_f16(d_tmem, a_hi, b_hi, idesc, accumulate);
+                        umma_f16(d_tmem, a_hi, b_lo, idesc, 1u);
+                        umma_f16(d_tmem, a_lo, b_hi, idesc, 1u);
+                    }
                     accumulate = 1u;
                     umma_commit(empty_bar(slot));
                     if (++slot == MID_SLOTS) { slot = 0; phase ^= 1u; }
@@ -731,8 +784,9 @@ k_mlp_mid(const MidArgs p) {
             }
         }
     } else {
-        // ===== epilogue warps =====
-        const int q = warp & 3, half = (warp - 2) >> 2;
+        // ===== epilogue warps: a warp may touch only TMEM lanes 32 (warp % 4) .. + 31; the four warps of a lane
+        //       quadrant take every fourth 16-column chunk =====
+        const int q = warp & 3, cg = (warp - 2) >> 2;
         const int r_in = q * 32 + lane;
         const uint32_t lane_base = tmem_base + ((uint32_t)(q * 32) << 16);
         int rs = 0; uint32_t rphase = 0;
@@ -755,71 +809,93 @@ k_mlp_mid(const MidArgs p) {
             const int rt = item / M, e = item - rt * M;
             const int s = max(p.row_species[rt * BM], 0);
             const int row = rt * BM + r_in;
-            uint32_t v[32];
-            float x[32], aux[32];
+            const int se = s * M + e;
+            uint32_t v[16];
+            float x[16], aux[16];
             // ---- G2: h2 = CELU(acc / 64 + b2) -> X; CELU'(z2) -> TMEM stash
+            load16(p.b2 + (size_t)se * H2 + cg * 16, aux);
             mbar_wait(accb_bar, bphase); bphase ^= 1u;
             tc_fence_after();
-            for (int c0 = half * 32; c0 < H2; c0 += 64) {
-                tmem_ld32_issue(lane_base + MID_RB + (uint32_t)c0, v);
-                load32(p.b2 + (size_t)(s * M + e) * H2 + c0, aux);
+            for (int c0 = cg * 16; c0 < H2 && !(MID_DBG & 1); c0 += 64) {
+                tmem_ld16_issue(lane_base + MID_RB + (uint32_t)c0, v);
                 tmem_ld_wait();
 #pragma unroll
-                for (int i = 0; i < 32; ++i) x[i] = celu_f(fmaf(__uint_as_float(v[i]), sc, aux[i]), p.alpha, kexp);
-                store_split32_x(x, x_ptr, c0, r_in);
+                for (int i = 0; i < 16; ++i) x[i] = celu_f(fmaf(__uint_as_float(v[i]), sc, aux[i]), p.alpha, kexp);
+                if (c0 + 64 < H2) load16(p.b2 + (size_t)se * H2 + c0 + 64, aux);
+                store_split16_x(x, x_ptr, c0, r_in);
 #pragma unroll
-                for (int i = 0; i < 32; ++i) v[i] = __float_as_uint(dcelu_from_h(x[i], inv_alpha));
-                tmem_st32(lane_base + MID_RA + (uint32_t)c0, v);
+                for (int i = 0; i < 16; ++i) v[i] = __float_as_uint(dcelu_from_h(x[i], inv_alpha));
+                tmem_st16(lane_base + MID_RA + (uint32_t)c0, v);
             }
             tmem_st_wait();
             publish_x();
             // ---- G3: h3 = CELU(acc / 64 + b3); E_i += (w4.h3 + b4)/M; d3 = w4 CELU'(z3) 2^10 / M -> X
+            float w4v[16];
+            load16(p.b3 + (size_t)se * H3 + cg * 16, aux);
+            load16(p.w4 + (size_t)se * H3 + cg * 16, w4v);
             mbar_wait(accb_bar, bphase); bphase ^= 1u;
             tc_fence_after();
             float e_acc = 0.f;
             const float dsc = p.inv_models * D_SCALE;
-            for (int c0 = half * 32; c0 < H3; c0 += 64) {
-                tmem_ld32_issue(lane_base + MID_RB + (uint32_t)c0, v);
-                load32(p.b3 + (size_t)(s * M + e) * H3 + c0, aux);
+            for (int c0 = cg * 16; c0 < H3 && !(MID_DBG & 1); c0 += 64) {
+                tmem_ld16_issue(lane_base + MID_RB + (uint32_t)c0, v);
                 tmem_ld_wait();
 #pragma unroll
-                for (int i = 0; i < 32; ++i) x[i] = celu_f(fmaf(__uint_as_float(v[i]), sc, aux[i]), p.alpha, kexp);
-                load32(p.w4 + (size_t)(s * M + e) * H3 + c0, aux);
-#pragma unroll
-                for (int i = 0; i < 32; ++i) {
-                    e_acc = fmaf(aux[i], x[i], e_acc);
-                    x[i] = aux[i] * dsc * dcelu_from_h(x[i], inv_alpha);
+                for (int i = 0; i < 16; ++i) {
+                    const float h = celu_f(fmaf(__uint_as_float(v[i]), sc, aux[i]), p.alpha, kexp);
+                    e_acc = fmaf(w4v[i], h, e_acc);
+                    x[i] = w4v[i] * dsc * dcelu_from_h(h, inv_alpha);
                 }
-                store_split32_x(x, x_ptr, c0, r_in);
+                if (c0 + 64 < H3) {
+                    load16(p.b3 + (size_t)se * H3 + c0 + 64, aux);
+                    load16(p.w4 + (size_t)se * H3 + c0 + 64, w4v);
+                }
+                store_split16_x(x, x_ptr, c0, r_in);
             }
-            atomicAdd(&p.e_atom[row], (e_acc + (half == 0 ? p.b4[s * M + e] : 0.f)) * p.inv_models);
             publish_x();
+            atomicAdd(&p.e_atom[row], (e_acc + (cg == 0 ? p.b4[se] : 0.f)) * p.inv_models);
             // ---- B3: d2 = (acc / 64) CELU'(z2) -> X
             mbar_wait(accb_bar, bphase); bphase ^= 1u;
             tc_fence_after();
-            for (int c0 = half * 32; c0 < H2; c0 += 64) {
-                uint32_t st[32];
-                tmem_ld32_issue(lane_base + MID_RB + (uint32_t)c0, v);
-                tmem_ld32_issue(lane_base + MID_RA + (uint32_t)c0, st);
+            for (int c0 = cg * 16; c0 < H2 && !(MID_DBG & 1); c0 += 64) {
+                uint32_t st[16];
+                tmem_ld16_issue(lane_base + MID_RB + (uint32_t)c0, v);
+                tmem_ld16_issue(lane_base + MID_RA + (uint32_t)c0, st);
                 tmem_ld_wait();
 #pragma unroll
-                for (int i = 0; i < 32; ++i) x[i] = __uint_as_float(v[i]) * sc * __uint_as_float(st[i]);
-                store_split32_x(x, x_ptr, c0, r_in);
+                for (int i = 0; i < 16; ++i) x[i] = __uint_as_float(v[i]) * sc * __uint_as_float(st[i]);
+                store_split16_x(x, x_ptr, c0, r_in);
             }
             publish_x();
-            // ---- B2: d1 = (acc / 64) CELU'(z1) -> global (tiled planes), CELU' from the saved h1
+            // ---- B2: d1 = (acc / 64) CELU'(z1) -> global (tiled planes), CELU' from the saved h1 (fetched ahead)
+            uint4 hh[2], hl[2];
+            auto h1_offsets = [&](int c0, size_t& o_hi, size_t& o_lo) {
+                const size_t in_tile = (size_t)(((c0 & 63) >> 3) * BM + r_in) * 8;
+                o_hi = tile_off(p.plane_tiles, M * 4, 0, rt, e * 4 + (c0 >> 6)) + in_tile;
+                o_lo = tile_off(p.plane_tiles, M * 4, 1, rt, e * 4 + (c0 >> 6)) + in_tile;
+            };
+            auto h1_fetch = [&](int c0) {
+                size_t o_hi, o_lo;
+                h1_offsets(c0, o_hi, o_lo);
+#pragma unroll
+                for (int i = 0; i < 2; ++i) {
+                    hh[i] = *reinterpret_cast<const uint4*>(p.h1 + o_hi + i * (BM * 8));
+                    hl[i] = *reinterpret_cast<const uint4*>(p.h1 + o_lo + i * (BM * 8));
+                }
+            };
+            h1_fetch(cg * 16);
             mbar_wait(acca_bar, aphase); aphase ^= 1u;
             tc_fence_after();
-            for (int c0 = half * 32; c0 < H1; c0 += 64) {
-                tmem_ld32_issue(lane_base + MID_RA + (uint32_t)c0, v);
-                const size_t in_tile = (size_t)(((c0 & 63) >> 3) * BM + r_in) * 8;
-                const size_t o_hi = tile_off(p.plane_tiles, M * 4, 0, rt, e * 4 + (c0 >> 6)) + in_tile;
-                const size_t o_lo = tile_off(p.plane_tiles, M * 4, 1, rt, e * 4 + (c0 >> 6)) + in_tile;
-                load_joined32_tiled(p.h1 + o_hi, p.h1 + o_lo, aux);
+            for (int c0 = cg * 16; c0 < H1 && !(MID_DBG & 1); c0 += 64) {
+                tmem_ld16_issue(lane_base + MID_RA + (uint32_t)c0, v);
+                join16(hh, hl, aux);
+                if (c0 + 64 < H1) h1_fetch(c0 + 64);
                 tmem_ld_wait();
 #pragma unroll
-                for (int i = 0; i < 32; ++i) x[i] = __uint_as_float(v[i]) * sc * dcelu_from_h(aux[i], inv_alpha);
-                store_split32_tiled(x, p.d1 + o_hi, p.d1 + o_lo);
+                for (int i = 0; i < 16; ++i) x[i] = __uint_as_float(v[i]) * sc * dcelu_from_h(aux[i], inv_alpha);
+                size_t o_hi, o_lo;
+                h1_offsets(c0, o_hi, o_lo);
+                store_split16_tiled(x, p.d1 + o_hi, p.d1 + o_lo);
             }
             tc_fence_before();
         }
@@ -1046,7 +1122,7 @@ void mlp_tc_weights_free(Ctx*, Weights* wt) {
 }
 
 int mlp_tc(Ctx* ctx, const Weights* wt) {
-    if (ctx->n_atoms == 0) return DHP_OK;
+    if (ctx->n_atoms == 0) { prof_mark(ctx, DHP_PHASE_MLP_MID); prof_mark(ctx, DHP_PHASE_MLP_B1); return DHP_OK; }
     TcWorkspace* ws = (TcWorkspace*)ctx->tc_ws;
     const TcWeights* t = (const TcWeights*)wt->tc;
     if (!ws || !t) return DHP_E_NOTIMPL;
@@ -1069,6 +1145,7 @@ int mlp_tc(Ctx* ctx, const Weights* wt) {
     a.a_tiled = nullptr; a.out_planes = ws->h1; a.out_kblocks = M * KB1; a.out_cols_per_tile = H1;
     a.sched = ctx->tc_sched + 0;
     if ((rc = launch_gemm<EPI_CELU, CMP_K>(ctx, ws->m_aev, t->m_w1f, a)) != DHP_OK) return rc;
+    prof_mark(ctx, DHP_PHASE_MLP_MID);
     if (ctx->mlp_mode != DHP_MLP_TENSOR_LAYERWISE) {
         // G2 .. B2 fused: h1 -> d1 with h2, d3, d2 kept on chip
         static bool attr = false;
@@ -1080,7 +1157,7 @@ int mlp_tc(Ctx* ctx, const Weights* wt) {
         m.row_species = ctx->row_species; m.sp_start = ctx->sp_start; m.n_models = M; m.plane_tiles = R / BM;
         m.h1 = ws->h1; m.d1 = ws->d1; m.wimg = t->wmid; m.b2 = t->b2; m.b3 = t->b3; m.w4 = t->w4; m.b4 = t->b4;
         m.inv_models = 1.0f / (float)M; m.alpha = ctx->params.celu_alpha; m.e_atom = ctx->e_atom; m.sched = ctx->tc_sched + 1;
-        DHP_LAUNCH(ctx, k_mlp_mid, ctx->sm_count, TC_THREADS, MID_SMEM, m);
+        DHP_LAUNCH(ctx, k_mlp_mid, ctx->sm_count, MID_THREADS, MID_SMEM, m);
     } else {
         // G2: h1 -> h2
         a.K = H1; a.BN = H2; a.b_rows_per_species = M * H2; a.b_rows_per_tile = H2; a.bias = t->b2;
@@ -1107,6 +1184,7 @@ int mlp_tc(Ctx* ctx, const Weights* wt) {
         a.sched = ctx->tc_sched + 4;
         if ((rc = launch_gemm<EPI_DCELU, CMP_NONE>(ctx, ws->m_aev, t->m_w2b, a)) != DHP_OK) return rc;
     }
+    prof_mark(ctx, DHP_PHASE_MLP_B1);
     // B1: d1 (all models along K) -> dE/dAEV, only the feature blocks that are active for the row tile
     a.K = M * H1; a.BN = 256; a.n_tiles = AEV_LD / 256; a.b_rows_per_species = AEV_LD; a.b_rows_per_tile = 256;
     a.a_tiled = ws->d1; a.a_kblocks = M * KB1; a.a_kb_per_tile = 0;
