@@ -195,9 +195,14 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
         const int t = T0 + lane;
         float A[NZ] = {0.f, 0.f, 0.f, 0.f};
         float B[NA] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        int my_blk = 0;                                  // angular block of this lane's slot
+        bool my_end = false;                             // this slot is the last one of its species pair
         if (t < T_pad) {
-            while (t >= S.tab[e + 1].x) ++e;
+            int next = S.tab[e + 1].x;
+            while (t >= next) { ++e; next = S.tab[e + 1].x; }
             const int4 E = S.tab[e];
+            my_blk = E.w;
+            my_end = t + 1 == next;
             const int u = t - E.x;
             if (u < E.z) {
                 // u -> (x, y) with u = x nk + y.  Different species: j = j0 + x, k = k0 + y.  Same species: distance
@@ -232,21 +237,18 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
 #pragma unroll
         for (int a = 0; a < NA; ++a) S.tB[a][lane] = B[a];
         __syncwarp();
-        // phase 2: the pairs present in this round, in order
-        const int e_first = __shfl_sync(FULL, e, 0);
-        const int e_last = __shfl_sync(FULL, e, (T0 + 31 < T_pad) ? 31 : (T_pad - 1 - T0));
-        for (int ee = e_first; ee <= e_last; ++ee) {
-            const int s0 = S.tab[ee].x, s1 = S.tab[ee + 1].x;
-            const int lo = max(s0, T0) - T0, hi = min(s1, T0 + 32) - T0;
-#pragma unroll 2
-            for (int q = lo; q < hi; q += 4) {
-                const float4 a4 = *reinterpret_cast<const float4*>(&S.tA[za][q]);
-                const float4 b4 = *reinterpret_cast<const float4*>(&S.tB[aa][q]);
-                facc = fmaf(a4.x, b4.x, facc); facc = fmaf(a4.y, b4.y, facc);
-                facc = fmaf(a4.z, b4.z, facc); facc = fmaf(a4.w, b4.w, facc);
-            }
-            if (s1 <= T0 + 32) {                              // pair complete: its 32 features go out, 64 (128) contiguous bytes
-                put_feature<PLANES>(facc, row_f32, row_hi, plane_stride, 32 * S.tab[ee].w + lane);
+        // phase 2: the 8 quads of the round in order (pairs are padded to whole quads, so a pair ends at a quad end);
+        // the branch is warp-uniform
+        const unsigned endmask = __ballot_sync(FULL, my_end);
+#pragma unroll
+        for (int qd = 0; qd < 8; ++qd) {
+            const float4 a4 = *reinterpret_cast<const float4*>(&S.tA[za][4 * qd]);
+            const float4 b4 = *reinterpret_cast<const float4*>(&S.tB[aa][4 * qd]);
+            facc = fmaf(a4.x, b4.x, facc); facc = fmaf(a4.y, b4.y, facc);
+            facc = fmaf(a4.z, b4.z, facc); facc = fmaf(a4.w, b4.w, facc);
+            if ((endmask >> (4 * qd + 3)) & 1u) {             // pair complete: its 32 features go out, 64 (128) contiguous bytes
+                const int blk = __shfl_sync(FULL, my_blk, 4 * qd + 3);
+                put_feature<PLANES>(facc, row_f32, row_hi, plane_stride, 32 * blk + lane);
                 facc = 0.f;
             }
         }
@@ -258,16 +260,22 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
     // (tensor path: the feature blocks that are active for the row's tile; fp32 rows: everything)
     unsigned mask = 0xffffu;
     if (PLANES) { mask = tile_mask[row / ROW_TILE]; if (mask == 0) mask = 1u << 14; }   // G1 runs one zero block for an all-zero tile
-    for (int p = 0; p < NPAIR; ++p)
-        if (((mask >> (p >> 1)) & 1u) && !((nz_pairs >> p) & 1u)) put_feature<PLANES>(0.f, row_f32, row_hi, plane_stride, 32 * p + lane);
-    for (int q = 0; q < 8; ++q) {                        // radial slots in priority order; slot 7 is the 16 padding columns
+    // lane p < 28: angular block p is read (its 64-wide block is active) but this atom has no such pair
+    unsigned zm = __ballot_sync(FULL, lane < NPAIR && ((mask >> (lane >> 1)) & 1u) && !((nz_pairs >> lane) & 1u));
+    for (; zm; zm &= zm - 1u) put_feature<PLANES>(0.f, row_f32, row_hi, plane_stride, 32 * (__ffs(zm) - 1) + lane);
+    // lane q < 8: radial slot q (priority order; slot 7 is the 16 padding columns) likewise
+    bool rz = false;
+    if (lane < 8) {
         bool absent = true;
-        if (q < NSP) {
-            const int s = prio_sp(q);
-            absent = __shfl_sync(FULL, cnt, s) + __shfl_sync(FULL, cnt, 8 + s) == 0;
+        if (lane < NSP) {
+            const int s = prio_sp(lane);
+            absent = nst == 0 || seg_cnt[(size_t)i * 16 + s] + seg_cnt[(size_t)i * 16 + 8 + s] == 0;
         }
-        if (((mask >> (14 + (q >> 2))) & 1u) && absent && lane < 16) put_feature<PLANES>(0.f, row_f32, row_hi, plane_stride, AEV_ANG + 16 * q + lane);
+        rz = absent && ((mask >> (14 + (lane >> 2))) & 1u);
     }
+    unsigned rm = __ballot_sync(FULL, rz);
+    for (; rm; rm &= rm - 1u)
+        if (lane < 16) put_feature<PLANES>(0.f, row_f32, row_hi, plane_stride, AEV_ANG + 16 * (__ffs(rm) - 1) + lane);
 }
 
 // -------------------------------------------------------------------------------------------------
