@@ -523,17 +523,21 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
 // ======================================================================================================
 // Fused middle of the chain.  G2, G3, B3 and B2 are small GEMMs whose split-fp16 activations (4 B per element)
 // cost more HBM time than MMA time when every layer is its own launch (profiles/r1c: 66-81 % DRAM).  Here one
-// work item = (row tile, network) runs   h1 -> h2 -> (E_i, d3) -> d2 -> d1   inside one CTA:
-//   * h2, d3 and d2 never leave the SM: the epilogue warps write each of them as the no-swizzle K-major A operand
-//     of the next GEMM into ONE 96 KB shared-memory region X (each is produced only after every MMA that reads its
-//     predecessor has completed);
-//   * CELU'(z2), needed again by B3's epilogue after X has been overwritten, is parked in spare TMEM columns
-//     (tcgen05.st / tcgen05.ld, fp32, 192 columns);
+// work item = (row tile, network) runs   h1 -> h2 -> (E_i, d3) -> d2 -> d1   inside one CTA, and the four GEMMs and
+// their epilogues are software-pipelined at 64-column granularity: the epilogue of GEMM p produces the A operand of
+// GEMM p+1 in 64-column blocks (= K blocks of p+1) and signals each block, so the MMAs of p+1 start after the first
+// epilogue round and run under the remaining ones.
+//   * h2 and d2 live in ONE 96 KB shared-memory region X as the no-swizzle K-major A operand (d2 overwrites h2 in
+//     place: B3's epilogue thread reads h2(r, n) for CELU'(z2) and writes d2(r, n) to the same bytes);
+//   * d3 is the A operand of B3 straight from TENSOR MEMORY (tcgen05.mma with A in TMEM: lane = row, 16-bit
+//     elements packed two per column along K), written by G3's epilogue with tcgen05.st - so h2 stays intact in X
+//     until B3's epilogue has used it and no activation needs a second shared-memory region;
 //   * weights stream from L2 as pre-tiled images (the exact shared-memory image of one 16-wide K step of one GEMM,
 //     hi plane then lo plane, fetched by one plain cp.async.bulk; no tensor map) through a ring of 6 x 20 KB slots;
 //     h1 (tiled activation layout) streams through the same slots.
-// TMEM: RA = columns [0,256): the CELU'(z2) stash, then B2's accumulator; RB = [256,448): accumulator of G2, G3, B3.
-// The next item's G2 MMAs (into RB) overlap this item's B2 epilogue (reading RA).
+// TMEM (512 columns, all used): P = [0,192) accumulator of G2 and of B3; Q = [192,352) accumulator of G3;
+// D = [352,512) d3 as fp16 A operand (hi 80 columns, lo 80 columns); B2 accumulates into Q u D = [192,448).
+// Every reuse is ordered by the data dependencies themselves (see the hazard notes at the barriers).
 // ======================================================================================================
 #ifndef MID_DBG
 #define MID_DBG 0      // timing experiments only: 1 = epilogues without work, 2 = no MMAs issued
@@ -544,7 +548,8 @@ constexpr int MID_A_OFF = 12288;                 // G2 slots: W2 image of the K 
 constexpr int MID_X_PLANE = BM * H2 * 2;         // 48 KB per plane
 constexpr int MID_X_BYTES = 2 * MID_X_PLANE;
 constexpr int MID_SMEM = MID_X_BYTES + MID_SLOTS * MID_SLOT_BYTES + 1024 /*align*/ + 256 /*barriers, TMEM word, ring*/;
-constexpr uint32_t MID_RA = 0, MID_RB = 256;
+constexpr uint32_t MID_P = 0, MID_Q = 192, MID_D = 352, MID_D_LO = MID_D + H3 / 2;
+static_assert(MID_D_LO + H3 / 2 == TMEM_COLS && MID_Q + H1 <= TMEM_COLS, "TMEM map");
 // weight image of one (species, network), in halves: per GEMM [K step][plane][8-column group (2)][n][8]
 constexpr int MID_W_G2 = 0;
 constexpr int MID_W_G3 = MID_W_G2 + (H1 / 16) * 32 * H2;
@@ -563,13 +568,20 @@ __device__ __forceinline__ void tmem_ld16_issue(uint32_t taddr, uint32_t (&v)[16
           "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
         : "r"(taddr) : "memory");
 }
-__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&v)[16]) {
+__device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t (&v)[8]) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
+                 ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7])
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+// D[tmem] (+)= A[tmem] * B[smem]: A is M x 16 fp16 in tensor memory (lane = row, two K elements per column)
+__device__ __forceinline__ void umma_f16_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
     asm volatile(
-        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
-        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
-        ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]),
-          "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15])
-        : "memory");
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+        ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
 }
 __device__ __forceinline__ void load16(const float* __restrict__ src, float (&x)[16]) {
 #pragma unroll
@@ -592,20 +604,6 @@ struct MidArgs {
     float* e_atom;
     int* sched;
 };
-
-__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32]) {
-    asm volatile(
-        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
-        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
-        "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};"
-        ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]),
-          "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]),
-          "r"(v[16]), "r"(v[17]), "r"(v[18]), "r"(v[19]), "r"(v[20]), "r"(v[21]), "r"(v[22]), "r"(v[23]),
-          "r"(v[24]), "r"(v[25]), "r"(v[26]), "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31])
-        : "memory");
-}
-__device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
-__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // K-major operand without swizzle, [8-column group][row][16 B]: leading byte offset = next group (rows * 16), stride
 // byte offset (next 8 rows) 128
@@ -630,7 +628,7 @@ __device__ __forceinline__ void store_split16_x(const float (&x)[16], uint8_t* x
         *reinterpret_cast<uint4*>(dst + MID_X_PLANE) = make_uint4(pl[4 * i], pl[4 * i + 1], pl[4 * i + 2], pl[4 * i + 3]);
     }
 }
-// the same to / from the tiled activation planes in global memory (pointers include group and row)
+// the same to the tiled activation planes in global memory (pointers include group and row)
 __device__ __forceinline__ void store_split16_tiled(const float (&x)[16], __half* hi_dst, __half* lo_dst) {
     uint32_t ph[8], pl[8];
 #pragma unroll
@@ -661,13 +659,14 @@ k_mlp_mid(const MidArgs p) {
     const uint32_t slots = base + MID_X_BYTES;
     const uint32_t bar0 = slots + MID_SLOTS * MID_SLOT_BYTES;
     uint64_t* bars = reinterpret_cast<uint64_t*>(x_ptr + MID_X_BYTES + MID_SLOTS * MID_SLOT_BYTES);
-    // barriers: full[SLOTS], empty[SLOTS], acc_b, acc_a, x_ready, sfull[RING], sempty[RING]; then TMEM word and item ring
-    constexpr int NBARS = 2 * MID_SLOTS + 3 + 2 * RING;
+    // barriers: full[SLOTS], empty[SLOTS], acc_p, acc_q, xr[3], sfull[RING], sempty[RING]; then TMEM word and item ring
+    constexpr int NBARS = 2 * MID_SLOTS + 5 + 2 * RING;
     auto full_bar = [&](int s) { return bar0 + 8u * s; };
     auto empty_bar = [&](int s) { return bar0 + 8u * (MID_SLOTS + s); };
-    const uint32_t accb_bar = bar0 + 8u * (2 * MID_SLOTS), acca_bar = accb_bar + 8u, xready_bar = accb_bar + 16u;
-    auto sfull_bar = [&](int s) { return bar0 + 8u * (2 * MID_SLOTS + 3 + s); };
-    auto sempty_bar = [&](int s) { return bar0 + 8u * (2 * MID_SLOTS + 3 + RING + s); };
+    const uint32_t accp_bar = bar0 + 8u * (2 * MID_SLOTS), accq_bar = accp_bar + 8u;
+    auto xr_bar = [&](int k) { return accp_bar + 16u + 8u * k; };      // 64-column block k of an epilogue's output is ready
+    auto sfull_bar = [&](int s) { return bar0 + 8u * (2 * MID_SLOTS + 5 + s); };
+    auto sempty_bar = [&](int s) { return bar0 + 8u * (2 * MID_SLOTS + 5 + RING + s); };
     volatile uint32_t* tmem_word = reinterpret_cast<volatile uint32_t*>(bars + NBARS);
     volatile int* ring = reinterpret_cast<volatile int*>(bars + NBARS + 1);
 
@@ -677,7 +676,8 @@ k_mlp_mid(const MidArgs p) {
 
     if (warp == 0 && lane == 0) {
         for (int s = 0; s < MID_SLOTS; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-        mbar_init(accb_bar, 1); mbar_init(acca_bar, 1); mbar_init(xready_bar, MID_EPI_WARPS);
+        mbar_init(accp_bar, 1); mbar_init(accq_bar, 1);
+        for (int k = 0; k < 3; ++k) mbar_init(xr_bar(k), MID_EPI_WARPS);
         for (int s = 0; s < RING; ++s) { mbar_init(sfull_bar(s), 1); mbar_init(sempty_bar(s), 1 + MID_EPI_WARPS); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -740,64 +740,79 @@ k_mlp_mid(const MidArgs p) {
         }
     } else if (warp == 1) {
         // ===== MMA issuer =====
+        // A source of a GEMM: the slot (G2: h1 streams in), X (G3: h2, B2: d2) or tensor memory (B3: d3).  A GEMM whose A is
+        // produced by the previous epilogue waits for 64-column block kb of it (xr[kb]) before its K steps 4 kb .. 4 kb + 3.
+        // Hazards, all covered by program order + these waits: a GEMM that overwrites an accumulator region is issued only
+        // after every epilogue warp has signalled a block that it produces AFTER its last read of that region.
         if (elect_one()) {
             int slot = 0; uint32_t phase = 0;
             int rs = 0; uint32_t rphase = 0;
-            uint32_t xphase = 0;
-            // one GEMM: `steps` K steps of 16, B (n x 16, hi plane then lo plane) from the slot, A from the slot (G2) or from X
-            auto run = [&](int n, int steps, bool a_in_slot, uint32_t d_tmem) {
+            uint32_t xphase = 0;                                   // bit k: parity of xr[k]
+            enum { A_SLOT = 0, A_X = 1, A_TMEM = 2 };
+            auto run = [&](int n, int steps, int a_src, uint32_t d_tmem) {
                 const uint32_t idesc = make_idesc(n);
                 const uint32_t lbo_b = (uint32_t)n * 16u;
                 uint32_t accumulate = 0u;
                 for (int j = 0; j < steps; ++j) {
+                    if (a_src != A_SLOT && (j & 3) == 0) {
+                        const int kb = j >> 2;
+                        mbar_wait(xr_bar(kb), (xphase >> kb) & 1u);
+                        xphase ^= 1u << kb;
+                        tc_fence_after();
+                    }
                     mbar_wait(full_bar(slot), phase);
                     tc_fence_after();
                     const uint32_t sa = slots + (uint32_t)slot * MID_SLOT_BYTES;
                     const uint64_t b_hi = make_desc_ns(sa, lbo_b), b_lo = make_desc_ns(sa + 2u * lbo_b, lbo_b);
-                    const uint32_t a0 = a_in_slot ? sa + MID_A_OFF : xs + (uint32_t)j * 4096u;
-                    const uint64_t a_hi = make_desc_ns(a0, 2048u);
-                    const uint64_t a_lo = make_desc_ns(a0 + (a_in_slot ? 4096u : (uint32_t)MID_X_PLANE), 2048u);
                     if (!(MID_DBG & 2)) {
-                        umma_f16(d_tmem, a_hi, b_hi, idesc, accumulate);
-                        umma_f16(d_tmem, a_hi, b_lo, idesc, 1u);
-                        umma_f16(d_tmem, a_lo, b_hi, idesc, 1u);
+                        if (a_src == A_TMEM) {
+                            const uint32_t a_hi = tmem_base + MID_D + (uint32_t)j * 8u, a_lo = tmem_base + MID_D_LO + (uint32_t)j * 8u;
+                            umma_f16_ts(d_tmem, a_hi, b_hi, idesc, accumulate);
+                            umma_f16_ts(d_tmem, a_hi, b_lo, idesc, 1u);
+                            umma_f16_ts(d_tmem, a_lo, b_hi, idesc, 1u);
+                        } else {
+                            const uint32_t a0 = a_src == A_SLOT ? sa + MID_A_OFF : xs + (uint32_t)j * 4096u;
+                            const uint64_t a_hi = make_desc_ns(a0, 2048u);
+                            const uint64_t a_lo = make_desc_ns(a0 + (a_src == A_SLOT ? 4096u : (uint32_t)MID_X_PLANE), 2048u);
+                            umma_f16(d_tmem, a_hi, b_hi, idesc, accumulate);
+                            umma_f16(d_tmem, a_hi, b_lo, idesc, 1u);
+                            umma_f16(d_tmem, a_lo, b_hi, idesc, 1u);
+                        }
                     }
                     accumulate = 1u;
                     umma_commit(empty_bar(slot));
                     if (++slot == MID_SLOTS) { slot = 0; phase ^= 1u; }
                 }
             };
-            auto wait_x = [&]() { mbar_wait(xready_bar, xphase); xphase ^= 1u; tc_fence_after(); };
             for (;;) {
                 mbar_wait(sfull_bar(rs), rphase);
                 const int item = ring[rs];
                 mbar_arrive(sempty_bar(rs));
                 if (++rs == RING) { rs = 0; rphase ^= 1u; }
                 if (item < 0) break;
-                run(H2, H1 / 16, true, tmem_base + MID_RB);  umma_commit(accb_bar);     // G2
-                wait_x();
-                run(H3, H2 / 16, false, tmem_base + MID_RB); umma_commit(accb_bar);     // G3
-                wait_x();
-                run(H2, H3 / 16, false, tmem_base + MID_RB); umma_commit(accb_bar);     // B3
-                wait_x();
-                run(H1, H2 / 16, false, tmem_base + MID_RA); umma_commit(acca_bar);     // B2
+                run(H2, H1 / 16, A_SLOT, tmem_base + MID_P); umma_commit(accp_bar);     // G2: h1 W2^T        -> P
+                run(H3, H2 / 16, A_X, tmem_base + MID_Q);    umma_commit(accq_bar);     // G3: h2 W3^T        -> Q
+                run(H2, H3 / 16, A_TMEM, tmem_base + MID_P); umma_commit(accp_bar);     // B3: d3 W3          -> P
+                run(H1, H2 / 16, A_X, tmem_base + MID_Q);    umma_commit(accq_bar);     // B2: d2 W2          -> Q u D
             }
         }
     } else {
         // ===== epilogue warps: a warp may touch only TMEM lanes 32 (warp % 4) .. + 31; the four warps of a lane
-        //       quadrant take every fourth 16-column chunk =====
+        //       quadrant take every fourth 16-column chunk, so round k of an epilogue covers columns 64 k .. 64 k + 63 =====
         const int q = warp & 3, cg = (warp - 2) >> 2;
         const int r_in = q * 32 + lane;
         const uint32_t lane_base = tmem_base + ((uint32_t)(q * 32) << 16);
         int rs = 0; uint32_t rphase = 0;
-        uint32_t bphase = 0, aphase = 0;
+        uint32_t pphase = 0, qphase = 0;
         const float kexp = 1.4426950408889634f / p.alpha, inv_alpha = 1.0f / p.alpha;
         const float sc = 1.0f / W_SCALE;
-        auto publish_x = [&]() {           // X written by this warp is visible to the tensor core, accumulator reads are done
+        // this warp's part of 64-column block k is written (shared memory made visible to the tensor core's proxy, tensor
+        // memory stores complete) and its accumulator reads of the round are done
+        auto signal_x = [&](int k) {
             fence_proxy_async_smem();
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive(xready_bar);
+            if (lane == 0) mbar_arrive(xr_bar(k));
         };
         for (;;) {
             mbar_wait(sfull_bar(rs), rphase);
@@ -812,63 +827,82 @@ k_mlp_mid(const MidArgs p) {
             const int se = s * M + e;
             uint32_t v[16];
             float x[16], aux[16];
-            // ---- G2: h2 = CELU(acc / 64 + b2) -> X; CELU'(z2) -> TMEM stash
+            // ---- G2 (P): h2 = CELU(acc / 64 + b2) -> X, block by block
             load16(p.b2 + (size_t)se * H2 + cg * 16, aux);
-            mbar_wait(accb_bar, bphase); bphase ^= 1u;
+            mbar_wait(accp_bar, pphase); pphase ^= 1u;
             tc_fence_after();
-            for (int c0 = cg * 16; c0 < H2 && !(MID_DBG & 1); c0 += 64) {
-                tmem_ld16_issue(lane_base + MID_RB + (uint32_t)c0, v);
-                tmem_ld_wait();
+#pragma unroll 1
+            for (int k = 0; k < 3; ++k) {
+                const int c0 = 64 * k + 16 * cg;
+                if (!(MID_DBG & 1)) {
+                    tmem_ld16_issue(lane_base + MID_P + (uint32_t)c0, v);
+                    tmem_ld_wait();
 #pragma unroll
-                for (int i = 0; i < 16; ++i) x[i] = celu_f(fmaf(__uint_as_float(v[i]), sc, aux[i]), p.alpha, kexp);
-                if (c0 + 64 < H2) load16(p.b2 + (size_t)se * H2 + c0 + 64, aux);
-                store_split16_x(x, x_ptr, c0, r_in);
-#pragma unroll
-                for (int i = 0; i < 16; ++i) v[i] = __float_as_uint(dcelu_from_h(x[i], inv_alpha));
-                tmem_st16(lane_base + MID_RA + (uint32_t)c0, v);
+                    for (int i = 0; i < 16; ++i) x[i] = celu_f(fmaf(__uint_as_float(v[i]), sc, aux[i]), p.alpha, kexp);
+                    if (k < 2) load16(p.b2 + (size_t)se * H2 + c0 + 64, aux);
+                    store_split16_x(x, x_ptr, c0, r_in);
+                }
+                signal_x(k);
             }
-            tmem_st_wait();
-            publish_x();
-            // ---- G3: h3 = CELU(acc / 64 + b3); E_i += (w4.h3 + b4)/M; d3 = w4 CELU'(z3) 2^10 / M -> X
+            // ---- G3 (Q): h3 = CELU(acc / 64 + b3); E_i += (w4.h3 + b4)/M; d3 = w4 CELU'(z3) 2^10 / M -> tensor memory (A of B3)
             float w4v[16];
             load16(p.b3 + (size_t)se * H3 + cg * 16, aux);
             load16(p.w4 + (size_t)se * H3 + cg * 16, w4v);
-            mbar_wait(accb_bar, bphase); bphase ^= 1u;
+            mbar_wait(accq_bar, qphase); qphase ^= 1u;
             tc_fence_after();
             float e_acc = 0.f;
             const float dsc = p.inv_models * D_SCALE;
-            for (int c0 = cg * 16; c0 < H3 && !(MID_DBG & 1); c0 += 64) {
-                tmem_ld16_issue(lane_base + MID_RB + (uint32_t)c0, v);
-                tmem_ld_wait();
+#pragma unroll 1
+            for (int k = 0; k < 3; ++k) {
+                const int c0 = 64 * k + 16 * cg;
+                if (c0 < H3 && !(MID_DBG & 1)) {
+                    tmem_ld16_issue(lane_base + MID_Q + (uint32_t)c0, v);
+                    tmem_ld_wait();
 #pragma unroll
-                for (int i = 0; i < 16; ++i) {
-                    const float h = celu_f(fmaf(__uint_as_float(v[i]), sc, aux[i]), p.alpha, kexp);
-                    e_acc = fmaf(w4v[i], h, e_acc);
-                    x[i] = w4v[i] * dsc * dcelu_from_h(h, inv_alpha);
+                    for (int i = 0; i < 16; ++i) {
+                        const float h = celu_f(fmaf(__uint_as_float(v[i]), sc, aux[i]), p.alpha, kexp);
+                        e_acc = fmaf(w4v[i], h, e_acc);
+                        x[i] = w4v[i] * dsc * dcelu_from_h(h, inv_alpha);
+                    }
+                    if (c0 + 64 < H3) {
+                        load16(p.b3 + (size_t)se * H3 + c0 + 64, aux);
+                        load16(p.w4 + (size_t)se * H3 + c0 + 64, w4v);
+                    }
+                    uint32_t ph[8], pl[8];
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) split_pair(x[2 * i], x[2 * i + 1], ph[i], pl[i]);   // K even -> low half
+                    tmem_st8(lane_base + MID_D + (uint32_t)(c0 >> 1), ph);
+                    tmem_st8(lane_base + MID_D_LO + (uint32_t)(c0 >> 1), pl);
+                    tmem_st_wait();
                 }
-                if (c0 + 64 < H3) {
-                    load16(p.b3 + (size_t)se * H3 + c0 + 64, aux);
-                    load16(p.w4 + (size_t)se * H3 + c0 + 64, w4v);
-                }
-                store_split16_x(x, x_ptr, c0, r_in);
+                signal_x(k);
             }
-            publish_x();
             atomicAdd(&p.e_atom[row], (e_acc + (cg == 0 ? p.b4[se] : 0.f)) * p.inv_models);
-            // ---- B3: d2 = (acc / 64) CELU'(z2) -> X
-            mbar_wait(accb_bar, bphase); bphase ^= 1u;
+            // ---- B3 (P): d2 = (acc / 64) CELU'(z2), CELU' from this thread's own h2 in X, d2 written over it
+            mbar_wait(accp_bar, pphase); pphase ^= 1u;
             tc_fence_after();
-            for (int c0 = cg * 16; c0 < H2 && !(MID_DBG & 1); c0 += 64) {
-                uint32_t st[16];
-                tmem_ld16_issue(lane_base + MID_RB + (uint32_t)c0, v);
-                tmem_ld16_issue(lane_base + MID_RA + (uint32_t)c0, st);
-                tmem_ld_wait();
+#pragma unroll 1
+            for (int k = 0; k < 3; ++k) {
+                const int c0 = 64 * k + 16 * cg;
+                if (!(MID_DBG & 1)) {
+                    tmem_ld16_issue(lane_base + MID_P + (uint32_t)c0, v);
+                    uint4 hh[2], hl[2];
 #pragma unroll
-                for (int i = 0; i < 16; ++i) x[i] = __uint_as_float(v[i]) * sc * __uint_as_float(st[i]);
-                store_split16_x(x, x_ptr, c0, r_in);
+                    for (int i = 0; i < 2; ++i) {
+                        const uint8_t* src = x_ptr + (size_t)(((c0 >> 3) + i) * BM + r_in) * 16;
+                        hh[i] = *reinterpret_cast<const uint4*>(src);
+                        hl[i] = *reinterpret_cast<const uint4*>(src + MID_X_PLANE);
+                    }
+                    join16(hh, hl, aux);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) x[i] = __uint_as_float(v[i]) * sc * dcelu_from_h(aux[i], inv_alpha);
+                    store_split16_x(x, x_ptr, c0, r_in);
+                }
+                signal_x(k);
             }
-            publish_x();
-            // ---- B2: d1 = (acc / 64) CELU'(z1) -> global (tiled planes), CELU' from the saved h1 (fetched ahead)
-            uint4 hh[2], hl[2];
+            // ---- B2 (Q u D): d1 = (acc / 64) CELU'(z1) -> global (tiled planes), CELU' from the saved h1 (fetched ahead)
+            uint4 gh[2], gl[2];
             auto h1_offsets = [&](int c0, size_t& o_hi, size_t& o_lo) {
                 const size_t in_tile = (size_t)(((c0 & 63) >> 3) * BM + r_in) * 8;
                 o_hi = tile_off(p.plane_tiles, M * 4, 0, rt, e * 4 + (c0 >> 6)) + in_tile;
@@ -879,16 +913,17 @@ k_mlp_mid(const MidArgs p) {
                 h1_offsets(c0, o_hi, o_lo);
 #pragma unroll
                 for (int i = 0; i < 2; ++i) {
-                    hh[i] = *reinterpret_cast<const uint4*>(p.h1 + o_hi + i * (BM * 8));
-                    hl[i] = *reinterpret_cast<const uint4*>(p.h1 + o_lo + i * (BM * 8));
+                    gh[i] = *reinterpret_cast<const uint4*>(p.h1 + o_hi + i * (BM * 8));
+                    gl[i] = *reinterpret_cast<const uint4*>(p.h1 + o_lo + i * (BM * 8));
                 }
             };
-            h1_fetch(cg * 16);
-            mbar_wait(acca_bar, aphase); aphase ^= 1u;
+            if (!(MID_DBG & 1)) h1_fetch(cg * 16);
+            mbar_wait(accq_bar, qphase); qphase ^= 1u;
             tc_fence_after();
+#pragma unroll 1
             for (int c0 = cg * 16; c0 < H1 && !(MID_DBG & 1); c0 += 64) {
-                tmem_ld16_issue(lane_base + MID_RA + (uint32_t)c0, v);
-                join16(hh, hl, aux);
+                tmem_ld16_issue(lane_base + MID_Q + (uint32_t)c0, v);
+                join16(gh, gl, aux);
                 if (c0 + 64 < H1) h1_fetch(c0 + 64);
                 tmem_ld_wait();
 #pragma unroll
