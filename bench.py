@@ -234,6 +234,17 @@ def main():
     clocks = sampler.stop() if rank == 0 else None
     assert d.dhp_status() == 0
 
+    # ---- energy-only call (a1-a3), same inputs, device-resident ---------------------------------
+    for k in range(3):
+        d.dhp_ani_energy(pos_sets[k % n_sets], system.box, species, w, mol, E=E)
+    barrier()
+    ev0.record(stream)
+    for k in range(args.steps):
+        d.dhp_ani_energy(pos_sets[k % n_sets], system.box, species, w, mol, E=E)
+    ev1.record(stream)
+    barrier()
+    ms_energy_only = ev0.elapsed_time(ev1) / args.steps
+
     # ---- end to end through the host entry point -----------------------------------------------------
     pos_h = [torch.from_numpy(W.jitter(system, 0.01, 500 + 17 * rank + k)).pin_memory() for k in range(n_sets)]
     sp_h = torch.from_numpy(system.species).pin_memory()
@@ -326,6 +337,7 @@ def main():
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "ms_per_step": e2e_ms / args.steps},
+            "energy_only_ms_per_step": ms_energy_only,
             "roofline": roof,
             "roofline_mlp_phase": mlp_phase,
             "roofline_kernels": kernels,

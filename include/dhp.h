@@ -136,6 +136,12 @@ int dhp_ani_energy_forces(dhp_ctx* ctx, const float* pos, const float* box, cons
                           int64_t n_atoms, const int32_t* mol_offsets, int64_t n_mol,
                           const dhp_weights* weights, int n_models, double* E, float* F);
 
+/* Energy only (a1, a2, a3): the same E as dhp_ani_energy_forces without the transpose-backward GEMMs (a4) and the
+ * AEV backward (a5).  This is what reweighting needs: PAPER.md L228, BAR reweighting of existing trajectories uses
+ * energies only and "avoids the costly computation of DNN gradients".  E as above; asynchronous. */
+int dhp_ani_energy(dhp_ctx* ctx, const float* pos, const float* box, const int32_t* species, int64_t n_atoms,
+                   const int32_t* mol_offsets, int64_t n_mol, const dhp_weights* weights, int n_models, double* E);
+
 /* Same computation with HOST buffers (pos, species, mol_offsets, E, F all host; pinned memory makes
  * the copies asynchronous): host->device copies, the kernels, device->host copies and one stream
  * synchronisation all happen inside the call.  This is the end-to-end entry point bench.py times. */

@@ -32,6 +32,7 @@ SYMBOLS = {
     "dhp_nlist_sizes": (C.c_int, [_vp, _vp, C.POINTER(_i64), C.POINTER(_i64)]),
     "dhp_nlist_export": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp]),
     "dhp_ani_energy_forces": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _vp, _i64, _vp, _i32, _vp, _vp]),
+    "dhp_ani_energy": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _vp, _i64, _vp, _i32, _vp]),
     "dhp_ani_energy_forces_host": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _vp, _i64, _vp, _i32, _vp, _vp]),
     "dhp_status": (C.c_int, [_vp]),
     "dhp_set_mlp_mode": (C.c_int, [_vp, _i32]),
@@ -207,6 +208,19 @@ class Dhp:
                                               _vp(_dptr(E)), _vp(_dptr(F))), self.ctx)
         self._n = n
         return E, F
+
+    def dhp_ani_energy(self, pos, box, species, weights, mol_offsets=None, E=None):
+        """Energy-only device-pointer call (a1, a2, a3).  Returns E fp64 [max(1,n_mol)] cuda tensor; asynchronous."""
+        t = self.torch
+        n = int(pos.shape[0])
+        boxh = None if box is None else np.ascontiguousarray(box, dtype=np.float32)
+        n_mol = 0 if mol_offsets is None else int(mol_offsets.shape[0]) - 1
+        if E is None:
+            E = t.empty(max(1, n_mol), dtype=t.float64, device=self.device)
+        _check(self.lib.dhp_ani_energy(self.ctx, _vp(_dptr(pos)), _vp(_dptr(boxh)), _vp(_dptr(species)), n,
+                                       _vp(_dptr(mol_offsets)), n_mol, weights, weights.n_models, _vp(_dptr(E))), self.ctx)
+        self._n = n
+        return E
 
     def dhp_ani_energy_forces_host(self, pos, box, species, weights, mol_offsets=None, E=None, F=None):
         """Host-buffer call (numpy arrays or pinned torch CPU tensors): copies in, kernels, copies out, one sync."""

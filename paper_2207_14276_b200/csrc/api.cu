@@ -97,17 +97,18 @@ static int run_energy_forces(Ctx* ctx, const float* pos, const float* box, const
     if (tensor && !w->tc) return DHP_E_NOTIMPL;
     if ((rc = aev_forward(ctx, tensor && ctx->aev_planes != nullptr)) != DHP_OK) return rc;
     prof_mark(ctx, DHP_PHASE_MLP_G1);
+    const bool forward_only = F == nullptr;      // dhp_ani_energy: a1, a2, a3 only
     if (tensor) {
-        rc = mlp_tc(ctx, w);                 // marks MLP_MID and MLP_B1 itself
+        rc = mlp_tc(ctx, w, forward_only);   // marks MLP_MID and MLP_B1 itself
     } else {
-        rc = mlp_simt(ctx, w);
+        rc = mlp_simt(ctx, w, forward_only);
         prof_mark(ctx, DHP_PHASE_MLP_MID);
         prof_mark(ctx, DHP_PHASE_MLP_B1);
     }
     if (rc != DHP_OK) return rc;
     if ((rc = energy_reduce(ctx, E)) != DHP_OK) return rc;
     prof_mark(ctx, DHP_PHASE_AEV_BWD);
-    if ((rc = aev_backward(ctx, F)) != DHP_OK) return rc;
+    if (!forward_only && (rc = aev_backward(ctx, F)) != DHP_OK) return rc;
     prof_mark(ctx, DHP_N_PHASES);
     ctx->prof.cur_slot = -1;
     ctx->n_models = w->n_models;
@@ -305,6 +306,16 @@ int dhp_ani_energy_forces(dhp_ctx* h, const float* pos, const float* box, const 
     int r = check_args(c, pos, box, species, n_atoms, mol_offsets, n_mol);
     if (r != DHP_OK) return r;
     return run_energy_forces(c, pos, box, species, n_atoms, mol_offsets, n_mol, &weights->w, E, F);
+}
+
+int dhp_ani_energy(dhp_ctx* h, const float* pos, const float* box, const int32_t* species, int64_t n_atoms,
+                   const int32_t* mol_offsets, int64_t n_mol, const dhp_weights* weights, int n_models, double* E) {
+    if (!h || !weights || !E) return DHP_E_BADARG;
+    Ctx* c = &h->c;
+    if (n_models != weights->w.n_models) return DHP_E_BADARG;
+    int r = check_args(c, pos, box, species, n_atoms, mol_offsets, n_mol);
+    if (r != DHP_OK) return r;
+    return run_energy_forces(c, pos, box, species, n_atoms, mol_offsets, n_mol, &weights->w, E, nullptr);
 }
 
 int dhp_ani_energy_forces_host(dhp_ctx* h, const float* pos, const float* box, const int32_t* species, int64_t n_atoms,

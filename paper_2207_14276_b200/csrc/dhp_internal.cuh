@@ -163,7 +163,7 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
 int nlist_export(Ctx* ctx, int32_t* row_ptr, int32_t* col, bool angular);
 int aev_forward(Ctx* ctx, bool planes);   // planes: write the tensor path's fp16 hi/lo planes instead of fp32 rows
 int aev_backward(Ctx* ctx, float* F_out);
-int mlp_simt(Ctx* ctx, const Weights* w);
+int mlp_simt(Ctx* ctx, const Weights* w, bool forward_only);
 int mlp_simt_alloc(Ctx* ctx);
 void mlp_simt_free(Ctx* ctx);
 int energy_reduce(Ctx* ctx, double* E_out);
@@ -174,7 +174,7 @@ int mlp_tc_alloc(Ctx* ctx);
 void mlp_tc_free(Ctx* ctx);
 int mlp_tc_weights(Ctx* ctx, Weights* w);
 void mlp_tc_weights_free(Ctx* ctx, Weights* w);
-int mlp_tc(Ctx* ctx, const Weights* w);
+int mlp_tc(Ctx* ctx, const Weights* w, bool forward_only);
 
 // upper-triangle row-major index of the unordered species pair (canonical layout of the angular block, Q9)
 __host__ __device__ inline int pairidx(int a, int b) {

@@ -145,7 +145,7 @@ void mlp_simt_free(Ctx* ctx) {
     for (int b = 0; b < 6; ++b) if (ctx->act[b]) cudaFree(ctx->act[b]);
 }
 
-int mlp_simt(Ctx* ctx, const Weights* w) {
+int mlp_simt(Ctx* ctx, const Weights* w, bool forward_only) {
     if (ctx->n_atoms == 0) return DHP_OK;
     const int M = w->n_models;
     const int row_tiles = (int)((ctx->n_atoms + NSP * (ROW_TILE - 1) + TM - 1) / TM);   // bound on sp_start[7]/TM
@@ -168,6 +168,7 @@ int mlp_simt(Ctx* ctx, const Weights* w) {
     const int64_t rows_bound = (int64_t)row_tiles * TM;
     DHP_LAUNCH(ctx, k_out_layer, (int)((rows_bound * 32 + 255) / 256), 256, 0, h3, w->blob, ctx->row_species, ctx->sp_start, M,
                alpha, d3, ctx->e_atom);
+    if (forward_only) { DHP_CUDA(ctx, cudaGetLastError()); return DHP_OK; }
     // backward: B(n,k) = W[k][n]
     g.A = d3; g.lda = M * H3; g.a_model_stride = H3; g.w_off = OFF_W3; g.sbn = 1; g.sbk = H2;
     g.Hs = h2; g.ldh = M * H2; g.h_model_stride = H2; g.C = d2; g.ldc = M * H2; g.c_model_stride = H2; g.N = H2; g.K = H3;

@@ -603,6 +603,7 @@ struct MidArgs {
     float inv_models, alpha;
     float* e_atom;
     int* sched;
+    int forward_only;         // stop after G3's epilogue (energies only): no d3, B3, B2, d1
 };
 
 // K-major operand without swizzle, [8-column group][row][16 B]: leading byte offset = next group (rows * 16), stride
@@ -724,6 +725,7 @@ k_mlp_mid(const MidArgs p) {
                     bulk_load(sa, w + MID_W_G3 + (size_t)j * 32 * H3, 32u * H3 * 2u, full_bar(slot));
                     advance();
                 }
+                if (p.forward_only) continue;
                 for (int j = 0; j < H3 / 16; ++j) {                       // B3
                     const uint32_t sa = next_slot();
                     mbar_expect_tx(full_bar(slot), 32u * H2 * 2u);
@@ -792,6 +794,7 @@ k_mlp_mid(const MidArgs p) {
                 if (item < 0) break;
                 run(H2, H1 / 16, A_SLOT, tmem_base + MID_P); umma_commit(accp_bar);     // G2: h1 W2^T        -> P
                 run(H3, H2 / 16, A_X, tmem_base + MID_Q);    umma_commit(accq_bar);     // G3: h2 W3^T        -> Q
+                if (p.forward_only) continue;
                 run(H2, H3 / 16, A_TMEM, tmem_base + MID_P); umma_commit(accp_bar);     // B3: d3 W3          -> P
                 run(H1, H2 / 16, A_X, tmem_base + MID_Q);    umma_commit(accq_bar);     // B2: d2 W2          -> Q u D
             }
@@ -868,16 +871,19 @@ k_mlp_mid(const MidArgs p) {
                         load16(p.b3 + (size_t)se * H3 + c0 + 64, aux);
                         load16(p.w4 + (size_t)se * H3 + c0 + 64, w4v);
                     }
-                    uint32_t ph[8], pl[8];
+                    if (!p.forward_only) {
+                        uint32_t ph[8], pl[8];
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) split_pair(x[2 * i], x[2 * i + 1], ph[i], pl[i]);   // K even -> low half
-                    tmem_st8(lane_base + MID_D + (uint32_t)(c0 >> 1), ph);
-                    tmem_st8(lane_base + MID_D_LO + (uint32_t)(c0 >> 1), pl);
-                    tmem_st_wait();
+                        for (int i = 0; i < 8; ++i) split_pair(x[2 * i], x[2 * i + 1], ph[i], pl[i]);   // K even -> low half
+                        tmem_st8(lane_base + MID_D + (uint32_t)(c0 >> 1), ph);
+                        tmem_st8(lane_base + MID_D_LO + (uint32_t)(c0 >> 1), pl);
+                        tmem_st_wait();
+                    }
                 }
-                signal_x(k);
+                if (!p.forward_only) signal_x(k);
             }
             atomicAdd(&p.e_atom[row], (e_acc + (cg == 0 ? p.b4[se] : 0.f)) * p.inv_models);
+            if (p.forward_only) { tc_fence_before(); continue; }
             // ---- B3 (P): d2 = (acc / 64) CELU'(z2), CELU' from this thread's own h2 in X, d2 written over it
             mbar_wait(accp_bar, pphase); pphase ^= 1u;
             tc_fence_after();
@@ -1156,7 +1162,7 @@ void mlp_tc_weights_free(Ctx*, Weights* wt) {
     wt->tc = nullptr;
 }
 
-int mlp_tc(Ctx* ctx, const Weights* wt) {
+int mlp_tc(Ctx* ctx, const Weights* wt, bool forward_only) {
     if (ctx->n_atoms == 0) { prof_mark(ctx, DHP_PHASE_MLP_MID); prof_mark(ctx, DHP_PHASE_MLP_B1); return DHP_OK; }
     TcWorkspace* ws = (TcWorkspace*)ctx->tc_ws;
     const TcWeights* t = (const TcWeights*)wt->tc;
@@ -1192,6 +1198,7 @@ int mlp_tc(Ctx* ctx, const Weights* wt) {
         m.row_species = ctx->row_species; m.sp_start = ctx->sp_start; m.n_models = M; m.plane_tiles = R / BM;
         m.h1 = ws->h1; m.d1 = ws->d1; m.wimg = t->wmid; m.b2 = t->b2; m.b3 = t->b3; m.w4 = t->w4; m.b4 = t->b4;
         m.inv_models = 1.0f / (float)M; m.alpha = ctx->params.celu_alpha; m.e_atom = ctx->e_atom; m.sched = ctx->tc_sched + 1;
+        m.forward_only = forward_only ? 1 : 0;
         DHP_LAUNCH(ctx, k_mlp_mid, ctx->sm_count, MID_THREADS, MID_SMEM, m);
     } else {
         // G2: h1 -> h2
@@ -1206,6 +1213,7 @@ int mlp_tc(Ctx* ctx, const Weights* wt) {
         a.out_planes = ws->d3; a.out_kblocks = M * KB2; a.out_cols_per_tile = H2;
         a.sched = ctx->tc_sched + 2;
         if ((rc = launch_gemm<EPI_OUT, CMP_NONE>(ctx, ws->m_aev, t->m_w3f, a)) != DHP_OK) return rc;
+        if (forward_only) { prof_mark(ctx, DHP_PHASE_MLP_B1); DHP_CUDA(ctx, cudaGetLastError()); return DHP_OK; }
         // B3: d3 -> d2
         a.K = H3; a.BN = H2; a.b_rows_per_species = M * H2; a.b_rows_per_tile = H2;
         a.a_tiled = ws->d3; a.a_kblocks = M * KB2; a.a_kb_per_tile = KB2;
@@ -1220,6 +1228,7 @@ int mlp_tc(Ctx* ctx, const Weights* wt) {
         if ((rc = launch_gemm<EPI_DCELU, CMP_NONE>(ctx, ws->m_aev, t->m_w2b, a)) != DHP_OK) return rc;
     }
     prof_mark(ctx, DHP_PHASE_MLP_B1);
+    if (forward_only) { DHP_CUDA(ctx, cudaGetLastError()); return DHP_OK; }
     // B1: d1 (all models along K) -> dE/dAEV, only the feature blocks that are active for the row tile
     a.K = M * H1; a.BN = 256; a.n_tiles = AEV_LD / 256; a.b_rows_per_species = AEV_LD; a.b_rows_per_tile = 256;
     a.a_tiled = ws->d1; a.a_kblocks = M * KB1; a.a_kb_per_tile = 0;

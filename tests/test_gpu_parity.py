@@ -206,6 +206,32 @@ def test_energy_forces_config5_sampled_molecules(torch, B, params, blob8):
     d.close()
 
 
+@pytest.mark.parametrize("name", ["water96", "mix600", "replicas16"])
+@pytest.mark.parametrize("mode", [1, 2, 3])
+def test_energy_only_call(torch, B, params, blob8, name, mode):
+    """dhp_ani_energy (a1-a3 only; reweighting needs energies, not gradients) against the oracle and
+    against the energy of the full call."""
+    s = SYSTEMS[name]()
+    blob = blob8[: s.n_models * 7 * W.PARAMS_PER_NET]
+    d = make_ctx(B, s, params)
+    d.dhp_set_mlp_mode(mode)
+    w = d.dhp_weights_load(blob, s.n_models)
+    pos, sp, mol = B.to_device(s)
+    for _ in range(2):                                   # twice: the second call starts from the first one's barrier phases
+        E = d.dhp_ani_energy(pos, s.box, sp, w, mol)
+    torch.cuda.synchronize()
+    assert d.dhp_status() == 0
+    Eo, _ = oracle.total_energy_forces(s, params, blob)
+    per = s.n_atoms if s.mol_offsets is None else np.diff(s.mol_offsets)
+    assert np.max(np.abs(E.cpu().numpy() - Eo) / per) <= E_TOL_PER_ATOM
+    E2, F2 = d.dhp_ani_energy_forces(pos, s.box, sp, w, mol)   # a full call after an energy-only call still works
+    torch.cuda.synchronize()
+    _, Fo = oracle.total_energy_forces(s, params, blob)
+    assert np.max(np.abs(E2.cpu().numpy() - Eo) / per) <= E_TOL_PER_ATOM
+    assert np.max(np.abs(F2.cpu().numpy() - Fo)) <= F_TOL
+    d.close()
+
+
 def test_host_entry_point_matches_device_entry_point(torch, B, params, blob8):
     s = SYSTEMS["mix600"]()
     d, E, F = run_gpu(B, torch, s, params, blob8)
