@@ -35,9 +35,9 @@ METRIC = "ani_energy_forces_atoms_evals_per_s"
 UNIT = "atoms*evals/s"
 NS_PER_DAY_PER_EVAL_PER_S = 0.5e-6 * 86400.0      # 0.5 fs step
 # DRAM bytes (read + write) per launch at configs[3], from the committed ncu --set full captures of this command
-# (profiles/r1d_ncu_full_summary.txt: G1, k_mlp_mid, B1; profiles/r1c_ncu_full_summary.txt: the others)
-TRAFFIC_98K = {"g1": 0.17083e9 + 0.74936e9, "mid": 0.85889e9 + 0.76818e9, "b1": 0.83663e9 + 0.09485e9,
-               "aev_fwd": 0.02738e9 + 0.12718e9, "aev_bwd": 0.11340e9 + 0.00464e9, "nlist": 0.00236e9 + 0.00077e9 + 0.02743e9 + 0.00004e9}
+# (profiles/r1e_ncu_full_summary.txt)
+TRAFFIC_98K = {"g1": 0.17065e9 + 0.74989e9, "mid": 0.84655e9 + 0.77066e9, "b1": 0.83645e9 + 0.09575e9,
+               "aev_fwd": 0.02731e9 + 0.05759e9, "aev_bwd": 0.11339e9 + 0.00412e9, "nlist": 0.00235e9 + 0.00077e9 + 0.02705e9 + 0.00006e9}
 
 
 def peaks():
