@@ -142,6 +142,20 @@ int dhp_ani_energy_forces(dhp_ctx* ctx, const float* pos, const float* box, cons
 int dhp_ani_energy(dhp_ctx* ctx, const float* pos, const float* box, const int32_t* species, int64_t n_atoms,
                    const int32_t* mol_offsets, int64_t n_mol, const dhp_weights* weights, int n_models, double* E);
 
+/* Partial evaluation over a subset of CENTRAL atoms - the building block of the multi-GPU decomposition.  The
+ * energy is a sum of atomic terms over local environments (Eq. 2), which the paper shards by
+ * spatial domains whose halo AEVs are recomputed redundantly (L134, L194: "~40 % loss").  Here a rank instead
+ * evaluates only the atoms it owns as centres and no AEV is computed twice:
+ *   central  dev uint8 [n_atoms], non-zero = atom i is a central atom of this call; NULL = all atoms
+ *   E        E_c = (1/n_models) sum_e sum_{i central} NN^{(e)}_{s_i}(G_i)   (per molecule with mol_offsets)
+ *   F        F_c = -dE_c/dr for ALL n_atoms atoms (a central atom's neighbours receive force from it)
+ * Every atom still acts as a neighbour.  Over a partition of the atoms into central sets, the E_c and F_c add up
+ * to the E and F of dhp_ani_energy_forces (up to fp32 summation order).  Asynchronous, like the full call. */
+int dhp_ani_energy_forces_partial(dhp_ctx* ctx, const float* pos, const float* box, const int32_t* species,
+                                  int64_t n_atoms, const int32_t* mol_offsets, int64_t n_mol,
+                                  const dhp_weights* weights, int n_models, const uint8_t* central,
+                                  double* E, float* F);
+
 /* Same computation with HOST buffers (pos, species, mol_offsets, E, F all host; pinned memory makes
  * the copies asynchronous): host->device copies, the kernels, device->host copies and one stream
  * synchronisation all happen inside the call.  This is the end-to-end entry point bench.py times. */

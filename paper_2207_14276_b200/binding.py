@@ -32,6 +32,7 @@ SYMBOLS = {
     "dhp_nlist_sizes": (C.c_int, [_vp, _vp, C.POINTER(_i64), C.POINTER(_i64)]),
     "dhp_nlist_export": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp]),
     "dhp_ani_energy_forces": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _vp, _i64, _vp, _i32, _vp, _vp]),
+    "dhp_ani_energy_forces_partial": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _vp, _i64, _vp, _i32, _vp, _vp, _vp]),
     "dhp_ani_energy": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _vp, _i64, _vp, _i32, _vp]),
     "dhp_ani_energy_forces_host": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _vp, _i64, _vp, _i32, _vp, _vp]),
     "dhp_status": (C.c_int, [_vp]),
@@ -206,6 +207,25 @@ class Dhp:
         _check(self.lib.dhp_ani_energy_forces(self.ctx, _vp(_dptr(pos)), _vp(_dptr(boxh)), _vp(_dptr(species)), n,
                                               _vp(_dptr(mol_offsets)), n_mol, weights, weights.n_models,
                                               _vp(_dptr(E)), _vp(_dptr(F))), self.ctx)
+        self._n = n
+        return E, F
+
+    def dhp_ani_energy_forces_partial(self, pos, box, species, weights, central, mol_offsets=None, E=None, F=None):
+        """Partial evaluation over the atoms with central[i] != 0 (cuda uint8 [N], or None = all): E_c and the force
+        F_c = -dE_c/dr on ALL atoms.  Over a partition of the atoms the results add up to the full call's."""
+        t = self.torch
+        n = int(pos.shape[0])
+        boxh = None if box is None else np.ascontiguousarray(box, dtype=np.float32)
+        n_mol = 0 if mol_offsets is None else int(mol_offsets.shape[0]) - 1
+        if central is not None and (central.dtype != t.uint8 or int(central.shape[0]) != n):
+            raise DhpError("central must be a uint8 tensor with one entry per atom")
+        if E is None:
+            E = t.empty(max(1, n_mol), dtype=t.float64, device=self.device)
+        if F is None:
+            F = t.empty((n, 3), dtype=t.float32, device=self.device)
+        _check(self.lib.dhp_ani_energy_forces_partial(self.ctx, _vp(_dptr(pos)), _vp(_dptr(boxh)), _vp(_dptr(species)), n,
+                                                      _vp(_dptr(mol_offsets)), n_mol, weights, weights.n_models,
+                                                      _vp(_dptr(central)), _vp(_dptr(E)), _vp(_dptr(F))), self.ctx)
         self._n = n
         return E, F
 

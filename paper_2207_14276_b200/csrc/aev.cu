@@ -129,6 +129,7 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
     const float4 pi = spos[i];
     const float inv_rcr = 1.0f / K.rcr, inv_rca = 1.0f / K.rca;
     const int row = rowmap[i];
+    if (row < 0) return;                               // not a central atom of this call (partial evaluation)
     float* row_f32 = aev + (size_t)row * AEV_LD;
     __half* row_hi = planes + (size_t)row * AEV_LD;
 
@@ -331,6 +332,7 @@ k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
     if (na > MAX_ANG || nst > MAX_RAD) { na = 0; nst = 0; cnt = 0; }     // capacity overflow: reported by the forward pass
 
     // ---- the blocks of dE/dG this atom uses ----------------------------------------------------------------
+    if (rowmap[i] < 0) return;                         // not a central atom of this call (partial evaluation)
     const float* grow = grad + (size_t)rowmap[i] * AEV_LD;
     {
         int psa = 0, psb = 0;

@@ -40,7 +40,7 @@ static bool dalloc(T** p, size_t count) {
 
 static void free_all(Ctx* c) {
     void* ptrs[] = {c->grid, c->status, c->bbox, c->cell_of, c->perm_tmp, c->cell_count, c->cell_start, c->cell_fill, c->perm,
-                    c->inv_perm, c->spos, c->smol, c->n_rad, c->n_ang, c->row_ptr, c->col, c->sp_count, c->sp_start,
+                    c->inv_perm, c->spos, c->smol, c->snc, c->n_rad, c->n_ang, c->row_ptr, c->col, c->sp_count, c->sp_start,
                     c->rowmap, c->row_species, c->row_slot, c->blk_hist, c->key_start, c->amask, c->tile_mask, c->tc_sched, c->col2feat, c->aev, c->grad, c->e_atom, c->fsorted,
                     c->e_out_tmp, c->export_tmp, c->tmp_col, c->blk_sum, c->blk_off, c->seg_cnt, c->st_pos, c->st_species, c->st_mol, c->st_E, c->st_F};
     for (void* p : ptrs) if (p) cudaFree(p);
@@ -82,7 +82,8 @@ static void prof_drain(Ctx* ctx) {
 }
 
 static int run_energy_forces(Ctx* ctx, const float* pos, const float* box, const int32_t* species, int64_t n,
-                             const int32_t* mol_offsets, int64_t n_mol, const Weights* w, double* E, float* F) {
+                             const int32_t* mol_offsets, int64_t n_mol, const Weights* w, double* E, float* F,
+                             const uint8_t* central = nullptr) {
     ctx->prof.cur_slot = -1;
     if (ctx->prof.on) {
         if (ctx->prof.n_pending == 64) prof_drain(ctx);
@@ -90,7 +91,7 @@ static int run_energy_forces(Ctx* ctx, const float* pos, const float* box, const
     }
     int rc;
     prof_mark(ctx, DHP_PHASE_NLIST);
-    if ((rc = nlist_build(ctx, pos, box, species, n, mol_offsets, n_mol)) != DHP_OK) return rc;
+    if ((rc = nlist_build(ctx, pos, box, species, n, mol_offsets, n_mol, central)) != DHP_OK) return rc;
     prof_mark(ctx, DHP_PHASE_AEV_FWD);
     const bool tensor = ctx->mlp_mode == DHP_MLP_TENSOR || ctx->mlp_mode == DHP_MLP_TENSOR_LAYERWISE ||
                         (ctx->mlp_mode == DHP_MLP_AUTO && w->tc != nullptr);
@@ -124,6 +125,10 @@ __global__ void k_gather_rows(const float* __restrict__ src, int ld_src, int nco
     int a = blockIdx.x;
     if (a >= n) return;
     const int row = rowmap[inv_perm[a]];
+    if (row < 0) {                                   // not a central atom of the last (partial) call
+        for (int c = threadIdx.x; c < ncol; c += blockDim.x) dst[(size_t)a * ncol + c] = 0.f;
+        return;
+    }
     const float* s = src + (size_t)row * ld_src;
     if (!col2feat) {
         for (int c = threadIdx.x; c < ncol; c += blockDim.x) dst[(size_t)a * ncol + c] = s[c];
@@ -140,6 +145,10 @@ __global__ void k_gather_planes(const __half* __restrict__ planes, size_t plane_
     int a = blockIdx.x;
     if (a >= n) return;
     const int row = rowmap[inv_perm[a]];
+    if (row < 0) {
+        for (int c = threadIdx.x; c < AEV_DIM; c += blockDim.x) dst[(size_t)a * AEV_DIM + c] = 0.f;
+        return;
+    }
     const __half* hi = planes + (size_t)row * AEV_LD;
     const __half* lo = hi + plane_stride;
     const unsigned mask = tile_mask[row / ROW_TILE];
@@ -190,7 +199,7 @@ int dhp_create(dhp_ctx** out, const dhp_params* params, int64_t max_atoms, int64
     bool ok = true;
     ok &= dalloc(&c->grid, 1) && dalloc(&c->status, 1) && dalloc(&c->bbox, 8);
     ok &= dalloc(&c->cell_of, N) && dalloc(&c->perm_tmp, N) && dalloc(&c->cell_count, NC + 1) && dalloc(&c->cell_start, NC + 1) && dalloc(&c->cell_fill, NC);
-    ok &= dalloc(&c->perm, N) && dalloc(&c->inv_perm, N) && dalloc(&c->spos, N) && dalloc(&c->smol, N);
+    ok &= dalloc(&c->perm, N) && dalloc(&c->inv_perm, N) && dalloc(&c->spos, N) && dalloc(&c->smol, N) && dalloc(&c->snc, N);
     ok &= dalloc(&c->n_rad, N) && dalloc(&c->n_ang, N) && dalloc(&c->row_ptr, N + 1) && dalloc(&c->col, (size_t)c->pair_cap);
     ok &= dalloc(&c->tmp_col, N * c->tmp_stride) && dalloc(&c->blk_sum, N / 64 + 3) && dalloc(&c->blk_off, N / 64 + 3) && dalloc(&c->seg_cnt, N * 16);
     ok &= dalloc(&c->sp_count, 8) && dalloc(&c->sp_start, 8) && dalloc(&c->rowmap, N);
@@ -306,6 +315,17 @@ int dhp_ani_energy_forces(dhp_ctx* h, const float* pos, const float* box, const 
     int r = check_args(c, pos, box, species, n_atoms, mol_offsets, n_mol);
     if (r != DHP_OK) return r;
     return run_energy_forces(c, pos, box, species, n_atoms, mol_offsets, n_mol, &weights->w, E, F);
+}
+
+int dhp_ani_energy_forces_partial(dhp_ctx* h, const float* pos, const float* box, const int32_t* species, int64_t n_atoms,
+                                  const int32_t* mol_offsets, int64_t n_mol, const dhp_weights* weights, int n_models,
+                                  const uint8_t* central, double* E, float* F) {
+    if (!h || !weights || !E || (n_atoms > 0 && !F)) return DHP_E_BADARG;
+    Ctx* c = &h->c;
+    if (n_models != weights->w.n_models) return DHP_E_BADARG;
+    int r = check_args(c, pos, box, species, n_atoms, mol_offsets, n_mol);
+    if (r != DHP_OK) return r;
+    return run_energy_forces(c, pos, box, species, n_atoms, mol_offsets, n_mol, &weights->w, E, F, central);
 }
 
 int dhp_ani_energy(dhp_ctx* h, const float* pos, const float* box, const int32_t* species, int64_t n_atoms,

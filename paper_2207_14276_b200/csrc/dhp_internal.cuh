@@ -108,6 +108,8 @@ struct Ctx {
     int* inv_perm;         // [N]
     float4* spos;          // [N] x,y,z, species bits
     int* smol;             // [N] molecule of sorted atom (0 if none)
+    unsigned char* snc;    // [N] 1 = sorted atom is NOT a central atom of this call (partial evaluation), else 0
+    bool partial;          // the last list was built with a central-atom mask
     int* n_rad;            // [N]
     int* n_ang;            // [N]
     int* row_ptr;          // [N+1]
@@ -159,7 +161,7 @@ void prof_mark(Ctx* ctx, int boundary);   // records event `boundary` (start of 
 
 // ---- phases (each enqueues kernels on ctx->stream) ------------------------------------------------
 int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t* species, int64_t n,
-                const int32_t* mol_offsets, int64_t n_mol);
+                const int32_t* mol_offsets, int64_t n_mol, const uint8_t* central = nullptr);
 int nlist_export(Ctx* ctx, int32_t* row_ptr, int32_t* col, bool angular);
 int aev_forward(Ctx* ctx, bool planes);   // planes: write the tensor path's fp16 hi/lo planes instead of fp32 rows
 int aev_backward(Ctx* ctx, float* F_out);

@@ -190,7 +190,7 @@ __global__ void k_scatter(const int* __restrict__ cell_of, int n, const int* __r
 __global__ void k_sort_gather(const float* __restrict__ pos, const int* __restrict__ species,
                               const Grid* __restrict__ g, const int* __restrict__ cell_start, const int* __restrict__ perm_in,
                               int* __restrict__ perm, int* __restrict__ inv_perm, float4* __restrict__ spos,
-                              int* __restrict__ smol) {
+                              int* __restrict__ smol, const uint8_t* __restrict__ central, unsigned char* __restrict__ snc) {
     const int c = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (c >= g->ncell) return;
     const int b = cell_start[c], e = cell_start[c + 1];
@@ -205,6 +205,7 @@ __global__ void k_sort_gather(const float* __restrict__ pos, const int* __restri
         s = min(max(s, 0), NSP - 1);
         spos[dst] = make_float4(pos[3 * v], pos[3 * v + 1], pos[3 * v + 2], __int_as_float(s));
         smol[dst] = g->by_molecule ? c : 0;
+        if (central) snc[dst] = central[v] ? 0 : 1;
     }
 }
 
@@ -230,12 +231,13 @@ __device__ __forceinline__ int row_key(int s, unsigned m) {
 
 // blk_hist is key-major: blk_hist[key * nrb + block]
 __global__ void __launch_bounds__(RB)
-k_rowkey_hist(const float4* __restrict__ spos, const unsigned* __restrict__ amask, int n, int nrb, int* __restrict__ blk_hist) {
+k_rowkey_hist(const float4* __restrict__ spos, const unsigned* __restrict__ amask, const unsigned char* __restrict__ snc, int n, int nrb,
+              int* __restrict__ blk_hist) {
     __shared__ int h[NKEY];
     for (int k = threadIdx.x; k < NKEY; k += RB) h[k] = 0;
     __syncthreads();
     const int a = blockIdx.x * RB + threadIdx.x;
-    if (a < n) atomicAdd(&h[row_key(__float_as_int(spos[a].w), amask[a])], 1);
+    if (a < n && !(snc && snc[a])) atomicAdd(&h[row_key(__float_as_int(spos[a].w), amask[a])], 1);   // non-central atoms get no row
     __syncthreads();
     for (int k = threadIdx.x; k < NKEY; k += RB) blk_hist[(size_t)k * nrb + blockIdx.x] = h[k];
 }
@@ -279,7 +281,8 @@ k_rowkey_scan(int* __restrict__ blk_hist, int nrb, int* __restrict__ sp_count, i
 }
 
 __global__ void __launch_bounds__(RB)
-k_rowkey_rank(const float4* __restrict__ spos, const unsigned* __restrict__ amask, int n, int nrb, const int* __restrict__ blk_hist,
+k_rowkey_rank(const float4* __restrict__ spos, const unsigned* __restrict__ amask, const unsigned char* __restrict__ snc, int n, int nrb,
+              const int* __restrict__ blk_hist,
               const int* __restrict__ key_start, int* __restrict__ rowmap, int* __restrict__ row_species,
               int* __restrict__ row_slot, unsigned* __restrict__ tile_mask) {
     __shared__ int wcnt[RB / 32][NKEY];
@@ -289,12 +292,13 @@ k_rowkey_rank(const float4* __restrict__ spos, const unsigned* __restrict__ amas
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     int s = 0, key = -1;
     unsigned m = 0;
-    if (a < n) { s = __float_as_int(spos[a].w); m = amask[a]; key = row_key(s, m); }
+    if (a < n && !(snc && snc[a])) { s = __float_as_int(spos[a].w); m = amask[a]; key = row_key(s, m); }
     const unsigned grp = __match_any_sync(0xffffffffu, key);
     const int rank_in_warp = __popc(grp & ((1u << lane) - 1u));
     if (key >= 0 && rank_in_warp == 0) wcnt[w][key] = __popc(grp);
     __syncthreads();
     if (a >= n) return;
+    if (key < 0) { rowmap[a] = -1; return; }
     int before = 0;
     for (int q = 0; q < w; ++q) before += wcnt[q][key];
     const int row = key_start[key] + blk_hist[(size_t)key * nrb + blockIdx.x] + before + rank_in_warp;
@@ -360,7 +364,7 @@ template <bool WRAP>
 __global__ void __launch_bounds__(P1_THREADS, 8)
 k_pairs(const float4* __restrict__ spos, const Grid* __restrict__ gp, const int* __restrict__ cell_start, double rcr2,
         double rca2, int stride, int* __restrict__ cnt, unsigned* __restrict__ tmp, int* __restrict__ blk_sum,
-        int* __restrict__ status) {
+        int* __restrict__ status, const unsigned char* __restrict__ snc) {
     __shared__ Grid g;
     __shared__ float4 cand[CAND_TILE + 32];
     __shared__ int seg_cell_b[28], seg_off[28], nseg_s;
@@ -449,6 +453,10 @@ k_pairs(const float4* __restrict__ spos, const Grid* __restrict__ gp, const int*
 
         // ---- centre atoms of this cell, one warp each ----------------------------------------
         for (int i = cb + warp; i < ce; i += P1_THREADS / 32) {
+            if (snc && snc[i]) {               // not a central atom of this call: an empty row
+                if (lane == 0 && t0 == 0) cnt[i] = 0;
+                continue;
+            }
             // the centre's own relative coordinates: same arithmetic as the staged copy
             const float4 pio = spos[i];
             double ri[3] = {(double)pio.x - ctr[0], (double)pio.y - ctr[1], (double)pio.z - ctr[2]};
@@ -624,7 +632,7 @@ k_rows(const unsigned* __restrict__ tmp, int stride, const int* __restrict__ cnt
 // host side
 // ---------------------------------------------------------------------------------------------
 int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t* species, int64_t n64,
-                const int32_t* mol_offsets, int64_t n_mol64) {
+                const int32_t* mol_offsets, int64_t n_mol64, const uint8_t* central) {
     const int n = (int)n64, n_mol = (int)n_mol64;
     const bool periodic = box_host != nullptr;
     const bool by_mol = mol_offsets != nullptr && n_mol > 0;
@@ -632,6 +640,8 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
     ctx->n_atoms = n;
     ctx->n_mol = by_mol ? n_mol : 0;
     ctx->periodic = periodic;
+    ctx->partial = central != nullptr;
+    const unsigned char* snc = central ? ctx->snc : nullptr;
     cudaStream_t st = ctx->stream;
     const int nblk = (n + ROWS_PER_BLK - 1) / ROWS_PER_BLK;
 
@@ -671,7 +681,7 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
         cell_bound = t < cell_bound ? t : cell_bound;
     }
     DHP_LAUNCH(ctx, k_sort_gather, (int)((cell_bound + 3) / 4), 128, 0, pos, species, ctx->grid, ctx->cell_start,
-               ctx->perm_tmp, ctx->perm, ctx->inv_perm, ctx->spos, ctx->smol);
+               ctx->perm_tmp, ctx->perm, ctx->inv_perm, ctx->spos, ctx->smol, central, ctx->snc);
     // pair list
     const double rcr2 = rcr * rcr, rca2 = rca * rca;
     bool wrap = false;     // same rule as k_setup_grid: a periodic axis with fewer than 3 cells
@@ -683,18 +693,18 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
     }
     if (wrap)
         DHP_LAUNCH(ctx, k_pairs<true>, (int)cell_bound, P1_THREADS, 0, ctx->spos, ctx->grid, ctx->cell_start, rcr2, rca2,
-                   ctx->tmp_stride, ctx->n_rad, ctx->tmp_col, ctx->blk_sum, ctx->status);
+                   ctx->tmp_stride, ctx->n_rad, ctx->tmp_col, ctx->blk_sum, ctx->status, snc);
     else
         DHP_LAUNCH(ctx, k_pairs<false>, (int)cell_bound, P1_THREADS, 0, ctx->spos, ctx->grid, ctx->cell_start, rcr2, rca2,
-                   ctx->tmp_stride, ctx->n_rad, ctx->tmp_col, ctx->blk_sum, ctx->status);
+                   ctx->tmp_stride, ctx->n_rad, ctx->tmp_col, ctx->blk_sum, ctx->status, snc);
     DHP_LAUNCH(ctx, k_scan_blocks, 1, 1024, 0, ctx->blk_sum, ctx->blk_off, nblk, ctx->pair_cap, ctx->status);
     DHP_LAUNCH(ctx, k_rows, nblk, P2_THREADS, 0, ctx->tmp_col, ctx->tmp_stride, ctx->n_rad, ctx->blk_off, nblk, n, ctx->row_ptr,
                ctx->col, ctx->n_rad, ctx->n_ang, ctx->seg_cnt, ctx->amask);
     // rows grouped by species, ordered by feature-block class inside a group; tile masks
     const int nrb = (n + RB - 1) / RB;
-    DHP_LAUNCH(ctx, k_rowkey_hist, nrb, RB, 0, ctx->spos, ctx->amask, n, nrb, ctx->blk_hist);
+    DHP_LAUNCH(ctx, k_rowkey_hist, nrb, RB, 0, ctx->spos, ctx->amask, snc, n, nrb, ctx->blk_hist);
     DHP_LAUNCH(ctx, k_rowkey_scan, 1, 1024, 0, ctx->blk_hist, nrb, ctx->sp_count, ctx->sp_start, ctx->key_start);
-    DHP_LAUNCH(ctx, k_rowkey_rank, nrb, RB, 0, ctx->spos, ctx->amask, n, nrb, ctx->blk_hist, ctx->key_start, ctx->rowmap,
+    DHP_LAUNCH(ctx, k_rowkey_rank, nrb, RB, 0, ctx->spos, ctx->amask, snc, n, nrb, ctx->blk_hist, ctx->key_start, ctx->rowmap,
                ctx->row_species, ctx->row_slot, ctx->tile_mask);
     DHP_CUDA(ctx, cudaGetLastError());
     return DHP_OK;

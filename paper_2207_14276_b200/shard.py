@@ -95,3 +95,35 @@ def sum_partial_forces(E_partial, F_partial, group=None):
     dist.all_reduce(F_partial, op=dist.ReduceOp.SUM, group=group)
     dist.all_reduce(E_partial, op=dist.ReduceOp.SUM, group=group)
     return E_partial, F_partial
+
+
+# ---- device side: one large system over N GPUs -------------------------------
+def slab_mask_device(pos, box, world: int, rank: int, axis: int = 0):
+    """`slab_owner(...) == rank` evaluated with torch ops on the device that holds `pos` (fp32 [N, 3]): the uint8
+    central-atom mask `dhp_ani_energy_forces_partial` takes.  Same rule as `slab_owner` (wrap into [0, L), stable
+    sort, equal counts), so every rank derives the same partition from the same positions.  Index arithmetic only."""
+    import torch
+    x = pos[:, axis].to(torch.float64)
+    if box is not None:
+        L = float(box[axis])
+        x = x - L * torch.floor(x / L)
+    order = torch.argsort(x, stable=True)
+    lo, hi = shard_range(int(x.numel()), world, rank)
+    mask = torch.zeros(x.numel(), dtype=torch.uint8, device=pos.device)
+    mask[order[lo:hi]] = 1
+    return mask
+
+
+def ani_energy_forces_sharded(dhp, pos, box, species, weights, central, mol_offsets=None, group=None):
+    """One evaluation of a system whose central atoms are partitioned over the ranks of `group`.
+
+    Every rank holds all positions (after an MD step: all-gather of the owned slices, 1.6 MB at 98 k atoms), runs
+    a1-a5 for its own central atoms only (`central`, from `slab_mask_device`) and the partial energies and forces
+    are summed over ranks - one all-reduce of F (1.2 MB) and one of E (8 B) on NCCL, enqueued on the stream the
+    kernels ran on, no host synchronisation.  Returns the total (E, F), identical on every rank."""
+    import torch.distributed as dist
+    E, F = dhp.dhp_ani_energy_forces_partial(pos, box, species, weights, central, mol_offsets)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1:
+        dist.all_reduce(F, op=dist.ReduceOp.SUM, group=group)
+        dist.all_reduce(E, op=dist.ReduceOp.SUM, group=group)
+    return E, F

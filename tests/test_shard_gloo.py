@@ -80,6 +80,18 @@ def _worker(rank, port, results):
         E_part = torch.tensor([Ec.sum()], dtype=torch.float64)
         F_part = torch.from_numpy(Fc.copy())
         shard.sum_partial_forces(E_part, F_part)
+        # (2b) the same through shard.ani_energy_forces_sharded with the device-side slab rule (torch ops, here on
+        # CPU tensors) and a stand-in context whose partial call is played by the oracle
+        class OracleCtx:
+            def dhp_ani_energy_forces_partial(self, pos, box, species, weights, central, mol_offsets=None):
+                c = np.nonzero(central.numpy())[0].astype(np.int32)
+                Ec, Fc, _ = oracle.energy_forces(pos.numpy(), species.numpy(), box, params, weights, 1, centres=c)
+                return torch.tensor([Ec.sum()], dtype=torch.float64), torch.from_numpy(Fc.copy())
+        pos_t, sp_t = torch.from_numpy(w.pos), torch.from_numpy(w.species)
+        mask = shard.slab_mask_device(pos_t, w.box, WORLD, rank)
+        assert np.array_equal(np.nonzero(mask.numpy())[0], centres)
+        E_sh, F_sh = shard.ani_energy_forces_sharded(OracleCtx(), pos_t, w.box, sp_t, blob, mask)
+        assert abs(E_sh.item() - E_part.item()) <= 1e-12 and np.max(np.abs(F_sh.numpy() - F_part.numpy())) <= 1e-14
         # (3) timing: slowest rank
         t = shard.max_over_ranks([1.0 + rank, 5.0 - rank])
         if rank == 0:
