@@ -118,6 +118,18 @@ int dhp_weights_free(dhp_ctx* ctx, dhp_weights* w);
 int dhp_nlist_build(dhp_ctx* ctx, const float* pos, const float* box, const int32_t* species, int64_t n_atoms,
                     const int32_t* mol_offsets, int64_t n_mol, float rc, dhp_nlist** out);
 
+/* Verlet-skin list reuse ("atomic positions do not move much between two time-steps").  skin > 0 (Å,
+ * <= 4): a full build also records every pair within rc + skin; later calls on the same context with the same
+ * n_atoms, box, mol_offsets pointer and masked/unmasked mode reuse the cell sort, the row assignment and that
+ * candidate list for as long as no atom has moved more than skin/2 from the positions of the last full build (and
+ * no atom changed species or central role) - checked on the device on every call, so a stale list is never used and
+ * no host synchronisation is needed.  The list of every call is still exactly the canonical one (candidates are
+ * filtered by the same fp64 predicate on the current positions).  skin = 0 (default) rebuilds on every call and
+ * frees the candidate storage.  Setup call: allocates, synchronises.  Errors: BADARG, NOMEM. */
+int dhp_set_skin(dhp_ctx* ctx, float skin);
+/* Full builds since dhp_set_skin(skin > 0) (synchronises); every other hot call reused the candidate list. */
+int64_t dhp_nlist_rebuild_count(dhp_ctx* ctx);
+
 /* Number of directed pairs in the radial (<= rcr) and angular (<= rca) lists.  Synchronises. */
 int dhp_nlist_sizes(dhp_ctx* ctx, const dhp_nlist* nl, int64_t* nnz, int64_t* nnz_ang);
 

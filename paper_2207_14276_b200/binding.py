@@ -29,6 +29,8 @@ SYMBOLS = {
     "dhp_weights_load": (C.c_int, [_vp, _vp, _i64, _i32, C.POINTER(_vp)]),
     "dhp_weights_free": (C.c_int, [_vp, _vp]),
     "dhp_nlist_build": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _vp, _i64, _f32, C.POINTER(_vp)]),
+    "dhp_set_skin": (C.c_int, [_vp, _f32]),
+    "dhp_nlist_rebuild_count": (_i64, [_vp]),
     "dhp_nlist_sizes": (C.c_int, [_vp, _vp, C.POINTER(_i64), C.POINTER(_i64)]),
     "dhp_nlist_export": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp]),
     "dhp_ani_energy_forces": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _vp, _i64, _vp, _i32, _vp, _vp]),
@@ -175,6 +177,12 @@ class Dhp:
                                         _vp(_dptr(mol_offsets)), n_mol, C.c_float(self.rcr), C.byref(h)), self.ctx)
         self._nlist, self._n = h, n
         return h
+
+    def dhp_set_skin(self, skin: float):
+        _check(self.lib.dhp_set_skin(self.ctx, C.c_float(float(skin))), self.ctx)
+
+    def dhp_nlist_rebuild_count(self) -> int:
+        return int(self.lib.dhp_nlist_rebuild_count(self.ctx))
 
     def dhp_nlist_sizes(self):
         a, b = _i64(), _i64()

@@ -1,5 +1,6 @@
 // C ABI of libdhp.so (include/dhp.h): context / workspace, weight handles, the two hot calls.
 #include <math.h>
+#include <initializer_list>
 #include <new>
 #include <stdio.h>
 #include <stdlib.h>
@@ -42,7 +43,7 @@ static void free_all(Ctx* c) {
     void* ptrs[] = {c->grid, c->status, c->bbox, c->cell_of, c->perm_tmp, c->cell_count, c->cell_start, c->cell_fill, c->perm,
                     c->inv_perm, c->spos, c->smol, c->snc, c->n_rad, c->n_ang, c->row_ptr, c->col, c->sp_count, c->sp_start,
                     c->rowmap, c->row_species, c->row_slot, c->blk_hist, c->key_start, c->amask, c->tile_mask, c->tc_sched, c->col2feat, c->aev, c->grad, c->e_atom, c->fsorted,
-                    c->e_out_tmp, c->export_tmp, c->tmp_col, c->blk_sum, c->blk_off, c->seg_cnt, c->st_pos, c->st_species, c->st_mol, c->st_E, c->st_F};
+                    c->e_out_tmp, c->export_tmp, c->cand, c->cand_cnt, c->pos_ref, c->rebuild, c->rebuild_count, c->tmp_col, c->blk_sum, c->blk_off, c->seg_cnt, c->st_pos, c->st_species, c->st_mol, c->st_E, c->st_F};
     for (void* p : ptrs) if (p) cudaFree(p);
     mlp_simt_free(c);
     mlp_tc_free(c);
@@ -377,6 +378,41 @@ int dhp_set_mlp_mode(dhp_ctx* h, int mode) {
     if (mode >= DHP_MLP_TENSOR && !mlp_tc_available(&h->c)) return DHP_E_NOTIMPL;
     h->c.mlp_mode = mode;
     return DHP_OK;
+}
+
+int dhp_set_skin(dhp_ctx* h, float skin) {
+    if (!h || !(skin >= 0.f) || skin > 4.0f) return DHP_E_BADARG;
+    Ctx* c = &h->c;
+    cudaStreamSynchronize(c->stream);
+    for (void* p : {(void*)c->cand, (void*)c->cand_cnt, (void*)c->pos_ref, (void*)c->rebuild, (void*)c->rebuild_count}) if (p) cudaFree(p);
+    c->cand = nullptr; c->cand_cnt = nullptr; c->pos_ref = nullptr; c->rebuild = nullptr; c->rebuild_count = nullptr;
+    c->skin = 0.f; c->cand_valid = false; c->cand_stride = 0;
+    if (skin == 0.f) return DHP_OK;
+    // candidate rows scale with the list volume: tmp_stride x ((rcr + skin) / rcr)^3, in whole warps
+    const double f = ((double)c->params.rcr + skin) / (double)c->params.rcr;
+    int64_t stride = ((int64_t)ceil(c->tmp_stride * f * f * f) + 31) / 32 * 32;
+    if (stride > c->max_atoms - 1) stride = c->max_atoms > 1 ? c->max_atoms - 1 : 1;
+    const size_t N = (size_t)c->max_atoms;
+    bool ok = dalloc(&c->cand, N * (size_t)stride) && dalloc(&c->cand_cnt, N) && dalloc(&c->pos_ref, 3 * N) && dalloc(&c->rebuild, 1) &&
+              dalloc(&c->rebuild_count, 1);
+    if (ok) ok = cudaMemset(c->rebuild_count, 0, sizeof(int)) == cudaSuccess;
+    if (!ok) {
+        cudaGetLastError();
+        for (void* p : {(void*)c->cand, (void*)c->cand_cnt, (void*)c->pos_ref, (void*)c->rebuild, (void*)c->rebuild_count}) if (p) cudaFree(p);
+        c->cand = nullptr; c->cand_cnt = nullptr; c->pos_ref = nullptr; c->rebuild = nullptr; c->rebuild_count = nullptr;
+        return DHP_E_NOMEM;
+    }
+    c->cand_stride = (int)stride;
+    c->skin = skin;
+    return DHP_OK;
+}
+
+int64_t dhp_nlist_rebuild_count(dhp_ctx* h) {
+    if (!h || !h->c.rebuild_count) return 0;
+    int v = 0;
+    if (cudaMemcpyAsync(&v, h->c.rebuild_count, sizeof(int), cudaMemcpyDeviceToHost, h->c.stream) != cudaSuccess) return -1;
+    if (cudaStreamSynchronize(h->c.stream) != cudaSuccess) return -1;
+    return v;
 }
 
 int dhp_tensor_path_available(dhp_ctx* h) { return h && mlp_tc_available(&h->c) ? 1 : 0; }

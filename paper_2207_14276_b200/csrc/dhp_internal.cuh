@@ -110,6 +110,20 @@ struct Ctx {
     int* smol;             // [N] molecule of sorted atom (0 if none)
     unsigned char* snc;    // [N] 1 = sorted atom is NOT a central atom of this call (partial evaluation), else 0
     bool partial;          // the last list was built with a central-atom mask
+    // Verlet-skin reuse (dhp_set_skin): candidate pairs within rcr + skin of the positions of the last full build
+    float skin;            // 0 = every call rebuilds from scratch
+    unsigned* cand;        // [N][cand_stride] candidate entries: sorted slot | species << 28
+    int* cand_cnt;         // [N]
+    int cand_stride;
+    float* pos_ref;        // [N][3] caller-order positions of the last full build
+    int* rebuild;          // device flag of the current call: 1 = full build, 0 = candidate list reused
+    bool cand_valid;       // host-side: a candidate list exists for (cand_n, cand_box, cand_mol, cand_nmol, cand_central)
+    int64_t cand_n, cand_nmol;
+    float cand_box[4];     // [3] = 1 if periodic
+    const void* cand_mol;
+    bool cand_central;
+    int64_t n_rebuilds;    // full builds since dhp_set_skin (read back lazily: device counter)
+    int* rebuild_count;    // device counter
     int* n_rad;            // [N]
     int* n_ang;            // [N]
     int* row_ptr;          // [N+1]

@@ -10,6 +10,7 @@
 // grouped by the central atom's species (stable in sorted order), each group starting at a multiple
 // of ROW_TILE rows so that one MLP tile never mixes networks.
 #include <algorithm>
+#include <string.h>
 
 #include "dhp_internal.cuh"
 
@@ -64,10 +65,16 @@ __device__ void block_scan_excl(const int* __restrict__ in, int* __restrict__ ou
     if (tid == 0) out[n] = carry_s;
 }
 
+// Verlet-skin reuse (dhp_set_skin): whether a call rebuilds the cell grid and the candidate list or reuses them is
+// decided ON THE DEVICE (k_reuse_check), so the host enqueues both paths and every kernel of the path not taken
+// returns at once.  gate == nullptr (skin off): no check.
+#define DHP_GATE(gate, want) do { if ((gate) != nullptr && *(gate) != (want)) return; } while (0)
+
 // ---------------------------------------------------------------------------------------------
 // grid setup
 // ---------------------------------------------------------------------------------------------
-__global__ void k_bbox(const float* __restrict__ pos, int n, unsigned* __restrict__ bbox) {
+__global__ void k_bbox(const float* __restrict__ pos, int n, unsigned* __restrict__ bbox, const int* __restrict__ gate) {
+    DHP_GATE(gate, 1);
     float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f};
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
         for (int c = 0; c < 3; ++c) {
@@ -88,8 +95,11 @@ __global__ void k_bbox(const float* __restrict__ pos, int n, unsigned* __restric
 }
 
 __global__ void k_setup_grid(Grid* g, int periodic, double Lx, double Ly, double Lz, double rc,
-                             const unsigned* __restrict__ bbox, int max_cells, int by_molecule, int n_mol) {
+                             const unsigned* __restrict__ bbox, int max_cells, int by_molecule, int n_mol,
+                             const int* __restrict__ gate, int* __restrict__ rebuild_count) {
+    DHP_GATE(gate, 1);
     if (threadIdx.x || blockIdx.x) return;
+    if (rebuild_count) ++*rebuild_count;
     const double edge = rc * (1.0 + 9.5367431640625e-07);   // rc (1 + 2^-20): binning slack
     double L[3] = {Lx, Ly, Lz};
     g->periodic = periodic;
@@ -151,7 +161,9 @@ __device__ __forceinline__ int cell_coord(double x, double L, double origin, dou
 
 __global__ void k_assign_cells(const float* __restrict__ pos, const int* __restrict__ species, int n,
                                const int* __restrict__ mol_offsets, int n_mol, const Grid* __restrict__ g,
-                               int* __restrict__ cell_of, int* __restrict__ cell_count, int* __restrict__ status) {
+                               int* __restrict__ cell_of, int* __restrict__ cell_count, int* __restrict__ status,
+                               const int* __restrict__ gate) {
+    DHP_GATE(gate, 1);
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     int s = species[i];
@@ -174,12 +186,15 @@ __global__ void k_assign_cells(const float* __restrict__ pos, const int* __restr
     atomicAdd(&cell_count[cell], 1);
 }
 
-__global__ void k_scan_cells(const int* __restrict__ cnt, int* __restrict__ start, const Grid* __restrict__ g) {
+__global__ void k_scan_cells(const int* __restrict__ cnt, int* __restrict__ start, const Grid* __restrict__ g,
+                             const int* __restrict__ gate) {
+    DHP_GATE(gate, 1);
     block_scan_excl(cnt, start, g->ncell);
 }
 
 __global__ void k_scatter(const int* __restrict__ cell_of, int n, const int* __restrict__ cell_start,
-                          int* __restrict__ cell_fill, int* __restrict__ perm) {
+                          int* __restrict__ cell_fill, int* __restrict__ perm, const int* __restrict__ gate) {
+    DHP_GATE(gate, 1);
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     int c = cell_of[i];
@@ -190,7 +205,9 @@ __global__ void k_scatter(const int* __restrict__ cell_of, int n, const int* __r
 __global__ void k_sort_gather(const float* __restrict__ pos, const int* __restrict__ species,
                               const Grid* __restrict__ g, const int* __restrict__ cell_start, const int* __restrict__ perm_in,
                               int* __restrict__ perm, int* __restrict__ inv_perm, float4* __restrict__ spos,
-                              int* __restrict__ smol, const uint8_t* __restrict__ central, unsigned char* __restrict__ snc) {
+                              int* __restrict__ smol, const uint8_t* __restrict__ central, unsigned char* __restrict__ snc,
+                              const int* __restrict__ gate, float* __restrict__ pos_ref) {
+    DHP_GATE(gate, 1);
     const int c = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (c >= g->ncell) return;
     const int b = cell_start[c], e = cell_start[c + 1];
@@ -206,6 +223,7 @@ __global__ void k_sort_gather(const float* __restrict__ pos, const int* __restri
         spos[dst] = make_float4(pos[3 * v], pos[3 * v + 1], pos[3 * v + 2], __int_as_float(s));
         smol[dst] = g->by_molecule ? c : 0;
         if (central) snc[dst] = central[v] ? 0 : 1;
+        if (pos_ref) { pos_ref[3 * v] = pos[3 * v]; pos_ref[3 * v + 1] = pos[3 * v + 1]; pos_ref[3 * v + 2] = pos[3 * v + 2]; }
     }
 }
 
@@ -232,7 +250,8 @@ __device__ __forceinline__ int row_key(int s, unsigned m) {
 // blk_hist is key-major: blk_hist[key * nrb + block]
 __global__ void __launch_bounds__(RB)
 k_rowkey_hist(const float4* __restrict__ spos, const unsigned* __restrict__ amask, const unsigned char* __restrict__ snc, int n, int nrb,
-              int* __restrict__ blk_hist) {
+              int* __restrict__ blk_hist, const int* __restrict__ gate) {
+    DHP_GATE(gate, 1);
     __shared__ int h[NKEY];
     for (int k = threadIdx.x; k < NKEY; k += RB) h[k] = 0;
     __syncthreads();
@@ -245,7 +264,9 @@ k_rowkey_hist(const float4* __restrict__ spos, const unsigned* __restrict__ amas
 // single block of 1024 threads, warps take keys round-robin: exclusive scan over blocks per key, then the key starts
 // (species groups aligned to ROW_TILE)
 __global__ void __launch_bounds__(1024)
-k_rowkey_scan(int* __restrict__ blk_hist, int nrb, int* __restrict__ sp_count, int* __restrict__ sp_start, int* __restrict__ key_start) {
+k_rowkey_scan(int* __restrict__ blk_hist, int nrb, int* __restrict__ sp_count, int* __restrict__ sp_start, int* __restrict__ key_start,
+              const int* __restrict__ gate) {
+    DHP_GATE(gate, 1);
     __shared__ int tot[NKEY];
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     for (int key = w; key < NKEY; key += 32) {
@@ -284,7 +305,8 @@ __global__ void __launch_bounds__(RB)
 k_rowkey_rank(const float4* __restrict__ spos, const unsigned* __restrict__ amask, const unsigned char* __restrict__ snc, int n, int nrb,
               const int* __restrict__ blk_hist,
               const int* __restrict__ key_start, int* __restrict__ rowmap, int* __restrict__ row_species,
-              int* __restrict__ row_slot, unsigned* __restrict__ tile_mask) {
+              int* __restrict__ row_slot, unsigned* __restrict__ tile_mask, const int* __restrict__ gate) {
+    DHP_GATE(gate, 1);
     __shared__ int wcnt[RB / 32][NKEY];
     for (int k = threadIdx.x; k < (RB / 32) * NKEY; k += RB) (&wcnt[0][0])[k] = 0;
     __syncthreads();
@@ -360,11 +382,13 @@ constexpr int ROWS_PER_BLK = 64;        // granularity of the block-sum scan tha
 constexpr int CAND_TILE = 1024;        // candidates staged per tile (16 KB)
 constexpr unsigned ENT_RADIAL_ONLY = 0x80000000u;   // temp-row entry: bit 31 = beyond rca, bits 28..30 = species, low 28 = slot
 
-template <bool WRAP>
+template <bool WRAP, bool SKIN>
 __global__ void __launch_bounds__(P1_THREADS, 8)
 k_pairs(const float4* __restrict__ spos, const Grid* __restrict__ gp, const int* __restrict__ cell_start, double rcr2,
         double rca2, int stride, int* __restrict__ cnt, unsigned* __restrict__ tmp, int* __restrict__ blk_sum,
-        int* __restrict__ status, const unsigned char* __restrict__ snc) {
+        int* __restrict__ status, const unsigned char* __restrict__ snc, const int* __restrict__ gate, float rs2f,
+        int cstride, int* __restrict__ cand_cnt, unsigned* __restrict__ cand_out) {
+    DHP_GATE(gate, 1);
     __shared__ Grid g;
     __shared__ float4 cand[CAND_TILE + 32];
     __shared__ int seg_cell_b[28], seg_off[28], nseg_s;
@@ -450,11 +474,13 @@ k_pairs(const float4* __restrict__ spos, const Grid* __restrict__ gp, const int*
         // fp32 error bound of R^2 near a cutoff rc: |err| <= rc B 2^-19 + rc^2 2^-22; doubled
         const float mr = rcr * B * 3.8146973e-06f + rcr2f * 4.7683716e-07f;
         const float ma = rca * B * 3.8146973e-06f + rca2f * 4.7683716e-07f;
+        // candidates of the Verlet-skin list: everything the fp32 test cannot exclude from R <= rcr + skin
+        const float rs2_incl = SKIN ? rs2f + (sqrtf(rs2f) * B * 3.8146973e-06f + rs2f * 4.7683716e-07f) : 0.f;
 
         // ---- centre atoms of this cell, one warp each ----------------------------------------
         for (int i = cb + warp; i < ce; i += P1_THREADS / 32) {
             if (snc && snc[i]) {               // not a central atom of this call: an empty row
-                if (lane == 0 && t0 == 0) cnt[i] = 0;
+                if (lane == 0 && t0 == 0) { cnt[i] = 0; if (SKIN) cand_cnt[i] = 0; }
                 continue;
             }
             // the centre's own relative coordinates: same arithmetic as the staged copy
@@ -466,6 +492,7 @@ k_pairs(const float4* __restrict__ spos, const Grid* __restrict__ gp, const int*
             }
             const float pix = (float)ri[0], piy = (float)ri[1], piz = (float)ri[2];
             int base = t0 ? cnt[i] : 0;
+            int cbase = (SKIN && t0) ? cand_cnt[i] : 0;
             for (int c0 = 0; c0 < tn; c0 += 32) {
                 const float4 c = cand[c0 + lane];          // the tile is padded with far-away dummies
                 const int jj = __float_as_int(c.w);
@@ -493,8 +520,21 @@ k_pairs(const float4* __restrict__ spos, const Grid* __restrict__ gp, const int*
                     if (pos < stride) tmp[(size_t)i * stride + pos] = (unsigned)jj | (in_a ? 0u : ENT_RADIAL_ONLY);
                 }
                 base += __popc(m);
+                if (SKIN) {
+                    const bool in_c = other && r2 <= rs2_incl;
+                    const unsigned mc = __ballot_sync(0xffffffffu, in_c);
+                    if (in_c) {
+                        const int pos = cbase + __popc(mc & lt);
+                        if (pos < cstride) cand_out[(size_t)i * cstride + pos] = (unsigned)jj;
+                    }
+                    cbase += __popc(mc);
+                }
             }
             if (lane == 0) {
+                if (SKIN) {
+                    if (cbase > cstride) { atomicExch(status, DHP_E_CAPACITY); cbase = cstride; }
+                    cand_cnt[i] = cbase;
+                }
                 if (base > stride) { atomicExch(status, DHP_E_CAPACITY); base = stride; }
                 cnt[i] = base;
                 if (t0 + CAND_TILE >= ncand) atomicAdd(&blk_sum[i / ROWS_PER_BLK], base);
@@ -628,6 +668,114 @@ k_rows(const unsigned* __restrict__ tmp, int stride, const int* __restrict__ cnt
     }
 }
 
+
+// ---------------------------------------------------------------------------------------------
+// Verlet-skin reuse ("atomic positions do not move much between two time-steps").
+// The full build records every pair within rcr + skin (candidates).  While no atom has moved more than skin / 2
+// from the positions of that build, every pair within rcr now is a candidate, so the exact list of this call is
+// the candidates filtered by the canonical predicate on the CURRENT positions: still bit-exact.  The cell grid,
+// the sorted order, the species-grouped row assignment and the candidate rows are reused; pairs, rows' internal
+// order, feature-block masks and tile masks are recomputed.
+// ---------------------------------------------------------------------------------------------
+__global__ void k_set_flag(int* flag, int v) { *flag = v; }
+
+// flag := 1 (rebuild) if any atom moved more than skin/2 (thr2 = (skin/2)^2, shaved so that fp32 rounding errs on
+// the safe side), changed species, or changed its central / non-central role
+__global__ void k_reuse_check(const float* __restrict__ pos, const int* __restrict__ species, const float* __restrict__ pos_ref,
+                              const float4* __restrict__ spos, const int* __restrict__ inv_perm, const uint8_t* __restrict__ central,
+                              const unsigned char* __restrict__ snc, int n, float thr2, int* __restrict__ flag) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    bool bad = false;
+    if (i < n) {
+        const float dx = pos[3 * i] - pos_ref[3 * i], dy = pos[3 * i + 1] - pos_ref[3 * i + 1], dz = pos[3 * i + 2] - pos_ref[3 * i + 2];
+        const float d2 = dx * dx + dy * dy + dz * dz;
+        const int slot = inv_perm[i];
+        bad = !(d2 <= thr2) || species[i] != __float_as_int(spos[slot].w);      // NaN positions also force a rebuild
+        if (central) bad |= (central[i] ? 0 : 1) != snc[slot];
+    }
+    if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) *flag = 1;
+}
+
+__global__ void k_reset_rows(int* __restrict__ row_slot, int* __restrict__ row_species, int max_rows, const int* __restrict__ gate) {
+    DHP_GATE(gate, 1);
+    for (int r = blockIdx.x * blockDim.x + threadIdx.x; r < max_rows; r += gridDim.x * blockDim.x) { row_slot[r] = -1; row_species[r] = -1; }
+}
+
+// reuse: current positions into the sorted copy (species bits stay)
+__global__ void k_regather(const float* __restrict__ pos, const int* __restrict__ perm, int n, float4* __restrict__ spos,
+                           const int* __restrict__ gate) {
+    DHP_GATE(gate, 0);
+    const int a = blockIdx.x * blockDim.x + threadIdx.x;
+    if (a >= n) return;
+    const int v = perm[a];
+    spos[a] = make_float4(pos[3 * v], pos[3 * v + 1], pos[3 * v + 2], spos[a].w);
+}
+
+// reuse: one warp per central atom filters its candidates.  fp32 R^2 of the fp64 minimum-image displacement
+// (relative error < 2^-21) decides; within 2^-19 rc^2 of a cutoff the canonical fp64 predicate does.
+constexpr int RF_WARPS = 8;
+__global__ void __launch_bounds__(RF_WARPS * 32)
+k_refilter(const float4* __restrict__ spos, const Grid* __restrict__ gp, const unsigned* __restrict__ cand, const int* __restrict__ cand_cnt,
+           int cstride, double rcr2, double rca2, int stride, int n, int* __restrict__ cnt, unsigned* __restrict__ tmp,
+           int* __restrict__ blk_sum, int* __restrict__ status, const unsigned char* __restrict__ snc, const int* __restrict__ gate) {
+    DHP_GATE(gate, 0);
+    __shared__ Grid g;
+    if (threadIdx.x == 0) g = *gp;
+    __syncthreads();
+    const int lane = threadIdx.x & 31;
+    const int i = blockIdx.x * RF_WARPS + (threadIdx.x >> 5);
+    if (i >= n) return;
+    if (snc && snc[i]) { if (lane == 0) cnt[i] = 0; return; }
+    const float rcr2f = (float)rcr2, rca2f = (float)rca2;
+    const float mr = rcr2f * 1.9073486e-06f, ma = rca2f * 1.9073486e-06f;
+    const unsigned lt = (1u << lane) - 1u;
+    const float4 pi = spos[i];
+    const int nc = cand_cnt[i];
+    const unsigned* row = cand + (size_t)i * cstride;
+    int base = 0;
+    for (int c0 = 0; c0 < nc; c0 += 32) {
+        const bool have = c0 + lane < nc;
+        const unsigned e = have ? row[c0 + lane] : 0u;
+        const float4 pj = spos[e & 0x0fffffffu];
+        double d[3] = {(double)pj.x - (double)pi.x, (double)pj.y - (double)pi.y, (double)pj.z - (double)pi.z};
+        if (g.periodic) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) d[c] -= g.L[c] * rint(d[c] * g.inv_L[c]);
+        }
+        const float x = (float)d[0], y = (float)d[1], z = (float)d[2];
+        const float r2 = x * x + y * y + z * z;
+        bool in_r = have && r2 <= rcr2f;
+        bool in_a = have && r2 <= rca2f;
+        if (have && (fabsf(r2 - rcr2f) <= mr || fabsf(r2 - rca2f) <= ma)) {
+            const double r2d = pair_r2(pi, pj, g);
+            in_r = r2d <= rcr2;
+            in_a = r2d <= rca2;
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, in_r);
+        if (in_r) {
+            const int pos = base + __popc(m & lt);
+            if (pos < stride) tmp[(size_t)i * stride + pos] = e | (in_a ? 0u : ENT_RADIAL_ONLY);
+        }
+        base += __popc(m);
+    }
+    if (lane == 0) {
+        if (base > stride) { atomicExch(status, DHP_E_CAPACITY); base = stride; }
+        cnt[i] = base;
+        atomicAdd(&blk_sum[i / ROWS_PER_BLK], base);
+    }
+}
+
+// reuse: the row assignment of the last full build stays; the tile masks follow the current feature-block masks
+__global__ void k_tilemask(const unsigned* __restrict__ amask, const int* __restrict__ rowmap, int n, unsigned* __restrict__ tile_mask,
+                           const int* __restrict__ gate) {
+    DHP_GATE(gate, 0);
+    const int a = blockIdx.x * blockDim.x + threadIdx.x;
+    if (a >= n) return;
+    const int row = rowmap[a];
+    const unsigned m = amask[a];
+    if (row >= 0 && m) atomicOr(&tile_mask[row / ROW_TILE], m);
+}
+
 // ---------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------
@@ -644,68 +792,102 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
     const unsigned char* snc = central ? ctx->snc : nullptr;
     cudaStream_t st = ctx->stream;
     const int nblk = (n + ROWS_PER_BLK - 1) / ROWS_PER_BLK;
+    const bool skin = ctx->skin > 0.f && ctx->cand != nullptr && n > 0;
+    const int* gate = skin ? ctx->rebuild : nullptr;             // nullptr: every kernel of the build path runs
+    const double rl = rcr + (skin ? (double)ctx->skin : 0.0);    // list radius: the cell grid must cover it
 
     DHP_CUDA(ctx, cudaMemsetAsync(ctx->status, 0, sizeof(int), st));
     DHP_CUDA(ctx, cudaMemsetAsync(ctx->cell_count, 0, sizeof(int) * (ctx->max_cells + 1), st));
     DHP_CUDA(ctx, cudaMemsetAsync(ctx->cell_fill, 0, sizeof(int) * ctx->max_cells, st));
-    DHP_CUDA(ctx, cudaMemsetAsync(ctx->row_slot, 0xFF, sizeof(int) * ctx->max_rows, st));
-    DHP_CUDA(ctx, cudaMemsetAsync(ctx->row_species, 0xFF, sizeof(int) * ctx->max_rows, st));
     DHP_CUDA(ctx, cudaMemsetAsync(ctx->tile_mask, 0, sizeof(unsigned) * (ctx->max_rows / ROW_TILE), st));
+    if (!skin) {
+        DHP_CUDA(ctx, cudaMemsetAsync(ctx->row_slot, 0xFF, sizeof(int) * ctx->max_rows, st));
+        DHP_CUDA(ctx, cudaMemsetAsync(ctx->row_species, 0xFF, sizeof(int) * ctx->max_rows, st));
+        ctx->cand_valid = false;
+    }
     if (n == 0) {
         DHP_CUDA(ctx, cudaMemsetAsync(ctx->row_ptr, 0, sizeof(int), st));
         DHP_CUDA(ctx, cudaMemsetAsync(ctx->sp_count, 0, sizeof(int) * 8, st));
         DHP_CUDA(ctx, cudaMemsetAsync(ctx->sp_start, 0, sizeof(int) * 8, st));
+        ctx->cand_valid = false;
         return DHP_OK;
     }
     DHP_CUDA(ctx, cudaMemsetAsync(ctx->blk_sum, 0, sizeof(int) * (nblk + 2), st));
     double L[3] = {0, 0, 0};
     if (periodic) for (int c = 0; c < 3; ++c) L[c] = (double)box_host[c];
+    const int nb = (n + 255) / 256;
+    if (skin) {
+        // reuse is possible only for the same problem (size, box, molecule table, masked or not); whether the atoms
+        // have stayed within skin / 2 of the last full build is decided on the device
+        const float bx[4] = {(float)L[0], (float)L[1], (float)L[2], periodic ? 1.f : 0.f};
+        const bool same = ctx->cand_valid && ctx->cand_n == n && ctx->cand_nmol == (by_mol ? n_mol : 0) && ctx->cand_mol == (const void*)mol_offsets &&
+                          ctx->cand_central == (central != nullptr) && memcmp(bx, ctx->cand_box, sizeof(bx)) == 0;
+        if (same) {
+            DHP_CUDA(ctx, cudaMemsetAsync(ctx->rebuild, 0, sizeof(int), st));
+            const float h = 0.5f * ctx->skin;
+            DHP_LAUNCH(ctx, k_reuse_check, nb, 256, 0, pos, species, ctx->pos_ref, ctx->spos, ctx->inv_perm, central, ctx->snc, n,
+                       h * h * 0.9999f, ctx->rebuild);
+        } else {
+            DHP_LAUNCH(ctx, k_set_flag, 1, 1, 0, ctx->rebuild, 1);
+        }
+        ctx->cand_valid = true; ctx->cand_n = n; ctx->cand_nmol = by_mol ? n_mol : 0; ctx->cand_mol = (const void*)mol_offsets;
+        ctx->cand_central = central != nullptr; memcpy(ctx->cand_box, bx, sizeof(bx));
+        DHP_LAUNCH(ctx, k_reset_rows, 2 * ctx->sm_count, 256, 0, ctx->row_slot, ctx->row_species, (int)ctx->max_rows, gate);
+    }
     if (!periodic && !by_mol) {
         static const unsigned init[6] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0u, 0u, 0u};
         DHP_CUDA(ctx, cudaMemcpyAsync(ctx->bbox, init, sizeof(init), cudaMemcpyHostToDevice, st));
         int blocks = (int)std::min<int64_t>((n + 255) / 256, 4 * ctx->sm_count);
-        DHP_LAUNCH(ctx, k_bbox, blocks, 256, 0, pos, n, ctx->bbox);
+        DHP_LAUNCH(ctx, k_bbox, blocks, 256, 0, pos, n, ctx->bbox, gate);
     }
-    DHP_LAUNCH(ctx, k_setup_grid, 1, 32, 0, ctx->grid, periodic ? 1 : 0, L[0], L[1], L[2], rcr, ctx->bbox,
-               (int)ctx->max_cells, by_mol ? 1 : 0, n_mol);
-    const int nb = (n + 255) / 256;
+    DHP_LAUNCH(ctx, k_setup_grid, 1, 32, 0, ctx->grid, periodic ? 1 : 0, L[0], L[1], L[2], rl, ctx->bbox,
+               (int)ctx->max_cells, by_mol ? 1 : 0, n_mol, gate, skin ? ctx->rebuild_count : (int*)nullptr);
     DHP_LAUNCH(ctx, k_assign_cells, nb, 256, 0, pos, species, n, mol_offsets, n_mol, ctx->grid, ctx->cell_of,
-               ctx->cell_count, ctx->status);
-    DHP_LAUNCH(ctx, k_scan_cells, 1, 1024, 0, ctx->cell_count, ctx->cell_start, ctx->grid);
-    DHP_LAUNCH(ctx, k_scatter, nb, 256, 0, ctx->cell_of, n, ctx->cell_start, ctx->cell_fill, ctx->perm_tmp);
+               ctx->cell_count, ctx->status, gate);
+    DHP_LAUNCH(ctx, k_scan_cells, 1, 1024, 0, ctx->cell_count, ctx->cell_start, ctx->grid, gate);
+    DHP_LAUNCH(ctx, k_scatter, nb, 256, 0, ctx->cell_of, n, ctx->cell_start, ctx->cell_fill, ctx->perm_tmp, gate);
     // the cell count lives on the device; launch for the bound and let surplus blocks exit
     int64_t cell_bound = by_mol ? n_mol : ctx->max_cells;
     if (periodic) {
         int64_t t = 1;
-        for (int c = 0; c < 3; ++c) t *= (int64_t)fmax(1.0, floor(L[c] / rcr));
+        for (int c = 0; c < 3; ++c) t *= (int64_t)fmax(1.0, floor(L[c] / rl));
         cell_bound = t < cell_bound ? t : cell_bound;
     }
     DHP_LAUNCH(ctx, k_sort_gather, (int)((cell_bound + 3) / 4), 128, 0, pos, species, ctx->grid, ctx->cell_start,
-               ctx->perm_tmp, ctx->perm, ctx->inv_perm, ctx->spos, ctx->smol, central, ctx->snc);
+               ctx->perm_tmp, ctx->perm, ctx->inv_perm, ctx->spos, ctx->smol, central, ctx->snc, gate,
+               skin ? ctx->pos_ref : (float*)nullptr);
     // pair list
     const double rcr2 = rcr * rcr, rca2 = rca * rca;
     bool wrap = false;     // same rule as k_setup_grid: a periodic axis with fewer than 3 cells
     if (periodic) {
-        const double edge = rcr * (1.0 + 9.5367431640625e-07);
+        const double edge = rl * (1.0 + 9.5367431640625e-07);
         for (int c = 0; c < 3; ++c) wrap |= floor(L[c] / edge) < 3.0;
         // k_setup_grid may coarsen the grid when it exceeds max_cells; be conservative then
         if ((double)floor(L[0] / edge) * floor(L[1] / edge) * floor(L[2] / edge) > (double)ctx->max_cells) wrap = true;
     }
-    if (wrap)
-        DHP_LAUNCH(ctx, k_pairs<true>, (int)cell_bound, P1_THREADS, 0, ctx->spos, ctx->grid, ctx->cell_start, rcr2, rca2,
-                   ctx->tmp_stride, ctx->n_rad, ctx->tmp_col, ctx->blk_sum, ctx->status, snc);
-    else
-        DHP_LAUNCH(ctx, k_pairs<false>, (int)cell_bound, P1_THREADS, 0, ctx->spos, ctx->grid, ctx->cell_start, rcr2, rca2,
-                   ctx->tmp_stride, ctx->n_rad, ctx->tmp_col, ctx->blk_sum, ctx->status, snc);
+    const float rs2f = (float)(rl * rl);
+#define DHP_PAIRS(W, S)                                                                                                        \
+    DHP_LAUNCH(ctx, (k_pairs<W, S>), (int)cell_bound, P1_THREADS, 0, ctx->spos, ctx->grid, ctx->cell_start, rcr2, rca2,       \
+               ctx->tmp_stride, ctx->n_rad, ctx->tmp_col, ctx->blk_sum, ctx->status, snc, gate, rs2f, ctx->cand_stride,       \
+               ctx->cand_cnt, ctx->cand)
+    if (wrap) { if (skin) DHP_PAIRS(true, true); else DHP_PAIRS(true, false); }
+    else      { if (skin) DHP_PAIRS(false, true); else DHP_PAIRS(false, false); }
+#undef DHP_PAIRS
+    if (skin) {
+        DHP_LAUNCH(ctx, k_regather, nb, 256, 0, pos, ctx->perm, n, ctx->spos, gate);
+        DHP_LAUNCH(ctx, k_refilter, (n + RF_WARPS - 1) / RF_WARPS, RF_WARPS * 32, 0, ctx->spos, ctx->grid, ctx->cand, ctx->cand_cnt,
+                   ctx->cand_stride, rcr2, rca2, ctx->tmp_stride, n, ctx->n_rad, ctx->tmp_col, ctx->blk_sum, ctx->status, snc, gate);
+    }
     DHP_LAUNCH(ctx, k_scan_blocks, 1, 1024, 0, ctx->blk_sum, ctx->blk_off, nblk, ctx->pair_cap, ctx->status);
     DHP_LAUNCH(ctx, k_rows, nblk, P2_THREADS, 0, ctx->tmp_col, ctx->tmp_stride, ctx->n_rad, ctx->blk_off, nblk, n, ctx->row_ptr,
                ctx->col, ctx->n_rad, ctx->n_ang, ctx->seg_cnt, ctx->amask);
     // rows grouped by species, ordered by feature-block class inside a group; tile masks
     const int nrb = (n + RB - 1) / RB;
-    DHP_LAUNCH(ctx, k_rowkey_hist, nrb, RB, 0, ctx->spos, ctx->amask, snc, n, nrb, ctx->blk_hist);
-    DHP_LAUNCH(ctx, k_rowkey_scan, 1, 1024, 0, ctx->blk_hist, nrb, ctx->sp_count, ctx->sp_start, ctx->key_start);
+    DHP_LAUNCH(ctx, k_rowkey_hist, nrb, RB, 0, ctx->spos, ctx->amask, snc, n, nrb, ctx->blk_hist, gate);
+    DHP_LAUNCH(ctx, k_rowkey_scan, 1, 1024, 0, ctx->blk_hist, nrb, ctx->sp_count, ctx->sp_start, ctx->key_start, gate);
     DHP_LAUNCH(ctx, k_rowkey_rank, nrb, RB, 0, ctx->spos, ctx->amask, snc, n, nrb, ctx->blk_hist, ctx->key_start, ctx->rowmap,
-               ctx->row_species, ctx->row_slot, ctx->tile_mask);
+               ctx->row_species, ctx->row_slot, ctx->tile_mask, gate);
+    if (skin) DHP_LAUNCH(ctx, k_tilemask, nb, 256, 0, ctx->amask, ctx->rowmap, n, ctx->tile_mask, gate);
     DHP_CUDA(ctx, cudaGetLastError());
     return DHP_OK;
 }
