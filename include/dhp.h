@@ -168,6 +168,28 @@ int dhp_ani_energy_forces_partial(dhp_ctx* ctx, const float* pos, const float* b
                                   const dhp_weights* weights, int n_models, const uint8_t* central,
                                   double* E, float* F);
 
+/* Multiple-timestep driver around the hot path (§2.4, Eqs. 8-9: the neural-network potential is
+ * evaluated only at the OUTERMOST timestep; velocity Verlet, L144).  V_slow = the ANI potential of this library,
+ * V_fast = harmonic bonds 1/2 k (r - r0)^2 - a stand-in for the bonded terms the paper keeps in the inner loop.
+ * One outer step of length dt with n_inner inner steps d = dt / n_inner:
+ *     v += (dt/2) a_slow ; [ v += (d/2) a_fast ; x += d v ; v += (d/2) a_fast ]^n_inner ; v += (dt/2) a_slow
+ * (n_inner = 1 or n_bonds = 0: plain velocity Verlet with the total force).
+ *   inv_mass  [n_atoms] acceleration per unit force, (Å/fs^2)/(Hartree/Å): 0.2625499639 / (mass in amu)
+ *   bonds     int32 [n_bonds][2] atom pairs; bond_k Hartree/Å^2; bond_r0 Å    (host or device; copied at create)
+ *   pos, vel  dev fp32 [n_atoms][3], Å and Å/fs, updated IN PLACE; positions are never re-wrapped into the box
+ *   box, species, weights, n_models  as in dhp_ani_energy_forces (no mol_offsets: one system)
+ *   E_out     dev fp64 [3] or NULL: E_ANI and E_bonds at the final positions, kinetic energy at the final velocities
+ * dhp_md_run enqueues n_steps outer steps on the context stream without any host synchronisation; with
+ * dhp_set_skin(skin > 0) the ANI calls reuse the neighbour list between outer steps.  The forces at the current
+ * positions are carried from one run to the next; call dhp_md_reset after changing pos from outside. */
+typedef struct dhp_md dhp_md;
+int dhp_md_create(dhp_ctx* ctx, int64_t n_atoms, const float* inv_mass, const int32_t* bonds, const float* bond_k,
+                  const float* bond_r0, int64_t n_bonds, dhp_md** out);
+int dhp_md_destroy(dhp_ctx* ctx, dhp_md* md);
+int dhp_md_reset(dhp_ctx* ctx, dhp_md* md);
+int dhp_md_run(dhp_ctx* ctx, dhp_md* md, float* pos, float* vel, const float* box, const int32_t* species,
+               const dhp_weights* weights, int n_models, float dt, int n_inner, int n_steps, double* E_out);
+
 /* Same computation with HOST buffers (pos, species, mol_offsets, E, F all host; pinned memory makes
  * the copies asynchronous): host->device copies, the kernels, device->host copies and one stream
  * synchronisation all happen inside the call.  This is the end-to-end entry point bench.py times. */

@@ -37,6 +37,10 @@ SYMBOLS = {
     "dhp_ani_energy_forces_partial": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _vp, _i64, _vp, _i32, _vp, _vp, _vp]),
     "dhp_ani_energy": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _vp, _i64, _vp, _i32, _vp]),
     "dhp_ani_energy_forces_host": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _vp, _i64, _vp, _i32, _vp, _vp]),
+    "dhp_md_create": (C.c_int, [_vp, _i64, _vp, _vp, _vp, _vp, _i64, C.POINTER(_vp)]),
+    "dhp_md_destroy": (C.c_int, [_vp, _vp]),
+    "dhp_md_reset": (C.c_int, [_vp, _vp]),
+    "dhp_md_run": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _i32, _f32, _i32, _i32, _vp]),
     "dhp_status": (C.c_int, [_vp]),
     "dhp_set_mlp_mode": (C.c_int, [_vp, _i32]),
     "dhp_tensor_path_available": (C.c_int, [_vp]),
@@ -264,6 +268,39 @@ class Dhp:
                                                    _vp(_dptr(E)), _vp(_dptr(F))), self.ctx)
         self._n = n
         return E, F
+
+    # ---- multiple-timestep driver (Eqs. 8-9)
+    def dhp_md_create(self, inv_mass, bonds=None, bond_k=None, bond_r0=None):
+        """inv_mass fp32 [N]; bonds int32 [n_bonds,2], bond_k / bond_r0 fp32 [n_bonds] (numpy or cuda tensors)."""
+        def prep(a, dt):
+            if a is None:
+                return None
+            return np.ascontiguousarray(a, dtype=dt) if isinstance(a, np.ndarray) else a.contiguous()
+        inv_mass, bonds = prep(inv_mass, np.float32), prep(bonds, np.int32)
+        bond_k, bond_r0 = prep(bond_k, np.float32), prep(bond_r0, np.float32)
+        nb = 0 if bonds is None else int(bonds.shape[0])
+        h = _vp()
+        _check(self.lib.dhp_md_create(self.ctx, int(inv_mass.shape[0]), _vp(_dptr(inv_mass)), _vp(_dptr(bonds)),
+                                      _vp(_dptr(bond_k)), _vp(_dptr(bond_r0)), nb, C.byref(h)), self.ctx)
+        return h
+
+    def dhp_md_destroy(self, md):
+        _check(self.lib.dhp_md_destroy(self.ctx, md), self.ctx)
+
+    def dhp_md_reset(self, md):
+        _check(self.lib.dhp_md_reset(self.ctx, md), self.ctx)
+
+    def dhp_md_run(self, md, pos, vel, box, species, weights, dt: float, n_inner: int, n_steps: int, E_out=None):
+        """n_steps outer steps in place on the cuda tensors pos, vel.  Returns E_out (fp64 [3] cuda: E_ANI, E_bonds, E_kin)."""
+        t = self.torch
+        boxh = None if box is None else np.ascontiguousarray(box, dtype=np.float32)
+        if E_out is None:
+            E_out = t.empty(3, dtype=t.float64, device=self.device)
+        _check(self.lib.dhp_md_run(self.ctx, md, _vp(_dptr(pos)), _vp(_dptr(vel)), _vp(_dptr(boxh)), _vp(_dptr(species)),
+                                   weights, weights.n_models, C.c_float(float(dt)), int(n_inner), int(n_steps),
+                                   _vp(_dptr(E_out))), self.ctx)
+        self._n = int(pos.shape[0])
+        return E_out
 
     def dhp_status(self) -> int:
         return int(self.lib.dhp_status(self.ctx))

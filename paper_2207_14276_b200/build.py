@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdhp.so")
-SOURCES = ["api.cu", "nlist.cu", "aev.cu", "mlp_simt.cu", "mlp_tc.cu"]
+SOURCES = ["api.cu", "nlist.cu", "aev.cu", "mlp_simt.cu", "mlp_tc.cu", "md.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-O2", "--fmad=true"]

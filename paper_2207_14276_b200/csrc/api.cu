@@ -163,7 +163,6 @@ using namespace dhp;
 
 extern "C" {
 
-struct dhp_ctx { Ctx c; };
 struct dhp_nlist { Ctx* owner; };
 struct dhp_weights { Weights w; };
 static dhp_nlist g_nlist_token;   // the list lives in the context workspace; the handle is a token

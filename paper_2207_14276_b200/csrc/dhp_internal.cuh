@@ -228,3 +228,5 @@ __host__ __device__ inline int col2feat(int c) {
 }
 
 }  // namespace dhp
+
+struct dhp_ctx { dhp::Ctx c; };   // the opaque handle of include/dhp.h

@@ -1,0 +1,184 @@
+// f1 — multiple-timestep driver around the hot path (§2.4, Eqs. 8-9; velocity Verlet L144).
+//
+// The paper's RESPA split evaluates the neural-network potential only at the OUTERMOST timestep and keeps cheap
+// bonded terms in the inner loop.  Here: V_slow = the ANI potential (dhp_ani_energy_forces, a1..a5), V_fast =
+// harmonic bonds 1/2 k (r - r0)^2 (a stand-in for the bonded terms; AMOEBA is out of scope).  One outer step of
+// length dt with n inner steps of length d = dt / n is the symmetric factorisation
+//     v += (dt/2) a_slow ; [ v += (d/2) a_fast ; x += d v ; v += (d/2) a_fast ]^n ; v += (dt/2) a_slow
+// which for n = 1 (or no bonds) is plain velocity Verlet with the total force.  Everything is enqueued on the
+// context's stream; there is no host synchronisation inside a run, and with dhp_set_skin the neighbour list of
+// the ANI call is reused between outer steps ("atomic positions do not move much between two time-steps", L134).
+#include <initializer_list>
+#include <new>
+#include <string.h>
+
+#include "dhp_internal.cuh"
+
+namespace dhp {
+
+struct Md {
+    int64_t n_atoms, n_bonds;
+    float* inv_mass;   // [N]  (Å/fs^2) per (Hartree/Å): acceleration = inv_mass * force
+    int* bonds;        // [n_bonds][2]
+    float* bond_k;     // [n_bonds] Hartree/Å^2
+    float* bond_r0;    // [n_bonds] Å
+    float* f_slow;     // [N][3]
+    float* f_fast;     // [N][3]
+    double* e;         // [3] E_slow, E_fast, E_kin
+    bool primed;       // f_slow / f_fast hold the forces at the current positions
+};
+
+// v += inv_m (ca Fa + cb Fb); optionally x += delta v
+__global__ void k_md_kick_drift(float* __restrict__ pos, float* __restrict__ vel, const float* __restrict__ inv_mass,
+                                const float* __restrict__ Fa, float ca, const float* __restrict__ Fb, float cb, float delta,
+                                int n3) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n3) return;
+    float f = 0.f;
+    if (Fa) f = ca * Fa[t];
+    if (Fb) f = fmaf(cb, Fb[t], f);
+    const float v = fmaf(inv_mass[t / 3], f, vel[t]);
+    vel[t] = v;
+    if (delta != 0.f) pos[t] = fmaf(delta, v, pos[t]);
+}
+
+// harmonic bonds: E = sum 1/2 k (r - r0)^2, F = -dE/dr (minimum image in a periodic box)
+__global__ void k_md_bonds(const float* __restrict__ pos, float Lx, float Ly, float Lz, int periodic, const int* __restrict__ bonds,
+                           const float* __restrict__ bond_k, const float* __restrict__ bond_r0, int n_bonds, float* __restrict__ F,
+                           double* __restrict__ E) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    double e = 0.0;
+    if (b < n_bonds) {
+        const int i = bonds[2 * b], j = bonds[2 * b + 1];
+        float dx = pos[3 * j] - pos[3 * i], dy = pos[3 * j + 1] - pos[3 * i + 1], dz = pos[3 * j + 2] - pos[3 * i + 2];
+        if (periodic) {
+            dx -= Lx * rintf(dx / Lx); dy -= Ly * rintf(dy / Ly); dz -= Lz * rintf(dz / Lz);
+        }
+        const float r = sqrtf(dx * dx + dy * dy + dz * dz);
+        const float dr = r - bond_r0[b], k = bond_k[b];
+        e = 0.5 * (double)k * (double)dr * (double)dr;
+        const float s = r > 0.f ? k * dr / r : 0.f;          // force on i is +s d, on j is -s d
+        atomicAdd(&F[3 * i], s * dx); atomicAdd(&F[3 * i + 1], s * dy); atomicAdd(&F[3 * i + 2], s * dz);
+        atomicAdd(&F[3 * j], -s * dx); atomicAdd(&F[3 * j + 1], -s * dy); atomicAdd(&F[3 * j + 2], -s * dz);
+    }
+    for (int o = 16; o; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
+    if ((threadIdx.x & 31) == 0 && e != 0.0) atomicAdd(E, e);
+}
+
+// E_kin = sum 1/2 v^2 / inv_mass
+__global__ void k_md_kinetic(const float* __restrict__ vel, const float* __restrict__ inv_mass, int n, double* __restrict__ E) {
+    double e = 0.0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const double vx = vel[3 * i], vy = vel[3 * i + 1], vz = vel[3 * i + 2];
+        e += 0.5 * (vx * vx + vy * vy + vz * vz) / (double)inv_mass[i];
+    }
+    for (int o = 16; o; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
+    if ((threadIdx.x & 31) == 0) atomicAdd(E, e);
+}
+
+static int fast_forces(Ctx* c, Md* m, const float* pos, const float* box) {
+    if (m->n_bonds == 0) return DHP_OK;
+    DHP_CUDA(c, cudaMemsetAsync(m->f_fast, 0, sizeof(float) * 3 * m->n_atoms, c->stream));
+    DHP_CUDA(c, cudaMemsetAsync(m->e + 1, 0, sizeof(double), c->stream));
+    DHP_LAUNCH(c, k_md_bonds, (int)((m->n_bonds + 127) / 128), 128, 0, pos, box ? box[0] : 0.f, box ? box[1] : 0.f, box ? box[2] : 0.f,
+               box ? 1 : 0, m->bonds, m->bond_k, m->bond_r0, (int)m->n_bonds, m->f_fast, m->e + 1);
+    return DHP_OK;
+}
+
+}  // namespace dhp
+
+using namespace dhp;
+
+// the hot call of api.cu
+extern "C" int dhp_ani_energy_forces(dhp_ctx* ctx, const float* pos, const float* box, const int32_t* species, int64_t n_atoms,
+                                     const int32_t* mol_offsets, int64_t n_mol, const dhp_weights* weights, int n_models,
+                                     double* E, float* F);
+struct dhp_md { Md m; };
+
+extern "C" {
+
+int dhp_md_create(dhp_ctx* h, int64_t n_atoms, const float* inv_mass, const int32_t* bonds, const float* bond_k,
+                  const float* bond_r0, int64_t n_bonds, dhp_md** out) {
+    if (!h || !out || n_atoms < 1 || !inv_mass || n_bonds < 0 || (n_bonds > 0 && (!bonds || !bond_k || !bond_r0))) return DHP_E_BADARG;
+    Ctx* c = &h->c;
+    if (n_atoms > c->max_atoms) return DHP_E_CAPACITY;
+    dhp_md* md = new (std::nothrow) dhp_md();
+    if (!md) return DHP_E_NOMEM;
+    Md* m = &md->m;
+    memset((void*)m, 0, sizeof(Md));
+    m->n_atoms = n_atoms; m->n_bonds = n_bonds;
+    const size_t N = (size_t)n_atoms, NB = (size_t)(n_bonds > 0 ? n_bonds : 1);
+    bool ok = cudaMalloc((void**)&m->inv_mass, sizeof(float) * N) == cudaSuccess && cudaMalloc((void**)&m->bonds, sizeof(int) * 2 * NB) == cudaSuccess &&
+              cudaMalloc((void**)&m->bond_k, sizeof(float) * NB) == cudaSuccess && cudaMalloc((void**)&m->bond_r0, sizeof(float) * NB) == cudaSuccess &&
+              cudaMalloc((void**)&m->f_slow, sizeof(float) * 3 * N) == cudaSuccess && cudaMalloc((void**)&m->f_fast, sizeof(float) * 3 * N) == cudaSuccess &&
+              cudaMalloc((void**)&m->e, sizeof(double) * 3) == cudaSuccess;
+    cudaStream_t st = c->stream;
+    if (ok) ok = cudaMemcpyAsync(m->inv_mass, inv_mass, sizeof(float) * N, cudaMemcpyDefault, st) == cudaSuccess;
+    if (ok && n_bonds > 0)
+        ok = cudaMemcpyAsync(m->bonds, bonds, sizeof(int) * 2 * NB, cudaMemcpyDefault, st) == cudaSuccess &&
+             cudaMemcpyAsync(m->bond_k, bond_k, sizeof(float) * NB, cudaMemcpyDefault, st) == cudaSuccess &&
+             cudaMemcpyAsync(m->bond_r0, bond_r0, sizeof(float) * NB, cudaMemcpyDefault, st) == cudaSuccess;
+    if (ok) ok = cudaMemsetAsync(m->e, 0, sizeof(double) * 3, st) == cudaSuccess && cudaMemsetAsync(m->f_fast, 0, sizeof(float) * 3 * N, st) == cudaSuccess &&
+                 cudaStreamSynchronize(st) == cudaSuccess;
+    if (!ok) {
+        cudaGetLastError();
+        for (void* p : {(void*)m->inv_mass, (void*)m->bonds, (void*)m->bond_k, (void*)m->bond_r0, (void*)m->f_slow, (void*)m->f_fast, (void*)m->e}) if (p) cudaFree(p);
+        delete md;
+        return DHP_E_NOMEM;
+    }
+    *out = md;
+    return DHP_OK;
+}
+
+int dhp_md_destroy(dhp_ctx* h, dhp_md* md) {
+    if (!h || !md) return DHP_E_BADARG;
+    cudaStreamSynchronize(h->c.stream);
+    Md* m = &md->m;
+    for (void* p : {(void*)m->inv_mass, (void*)m->bonds, (void*)m->bond_k, (void*)m->bond_r0, (void*)m->f_slow, (void*)m->f_fast, (void*)m->e}) if (p) cudaFree(p);
+    delete md;
+    return DHP_OK;
+}
+
+int dhp_md_reset(dhp_ctx* h, dhp_md* md) {
+    if (!h || !md) return DHP_E_BADARG;
+    md->m.primed = false;
+    return DHP_OK;
+}
+
+int dhp_md_run(dhp_ctx* h, dhp_md* md, float* pos, float* vel, const float* box, const int32_t* species,
+               const dhp_weights* weights, int n_models, float dt, int n_inner, int n_steps, double* E_out) {
+    if (!h || !md || !pos || !vel || !species || !weights || n_inner < 1 || n_steps < 0 || !(dt > 0.f)) return DHP_E_BADARG;
+    Ctx* c = &h->c;
+    Md* m = &md->m;
+    const int64_t n = m->n_atoms;
+    const int n3 = (int)(3 * n), nb = (n3 + 255) / 256;
+    const float* ff = m->n_bonds > 0 ? m->f_fast : nullptr;
+    if (m->n_bonds == 0) n_inner = 1;                     // nothing in the inner loop: plain velocity Verlet
+    const float d = dt / (float)n_inner;
+    int rc;
+    if (!m->primed) {
+        if ((rc = dhp_ani_energy_forces(h, pos, box, species, n, nullptr, 0, weights, n_models, m->e, m->f_slow)) != DHP_OK) return rc;
+        if ((rc = fast_forces(c, m, pos, box)) != DHP_OK) return rc;
+        m->primed = true;
+    }
+    for (int s = 0; s < n_steps; ++s) {
+        for (int k = 0; k < n_inner; ++k) {
+            // k = 0: the outer half kick rides along; k > 0: the closing half kick of inner step k-1 and the opening
+            // one of step k use the same fast force, so they are one kick of d
+            DHP_LAUNCH(c, k_md_kick_drift, nb, 256, 0, pos, vel, m->inv_mass, k == 0 ? m->f_slow : (const float*)nullptr, 0.5f * dt, ff,
+                       k == 0 ? 0.5f * d : d, d, n3);
+            if ((rc = fast_forces(c, m, pos, box)) != DHP_OK) return rc;
+        }
+        if ((rc = dhp_ani_energy_forces(h, pos, box, species, n, nullptr, 0, weights, n_models, m->e, m->f_slow)) != DHP_OK) return rc;
+        DHP_LAUNCH(c, k_md_kick_drift, nb, 256, 0, pos, vel, m->inv_mass, m->f_slow, 0.5f * dt, ff, 0.5f * d, 0.f, n3);
+    }
+    if (E_out) {
+        DHP_CUDA(c, cudaMemsetAsync(m->e + 2, 0, sizeof(double), c->stream));
+        DHP_LAUNCH(c, k_md_kinetic, 2 * c->sm_count, 256, 0, vel, m->inv_mass, (int)n, m->e + 2);
+        DHP_CUDA(c, cudaMemcpyAsync(E_out, m->e, sizeof(double) * 3, cudaMemcpyDeviceToDevice, c->stream));
+    }
+    DHP_CUDA(c, cudaGetLastError());
+    return DHP_OK;
+}
+
+}  // extern "C"

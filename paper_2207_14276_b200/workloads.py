@@ -329,3 +329,51 @@ def jitter(system: System, sigma: float, seed: int) -> np.ndarray:
     """Positions displaced by N(0, sigma^2) per coordinate (timing protocol)."""
     rng = np.random.default_rng(seed)
     return (system.pos.astype(np.float64) + rng.normal(0.0, sigma, system.pos.shape)).astype(np.float32)
+
+
+# --------------------------------------------------------------------------------------
+# inputs of the multiple-timestep driver (SURVEY.md §8(f1)): masses, water O-H bonds, thermal velocities
+# --------------------------------------------------------------------------------------
+AMU_MASS = np.array([1.008, 12.011, 14.007, 15.999, 32.06, 18.998, 35.45])   # H C N O S F Cl
+ACCEL_PER_FORCE = 0.2625499639     # (Å/fs^2) per (Hartree/Å/amu): 4.3597447222e-18 J / 1e-10 m / 1.6605390666e-27 kg
+KB_HARTREE = 3.166811563e-6        # Boltzmann constant, Hartree/K
+
+
+@dataclasses.dataclass
+class MdInputs:
+    inv_mass: np.ndarray   # f32 [N]  (Å/fs^2)/(Hartree/Å)
+    bonds: np.ndarray      # i32 [n_bonds, 2]
+    bond_k: np.ndarray     # f32 [n_bonds] Hartree/Å^2 (E = 1/2 k (r - r0)^2)
+    bond_r0: np.ndarray    # f32 [n_bonds] Å
+    vel: np.ndarray        # f32 [N, 3] Å/fs
+
+
+def md_inputs(system: System, temperature: float = 300.0, seed: int = 4001, n_protein: Optional[int] = None) -> MdInputs:
+    """Masses of the 7 elements; harmonic O-H bonds (k = 1.434 Hartree/Å^2, i.e. 450 kcal/mol/Å^2 in the k (r - r0)^2
+    convention; r0 = 0.9572 Å) for every water of the system - the generators above lay waters out as consecutive
+    (O, H, H) triples after `n_protein` leading atoms (0 for water96; derived from the recipe for the protein boxes
+    when not given); Maxwell-Boltzmann velocities at `temperature` with the centre-of-mass motion removed."""
+    n = system.n_atoms
+    if n_protein is None:
+        n_protein = 0
+        if system.name in ("proteinbox23k", "biosystem98k"):
+            L = float(system.box[0])
+            radius = 30.0 if system.name == "proteinbox23k" else 45.0
+            n_protein = int(round(n / L ** 3 * 4.0 / 3.0 * math.pi * radius ** 3))
+            while (n - n_protein) % 3 != 0:
+                n_protein += 1
+        elif system.name != "water96":
+            n_protein = n                      # no waters known: no bonds
+    sp = system.species
+    bonds = []
+    for base in range(n_protein, n - 2, 3):
+        if sp[base] == O and sp[base + 1] == H and sp[base + 2] == H:
+            bonds += [(base, base + 1), (base, base + 2)]
+    bonds = np.array(bonds, dtype=np.int32).reshape(-1, 2)
+    mass = AMU_MASS[sp]
+    rng = np.random.default_rng(seed)
+    sigma = np.sqrt(KB_HARTREE * temperature * ACCEL_PER_FORCE / mass)          # Å/fs per component
+    vel = rng.normal(0.0, 1.0, (n, 3)) * sigma[:, None]
+    vel -= (vel * mass[:, None]).sum(0) / mass.sum()
+    return MdInputs((ACCEL_PER_FORCE / mass).astype(np.float32), bonds, np.full(len(bonds), 1.434, np.float32),
+                    np.full(len(bonds), 0.9572, np.float32), vel.astype(np.float32))

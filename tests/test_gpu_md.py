@@ -1,0 +1,103 @@
+"""The multiple-timestep driver (include/dhp.h: dhp_md_run; §2.3.5, Eqs. 8-9) against the fp64 oracle
+integrator oracle/md_oracle.py driven by the fp64 ANI oracle: same inputs, same number of steps, trajectories compared
+atom by atom.  Tolerances: the GPU integrates in fp32 (positions ~ 15 Å: 1 ulp = 1e-6 Å, a handful of roundings per
+step), forces carry <= 5e-5 Hartree/Å (measured ~ 2e-6) x inv_mass 0.26 x dt: |dx| <= 2e-5 Å, |dv| <= 5e-6 Å/fs after
+ten inner steps."""
+import numpy as np
+import pytest
+
+import oracle
+from oracle import md_oracle as M
+from paper_2207_14276_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+X_TOL, V_TOL = 2e-5, 5e-6
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2207_14276_b200 import binding
+    return binding
+
+
+def oracle_run(s, md, params, blob, dt, n_inner, n_steps, bonds=True):
+    slow = lambda x: (lambda E, F: (float(E.sum()), F.astype(np.float64)))(
+        *oracle.energy_forces(x.astype(np.float32), s.species, s.box, params, blob, s.n_models)[:2])
+    fast = (lambda x: M.bond_energy_forces(x, s.box, md.bonds, md.bond_k.astype(np.float64), md.bond_r0.astype(np.float64))) \
+        if bonds and len(md.bonds) else None
+    return M.respa_run(s.pos, md.vel, md.inv_mass, slow, fast, dt, n_inner, n_steps)
+
+
+def gpu_run(B, torch, s, md, params, blob, dt, n_inner, chunks, skin=0.0, mode=None, bonds=True):
+    d = B.Dhp(s.n_atoms, params=params)
+    if mode is not None:
+        d.dhp_set_mlp_mode(mode)
+    if skin:
+        d.dhp_set_skin(skin)
+    w = d.dhp_weights_load(blob, s.n_models)
+    pos = torch.from_numpy(s.pos.copy()).cuda()
+    vel = torch.from_numpy(md.vel.copy()).cuda()
+    sp = torch.from_numpy(s.species).cuda()
+    h = d.dhp_md_create(md.inv_mass, md.bonds, md.bond_k, md.bond_r0) if bonds and len(md.bonds) else d.dhp_md_create(md.inv_mass)
+    for n in chunks:
+        E = d.dhp_md_run(h, pos, vel, s.box, sp, w, dt, n_inner, n)
+    torch.cuda.synchronize()
+    assert d.dhp_status() == 0
+    out = pos.cpu().numpy(), vel.cpu().numpy(), E.cpu().numpy(), d.dhp_nlist_rebuild_count()
+    d.dhp_md_destroy(h)
+    d.close()
+    return out
+
+
+@pytest.mark.parametrize("mode", [1, 2])
+def test_respa_trajectory_water96(torch, B, params, mode):
+    s = W.make_system(1)
+    blob = W.make_weights(1)
+    md = W.md_inputs(s)
+    xo, vo, Eo = oracle_run(s, md, params, blob, 0.2, 2, 5)
+    x, v, E, _ = gpu_run(B, torch, s, md, params, blob, 0.2, 2, [5], mode=mode)
+    assert np.abs(x - xo).max() <= X_TOL and np.abs(v - vo).max() <= V_TOL
+    assert abs(E[0] - Eo[0]) / s.n_atoms <= 1e-6                       # E_ANI at the final positions
+    assert abs(E[1] - Eo[1]) <= 1e-5 + 1e-4 * abs(Eo[1])               # bond energy (fp32 distances)
+    assert abs(E[2] - Eo[2]) <= 1e-4 * Eo[2]                           # kinetic energy
+    # the forces at the current positions are carried between runs: 3 + 2 steps == 5 steps
+    x2, v2, E2, _ = gpu_run(B, torch, s, md, params, blob, 0.2, 2, [3, 2], mode=mode)
+    assert np.abs(x2 - xo).max() <= X_TOL and np.abs(v2 - vo).max() <= V_TOL
+    # with list reuse: same trajectory, one full build for the 6 evaluations
+    x3, v3, E3, nb = gpu_run(B, torch, s, md, params, blob, 0.2, 2, [5], skin=1.0, mode=mode)
+    assert nb == 1
+    assert np.abs(x3 - xo).max() <= X_TOL and np.abs(v3 - vo).max() <= V_TOL and abs(E3[0] - Eo[0]) / s.n_atoms <= 1e-6
+
+
+def test_velocity_verlet_without_bonds_mixed_box(torch, B, params):
+    """No fast part: plain velocity Verlet (the paper's benchmark integrator) on a 7-species periodic box."""
+    s = W.small_periodic_mix(600, 18.3, seed=77, n_models=2)
+    blob = W.make_weights(2)
+    md = W.md_inputs(s)
+    assert len(md.bonds) == 0
+    xo, vo, Eo = oracle_run(s, md, params, blob, 0.1, 1, 4)
+    x, v, E, nb = gpu_run(B, torch, s, md, params, blob, 0.1, 3, [4], skin=0.6)      # n_inner is ignored without bonds
+    assert nb == 1
+    assert np.abs(x - xo).max() <= X_TOL and np.abs(v - vo).max() <= V_TOL
+    assert abs(E[0] - Eo[0]) / s.n_atoms <= 1e-6 and E[1] == 0.0 and abs(E[2] - Eo[2]) <= 1e-4 * Eo[2]
+
+
+def test_long_run_rebuilds_when_atoms_leave_the_skin(torch, B, params):
+    """40 outer steps with a thin skin: the device-side displacement check must trigger rebuilds on its own, and the
+    final state must still match a run without any reuse."""
+    s = W.make_system(1)
+    blob = W.make_weights(1)
+    md = W.md_inputs(s, temperature=600.0)
+    x0, v0, E0, _ = gpu_run(B, torch, s, md, params, blob, 0.25, 1, [40], bonds=False)
+    x1, v1, E1, nb = gpu_run(B, torch, s, md, params, blob, 0.25, 1, [40], skin=0.1, bonds=False)
+    assert 2 <= nb <= 41
+    assert np.abs(x1 - x0).max() <= 1e-4 and abs(E1[0] - E0[0]) / s.n_atoms <= 1e-6
+    print(f"rebuilds with skin 0.1 over 40 steps: {nb}; max |x - x0| = {np.abs(x1 - s.pos).max():.3f} A")
