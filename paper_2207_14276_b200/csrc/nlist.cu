@@ -564,9 +564,13 @@ constexpr int MAX_STRIDE_CHUNKS = 6;    // tmp_stride <= 192
 __global__ void __launch_bounds__(P2_THREADS)
 k_rows(const unsigned* __restrict__ tmp, int stride, const int* __restrict__ cnt, const int* __restrict__ blk_off, int nblk,
        int n, int* __restrict__ row_ptr, int* __restrict__ col, int* __restrict__ n_rad, int* __restrict__ n_ang,
-       unsigned short* __restrict__ seg_cnt, unsigned* __restrict__ amask) {
+       unsigned short* __restrict__ seg_cnt, unsigned* __restrict__ amask, const int* __restrict__ gate,
+       const int* __restrict__ rowmap, unsigned* __restrict__ tile_mask) {
     __shared__ int wsum[ROWS_PER_BLK / 32];
     __shared__ int rstart[ROWS_PER_BLK];
+    __shared__ int rcnt[ROWS_PER_BLK];
+    // list reuse: the row assignment of the last full build stays, the tile masks follow the current feature-block masks
+    const bool reuse_rows = gate != nullptr && *gate == 0;
     __shared__ int segs[P2_THREADS / 32][16];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int i0 = blockIdx.x * ROWS_PER_BLK;
@@ -593,6 +597,7 @@ k_rows(const unsigned* __restrict__ tmp, int stride, const int* __restrict__ cnt
         if (a < n) { row_ptr[a] = start; n_rad[a] = c; }
         if (a == n - 1) row_ptr[n] = start + c;
         rstart[tid] = start;
+        rcnt[tid] = c;
     }
     __syncthreads();
 
@@ -601,7 +606,7 @@ k_rows(const unsigned* __restrict__ tmp, int stride, const int* __restrict__ cnt
     for (int q = warp; q < ROWS_PER_BLK; q += P2_THREADS / 32) {
         const int i = i0 + q;
         if (i >= n) break;
-        const int ni = ovf ? 0 : n_rad[i];
+        const int ni = rcnt[q];
         const unsigned* src = tmp + (size_t)i * stride;
         unsigned e[MAX_STRIDE_CHUNKS];
 #pragma unroll
@@ -634,7 +639,13 @@ k_rows(const unsigned* __restrict__ tmp, int stride, const int* __restrict__ cnt
             const unsigned pm = __ballot_sync(0xffffffffu, pp);
             const bool bb = lane < 14 ? ((pm >> (2 * lane)) & 3u) != 0 : lane == 14 ? (rm & 0x0fu) != 0 : lane == 15 ? (rm & 0x70u) != 0 : false;
             const unsigned bmask = __ballot_sync(0xffffffffu, bb);
-            if (lane == 0) amask[i] = bmask;
+            if (lane == 0) {
+                amask[i] = bmask;
+                if (reuse_rows && bmask) {
+                    const int row = rowmap[i];
+                    if (row >= 0) atomicOr(&tile_mask[row / ROW_TILE], bmask);
+                }
+            }
         }
         int x = cnt_k;
 #pragma unroll
@@ -711,69 +722,88 @@ __global__ void k_regather(const float* __restrict__ pos, const int* __restrict_
     spos[a] = make_float4(pos[3 * v], pos[3 * v + 1], pos[3 * v + 2], spos[a].w);
 }
 
-// reuse: one warp per central atom filters its candidates.  fp32 R^2 of the fp64 minimum-image displacement
-// (relative error < 2^-21) decides; within 2^-19 rc^2 of a cutoff the canonical fp64 predicate does.
-constexpr int RF_WARPS = 8;
+// reuse: one warp per central atom filters its candidates in fp32.  The inputs are fp32, so pj - pi in fp32 is the
+// correctly rounded exact difference (relative error 2^-24); the minimum-image shift by the fp32 box edge (exact: the
+// box IS fp32) adds at most 2 * 2^-24 dm, dm = the largest raw coordinate difference of the pair, so a component is
+// off by <= 3 * 2^-24 dm.  Pairs whose fp32 R^2 lies within the resulting margin of a cutoff are decided by the
+// canonical fp64 predicate, all others by fp32 alone: the list stays bit-exact.
+constexpr int RF_WARPS = 4;
+constexpr int RF_UNROLL = 4;
+struct BoxArg { double L[3]; float Lf[3], iLf[3]; int periodic; };
+__device__ __forceinline__ double pair_r2_box(const float4& pi, const float4& pj, const BoxArg& bx) {
+    double d[3] = {(double)pj.x - (double)pi.x, (double)pj.y - (double)pi.y, (double)pj.z - (double)pi.z};
+    if (bx.periodic) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) d[c] = __dsub_rn(d[c], __dmul_rn(bx.L[c], rint(__ddiv_rn(d[c], bx.L[c]))));
+    }
+    return __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
+}
+
 __global__ void __launch_bounds__(RF_WARPS * 32)
-k_refilter(const float4* __restrict__ spos, const Grid* __restrict__ gp, const unsigned* __restrict__ cand, const int* __restrict__ cand_cnt,
-           int cstride, double rcr2, double rca2, int stride, int n, int* __restrict__ cnt, unsigned* __restrict__ tmp,
-           int* __restrict__ blk_sum, int* __restrict__ status, const unsigned char* __restrict__ snc, const int* __restrict__ gate) {
-    DHP_GATE(gate, 0);
-    __shared__ Grid g;
-    if (threadIdx.x == 0) g = *gp;
-    __syncthreads();
+k_refilter(const float4* __restrict__ spos, const __grid_constant__ BoxArg bx, const unsigned* __restrict__ cand,
+           const int* __restrict__ cand_cnt, int cstride, double rcr2, double rca2, int stride, int n, int* __restrict__ cnt,
+           unsigned* __restrict__ tmp, int* __restrict__ blk_sum, int* __restrict__ status, const unsigned char* __restrict__ snc,
+           const int* __restrict__ gate) {
     const int lane = threadIdx.x & 31;
     const int i = blockIdx.x * RF_WARPS + (threadIdx.x >> 5);
     if (i >= n) return;
-    if (snc && snc[i]) { if (lane == 0) cnt[i] = 0; return; }
-    const float rcr2f = (float)rcr2, rca2f = (float)rca2;
-    const float mr = rcr2f * 1.9073486e-06f, ma = rca2f * 1.9073486e-06f;
-    const unsigned lt = (1u << lane) - 1u;
-    const float4 pi = spos[i];
-    const int nc = cand_cnt[i];
+    // everything the warp needs first is requested at once (the candidate row's address does not depend on its
+    // length), so a warp pays two dependent memory latencies - this batch, then the gathers - not five
     const unsigned* row = cand + (size_t)i * cstride;
-    int base = 0;
-    for (int c0 = 0; c0 < nc; c0 += 32) {
-        const bool have = c0 + lane < nc;
-        const unsigned e = have ? row[c0 + lane] : 0u;
-        const float4 pj = spos[e & 0x0fffffffu];
-        double d[3] = {(double)pj.x - (double)pi.x, (double)pj.y - (double)pi.y, (double)pj.z - (double)pi.z};
-        if (g.periodic) {
+    unsigned e[RF_UNROLL];
 #pragma unroll
-            for (int c = 0; c < 3; ++c) d[c] -= g.L[c] * rint(d[c] * g.inv_L[c]);
+    for (int u = 0; u < RF_UNROLL; ++u) e[u] = (32 * u + lane < cstride) ? row[32 * u + lane] : 0u;
+    const int gv = *gate;
+    const int nc = cand_cnt[i];
+    const float4 pi = spos[i];
+    const bool skip = snc != nullptr && snc[i] != 0;
+    if (gv != 0) return;                                      // this call rebuilds: nothing to do here
+    if (skip) { if (lane == 0) cnt[i] = 0; return; }
+    const bool per = bx.periodic != 0;
+    const float Lx = bx.Lf[0], Ly = bx.Lf[1], Lz = bx.Lf[2], iLx = bx.iLf[0], iLy = bx.iLf[1], iLz = bx.iLf[2];
+    const float rcr2f = (float)rcr2, rca2f = (float)rca2;
+    const float rcr = sqrtf(rcr2f), rca = sqrtf(rca2f);
+    // margin of a pair: |err(R^2)| <= 2 sqrt(3) R (3 * 2^-24 dm) + 3 * 2^-24 R^2 with dm its largest raw coordinate difference; doubled
+    const float kr = 2.0f * 2.0f * rcr * 3.0f * 5.9604645e-08f, ka = 2.0f * 2.0f * rca * 3.0f * 5.9604645e-08f;
+    const float mr0 = 2.0f * rcr2f * 2.3841858e-07f, ma0 = 2.0f * rca2f * 2.3841858e-07f;
+    const unsigned lt = (1u << lane) - 1u;
+    int base = 0;
+    for (int c0 = 0; c0 < nc; c0 += 32 * RF_UNROLL) {
+        float4 pj[RF_UNROLL];
+        if (c0 > 0) {
+#pragma unroll
+            for (int u = 0; u < RF_UNROLL; ++u) e[u] = (c0 + 32 * u + lane < nc) ? row[c0 + 32 * u + lane] : 0u;
         }
-        const float x = (float)d[0], y = (float)d[1], z = (float)d[2];
-        const float r2 = x * x + y * y + z * z;
-        bool in_r = have && r2 <= rcr2f;
-        bool in_a = have && r2 <= rca2f;
-        if (have && (fabsf(r2 - rcr2f) <= mr || fabsf(r2 - rca2f) <= ma)) {
-            const double r2d = pair_r2(pi, pj, g);
-            in_r = r2d <= rcr2;
-            in_a = r2d <= rca2;
+#pragma unroll
+        for (int u = 0; u < RF_UNROLL; ++u) pj[u] = spos[(c0 + 32 * u + lane < nc) ? (e[u] & 0x0fffffffu) : i];
+#pragma unroll
+        for (int u = 0; u < RF_UNROLL; ++u) {
+            if (c0 + 32 * u >= nc) break;                                  // warp-uniform
+            const bool have = c0 + 32 * u + lane < nc;
+            float dx = pj[u].x - pi.x, dy = pj[u].y - pi.y, dz = pj[u].z - pi.z;
+            const float dm = fmaxf(fabsf(dx), fmaxf(fabsf(dy), fabsf(dz)));
+            if (per) { dx -= Lx * rintf(dx * iLx); dy -= Ly * rintf(dy * iLy); dz -= Lz * rintf(dz * iLz); }
+            const float r2 = dx * dx + dy * dy + dz * dz;
+            bool in_r = have && r2 <= rcr2f;
+            bool in_a = have && r2 <= rca2f;
+            if (have && (fabsf(r2 - rcr2f) <= fmaf(kr, dm, mr0) || fabsf(r2 - rca2f) <= fmaf(ka, dm, ma0))) {
+                const double r2d = pair_r2_box(pi, pj[u], bx);
+                in_r = r2d <= rcr2;
+                in_a = r2d <= rca2;
+            }
+            const unsigned m = __ballot_sync(0xffffffffu, in_r);
+            if (in_r) {
+                const int pos = base + __popc(m & lt);
+                if (pos < stride) tmp[(size_t)i * stride + pos] = e[u] | (in_a ? 0u : ENT_RADIAL_ONLY);
+            }
+            base += __popc(m);
         }
-        const unsigned m = __ballot_sync(0xffffffffu, in_r);
-        if (in_r) {
-            const int pos = base + __popc(m & lt);
-            if (pos < stride) tmp[(size_t)i * stride + pos] = e | (in_a ? 0u : ENT_RADIAL_ONLY);
-        }
-        base += __popc(m);
     }
     if (lane == 0) {
         if (base > stride) { atomicExch(status, DHP_E_CAPACITY); base = stride; }
         cnt[i] = base;
         atomicAdd(&blk_sum[i / ROWS_PER_BLK], base);
     }
-}
-
-// reuse: the row assignment of the last full build stays; the tile masks follow the current feature-block masks
-__global__ void k_tilemask(const unsigned* __restrict__ amask, const int* __restrict__ rowmap, int n, unsigned* __restrict__ tile_mask,
-                           const int* __restrict__ gate) {
-    DHP_GATE(gate, 0);
-    const int a = blockIdx.x * blockDim.x + threadIdx.x;
-    if (a >= n) return;
-    const int row = rowmap[a];
-    const unsigned m = amask[a];
-    if (row >= 0 && m) atomicOr(&tile_mask[row / ROW_TILE], m);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -875,19 +905,21 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
 #undef DHP_PAIRS
     if (skin) {
         DHP_LAUNCH(ctx, k_regather, nb, 256, 0, pos, ctx->perm, n, ctx->spos, gate);
-        DHP_LAUNCH(ctx, k_refilter, (n + RF_WARPS - 1) / RF_WARPS, RF_WARPS * 32, 0, ctx->spos, ctx->grid, ctx->cand, ctx->cand_cnt,
+        BoxArg bxa;
+        for (int c = 0; c < 3; ++c) { bxa.L[c] = L[c]; bxa.Lf[c] = (float)L[c]; bxa.iLf[c] = periodic ? (float)(1.0 / L[c]) : 0.f; }
+        bxa.periodic = periodic ? 1 : 0;
+        DHP_LAUNCH(ctx, k_refilter, (n + RF_WARPS - 1) / RF_WARPS, RF_WARPS * 32, 0, ctx->spos, bxa, ctx->cand, ctx->cand_cnt,
                    ctx->cand_stride, rcr2, rca2, ctx->tmp_stride, n, ctx->n_rad, ctx->tmp_col, ctx->blk_sum, ctx->status, snc, gate);
     }
     DHP_LAUNCH(ctx, k_scan_blocks, 1, 1024, 0, ctx->blk_sum, ctx->blk_off, nblk, ctx->pair_cap, ctx->status);
     DHP_LAUNCH(ctx, k_rows, nblk, P2_THREADS, 0, ctx->tmp_col, ctx->tmp_stride, ctx->n_rad, ctx->blk_off, nblk, n, ctx->row_ptr,
-               ctx->col, ctx->n_rad, ctx->n_ang, ctx->seg_cnt, ctx->amask);
+               ctx->col, ctx->n_rad, ctx->n_ang, ctx->seg_cnt, ctx->amask, gate, ctx->rowmap, ctx->tile_mask);
     // rows grouped by species, ordered by feature-block class inside a group; tile masks
     const int nrb = (n + RB - 1) / RB;
     DHP_LAUNCH(ctx, k_rowkey_hist, nrb, RB, 0, ctx->spos, ctx->amask, snc, n, nrb, ctx->blk_hist, gate);
     DHP_LAUNCH(ctx, k_rowkey_scan, 1, 1024, 0, ctx->blk_hist, nrb, ctx->sp_count, ctx->sp_start, ctx->key_start, gate);
     DHP_LAUNCH(ctx, k_rowkey_rank, nrb, RB, 0, ctx->spos, ctx->amask, snc, n, nrb, ctx->blk_hist, ctx->key_start, ctx->rowmap,
                ctx->row_species, ctx->row_slot, ctx->tile_mask, gate);
-    if (skin) DHP_LAUNCH(ctx, k_tilemask, nb, 256, 0, ctx->amask, ctx->rowmap, n, ctx->tile_mask, gate);
     DHP_CUDA(ctx, cudaGetLastError());
     return DHP_OK;
 }
