@@ -69,13 +69,17 @@ typedef struct dhp_ctx dhp_ctx;         /* workspace sized for max_atoms, bound 
 typedef struct dhp_nlist dhp_nlist;     /* device-resident CSR pair list, owned by the context     */
 typedef struct dhp_weights dhp_weights; /* device-resident network parameters, owned by the context */
 
-/* MLP arithmetic, dhp_set_mlp_mode(): both meet the parity tolerances against the fp64 oracle. */
+/* MLP arithmetic, dhp_set_mlp_mode().  AUTO, SIMT, TENSOR and TENSOR_LAYERWISE meet the parity tolerances against the
+ * fp64 oracle; TENSOR_FP16 is the opt-in mixed-precision trade of PAPER.md L161 and does not. */
 enum {
     DHP_MLP_AUTO = 0,   /* tensor path when available, else SIMT                                   */
     DHP_MLP_SIMT = 1,   /* fp32 FFMA GEMMs                                                          */
     DHP_MLP_TENSOR = 2, /* tcgen05 / TMEM GEMMs, fp16 two-term split operands, fp32 accumulate; the four
                            middle GEMMs of the chain fused into one kernel (activations stay on chip)   */
-    DHP_MLP_TENSOR_LAYERWISE = 3 /* same arithmetic, one launch per GEMM (bring-up / comparison path)   */
+    DHP_MLP_TENSOR_LAYERWISE = 3, /* same arithmetic, one launch per GEMM (bring-up / comparison path)  */
+    DHP_MLP_TENSOR_FP16 = 4 /* the fused tensor path with ONE fp16 MMA per product (operands rounded to fp16, fp32
+                               accumulate): the "mixed precision" option of PAPER.md L161.  About 2x faster MLP; force
+                               errors ~1e-3 Hartree/Å, i.e. outside the 5e-5 bar - never selected by AUTO             */
 };
 
 /* Phases timed by dhp_profile_* (CUDA events on the context stream). */

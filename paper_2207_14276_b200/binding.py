@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(HERE, "libdhp.so")
 
 N_PHASES = 6
 PHASES = ("nlist", "aev_fwd", "mlp_g1", "mlp_mid", "mlp_b1", "aev_bwd")
-MLP_AUTO, MLP_SIMT, MLP_TENSOR, MLP_TENSOR_LAYERWISE = 0, 1, 2, 3
+MLP_AUTO, MLP_SIMT, MLP_TENSOR, MLP_TENSOR_LAYERWISE, MLP_TENSOR_FP16 = 0, 1, 2, 3, 4
 OK = 0
 
 # every symbol include/dhp.h declares: (name, restype, argtypes)

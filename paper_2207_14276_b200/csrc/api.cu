@@ -94,7 +94,7 @@ static int run_energy_forces(Ctx* ctx, const float* pos, const float* box, const
     prof_mark(ctx, DHP_PHASE_NLIST);
     if ((rc = nlist_build(ctx, pos, box, species, n, mol_offsets, n_mol, central)) != DHP_OK) return rc;
     prof_mark(ctx, DHP_PHASE_AEV_FWD);
-    const bool tensor = ctx->mlp_mode == DHP_MLP_TENSOR || ctx->mlp_mode == DHP_MLP_TENSOR_LAYERWISE ||
+    const bool tensor = ctx->mlp_mode == DHP_MLP_TENSOR || ctx->mlp_mode == DHP_MLP_TENSOR_LAYERWISE || ctx->mlp_mode == DHP_MLP_TENSOR_FP16 ||
                         (ctx->mlp_mode == DHP_MLP_AUTO && w->tc != nullptr);
     if (tensor && !w->tc) return DHP_E_NOTIMPL;
     if ((rc = aev_forward(ctx, tensor && ctx->aev_planes != nullptr)) != DHP_OK) return rc;
@@ -373,7 +373,7 @@ int dhp_status(dhp_ctx* h) {
 }
 
 int dhp_set_mlp_mode(dhp_ctx* h, int mode) {
-    if (!h || mode < DHP_MLP_AUTO || mode > DHP_MLP_TENSOR_LAYERWISE) return DHP_E_BADARG;
+    if (!h || mode < DHP_MLP_AUTO || mode > DHP_MLP_TENSOR_FP16) return DHP_E_BADARG;
     if (mode >= DHP_MLP_TENSOR && !mlp_tc_available(&h->c)) return DHP_E_NOTIMPL;
     h->c.mlp_mode = mode;
     return DHP_OK;

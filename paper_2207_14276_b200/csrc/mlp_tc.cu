@@ -61,6 +61,7 @@ constexpr float D_SCALE = 1024.0f;     // 2^10 on the back-propagated deltas
 enum { EPI_CELU = 0, EPI_OUT = 1, EPI_DCELU = 2, EPI_GRAD = 3 };
 
 struct TcArgs {
+    int single;               // 1: single-pass fp16 (hi x hi only; opt-in mixed precision, DHP_MLP_TENSOR_FP16)
     int K;                    // reduction length in elements (multiple of 16)
     int BN;                   // tile width (multiple of 16, <= 256)
     int n_tiles;              // column tiles per row block
@@ -425,8 +426,10 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                     for (int k = 0; k < ksteps; ++k) {
                         const uint64_t adv = (uint64_t)(k * 2), a_adv = (uint64_t)k * a_step;
                         umma_f16(d_tmem, a_hi + a_adv, b_hi + adv, idesc, accumulate);
-                        umma_f16(d_tmem, a_hi + a_adv, b_lo + adv, idesc, 1u);
-                        umma_f16(d_tmem, a_lo + a_adv, b_hi + adv, idesc, 1u);
+                        if (!p.single) {
+                            umma_f16(d_tmem, a_hi + a_adv, b_lo + adv, idesc, 1u);
+                            umma_f16(d_tmem, a_lo + a_adv, b_hi + adv, idesc, 1u);
+                        }
                         accumulate = 1u;
                     }
                     umma_commit(empty_bar(stage));                     // frees the smem stage when the MMAs retire
@@ -592,6 +595,7 @@ __device__ __forceinline__ void load16(const float* __restrict__ src, float (&x)
 }
 
 struct MidArgs {
+    int single;               // 1: single-pass fp16 (hi x hi only)
     const int* row_species;
     const int* sp_start;
     int n_models;
@@ -770,15 +774,19 @@ k_mlp_mid(const MidArgs p) {
                         if (a_src == A_TMEM) {
                             const uint32_t a_hi = tmem_base + MID_D + (uint32_t)j * 8u, a_lo = tmem_base + MID_D_LO + (uint32_t)j * 8u;
                             umma_f16_ts(d_tmem, a_hi, b_hi, idesc, accumulate);
-                            umma_f16_ts(d_tmem, a_hi, b_lo, idesc, 1u);
-                            umma_f16_ts(d_tmem, a_lo, b_hi, idesc, 1u);
+                            if (!p.single) {
+                                umma_f16_ts(d_tmem, a_hi, b_lo, idesc, 1u);
+                                umma_f16_ts(d_tmem, a_lo, b_hi, idesc, 1u);
+                            }
                         } else {
                             const uint32_t a0 = a_src == A_SLOT ? sa + MID_A_OFF : xs + (uint32_t)j * 4096u;
                             const uint64_t a_hi = make_desc_ns(a0, 2048u);
                             const uint64_t a_lo = make_desc_ns(a0 + (a_src == A_SLOT ? 4096u : (uint32_t)MID_X_PLANE), 2048u);
                             umma_f16(d_tmem, a_hi, b_hi, idesc, accumulate);
-                            umma_f16(d_tmem, a_hi, b_lo, idesc, 1u);
-                            umma_f16(d_tmem, a_lo, b_hi, idesc, 1u);
+                            if (!p.single) {
+                                umma_f16(d_tmem, a_hi, b_lo, idesc, 1u);
+                                umma_f16(d_tmem, a_lo, b_hi, idesc, 1u);
+                            }
                         }
                     }
                     accumulate = 1u;
@@ -1176,6 +1184,7 @@ int mlp_tc(Ctx* ctx, const Weights* wt, bool forward_only) {
         DHP_LAUNCH(ctx, k_split_rows, 4 * ctx->sm_count, 256, 0, ctx->aev, AEV_LD, ctx->sp_start, AEV_LD, ws->aev, R);
 
     TcArgs a{};
+    a.single = ctx->mlp_mode == DHP_MLP_TENSOR_FP16 ? 1 : 0;
     a.row_species = ctx->row_species; a.sp_start = ctx->sp_start; a.alpha = ctx->params.celu_alpha;
     a.inv_models = 1.0f / (float)M; a.a_plane_rows = R; a.plane_tiles = R / BM; a.e_atom = ctx->e_atom;
     a.w4 = t->w4; a.b4 = t->b4; a.tile_mask = ctx->tile_mask;
@@ -1195,6 +1204,7 @@ int mlp_tc(Ctx* ctx, const Weights* wt, bool forward_only) {
             attr = true;
         }
         MidArgs m{};
+        m.single = a.single;
         m.row_species = ctx->row_species; m.sp_start = ctx->sp_start; m.n_models = M; m.plane_tiles = R / BM;
         m.h1 = ws->h1; m.d1 = ws->d1; m.wimg = t->wmid; m.b2 = t->b2; m.b3 = t->b3; m.w4 = t->w4; m.b4 = t->b4;
         m.inv_models = 1.0f / (float)M; m.alpha = ctx->params.celu_alpha; m.e_atom = ctx->e_atom; m.sched = ctx->tc_sched + 1;

@@ -232,6 +232,27 @@ def test_energy_only_call(torch, B, params, blob8, name, mode):
     d.close()
 
 
+@pytest.mark.parametrize("name", ["water96", "mix600"])
+def test_mixed_precision_mode_error_is_bounded_and_documented(torch, B, params, blob8, name):
+    """DHP_MLP_TENSOR_FP16 (one fp16 MMA per product; the paper's mixed-precision option) is an opt-in
+    trade: measured on B200 |dE|/N = 4e-6 .. 1e-5 Hartree and max |dF| = 3e-4 .. 4e-4 Hartree/Å, i.e.
+    5-10x outside the parity bars that every other mode meets.  The test pins that order of magnitude from both sides:
+    the mode must stay usable (errors well below the force scale of 0.1 Hartree/Å) and must never be mistaken for a
+    mode that meets the bar."""
+    s = SYSTEMS[name]()
+    probe = make_ctx(B, s, params)
+    ok = probe.dhp_tensor_path_available()
+    probe.close()
+    if not ok:
+        pytest.skip("tensor path not available in this build")
+    d, E, F = run_gpu(B, torch, s, params, blob8, B.MLP_TENSOR_FP16)
+    Eo, Fo = oracle.total_energy_forces(s, params, blob8[: s.n_models * 7 * W.PARAMS_PER_NET])
+    dE, dF = abs(E[0] - Eo[0]) / s.n_atoms, np.max(np.abs(F - Fo))
+    assert dE <= 5e-5 and dF <= 2e-3
+    assert dF > F_TOL                     # if this ever passes the bar, make it the default and delete this test
+    d.close()
+
+
 def test_host_entry_point_matches_device_entry_point(torch, B, params, blob8):
     s = SYSTEMS["mix600"]()
     d, E, F = run_gpu(B, torch, s, params, blob8)
