@@ -182,10 +182,11 @@ int dhp_create(dhp_ctx** out, const dhp_params* params, int64_t max_atoms, int64
     cudaDeviceProp prop;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) { delete h; return DHP_E_CUDA; }
     c->sm_count = prop.multiProcessorCount;
+    { const char* e = getenv("DHP_TC_PAIRS"); c->tc_pairs = e && e[0] == '1'; }   // experimental cta_group::2 path of G1 / B1
     c->cc_major = prop.major;
     c->max_atoms = max_atoms;
     c->max_mols = max_mols;
-    c->max_rows = (max_atoms + NSP * (ROW_TILE - 1) + ROW_TILE - 1) / ROW_TILE * ROW_TILE + ROW_TILE;
+    c->max_rows = (max_atoms + NSP * (ROW_ALIGN - 1) + ROW_ALIGN - 1) / ROW_ALIGN * ROW_ALIGN + ROW_ALIGN;
     c->max_cells = max_atoms * 2 > 256 ? max_atoms * 2 : 256;
     if (max_mols > c->max_cells) c->max_cells = max_mols;
     // neighbour storage: 160 directed pairs per atom on average (rho = 0.1 A^-3 gives 55 at 5.1 A); for tiny

@@ -31,7 +31,10 @@ constexpr int OFF_W4 = OFF_B3 + H3;
 constexpr int OFF_B4 = OFF_W4 + H3;
 static_assert(OFF_B4 + 1 == NET_PARAMS, "blob layout");
 
-constexpr int ROW_TILE = 128;                   // species groups start at multiples of this many rows
+constexpr int ROW_TILE = 128;                   // rows of one MLP tile (UMMA M of one CTA)
+constexpr int ROW_ALIGN = 2 * ROW_TILE;         // species groups start at multiples of this many rows: the two row tiles of a
+                                                // CTA pair (tcgen05 cta_group::2) always run the same network; tile masks are
+                                                // kept equal within such a pair
 constexpr int KBLK = 64;                        // feature-block width: the unit in which zero columns are skipped
 constexpr int N_KBLK = AEV_LD / KBLK;           // 16 blocks: 14 angular (2 species pairs each) + 2 radial
 constexpr int MAX_MODELS = 8;
@@ -86,6 +89,8 @@ struct Ctx {
     int64_t max_atoms, max_mols, max_rows, max_cells, pair_cap;
     int sm_count, cc_major;
     int mlp_mode;
+    bool tc_pairs;         // G1 / B1 run on CTA pairs (tcgen05 cta_group::2): DHP_TC_PAIRS=1 in the environment at dhp_create; off by default
+                           // (measured equal on G1, slower on B1 - DESIGN.md §6.3)
     int64_t launches;
     char cuda_err[256];
     Profile prof;

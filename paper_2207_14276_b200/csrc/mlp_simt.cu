@@ -2,7 +2,7 @@
 //
 // This is the small-system path and the numerical scaffold of the tensor path (mlp_tc.cu): plain tiled
 // SGEMM, 64x64 tiles, 4x4 register micro-tiles, activations kept in HBM between layers.
-// Rows are grouped by the central atom's species (groups start at multiples of ROW_TILE = 128 rows), so a
+// Rows are grouped by the central atom's species (groups start at multiples of ROW_ALIGN = 256 rows), so a
 // 64-row tile uses one network; blockIdx.z is the ensemble member.
 //   forward : h1 = CELU(G W1^T + b1), h2 = CELU(h1 W2^T + b2), h3 = CELU(h2 W3^T + b3),
 //             E_i = (1/M) sum_e (w4 . h3 + b4)
@@ -148,7 +148,7 @@ void mlp_simt_free(Ctx* ctx) {
 int mlp_simt(Ctx* ctx, const Weights* w, bool forward_only) {
     if (ctx->n_atoms == 0) return DHP_OK;
     const int M = w->n_models;
-    const int row_tiles = (int)((ctx->n_atoms + NSP * (ROW_TILE - 1) + TM - 1) / TM);   // bound on sp_start[7]/TM
+    const int row_tiles = (int)((ctx->n_atoms + NSP * (ROW_ALIGN - 1) + TM - 1) / TM);   // bound on sp_start[7]/TM
     float *h1 = ctx->act[0], *h2 = ctx->act[1], *h3 = ctx->act[2], *d3 = ctx->act[3], *d2 = ctx->act[4], *d1 = ctx->act[5];
     const float alpha = ctx->params.celu_alpha;
     GemmArgs g{};

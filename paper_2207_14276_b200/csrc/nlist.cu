@@ -8,7 +8,7 @@
 // temporary row; a second pass assigns CSR offsets and orders each row by (angular first, then
 // radial-only) x neighbour species.  Rows hold sorted-slot indices.  Rows of the AEV / MLP buffers are
 // grouped by the central atom's species (stable in sorted order), each group starting at a multiple
-// of ROW_TILE rows so that one MLP tile never mixes networks.
+// of ROW_ALIGN rows so that one MLP tile (and one CTA pair of two tiles) never mixes networks.
 #include <algorithm>
 #include <string.h>
 
@@ -262,7 +262,7 @@ k_rowkey_hist(const float4* __restrict__ spos, const unsigned* __restrict__ amas
 }
 
 // single block of 1024 threads, warps take keys round-robin: exclusive scan over blocks per key, then the key starts
-// (species groups aligned to ROW_TILE)
+// (species groups aligned to ROW_ALIGN)
 __global__ void __launch_bounds__(1024)
 k_rowkey_scan(int* __restrict__ blk_hist, int nrb, int* __restrict__ sp_count, int* __restrict__ sp_start, int* __restrict__ key_start,
               const int* __restrict__ gate) {
@@ -294,7 +294,7 @@ k_rowkey_scan(int* __restrict__ blk_hist, int nrb, int* __restrict__ sp_count, i
             int c = 0;
             for (int k = 0; k < NCLS; ++k) { key_start[s * NCLS + k] = start + c; c += tot[s * NCLS + k]; }
             sp_count[s] = c;
-            start += (c + ROW_TILE - 1) / ROW_TILE * ROW_TILE;
+            start += (c + ROW_ALIGN - 1) / ROW_ALIGN * ROW_ALIGN;
         }
         sp_start[NSP] = start;
         sp_count[NSP] = 0;
@@ -327,7 +327,11 @@ k_rowkey_rank(const float4* __restrict__ spos, const unsigned* __restrict__ amas
     rowmap[a] = row;
     row_species[row] = s;
     row_slot[row] = a;
-    if (m) atomicOr(&tile_mask[row / ROW_TILE], m);
+    if (m) {                                  // pair-uniform masks; most rows add nothing new to their tile pair
+        volatile unsigned* t = tile_mask + ((row / ROW_TILE) & ~1);
+        if ((t[0] & m) != m) atomicOr((unsigned*)t, m);
+        if ((t[1] & m) != m) atomicOr((unsigned*)t + 1, m);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -643,7 +647,7 @@ k_rows(const unsigned* __restrict__ tmp, int stride, const int* __restrict__ cnt
                 amask[i] = bmask;
                 if (reuse_rows && bmask) {
                     const int row = rowmap[i];
-                    if (row >= 0) atomicOr(&tile_mask[row / ROW_TILE], bmask);
+                    if (row >= 0) { atomicOr(&tile_mask[(row / ROW_TILE) & ~1], bmask); atomicOr(&tile_mask[(row / ROW_TILE) | 1], bmask); }
                 }
             }
         }

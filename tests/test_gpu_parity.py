@@ -253,6 +253,25 @@ def test_mixed_precision_mode_error_is_bounded_and_documented(torch, B, params, 
     d.close()
 
 
+@pytest.mark.parametrize("name", ["water96", "mix600", "replicas16"])
+def test_cta_pair_kernels_opt_in(torch, B, params, blob8, name, monkeypatch):
+    """DHP_TC_PAIRS=1 runs G1 and B1 as tcgen05 cta_group::2 kernels (two row tiles per MMA, half of the weight tile per
+    CTA, cost-balanced static schedule).  Same arithmetic as the default kernels, so the same bars apply."""
+    monkeypatch.setenv("DHP_TC_PAIRS", "1")
+    s = SYSTEMS[name]()
+    probe = make_ctx(B, s, params)
+    ok = probe.dhp_tensor_path_available()
+    probe.close()
+    if not ok:
+        pytest.skip("tensor path not available in this build")
+    d, E, F = run_gpu(B, torch, s, params, blob8, B.MLP_TENSOR)
+    Eo, Fo = oracle.total_energy_forces(s, params, blob8[: s.n_models * 7 * W.PARAMS_PER_NET])
+    per = s.n_atoms if s.mol_offsets is None else np.diff(s.mol_offsets)
+    assert np.max(np.abs(E - Eo) / per) <= E_TOL_PER_ATOM
+    assert np.max(np.abs(F - Fo)) <= F_TOL
+    d.close()
+
+
 def test_host_entry_point_matches_device_entry_point(torch, B, params, blob8):
     s = SYSTEMS["mix600"]()
     d, E, F = run_gpu(B, torch, s, params, blob8)
@@ -333,7 +352,8 @@ def test_rows_are_ordered_by_feature_block_class(torch, B, params, blob8):
     s = W.make_system(1)
     d, _, _ = run_gpu(B, torch, s, params, blob8)
     tiles, blocks = d.dhp_debug_tile_blocks()
-    assert tiles == 3 and blocks == 9                      # 192 H -> 2 tiles, 96 O -> 1 tile
+    assert tiles == 4 and blocks == 12                     # 192 H -> 2 tiles, 96 O -> 1 tile + 1 padding tile (groups are
+                                                           # aligned to tile PAIRS and a pair shares its mask)
     d.close()
     s = W.make_system(3)
     d, _, _ = run_gpu(B, torch, s, params, blob8)
