@@ -332,8 +332,23 @@ k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
     if (na > MAX_ANG || nst > MAX_RAD) { na = 0; nst = 0; cnt = 0; }     // capacity overflow: reported by the forward pass
 
     // ---- the blocks of dE/dG this atom uses ----------------------------------------------------------------
-    if (rowmap[i] < 0) return;                         // not a central atom of this call (partial evaluation)
-    const float* grow = grad + (size_t)rowmap[i] * AEV_LD;
+    const int row_i = rowmap[i];
+    if (row_i < 0) return;                             // not a central atom of this call (partial evaluation)
+    const float* grow = grad + (size_t)row_i * AEV_LD;
+    // The neighbour chain (row_ptr -> col -> spos) and the dE/dG rows (DRAM) are independent: request the first two
+    // rounds of neighbours now, so that their latency runs under the staging of the gradient blocks below
+    const int rb = row_ptr[i];
+    const float4 pi = spos[i];
+    constexpr int PRE = 2;
+    int jg_pre[PRE];
+    float4 pj_pre[PRE];
+#pragma unroll
+    for (int q = 0; q < PRE; ++q) {
+        const int a = lane + 32 * q;
+        jg_pre[q] = a < nst ? col[rb + a] : i;
+    }
+#pragma unroll
+    for (int q = 0; q < PRE; ++q) pj_pre[q] = spos[jg_pre[q]];
     {
         int psa = 0, psb = 0;
         if (lane < NPAIR) { const int e = c_pair_sp[lane]; psa = e & 15; psb = e >> 4; }
@@ -348,8 +363,6 @@ k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
     }
     __syncwarp();
 
-    const int rb = row_ptr[i];
-    const float4 pi = spos[i];
     const float inv_rcr = 1.0f / K.rcr, inv_rca = 1.0f / K.rca;
     float fix = 0.f, fiy = 0.f, fiz = 0.f;              // force on the centre, summed over this lane's terms
     float Fx[OWN], Fy[OWN], Fz[OWN];                    // forces on the neighbours lane, lane + 32, lane + 64
@@ -362,8 +375,8 @@ k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
     for (int q = 0; q < MAX_RAD / 32; ++q) {
         const int a = lane + 32 * q;
         if (32 * q < nst && a < nst) {
-            const int jg = col[rb + a];
-            const NbrGeom nbq = neighbour_geom(pi, spos[jg], g);
+            const int jg = q < PRE ? jg_pre[q < PRE ? q : 0] : col[rb + a];
+            const NbrGeom nbq = neighbour_geom(pi, q < PRE ? pj_pre[q < PRE ? q : 0] : spos[jg], g);
             const float fc = fcut(nbq.R, inv_rcr), dfc = dfcut(nbq.R, inv_rcr, K.pi_over_rcr);
             const float c1 = -2.0f * K.eta_r * fc;
             const float4* gr = reinterpret_cast<const float4*>(&S.g_rad[NR * nbq.sp]);

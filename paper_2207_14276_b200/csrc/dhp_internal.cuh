@@ -89,8 +89,8 @@ struct Ctx {
     int64_t max_atoms, max_mols, max_rows, max_cells, pair_cap;
     int sm_count, cc_major;
     int mlp_mode;
-    bool tc_pairs;         // G1 / B1 run on CTA pairs (tcgen05 cta_group::2): DHP_TC_PAIRS=1 in the environment at dhp_create; off by default
-                           // (measured equal on G1, slower on B1 - DESIGN.md §6.3)
+    int tc_pairs;          // bit 0: G1, bit 1: B1 run on CTA pairs (tcgen05 cta_group::2); DHP_TC_PAIRS=<bits> in the environment
+                           // at dhp_create overrides the default
     int64_t launches;
     char cuda_err[256];
     Profile prof;

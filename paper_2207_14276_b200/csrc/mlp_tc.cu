@@ -537,7 +537,8 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
 //                   warps 2..9: epilogue of the CTA's own 128 rows (own TMEM lanes)
 //   barriers        empty[stage], tfull[acc]: tcgen05.commit multicast to both CTAs; tempty[acc] lives in the leader and
 //                   counts the epilogue warps of both CTAs (the peer's arrive remotely)
-//   schedule        static: item = column tile nt (major) x row-tile pair, cluster c takes items c, c + n_clusters, ...
+//   schedule        static and cost-balanced (k_pair_schedule): cluster c takes a contiguous range of items; G1 orders them
+//                   pair-major (a pair's AEV tile is reused by its 8 networks out of L2), B1 column-tile-major
 // B1's column tile = up to 4 selected 64-wide feature blocks; the N split gives CTA r the r-th 32-row half of every
 // selected block, so accumulator columns [0, 32 nb) are the first halves and [32 nb, 64 nb) the second halves.
 // ======================================================================================================
@@ -622,7 +623,11 @@ k_pair_schedule(const unsigned* __restrict__ tile_mask, const int* __restrict__ 
         for (int b = 0; b < n_items; b += 1024) {                         // inclusive prefix of the item costs -> scratch
             const int i = b + tid;
             int v = 0;
-            if (i < n_items) { const int nt = i / n_pairs, pr = i - nt * n_pairs; v = pair_item_cost(tile_mask[2 * pr], nt, which); }
+            if (i < n_items) {                          // G1: pair-major (the 8 networks of a pair back to back: its AEV tile
+                int nt, pr;                             // stays in L2); B1: column-tile-major
+                if (which == 0) { pr = i / n_tiles; nt = i - pr * n_tiles; } else { nt = i / n_pairs; pr = i - nt * n_pairs; }
+                v = pair_item_cost(tile_mask[2 * pr], nt, which);
+            }
             int x = v;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
@@ -722,7 +727,7 @@ k_gemm_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
         if (elect_one()) {
             int stage = 0; uint32_t phase = 0;
             for (int item = item_lo; item < item_hi; ++item) {
-                const int nt = item / n_pairs, pr = item - nt * n_pairs;
+                const int nt = CMP == CMP_K ? item % p.n_tiles : item / n_pairs, pr = CMP == CMP_K ? item / p.n_tiles : item - nt * n_pairs;
                 if (!has_work(pr, nt)) continue;
                 const int rt = 2 * pr + rank, row0 = rt * BM;
                 const int s = pair_species(pr);
@@ -788,7 +793,7 @@ k_gemm_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
                 // ===== MMA issuer of the pair =====
                 int acc = 0; uint32_t acc_phase = 0;
                 for (int item = item_lo; item < item_hi; ++item) {
-                    const int nt = item / n_pairs, pr = item - nt * n_pairs;
+                    const int nt = CMP == CMP_K ? item % p.n_tiles : item / n_pairs, pr = CMP == CMP_K ? item / p.n_tiles : item - nt * n_pairs;
                     if (!has_work(pr, nt)) continue;
                     int bn = p.BN;
                     if (CMP == CMP_N) bn = KBLK * min(4, __popc(pair_mask(pr)) - 4 * nt);
@@ -828,7 +833,7 @@ k_gemm_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
             } else if (!DIRECT) {
                 // ===== relay: this CTA's stage is full -> tell the leader's MMA issuer =====
                 for (int item = item_lo; item < item_hi; ++item) {
-                    const int nt = item / n_pairs, pr = item - nt * n_pairs;
+                    const int nt = CMP == CMP_K ? item % p.n_tiles : item / n_pairs, pr = CMP == CMP_K ? item / p.n_tiles : item - nt * n_pairs;
                     if (!has_work(pr, nt)) continue;
                     for (unsigned km = k_mask(pr); km; km &= km - 1u) {
                         mbar_wait(full_bar(stage), phase);
@@ -844,7 +849,7 @@ k_gemm_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
         int acc = 0; uint32_t acc_phase = 0;
         const float kexp = 1.4426950408889634f / p.alpha;
         for (int item = item_lo; item < item_hi; ++item) {
-            const int nt = item / n_pairs, pr = item - nt * n_pairs;
+            const int nt = CMP == CMP_K ? item % p.n_tiles : item / n_pairs, pr = CMP == CMP_K ? item / p.n_tiles : item - nt * n_pairs;
             if (!has_work(pr, nt)) continue;
             const int rt = 2 * pr + rank;
             const int row = rt * BM + q * 32 + lane;
@@ -1591,9 +1596,10 @@ int mlp_tc(Ctx* ctx, const Weights* wt, bool forward_only) {
     a.acc_scale = 1.0f / W_SCALE; a.bias = t->b1;
     a.a_tiled = nullptr; a.out_planes = ws->h1; a.out_kblocks = M * KB1; a.out_cols_per_tile = H1;
     a.sched = ctx->tc_sched + 0;
-    const bool pairs = ctx->tc_pairs && ctx->mlp_mode != DHP_MLP_TENSOR_LAYERWISE;      // G1 / B1 on CTA pairs (cta_group::2)
+    const bool fusedp = ctx->mlp_mode != DHP_MLP_TENSOR_LAYERWISE;
+    const bool pairs = (ctx->tc_pairs & 1) && fusedp, pairs_b1 = (ctx->tc_pairs & 2) && fusedp;    // G1 / B1 on CTA pairs (cta_group::2)
     const int ncl = ctx->sm_count / 2;
-    if (pairs) {
+    if (pairs || pairs_b1) {
         DHP_LAUNCH(ctx, k_pair_schedule, 1, 1024, 0, ctx->tile_mask, ctx->sp_start, M, ncl, ws->pair_scratch, ws->pair_sched);
         a.pair_start = ws->pair_sched;
     }
@@ -1650,7 +1656,7 @@ int mlp_tc(Ctx* ctx, const Weights* wt, bool forward_only) {
     a.acc_scale = 1.0f / (W_SCALE * D_SCALE); a.out_f32 = ctx->grad; a.out_ld = AEV_LD;
     a.sched = ctx->tc_sched + 5;
     a.pair_start = ws->pair_sched + (ncl + 1);
-    if (pairs) rc = launch_pair<EPI_GRAD, CMP_N>(ctx, ws->m_aev, t->m_w1b_half, a);
+    if (pairs_b1) rc = launch_pair<EPI_GRAD, CMP_N>(ctx, ws->m_aev, t->m_w1b_half, a);
     else rc = launch_gemm<EPI_GRAD, CMP_N>(ctx, ws->m_aev, t->m_w1b, a);
     if (rc != DHP_OK) return rc;
     DHP_CUDA(ctx, cudaGetLastError());

@@ -272,17 +272,24 @@ k_rowkey_scan(int* __restrict__ blk_hist, int nrb, int* __restrict__ sp_count, i
     for (int key = w; key < NKEY; key += 32) {
         int* hk = blk_hist + (size_t)key * nrb;
         int run = 0;
-        for (int base = 0; base < nrb; base += 32) {
-            const int b = base + lane;
-            const int v = b < nrb ? hk[b] : 0;
-            int x = v;
+        constexpr int CH = 16;                              // 16 x 32 counts are requested at once: one memory latency per
+        for (int base = 0; base < nrb; base += 32 * CH) {   // 512 blocks of a key instead of one per 32
+            int v[CH];
 #pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                int y = __shfl_up_sync(0xffffffffu, x, o);
-                if (lane >= o) x += y;
+            for (int c = 0; c < CH; ++c) { const int bb = base + 32 * c + lane; v[c] = bb < nrb ? hk[bb] : 0; }
+#pragma unroll
+            for (int c = 0; c < CH; ++c) {
+                if (base + 32 * c >= nrb) break;
+                const int bb = base + 32 * c + lane;
+                int x = v[c];
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    int y = __shfl_up_sync(0xffffffffu, x, o);
+                    if (lane >= o) x += y;
+                }
+                if (bb < nrb) hk[bb] = run + x - v[c];
+                run += __shfl_sync(0xffffffffu, x, 31);
             }
-            if (b < nrb) hk[b] = run + x - v;
-            run += __shfl_sync(0xffffffffu, x, 31);
         }
         if (lane == 0) tot[key] = run;
     }
@@ -327,10 +334,15 @@ k_rowkey_rank(const float4* __restrict__ spos, const unsigned* __restrict__ amas
     rowmap[a] = row;
     row_species[row] = s;
     row_slot[row] = a;
-    if (m) {                                  // pair-uniform masks; most rows add nothing new to their tile pair
-        volatile unsigned* t = tile_mask + ((row / ROW_TILE) & ~1);
-        if ((t[0] & m) != m) atomicOr((unsigned*)t, m);
-        if ((t[1] & m) != m) atomicOr((unsigned*)t + 1, m);
+    // tile masks, kept equal within a tile pair (ROW_ALIGN): the lanes of the warp that fall into the same pair combine
+    // their masks first, one lane per pair does the atomics
+    const int pair = row / ROW_ALIGN;
+    const unsigned act = __activemask();
+    const unsigned grp2 = __match_any_sync(act, pair);
+    const unsigned mm = __reduce_or_sync(grp2, m);
+    if (mm && lane == __ffs(grp2) - 1) {
+        atomicOr(&tile_mask[2 * pair], mm);
+        atomicOr(&tile_mask[2 * pair + 1], mm);
     }
 }
 

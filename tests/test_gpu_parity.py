@@ -257,7 +257,7 @@ def test_mixed_precision_mode_error_is_bounded_and_documented(torch, B, params, 
 def test_cta_pair_kernels_opt_in(torch, B, params, blob8, name, monkeypatch):
     """DHP_TC_PAIRS=1 runs G1 and B1 as tcgen05 cta_group::2 kernels (two row tiles per MMA, half of the weight tile per
     CTA, cost-balanced static schedule).  Same arithmetic as the default kernels, so the same bars apply."""
-    monkeypatch.setenv("DHP_TC_PAIRS", "1")
+    monkeypatch.setenv("DHP_TC_PAIRS", "3")
     s = SYSTEMS[name]()
     probe = make_ctx(B, s, params)
     ok = probe.dhp_tensor_path_available()
