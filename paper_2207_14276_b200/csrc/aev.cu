@@ -68,7 +68,11 @@ __device__ __forceinline__ float dfcut(float R, float inv_rc, float pi_over_rc) 
 constexpr int AEV_WARPS = 8;
 constexpr int MAX_RAD = 192;    // radial neighbours staged per centre (= the pair list's per-row capacity)
 
-__constant__ unsigned char c_pair_sp[NPAIR];    // internal pair p -> species a | species b << 4
+// internal pair p = hi (hi + 1) / 2 + lo over priority positions -> species(lo) | species(hi) << 4 (prio_sp(), dhp_internal.cuh);
+// a static initialiser, so every device of the process has it without a per-device upload
+#define DHP_PAIR_SP_TABLE {0, 48, 51, 16, 19, 17, 32, 35, 33, 34, 64, 67, 65, 66, 68, 80, 83, 81, 82, 84, 85, 96, 99, 97, 98, 100, 101, 102}
+__constant__ unsigned char c_pair_sp[NPAIR] = DHP_PAIR_SP_TABLE;
+static const unsigned char h_pair_sp[NPAIR] = DHP_PAIR_SP_TABLE;
 
 constexpr int TP = 36;          // pitch of the staged factor rows: 16-byte aligned, rows 4 banks apart (conflict-free float4 reads)
 
@@ -536,21 +540,22 @@ __global__ void k_energy_reduce(const float* __restrict__ e_atom, const int* __r
 }
 
 // -------------------------------------------------------------------------------------------------
+// per-device kernel attributes (dynamic shared memory above 48 KB); called once per context from dhp_create
+int aev_init(Ctx* ctx) {
+    for (int hi = 0, p = 0; hi < NSP; ++hi)            // the literal table above must match prio_sp()
+        for (int lo = 0; lo <= hi; ++lo, ++p)
+            if ((prio_sp(lo) | (prio_sp(hi) << 4)) != (int)h_pair_sp[p]) return DHP_E_BADARG;
+    DHP_CUDA(ctx, cudaFuncSetAttribute(k_aev_fwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(WarpSmemFwd) * AEV_WARPS)));
+    DHP_CUDA(ctx, cudaFuncSetAttribute(k_aev_fwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(WarpSmemFwd) * AEV_WARPS)));
+    DHP_CUDA(ctx, cudaFuncSetAttribute(k_aev_bwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(WarpSmemBwd) * BWD_WARPS)));
+    return DHP_OK;
+}
+
 int aev_forward(Ctx* ctx, bool planes) {
     const int n = (int)ctx->n_atoms;
     ctx->aev_in_planes = planes;
     if (n == 0) return DHP_OK;
-    static bool init = false;
     const size_t smem = sizeof(WarpSmemFwd) * AEV_WARPS;
-    if (!init) {
-        DHP_CUDA(ctx, cudaFuncSetAttribute(k_aev_fwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        DHP_CUDA(ctx, cudaFuncSetAttribute(k_aev_fwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        unsigned char tab[NPAIR];
-        for (int hi = 0, p = 0; hi < NSP; ++hi)
-            for (int lo = 0; lo <= hi; ++lo, ++p) tab[p] = (unsigned char)(prio_sp(lo) | (prio_sp(hi) << 4));
-        DHP_CUDA(ctx, cudaMemcpyToSymbol(c_pair_sp, tab, sizeof(tab)));
-        init = true;
-    }
     const int blocks = (n + AEV_WARPS - 1) / AEV_WARPS;
     const size_t plane_stride = (size_t)ctx->max_rows * AEV_LD;
     if (planes)
@@ -566,12 +571,7 @@ int aev_forward(Ctx* ctx, bool planes) {
 int aev_backward(Ctx* ctx, float* F_out) {
     const int n = (int)ctx->n_atoms;
     if (n == 0) return DHP_OK;
-    static bool attr_set = false;
     const size_t smem = sizeof(WarpSmemBwd) * BWD_WARPS;
-    if (!attr_set) {
-        DHP_CUDA(ctx, cudaFuncSetAttribute(k_aev_bwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
-    }
     DHP_CUDA(ctx, cudaMemsetAsync(ctx->fsorted, 0, sizeof(float) * 3 * n, ctx->stream));
     DHP_LAUNCH(ctx, k_aev_bwd, (n + BWD_WARPS - 1) / BWD_WARPS, BWD_WARPS * 32, smem, ctx->spos, ctx->row_ptr, ctx->col,
                ctx->seg_cnt, ctx->rowmap, ctx->grid, ctx->aevc, n, ctx->grad, ctx->fsorted);

@@ -209,6 +209,7 @@ int dhp_create(dhp_ctx** out, const dhp_params* params, int64_t max_atoms, int64
     ok &= dalloc(&c->tile_mask, R / ROW_TILE) && dalloc(&c->tc_sched, 8) && dalloc(&c->col2feat, AEV_LD);
     ok &= dalloc(&c->fsorted, 3 * N) && dalloc(&c->e_out_tmp, NM) && dalloc(&c->export_tmp, N + 1);
     ok &= dalloc(&c->st_pos, 3 * N) && dalloc(&c->st_species, N) && dalloc(&c->st_mol, NM + 1) && dalloc(&c->st_E, NM) && dalloc(&c->st_F, 3 * N);
+    if (ok) ok = aev_init(c) == DHP_OK;
     if (ok) ok = mlp_simt_alloc(c) == DHP_OK;
     if (ok && mlp_tc_available(c)) ok = mlp_tc_alloc(c) == DHP_OK;
     if (ok) {

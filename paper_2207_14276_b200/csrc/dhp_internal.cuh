@@ -182,6 +182,7 @@ void prof_mark(Ctx* ctx, int boundary);   // records event `boundary` (start of 
 int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t* species, int64_t n,
                 const int32_t* mol_offsets, int64_t n_mol, const uint8_t* central = nullptr);
 int nlist_export(Ctx* ctx, int32_t* row_ptr, int32_t* col, bool angular);
+int aev_init(Ctx* ctx);                    // per-device kernel attributes
 int aev_forward(Ctx* ctx, bool planes);   // planes: write the tensor path's fp16 hi/lo planes instead of fp32 rows
 int aev_backward(Ctx* ctx, float* F_out);
 int mlp_simt(Ctx* ctx, const Weights* w, bool forward_only);

@@ -1478,22 +1478,12 @@ struct TcWeights {                    // per weight handle
 
 template <int EPI, int CMP>
 int launch_gemm(Ctx* ctx, const CUtensorMap& a, const CUtensorMap& b, const TcArgs& args) {
-    static bool attr = false;
-    if (!attr) {
-        DHP_CUDA(ctx, cudaFuncSetAttribute((k_gemm_tc<EPI, CMP>), cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
-        attr = true;
-    }
     DHP_LAUNCH(ctx, (k_gemm_tc<EPI, CMP>), ctx->sm_count, TC_THREADS, SMEM_BYTES, a, b, args);
     return DHP_OK;
 }
 
 template <int EPI, int CMP>
 int launch_pair(Ctx* ctx, const CUtensorMap& a, const CUtensorMap& b, const TcArgs& args) {
-    static bool attr = false;
-    if (!attr) {
-        DHP_CUDA(ctx, cudaFuncSetAttribute((k_gemm_pair<EPI, CMP>), cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM_BYTES));
-        attr = true;
-    }
     DHP_LAUNCH(ctx, (k_gemm_pair<EPI, CMP>), ctx->sm_count & ~1, TC_THREADS, P_SMEM_BYTES, a, b, args);
     return DHP_OK;
 }
@@ -1502,7 +1492,22 @@ int launch_pair(Ctx* ctx, const CUtensorMap& a, const CUtensorMap& b, const TcAr
 
 bool mlp_tc_available(Ctx* ctx) { return ctx->cc_major == 10 && get_encode() != nullptr; }
 
+template <int EPI, int CMP>
+static int set_smem_tc(Ctx* ctx) {
+    DHP_CUDA(ctx, cudaFuncSetAttribute((k_gemm_tc<EPI, CMP>), cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
+    return DHP_OK;
+}
+
 int mlp_tc_alloc(Ctx* ctx) {
+    // per-device kernel attributes (dynamic shared memory above 48 KB), once per context
+    int rc;
+    if ((rc = set_smem_tc<EPI_CELU, CMP_K>(ctx)) != DHP_OK || (rc = set_smem_tc<EPI_CELU, CMP_NONE>(ctx)) != DHP_OK ||
+        (rc = set_smem_tc<EPI_OUT, CMP_NONE>(ctx)) != DHP_OK || (rc = set_smem_tc<EPI_DCELU, CMP_NONE>(ctx)) != DHP_OK ||
+        (rc = set_smem_tc<EPI_GRAD, CMP_N>(ctx)) != DHP_OK)
+        return rc;
+    DHP_CUDA(ctx, cudaFuncSetAttribute((k_gemm_pair<EPI_CELU, CMP_K>), cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM_BYTES));
+    DHP_CUDA(ctx, cudaFuncSetAttribute((k_gemm_pair<EPI_GRAD, CMP_N>), cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM_BYTES));
+    DHP_CUDA(ctx, cudaFuncSetAttribute(k_mlp_mid, cudaFuncAttributeMaxDynamicSharedMemorySize, MID_SMEM));
     TcWorkspace* w = new (std::nothrow) TcWorkspace();
     if (!w) return DHP_E_NOMEM;
     memset((void*)w, 0, sizeof(*w));
@@ -1609,11 +1614,6 @@ int mlp_tc(Ctx* ctx, const Weights* wt, bool forward_only) {
     prof_mark(ctx, DHP_PHASE_MLP_MID);
     if (ctx->mlp_mode != DHP_MLP_TENSOR_LAYERWISE) {
         // G2 .. B2 fused: h1 -> d1 with h2, d3, d2 kept on chip
-        static bool attr = false;
-        if (!attr) {
-            DHP_CUDA(ctx, cudaFuncSetAttribute(k_mlp_mid, cudaFuncAttributeMaxDynamicSharedMemorySize, MID_SMEM));
-            attr = true;
-        }
         MidArgs m{};
         m.single = a.single;
         m.row_species = ctx->row_species; m.sp_start = ctx->sp_start; m.n_models = M; m.plane_tiles = R / BM;
