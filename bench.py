@@ -94,20 +94,20 @@ def oracle_sample_rate(system, params, blob, target_s: float = 15.0, seed: int =
     n_try = min(system.n_atoms, 4 * oracle.num_threads())
     centres = rng.choice(system.n_atoms, n_try, replace=False).astype(np.int32)
     t0 = time.perf_counter()
-    oracle.energy_forces(system.pos, system.species, system.box, params, blob, system.n_models, centres=centres,
-                         mol_offsets=system.mol_offsets)
+    Ea, Fo, _ = oracle.energy_forces(system.pos, system.species, system.box, params, blob, system.n_models, centres=centres,
+                                     mol_offsets=system.mol_offsets)
     dt = time.perf_counter() - t0
     n = n_try
     for _ in range(3):          # the probe over-estimates the per-atom cost (thread start-up): refine until ~target_s
         n = int(min(system.n_atoms, max(n_try, n * target_s / max(dt, 1e-3))))
         centres = rng.choice(system.n_atoms, n, replace=False).astype(np.int32)
         t0 = time.perf_counter()
-        oracle.energy_forces(system.pos, system.species, system.box, params, blob, system.n_models, centres=centres,
-                             mol_offsets=system.mol_offsets)
+        Ea, Fo, _ = oracle.energy_forces(system.pos, system.species, system.box, params, blob, system.n_models, centres=centres,
+                                         mol_offsets=system.mol_offsets)
         dt = time.perf_counter() - t0
         if dt >= 0.6 * target_s or n == system.n_atoms:
             break
-    return n / dt, n, dt, oracle.num_threads()
+    return n / dt, n, dt, oracle.num_threads(), centres, Ea, Fo
 
 
 def run_reference(args, system, params, blob):
@@ -391,10 +391,22 @@ def main():
             "roofline_kernels": kernels,
         }
         if world == 1 and not args.no_cpu_baseline:
-            rate, n, dt, cores = oracle_sample_rate(system, params, blob)
+            rate, n, dt, cores, centres, Ea, Fo = oracle_sample_rate(system, params, blob)
             out["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
                                    "sample": f"{n} random central atoms of {system.name} (energies + the forces they exert) "
                                              f"in {dt:.1f} s, fp64, brute-force neighbours"}
+            # the same sample through the library (partial evaluation over exactly these central atoms, unjittered
+            # positions): parity of this launch configuration at full size, beside the timing
+            mask = torch.zeros(system.n_atoms, dtype=torch.uint8, device=dev)
+            mask[torch.from_numpy(centres.astype(np.int64)).to(dev)] = 1
+            pos0 = torch.from_numpy(system.pos).to(dev)
+            Ec, Fc = d.dhp_ani_energy_forces_partial(pos0, system.box, species, w, mask, mol)
+            torch.cuda.synchronize()
+            ea = d.dhp_debug_atomic_energy().cpu().numpy()
+            out["parity_sample"] = {"central_atoms": int(n), "abs_dE_per_atom": float(abs(Ec.sum().item() - Ea.sum()) / n),
+                                    "max_abs_dE_atom": float(np.abs(ea[centres] - Ea).max()),
+                                    "max_abs_dF": float(np.abs(Fc.cpu().numpy() - Fo).max()),
+                                    "bars": {"abs_dE_per_atom": 1e-6, "max_abs_dF": 5e-5}, "status": int(d.dhp_status())}
         print(json.dumps(out))
     d.close()
     if world > 1:

@@ -572,7 +572,7 @@ int aev_backward(Ctx* ctx, float* F_out) {
     const int n = (int)ctx->n_atoms;
     if (n == 0) return DHP_OK;
     const size_t smem = sizeof(WarpSmemBwd) * BWD_WARPS;
-    DHP_CUDA(ctx, cudaMemsetAsync(ctx->fsorted, 0, sizeof(float) * 3 * n, ctx->stream));
+    // fsorted was zeroed with the rest of the per-call arena at the start of the call (nlist_build)
     DHP_LAUNCH(ctx, k_aev_bwd, (n + BWD_WARPS - 1) / BWD_WARPS, BWD_WARPS * 32, smem, ctx->spos, ctx->row_ptr, ctx->col,
                ctx->seg_cnt, ctx->rowmap, ctx->grid, ctx->aevc, n, ctx->grad, ctx->fsorted);
     DHP_LAUNCH(ctx, k_unsort_forces, (n + 255) / 256, 256, 0, ctx->fsorted, ctx->perm, n, F_out);

@@ -40,10 +40,10 @@ static bool dalloc(T** p, size_t count) {
 }
 
 static void free_all(Ctx* c) {
-    void* ptrs[] = {c->grid, c->status, c->bbox, c->cell_of, c->perm_tmp, c->cell_count, c->cell_start, c->cell_fill, c->perm,
+    void* ptrs[] = {c->grid, c->zero_arena, c->ff_arena, c->bbox, c->cell_of, c->perm_tmp, c->cell_start, c->perm,
                     c->inv_perm, c->spos, c->smol, c->snc, c->n_rad, c->n_ang, c->row_ptr, c->col, c->sp_count, c->sp_start,
-                    c->rowmap, c->row_species, c->row_slot, c->blk_hist, c->key_start, c->amask, c->tile_mask, c->tc_sched, c->col2feat, c->aev, c->grad, c->e_atom, c->fsorted,
-                    c->e_out_tmp, c->export_tmp, c->cand, c->cand_cnt, c->pos_ref, c->rebuild, c->rebuild_count, c->tmp_col, c->blk_sum, c->blk_off, c->seg_cnt, c->st_pos, c->st_species, c->st_mol, c->st_E, c->st_F};
+                    c->rowmap, c->blk_hist, c->key_start, c->amask, c->col2feat, c->aev, c->grad,
+                    c->e_out_tmp, c->export_tmp, c->cand, c->cand_cnt, c->pos_ref, c->rebuild, c->rebuild_count, c->tmp_col, c->blk_off, c->seg_cnt, c->st_pos, c->st_species, c->st_mol, c->st_E, c->st_F};
     for (void* p : ptrs) if (p) cudaFree(p);
     mlp_simt_free(c);
     mlp_tc_free(c);
@@ -198,16 +198,31 @@ int dhp_create(dhp_ctx** out, const dhp_params* params, int64_t max_atoms, int64
     const size_t N = (size_t)max_atoms, R = (size_t)c->max_rows, NC = (size_t)c->max_cells;
     const size_t NM = (size_t)(max_mols > 0 ? max_mols : 1);
     bool ok = true;
-    ok &= dalloc(&c->grid, 1) && dalloc(&c->status, 1) && dalloc(&c->bbox, 8);
-    ok &= dalloc(&c->cell_of, N) && dalloc(&c->perm_tmp, N) && dalloc(&c->cell_count, NC + 1) && dalloc(&c->cell_start, NC + 1) && dalloc(&c->cell_fill, NC);
+    ok &= dalloc(&c->grid, 1) && dalloc(&c->bbox, 8);
+    ok &= dalloc(&c->cell_of, N) && dalloc(&c->perm_tmp, N) && dalloc(&c->cell_start, NC + 1);
     ok &= dalloc(&c->perm, N) && dalloc(&c->inv_perm, N) && dalloc(&c->spos, N) && dalloc(&c->smol, N) && dalloc(&c->snc, N);
     ok &= dalloc(&c->n_rad, N) && dalloc(&c->n_ang, N) && dalloc(&c->row_ptr, N + 1) && dalloc(&c->col, (size_t)c->pair_cap);
-    ok &= dalloc(&c->tmp_col, N * c->tmp_stride) && dalloc(&c->blk_sum, N / 64 + 3) && dalloc(&c->blk_off, N / 64 + 3) && dalloc(&c->seg_cnt, N * 16);
+    ok &= dalloc(&c->tmp_col, N * c->tmp_stride) && dalloc(&c->blk_off, N / 64 + 3) && dalloc(&c->seg_cnt, N * 16);
     ok &= dalloc(&c->sp_count, 8) && dalloc(&c->sp_start, 8) && dalloc(&c->rowmap, N);
-    ok &= dalloc(&c->row_species, R) && dalloc(&c->row_slot, R) && dalloc(&c->blk_hist, (N / 256 + 2) * 224) && dalloc(&c->key_start, 224) && dalloc(&c->amask, N);
-    ok &= dalloc(&c->aev, R * AEV_LD) && dalloc(&c->grad, R * AEV_LD) && dalloc(&c->e_atom, R);
-    ok &= dalloc(&c->tile_mask, R / ROW_TILE) && dalloc(&c->tc_sched, 8) && dalloc(&c->col2feat, AEV_LD);
-    ok &= dalloc(&c->fsorted, 3 * N) && dalloc(&c->e_out_tmp, NM) && dalloc(&c->export_tmp, N + 1);
+    ok &= dalloc(&c->blk_hist, (N / 256 + 2) * 224) && dalloc(&c->key_start, 224) && dalloc(&c->amask, N);
+    ok &= dalloc(&c->aev, R * AEV_LD) && dalloc(&c->grad, R * AEV_LD);
+    ok &= dalloc(&c->col2feat, AEV_LD);
+    ok &= dalloc(&c->e_out_tmp, NM) && dalloc(&c->export_tmp, N + 1);
+    {   // everything a hot call needs zeroed (or set to -1) lives in two arenas: two memsets per call instead of eleven
+        size_t off = 0;
+        auto take = [&](size_t words) { const size_t o = off; off += (words + 3) & ~(size_t)3; return o; };
+        const size_t o_status = take(1), o_sched = take(8), o_tmask = take(R / ROW_TILE), o_bsum = take(N / 64 + 3), o_ccnt = take(NC + 1),
+                     o_cfill = take(NC), o_eatom = take(R), o_fs = take(3 * N);
+        c->zero_words = off;
+        ok &= dalloc(&c->zero_arena, off) && dalloc(&c->ff_arena, 2 * R);
+        if (ok) {
+            c->status = (int*)c->zero_arena + o_status; c->tc_sched = (int*)c->zero_arena + o_sched;
+            c->tile_mask = (unsigned*)c->zero_arena + o_tmask; c->blk_sum = (int*)c->zero_arena + o_bsum;
+            c->cell_count = (int*)c->zero_arena + o_ccnt; c->cell_fill = (int*)c->zero_arena + o_cfill;
+            c->e_atom = (float*)c->zero_arena + o_eatom; c->fsorted = (float*)c->zero_arena + o_fs;
+            c->row_slot = c->ff_arena; c->row_species = c->ff_arena + R;
+        }
+    }
     ok &= dalloc(&c->st_pos, 3 * N) && dalloc(&c->st_species, N) && dalloc(&c->st_mol, NM + 1) && dalloc(&c->st_E, NM) && dalloc(&c->st_F, 3 * N);
     if (ok) ok = aev_init(c) == DHP_OK;
     if (ok) ok = mlp_simt_alloc(c) == DHP_OK;

@@ -101,6 +101,9 @@ struct Ctx {
     bool periodic;
 
     // workspace (device)
+    unsigned* zero_arena;  // status, tc_sched, tile_mask, blk_sum, cell_count, cell_fill, e_atom, fsorted: zeroed by ONE memset per hot call
+    size_t zero_words;
+    int* ff_arena;         // row_slot, row_species: set to -1 by one memset per hot call
     Grid* grid;
     int* status;
     unsigned* bbox;        // 6 ordered-uint min/max

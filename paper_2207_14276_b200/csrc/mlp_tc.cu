@@ -91,6 +91,9 @@ struct TcArgs {
     const unsigned* tile_mask;  // [row tiles] active 64-wide feature blocks (G1: K blocks to visit, B1: N blocks to produce)
     int* sched;               // dynamic tile counter of this launch (zeroed by the host)
     const int* pair_start;    // pair kernels: [n_clusters + 1] item range of every cluster (k_pair_schedule)
+    int ksplit;               // EPI_GRAD only: the K blocks of a tile are split over this many work items (power of two
+                              // <= KB) which add their partial results into out_f32 (zeroed by the host) - small systems,
+                              // where one tile's 32 sequential K blocks would leave most SMs idle
 };
 
 // how the feature-block mask of a row tile is used
@@ -302,9 +305,16 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n_row_tiles = p.sp_start[NSP] / BM;
-    const int total_tiles = n_row_tiles * p.n_tiles;
+    const int ksplit = (EPI == EPI_GRAD && p.ksplit > 1) ? p.ksplit : 1;
+    const int total_tiles = n_row_tiles * p.n_tiles * ksplit;
     const int KB = (p.K + BK - 1) / BK;
     const unsigned all_k = KB >= 32 ? 0xffffffffu : ((1u << KB) - 1u);
+    // K blocks of split ks of a tile: [ks KB / ksplit, (ks + 1) KB / ksplit)
+    auto split_mask = [&](int ks) -> unsigned {
+        if (ksplit == 1) return 0xffffffffu;
+        const int per = KB / ksplit;
+        return ((per >= 32 ? 0xffffffffu : ((1u << per) - 1u)) << (ks * per));
+    };
 
     if (warp == 0 && lane == 0) {
         for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
@@ -338,7 +348,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                 for (;;) {
                     tile = atomicAdd(p.sched, 1);
                     if (tile >= total_tiles) { tile = -1; break; }
-                    rt = tile / p.n_tiles; nt = tile - rt * p.n_tiles;
+                    rt = (tile / ksplit) / p.n_tiles; nt = (tile / ksplit) - rt * p.n_tiles;
                     if (CMP != CMP_N || 4 * nt < __popc(p.tile_mask[rt])) break;      // B1: nothing to produce
                 }
                 mbar_wait(sempty_bar(slot), sphase ^ 1u);
@@ -359,7 +369,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                     brow += nt * p.b_rows_per_tile;
                     tx = 2u * A_PLANE_BYTES + 2u * (uint32_t)p.BN * BK * 2u;
                 }
-                for (unsigned km = k_mask(rt); km; km &= km - 1u) {
+                for (unsigned km = k_mask(rt) & split_mask(tile % ksplit); km; km &= km - 1u) {
                     const int kb = __ffs(km) - 1;
                     mbar_wait(empty_bar(stage), phase ^ 1u);
                     const uint32_t sa = base + stage * STAGE_BYTES;
@@ -403,7 +413,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                 mbar_arrive(sempty_bar(slot));
                 if (++slot == RING) { slot = 0; sphase ^= 1u; }
                 if (tile < 0) break;
-                const int rt = tile / p.n_tiles, nt = tile - rt * p.n_tiles;
+                const int rt = (tile / ksplit) / p.n_tiles, nt = (tile / ksplit) - rt * p.n_tiles;
                 int bn = p.BN;
                 if (CMP == CMP_N) bn = KBLK * min(4, __popc(p.tile_mask[rt]) - 4 * nt);
                 const uint32_t idesc = make_idesc(bn);
@@ -411,7 +421,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + (uint32_t)(acc * ACC_STRIDE);
                 uint32_t accumulate = 0u;
-                for (unsigned km = k_mask(rt); km; km &= km - 1u) {
+                for (unsigned km = k_mask(rt) & split_mask(tile % ksplit); km; km &= km - 1u) {
                     const int kb = __ffs(km) - 1;
                     mbar_wait(full_bar(stage), phase);
                     tc_fence_after();
@@ -454,7 +464,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
             if (lane == 0) mbar_arrive(sempty_bar(slot));
             if (++slot == RING) { slot = 0; sphase ^= 1u; }
             if (tile < 0) break;
-            const int rt = tile / p.n_tiles, nt = tile - rt * p.n_tiles;
+            const int rt = (tile / ksplit) / p.n_tiles, nt = (tile / ksplit) - rt * p.n_tiles;
             const int row = rt * BM + q * 32 + lane;
             const int s = max(p.row_species[rt * BM], 0);
             const int ncols = p.n_tiles * p.BN;
@@ -507,9 +517,12 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                     }
                     float4* dst = reinterpret_cast<float4*>(p.out_f32 + (size_t)row * p.out_ld + gcol);
 #pragma unroll
-                    for (int i = 0; i < 8; ++i)
-                        dst[i] = make_float4(__uint_as_float(v[4 * i]) * p.acc_scale, __uint_as_float(v[4 * i + 1]) * p.acc_scale,
-                                             __uint_as_float(v[4 * i + 2]) * p.acc_scale, __uint_as_float(v[4 * i + 3]) * p.acc_scale);
+                    for (int i = 0; i < 8; ++i) {
+                        const float4 o = make_float4(__uint_as_float(v[4 * i]) * p.acc_scale, __uint_as_float(v[4 * i + 1]) * p.acc_scale,
+                                                     __uint_as_float(v[4 * i + 2]) * p.acc_scale, __uint_as_float(v[4 * i + 3]) * p.acc_scale);
+                        if (ksplit == 1) dst[i] = o;
+                        else atomicAdd(dst + i, o);              // partial sum over this item's K blocks (16-byte vector atomic)
+                    }
                 }
             }
             if (EPI == EPI_OUT) atomicAdd(&p.e_atom[row], (e_acc + (half == 0 ? p.b4[s * p.n_tiles + nt] : 0.f)) * p.inv_models);
@@ -1585,8 +1598,7 @@ int mlp_tc(Ctx* ctx, const Weights* wt, bool forward_only) {
     const int M = wt->n_models;
     const int R = (int)ctx->max_rows;
     int rc;
-    DHP_CUDA(ctx, cudaMemsetAsync(ctx->e_atom, 0, sizeof(float) * ctx->max_rows, ctx->stream));
-    DHP_CUDA(ctx, cudaMemsetAsync(ctx->tc_sched, 0, sizeof(int) * 8, ctx->stream));
+    // e_atom and the tile schedulers were zeroed with the rest of the per-call arena at the start of the call (nlist_build)
     if (!ctx->aev_in_planes)     // rows came from a forward pass in fp32 (debug / mixed use): split them here
         DHP_LAUNCH(ctx, k_split_rows, 4 * ctx->sm_count, 256, 0, ctx->aev, AEV_LD, ctx->sp_start, AEV_LD, ws->aev, R);
 
@@ -1655,6 +1667,16 @@ int mlp_tc(Ctx* ctx, const Weights* wt, bool forward_only) {
     a.a_tiled = ws->d1; a.a_kblocks = M * KB1; a.a_kb_per_tile = 0;
     a.acc_scale = 1.0f / (W_SCALE * D_SCALE); a.out_f32 = ctx->grad; a.out_ld = AEV_LD;
     a.sched = ctx->tc_sched + 5;
+    {   // small systems: fewer row tiles than SMs -> split K (all networks' 64-wide blocks) over several CTAs per tile
+        const int64_t tiles_bound = (ctx->n_atoms + ROW_TILE - 1) / ROW_TILE + 2 * NSP;   // row tiles incl. group padding
+        const int KBt = (M * H1) / BK;                                                       // 4 K blocks per network
+        int ks = 1;
+        while (ks * 2 <= KBt && KBt % (ks * 2) == 0 && tiles_bound * ks * 2 <= ctx->sm_count) ks *= 2;
+        a.ksplit = pairs_b1 ? 1 : ks;
+        if (a.ksplit > 1)
+            DHP_CUDA(ctx, cudaMemsetAsync(ctx->grad, 0, sizeof(float) * (size_t)std::min<int64_t>(tiles_bound * ROW_TILE, ctx->max_rows) * AEV_LD,
+                                          ctx->stream));
+    }
     a.pair_start = ws->pair_sched + (ncl + 1);
     if (pairs_b1) rc = launch_pair<EPI_GRAD, CMP_N>(ctx, ws->m_aev, t->m_w1b_half, a);
     else rc = launch_gemm<EPI_GRAD, CMP_N>(ctx, ws->m_aev, t->m_w1b, a);

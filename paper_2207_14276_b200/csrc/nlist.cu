@@ -842,13 +842,11 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
     const int* gate = skin ? ctx->rebuild : nullptr;             // nullptr: every kernel of the build path runs
     const double rl = rcr + (skin ? (double)ctx->skin : 0.0);    // list radius: the cell grid must cover it
 
-    DHP_CUDA(ctx, cudaMemsetAsync(ctx->status, 0, sizeof(int), st));
-    DHP_CUDA(ctx, cudaMemsetAsync(ctx->cell_count, 0, sizeof(int) * (ctx->max_cells + 1), st));
-    DHP_CUDA(ctx, cudaMemsetAsync(ctx->cell_fill, 0, sizeof(int) * ctx->max_cells, st));
-    DHP_CUDA(ctx, cudaMemsetAsync(ctx->tile_mask, 0, sizeof(unsigned) * (ctx->max_rows / ROW_TILE), st));
+    // one memset zeroes everything this call accumulates into (status word, cell counters, tile masks, block sums, and for
+    // the later phases the tile schedulers, atomic energies and sorted forces), one sets the row tables to -1
+    DHP_CUDA(ctx, cudaMemsetAsync(ctx->zero_arena, 0, sizeof(unsigned) * ctx->zero_words, st));
     if (!skin) {
-        DHP_CUDA(ctx, cudaMemsetAsync(ctx->row_slot, 0xFF, sizeof(int) * ctx->max_rows, st));
-        DHP_CUDA(ctx, cudaMemsetAsync(ctx->row_species, 0xFF, sizeof(int) * ctx->max_rows, st));
+        DHP_CUDA(ctx, cudaMemsetAsync(ctx->ff_arena, 0xFF, sizeof(int) * 2 * ctx->max_rows, st));
         ctx->cand_valid = false;
     }
     if (n == 0) {
@@ -858,7 +856,6 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
         ctx->cand_valid = false;
         return DHP_OK;
     }
-    DHP_CUDA(ctx, cudaMemsetAsync(ctx->blk_sum, 0, sizeof(int) * (nblk + 2), st));
     double L[3] = {0, 0, 0};
     if (periodic) for (int c = 0; c < 3; ++c) L[c] = (double)box_host[c];
     const int nb = (n + 255) / 256;
