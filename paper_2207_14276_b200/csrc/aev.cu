@@ -295,12 +295,11 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
 //   scatter      one global atomic triple per neighbour and one for the centre.
 // -------------------------------------------------------------------------------------------------
 constexpr int BWD_WARPS = 8;
-constexpr int GP = 36;   // pitch of one 32-float angular block of the staged gradient row (bank spread, 16 B aligned)
+
 constexpr int OWN = 3;   // neighbour slots per lane that can be angular (MAX_ANG = 96 = 3 x 32)
 static_assert(MAX_ANG <= OWN * 32, "angular neighbours must fit the per-lane force registers");
 
 struct __align__(16) WarpSmemBwd {
-    float g_ang[NPAIR * GP];     // dE/dG angular blocks of the row, [internal pair][32] at pitch GP
     float g_rad[NSP * NR];       // radial blocks by neighbour species
     float4 nb[MAX_ANG];          // ux, uy, uz, R of the angular neighbours
     float2 fd[MAX_ANG];          // f_c(R; Rca), f_c'(R; Rca)
@@ -308,7 +307,7 @@ struct __align__(16) WarpSmemBwd {
     int sp[MAX_ANG];
 };
 
-__global__ void __launch_bounds__(BWD_WARPS * 32)
+__global__ void __launch_bounds__(BWD_WARPS * 32, 4)
 k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, const int* __restrict__ col,
           const unsigned short* __restrict__ seg_cnt, const int* __restrict__ rowmap, const Grid* __restrict__ gp,
           const __grid_constant__ AevConst K, int n, const float* __restrict__ grad, float* __restrict__ fsorted) {
@@ -357,10 +356,12 @@ k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
         int psa = 0, psb = 0;
         if (lane < NPAIR) { const int e = c_pair_sp[lane]; psa = e & 15; psb = e >> 4; }
         const int ca = __shfl_sync(FULL, cnt, psa), cb = __shfl_sync(FULL, cnt, psb);
+        // the angular blocks of dE/dG are read straight from the row (4 KB, L1-resident after the first touch): no staging
+        // copy, and 4 KB less shared memory per warp (occupancy); touch the blocks this atom uses now so the lines arrive early
         unsigned nz = __ballot_sync(FULL, lane < NPAIR && ((psa == psb) ? ca > 1 : (ca > 0 && cb > 0)));
         for (; nz; nz &= nz - 1u) {
             const int p = __ffs(nz) - 1;
-            S.g_ang[p * GP + lane] = grow[32 * p + lane];
+            asm volatile("prefetch.global.L1 [%0];" ::"l"(grow + 32 * p + (lane & 1) * 16));
         }
         for (int s = 0; s < NSP; ++s)
             if (__shfl_sync(FULL, cnt, s) + __shfl_sync(FULL, cnt, 8 + s) > 0 && lane < NR) S.g_rad[NR * s + lane] = grow[rad_col(s) + lane];
@@ -430,7 +431,7 @@ k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
             const float cx = qj.y * qk.z - qj.z * qk.y, cy = qj.z * qk.x - qj.x * qk.z, cz = qj.x * qk.y - qj.y * qk.x;
             const float sn = fast_sqrt(cx * cx + cy * cy + cz * cz);
             const float Rm = 0.5f * (qj.w + qk.w);
-            const float4* gb = reinterpret_cast<const float4*>(&S.g_ang[GP * ipair(S.sp[j], S.sp[k])]);
+            const float4* gb = reinterpret_cast<const float4*>(grow + 32 * ipair(S.sp[j], S.sp[k]));
             float Az[NZ], dAz[NZ];
 #pragma unroll
             for (int z = 0; z < NZ; ++z) {
@@ -442,7 +443,7 @@ k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
             float S0 = 0.f, Sm = 0.f, St = 0.f;
 #pragma unroll
             for (int a = 0; a < NA; ++a) {
-                const float4 g4 = gb[a];
+                const float4 g4 = __ldg(gb + a);
                 const float mm = Rm - K.shf_a[a];
                 const float B = fast_exp2(-K.eta_a_l2e * mm * mm);
                 const float dB = -K.eta_a * mm * B;                                // dB/dR_ij = dB/dR_ik
