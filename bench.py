@@ -35,9 +35,9 @@ METRIC = "ani_energy_forces_atoms_evals_per_s"
 UNIT = "atoms*evals/s"
 NS_PER_DAY_PER_EVAL_PER_S = 0.5e-6 * 86400.0      # 0.5 fs step
 # DRAM bytes (read + write) per launch at configs[3], from the committed ncu --set full captures of this command
-# (profiles/r1e_ncu_full_summary.txt)
-TRAFFIC_98K = {"g1": 0.17065e9 + 0.74989e9, "mid": 0.84655e9 + 0.77066e9, "b1": 0.83645e9 + 0.09575e9,
-               "aev_fwd": 0.02731e9 + 0.05759e9, "aev_bwd": 0.11339e9 + 0.00412e9, "nlist": 0.00235e9 + 0.00077e9 + 0.02705e9 + 0.00006e9}
+# (profiles/r1g_ncu_full_summary.txt)
+TRAFFIC_98K = {"g1": 0.18217e9 + 0.75396e9, "mid": 0.86862e9 + 0.77926e9, "b1": 0.84906e9 + 0.09946e9,
+               "aev_fwd": 0.02731e9 + 0.05850e9, "aev_bwd": 0.11341e9 + 0.00377e9, "nlist": 0.00235e9 + 0.00075e9 + 0.02705e9 + 0.00006e9}
 
 
 def peaks():
@@ -354,7 +354,7 @@ def main():
                         tensor_entry("k_mlp_mid (G2+G3+out+B3+B2 fused: h1 -> E_i, d1)", ph["mlp_mid"], f_mid * M * N, i_mid, tr.get("mid")),
                         tensor_entry("k_gemm_tc<GRAD,N-skip> (B1: d1 -> dE/dAEV) + energy reduction", ph["mlp_b1"], f_b1 * M * N, i_g1, tr.get("b1"))]
         kernels += [hbm_entry("nlist (a1: all kernels)", ph["nlist"], 264.0, tr.get("nlist"), "working set is L2-resident; instruction-bound"),
-                    hbm_entry("k_aev_fwd (a2)", ph["aev_fwd"], 4256.0, tr.get("aev_fwd"), "issue-bound (3.1 k warp instructions per atom)"),
+                    hbm_entry("k_aev_fwd (a2)", ph["aev_fwd"], 4256.0, tr.get("aev_fwd"), "issue-bound (2.6 k warp instructions per atom, 79 % of the issue slots)"),
                     hbm_entry("k_aev_bwd + k_unsort_forces (a5)", ph["aev_bwd"], 4268.0, tr.get("aev_bwd"), "issue-bound")]
         if tensor_path:
             roof = dict(max(kernels[:3], key=lambda k: k["ms_per_launch"]))          # the dominant kernel of the step
