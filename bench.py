@@ -9,10 +9,14 @@ configs[3], the 98 000-atom biosystem the north_star targets are quoted on.  Pri
 
   value   atoms*evals/s, inputs resident in HBM, CUDA events over exactly K steps, max over ranks
   e2e     same metric through dhp_ani_energy_forces_host: pinned host buffers, H2D + D2H inside
-  roofline  the MLP phase (dominant, tensor-bound): algorithmic FLOPs / device time vs measured bf16 peak
+  roofline  the dominant kernel (k_mlp_mid, tensor-bound): algorithmic FLOPs / device time vs measured sustained bf16 peak
+  roofline_mlp_phase / roofline_kernels   the same for the whole MLP phase and for every kernel group (HBM-bound ones vs copy bandwidth)
   cpu_baseline  the fp64 oracle, as it stands, on a bounded sample of the same workload (rank 0, N=1)
+  parity_sample  that oracle sample against dhp_ani_energy_forces_partial over the same central atoms (|dE|/n, max |dF|)
+  energy_only_ms_per_step, md   the energy-only call and the multiple-timestep driver with list reuse, beside the headline
 With N > 1 every rank evaluates its own replica of the system (independent problems, no collective on
-the data path): weak scaling.  --impl reference times the oracle itself.
+the data path): weak scaling; --shard slab decomposes ONE system over the ranks instead (strong scaling).
+--impl reference times the oracle itself.
 """
 from __future__ import annotations
 
