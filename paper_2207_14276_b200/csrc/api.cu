@@ -211,12 +211,12 @@ int dhp_create(dhp_ctx** out, const dhp_params* params, int64_t max_atoms, int64
     {   // everything a hot call needs zeroed (or set to -1) lives in two arenas: two memsets per call instead of eleven
         size_t off = 0;
         auto take = [&](size_t words) { const size_t o = off; off += (words + 3) & ~(size_t)3; return o; };
-        const size_t o_status = take(1), o_sched = take(8), o_tmask = take(R / ROW_TILE), o_bsum = take(N / 64 + 3), o_ccnt = take(NC + 1),
+        const size_t o_status = take(1), o_done = take(1), o_sched = take(8), o_tmask = take(R / ROW_TILE), o_bsum = take(N / 64 + 3), o_ccnt = take(NC + 1),
                      o_cfill = take(NC), o_eatom = take(R), o_fs = take(3 * N);
         c->zero_words = off;
         ok &= dalloc(&c->zero_arena, off) && dalloc(&c->ff_arena, 2 * R);
         if (ok) {
-            c->status = (int*)c->zero_arena + o_status; c->tc_sched = (int*)c->zero_arena + o_sched;
+            c->status = (int*)c->zero_arena + o_status; c->rowkey_done = (int*)c->zero_arena + o_done; c->tc_sched = (int*)c->zero_arena + o_sched;
             c->tile_mask = (unsigned*)c->zero_arena + o_tmask; c->blk_sum = (int*)c->zero_arena + o_bsum;
             c->cell_count = (int*)c->zero_arena + o_ccnt; c->cell_fill = (int*)c->zero_arena + o_cfill;
             c->e_atom = (float*)c->zero_arena + o_eatom; c->fsorted = (float*)c->zero_arena + o_fs;

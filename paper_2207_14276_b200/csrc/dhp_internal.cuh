@@ -147,6 +147,7 @@ struct Ctx {
     int* row_species;      // [max_rows] species of each row (-1 for padding rows)
     int* row_slot;         // [max_rows] sorted slot of each row (-1 for padding)
     int* blk_hist;         // [224 row keys][N/256 + 2] per-block histograms for the stable row assignment (key-major)
+    int* rowkey_done;      // ticket counter of k_rowkey_scan's blocks (in the zero arena)
     int* key_start;        // [224] first row of each (species, feature-block class) key
     unsigned* amask;       // [N] feature blocks the atom's own AEV row can touch (bit b = 64-wide block b)
     unsigned* tile_mask;   // [max_rows / ROW_TILE] bit b: feature block b is non-zero for some row of the tile

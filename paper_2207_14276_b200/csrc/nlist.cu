@@ -263,13 +263,18 @@ k_rowkey_hist(const float4* __restrict__ spos, const unsigned* __restrict__ amas
 
 // single block of 1024 threads, warps take keys round-robin: exclusive scan over blocks per key, then the key starts
 // (species groups aligned to ROW_ALIGN)
+// one block per species, one warp per class key: exclusive scan of the key's counts over the row blocks; the block that
+// finishes last (ticket counter, zeroed with the per-call arena) turns the species totals into the group starts
 __global__ void __launch_bounds__(1024)
 k_rowkey_scan(int* __restrict__ blk_hist, int nrb, int* __restrict__ sp_count, int* __restrict__ sp_start, int* __restrict__ key_start,
-              const int* __restrict__ gate) {
+              int* __restrict__ done, const int* __restrict__ gate) {
     DHP_GATE(gate, 1);
-    __shared__ int tot[NKEY];
+    __shared__ int tot[NCLS];
+    __shared__ int last_s;
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    for (int key = w; key < NKEY; key += 32) {
+    const int s = blockIdx.x;
+    {
+        const int key = s * NCLS + w;
         int* hk = blk_hist + (size_t)key * nrb;
         int run = 0;
         constexpr int CH = 16;                              // 16 x 32 counts are requested at once: one memory latency per
@@ -291,21 +296,41 @@ k_rowkey_scan(int* __restrict__ blk_hist, int nrb, int* __restrict__ sp_count, i
                 run += __shfl_sync(0xffffffffu, x, 31);
             }
         }
-        if (lane == 0) tot[key] = run;
+        if (lane == 0) tot[w] = run;
     }
     __syncthreads();
+    if (w == 0) {                                          // lane = class: offsets of the keys inside the species group
+        const int c = tot[lane];
+        int x = c;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
+        }
+        key_start[s * NCLS + lane] = x - c;
+        if (lane == 31) sp_count[s] = x;
+        __threadfence();                                   // every lane's writes are device-visible before the ticket is taken
+        __syncwarp();
+        if (lane == 31) last_s = atomicAdd(done, 1) == NSP - 1;
+    }
+    __syncthreads();
+    if (!last_s) return;
+    __threadfence();
+    __shared__ int starts[NSP + 1];
     if (threadIdx.x == 0) {
         int start = 0;
-        for (int s = 0; s < NSP; ++s) {
-            sp_start[s] = start;
-            int c = 0;
-            for (int k = 0; k < NCLS; ++k) { key_start[s * NCLS + k] = start + c; c += tot[s * NCLS + k]; }
-            sp_count[s] = c;
+        for (int q = 0; q < NSP; ++q) {
+            starts[q] = start;
+            sp_start[q] = start;
+            const int c = ((volatile int*)sp_count)[q];
             start += (c + ROW_ALIGN - 1) / ROW_ALIGN * ROW_ALIGN;
         }
+        starts[NSP] = start;
         sp_start[NSP] = start;
         sp_count[NSP] = 0;
     }
+    __syncthreads();
+    if (threadIdx.x < NKEY) key_start[threadIdx.x] = ((volatile int*)key_start)[threadIdx.x] + starts[threadIdx.x / NCLS];
 }
 
 __global__ void __launch_bounds__(RB)
@@ -930,7 +955,7 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
     // rows grouped by species, ordered by feature-block class inside a group; tile masks
     const int nrb = (n + RB - 1) / RB;
     DHP_LAUNCH(ctx, k_rowkey_hist, nrb, RB, 0, ctx->spos, ctx->amask, snc, n, nrb, ctx->blk_hist, gate);
-    DHP_LAUNCH(ctx, k_rowkey_scan, 1, 1024, 0, ctx->blk_hist, nrb, ctx->sp_count, ctx->sp_start, ctx->key_start, gate);
+    DHP_LAUNCH(ctx, k_rowkey_scan, NSP, 1024, 0, ctx->blk_hist, nrb, ctx->sp_count, ctx->sp_start, ctx->key_start, ctx->rowkey_done, gate);
     DHP_LAUNCH(ctx, k_rowkey_rank, nrb, RB, 0, ctx->spos, ctx->amask, snc, n, nrb, ctx->blk_hist, ctx->key_start, ctx->rowmap,
                ctx->row_species, ctx->row_slot, ctx->tile_mask, gate);
     DHP_CUDA(ctx, cudaGetLastError());
