@@ -27,17 +27,22 @@ __device__ __forceinline__ float ord2f(unsigned u) {
     return __uint_as_float((u & 0x80000000u) ? (u & 0x7fffffffu) : ~u);
 }
 
-// exclusive scan of n ints by ONE block of 1024 threads; out[n] = total
+// exclusive scan of n ints by ONE block of 1024 threads; out[n] = total.  Every thread takes 8 consecutive elements,
+// so 8192 elements go through one round of warp / block scans (the 6 859 cells of the 98 k box: one round)
 __device__ void block_scan_excl(const int* __restrict__ in, int* __restrict__ out, int n) {
+    constexpr int IPT = 8;
     __shared__ int warp_sums[32];
     __shared__ int carry_s;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     if (tid == 0) carry_s = 0;
     __syncthreads();
-    for (int base = 0; base < n; base += 1024) {
-        int idx = base + tid;
-        int v = idx < n ? in[idx] : 0;
-        int x = v;
+    for (int base = 0; base < n; base += 1024 * IPT) {
+        const int i0 = base + tid * IPT;
+        int v[IPT];
+        int sum = 0;
+#pragma unroll
+        for (int i = 0; i < IPT; ++i) { v[i] = i0 + i < n ? in[i0 + i] : 0; sum += v[i]; }
+        int x = sum;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             int y = __shfl_up_sync(0xffffffffu, x, o);
@@ -55,9 +60,13 @@ __device__ void block_scan_excl(const int* __restrict__ in, int* __restrict__ ou
             warp_sums[lane] = w;
         }
         __syncthreads();
-        int carry = carry_s;
-        int excl = carry + (wid ? warp_sums[wid - 1] : 0) + x - v;
-        if (idx < n) out[idx] = excl;
+        const int carry = carry_s;
+        int run = carry + (wid ? warp_sums[wid - 1] : 0) + x - sum;
+#pragma unroll
+        for (int i = 0; i < IPT; ++i) {
+            if (i0 + i < n) out[i0 + i] = run;
+            run += v[i];
+        }
         __syncthreads();
         if (tid == 1023) carry_s = carry + warp_sums[31];
         __syncthreads();
