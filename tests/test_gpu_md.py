@@ -101,3 +101,37 @@ def test_long_run_rebuilds_when_atoms_leave_the_skin(torch, B, params):
     assert 2 <= nb <= 41
     assert np.abs(x1 - x0).max() <= 1e-4 and abs(E1[0] - E0[0]) / s.n_atoms <= 1e-6
     print(f"rebuilds with skin 0.1 over 40 steps: {nb}; max |x - x0| = {np.abs(x1 - s.pos).max():.3f} A")
+
+
+def test_nve_energy_conservation_and_time_reversal(torch, B, params):
+    """Properties that need no oracle value: the total energy E_ANI + E_bonds + E_kin of an NVE run fluctuates at O(dt^2)
+    (second-order symplectic scheme: halving the timestep must shrink the error about fourfold), and integrating forward,
+    flipping the velocities and integrating the same number of steps returns to the start (to fp32 round-off)."""
+    s = W.make_system(1)
+    blob = W.make_weights(1)
+    md = W.md_inputs(s)
+    d = B.Dhp(s.n_atoms, params=params)
+    w = d.dhp_weights_load(blob, 1)
+    sp = torch.from_numpy(s.species).cuda()
+    h = d.dhp_md_create(md.inv_mass, md.bonds, md.bond_k, md.bond_r0)
+
+    def run(dt, n_outer, pos0, vel0):
+        pos = torch.from_numpy(pos0.copy()).cuda()
+        vel = torch.from_numpy(vel0.copy()).cuda()
+        d.dhp_md_reset(h)
+        E0 = d.dhp_md_run(h, pos, vel, s.box, sp, w, dt, 2, 0).cpu().numpy().sum()
+        worst = 0.0
+        for _ in range(n_outer // 4):
+            E = d.dhp_md_run(h, pos, vel, s.box, sp, w, dt, 2, 4).cpu().numpy().sum()
+            worst = max(worst, abs(E - E0))
+        return worst, pos.cpu().numpy(), vel.cpu().numpy()
+
+    e1, x1, v1 = run(0.2, 40, s.pos, md.vel)            # 8 fs
+    e2, _, _ = run(0.1, 80, s.pos, md.vel)              # the same 8 fs at half the timestep
+    kin0 = M.kinetic_energy(md.vel, md.inv_mass)
+    print(f"NVE water96, 8 fs: max |dE_tot| = {e1:.3e} Ha (dt 0.2 fs), {e2:.3e} Ha (dt 0.1 fs); E_kin(0) = {kin0:.3e} Ha")
+    assert e2 < 0.5 * e1 and e1 < 0.2 * kin0
+    _, x0, v0 = run(0.2, 40, x1, -v1)
+    assert np.abs(x0 - s.pos).max() < 5e-4 and np.abs(v0 + md.vel).max() < 5e-5
+    d.dhp_md_destroy(h)
+    d.close()
