@@ -578,15 +578,8 @@ __device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const CUtensorMap
                  "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [rb];\n\t}"
                  ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar) : "memory");
 }
-__device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity) {
-    asm volatile(
-        "{\n\t.reg .pred P;\n"
-        "WAITC_LOOP:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 P, [%0], %1;\n\t"
-        "@P bra DONEC;\n\t"
-        "bra WAITC_LOOP;\n"
-        "DONEC:\n\t}" ::"r"(bar), "r"(parity) : "memory");
-}
+// (barriers that receive remote arrivals are waited on with the plain mbar_wait: polling with .acquire.cluster cost
+// 0.05 ms per kernel)
 __device__ __forceinline__ void tmem_alloc2(uint32_t smem_dst, uint32_t cols) {
     asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(cols) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
@@ -811,14 +804,14 @@ k_gemm_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
                     int bn = p.BN;
                     if (CMP == CMP_N) bn = KBLK * min(4, __popc(pair_mask(pr)) - 4 * nt);
                     const uint32_t idesc = make_idesc2(bn);
-                    mbar_wait_cluster(tempty_bar(acc), acc_phase ^ 1u);
+                    mbar_wait(tempty_bar(acc), acc_phase ^ 1u);
                     tc_fence_after();
                     const uint32_t d_tmem = tmem_base + (uint32_t)(acc * ACC_STRIDE);
                     uint32_t accumulate = 0u;
                     for (unsigned km = k_mask(pr); km; km &= km - 1u) {
                         const int kb = __ffs(km) - 1;
                         mbar_wait(full_bar(stage), phase);
-                        if (!DIRECT) mbar_wait_cluster(pfull_bar(stage), phase);
+                        if (!DIRECT) mbar_wait(pfull_bar(stage), phase);
                         tc_fence_after();
                         const uint32_t sa = base + stage * P_STAGE_BYTES;
                         const bool tiled = p.a_tiled != nullptr;
