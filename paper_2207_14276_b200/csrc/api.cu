@@ -182,6 +182,7 @@ int dhp_create(dhp_ctx** out, const dhp_params* params, int64_t max_atoms, int64
     cudaDeviceProp prop;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) { delete h; return DHP_E_CUDA; }
     c->sm_count = prop.multiProcessorCount;
+    { const char* e = getenv("DHP_NO_SMALL_PATH"); c->no_small_path = e && e[0] == '1'; }
     { const char* e = getenv("DHP_TC_PAIRS"); c->tc_pairs = (e && e[0] >= '0' && e[0] <= '3') ? e[0] - '0' : 0; }   // cta_group::2 kernels
     c->cc_major = prop.major;
     c->max_atoms = max_atoms;

@@ -89,6 +89,7 @@ struct Ctx {
     int64_t max_atoms, max_mols, max_rows, max_cells, pair_cap;
     int sm_count, cc_major;
     int mlp_mode;
+    bool no_small_path;    // DHP_NO_SMALL_PATH=1 at dhp_create: small systems also take the general (cell list) path (tests)
     int tc_pairs;          // bit 0: G1, bit 1: B1 run on CTA pairs (tcgen05 cta_group::2); DHP_TC_PAIRS=<bits> in the environment
                            // at dhp_create overrides the default
     int64_t launches;

@@ -606,10 +606,91 @@ __global__ void k_scan_blocks(const int* __restrict__ blk_sum, int* __restrict__
     }
 }
 
+constexpr int MAX_STRIDE_CHUNKS = 6;    // tmp_stride <= 192
+
+// one row of the pair list, by one warp: the ni unordered entries at src (pass-1 format) are ordered by (angular first,
+// then radial-only) x neighbour species into col[row_start ..), the 14 run lengths, the angular count and the
+// feature-block mask of the atom are stored; with reuse_rows the tile mask of the atom's (kept) row is refreshed too.
+// sg: 16 ints of shared memory private to the warp.
+__device__ __forceinline__ void order_row(const unsigned* __restrict__ src, int ni, int row_start, int i, int lane, int* sg,
+                                          int* __restrict__ col, int* __restrict__ n_ang, unsigned short* __restrict__ seg_cnt,
+                                          unsigned* __restrict__ amask, bool reuse_rows, const int* __restrict__ rowmap,
+                                          unsigned* __restrict__ tile_mask) {
+    const unsigned lt = (1u << lane) - 1u;
+    unsigned e[MAX_STRIDE_CHUNKS];
+#pragma unroll
+    for (int k = 0; k < MAX_STRIDE_CHUNKS; ++k) e[k] = (k * 32 + lane < ni) ? src[k * 32 + lane] : 0xffffffffu;
+    if (lane < 16) sg[lane] = 0;
+    __syncwarp();
+    // counts per key = class * 8 + species (class 0: angular, 1: radial-only); 15 = no entry
+#pragma unroll
+    for (int k = 0; k < MAX_STRIDE_CHUNKS; ++k) {
+        if (k * 32 < ni) {
+            const int key = (e[k] == 0xffffffffu) ? 15 : (int)((e[k] >> 28) & 15u);
+            const unsigned m = __match_any_sync(0xffffffffu, key);
+            if ((m & lt) == 0) sg[key] += __popc(m);      // group leader; keys are distinct across leaders
+            __syncwarp();
+        }
+    }
+    // lane k < 16 owns key k: exclusive prefix over keys -> segment starts
+    int cnt_k = lane < 16 ? sg[lane] : 0;
+    if (lane == 15 || lane == 7) cnt_k = 0;
+    {   // which 64-wide feature blocks of this row's AEV can be non-zero (internal column order, dhp_internal.cuh)
+        const unsigned has1 = __ballot_sync(0xffffffffu, cnt_k > 0), has2 = __ballot_sync(0xffffffffu, cnt_k > 1);
+        const unsigned am = has1 & 0x7fu, am2 = has2 & 0x7fu, rm = (am | (has1 >> 8)) & 0x7fu;
+        bool pp = false;
+        if (lane < NPAIR) {                                   // lane = internal pair index
+            int hi = 0;
+            while ((hi + 1) * (hi + 2) / 2 <= lane) ++hi;
+            const int sa = prio_sp(lane - hi * (hi + 1) / 2), sb = prio_sp(hi);
+            pp = (sa == sb) ? ((am2 >> sa) & 1u) != 0 : (((am >> sa) & (am >> sb)) & 1u) != 0;
+        }
+        const unsigned pm = __ballot_sync(0xffffffffu, pp);
+        const bool bb = lane < 14 ? ((pm >> (2 * lane)) & 3u) != 0 : lane == 14 ? (rm & 0x0fu) != 0 : lane == 15 ? (rm & 0x70u) != 0 : false;
+        const unsigned bmask = __ballot_sync(0xffffffffu, bb);
+        if (lane == 0) {
+            amask[i] = bmask;
+            if (reuse_rows && bmask) {
+                const int row = rowmap[i];
+                if (row >= 0) { atomicOr(&tile_mask[(row / ROW_TILE) & ~1], bmask); atomicOr(&tile_mask[(row / ROW_TILE) | 1], bmask); }
+            }
+        }
+    }
+    int x = cnt_k;
+#pragma unroll
+    for (int o = 1; o < 16; o <<= 1) {
+        int y = __shfl_up_sync(0xffffffffu, x, o);
+        if (lane >= o) x += y;
+    }
+    const int na = __shfl_sync(0xffffffffu, x, 7);
+    if (lane < 16) {
+        int v = cnt_k;
+        if (lane == 7) v = na;
+        if (lane == 15) v = ni - na;
+        seg_cnt[(size_t)i * 16 + lane] = (unsigned short)v;
+    }
+    if (lane == 0) n_ang[i] = na;
+    __syncwarp();
+    if (lane < 16) sg[lane] = row_start + x - cnt_k;
+    __syncwarp();
+#pragma unroll
+    for (int k = 0; k < MAX_STRIDE_CHUNKS; ++k) {
+        if (k * 32 < ni) {
+            const int key = (e[k] == 0xffffffffu) ? 15 : (int)((e[k] >> 28) & 15u);
+            const unsigned m = __match_any_sync(0xffffffffu, key);
+            const int base = sg[key];
+            if (key != 15) col[base + __popc(m & lt)] = (int)(e[k] & 0x0fffffffu);
+            __syncwarp();
+            if ((m & lt) == 0) sg[key] = base + __popc(m);
+            __syncwarp();
+        }
+    }
+
+}
+
 // pass 2: ROWS_PER_BLK atoms per block; rows get their CSR offsets, entries are ordered by (angular first, then
 // radial-only) x neighbour species, and the 14 segment sizes of every row are stored for the AEV kernels.
 constexpr int P2_THREADS = 256;
-constexpr int MAX_STRIDE_CHUNKS = 6;    // tmp_stride <= 192
 
 __global__ void __launch_bounds__(P2_THREADS)
 k_rows(const unsigned* __restrict__ tmp, int stride, const int* __restrict__ cnt, const int* __restrict__ blk_off, int nblk,
@@ -651,84 +732,13 @@ k_rows(const unsigned* __restrict__ tmp, int stride, const int* __restrict__ cnt
     }
     __syncthreads();
 
-    const unsigned lt = (1u << lane) - 1u;
     int* sg = segs[warp];
     for (int q = warp; q < ROWS_PER_BLK; q += P2_THREADS / 32) {
         const int i = i0 + q;
         if (i >= n) break;
-        const int ni = rcnt[q];
-        const unsigned* src = tmp + (size_t)i * stride;
-        unsigned e[MAX_STRIDE_CHUNKS];
-#pragma unroll
-        for (int k = 0; k < MAX_STRIDE_CHUNKS; ++k) e[k] = (k * 32 + lane < ni) ? src[k * 32 + lane] : 0xffffffffu;
-        if (lane < 16) sg[lane] = 0;
-        __syncwarp();
-        // counts per key = class * 8 + species (class 0: angular, 1: radial-only); 15 = no entry
-#pragma unroll
-        for (int k = 0; k < MAX_STRIDE_CHUNKS; ++k) {
-            if (k * 32 < ni) {
-                const int key = (e[k] == 0xffffffffu) ? 15 : (int)((e[k] >> 28) & 15u);
-                const unsigned m = __match_any_sync(0xffffffffu, key);
-                if ((m & lt) == 0) sg[key] += __popc(m);      // group leader; keys are distinct across leaders
-                __syncwarp();
-            }
-        }
-        // lane k < 16 owns key k: exclusive prefix over keys -> segment starts
-        int cnt_k = lane < 16 ? sg[lane] : 0;
-        if (lane == 15 || lane == 7) cnt_k = 0;
-        {   // which 64-wide feature blocks of this row's AEV can be non-zero (internal column order, dhp_internal.cuh)
-            const unsigned has1 = __ballot_sync(0xffffffffu, cnt_k > 0), has2 = __ballot_sync(0xffffffffu, cnt_k > 1);
-            const unsigned am = has1 & 0x7fu, am2 = has2 & 0x7fu, rm = (am | (has1 >> 8)) & 0x7fu;
-            bool pp = false;
-            if (lane < NPAIR) {                                   // lane = internal pair index
-                int hi = 0;
-                while ((hi + 1) * (hi + 2) / 2 <= lane) ++hi;
-                const int sa = prio_sp(lane - hi * (hi + 1) / 2), sb = prio_sp(hi);
-                pp = (sa == sb) ? ((am2 >> sa) & 1u) != 0 : (((am >> sa) & (am >> sb)) & 1u) != 0;
-            }
-            const unsigned pm = __ballot_sync(0xffffffffu, pp);
-            const bool bb = lane < 14 ? ((pm >> (2 * lane)) & 3u) != 0 : lane == 14 ? (rm & 0x0fu) != 0 : lane == 15 ? (rm & 0x70u) != 0 : false;
-            const unsigned bmask = __ballot_sync(0xffffffffu, bb);
-            if (lane == 0) {
-                amask[i] = bmask;
-                if (reuse_rows && bmask) {
-                    const int row = rowmap[i];
-                    if (row >= 0) { atomicOr(&tile_mask[(row / ROW_TILE) & ~1], bmask); atomicOr(&tile_mask[(row / ROW_TILE) | 1], bmask); }
-                }
-            }
-        }
-        int x = cnt_k;
-#pragma unroll
-        for (int o = 1; o < 16; o <<= 1) {
-            int y = __shfl_up_sync(0xffffffffu, x, o);
-            if (lane >= o) x += y;
-        }
-        const int na = __shfl_sync(0xffffffffu, x, 7);
-        if (lane < 16) {
-            int v = cnt_k;
-            if (lane == 7) v = na;
-            if (lane == 15) v = ni - na;
-            seg_cnt[(size_t)i * 16 + lane] = (unsigned short)v;
-        }
-        if (lane == 0) n_ang[i] = na;
-        __syncwarp();
-        if (lane < 16) sg[lane] = rstart[q] + x - cnt_k;
-        __syncwarp();
-#pragma unroll
-        for (int k = 0; k < MAX_STRIDE_CHUNKS; ++k) {
-            if (k * 32 < ni) {
-                const int key = (e[k] == 0xffffffffu) ? 15 : (int)((e[k] >> 28) & 15u);
-                const unsigned m = __match_any_sync(0xffffffffu, key);
-                const int base = sg[key];
-                if (key != 15) col[base + __popc(m & lt)] = (int)(e[k] & 0x0fffffffu);
-                __syncwarp();
-                if ((m & lt) == 0) sg[key] = base + __popc(m);
-                __syncwarp();
-            }
-        }
+        order_row(tmp + (size_t)i * stride, rcnt[q], rstart[q], i, lane, sg, col, n_ang, seg_cnt, amask, reuse_rows, rowmap, tile_mask);
     }
 }
-
 
 // ---------------------------------------------------------------------------------------------
 // Verlet-skin reuse ("atomic positions do not move much between two time-steps").
@@ -857,6 +867,162 @@ k_refilter(const float4* __restrict__ spos, const __grid_constant__ BoxArg bx, c
 }
 
 // ---------------------------------------------------------------------------------------------
+// Small systems (n <= SMALL_N; the hybrid scheme's solute, BASELINE.json configs[0]-[1]): the whole of a1 in ONE block.
+// Thirteen launches with 3-15 us floors cost ~90 us for 50 atoms; here the atoms stay in the caller's order (perm =
+// identity), every pair is tested (fp32 with the error margin of k_refilter, the canonical fp64 predicate inside it: the
+// list is the same bit-exact list), rows are ordered by order_row() and the species-grouped, class-ordered row
+// assignment is a stable count over at most SMALL_N keys in shared memory.
+// ---------------------------------------------------------------------------------------------
+constexpr int SMALL_N = 320;      // above ~300 atoms one SM is slower than the thirteen small launches of the general path
+constexpr int SMALL_THREADS = 1024;
+
+__global__ void __launch_bounds__(SMALL_THREADS)
+k_nlist_small(const float* __restrict__ pos, const int* __restrict__ species, int n, const int* __restrict__ mol_offsets, int n_mol,
+              const uint8_t* __restrict__ central, int periodic, double Lx, double Ly, double Lz, double rcr2, double rca2, int stride,
+              int64_t pair_cap, Grid* __restrict__ grid, int* __restrict__ status, int* __restrict__ perm, int* __restrict__ inv_perm,
+              float4* __restrict__ spos, int* __restrict__ smol, unsigned char* __restrict__ snc, unsigned* __restrict__ tmp,
+              int* __restrict__ n_rad, int* __restrict__ n_ang, int* __restrict__ row_ptr, int* __restrict__ col,
+              unsigned short* __restrict__ seg_cnt, unsigned* __restrict__ amask, int* __restrict__ sp_count, int* __restrict__ sp_start,
+              int* __restrict__ rowmap, int* __restrict__ row_species, int* __restrict__ row_slot, unsigned* __restrict__ tile_mask) {
+    __shared__ Grid g;
+    __shared__ float4 sp4[SMALL_N];
+    __shared__ int mol_s[SMALL_N];
+    __shared__ short key_s[SMALL_N];
+    __shared__ unsigned char nc_s[SMALL_N];
+    __shared__ int segs[SMALL_THREADS / 32][16];
+    __shared__ int tot_s[NKEY], kstart_s[NKEY];
+    __shared__ int ovf_s;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const bool by_mol = mol_offsets != nullptr && n_mol > 0;
+    // ---- phase 0: grid description (what the AEV kernels read), atoms in the caller's order
+    if (tid == 0) {
+        const double L[3] = {Lx, Ly, Lz};
+        g.periodic = periodic; g.by_molecule = by_mol ? 1 : 0; g.ncell = 1;
+        for (int c = 0; c < 3; ++c) {
+            g.L[c] = periodic ? L[c] : 0.0; g.origin[c] = 0.0; g.inv_cell[c] = 0.0; g.nc[c] = 1; g.edge[c] = 0.0;
+            g.inv_L[c] = periodic ? 1.0 / L[c] : 0.0; g.wrap[c] = periodic ? 1 : 0;
+            g.Lf[c] = (float)L[c]; g.inv_Lf[c] = periodic ? (float)(1.0 / L[c]) : 0.f;
+        }
+        *grid = g;
+        ovf_s = 0;
+    }
+    for (int k = tid; k < NKEY; k += SMALL_THREADS) tot_s[k] = 0;
+    if (tid < n) {
+        int s = species[tid];
+        if (s < 0 || s >= NSP) atomicExch(status, DHP_E_SPECIES);
+        s = min(max(s, 0), NSP - 1);
+        const float4 p4 = make_float4(pos[3 * tid], pos[3 * tid + 1], pos[3 * tid + 2], __int_as_float(s));
+        int m = 0;
+        if (by_mol) {
+            int lo = 0, hi = n_mol;            // largest m with mol_offsets[m] <= tid
+            while (hi - lo > 1) {
+                const int mid = (lo + hi) >> 1;
+                if (mol_offsets[mid] <= tid) lo = mid; else hi = mid;
+            }
+            m = lo;
+        }
+        const unsigned char nc = central ? (central[tid] ? 0 : 1) : 0;
+        sp4[tid] = p4; mol_s[tid] = m; nc_s[tid] = nc;
+        spos[tid] = p4; smol[tid] = m; snc[tid] = nc; perm[tid] = tid; inv_perm[tid] = tid;
+    }
+    __syncthreads();
+    // ---- phase 1: all pairs of a row by one warp -> unordered entries (pass-1 format), counts
+    {
+        const float rcr2f = (float)rcr2, rca2f = (float)rca2;
+        const float rcr = sqrtf(rcr2f), rca = sqrtf(rca2f);
+        const float kr = 2.0f * 2.0f * rcr * 3.0f * 5.9604645e-08f, ka = 2.0f * 2.0f * rca * 3.0f * 5.9604645e-08f;
+        const float mr0 = 2.0f * rcr2f * 2.3841858e-07f, ma0 = 2.0f * rca2f * 2.3841858e-07f;
+        const float Lfx = g.Lf[0], Lfy = g.Lf[1], Lfz = g.Lf[2], iLx = g.inv_Lf[0], iLy = g.inv_Lf[1], iLz = g.inv_Lf[2];
+        const unsigned lt = (1u << lane) - 1u;
+        for (int i = warp; i < n; i += SMALL_THREADS / 32) {
+            int base = 0;
+            if (!nc_s[i]) {
+                const float4 pi = sp4[i];
+                const int mi = mol_s[i];
+                for (int c0 = 0; c0 < n; c0 += 32) {
+                    const int j = c0 + lane;
+                    const bool have = j < n && j != i && mol_s[min(j, n - 1)] == mi;
+                    const float4 pj = sp4[min(j, n - 1)];
+                    float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+                    const float dm = fmaxf(fabsf(dx), fmaxf(fabsf(dy), fabsf(dz)));
+                    if (periodic) { dx -= Lfx * rintf(dx * iLx); dy -= Lfy * rintf(dy * iLy); dz -= Lfz * rintf(dz * iLz); }
+                    const float r2 = dx * dx + dy * dy + dz * dz;
+                    bool in_r = have && r2 <= rcr2f;
+                    bool in_a = have && r2 <= rca2f;
+                    if (have && (fabsf(r2 - rcr2f) <= fmaf(kr, dm, mr0) || fabsf(r2 - rca2f) <= fmaf(ka, dm, ma0))) {
+                        const double r2d = pair_r2(pi, pj, g);
+                        in_r = r2d <= rcr2;
+                        in_a = r2d <= rca2;
+                    }
+                    const unsigned m = __ballot_sync(0xffffffffu, in_r);
+                    if (in_r) {
+                        const int o = base + __popc(m & lt);
+                        if (o < stride) tmp[(size_t)i * stride + o] = (unsigned)j | ((unsigned)__float_as_int(pj.w) << 28) | (in_a ? 0u : ENT_RADIAL_ONLY);
+                    }
+                    base += __popc(m);
+                }
+            }
+            if (lane == 0) {
+                if (base > stride) { atomicExch(status, DHP_E_CAPACITY); base = stride; }
+                n_rad[i] = base;
+            }
+        }
+    }
+    __syncthreads();
+    // ---- phase 2: CSR offsets
+    block_scan_excl(n_rad, row_ptr, n);
+    __syncthreads();
+    if (tid == 0 && (row_ptr[n] < 0 || (int64_t)row_ptr[n] > pair_cap)) { atomicExch(status, DHP_E_CAPACITY); ovf_s = 1; }
+    __syncthreads();
+    if (ovf_s) {                                            // neighbour storage overflow: an empty list, as in the general path
+        for (int a = tid; a <= n; a += SMALL_THREADS) { row_ptr[a] = 0; if (a < n) n_rad[a] = 0; }
+        __syncthreads();
+    }
+    // ---- phase 3: order every row, run lengths, feature-block masks
+    for (int i = warp; i < n; i += SMALL_THREADS / 32)
+        order_row(tmp + (size_t)i * stride, n_rad[i], row_ptr[i], i, lane, segs[warp], col, n_ang, seg_cnt, amask, false, nullptr, nullptr);
+    __syncthreads();
+    // ---- phase 4: species-grouped, class-ordered rows (stable in atom order), tile masks
+    int key = -1, sp = 0;
+    unsigned am = 0;
+    if (tid < n && !nc_s[tid]) { sp = __float_as_int(sp4[tid].w); am = amask[tid]; key = row_key(sp, am); }
+    if (tid < n) key_s[tid] = (short)key;
+    __syncthreads();
+    int rank = 0;
+    if (key >= 0) {
+        int same = 0;
+        for (int b = 0; b < n; ++b) {
+            const bool eq = key_s[b] == (short)key;
+            same += eq;
+            rank += eq && b < tid;
+        }
+        if (rank == 0) tot_s[key] = same;
+    }
+    __syncthreads();
+    if (tid == 0) {
+        int start = 0;
+        for (int s = 0; s < NSP; ++s) {
+            sp_start[s] = start;
+            int c = 0;
+            for (int k = 0; k < NCLS; ++k) { kstart_s[s * NCLS + k] = start + c; c += tot_s[s * NCLS + k]; }
+            sp_count[s] = c;
+            start += (c + ROW_ALIGN - 1) / ROW_ALIGN * ROW_ALIGN;
+        }
+        sp_start[NSP] = start;
+        sp_count[NSP] = 0;
+    }
+    __syncthreads();
+    if (tid < n) {
+        if (key < 0) { rowmap[tid] = -1; return; }
+        const int row = kstart_s[key] + rank;
+        rowmap[tid] = row;
+        row_species[row] = sp;
+        row_slot[row] = tid;
+        if (am) { atomicOr(&tile_mask[(row / ROW_TILE) & ~1], am); atomicOr(&tile_mask[(row / ROW_TILE) | 1], am); }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------
 int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t* species, int64_t n64,
@@ -892,6 +1058,14 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
     }
     double L[3] = {0, 0, 0};
     if (periodic) for (int c = 0; c < 3; ++c) L[c] = (double)box_host[c];
+    if (!skin && n <= SMALL_N && !ctx->no_small_path) {          // small systems: the whole of a1 in one block
+        DHP_LAUNCH(ctx, k_nlist_small, 1, SMALL_THREADS, 0, pos, species, n, mol_offsets, by_mol ? n_mol : 0, central, periodic ? 1 : 0,
+                   L[0], L[1], L[2], rcr * rcr, rca * rca, ctx->tmp_stride, ctx->pair_cap, ctx->grid, ctx->status, ctx->perm, ctx->inv_perm,
+                   ctx->spos, ctx->smol, ctx->snc, ctx->tmp_col, ctx->n_rad, ctx->n_ang, ctx->row_ptr, ctx->col, ctx->seg_cnt, ctx->amask,
+                   ctx->sp_count, ctx->sp_start, ctx->rowmap, ctx->row_species, ctx->row_slot, ctx->tile_mask);
+        DHP_CUDA(ctx, cudaGetLastError());
+        return DHP_OK;
+    }
     const int nb = (n + 255) / 256;
     if (skin) {
         // reuse is possible only for the same problem (size, box, molecule table, masked or not); whether the atoms

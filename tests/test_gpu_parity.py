@@ -74,6 +74,32 @@ def test_pair_lists_bit_exact_small(torch, B, params, name):
     d.close()
 
 
+@pytest.mark.parametrize("name", ["water96", "ligand50", "replicas16"])
+def test_small_systems_through_the_general_path(torch, B, params, blob8, name, monkeypatch):
+    """Systems of <= 320 atoms normally take the single-block list build; DHP_NO_SMALL_PATH=1 sends them through the
+    cell-list kernels instead, which keeps those kernels' small-box branches under test: two cells per periodic edge with
+    the per-pair minimum image (water96), the bounding-box grid of open boundaries (ligand50), one cell per molecule
+    (replicas16).  Lists bit-exact, energies and forces inside the bars, on both paths."""
+    monkeypatch.setenv("DHP_NO_SMALL_PATH", "1")
+    s = SYSTEMS[name]()
+    d = make_ctx(B, s, params)
+    pos, sp, mol = B.to_device(s)
+    d.dhp_nlist_build(pos, s.box, sp, mol)
+    assert d.dhp_status() == 0
+    rp, col, rpa, cola = d.dhp_nlist_export()
+    rpo, colo = oracle.pairs(s.pos, s.box, params.rcr, s.mol_offsets)
+    assert csr_equal(rp, col, rpo, colo)
+    rpo, colo = oracle.pairs(s.pos, s.box, params.rca, s.mol_offsets)
+    assert csr_equal(rpa, cola, rpo, colo)
+    d.close()
+    d, E, F = run_gpu(B, torch, s, params, blob8, B.MLP_TENSOR if make_ctx(B, s, params).dhp_tensor_path_available() else B.MLP_SIMT)
+    Eo, Fo = oracle.total_energy_forces(s, params, blob8[: s.n_models * 7 * W.PARAMS_PER_NET])
+    per = s.n_atoms if s.mol_offsets is None else np.diff(s.mol_offsets)
+    assert np.max(np.abs(E - Eo) / per) <= E_TOL_PER_ATOM
+    assert np.max(np.abs(F - Fo)) <= F_TOL
+    d.close()
+
+
 @pytest.mark.parametrize("cfg", [3, 5, 4])
 def test_pair_lists_bit_exact_full_size(torch, B, params, cfg):
     s = W.make_system(cfg)
