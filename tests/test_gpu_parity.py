@@ -92,7 +92,7 @@ def test_small_systems_through_the_general_path(torch, B, params, blob8, name, m
     rpo, colo = oracle.pairs(s.pos, s.box, params.rca, s.mol_offsets)
     assert csr_equal(rpa, cola, rpo, colo)
     d.close()
-    d, E, F = run_gpu(B, torch, s, params, blob8, B.MLP_TENSOR if make_ctx(B, s, params).dhp_tensor_path_available() else B.MLP_SIMT)
+    d, E, F = run_gpu(B, torch, s, params, blob8)              # AUTO: tensor path on B200
     Eo, Fo = oracle.total_energy_forces(s, params, blob8[: s.n_models * 7 * W.PARAMS_PER_NET])
     per = s.n_atoms if s.mol_offsets is None else np.diff(s.mol_offsets)
     assert np.max(np.abs(E - Eo) / per) <= E_TOL_PER_ATOM
