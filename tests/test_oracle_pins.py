@@ -383,6 +383,30 @@ def test_partial_centres_give_exact_forces_on_interior_atom(params):
     assert np.allclose(Fa[a], F[a], atol=1e-13)
 
 
+def test_partial_centres_are_additive_and_local(params):
+    """Eq. 2: E is a sum of atomic terms, so the oracle restricted to a subset of central atoms - the
+    ground truth of the partial-evaluation (multi-GPU) tests - must be additive over any partition of the atoms, give the
+    same atomic energies as the full evaluation, and a single centre may push only itself and its neighbours."""
+    s = W.small_periodic_mix(300, 15.0, seed=3, n_models=1)
+    blob = W.make_weights(1)
+    E, F, _ = oracle.energy_forces(s.pos, s.species, s.box, params, blob, 1)
+    rng = np.random.default_rng(1)
+    owner = rng.integers(0, 3, s.n_atoms)
+    Esum, Fsum = 0.0, np.zeros_like(F)
+    for r in range(3):
+        c = np.nonzero(owner == r)[0].astype(np.int32)
+        Ec, Fc, _ = oracle.energy_forces(s.pos, s.species, s.box, params, blob, 1, centres=c)
+        assert np.allclose(Ec, E[c], atol=1e-14)                 # the same atomic energies, centre by centre
+        Esum += Ec.sum()
+        Fsum += Fc
+    assert abs(Esum - E.sum()) < 1e-11 and np.abs(Fsum - F).max() < 1e-12
+    rp, col = oracle.pairs(s.pos, s.box, 5.1)
+    _, F1, _ = oracle.energy_forces(s.pos, s.species, s.box, params, blob, 1, centres=np.array([42], np.int32))
+    touched = set(np.nonzero(np.abs(F1).sum(1))[0])
+    assert touched <= set(col[rp[42]:rp[43]]) | {42}
+    assert np.abs(F1.sum(0)).max() < 1e-13                       # Newton's third law holds centre by centre
+
+
 def test_batched_molecules_are_independent(params):
     s = W.replicas_1024x30(n_mol=4)
     blob = W.make_weights(8)
