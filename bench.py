@@ -13,7 +13,8 @@ configs[3], the 98 000-atom biosystem the north_star targets are quoted on.  Pri
   roofline_mlp_phase / roofline_kernels   the same for the whole MLP phase and for every kernel group (HBM-bound ones vs copy bandwidth)
   cpu_baseline  the fp64 oracle, as it stands, on a bounded sample of the same workload (rank 0, N=1)
   parity_sample  that oracle sample against dhp_ani_energy_forces_partial over the same central atoms (|dE|/n, max |dF|)
-  energy_only_ms_per_step, md   the energy-only call and the multiple-timestep driver with list reuse, beside the headline
+  energy_only_ms_per_step, md, sustained   the energy-only call, the multiple-timestep driver with list reuse, and the same
+                loop run for ~1 s (power-capped steady state) with its clocks, beside the headline
 With N > 1 every rank evaluates its own replica of the system (independent problems, no collective on
 the data path): weak scaling; --shard slab decomposes ONE system over the ranks instead (strong scaling).
 --impl reference times the oracle itself.
@@ -56,7 +57,7 @@ def peaks():
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
     Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
-        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap,power.draw"
 
     def __init__(self, index: int):
         self.index, self.rows, self.proc = index, [], None
@@ -87,6 +88,8 @@ class ClockSampler:
         mx = [float(r[1]) for r in self.rows if len(r) >= 6 and r[1].replace(".", "").isdigit()]
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         reasons = sorted({names[i] for r in self.rows if len(r) >= 6 for i in range(4) if r[2 + i].lower().startswith("active")})
+        pw = [float(r[6]) for r in self.rows if len(r) >= 7 and r[6].replace(".", "").isdigit()]
+        self.power_w = float(max(pw)) if pw else None           # peak board power seen while sampling
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
                 "reasons": reasons, "samples": len(sm)}
 
@@ -168,6 +171,7 @@ def main():
                          "'slab' = ONE system, central atoms partitioned into spatial slabs, partial E / F summed over NCCL (strong scaling)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-md", action="store_true", help="skip the multiple-timestep driver measurement")
+    ap.add_argument("--no-sustained", action="store_true", help="skip the ~1 s sustained-rate loop")
     ap.add_argument("--md-steps", type=int, default=40)
     ap.add_argument("--skin", type=float, default=1.0, help="Verlet skin (A) of the MD measurement")
     args = ap.parse_args()
@@ -255,6 +259,26 @@ def main():
     n_row_tiles, n_active_blocks = d.dhp_debug_tile_blocks()
     clocks = sampler.stop() if rank == 0 else None
     assert d.dhp_status() == 0
+
+    # ---- sustained rate: the same loop for ~1 s, long enough for the board's power management to settle (the 20-step
+    # headline is a 50 ms burst); reported beside the headline with the clocks and power sampled during it -------------
+    sustained = None
+    if not args.no_sustained:
+        n_sus = max(args.steps, int(1000.0 / max(ms_total / args.steps, 1e-3)))
+        s2 = ClockSampler(local)
+        if rank == 0:
+            s2.start()
+        barrier()
+        ev0.record(stream)
+        for k in range(n_sus):
+            step(k)
+        ev1.record(stream)
+        barrier()
+        ms_sus = ev0.elapsed_time(ev1) / n_sus
+        if rank == 0:
+            c2 = s2.stop()
+            sustained = {"ms_per_step": ms_sus, "steps": n_sus, "sm_mhz": c2["sm_mhz"], "reasons": c2["reasons"],
+                         "power_w": getattr(s2, "power_w", None), "samples": c2.get("samples")}
 
     # ---- energy-only call (a1-a3), same inputs, device-resident ---------------------------------
     for k in range(3):
@@ -405,7 +429,7 @@ def main():
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "ms_per_step": e2e_ms / args.steps},
-            "energy_only_ms_per_step": ms_energy_only, "md": md_out,
+            "energy_only_ms_per_step": ms_energy_only, "md": md_out, "sustained": sustained,
             "roofline": roof,
             "roofline_mlp_phase": mlp_phase,
             "roofline_kernels": kernels,
