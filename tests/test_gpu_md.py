@@ -135,3 +135,33 @@ def test_nve_energy_conservation_and_time_reversal(torch, B, params):
     assert np.abs(x0 - s.pos).max() < 5e-4 and np.abs(v0 + md.vel).max() < 5e-5
     d.dhp_md_destroy(h)
     d.close()
+
+
+def test_argument_errors_of_the_driver_and_the_skin(torch, B, params):
+    s = W.make_system(1)
+    md = W.md_inputs(s)
+    d = B.Dhp(s.n_atoms, params=params)
+    w = d.dhp_weights_load(W.make_weights(1), 1)
+    for bad in (-0.1, 4.5, float("nan")):
+        with pytest.raises(B.DhpError, match="-1"):
+            d.dhp_set_skin(bad)
+    with pytest.raises(B.DhpError, match="-2"):                       # more atoms than the context holds
+        d.dhp_md_create(np.ones(s.n_atoms + 1, np.float32))
+    with pytest.raises(B.DhpError, match="-1"):                       # bonds without force constants
+        import ctypes as C
+        h = C.c_void_p()
+        rc = d.lib.dhp_md_create(d.ctx, s.n_atoms, C.c_void_p(md.inv_mass.ctypes.data), C.c_void_p(md.bonds.ctypes.data), None, None,
+                                 len(md.bonds), C.byref(h))
+        B._check(rc, d.ctx)
+    h = d.dhp_md_create(md.inv_mass, md.bonds, md.bond_k, md.bond_r0)
+    pos = torch.from_numpy(s.pos.copy()).cuda()
+    vel = torch.from_numpy(md.vel.copy()).cuda()
+    sp = torch.from_numpy(s.species).cuda()
+    for dt, n_inner, n_steps in ((0.0, 1, 1), (0.5, 0, 1), (0.5, 1, -1)):
+        with pytest.raises(B.DhpError, match="-1"):
+            d.dhp_md_run(h, pos, vel, s.box, sp, w, dt, n_inner, n_steps)
+    E = d.dhp_md_run(h, pos, vel, s.box, sp, w, 0.5, 1, 0)            # zero steps: energies of the initial state
+    torch.cuda.synchronize()
+    assert np.isfinite(E.cpu().numpy()).all() and np.array_equal(pos.cpu().numpy(), s.pos)
+    d.dhp_md_destroy(h)
+    d.close()
