@@ -79,9 +79,10 @@ constexpr int TP = 36;          // pitch of the staged factor rows: 16-byte alig
 struct __align__(16) WarpSmemFwd {
     float4 nb[MAX_ANG];          // ux, uy, uz, R of the angular neighbours
     float fca[MAX_ANG];          // f_c(R; Rca)
-    float2 rr[MAX_RAD];          // all neighbours: R, f_c(R; Rcr)
-    float tA[NZ][TP];
-    float tB[NA][TP];
+    union {                      // the radial part is finished before the first angular round is staged: same bytes
+        float2 rr[MAX_RAD];      // all neighbours: R, f_c(R; Rcr)
+        struct { float tA[NZ][TP]; float tB[NA][TP]; } st;
+    };
     int4 tab[NPAIR + 1];         // non-empty species pairs in slot order: first slot, j0 | k0 << 8 | nk << 16 | same << 24,
                                  // triplets, angular block; terminated by {total slots, ...}
 };
@@ -97,7 +98,7 @@ __device__ __forceinline__ void put_feature(float v, float* __restrict__ row_f32
 }
 
 template <bool PLANES>
-__global__ void __launch_bounds__(AEV_WARPS * 32)
+__global__ void __launch_bounds__(AEV_WARPS * 32, 5)
 k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, const int* __restrict__ col,
           const unsigned short* __restrict__ seg_cnt, const int* __restrict__ rowmap, const unsigned* __restrict__ tile_mask,
           const Grid* __restrict__ gp, const __grid_constant__ AevConst K, int n, float* __restrict__ aev,
@@ -192,6 +193,7 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
         }
     }
 
+    __syncwarp();                                        // rr is dead from here on: its bytes become the staging rows
     // ---- angular (Eq. 5) ------------------------------------------------------------------------------
     const int za = lane & 3, aa = lane >> 2;
     float facc = 0.f;                                    // running sum of feature (aa, za) of the current pair
@@ -238,17 +240,17 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
             }
         }
 #pragma unroll
-        for (int z = 0; z < NZ; ++z) S.tA[z][lane] = A[z];
+        for (int z = 0; z < NZ; ++z) S.st.tA[z][lane] = A[z];
 #pragma unroll
-        for (int a = 0; a < NA; ++a) S.tB[a][lane] = B[a];
+        for (int a = 0; a < NA; ++a) S.st.tB[a][lane] = B[a];
         __syncwarp();
         // phase 2: the 8 quads of the round in order (pairs are padded to whole quads, so a pair ends at a quad end);
         // the branch is warp-uniform
         const unsigned endmask = __ballot_sync(FULL, my_end);
 #pragma unroll
         for (int qd = 0; qd < 8; ++qd) {
-            const float4 a4 = *reinterpret_cast<const float4*>(&S.tA[za][4 * qd]);
-            const float4 b4 = *reinterpret_cast<const float4*>(&S.tB[aa][4 * qd]);
+            const float4 a4 = *reinterpret_cast<const float4*>(&S.st.tA[za][4 * qd]);
+            const float4 b4 = *reinterpret_cast<const float4*>(&S.st.tB[aa][4 * qd]);
             facc = fmaf(a4.x, b4.x, facc); facc = fmaf(a4.y, b4.y, facc);
             facc = fmaf(a4.z, b4.z, facc); facc = fmaf(a4.w, b4.w, facc);
             if ((endmask >> (4 * qd + 3)) & 1u) {             // pair complete: its 32 features go out, 64 (128) contiguous bytes
