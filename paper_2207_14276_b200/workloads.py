@@ -356,9 +356,9 @@ def md_inputs(system: System, temperature: float = 300.0, seed: int = 4001, n_pr
     n = system.n_atoms
     if n_protein is None:
         n_protein = 0
-        if system.name in ("proteinbox23k", "biosystem98k"):
+        if system.name in ("protein23k", "biosystem98k"):
             L = float(system.box[0])
-            radius = 30.0 if system.name == "proteinbox23k" else 45.0
+            radius = 30.0 if system.name == "protein23k" else 45.0
             n_protein = int(round(n / L ** 3 * 4.0 / 3.0 * math.pi * radius ** 3))
             while (n - n_protein) % 3 != 0:
                 n_protein += 1

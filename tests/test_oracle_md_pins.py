@@ -117,3 +117,21 @@ def test_respa_with_the_ani_oracle_is_time_reversible_and_second_order():
         _, _, E = M.respa_run(s.pos, md.vel, md.inv_mass, slow, fast, dt, 2, n)
         errs.append(abs(sum(E) - E_start))
     assert errs[1] < 0.45 * errs[0]
+
+
+def test_md_inputs_find_the_waters_of_every_generator():
+    """The fast force of the driver is the O-H bonds of the generators' waters; a protein box whose
+    name the helper does not recognise would silently get none (round-1 bug: "proteinbox23k" vs "protein23k")."""
+    s = W.make_system(3)
+    m = W.md_inputs(s)
+    assert len(m.bonds) > 0 and len(m.bonds) % 2 == 0
+    # every bond is an O-H pair at the TIP3P length (minimum image)
+    d = s.pos[m.bonds[:, 1]].astype(np.float64) - s.pos[m.bonds[:, 0]].astype(np.float64)
+    L = float(s.box[0])
+    d -= L * np.rint(d / L)
+    assert np.all(s.species[m.bonds[:, 0]] == W.O) and np.all(s.species[m.bonds[:, 1]] == W.H)
+    assert np.abs(np.sqrt((d * d).sum(1)) - W.OH_BOND).max() < 1e-4
+    # the waters are everything outside the protein-like sphere: 3 atoms per 2 bonds
+    n_prot = s.n_atoms - 3 * (len(m.bonds) // 2)
+    assert 0.40 < n_prot / s.n_atoms < 0.55
+    assert len(W.md_inputs(W.make_system(1)).bonds) == 2 * 96

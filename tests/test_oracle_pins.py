@@ -416,3 +416,41 @@ def test_batched_molecules_are_independent(params):
         Em, Fm, _ = oracle.energy_forces(s.pos[30 * m:30 * m + 30], s.species[30 * m:30 * m + 30], None, params, blob, 8)
         assert Em.sum() == pytest.approx(E[m], abs=1e-12)
         assert np.allclose(Fm, F[30 * m:30 * m + 30], atol=1e-13)
+
+
+# ------------------------------------------------------------------ composition (Eq. 2; ensemble L159, Q11)
+@pytest.mark.parametrize("cfg", [2, 1])
+def test_energy_forces_composes_mlp_of_aev(params, cfg):
+    """`energy_forces` has its own ensemble loop (network selection by the central atom's species, 1/n_models on E and
+    on dE/dG).  `oracle.mlp` is tied to torch autograd above and `oracle.aev` to the closed forms, so
+    energy_forces == mlp(aev) pins "one network per element" and the ensemble mean (L159, Q11):
+    a dropped 1/n_models or a wrong network index fails here."""
+    s = W.make_system(cfg)
+    blob = W.make_weights(s.n_models)
+    E, _, g = oracle.energy_forces(s.pos, s.species, s.box, params, blob, s.n_models, want_dEdG=True)
+    rows = oracle.aev(s.pos, s.species, s.box, params)
+    E2, g2 = oracle.mlp(rows, s.species, blob, s.n_models, params)
+    assert np.allclose(E, E2, rtol=0, atol=1e-12)
+    assert np.allclose(g, g2, rtol=0, atol=1e-12)
+    # and against torch autograd directly on a few centres of different species (not through oracle.mlp)
+    pick = [int(np.nonzero(s.species == sp)[0][0]) for sp in sorted(set(s.species.tolist()))]
+    Et, gt = torch_mlp(rows[pick], s.species[pick], blob, s.n_models, float(np.float32(0.1)))
+    assert np.allclose(E[pick], Et, rtol=0, atol=1e-12)
+    assert np.allclose(g[pick], gt, rtol=0, atol=1e-12)
+
+
+def test_forces_follow_from_dEdG_by_finite_differences_of_the_aev(params):
+    """F = -sum_i g_i . dG_i/dr with g_i from the (pinned) network gradient: contract oracle.mlp's dE/dG with central
+    finite differences of oracle.aev rows - the chain rule of centre_forces without using energy_forces' own energy."""
+    s = W.make_system(2)
+    blob = W.make_weights(8)
+    _, F, _ = oracle.energy_forces(s.pos, s.species, None, params, blob, 8)
+    rows = oracle.aev(s.pos, s.species, None, params)
+    _, g = oracle.mlp(rows, s.species, blob, 8, params)
+    h = 2.0 ** -14
+    for a, c in ((5, 0), (23, 2)):
+        pp = s.pos.copy(); pm = s.pos.copy()
+        pp[a, c] += np.float32(h); pm[a, c] -= np.float32(h)
+        step = float(pp[a, c]) - float(pm[a, c])
+        dG = (oracle.aev(pp, s.species, None, params) - oracle.aev(pm, s.species, None, params)) / step
+        assert -(g * dG).sum() == pytest.approx(F[a, c], abs=5e-7, rel=5e-6)
