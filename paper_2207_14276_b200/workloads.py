@@ -325,6 +325,26 @@ def small_periodic_mix(n_atoms: int = 600, L: float = 18.3, seed: int = 77, n_mo
                   np.array([L, L, L], dtype=np.float32), None, n_models=n_models)
 
 
+def small_periodic_ortho(n_atoms: int = 900, box=(17.3, 21.9, 24.6), seed: int = 78, n_models: int = 2) -> System:
+    """A periodic ORTHORHOMBIC box with three different edges (include/dhp.h: "cubic/orthorhombic periodic edges") at
+    roughly the density of configs[2]: random sequential addition with the 0.95 Å minimum distance (minimum image per
+    axis), all 7 species.  Edge-case input of the parity tests; no arithmetic of the method."""
+    rng = np.random.default_rng(seed)
+    L = np.asarray(box, dtype=np.float64)
+    pts = np.empty((0, 3))
+    while pts.shape[0] < n_atoms:
+        c = rng.uniform(0.0, 1.0, size=3) * L
+        if pts.shape[0]:
+            d = pts - c
+            d -= L * np.rint(d / L)
+            if (d * d).sum(-1).min() < MIN_DIST ** 2:
+                continue
+        pts = np.concatenate([pts, c[None, :]], axis=0)
+    species = rng.choice(np.arange(7, dtype=np.int32), size=n_atoms,
+                         p=[0.46, 0.28, 0.08, 0.09, 0.03, 0.03, 0.03]).astype(np.int32)
+    return System(f"ortho{n_atoms}", pts.astype(np.float32), species, L.astype(np.float32), None, n_models=n_models)
+
+
 def jitter(system: System, sigma: float, seed: int) -> np.ndarray:
     """Positions displaced by N(0, sigma^2) per coordinate (timing protocol)."""
     rng = np.random.default_rng(seed)

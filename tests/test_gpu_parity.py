@@ -344,9 +344,10 @@ def test_dense_cluster_more_than_32_angular_neighbours(torch, B, params, blob8):
     assert np.diff(rp).max() > 40
     d, E, F = run_gpu(B, torch, s, params, blob8)
     Eo, Fo = oracle.total_energy_forces(s, params, blob8[: 7 * W.PARAMS_PER_NET])
-    # terms are larger here (up to ~60 neighbours at short range): scale the force bar with the force size
-    assert abs(E[0] - Eo[0]) / s.n_atoms <= 5e-6
-    assert np.max(np.abs(F - Fo)) <= max(F_TOL, 2e-5 * np.abs(Fo).max())
+    # measured on B200 (round 2): |dE|/N = 1.4e-7, max|dF| = 3.9e-6 with max|F| = 0.98 and up to 59 angular neighbours:
+    # the north_star bars hold here too
+    assert abs(E[0] - Eo[0]) / s.n_atoms <= E_TOL_PER_ATOM
+    assert np.max(np.abs(F - Fo)) <= F_TOL
     d.close()
 
 

@@ -49,12 +49,19 @@ def test_slab_owner_is_a_balanced_partition_and_periodic_wrap_invariant():
     s = W.make_system(1)
     own = shard.slab_owner(s.pos, s.box, 4)
     assert sorted(np.bincount(own, minlength=4)) == [72, 72, 72, 72]
-    shifted = s.pos.copy()
-    shifted[::5, 0] += 3 * s.box[0]            # whole-box shifts do not move an atom to another slab
-    assert np.array_equal(shard.slab_owner(shifted.astype(np.float64), s.box, 4), own) or \
-        np.mean(shard.slab_owner(shifted, s.box, 4) == own) > 0.98      # fp32 shift rounding may move an edge atom
     cs = [shard.slab_centres(s.pos, s.box, 4, r) for r in range(4)]
     assert np.array_equal(np.sort(np.concatenate(cs)), np.arange(s.n_atoms))
+    # whole-box shifts do not move an atom to another slab: positions on a 2^-10 grid in a 16 Å box, so that the shift
+    # by 3 L is exact in fp32 and the partition must be EQUAL, not approximately equal
+    box = np.array([16.0, 16.0, 16.0], np.float32)
+    q = (np.round(np.mod(s.pos.astype(np.float64), 16.0) * 1024) / 1024).astype(np.float32)
+    own = shard.slab_owner(q, box, 4)
+    shifted = q.copy()
+    shifted[::5, 0] += np.float32(48.0)
+    shifted[1::7, 0] -= np.float32(32.0)
+    delta = shifted[:, 0].astype(np.float64) - q[:, 0].astype(np.float64)
+    assert set(np.unique(delta)) <= {0.0, 48.0, -32.0, 16.0} and np.count_nonzero(delta) > 80     # exact whole-box shifts
+    assert np.array_equal(shard.slab_owner(shifted, box, 4), own)
 
 
 def _worker(rank, port, results):
