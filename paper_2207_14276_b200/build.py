@@ -16,6 +16,7 @@ SOURCES = ["api.cu", "nlist.cu", "aev.cu", "mlp_simt.cu", "mlp_tc.cu", "md.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-O2", "--fmad=true"]
+FLAGS += os.environ.get("DHP_NVCC_EXTRA", "").split()      # e.g. -DMID_TRACE=1 for a timing experiment (never the default)
 
 
 def _stale() -> bool:

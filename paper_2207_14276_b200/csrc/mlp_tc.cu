@@ -933,12 +933,25 @@ k_gemm_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
 #ifndef MID_DBG
 #define MID_DBG 0      // timing experiments only: 1 = epilogues without work, 2 = no MMAs issued
 #endif
-constexpr int MID_SLOTS = 6;
-constexpr int MID_SLOT_BYTES = 20480;
-constexpr int MID_A_OFF = 12288;                 // G2 slots: W2 image of the K step (12 KB), then h1 hi (4 KB), h1 lo (4 KB)
+#ifndef MID_TRACE
+#define MID_TRACE 0    // timing experiments only: CTA 0 records clock64() per role for a few items and prints them at the end
+#endif
+#if MID_TRACE
+__device__ long long g_tr[3][8][24];
+#define TR(role, it, ev) do { if (blockIdx.x == 0 && (it) >= 8 && (it) < 16) g_tr[role][(it) - 8][ev] = clock64(); } while (0)
+#else
+#define TR(role, it, ev) do { } while (0)
+#endif
+constexpr int MID_SLOTS = 3;                     // ring slots of TWO 16-wide K steps each: one full-barrier wait and one commit per 6 MMAs
+constexpr int MID_SLOT_BYTES = 40960;
+constexpr int MID_A_OFF = 24576;                 // G2 slots: W2 images of the two K steps (24 KB), then h1 hi (8 KB), h1 lo (8 KB)
 constexpr int MID_X_PLANE = BM * H2 * 2;         // 48 KB per plane
 constexpr int MID_X_BYTES = 2 * MID_X_PLANE;
-constexpr int MID_SMEM = MID_X_BYTES + MID_SLOTS * MID_SLOT_BYTES + 1024 /*align*/ + 256 /*barriers, TMEM word, ring*/;
+constexpr int MID_CONST_FLOATS = H2 + H3 + H3;   // b2, b3, w4 of one (species, network), staged in shared memory (two buffers)
+constexpr int MID_CONST_BYTES = MID_CONST_FLOATS * 4;
+constexpr int MID_H_ROUND = 32768;               // one 64-column block of h1, hi plane then lo plane (B2's epilogue reads it from X)
+constexpr int MID_SMEM = MID_X_BYTES + MID_SLOTS * MID_SLOT_BYTES + 2 * MID_CONST_BYTES + 1024 /*align*/ + 512 /*barriers, TMEM word, ring*/;
+static_assert(3 * MID_H_ROUND == MID_X_BYTES, "three rounds of h1 fill X exactly");
 constexpr uint32_t MID_P = 0, MID_Q = 192, MID_D = 352, MID_D_LO = MID_D + H3 / 2;
 static_assert(MID_D_LO + H3 / 2 == TMEM_COLS && MID_Q + H1 <= TMEM_COLS, "TMEM map");
 // weight image of one (species, network), in halves: per GEMM [K step][plane][8-column group (2)][n][8]
@@ -1050,16 +1063,23 @@ k_mlp_mid(const MidArgs p) {
     uint8_t* x_ptr = smem_raw + (base - raw);                         // X region (generic pointer), xs its shared address
     const uint32_t xs = base;
     const uint32_t slots = base + MID_X_BYTES;
-    const uint32_t bar0 = slots + MID_SLOTS * MID_SLOT_BYTES;
-    uint64_t* bars = reinterpret_cast<uint64_t*>(x_ptr + MID_X_BYTES + MID_SLOTS * MID_SLOT_BYTES);
-    // barriers: full[SLOTS], empty[SLOTS], acc_p, acc_q, xr[3], sfull[RING], sempty[RING]; then TMEM word and item ring
-    constexpr int NBARS = 2 * MID_SLOTS + 5 + 2 * RING;
+    const uint32_t cst_s = slots + MID_SLOTS * MID_SLOT_BYTES;        // per-item constants b2 | b3 | w4, two buffers
+    const float* cst_ptr = reinterpret_cast<const float*>(x_ptr + MID_X_BYTES + MID_SLOTS * MID_SLOT_BYTES);
+    const uint32_t bar0 = cst_s + 2 * MID_CONST_BYTES;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(x_ptr + MID_X_BYTES + MID_SLOTS * MID_SLOT_BYTES + 2 * MID_CONST_BYTES);
+    // barriers: full[SLOTS], empty[SLOTS], acc_p, acc_q, xr[3], xfree, hfull[3], cfull[2], cempty[2], sfull[RING], sempty[RING];
+    // then the TMEM word and the item ring
+    constexpr int NBARS = 2 * MID_SLOTS + 13 + 2 * RING;
     auto full_bar = [&](int s) { return bar0 + 8u * s; };
     auto empty_bar = [&](int s) { return bar0 + 8u * (MID_SLOTS + s); };
     const uint32_t accp_bar = bar0 + 8u * (2 * MID_SLOTS), accq_bar = accp_bar + 8u;
     auto xr_bar = [&](int k) { return accp_bar + 16u + 8u * k; };      // 64-column block k of an epilogue's output is ready
-    auto sfull_bar = [&](int s) { return bar0 + 8u * (2 * MID_SLOTS + 5 + s); };
-    auto sempty_bar = [&](int s) { return bar0 + 8u * (2 * MID_SLOTS + 5 + RING + s); };
+    const uint32_t xfree_bar = accp_bar + 40u;                         // B2's MMAs have completed: X (d2) is dead
+    auto hfull_bar = [&](int k) { return accp_bar + 48u + 8u * k; };   // h1 block k of the item has landed in X (for CELU'(z1))
+    auto cfull_bar = [&](int b) { return accp_bar + 72u + 8u * b; };
+    auto cempty_bar = [&](int b) { return accp_bar + 88u + 8u * b; };
+    auto sfull_bar = [&](int s) { return bar0 + 8u * (2 * MID_SLOTS + 13 + s); };
+    auto sempty_bar = [&](int s) { return bar0 + 8u * (2 * MID_SLOTS + 13 + RING + s); };
     volatile uint32_t* tmem_word = reinterpret_cast<volatile uint32_t*>(bars + NBARS);
     volatile int* ring = reinterpret_cast<volatile int*>(bars + NBARS + 1);
 
@@ -1069,8 +1089,9 @@ k_mlp_mid(const MidArgs p) {
 
     if (warp == 0 && lane == 0) {
         for (int s = 0; s < MID_SLOTS; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-        mbar_init(accp_bar, 1); mbar_init(accq_bar, 1);
-        for (int k = 0; k < 3; ++k) mbar_init(xr_bar(k), MID_EPI_WARPS);
+        mbar_init(accp_bar, 1); mbar_init(accq_bar, 1); mbar_init(xfree_bar, 1);
+        for (int k = 0; k < 3; ++k) { mbar_init(xr_bar(k), MID_EPI_WARPS); mbar_init(hfull_bar(k), 1); }
+        for (int b = 0; b < 2; ++b) { mbar_init(cfull_bar(b), 1); mbar_init(cempty_bar(b), MID_EPI_WARPS); }
         for (int s = 0; s < RING; ++s) { mbar_init(sfull_bar(s), 1); mbar_init(sempty_bar(s), 1 + MID_EPI_WARPS); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -1085,11 +1106,25 @@ k_mlp_mid(const MidArgs p) {
         if (elect_one()) {
             int slot = 0; uint32_t phase = 0;
             int rs = 0; uint32_t rphase = 0;
+            int cb = 0; uint32_t cphase = 0;
+            uint32_t hphase = 0;
+            int prev_rt = -1, prev_e = 0;
             auto next_slot = [&]() -> uint32_t {
                 mbar_wait(empty_bar(slot), phase ^ 1u);
                 return slots + (uint32_t)slot * MID_SLOT_BYTES;
             };
             auto advance = [&]() { if (++slot == MID_SLOTS) { slot = 0; phase ^= 1u; } };
+            // h1 of the PREVIOUS item -> X once its B2 MMAs (the last readers of d2 in X) have completed: three 64-column
+            // blocks (hi plane then lo plane) for CELU'(z1) in B2's epilogue; the fourth block comes by plain loads
+            auto load_h1_for_b2 = [&]() {
+                mbar_wait(xfree_bar, hphase); hphase ^= 1u;
+                for (int k = 0; k < 3; ++k) {
+                    mbar_expect_tx(hfull_bar(k), (uint32_t)MID_H_ROUND);
+                    bulk_load(xs + (uint32_t)(k * MID_H_ROUND), p.h1 + tile_off(p.plane_tiles, M * 4, 0, prev_rt, prev_e * 4 + k), 16384u, hfull_bar(k));
+                    bulk_load(xs + (uint32_t)(k * MID_H_ROUND) + 16384u, p.h1 + tile_off(p.plane_tiles, M * 4, 1, prev_rt, prev_e * 4 + k), 16384u,
+                              hfull_bar(k));
+                }
+            };
             for (;;) {
                 int item = atomicAdd(p.sched, 1);
                 if (item >= total_items) item = -1;
@@ -1100,37 +1135,51 @@ k_mlp_mid(const MidArgs p) {
                 if (item < 0) break;
                 const int rt = item / M, e = item - rt * M;
                 const int s = max(p.row_species[rt * BM], 0);
-                const __half* w = p.wimg + (size_t)(s * M + e) * MID_W_TOTAL;
-                for (int j = 0; j < H1 / 16; ++j) {                       // G2: W2 K step + the matching 16 columns of h1
+                const int se = s * M + e;
+                const __half* w = p.wimg + (size_t)se * MID_W_TOTAL;
+                {   // b2 | b3 | w4 of this network
+                    mbar_wait(cempty_bar(cb), cphase ^ 1u);
+                    const uint32_t dst = cst_s + (uint32_t)(cb * MID_CONST_BYTES);
+                    mbar_expect_tx(cfull_bar(cb), (uint32_t)MID_CONST_BYTES);
+                    bulk_load(dst, p.b2 + (size_t)se * H2, H2 * 4u, cfull_bar(cb));
+                    bulk_load(dst + H2 * 4u, p.b3 + (size_t)se * H3, H3 * 4u, cfull_bar(cb));
+                    bulk_load(dst + (H2 + H3) * 4u, p.w4 + (size_t)se * H3, H3 * 4u, cfull_bar(cb));
+                    if (++cb == 2) { cb = 0; cphase ^= 1u; }
+                }
+                for (int j = 0; j < H1 / 32; ++j) {                       // G2: W2 K steps 2j, 2j+1 + the matching 32 columns of h1
+                    // the ring's slots free up while the previous item's B2 runs; once they are refilled, wait for that B2
+                    if (j == MID_SLOTS && prev_rt >= 0) load_h1_for_b2();
                     const uint32_t sa = next_slot();
-                    mbar_expect_tx(full_bar(slot), 32u * H2 * 2u + 8192u);
-                    bulk_load(sa, w + MID_W_G2 + (size_t)j * 32 * H2, 32u * H2 * 2u, full_bar(slot));
-                    const size_t goff = (size_t)((j & 3) * 2) * BM * 8;
-                    bulk_load(sa + MID_A_OFF, p.h1 + tile_off(p.plane_tiles, M * 4, 0, rt, e * 4 + (j >> 2)) + goff, 4096u, full_bar(slot));
-                    bulk_load(sa + MID_A_OFF + 4096, p.h1 + tile_off(p.plane_tiles, M * 4, 1, rt, e * 4 + (j >> 2)) + goff, 4096u,
+                    mbar_expect_tx(full_bar(slot), 64u * H2 * 2u + 16384u);
+                    bulk_load(sa, w + MID_W_G2 + (size_t)j * 64 * H2, 64u * H2 * 2u, full_bar(slot));
+                    const size_t goff = (size_t)((j & 1) * 4) * BM * 8;
+                    bulk_load(sa + MID_A_OFF, p.h1 + tile_off(p.plane_tiles, M * 4, 0, rt, e * 4 + (j >> 1)) + goff, 8192u, full_bar(slot));
+                    bulk_load(sa + MID_A_OFF + 8192, p.h1 + tile_off(p.plane_tiles, M * 4, 1, rt, e * 4 + (j >> 1)) + goff, 8192u,
                               full_bar(slot));
                     advance();
                 }
-                for (int j = 0; j < H2 / 16; ++j) {                       // G3
+                for (int j = 0; j < H2 / 32; ++j) {                       // G3
                     const uint32_t sa = next_slot();
-                    mbar_expect_tx(full_bar(slot), 32u * H3 * 2u);
-                    bulk_load(sa, w + MID_W_G3 + (size_t)j * 32 * H3, 32u * H3 * 2u, full_bar(slot));
+                    mbar_expect_tx(full_bar(slot), 64u * H3 * 2u);
+                    bulk_load(sa, w + MID_W_G3 + (size_t)j * 64 * H3, 64u * H3 * 2u, full_bar(slot));
                     advance();
                 }
                 if (p.forward_only) continue;
-                for (int j = 0; j < H3 / 16; ++j) {                       // B3
+                for (int j = 0; j < H3 / 32; ++j) {                       // B3
                     const uint32_t sa = next_slot();
-                    mbar_expect_tx(full_bar(slot), 32u * H2 * 2u);
-                    bulk_load(sa, w + MID_W_B3 + (size_t)j * 32 * H2, 32u * H2 * 2u, full_bar(slot));
+                    mbar_expect_tx(full_bar(slot), 64u * H2 * 2u);
+                    bulk_load(sa, w + MID_W_B3 + (size_t)j * 64 * H2, 64u * H2 * 2u, full_bar(slot));
                     advance();
                 }
-                for (int j = 0; j < H2 / 16; ++j) {                       // B2
+                for (int j = 0; j < H2 / 32; ++j) {                       // B2
                     const uint32_t sa = next_slot();
-                    mbar_expect_tx(full_bar(slot), 32u * H1 * 2u);
-                    bulk_load(sa, w + MID_W_B2 + (size_t)j * 32 * H1, 32u * H1 * 2u, full_bar(slot));
+                    mbar_expect_tx(full_bar(slot), 64u * H1 * 2u);
+                    bulk_load(sa, w + MID_W_B2 + (size_t)j * 64 * H1, 64u * H1 * 2u, full_bar(slot));
                     advance();
                 }
+                prev_rt = rt; prev_e = e;
             }
+            if (prev_rt >= 0) load_h1_for_b2();                          // the last item of this CTA
         }
     } else if (warp == 1) {
         // ===== MMA issuer =====
@@ -1142,14 +1191,15 @@ k_mlp_mid(const MidArgs p) {
             int slot = 0; uint32_t phase = 0;
             int rs = 0; uint32_t rphase = 0;
             uint32_t xphase = 0;                                   // bit k: parity of xr[k]
+            int nit = 0; (void)nit;
             enum { A_SLOT = 0, A_X = 1, A_TMEM = 2 };
             auto run = [&](int n, int steps, int a_src, uint32_t d_tmem) {
                 const uint32_t idesc = make_idesc(n);
                 const uint32_t lbo_b = (uint32_t)n * 16u;
                 uint32_t accumulate = 0u;
-                for (int j = 0; j < steps; ++j) {
-                    if (a_src != A_SLOT && (j & 3) == 0) {
-                        const int kb = j >> 2;
+                for (int sl = 0; sl < steps / 2; ++sl) {                 // one ring slot = K steps 2 sl, 2 sl + 1
+                    if (a_src != A_SLOT && (sl & 1) == 0) {
+                        const int kb = sl >> 1;
                         mbar_wait(xr_bar(kb), (xphase >> kb) & 1u);
                         xphase ^= 1u << kb;
                         tc_fence_after();
@@ -1157,27 +1207,32 @@ k_mlp_mid(const MidArgs p) {
                     mbar_wait(full_bar(slot), phase);
                     tc_fence_after();
                     const uint32_t sa = slots + (uint32_t)slot * MID_SLOT_BYTES;
-                    const uint64_t b_hi = make_desc_ns(sa, lbo_b), b_lo = make_desc_ns(sa + 2u * lbo_b, lbo_b);
-                    if (!(MID_DBG & 2)) {
-                        if (a_src == A_TMEM) {
-                            const uint32_t a_hi = tmem_base + MID_D + (uint32_t)j * 8u, a_lo = tmem_base + MID_D_LO + (uint32_t)j * 8u;
-                            umma_f16_ts(d_tmem, a_hi, b_hi, idesc, accumulate);
-                            if (!p.single) {
-                                umma_f16_ts(d_tmem, a_hi, b_lo, idesc, 1u);
-                                umma_f16_ts(d_tmem, a_lo, b_hi, idesc, 1u);
-                            }
-                        } else {
-                            const uint32_t a0 = a_src == A_SLOT ? sa + MID_A_OFF : xs + (uint32_t)j * 4096u;
-                            const uint64_t a_hi = make_desc_ns(a0, 2048u);
-                            const uint64_t a_lo = make_desc_ns(a0 + (a_src == A_SLOT ? 4096u : (uint32_t)MID_X_PLANE), 2048u);
-                            umma_f16(d_tmem, a_hi, b_hi, idesc, accumulate);
-                            if (!p.single) {
-                                umma_f16(d_tmem, a_hi, b_lo, idesc, 1u);
-                                umma_f16(d_tmem, a_lo, b_hi, idesc, 1u);
+#pragma unroll
+                    for (int t = 0; t < 2; ++t) {
+                        const int j = 2 * sl + t;
+                        const uint32_t sb = sa + (uint32_t)t * 4u * lbo_b;
+                        const uint64_t b_hi = make_desc_ns(sb, lbo_b), b_lo = make_desc_ns(sb + 2u * lbo_b, lbo_b);
+                        if (!(MID_DBG & 2)) {
+                            if (a_src == A_TMEM) {
+                                const uint32_t a_hi = tmem_base + MID_D + (uint32_t)j * 8u, a_lo = tmem_base + MID_D_LO + (uint32_t)j * 8u;
+                                umma_f16_ts(d_tmem, a_hi, b_hi, idesc, accumulate);
+                                if (!p.single) {
+                                    umma_f16_ts(d_tmem, a_hi, b_lo, idesc, 1u);
+                                    umma_f16_ts(d_tmem, a_lo, b_hi, idesc, 1u);
+                                }
+                            } else {
+                                const uint32_t a0 = a_src == A_SLOT ? sa + MID_A_OFF + (uint32_t)t * 4096u : xs + (uint32_t)j * 4096u;
+                                const uint64_t a_hi = make_desc_ns(a0, 2048u);
+                                const uint64_t a_lo = make_desc_ns(a0 + (a_src == A_SLOT ? 8192u : (uint32_t)MID_X_PLANE), 2048u);
+                                umma_f16(d_tmem, a_hi, b_hi, idesc, accumulate);
+                                if (!p.single) {
+                                    umma_f16(d_tmem, a_hi, b_lo, idesc, 1u);
+                                    umma_f16(d_tmem, a_lo, b_hi, idesc, 1u);
+                                }
                             }
                         }
+                        accumulate = 1u;
                     }
-                    accumulate = 1u;
                     umma_commit(empty_bar(slot));
                     if (++slot == MID_SLOTS) { slot = 0; phase ^= 1u; }
                 }
@@ -1188,11 +1243,18 @@ k_mlp_mid(const MidArgs p) {
                 mbar_arrive(sempty_bar(rs));
                 if (++rs == RING) { rs = 0; rphase ^= 1u; }
                 if (item < 0) break;
+                TR(0, nit, 0);
                 run(H2, H1 / 16, A_SLOT, tmem_base + MID_P); umma_commit(accp_bar);     // G2: h1 W2^T        -> P
+                TR(0, nit, 1);
                 run(H3, H2 / 16, A_X, tmem_base + MID_Q);    umma_commit(accq_bar);     // G3: h2 W3^T        -> Q
+                TR(0, nit, 2);
                 if (p.forward_only) continue;
                 run(H2, H3 / 16, A_TMEM, tmem_base + MID_P); umma_commit(accp_bar);     // B3: d3 W3          -> P
+                TR(0, nit, 3);
                 run(H1, H2 / 16, A_X, tmem_base + MID_Q);    umma_commit(accq_bar);     // B2: d2 W2          -> Q u D
+                umma_commit(xfree_bar);                                                  // ... and X is free for h1 (producer)
+                TR(0, nit, 4);
+                ++nit;
             }
         }
     } else {
@@ -1202,7 +1264,10 @@ k_mlp_mid(const MidArgs p) {
         const int r_in = q * 32 + lane;
         const uint32_t lane_base = tmem_base + ((uint32_t)(q * 32) << 16);
         int rs = 0; uint32_t rphase = 0;
-        uint32_t pphase = 0, qphase = 0;
+        uint32_t pphase = 0, qphase = 0, hph = 0;
+        int cb = 0; uint32_t cphase = 0;
+        int nit = 0; (void)nit;
+        const bool trw = warp == 2 && lane == 0; (void)trw;
         const float kexp = 1.4426950408889634f / p.alpha, inv_alpha = 1.0f / p.alpha;
         const float sc = 1.0f / W_SCALE;
         // this warp's part of 64-column block k is written (shared memory made visible to the tensor core's proxy, tensor
@@ -1212,6 +1277,18 @@ k_mlp_mid(const MidArgs p) {
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(xr_bar(k));
+        };
+        auto signal_t = [&](int k) {                         // the same when the block went to tensor memory only
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(xr_bar(k));
+        };
+        auto lds16 = [&](const float* src, float (&x)[16]) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const float4 t4 = *reinterpret_cast<const float4*>(src + 4 * i);
+                x[4 * i] = t4.x; x[4 * i + 1] = t4.y; x[4 * i + 2] = t4.z; x[4 * i + 3] = t4.w;
+            }
         };
         for (;;) {
             mbar_wait(sfull_bar(rs), rphase);
@@ -1226,29 +1303,33 @@ k_mlp_mid(const MidArgs p) {
             const int se = s * M + e;
             uint32_t v[16];
             float x[16], aux[16];
+            // the item's constants (b2 | b3 | w4) arrive in shared memory by bulk copy: no global load inside the rounds
+            mbar_wait(cfull_bar(cb), cphase);
+            const float* cst = cst_ptr + cb * MID_CONST_FLOATS;
             // ---- G2 (P): h2 = CELU(acc / 64 + b2) -> X, block by block
-            load16(p.b2 + (size_t)se * H2 + cg * 16, aux);
+            if (trw) TR(1, nit, 0);
             mbar_wait(accp_bar, pphase); pphase ^= 1u;
             tc_fence_after();
+            if (trw) TR(1, nit, 1);
 #pragma unroll 1
             for (int k = 0; k < 3; ++k) {
                 const int c0 = 64 * k + 16 * cg;
                 if (!(MID_DBG & 1)) {
                     tmem_ld16_issue(lane_base + MID_P + (uint32_t)c0, v);
+                    lds16(cst + c0, aux);
                     tmem_ld_wait();
 #pragma unroll
                     for (int i = 0; i < 16; ++i) x[i] = celu_f(fmaf(__uint_as_float(v[i]), sc, aux[i]), p.alpha, kexp);
-                    if (k < 2) load16(p.b2 + (size_t)se * H2 + c0 + 64, aux);
                     store_split16_x(x, x_ptr, c0, r_in);
                 }
                 signal_x(k);
+                if (trw) TR(1, nit, 2 + k);
             }
             // ---- G3 (Q): h3 = CELU(acc / 64 + b3); E_i += (w4.h3 + b4)/M; d3 = w4 CELU'(z3) 2^10 / M -> tensor memory (A of B3)
             float w4v[16];
-            load16(p.b3 + (size_t)se * H3 + cg * 16, aux);
-            load16(p.w4 + (size_t)se * H3 + cg * 16, w4v);
             mbar_wait(accq_bar, qphase); qphase ^= 1u;
             tc_fence_after();
+            if (trw) TR(1, nit, 5);
             float e_acc = 0.f;
             const float dsc = p.inv_models * D_SCALE;
 #pragma unroll 1
@@ -1256,16 +1337,14 @@ k_mlp_mid(const MidArgs p) {
                 const int c0 = 64 * k + 16 * cg;
                 if (c0 < H3 && !(MID_DBG & 1)) {
                     tmem_ld16_issue(lane_base + MID_Q + (uint32_t)c0, v);
+                    lds16(cst + H2 + c0, aux);
+                    lds16(cst + H2 + H3 + c0, w4v);
                     tmem_ld_wait();
 #pragma unroll
                     for (int i = 0; i < 16; ++i) {
                         const float h = celu_f(fmaf(__uint_as_float(v[i]), sc, aux[i]), p.alpha, kexp);
                         e_acc = fmaf(w4v[i], h, e_acc);
                         x[i] = w4v[i] * dsc * dcelu_from_h(h, inv_alpha);
-                    }
-                    if (c0 + 64 < H3) {
-                        load16(p.b3 + (size_t)se * H3 + c0 + 64, aux);
-                        load16(p.w4 + (size_t)se * H3 + c0 + 64, w4v);
                     }
                     if (!p.forward_only) {
                         uint32_t ph[8], pl[8];
@@ -1276,13 +1355,18 @@ k_mlp_mid(const MidArgs p) {
                         tmem_st_wait();
                     }
                 }
-                if (!p.forward_only) signal_x(k);
+                if (!p.forward_only) signal_t(k);
+                if (trw) TR(1, nit, 6 + k);
             }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(cempty_bar(cb));                 // the constants buffer may be refilled
+            if (++cb == 2) { cb = 0; cphase ^= 1u; }
             atomicAdd(&p.e_atom[row], (e_acc + (cg == 0 ? p.b4[se] : 0.f)) * p.inv_models);
             if (p.forward_only) { tc_fence_before(); continue; }
             // ---- B3 (P): d2 = (acc / 64) CELU'(z2), CELU' from this thread's own h2 in X, d2 written over it
             mbar_wait(accp_bar, pphase); pphase ^= 1u;
             tc_fence_after();
+            if (trw) TR(1, nit, 9);
 #pragma unroll 1
             for (int k = 0; k < 3; ++k) {
                 const int c0 = 64 * k + 16 * cg;
@@ -1302,31 +1386,46 @@ k_mlp_mid(const MidArgs p) {
                     store_split16_x(x, x_ptr, c0, r_in);
                 }
                 signal_x(k);
+                if (trw) TR(1, nit, 10 + k);
             }
-            // ---- B2 (Q u D): d1 = (acc / 64) CELU'(z1) -> global (tiled planes), CELU' from the saved h1 (fetched ahead)
+            // ---- B2 (Q u D): d1 = (acc / 64) CELU'(z1) -> global (tiled planes).  CELU' needs the saved h1: its first three
+            //      64-column blocks arrive in X by bulk copy once B2's MMAs are done with d2 (producer), the fourth by plain
+            //      loads issued here, whose latency runs under the first three rounds
             uint4 gh[2], gl[2];
             auto h1_offsets = [&](int c0, size_t& o_hi, size_t& o_lo) {
                 const size_t in_tile = (size_t)(((c0 & 63) >> 3) * BM + r_in) * 8;
                 o_hi = tile_off(p.plane_tiles, M * 4, 0, rt, e * 4 + (c0 >> 6)) + in_tile;
                 o_lo = tile_off(p.plane_tiles, M * 4, 1, rt, e * 4 + (c0 >> 6)) + in_tile;
             };
-            auto h1_fetch = [&](int c0) {
+            uint4 lh[2], ll[2];
+            if (!(MID_DBG & 1)) {
                 size_t o_hi, o_lo;
-                h1_offsets(c0, o_hi, o_lo);
+                h1_offsets(192 + cg * 16, o_hi, o_lo);
 #pragma unroll
                 for (int i = 0; i < 2; ++i) {
-                    gh[i] = *reinterpret_cast<const uint4*>(p.h1 + o_hi + i * (BM * 8));
-                    gl[i] = *reinterpret_cast<const uint4*>(p.h1 + o_lo + i * (BM * 8));
+                    lh[i] = *reinterpret_cast<const uint4*>(p.h1 + o_hi + i * (BM * 8));
+                    ll[i] = *reinterpret_cast<const uint4*>(p.h1 + o_lo + i * (BM * 8));
                 }
-            };
-            if (!(MID_DBG & 1)) h1_fetch(cg * 16);
+            }
             mbar_wait(accq_bar, qphase); qphase ^= 1u;
             tc_fence_after();
+            if (trw) TR(1, nit, 13);
 #pragma unroll 1
-            for (int c0 = cg * 16; c0 < H1 && !(MID_DBG & 1); c0 += 64) {
+            for (int k = 0; k < 4 && !(MID_DBG & 1); ++k) {
+                const int c0 = 64 * k + 16 * cg;
                 tmem_ld16_issue(lane_base + MID_Q + (uint32_t)c0, v);
-                join16(gh, gl, aux);
-                if (c0 + 64 < H1) h1_fetch(c0 + 64);
+                if (k < 3) {
+                    mbar_wait(hfull_bar(k), hph);
+                    const uint8_t* src = x_ptr + (size_t)k * MID_H_ROUND + (size_t)((2 * cg) * BM + r_in) * 16;
+#pragma unroll
+                    for (int i = 0; i < 2; ++i) {
+                        gh[i] = *reinterpret_cast<const uint4*>(src + i * (BM * 16));
+                        gl[i] = *reinterpret_cast<const uint4*>(src + 16384 + i * (BM * 16));
+                    }
+                    join16(gh, gl, aux);
+                } else {
+                    join16(lh, ll, aux);
+                }
                 tmem_ld_wait();
 #pragma unroll
                 for (int i = 0; i < 16; ++i) x[i] = __uint_as_float(v[i]) * sc * dcelu_from_h(aux[i], inv_alpha);
@@ -1334,13 +1433,31 @@ k_mlp_mid(const MidArgs p) {
                 h1_offsets(c0, o_hi, o_lo);
                 store_split16_tiled(x, p.d1 + o_hi, p.d1 + o_lo);
             }
+            hph ^= 1u;
             tc_fence_before();
+            // every epilogue warp has read its h1 out of X before any of them writes the next item's h2 into it
+            asm volatile("bar.sync 1, %0;" ::"n"(32 * MID_EPI_WARPS) : "memory");
+            if (trw) TR(1, nit, 14);
+            ++nit;
         }
     }
     tc_fence_before();
     __syncthreads();
     if (warp == 1) tmem_dealloc(tmem_base, TMEM_COLS);
+#if MID_TRACE
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        const long long t0 = g_tr[0][0][0];
+        for (int it = 0; it < 8; ++it) {
+            printf("MMA item %d:", it);
+            for (int e = 0; e < 5; ++e) printf(" %lld", g_tr[0][it][e] - t0);
+            printf("\nEPI item %d:", it);
+            for (int e = 0; e < 15; ++e) printf(" %lld", g_tr[1][it][e] - t0);
+            printf("\n");
+        }
+    }
+#endif
 }
+
 
 // weight images for k_mlp_mid: img[(s*M + e)][MID_W_TOTAL], see the layout above
 __global__ void k_prep_mid(const float* __restrict__ blob, int n_models, __half* __restrict__ img) {
