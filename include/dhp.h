@@ -17,7 +17,7 @@
  *     on the same context.
  *   - Hot calls (dhp_nlist_build, dhp_ani_energy_forces) only enqueue work on the context's stream:
  *     no allocation, no host synchronisation.  Data-dependent faults (species outside 0..6, neighbour
- *     capacity overflow) set a device-side status word, read with dhp_status().
+ *     capacity overflow) set a device-side status word that stays set until dhp_status() reads it.
  *   - Units are the caller's: Å in, Hartree and Hartree/Å out (F = -dE/dr); no conversion inside.
  *   - Species index 0..6 = H, C, N, O, S, F, Cl.  The shape is fixed at compile time:
  *     16 radial shifts, 8 x 4 angular shifts, AEV length 7*16 + 28*32 = 1008,
@@ -99,6 +99,14 @@ enum {
 int dhp_create(dhp_ctx** out, const dhp_params* params, int64_t max_atoms, int64_t max_mols, void* cuda_stream);
 int dhp_destroy(dhp_ctx* ctx);
 
+/* Fixed limits of this build (compile-time constants of the kernels):
+ *   n_models <= 8 (DHP_MAX_MODELS); at most 96 neighbours within rca and 192 within rcr of one atom (DHP_MAX_ANG,
+ *   DHP_MAX_RAD: 3.4x / 3.5x the counts at 0.1 atoms/Å^3) - beyond that the call flags DHP_E_CAPACITY;
+ *   total pair storage 160 directed pairs per atom of max_atoms. */
+#define DHP_MAX_MODELS 8
+#define DHP_MAX_ANG 96
+#define DHP_MAX_RAD 192
+
 /* Upload network parameters.  blob: HOST or DEVICE pointer to fp32, layout
  *   for e in 0..n_models-1: for s in 0..6: W1[256][1008], b1[256], W2[192][256], b2[192],
  *                                           W3[160][192], b3[160], W4[1][160], b4[1]
@@ -134,7 +142,10 @@ int dhp_set_skin(dhp_ctx* ctx, float skin);
 /* Full builds since dhp_set_skin(skin > 0) (synchronises); every other hot call reused the candidate list. */
 int64_t dhp_nlist_rebuild_count(dhp_ctx* ctx);
 
-/* Number of directed pairs in the radial (<= rcr) and angular (<= rca) lists.  Synchronises. */
+/* Number of directed pairs in the radial (<= rcr) and angular (<= rca) lists.  Synchronises.
+ * (SURVEY.md §8(b) proposed these counts as outputs of dhp_nlist_export; they are a call of their own because the
+ * caller needs them BEFORE it can allocate the col / col_ang buffers that dhp_nlist_export fills.)
+ * A dhp_nlist handle is a token of the context that built it: passing it to another context is DHP_E_BADARG. */
 int dhp_nlist_sizes(dhp_ctx* ctx, const dhp_nlist* nl, int64_t* nnz, int64_t* nnz_ang);
 
 /* Canonical form for parity: caller's atom numbering, both directions, each row ascending in j.
@@ -201,8 +212,12 @@ int dhp_ani_energy_forces_host(dhp_ctx* ctx, const float* pos, const float* box,
                                int64_t n_atoms, const int32_t* mol_offsets, int64_t n_mol,
                                const dhp_weights* weights, int n_models, double* E, float* F);
 
-/* Synchronises the stream and returns the device status word of the last hot call:
- * DHP_OK, DHP_E_SPECIES, DHP_E_CAPACITY, or DHP_E_CUDA. */
+/* Synchronises the stream and returns the first data-dependent fault of ANY hot call since the previous dhp_status()
+ * (DHP_E_SPECIES, DHP_E_CAPACITY), DHP_OK if there was none, or DHP_E_CUDA.  The word is sticky: every hot call folds its
+ * own status into it on the device, so a fault at an intermediate call of an unsynchronised sequence (dhp_md_run
+ * enqueues n_steps calls) is not lost; reading clears it.  After DHP_E_CAPACITY the results of the faulting call are
+ * those of a truncated list (or of an empty one if the total pair storage overflowed); with list reuse the candidate
+ * list is discarded and the next call rebuilds. */
 int dhp_status(dhp_ctx* ctx);
 
 int dhp_set_mlp_mode(dhp_ctx* ctx, int mode);

@@ -104,6 +104,32 @@ def _dptr(t) -> Optional[int]:
     return t.data_ptr()
 
 
+def _check_inputs(torch, device, pos, species, mol_offsets=None, host: bool = False):
+    """The C ABI reads raw addresses: refuse anything it would misread (wrong dtype, a strided view, the wrong device)
+    instead of returning garbage with DHP_OK.  `host`: buffers of the host entry point (numpy or CPU tensors)."""
+    def one(name, a, dtype_np, dtype_t, shape_tail):
+        if isinstance(a, np.ndarray):
+            if not host:
+                raise DhpError(f"{name}: a numpy array was passed to a device-pointer call")
+            ok = a.dtype == dtype_np and a.flags["C_CONTIGUOUS"]
+        else:
+            ok = a.dtype == dtype_t and a.is_contiguous() and ((a.device.type == "cpu") if host else (a.device == device))
+        if not ok or tuple(a.shape[1:]) != shape_tail:
+            raise DhpError(f"{name} must be a contiguous {dtype_np.__name__} array of shape [N{', 3' if shape_tail else ''}] "
+                           f"{'in host memory' if host else f'on {device}'}")
+    one("pos", pos, np.float32, torch.float32, (3,))
+    one("species", species, np.int32, torch.int32, ())
+    n = int(pos.shape[0])
+    if int(species.shape[0]) != n:
+        raise DhpError("species must have one entry per atom")
+    if mol_offsets is not None:
+        one("mol_offsets", mol_offsets, np.int32, torch.int32, ())
+        if int(mol_offsets.shape[0]) < 2:
+            raise DhpError("mol_offsets needs n_mol + 1 >= 2 entries")
+        if host and (int(mol_offsets[0]) != 0 or int(mol_offsets[-1]) != n):     # values of device tables are not read here:
+            raise DhpError("mol_offsets must start at 0 and end at n_atoms")      # that would synchronise the hot call
+
+
 def make_params(p) -> DhpParams:
     """`workloads.AniParams` (fp32 values) -> C struct."""
     q = DhpParams()
@@ -173,6 +199,7 @@ class Dhp:
 
     def dhp_nlist_build(self, pos, box, species, mol_offsets=None):
         """pos/species/mol_offsets: cuda tensors (fp32 [N,3], int32 [N], int32 [n_mol+1]); box: host fp32[3] or None."""
+        _check_inputs(self.torch, self.device, pos, species, mol_offsets)
         n = int(pos.shape[0])
         boxh = None if box is None else np.ascontiguousarray(box, dtype=np.float32)
         n_mol = 0 if mol_offsets is None else int(mol_offsets.shape[0]) - 1
@@ -209,6 +236,7 @@ class Dhp:
     def dhp_ani_energy_forces(self, pos, box, species, weights, mol_offsets=None, E=None, F=None):
         """Device-pointer hot call.  Returns (E fp64 [max(1,n_mol)], F fp32 [N,3]) cuda tensors; asynchronous."""
         t = self.torch
+        _check_inputs(t, self.device, pos, species, mol_offsets)
         n = int(pos.shape[0])
         boxh = None if box is None else np.ascontiguousarray(box, dtype=np.float32)
         n_mol = 0 if mol_offsets is None else int(mol_offsets.shape[0]) - 1
@@ -226,6 +254,7 @@ class Dhp:
         """Partial evaluation over the atoms with central[i] != 0 (cuda uint8 [N], or None = all): E_c and the force
         F_c = -dE_c/dr on ALL atoms.  Over a partition of the atoms the results add up to the full call's."""
         t = self.torch
+        _check_inputs(t, self.device, pos, species, mol_offsets)
         n = int(pos.shape[0])
         boxh = None if box is None else np.ascontiguousarray(box, dtype=np.float32)
         n_mol = 0 if mol_offsets is None else int(mol_offsets.shape[0]) - 1
@@ -244,6 +273,7 @@ class Dhp:
     def dhp_ani_energy(self, pos, box, species, weights, mol_offsets=None, E=None):
         """Energy-only device-pointer call (a1, a2, a3).  Returns E fp64 [max(1,n_mol)] cuda tensor; asynchronous."""
         t = self.torch
+        _check_inputs(t, self.device, pos, species, mol_offsets)
         n = int(pos.shape[0])
         boxh = None if box is None else np.ascontiguousarray(box, dtype=np.float32)
         n_mol = 0 if mol_offsets is None else int(mol_offsets.shape[0]) - 1
@@ -256,6 +286,7 @@ class Dhp:
 
     def dhp_ani_energy_forces_host(self, pos, box, species, weights, mol_offsets=None, E=None, F=None):
         """Host-buffer call (numpy arrays or pinned torch CPU tensors): copies in, kernels, copies out, one sync."""
+        _check_inputs(self.torch, self.device, pos, species, mol_offsets, host=True)
         n = int(pos.shape[0])
         boxh = None if box is None else np.ascontiguousarray(box, dtype=np.float32)
         n_mol = 0 if mol_offsets is None else int(mol_offsets.shape[0]) - 1
@@ -293,6 +324,7 @@ class Dhp:
     def dhp_md_run(self, md, pos, vel, box, species, weights, dt: float, n_inner: int, n_steps: int, E_out=None):
         """n_steps outer steps in place on the cuda tensors pos, vel.  Returns E_out (fp64 [3] cuda: E_ANI, E_bonds, E_kin)."""
         t = self.torch
+        _check_inputs(t, self.device, pos, species)
         boxh = None if box is None else np.ascontiguousarray(box, dtype=np.float32)
         if E_out is None:
             E_out = t.empty(3, dtype=t.float64, device=self.device)

@@ -66,7 +66,7 @@ __device__ __forceinline__ float dfcut(float R, float inv_rc, float pi_over_rc) 
 // Output: PLANES = false, full fp32 rows (SIMT MLP path); PLANES = true, the two-term fp16 split of the
 // feature blocks that are active for the row's tile (what G1 reads), written straight into the tensor path's planes.
 constexpr int AEV_WARPS = 8;
-constexpr int MAX_RAD = 192;    // radial neighbours staged per centre (= the pair list's per-row capacity)
+constexpr int MAX_RAD = DHP_MAX_RAD;    // radial neighbours staged per centre (= the pair list's per-row capacity)
 
 // internal pair p = hi (hi + 1) / 2 + lo over priority positions -> species(lo) | species(hi) << 4 (prio_sp(), dhp_internal.cuh);
 // a static initialiser, so every device of the process has it without a per-device upload
@@ -520,8 +520,10 @@ __global__ void k_unsort_forces(const float* __restrict__ fsorted, const int* __
 // E (per molecule, or one total): fp64 sum of the per-row atomic energies
 __global__ void k_energy_reduce(const float* __restrict__ e_atom, const int* __restrict__ row_slot,
                                 const int* __restrict__ smol, const int* __restrict__ sp_start, int per_mol,
-                                double* __restrict__ E) {
+                                double* __restrict__ E, const int* __restrict__ status, int* __restrict__ sticky) {
     __shared__ double part[32];
+    // every kernel that can raise a data-dependent fault has run by now: fold the call's status word into the sticky one
+    if (blockIdx.x == 0 && threadIdx.x == 0) { const int s = *status; if (s != 0) atomicCAS(sticky, 0, s); }
     const int nrows = sp_start[NSP];
     double acc = 0.0;
     for (int r = blockIdx.x * blockDim.x + threadIdx.x; r < nrows; r += gridDim.x * blockDim.x) {
@@ -589,7 +591,7 @@ int energy_reduce(Ctx* ctx, double* E_out) {
     DHP_CUDA(ctx, cudaMemsetAsync(E_out, 0, sizeof(double) * ne, ctx->stream));
     if (ctx->n_atoms == 0) return DHP_OK;
     int blocks = (int)std::min<int64_t>((ctx->n_atoms + 255) / 256 + NSP, 2 * ctx->sm_count);
-    DHP_LAUNCH(ctx, k_energy_reduce, blocks, 256, 0, ctx->e_atom, ctx->row_slot, ctx->smol, ctx->sp_start, per_mol, E_out);
+    DHP_LAUNCH(ctx, k_energy_reduce, blocks, 256, 0, ctx->e_atom, ctx->row_slot, ctx->smol, ctx->sp_start, per_mol, E_out, ctx->status, ctx->sticky);
     DHP_CUDA(ctx, cudaGetLastError());
     return DHP_OK;
 }

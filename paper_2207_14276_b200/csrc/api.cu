@@ -40,7 +40,7 @@ static bool dalloc(T** p, size_t count) {
 }
 
 static void free_all(Ctx* c) {
-    void* ptrs[] = {c->grid, c->zero_arena, c->ff_arena, c->bbox, c->cell_of, c->perm_tmp, c->cell_start, c->perm,
+    void* ptrs[] = {c->sticky, c->cand_bad, c->grid, c->zero_arena, c->ff_arena, c->bbox, c->cell_of, c->perm_tmp, c->cell_start, c->perm,
                     c->inv_perm, c->spos, c->smol, c->snc, c->n_rad, c->n_ang, c->row_ptr, c->col, c->sp_count, c->sp_start,
                     c->rowmap, c->blk_hist, c->key_start, c->amask, c->col2feat, c->aev, c->grad,
                     c->e_out_tmp, c->export_tmp, c->cand, c->cand_cnt, c->pos_ref, c->rebuild, c->rebuild_count, c->tmp_col, c->blk_off, c->seg_cnt, c->st_pos, c->st_species, c->st_mol, c->st_E, c->st_F};
@@ -163,9 +163,7 @@ using namespace dhp;
 
 extern "C" {
 
-struct dhp_nlist { Ctx* owner; };
 struct dhp_weights { Weights w; };
-static dhp_nlist g_nlist_token;   // the list lives in the context workspace; the handle is a token
 
 int dhp_create(dhp_ctx** out, const dhp_params* params, int64_t max_atoms, int64_t max_mols, void* cuda_stream) {
     if (!out || max_atoms < 1 || max_mols < 0) return DHP_E_BADARG;
@@ -199,7 +197,7 @@ int dhp_create(dhp_ctx** out, const dhp_params* params, int64_t max_atoms, int64
     const size_t N = (size_t)max_atoms, R = (size_t)c->max_rows, NC = (size_t)c->max_cells;
     const size_t NM = (size_t)(max_mols > 0 ? max_mols : 1);
     bool ok = true;
-    ok &= dalloc(&c->grid, 1) && dalloc(&c->bbox, 8);
+    ok &= dalloc(&c->grid, 1) && dalloc(&c->bbox, 8) && dalloc(&c->sticky, 1) && dalloc(&c->cand_bad, 1);
     ok &= dalloc(&c->cell_of, N) && dalloc(&c->perm_tmp, N) && dalloc(&c->cell_start, NC + 1);
     ok &= dalloc(&c->perm, N) && dalloc(&c->inv_perm, N) && dalloc(&c->spos, N) && dalloc(&c->smol, N) && dalloc(&c->snc, N);
     ok &= dalloc(&c->n_rad, N) && dalloc(&c->n_ang, N) && dalloc(&c->row_ptr, N + 1) && dalloc(&c->col, (size_t)c->pair_cap);
@@ -234,6 +232,7 @@ int dhp_create(dhp_ctx** out, const dhp_params* params, int64_t max_atoms, int64
         ok &= cudaMemset(c->aev, 0, sizeof(float) * R * AEV_LD) == cudaSuccess;
         ok &= cudaMemset(c->grad, 0, sizeof(float) * R * AEV_LD) == cudaSuccess;
         ok &= cudaMemset(c->status, 0, sizeof(int)) == cudaSuccess;
+        ok &= cudaMemset(c->sticky, 0, sizeof(int)) == cudaSuccess && cudaMemset(c->cand_bad, 0, sizeof(int)) == cudaSuccess;
         int map[AEV_LD];
         for (int col = 0; col < AEV_LD; ++col) map[col] = col2feat(col);
         ok &= cudaMemcpy(c->col2feat, map, sizeof(map), cudaMemcpyHostToDevice) == cudaSuccess;
@@ -264,7 +263,7 @@ int dhp_weights_load(dhp_ctx* h, const float* blob, int64_t n_floats, int n_mode
     if (e != cudaSuccess) { cudaFree(w->w.blob); delete w; return cuda_fail(c, e, "weights upload"); }
     if (mlp_tc_available(c)) {
         int rc = mlp_tc_weights(c, &w->w);
-        if (rc != DHP_OK) { cudaFree(w->w.blob); delete w; return rc; }
+        if (rc != DHP_OK) { mlp_tc_weights_free(c, &w->w); cudaFree(w->w.blob); delete w; return rc; }
     }
     *out = w;
     return DHP_OK;
@@ -288,12 +287,12 @@ int dhp_nlist_build(dhp_ctx* h, const float* pos, const float* box, const int32_
     if (rc != c->params.rcr) return DHP_E_BADARG;
     r = nlist_build(c, pos, box, species, n_atoms, mol_offsets, n_mol);
     if (r != DHP_OK) return r;
-    if (out) { g_nlist_token.owner = c; *out = &g_nlist_token; }
+    if (out) { h->nl.owner = c; *out = &h->nl; }     // the list lives in the context workspace; the handle is a per-context token
     return DHP_OK;
 }
 
 int dhp_nlist_sizes(dhp_ctx* h, const dhp_nlist* nl, int64_t* nnz, int64_t* nnz_ang) {
-    if (!h || !nl) return DHP_E_BADARG;
+    if (!h || !nl || nl->owner != &h->c) return DHP_E_BADARG;      // a list handle belongs to the context that built it
     Ctx* c = &h->c;
     const int n = (int)c->n_atoms;
     int total = 0;
@@ -316,7 +315,7 @@ int dhp_nlist_sizes(dhp_ctx* h, const dhp_nlist* nl, int64_t* nnz, int64_t* nnz_
 }
 
 int dhp_nlist_export(dhp_ctx* h, const dhp_nlist* nl, int32_t* row_ptr, int32_t* col, int32_t* row_ptr_ang, int32_t* col_ang) {
-    if (!h || !nl) return DHP_E_BADARG;
+    if (!h || !nl || nl->owner != &h->c) return DHP_E_BADARG;
     Ctx* c = &h->c;
     int r = DHP_OK;
     if (row_ptr) r = nlist_export(c, row_ptr, col, false);
@@ -383,11 +382,15 @@ int dhp_ani_energy_forces_host(dhp_ctx* h, const float* pos, const float* box, c
 int dhp_status(dhp_ctx* h) {
     if (!h) return DHP_E_BADARG;
     Ctx* c = &h->c;
-    int s = 0;
+    // the sticky word holds the first fault of any hot call since the last dhp_status(); the per-call word covers calls
+    // that end before the fold (dhp_nlist_build alone)
+    int s = 0, sticky = 0;
     cudaError_t e = cudaMemcpyAsync(&s, c->status, sizeof(int), cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&sticky, c->sticky, sizeof(int), cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->sticky, 0, sizeof(int), c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e, "status");
-    return s;
+    return sticky != 0 ? sticky : s;
 }
 
 int dhp_set_mlp_mode(dhp_ctx* h, int mode) {

@@ -37,8 +37,8 @@ constexpr int ROW_ALIGN = 2 * ROW_TILE;         // species groups start at multi
                                                 // kept equal within such a pair
 constexpr int KBLK = 64;                        // feature-block width: the unit in which zero columns are skipped
 constexpr int N_KBLK = AEV_LD / KBLK;           // 16 blocks: 14 angular (2 species pairs each) + 2 radial
-constexpr int MAX_MODELS = 8;
-constexpr int MAX_ANG = 96;                     // angular neighbours staged per centre (status CAPACITY beyond)
+constexpr int MAX_MODELS = DHP_MAX_MODELS;
+constexpr int MAX_ANG = DHP_MAX_ANG;                    // angular neighbours staged per centre (status CAPACITY beyond)
 
 // Device-side description of the cell grid, written by a setup kernel (periodic: from host box;
 // open: from the bounding box reduction) so that no hot call needs a host round trip.
@@ -106,7 +106,10 @@ struct Ctx {
     size_t zero_words;
     int* ff_arena;         // row_slot, row_species: set to -1 by one memset per hot call
     Grid* grid;
-    int* status;
+    int* status;           // status word of the CURRENT hot call (in the zero arena)
+    int* sticky;           // first fault since the last dhp_status(): survives the per-call memset, so a fault at an intermediate
+                           // step of dhp_md_run (n calls, no host sync) is still reported
+    int* cand_bad;         // device flag: a capacity fault truncated the candidate list - the next reuse call must rebuild
     unsigned* bbox;        // 6 ordered-uint min/max
     int* cell_of;          // [N] cell of caller's atom i
     int* perm_tmp;         // [N] cell-bucketed caller indices before the in-cell ordering
@@ -240,4 +243,5 @@ __host__ __device__ inline int col2feat(int c) {
 
 }  // namespace dhp
 
-struct dhp_ctx { dhp::Ctx c; };   // the opaque handle of include/dhp.h
+struct dhp_nlist { dhp::Ctx* owner; };
+struct dhp_ctx { dhp::Ctx c; dhp_nlist nl; };   // the opaque handles of include/dhp.h

@@ -105,10 +105,11 @@ __global__ void k_bbox(const float* __restrict__ pos, int n, unsigned* __restric
 
 __global__ void k_setup_grid(Grid* g, int periodic, double Lx, double Ly, double Lz, double rc,
                              const unsigned* __restrict__ bbox, int max_cells, int by_molecule, int n_mol,
-                             const int* __restrict__ gate, int* __restrict__ rebuild_count) {
+                             const int* __restrict__ gate, int* __restrict__ rebuild_count, int* __restrict__ cand_bad) {
     DHP_GATE(gate, 1);
     if (threadIdx.x || blockIdx.x) return;
     if (rebuild_count) ++*rebuild_count;
+    *cand_bad = 0;                                           // a full build starts a fresh candidate list
     const double edge = rc * (1.0 + 9.5367431640625e-07);   // rc (1 + 2^-20): binning slack
     double L[3] = {Lx, Ly, Lz};
     g->periodic = periodic;
@@ -595,14 +596,18 @@ k_pairs(const float4* __restrict__ spos, const Grid* __restrict__ gp, const int*
 }
 
 // exclusive scan of the per-256-atom block sums; total > pair_cap empties the list (status CAPACITY)
+// A capacity fault of this call (a truncated temporary or candidate row in k_pairs / k_refilter, or the overflow above)
+// also marks the candidate list as unusable (cand_bad): the next call with list reuse then rebuilds instead of
+// filtering a truncated candidate list (k_reuse_check reads the flag, a full build clears it).
 __global__ void k_scan_blocks(const int* __restrict__ blk_sum, int* __restrict__ blk_off, int nblk, int64_t pair_cap,
-                              int* __restrict__ status) {
+                              int* __restrict__ status, int* __restrict__ cand_bad) {
     block_scan_excl(blk_sum, blk_off, nblk);
     __syncthreads();
     if (threadIdx.x == 0) {
         const int ovf = (blk_off[nblk] < 0 || (int64_t)blk_off[nblk] > pair_cap) ? 1 : 0;
         if (ovf) atomicExch(status, DHP_E_CAPACITY);
         blk_off[nblk + 1] = ovf;
+        if (*(volatile int*)status == DHP_E_CAPACITY) *cand_bad = 1;
     }
 }
 
@@ -754,15 +759,19 @@ __global__ void k_set_flag(int* flag, int v) { *flag = v; }
 // the safe side), changed species, or changed its central / non-central role
 __global__ void k_reuse_check(const float* __restrict__ pos, const int* __restrict__ species, const float* __restrict__ pos_ref,
                               const float4* __restrict__ spos, const int* __restrict__ inv_perm, const uint8_t* __restrict__ central,
-                              const unsigned char* __restrict__ snc, int n, float thr2, int* __restrict__ flag) {
+                              const unsigned char* __restrict__ snc, int n, float thr2, int* __restrict__ flag,
+                              const int* __restrict__ cand_bad, const int* __restrict__ mol_offsets, const int* __restrict__ smol) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    bool bad = false;
+    bool bad = i == 0 && *cand_bad != 0;                     // the candidate list was truncated by a capacity fault
     if (i < n) {
         const float dx = pos[3 * i] - pos_ref[3 * i], dy = pos[3 * i + 1] - pos_ref[3 * i + 1], dz = pos[3 * i + 2] - pos_ref[3 * i + 2];
         const float d2 = dx * dx + dy * dy + dz * dz;
         const int slot = inv_perm[i];
         bad = !(d2 <= thr2) || species[i] != __float_as_int(spos[slot].w);      // NaN positions also force a rebuild
         if (central) bad |= (central[i] ? 0 : 1) != snc[slot];
+        // the molecule table is identified by its address on the host side; its CONTENTS are checked here: atom i must
+        // still lie in the molecule it was binned into
+        if (mol_offsets) { const int m = smol[slot]; bad |= !(mol_offsets[m] <= i && i < mol_offsets[m + 1]); }
     }
     if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) *flag = 1;
 }
@@ -1077,7 +1086,7 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
             DHP_CUDA(ctx, cudaMemsetAsync(ctx->rebuild, 0, sizeof(int), st));
             const float h = 0.5f * ctx->skin;
             DHP_LAUNCH(ctx, k_reuse_check, nb, 256, 0, pos, species, ctx->pos_ref, ctx->spos, ctx->inv_perm, central, ctx->snc, n,
-                       h * h * 0.9999f, ctx->rebuild);
+                       h * h * 0.9999f, ctx->rebuild, ctx->cand_bad, by_mol ? mol_offsets : (const int32_t*)nullptr, ctx->smol);
         } else {
             DHP_LAUNCH(ctx, k_set_flag, 1, 1, 0, ctx->rebuild, 1);
         }
@@ -1092,7 +1101,7 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
         DHP_LAUNCH(ctx, k_bbox, blocks, 256, 0, pos, n, ctx->bbox, gate);
     }
     DHP_LAUNCH(ctx, k_setup_grid, 1, 32, 0, ctx->grid, periodic ? 1 : 0, L[0], L[1], L[2], rl, ctx->bbox,
-               (int)ctx->max_cells, by_mol ? 1 : 0, n_mol, gate, skin ? ctx->rebuild_count : (int*)nullptr);
+               (int)ctx->max_cells, by_mol ? 1 : 0, n_mol, gate, skin ? ctx->rebuild_count : (int*)nullptr, ctx->cand_bad);
     DHP_LAUNCH(ctx, k_assign_cells, nb, 256, 0, pos, species, n, mol_offsets, n_mol, ctx->grid, ctx->cell_of,
                ctx->cell_count, ctx->status, gate);
     DHP_LAUNCH(ctx, k_scan_cells, 1, 1024, 0, ctx->cell_count, ctx->cell_start, ctx->grid, gate);
@@ -1132,7 +1141,7 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
         DHP_LAUNCH(ctx, k_refilter, (n + RF_WARPS - 1) / RF_WARPS, RF_WARPS * 32, 0, ctx->spos, bxa, ctx->cand, ctx->cand_cnt,
                    ctx->cand_stride, rcr2, rca2, ctx->tmp_stride, n, ctx->n_rad, ctx->tmp_col, ctx->blk_sum, ctx->status, snc, gate);
     }
-    DHP_LAUNCH(ctx, k_scan_blocks, 1, 1024, 0, ctx->blk_sum, ctx->blk_off, nblk, ctx->pair_cap, ctx->status);
+    DHP_LAUNCH(ctx, k_scan_blocks, 1, 1024, 0, ctx->blk_sum, ctx->blk_off, nblk, ctx->pair_cap, ctx->status, ctx->cand_bad);
     DHP_LAUNCH(ctx, k_rows, nblk, P2_THREADS, 0, ctx->tmp_col, ctx->tmp_stride, ctx->n_rad, ctx->blk_off, nblk, n, ctx->row_ptr,
                ctx->col, ctx->n_rad, ctx->n_ang, ctx->seg_cnt, ctx->amask, gate, ctx->rowmap, ctx->tile_mask);
     // rows grouped by species, ordered by feature-block class inside a group; tile masks

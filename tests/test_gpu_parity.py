@@ -403,3 +403,72 @@ def test_launch_counter_and_profile(torch, B, params, blob8):
     assert calls == 3 and all(v > 0 for v in ms.values())
     assert d.dhp_launch_count() - n0 >= 3 * 10
     d.close()
+
+
+def test_status_is_sticky_until_read(torch, B, params, blob8):
+    """the per-call status word is cleared at the start of every hot call, so a fault at an intermediate call
+    of an unsynchronised sequence used to be lost.  The library now folds every call's word into a sticky one that only
+    dhp_status() clears."""
+    d = B.Dhp(32, params=params)
+    w = d.dhp_weights_load(blob8[: 7 * W.PARAMS_PER_NET], 1)
+    pos = torch.zeros((4, 3), dtype=torch.float32, device="cuda")
+    pos[:, 0] = torch.arange(4) * 1.1
+    good = torch.tensor([0, 1, 2, 3], dtype=torch.int32, device="cuda")
+    bad = torch.tensor([0, 1, 9, 3], dtype=torch.int32, device="cuda")
+    d.dhp_ani_energy_forces(pos, None, good, w)
+    d.dhp_ani_energy_forces(pos, None, bad, w)           # fault in the middle of a sequence ...
+    d.dhp_ani_energy_forces(pos, None, good, w)
+    d.dhp_ani_energy_forces(pos, None, good, w)
+    assert d.dhp_status() == -4                           # ... is still reported
+    assert d.dhp_status() == 0                            # and reading clears it
+    with pytest.raises(B.DhpError):                       # the binding refuses buffers the C ABI would misread
+        d.dhp_ani_energy_forces(pos, None, good.to(torch.int64), w)
+    with pytest.raises(B.DhpError):
+        d.dhp_ani_energy_forces(pos.double(), None, good, w)
+    with pytest.raises(B.DhpError):
+        d.dhp_ani_energy_forces(torch.zeros((4, 6), dtype=torch.float32, device="cuda")[:, ::2], None, good, w)
+    d.close()
+
+
+@pytest.mark.parametrize("skin", [0.0, 1.0])
+def test_capacity_fault_in_the_middle_of_an_md_run_is_reported(torch, B, params, blob8, skin):
+    """dhp_md_run enqueues n calls without a host sync.  Atoms of infinite mass (inv_mass = 0: ballistic
+    motion) fly towards the origin; after a few outer steps every atom has more neighbours than a list row holds
+    (192), the rows are truncated and the call flags CAPACITY - which must survive to the dhp_status() after the run,
+    with and without list reuse (a truncated candidate list must also force the next call to rebuild)."""
+    rng = np.random.default_rng(12)
+    n = 420
+    pts = np.empty((0, 3))
+    while pts.shape[0] < n:                                            # ~0.1 atoms / Å^3 in a 10 Å sphere
+        c = rng.uniform(-10, 10, 3)
+        if np.linalg.norm(c) <= 10 and (pts.shape[0] == 0 or np.linalg.norm(pts - c, axis=1).min() >= 1.2):
+            pts = np.concatenate([pts, c[None]])
+    pos0 = pts.astype(np.float32)
+    sp = rng.integers(0, 4, n).astype(np.int32)
+    vel0 = (-0.16 * pts).astype(np.float32)                            # Å/fs, towards the origin
+    d = B.Dhp(n, params=params)
+    w = d.dhp_weights_load(blob8[: 7 * W.PARAMS_PER_NET], 1)
+    if skin:
+        d.dhp_set_skin(skin)
+    md = d.dhp_md_create(np.zeros(n, np.float32))
+    pos, vel = torch.from_numpy(pos0.copy()).cuda(), torch.from_numpy(vel0.copy()).cuda()
+    spd = torch.from_numpy(sp).cuda()
+    # ballistic: r(t) = r0 (1 - 0.16 t / fs).  2 steps: scale 0.84, ~95 neighbours per atom - no fault yet
+    d.dhp_md_run(md, pos, vel, None, spd, w, 0.5, 1, 2)
+    assert d.dhp_status() == 0                                         # and the sticky word stays clear
+    d.dhp_md_run(md, pos, vel, None, spd, w, 0.5, 1, 5)                # scale 0.44: ~12 x the density, rows overflow
+    # expand again so that the LAST calls of the sequence are clean: only the sticky word can know about the fault
+    vel.mul_(-1.0)
+    d.dhp_md_run(md, pos, vel, None, spd, w, 0.5, 1, 7)
+    E_last, F_last = d.dhp_ani_energy_forces(pos, None, spd, w)
+    torch.cuda.synchronize()
+    assert d.dhp_status() == -2
+    assert d.dhp_status() == 0
+    # and the state after the fault is sound: the list of the final (dilute again) positions is the canonical one
+    d.dhp_nlist_build(pos, None, spd)
+    rp, col, _, _ = d.dhp_nlist_export()
+    rpo, colo = oracle.pairs(pos.cpu().numpy(), None, params.rcr)
+    assert csr_equal(rp, col, rpo, colo)
+    assert d.dhp_status() == 0
+    d.dhp_md_destroy(md)
+    d.close()
