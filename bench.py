@@ -9,7 +9,8 @@ configs[3], the 98 000-atom biosystem the north_star targets are quoted on.  Pri
 
   value   atoms*evals/s, inputs resident in HBM, CUDA events over exactly K steps, max over ranks
   e2e     same metric through dhp_ani_energy_forces_host: pinned host buffers, H2D + D2H inside
-  roofline  the dominant kernel (k_mlp_mid, tensor-bound): algorithmic FLOPs / device time vs measured sustained bf16 peak
+  roofline  the dominant kernel (k_mlp_mid, tensor-bound): algorithmic FLOPs / device time of the timed (burst) loop vs the
+            measured BURST bf16 peak; `frac` counts a product once, `issued_frac` the 3 MMAs issued per product
   roofline_mlp_phase / roofline_kernels   the same for the whole MLP phase and for every kernel group (HBM-bound ones vs copy bandwidth)
   cpu_baseline  the fp64 oracle, as it stands, on a bounded sample of the same workload (rank 0, N=1)
   parity_sample  that oracle sample against dhp_ani_energy_forces_partial over the same central atoms (|dE|/n, max |dF|)
@@ -39,10 +40,25 @@ from paper_2207_14276_b200 import workloads as W  # noqa: E402
 METRIC = "ani_energy_forces_atoms_evals_per_s"
 UNIT = "atoms*evals/s"
 NS_PER_DAY_PER_EVAL_PER_S = 0.5e-6 * 86400.0      # 0.5 fs step
-# DRAM bytes (read + write) per launch at configs[3], from the committed ncu --set full captures of this command
-# (profiles/r1g_ncu_full_summary.txt)
-TRAFFIC_98K = {"g1": 0.18217e9 + 0.75396e9, "mid": 0.86862e9 + 0.77926e9, "b1": 0.84906e9 + 0.09946e9,
-               "aev_fwd": 0.02731e9 + 0.05850e9, "aev_bwd": 0.11341e9 + 0.00377e9, "nlist": 0.00235e9 + 0.00075e9 + 0.02705e9 + 0.00006e9}
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r2_traffic_98k.csv")
+
+
+def traffic_98k():
+    """DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per launch at configs[3], read from the committed summary of
+    the `ncu --set full` capture of this same command (profiles/r2_traffic_98k.csv; the README beside it names the command
+    and the commit it was taken at).  Returns {} when the file is missing: `traffic` is then null, never a stale constant."""
+    out = {}
+    try:
+        with open(TRAFFIC_FILE) as f:
+            for line in f:
+                line = line.strip()
+                if not line or line.startswith("#") or line.startswith("key,"):
+                    continue
+                key, rd, wr = line.split(",")[:3]
+                out[key] = out.get(key, 0.0) + float(rd) + float(wr)
+    except OSError:
+        pass
+    return out
 
 
 def peaks():
@@ -269,16 +285,25 @@ def main():
         if rank == 0:
             s2.start()
         barrier()
+        d.dhp_profile_enable(True)
+        d.dhp_profile_reset()
         ev0.record(stream)
         for k in range(n_sus):
             step(k)
         ev1.record(stream)
         barrier()
         ms_sus = ev0.elapsed_time(ev1) / n_sus
+        ph_sus, calls_sus = d.dhp_profile_read()
+        d.dhp_profile_enable(False)
         if rank == 0:
             c2 = s2.stop()
-            sustained = {"ms_per_step": ms_sus, "steps": n_sus, "sm_mhz": c2["sm_mhz"], "reasons": c2["reasons"],
-                         "power_w": getattr(s2, "power_w", None), "samples": c2.get("samples")}
+            atoms_s = system.n_atoms * (1 if slab else world)
+            sustained = {"ms_per_step": ms_sus, "steps": n_sus, "value": atoms_s / (ms_sus * 1e-3), "unit": UNIT,
+                         "ns_per_day_at_0.5fs": NS_PER_DAY_PER_EVAL_PER_S / (ms_sus * 1e-3),
+                         "phase_ms": {k: v / max(calls_sus, 1) for k, v in ph_sus.items()},
+                         "sm_mhz": c2["sm_mhz"], "reasons": c2["reasons"],
+                         "power_w": getattr(s2, "power_w", None), "samples": c2.get("samples"),
+                         "note": "steady state of a long run (board power management settled): the number an MD run gets"}
 
     # ---- energy-only call (a1-a3), same inputs, device-resident ---------------------------------
     for k in range(3):
@@ -366,50 +391,74 @@ def main():
         ph["mlp"] = ph["mlp_g1"] + ph["mlp_mid"] + ph["mlp_b1"]
         N, M = system.n_atoms, system.n_models
         passes = (1 if args.mlp == "fp16" else 3) if tensor_path else 1
-        peak_t = pk["bf16_tflops_sustained"]
-        # algorithmic FLOPs (forward + input gradient) per atom and network, by kernel
-        f_g1 = 2.0 * 1008 * 256
+        # The timed region is a burst (K steps, ~50 ms at the default K = 20): the phase times are divided by the BURST bf16
+        # peak.  The ~1 s `sustained` loop below carries its own phase times and is divided by the SUSTAINED peak.
+        peak_t, peak_kind = pk["bf16_tflops"], "burst"
+        # algorithmic FLOPs (forward + input gradient) per atom and network, by kernel; one product = one multiply-add
+        f_g1_dense = 2.0 * 1008 * 256
         f_mid = 2.0 * (256 * 192 + 192 * 160 + 160 + 160 * 192 + 192 * 256)
-        f_b1 = 2.0 * 256 * 1008
-        # MMAs actually issued: 3 passes; G1 visits / B1 produces only the active 64-wide feature blocks of a tile
-        rows_pad = 128.0 * n_row_tiles
+        # G1 visits / B1 produces only the 64-wide feature blocks that are non-zero for the row tile: the zero blocks are
+        # not work of the method (absent neighbour species), so the ALGORITHMIC count is over the active blocks only; the
+        # dense-K figure is reported under its own key
+        rows_pad = 128.0 * max(n_row_tiles, 1)
+        act = n_active_blocks / max(n_row_tiles, 1)                        # active blocks per tile (of 16)
+        f_g1 = 2.0 * 64 * 256 * act                                        # per atom and network
+        # MMAs actually issued (3 passes per product, padded rows included)
         i_g1 = passes * 2.0 * M * 128.0 * 64 * 256 * n_active_blocks
         i_mid = passes * 2.0 * M * rows_pad * (256 * 192 + 192 * 160 + 160 * 192 + 192 * 256)
 
-        def tensor_entry(name, ms, alg_flop, issued_flop, traffic):
+        def tensor_entry(name, ms, alg_flop, issued_flop, traffic, dense_flop=None, peak=None, kind=None):
+            peak = peak or peak_t
             ach = alg_flop / (ms * 1e-3) / 1e12
-            return {"kernel": name, "bound": "tensor", "achieved": ach, "peak": peak_t, "unit": "TFLOP/s", "frac": ach / peak_t,
-                    "traffic": traffic, "ms_per_launch": ms, "algorithmic_flop_per_launch": alg_flop,
-                    "issued_tflops": issued_flop / (ms * 1e-3) / 1e12, "issued_frac": issued_flop / (ms * 1e-3) / 1e12 / peak_t}
+            e = {"kernel": name, "bound": "tensor", "achieved": ach, "peak": peak, "peak_kind": kind or peak_kind, "unit": "TFLOP/s",
+                 "frac": ach / peak, "traffic": traffic, "ms_per_launch": ms, "algorithmic_flop_per_launch": alg_flop,
+                 "issued_tflops": issued_flop / (ms * 1e-3) / 1e12, "issued_frac": issued_flop / (ms * 1e-3) / 1e12 / peak}
+            if dense_flop is not None:
+                e["dense_k_tflops"] = dense_flop / (ms * 1e-3) / 1e12     # counts the skipped zero blocks: NOT a utilisation
+            return e
 
-        def hbm_entry(name, ms, bytes_per_atom, traffic, note):
+        def hbm_entry(name, ms, bytes_per_atom, traffic, note, floor_us=None):
             ach = bytes_per_atom * N / (ms * 1e-3) / 1e9
-            return {"kernel": name, "bound": "hbm", "achieved": ach, "peak": pk["hbm_gbs"], "unit": "GB/s",
-                    "frac": ach / pk["hbm_gbs"], "traffic": traffic, "ms_per_launch": ms,
-                    "algorithmic_bytes_per_launch": bytes_per_atom * N, "note": note}
+            e = {"kernel": name, "bound": "hbm", "achieved": ach, "peak": pk["hbm_gbs"], "unit": "GB/s",
+                 "frac": ach / pk["hbm_gbs"], "traffic": traffic, "ms_per_launch": ms,
+                 "algorithmic_bytes_per_launch": bytes_per_atom * N, "note": note}
+            if floor_us is not None:                                      # the kernel's real floor is arithmetic, not bytes
+                e["arithmetic_floor_us"] = floor_us
+                e["time_over_arithmetic_floor"] = ms * 1e3 / floor_us
+            return e
 
-        # `traffic`: dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures of
-        # this same command (profiles/r1d_ncu_full_summary.txt for the MLP kernels, r1c for the others); configs[3] only
-        tr = TRAFFIC_98K if (args.config == 4 and tensor_path) else {}
+        tr = traffic_98k() if (args.config == 4 and tensor_path) else {}
+        scale_n = N / 98000.0
         kernels = []
         if tensor_path:
-            kernels += [tensor_entry("k_gemm_tc<CELU,K-skip> (G1: AEV -> h1)", ph["mlp_g1"], f_g1 * M * N, i_g1, tr.get("g1")),
+            kernels += [tensor_entry("k_gemm_tc<CELU,K-skip> (G1: AEV -> h1)", ph["mlp_g1"], f_g1 * M * N, i_g1, tr.get("g1"), f_g1_dense * M * N),
                         tensor_entry("k_mlp_mid (G2+G3+out+B3+B2 fused: h1 -> E_i, d1)", ph["mlp_mid"], f_mid * M * N, i_mid, tr.get("mid")),
-                        tensor_entry("k_gemm_tc<GRAD,N-skip> (B1: d1 -> dE/dAEV) + energy reduction", ph["mlp_b1"], f_b1 * M * N, i_g1, tr.get("b1"))]
-        kernels += [hbm_entry("nlist (a1: all kernels)", ph["nlist"], 264.0, tr.get("nlist"), "working set is L2-resident; instruction-bound"),
-                    hbm_entry("k_aev_fwd (a2)", ph["aev_fwd"], 4256.0, tr.get("aev_fwd"), "issue-bound (2.6 k warp instructions per atom, 79 % of the issue slots)"),
-                    hbm_entry("k_aev_bwd + k_unsort_forces (a5)", ph["aev_bwd"], 4268.0, tr.get("aev_bwd"), "issue-bound")]
+                        tensor_entry("k_gemm_tc<GRAD,N-skip> (B1: d1 -> dE/dAEV) + energy reduction", ph["mlp_b1"], f_g1 * M * N, i_g1, tr.get("b1"),
+                                     f_g1_dense * M * N)]
+        # arithmetic floors at configs[3]: a1 386 candidate tests x ~12 fp64 ops per atom; a2 3.3 k MUFU
+        # ops per atom at 16 / clk / SM; a5 about twice a2's arithmetic
+        kernels += [hbm_entry("nlist (a1: all kernels)", ph["nlist"], 264.0, tr.get("nlist"), "working set is L2-resident; instruction-bound",
+                              11.0 * scale_n),
+                    hbm_entry("k_aev_fwd (a2)", ph["aev_fwd"], 4256.0, tr.get("aev_fwd"), "issue-bound; the floor that binds is MUFU, not HBM", 69.0 * scale_n),
+                    hbm_entry("k_aev_bwd + k_unsort_forces (a5)", ph["aev_bwd"], 4268.0, tr.get("aev_bwd"), "issue-bound", 140.0 * scale_n)]
         if tensor_path:
             roof = dict(max(kernels[:3], key=lambda k: k["ms_per_launch"]))          # the dominant kernel of the step
-            roof["peak_source"] = f"{pk['source']} sustained bf16 (fp16 operands, same rate)"
+            roof["peak_source"] = f"{pk['source']} {peak_kind} bf16 peak (fp16 operands, same rate); the timed loop is a burst"
             roof["arithmetic"] = ("fp16 operands, 1 tcgen05 MMA per product, fp32 accumulate (opt-in mixed precision, outside the parity bar)"
-                                  if args.mlp == "fp16" else "fp16 two-term split, 3 tcgen05 MMAs per product, fp32 accumulate")
-            mlp_phase = tensor_entry("MLP phase (G1 + k_mlp_mid + B1)", ph["mlp"], (f_g1 + f_mid + f_b1) * M * N, 2 * i_g1 + i_mid,
-                                     sum(tr.values()) if {"g1", "mid", "b1"} <= set(tr) else None)
-            mlp_phase["traffic"] = (tr["g1"] + tr["mid"] + tr["b1"]) if {"g1", "mid", "b1"} <= set(tr) else None
-            mlp_phase.update({"row_tiles": n_row_tiles, "active_feature_blocks_per_tile": n_active_blocks / max(n_row_tiles, 1)})
+                                  if args.mlp == "fp16" else "fp16 two-term split, 3 tcgen05 MMAs per product, fp32 accumulate: `frac` counts one "
+                                  "product once (ceiling 1/3), `issued_frac` counts the MMAs issued")
+            tsum = (tr["g1"] + tr["mid"] + tr["b1"]) if {"g1", "mid", "b1"} <= set(tr) else None
+            mlp_phase = tensor_entry("MLP phase (G1 + k_mlp_mid + B1)", ph["mlp"], (2 * f_g1 + f_mid) * M * N, 2 * i_g1 + i_mid, tsum,
+                                     (2 * f_g1_dense + f_mid) * M * N)
+            mlp_phase.update({"row_tiles": n_row_tiles, "active_feature_blocks_per_tile": act})
+            if sustained is not None and sustained.get("phase_ms"):
+                sp = sustained["phase_ms"]
+                sustained["roofline"] = tensor_entry(roof["kernel"], sp["mlp_mid"] if "k_mlp_mid" in roof["kernel"] else sp["mlp_g1"],
+                                                     roof["algorithmic_flop_per_launch"],
+                                                     roof["issued_tflops"] * roof["ms_per_launch"] * 1e9, roof["traffic"],
+                                                     peak=pk["bf16_tflops_sustained"], kind="sustained")
         else:
-            flops = (f_g1 + f_mid + f_b1) * M * N
+            flops = (2 * f_g1_dense + f_mid) * M * N
             roof = tensor_entry("mlp_simt (fp32 FFMA scaffold; tensor path not in use)", ph["mlp"], flops, flops, None)
             mlp_phase = roof
         out = {

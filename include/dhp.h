@@ -205,6 +205,19 @@ int dhp_md_reset(dhp_ctx* ctx, dhp_md* md);
 int dhp_md_run(dhp_ctx* ctx, dhp_md* md, float* pos, float* vel, const float* box, const int32_t* species,
                const dhp_weights* weights, int n_models, float dt, int n_inner, int n_steps, double* E_out);
 
+/* One outer step of the same scheme, split at the slow-force evaluation and restricted to the atoms [lo, hi) that a rank
+ * OWNS - the building blocks of the multi-GPU MD loop (domain decomposition):
+ *   dhp_md_open   v += (dt/2) a_slow ; [ v += (d/2) a_fast ; x += d v ; v += (d/2) a_fast ]^n_inner   for atoms [lo, hi)
+ *   ... the caller all-gathers the new positions, evaluates its partial slow force with
+ *       dhp_ani_energy_forces_partial and reduce-scatters it (paper_2207_14276_b200/shard.py) ...
+ *   dhp_md_close  v += (dt/2) a_slow                                                               for atoms [lo, hi)
+ * F_slow: dev fp32 [n_atoms][3], the TOTAL slow force; only rows [lo, hi) are read.  The md handle must have been
+ * created with the bonds whose two atoms both lie in [lo, hi) (ranges are cut at molecule boundaries).  pos / vel are
+ * the full [n_atoms][3] arrays; only rows [lo, hi) are written.  Asynchronous.  Errors: BADARG. */
+int dhp_md_open(dhp_ctx* ctx, dhp_md* md, float* pos, float* vel, const float* box, const float* F_slow, float dt,
+                int n_inner, int64_t lo, int64_t hi);
+int dhp_md_close(dhp_ctx* ctx, dhp_md* md, float* vel, const float* F_slow, float dt, int n_inner, int64_t lo, int64_t hi);
+
 /* Same computation with HOST buffers (pos, species, mol_offsets, E, F all host; pinned memory makes
  * the copies asynchronous): host->device copies, the kernels, device->host copies and one stream
  * synchronisation all happen inside the call.  This is the end-to-end entry point bench.py times. */

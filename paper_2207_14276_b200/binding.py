@@ -41,6 +41,8 @@ SYMBOLS = {
     "dhp_md_destroy": (C.c_int, [_vp, _vp]),
     "dhp_md_reset": (C.c_int, [_vp, _vp]),
     "dhp_md_run": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _i32, _f32, _i32, _i32, _vp]),
+    "dhp_md_open": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _f32, _i32, _i64, _i64]),
+    "dhp_md_close": (C.c_int, [_vp, _vp, _vp, _vp, _f32, _i32, _i64, _i64]),
     "dhp_status": (C.c_int, [_vp]),
     "dhp_set_mlp_mode": (C.c_int, [_vp, _i32]),
     "dhp_tensor_path_available": (C.c_int, [_vp]),
@@ -333,6 +335,17 @@ class Dhp:
                                    _vp(_dptr(E_out))), self.ctx)
         self._n = int(pos.shape[0])
         return E_out
+
+    def dhp_md_open(self, md, pos, vel, box, F_slow, dt: float, n_inner: int, lo: int, hi: int):
+        """First half kick + inner loop for the owned atoms [lo, hi) (in place on the cuda tensors pos, vel)."""
+        boxh = None if box is None else np.ascontiguousarray(box, dtype=np.float32)
+        _check(self.lib.dhp_md_open(self.ctx, md, _vp(_dptr(pos)), _vp(_dptr(vel)), _vp(_dptr(boxh)), _vp(_dptr(F_slow)),
+                                    C.c_float(float(dt)), int(n_inner), int(lo), int(hi)), self.ctx)
+
+    def dhp_md_close(self, md, vel, F_slow, dt: float, n_inner: int, lo: int, hi: int):
+        """Second half kick for the owned atoms [lo, hi)."""
+        _check(self.lib.dhp_md_close(self.ctx, md, _vp(_dptr(vel)), _vp(_dptr(F_slow)), C.c_float(float(dt)), int(n_inner),
+                                     int(lo), int(hi)), self.ctx)
 
     def dhp_status(self) -> int:
         return int(self.lib.dhp_status(self.ctx))

@@ -31,8 +31,8 @@ struct Md {
 // v += inv_m (ca Fa + cb Fb); optionally x += delta v
 __global__ void k_md_kick_drift(float* __restrict__ pos, float* __restrict__ vel, const float* __restrict__ inv_mass,
                                 const float* __restrict__ Fa, float ca, const float* __restrict__ Fb, float cb, float delta,
-                                int n3) {
-    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+                                int n3, int t0 = 0) {
+    const int t = t0 + blockIdx.x * blockDim.x + threadIdx.x;      // components [t0, n3): all atoms, or the range a rank owns
     if (t >= n3) return;
     float f = 0.f;
     if (Fa) f = ca * Fa[t];
@@ -177,6 +177,51 @@ int dhp_md_run(dhp_ctx* h, dhp_md* md, float* pos, float* vel, const float* box,
         DHP_LAUNCH(c, k_md_kinetic, 2 * c->sm_count, 256, 0, vel, m->inv_mass, (int)n, m->e + 2);
         DHP_CUDA(c, cudaMemcpyAsync(E_out, m->e, sizeof(double) * 3, cudaMemcpyDeviceToDevice, c->stream));
     }
+    DHP_CUDA(c, cudaGetLastError());
+    return DHP_OK;
+}
+
+// ---- one outer step split at the slow-force evaluation, over the atoms [lo, hi) a rank owns (multi-GPU decomposition,
+// PAPER.md L134 / L194): dhp_md_open = first half kick with the slow force + the whole inner loop (the
+// rank's own bonds: both atoms of every bond of this md handle must lie in [lo, hi)), dhp_md_close = second half kick.
+// Between the two the caller all-gathers the positions, evaluates its partial slow force (dhp_ani_energy_forces_partial)
+// and reduce-scatters it (paper_2207_14276_b200/shard.py).  F_slow is dev fp32 [n_atoms][3]; only rows [lo, hi) are read.
+int dhp_md_open(dhp_ctx* h, dhp_md* md, float* pos, float* vel, const float* box, const float* F_slow, float dt, int n_inner,
+                int64_t lo, int64_t hi) {
+    if (!h || !md || !pos || !vel || !F_slow || n_inner < 1 || !(dt > 0.f)) return DHP_E_BADARG;
+    Ctx* c = &h->c;
+    Md* m = &md->m;
+    if (lo < 0 || hi < lo || hi > m->n_atoms) return DHP_E_BADARG;
+    if (hi == lo) return DHP_OK;
+    const int t0 = (int)(3 * lo), t1 = (int)(3 * hi), nb = (t1 - t0 + 255) / 256;
+    const float* ff = m->n_bonds > 0 ? m->f_fast : nullptr;
+    if (m->n_bonds == 0) n_inner = 1;
+    const float d = dt / (float)n_inner;
+    int rc;
+    if (!m->primed) {                                    // fast force at the starting positions
+        if ((rc = fast_forces(c, m, pos, box)) != DHP_OK) return rc;
+        m->primed = true;
+    }
+    for (int k = 0; k < n_inner; ++k) {
+        DHP_LAUNCH(c, k_md_kick_drift, nb, 256, 0, pos, vel, m->inv_mass, k == 0 ? F_slow : (const float*)nullptr, 0.5f * dt, ff,
+                   k == 0 ? 0.5f * d : d, d, t1, t0);
+        if ((rc = fast_forces(c, m, pos, box)) != DHP_OK) return rc;
+    }
+    DHP_CUDA(c, cudaGetLastError());
+    return DHP_OK;
+}
+
+int dhp_md_close(dhp_ctx* h, dhp_md* md, float* vel, const float* F_slow, float dt, int n_inner, int64_t lo, int64_t hi) {
+    if (!h || !md || !vel || !F_slow || n_inner < 1 || !(dt > 0.f)) return DHP_E_BADARG;
+    Ctx* c = &h->c;
+    Md* m = &md->m;
+    if (lo < 0 || hi < lo || hi > m->n_atoms) return DHP_E_BADARG;
+    if (hi == lo) return DHP_OK;
+    const int t0 = (int)(3 * lo), t1 = (int)(3 * hi), nb = (t1 - t0 + 255) / 256;
+    const float* ff = m->n_bonds > 0 ? m->f_fast : nullptr;
+    if (m->n_bonds == 0) n_inner = 1;
+    const float d = dt / (float)n_inner;
+    DHP_LAUNCH(c, k_md_kick_drift, nb, 256, 0, (float*)nullptr, vel, m->inv_mass, F_slow, 0.5f * dt, ff, 0.5f * d, 0.f, t1, t0);
     DHP_CUDA(c, cudaGetLastError());
     return DHP_OK;
 }

@@ -127,3 +127,141 @@ def ani_energy_forces_sharded(dhp, pos, box, species, weights, central, mol_offs
         dist.all_reduce(F, op=dist.ReduceOp.SUM, group=group)
         dist.all_reduce(E, op=dist.ReduceOp.SUM, group=group)
     return E, F
+
+
+# ---- the exchange SURVEY.md §8(e) specifies: all-gather of owned positions, reduce-scatter of partial forces ----------
+def owner_bounds(n_atoms: int, world: int, unit: int = 1, first_unit_atom: int = 0) -> np.ndarray:
+    """Index ranges of the atoms each rank OWNS for integration: [bounds[r], bounds[r+1]).  Ownership is by atom index
+    (fixed for a run - it decides who integrates an atom and who receives its total force), independent of the spatial
+    slabs that decide who evaluates an atom as a CENTRE.  Cuts fall on multiples of `unit` atoms counted from
+    `first_unit_atom` (3 for the waters of the generators, so that no O-H bond is split between two ranks)."""
+    b = np.empty(world + 1, dtype=np.int64)
+    b[0], b[world] = 0, n_atoms
+    for r in range(1, world):
+        cut = shard_range(n_atoms, world, r)[0]
+        if unit > 1 and cut > first_unit_atom:
+            cut = first_unit_atom + (cut - first_unit_atom) // unit * unit
+        b[r] = cut
+    if np.any(np.diff(b) < 0):
+        raise ValueError("bad ownership bounds")
+    return b
+
+
+class Exchange:
+    """Padded layout for collectives with equal chunks: rank r's atoms [bounds[r], bounds[r+1]) occupy rows
+    [r * chunk, r * chunk + len_r) of a [world * chunk, 3] buffer.  Index arithmetic and torch.distributed calls only."""
+
+    def __init__(self, bounds, device, group=None):
+        import torch
+        import torch.distributed as dist
+        self.torch, self.dist, self.group = torch, dist, group
+        self.bounds = np.asarray(bounds, dtype=np.int64)
+        self.world = int(self.bounds.size - 1)
+        self.n = int(self.bounds[-1])
+        self.chunk = int(max(1, np.diff(self.bounds).max()))
+        self.rank = dist.get_rank(group) if (dist.is_available() and dist.is_initialized()) else 0
+        live = self.world > 1 and dist.is_available() and dist.is_initialized()
+        self.live = live
+        self.backend = dist.get_backend(group) if live else None
+        to_pad = np.full(self.world * self.chunk, self.n, dtype=np.int64)          # padding rows read the extra zero row
+        to_atom = np.empty(self.n, dtype=np.int64)
+        for r in range(self.world):
+            lo, hi = int(self.bounds[r]), int(self.bounds[r + 1])
+            to_pad[r * self.chunk: r * self.chunk + hi - lo] = np.arange(lo, hi)
+            to_atom[lo:hi] = r * self.chunk + np.arange(hi - lo)
+        self.to_pad = torch.from_numpy(to_pad).to(device)
+        self.to_atom = torch.from_numpy(to_atom).to(device)
+        self.lo, self.hi = int(self.bounds[self.rank]), int(self.bounds[self.rank + 1])
+
+    def reduce_scatter_forces(self, F_partial, F_total):
+        """F_total[lo:hi] = sum over ranks of F_partial[lo:hi] (the rows this rank owns); other rows are left alone.
+        NCCL: one reduce-scatter of the padded buffer (1.2 MB / world per rank at 98 k atoms); gloo (CPU tests) has no
+        reduce-scatter, there the same result comes from an all-reduce and a slice."""
+        t = self.torch
+        if not self.live:
+            F_total[self.lo:self.hi] = F_partial[self.lo:self.hi]
+            return F_total
+        src = t.cat([F_partial, t.zeros((1, 3), dtype=F_partial.dtype, device=F_partial.device)])[self.to_pad]
+        if self.backend == "nccl":
+            out = t.empty((self.chunk, 3), dtype=F_partial.dtype, device=F_partial.device)
+            self.dist.reduce_scatter_tensor(out, src, op=self.dist.ReduceOp.SUM, group=self.group)
+        else:
+            self.dist.all_reduce(src, op=self.dist.ReduceOp.SUM, group=self.group)
+            out = src[self.rank * self.chunk:(self.rank + 1) * self.chunk]
+        F_total[self.lo:self.hi] = out[: self.hi - self.lo]
+        return F_total
+
+    def all_gather_positions(self, pos):
+        """Every rank has integrated its own rows of `pos` [N, 3]; afterwards every rank holds all rows (in place)."""
+        t = self.torch
+        if not self.live:
+            return pos
+        mine = t.zeros((self.chunk, 3), dtype=pos.dtype, device=pos.device)
+        mine[: self.hi - self.lo] = pos[self.lo:self.hi]
+        full = t.empty((self.world * self.chunk, 3), dtype=pos.dtype, device=pos.device)
+        self.dist.all_gather_into_tensor(full, mine, group=self.group)
+        pos.copy_(full[self.to_atom])
+        return pos
+
+    def all_reduce_energy(self, E):
+        if self.live:
+            self.dist.all_reduce(E, op=self.dist.ReduceOp.SUM, group=self.group)
+        return E
+
+
+class ShardedMd:
+    """The multiple-timestep driver over `world` ranks.
+
+    Every rank owns an index range of atoms (it integrates them) and, per evaluation, a spatial slab of CENTRAL atoms (it
+    evaluates their atomic energies and the forces they exert).  One outer step:
+        dhp_md_open   (own atoms: half kick with the slow force, inner loop with the own bonds)
+        all-gather    positions
+        dhp_ani_energy_forces_partial over the own slab (mask refreshed every `mask_every` steps: the argsort is on the
+                      list-rebuild cadence, not on every step)
+        reduce-scatter of the partial forces -> total slow force of the own atoms; all-reduce of E (8 bytes)
+        dhp_md_close  (own atoms: second half kick)
+    `dhp` is a binding.Dhp (or, in the CPU tests, a stand-in with the same four methods)."""
+
+    def __init__(self, dhp, weights, species, box, bounds, inv_mass, bonds=None, bond_k=None, bond_r0=None,
+                 mask_every: int = 10, group=None, dtype=None):
+        import torch
+        self.torch = torch
+        self.dhp, self.weights, self.species, self.box = dhp, weights, species, box
+        self.ex = Exchange(bounds, species.device, group)
+        lo, hi = self.ex.lo, self.ex.hi
+        if bonds is not None and len(bonds):
+            b = np.asarray(bonds)
+            own = (b[:, 0] >= lo) & (b[:, 0] < hi)
+            if np.any(own != ((b[:, 1] >= lo) & (b[:, 1] < hi))):
+                raise ValueError("a bond is split between two ranks: cut the ownership ranges at molecule boundaries")
+            bonds, bond_k, bond_r0 = b[own], np.asarray(bond_k)[own], np.asarray(bond_r0)[own]
+        self.md = dhp.dhp_md_create(inv_mass, bonds if bonds is not None and len(bonds) else None,
+                                    bond_k if bonds is not None and len(bonds) else None,
+                                    bond_r0 if bonds is not None and len(bonds) else None)
+        self.mask_every, self.steps_since_mask, self.mask = int(mask_every), 0, None
+        self.F_total = torch.zeros((self.ex.n, 3), dtype=dtype or torch.float32, device=species.device)
+        self.E = None
+        self.primed = False
+
+    def _slow(self, pos):
+        if self.mask is None or self.steps_since_mask >= self.mask_every:
+            self.mask = slab_mask_device(pos, self.box, self.ex.world, self.ex.rank)
+            self.steps_since_mask = 0
+        self.steps_since_mask += 1
+        E, F = self.dhp.dhp_ani_energy_forces_partial(pos, self.box, self.species, self.weights, self.mask)
+        self.ex.reduce_scatter_forces(F, self.F_total)
+        self.E = self.ex.all_reduce_energy(E)
+
+    def run(self, pos, vel, dt: float, n_inner: int, n_steps: int):
+        """`n_steps` outer steps in place on pos / vel [N, 3] (all rows of pos are current on every rank on return; only
+        the own rows of vel are).  Returns the total E_ANI at the final positions (identical on every rank)."""
+        lo, hi = self.ex.lo, self.ex.hi
+        if not self.primed:
+            self._slow(pos)
+            self.primed = True
+        for _ in range(n_steps):
+            self.dhp.dhp_md_open(self.md, pos, vel, self.box, self.F_total, dt, n_inner, lo, hi)
+            self.ex.all_gather_positions(pos)
+            self._slow(pos)
+            self.dhp.dhp_md_close(self.md, vel, self.F_total, dt, n_inner, lo, hi)
+        return self.E

@@ -165,3 +165,45 @@ def test_argument_errors_of_the_driver_and_the_skin(torch, B, params):
     assert np.isfinite(E.cpu().numpy()).all() and np.array_equal(pos.cpu().numpy(), s.pos)
     d.dhp_md_destroy(h)
     d.close()
+
+
+def test_sharded_driver_on_one_rank_equals_the_oracle_trajectory(torch, B, params):
+    """shard.ShardedMd (dhp_md_open -> all-gather -> dhp_ani_energy_forces_partial over the own slab -> reduce-scatter ->
+    dhp_md_close) on the one GPU there is: world size 1 takes the same code path with the collectives
+    reduced to copies, and must reproduce the oracle trajectory like dhp_md_run does.  (World size 2 runs on gloo with an
+    oracle-backed stand-in: tests/test_shard_gloo.py.)"""
+    from paper_2207_14276_b200 import shard
+    s = W.make_system(1)
+    md = W.md_inputs(s)
+    blob = W.make_weights(1)
+    d = B.Dhp(s.n_atoms, params=params)
+    w = d.dhp_weights_load(blob, 1)
+    pos = torch.from_numpy(s.pos.copy()).cuda()
+    vel = torch.from_numpy(md.vel.copy()).cuda()
+    sp = torch.from_numpy(s.species).cuda()
+    drv = shard.ShardedMd(d, w, sp, s.box, shard.owner_bounds(s.n_atoms, 1, unit=3), md.inv_mass, md.bonds, md.bond_k, md.bond_r0,
+                          mask_every=2)
+    E = drv.run(pos, vel, 0.5, 2, 3)
+    E = drv.run(pos, vel, 0.5, 2, 2)
+    torch.cuda.synchronize()
+    assert d.dhp_status() == 0
+    xo, vo, (Es, _, _) = oracle_run(s, md, params, blob, 0.5, 2, 5)
+    assert np.max(np.abs(pos.cpu().numpy() - xo)) <= X_TOL and np.max(np.abs(vel.cpu().numpy() - vo)) <= V_TOL
+    assert abs(E.item() - Es) / s.n_atoms <= 1e-6
+    # an owned sub-range: only those rows move
+    pos2 = torch.from_numpy(s.pos.copy()).cuda()
+    vel2 = torch.from_numpy(md.vel.copy()).cuda()
+    h = d.dhp_md_create(md.inv_mass)
+    F = torch.randn((s.n_atoms, 3), device="cuda")
+    d.dhp_md_open(h, pos2, vel2, s.box, F, 0.5, 1, 30, 90)
+    d.dhp_md_close(h, vel2, F, 0.5, 1, 30, 90)
+    torch.cuda.synchronize()
+    moved = np.nonzero(np.abs(pos2.cpu().numpy() - s.pos).sum(1))[0]
+    assert moved.min() == 30 and moved.max() == 89
+    dv = vel2.cpu().numpy() - md.vel
+    assert np.all(dv[:30] == 0) and np.all(dv[90:] == 0)
+    assert np.allclose(dv[30:90], 0.5 * md.inv_mass[30:90, None] * F.cpu().numpy()[30:90], rtol=1e-5, atol=1e-9)
+    with pytest.raises(B.DhpError):
+        d.dhp_md_open(h, pos2, vel2, s.box, F, 0.5, 1, 90, 30)
+    d.dhp_md_destroy(h)
+    d.close()

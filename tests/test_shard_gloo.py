@@ -131,3 +131,129 @@ def test_world2_gloo_sharded_results_equal_single_process():
     assert abs(E_sum[0] - Ew[0]) <= 1e-10
     assert np.max(np.abs(F_sum - Fw)) <= 1e-12
     assert t == [2.0, 5.0]
+
+
+# ---- the exchange of SURVEY.md §8(e) and the sharded multiple-timestep step ---------------------------------------------
+def test_owner_bounds_cut_at_molecule_boundaries():
+    b = shard.owner_bounds(98000, 8)
+    assert b[0] == 0 and b[-1] == 98000 and np.all(np.diff(b) > 0) and np.diff(b).max() - np.diff(b).min() <= 1
+    b = shard.owner_bounds(23558, 4, unit=3, first_unit_atom=11084)          # waters start after 11 084 protein atoms
+    assert all(c <= 11084 or (c - 11084) % 3 == 0 for c in b[1:-1])
+    s = W.make_system(1)
+    m = W.md_inputs(s)
+    b = shard.owner_bounds(s.n_atoms, 2, unit=3)
+    for i, j in m.bonds:
+        assert np.searchsorted(b, i, side="right") == np.searchsorted(b, j, side="right")   # no bond is split
+
+
+class _OracleDhp:
+    """CPU stand-in for binding.Dhp in the gloo tests: the four calls ShardedMd makes, played in fp64 by the oracles
+    (tests may use them).  What is under test is shard.py's ownership / mask / exchange logic, not this class."""
+
+    def __init__(self, params, blob, n_models):
+        self.params, self.blob, self.n_models = params, blob, n_models
+
+    def dhp_md_create(self, inv_mass, bonds=None, bond_k=None, bond_r0=None):
+        return {"w": np.asarray(inv_mass, np.float64)[:, None], "bonds": bonds, "k": bond_k, "r0": bond_r0, "Ff": None}
+
+    def _fast(self, md, x, box):
+        from oracle import md_oracle as M
+        if md["bonds"] is None:
+            return np.zeros_like(x)
+        return M.bond_energy_forces(x, box, md["bonds"], md["k"], md["r0"])[1]
+
+    def dhp_ani_energy_forces_partial(self, pos, box, species, weights, central, mol_offsets=None):
+        import torch
+        import oracle
+        c = np.nonzero(central.numpy())[0].astype(np.int32)
+        Ec, Fc, _ = oracle.energy_forces(pos.numpy(), species.numpy(), box, self.params, self.blob, self.n_models, centres=c)
+        return torch.tensor([Ec.sum()], dtype=torch.float64), torch.from_numpy(Fc.copy())
+
+    def dhp_md_open(self, md, pos, vel, box, F_slow, dt, n_inner, lo, hi):
+        x, v, w = pos.numpy(), vel.numpy(), md["w"]
+        if md["bonds"] is None:
+            n_inner = 1
+        d = dt / n_inner
+        if md["Ff"] is None:
+            md["Ff"] = self._fast(md, x, box)
+        v[lo:hi] += 0.5 * dt * w[lo:hi] * F_slow.numpy()[lo:hi]
+        for _ in range(n_inner):
+            v[lo:hi] += 0.5 * d * w[lo:hi] * md["Ff"][lo:hi]
+            x[lo:hi] += d * v[lo:hi]
+            md["Ff"] = self._fast(md, x, box)          # own bonds only touch own atoms
+            v[lo:hi] += 0.5 * d * w[lo:hi] * md["Ff"][lo:hi]
+
+    def dhp_md_close(self, md, vel, F_slow, dt, n_inner, lo, hi):
+        vel.numpy()[lo:hi] += 0.5 * dt * md["w"][lo:hi] * F_slow.numpy()[lo:hi]
+
+
+def _md_worker(rank, port, results):
+    import torch
+    import torch.distributed as dist
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=WORLD)
+    try:
+        params = W.default_params()
+        blob = W.make_weights(1)
+        s = W.make_system(1)
+        mdi = W.md_inputs(s)
+        bounds = shard.owner_bounds(s.n_atoms, WORLD, unit=3)
+        pos = torch.from_numpy(s.pos.astype(np.float64))
+        vel = torch.from_numpy(mdi.vel.astype(np.float64))
+        # the exchange alone: reduce-scatter of partial forces and all-gather of owned rows
+        ex = shard.Exchange(bounds, pos.device)
+        part = torch.from_numpy(np.random.default_rng(rank).normal(size=(s.n_atoms, 3)))
+        tot = torch.zeros_like(part)
+        ex.reduce_scatter_forces(part, tot)
+        want = sum(np.random.default_rng(r).normal(size=(s.n_atoms, 3)) for r in range(WORLD))
+        assert np.allclose(tot.numpy()[ex.lo:ex.hi], want[ex.lo:ex.hi], atol=1e-14)
+        assert np.all(tot.numpy()[:ex.lo] == 0) and np.all(tot.numpy()[ex.hi:] == 0)
+        scr = torch.full((s.n_atoms, 3), float(rank) + 1.0, dtype=torch.float64)
+        ex.all_gather_positions(scr)
+        for r in range(WORLD):
+            assert np.all(scr.numpy()[bounds[r]:bounds[r + 1]] == r + 1.0)
+        # two outer steps of the sharded driver (2 inner steps, O-H bonds, slab masks refreshed every step)
+        drv = shard.ShardedMd(_OracleDhp(params, blob, 1), blob, torch.from_numpy(s.species), s.box, bounds,
+                              mdi.inv_mass, mdi.bonds, mdi.bond_k, mdi.bond_r0, mask_every=1, dtype=torch.float64)
+        E = drv.run(pos, vel, 0.5, 2, 2)
+        own = vel.numpy()[ex.lo:ex.hi].copy()
+        allv = [torch.zeros_like(vel) for _ in range(WORLD)]
+        dist.all_gather(allv, vel)
+        if rank == 0:
+            v = np.concatenate([allv[r].numpy()[bounds[r]:bounds[r + 1]] for r in range(WORLD)])
+            results.put((pos.numpy().copy(), v, float(E.item())))
+        del own
+    finally:
+        dist.destroy_process_group()
+
+
+def test_world2_gloo_sharded_md_steps_equal_the_single_process_oracle_trajectory():
+    import torch.multiprocessing as mp
+    import oracle
+    from oracle import md_oracle as M
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_md_worker, args=(r, port, q)) for r in range(WORLD)]
+    for p in procs:
+        p.start()
+    x_sh, v_sh, E_sh = q.get(timeout=300)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    params = W.default_params()
+    blob = W.make_weights(1)
+    s = W.make_system(1)
+    mdi = W.md_inputs(s)
+
+    def slow(x):
+        Ea, F, _ = oracle.energy_forces(x, s.species, s.box, params, blob, 1)
+        return Ea.sum(), F
+
+    def fast(x):
+        return M.bond_energy_forces(x, s.box, mdi.bonds, mdi.bond_k, mdi.bond_r0)
+
+    x, v, (E_s, _, _) = M.respa_run(s.pos, mdi.vel, mdi.inv_mass, slow, fast, 0.5, 2, 2)
+    assert np.max(np.abs(x_sh - x)) <= 1e-11 and np.max(np.abs(v_sh - v)) <= 1e-11
+    assert abs(E_sh - E_s) <= 1e-9
