@@ -185,6 +185,10 @@ def main():
     ap.add_argument("--shard", default="replicas", choices=["replicas", "slab"],
                     help="N > 1: 'replicas' = one independent system per GPU (weak scaling, the default the contract asks for); "
                          "'slab' = ONE system, central atoms partitioned into spatial slabs, partial E / F summed over NCCL (strong scaling)")
+    ap.add_argument("--simulate-world", type=int, default=0,
+                    help="ONE GPU: time dhp_ani_energy_forces_partial for each of W slab masks of the system in turn (what each of W "
+                         "ranks would run under --shard slab) and report the per-rank times and the strong-scaling ceiling "
+                         "t_full / max_r t_r they predict; no collective is timed")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-md", action="store_true", help="skip the multiple-timestep driver measurement")
     ap.add_argument("--no-sustained", action="store_true", help="skip the ~1 s sustained-rate loop")
@@ -304,6 +308,40 @@ def main():
                          "sm_mhz": c2["sm_mhz"], "reasons": c2["reasons"],
                          "power_w": getattr(s2, "power_w", None), "samples": c2.get("samples"),
                          "note": "steady state of a long run (board power management settled): the number an MD run gets"}
+
+    # ---- strong-scaling prediction without a multi-GPU node: every slab's partial call on this one GPU -------------------
+    simulated = None
+    if args.simulate_world > 1 and system.mol_offsets is None and world == 1:
+        from paper_2207_14276_b200 import shard
+        Wn = args.simulate_world
+        per_rank, per_phase = [], []
+        for r in range(Wn):
+            # the mask is derived inside the timed region on the first of every `mask_every` = 10 steps, as shard.ShardedMd does
+            m_r = [shard.slab_mask_device(p_, system.box, Wn, r) for p_ in pos_sets]
+            for k in range(3):
+                d.dhp_ani_energy_forces_partial(pos_sets[k % n_sets], system.box, species, w, m_r[k % n_sets], mol, E=E, F=F)
+            barrier()
+            d.dhp_profile_enable(True)
+            d.dhp_profile_reset()
+            ev0.record(stream)
+            for k in range(args.steps):
+                if k % 10 == 0:
+                    m_r[k % n_sets] = shard.slab_mask_device(pos_sets[k % n_sets], system.box, Wn, r)
+                d.dhp_ani_energy_forces_partial(pos_sets[k % n_sets], system.box, species, w, m_r[k % n_sets], mol, E=E, F=F)
+            ev1.record(stream)
+            barrier()
+            phr, cr = d.dhp_profile_read()
+            d.dhp_profile_enable(False)
+            per_rank.append(ev0.elapsed_time(ev1) / args.steps)
+            per_phase.append({k_: v_ / max(cr, 1) for k_, v_ in phr.items()})
+        t_full = ms_total / args.steps
+        simulated = {"world": Wn, "ms_per_rank": per_rank, "phase_ms_slowest_rank": per_phase[int(np.argmax(per_rank))],
+                     "ms_full_call_one_gpu": t_full, "predicted_speedup_ceiling": t_full / max(per_rank),
+                     "predicted_parallel_efficiency_ceiling": t_full / max(per_rank) / Wn,
+                     "exchange_bytes_per_rank_per_step": {"all_gather_positions": system.n_atoms * 12,
+                                                          "reduce_scatter_forces": system.n_atoms * 12},
+                     "note": "per-rank device time of the masked call measured on ONE GPU (slab mask refreshed every 10 steps inside "
+                             "the timed loop); the NVLink exchange (2 x 1.2 MB per step) is not included - unmeasured at N > 1"}
 
     # ---- energy-only call (a1-a3), same inputs, device-resident ---------------------------------
     for k in range(3):
@@ -478,7 +516,7 @@ def main():
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "ms_per_step": e2e_ms / args.steps},
-            "energy_only_ms_per_step": ms_energy_only, "md": md_out, "sustained": sustained,
+            "energy_only_ms_per_step": ms_energy_only, "md": md_out, "sustained": sustained, "simulated_world": simulated,
             "roofline": roof,
             "roofline_mlp_phase": mlp_phase,
             "roofline_kernels": kernels,

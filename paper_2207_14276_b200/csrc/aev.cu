@@ -102,14 +102,18 @@ __global__ void __launch_bounds__(AEV_WARPS * 32, 5)
 k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, const int* __restrict__ col,
           const unsigned short* __restrict__ seg_cnt, const int* __restrict__ rowmap, const unsigned* __restrict__ tile_mask,
           const Grid* __restrict__ gp, const __grid_constant__ AevConst K, int n, float* __restrict__ aev,
-          __half* __restrict__ planes, size_t plane_stride, int* __restrict__ status) {
+          __half* __restrict__ planes, size_t plane_stride, int* __restrict__ status, const int* __restrict__ row_slot) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ Grid g;
     if (threadIdx.x == 0) g = *gp;
     __syncthreads();
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int i = blockIdx.x * AEV_WARPS + w;
+    // full evaluation: warp <-> atom in sorted (cell) order, so that the warps of a block share neighbours; partial
+    // evaluation (row_slot != null, n = an upper bound of the rows): warp <-> row, so that no warp is spent on the atoms
+    // that are not central in this call
+    int i = blockIdx.x * AEV_WARPS + w;
     if (i >= n) return;
+    if (row_slot) { i = row_slot[i]; if (i < 0) return; }
     WarpSmemFwd& S = reinterpret_cast<WarpSmemFwd*>(smem_raw)[w];
     const unsigned FULL = 0xffffffffu;
     const unsigned lt = (1u << lane) - 1u;
@@ -312,14 +316,16 @@ struct __align__(16) WarpSmemBwd {
 __global__ void __launch_bounds__(BWD_WARPS * 32, 4)
 k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, const int* __restrict__ col,
           const unsigned short* __restrict__ seg_cnt, const int* __restrict__ rowmap, const Grid* __restrict__ gp,
-          const __grid_constant__ AevConst K, int n, const float* __restrict__ grad, float* __restrict__ fsorted) {
+          const __grid_constant__ AevConst K, int n, const float* __restrict__ grad, float* __restrict__ fsorted,
+          const int* __restrict__ row_slot) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ Grid g;
     if (threadIdx.x == 0) g = *gp;
     __syncthreads();
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int i = blockIdx.x * BWD_WARPS + w;
+    int i = blockIdx.x * BWD_WARPS + w;                 // warp <-> atom, or warp <-> row in a partial evaluation (see k_aev_fwd)
     if (i >= n) return;
+    if (row_slot) { i = row_slot[i]; if (i < 0) return; }
     WarpSmemBwd& S = reinterpret_cast<WarpSmemBwd*>(smem_raw)[w];
     const unsigned FULL = 0xffffffffu;
 
@@ -561,14 +567,19 @@ int aev_forward(Ctx* ctx, bool planes) {
     ctx->aev_in_planes = planes;
     if (n == 0) return DHP_OK;
     const size_t smem = sizeof(WarpSmemFwd) * AEV_WARPS;
-    const int blocks = (n + AEV_WARPS - 1) / AEV_WARPS;
+    // partial evaluation: one warp per ROW; the host knows an upper bound of the row count only when it knows the number
+    // of central atoms, which it does not (the mask lives on the device) - the row tables are walked up to max_rows of the
+    // call's atom count instead, and rows beyond the last group hold -1
+    const int* row_slot = ctx->partial ? ctx->row_slot : nullptr;
+    const int nw = ctx->partial ? (int)std::min<int64_t>(ctx->max_rows, (int64_t)n + NSP * ROW_ALIGN) : n;
+    const int blocks = (nw + AEV_WARPS - 1) / AEV_WARPS;
     const size_t plane_stride = (size_t)ctx->max_rows * AEV_LD;
     if (planes)
         DHP_LAUNCH(ctx, k_aev_fwd<true>, blocks, AEV_WARPS * 32, smem, ctx->spos, ctx->row_ptr, ctx->col, ctx->seg_cnt, ctx->rowmap,
-                   ctx->tile_mask, ctx->grid, ctx->aevc, n, ctx->aev, ctx->aev_planes, plane_stride, ctx->status);
+                   ctx->tile_mask, ctx->grid, ctx->aevc, nw, ctx->aev, ctx->aev_planes, plane_stride, ctx->status, row_slot);
     else
         DHP_LAUNCH(ctx, k_aev_fwd<false>, blocks, AEV_WARPS * 32, smem, ctx->spos, ctx->row_ptr, ctx->col, ctx->seg_cnt, ctx->rowmap,
-                   ctx->tile_mask, ctx->grid, ctx->aevc, n, ctx->aev, ctx->aev_planes, plane_stride, ctx->status);
+                   ctx->tile_mask, ctx->grid, ctx->aevc, nw, ctx->aev, ctx->aev_planes, plane_stride, ctx->status, row_slot);
     DHP_CUDA(ctx, cudaGetLastError());
     return DHP_OK;
 }
@@ -578,8 +589,10 @@ int aev_backward(Ctx* ctx, float* F_out) {
     if (n == 0) return DHP_OK;
     const size_t smem = sizeof(WarpSmemBwd) * BWD_WARPS;
     // fsorted was zeroed with the rest of the per-call arena at the start of the call (nlist_build)
-    DHP_LAUNCH(ctx, k_aev_bwd, (n + BWD_WARPS - 1) / BWD_WARPS, BWD_WARPS * 32, smem, ctx->spos, ctx->row_ptr, ctx->col,
-               ctx->seg_cnt, ctx->rowmap, ctx->grid, ctx->aevc, n, ctx->grad, ctx->fsorted);
+    const int* row_slot = ctx->partial ? ctx->row_slot : nullptr;
+    const int nw = ctx->partial ? (int)std::min<int64_t>(ctx->max_rows, (int64_t)n + NSP * ROW_ALIGN) : n;
+    DHP_LAUNCH(ctx, k_aev_bwd, (nw + BWD_WARPS - 1) / BWD_WARPS, BWD_WARPS * 32, smem, ctx->spos, ctx->row_ptr, ctx->col,
+               ctx->seg_cnt, ctx->rowmap, ctx->grid, ctx->aevc, nw, ctx->grad, ctx->fsorted, row_slot);
     DHP_LAUNCH(ctx, k_unsort_forces, (n + 255) / 256, 256, 0, ctx->fsorted, ctx->perm, n, F_out);
     DHP_CUDA(ctx, cudaGetLastError());
     return DHP_OK;

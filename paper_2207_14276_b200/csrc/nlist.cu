@@ -451,6 +451,16 @@ k_pairs(const float4* __restrict__ spos, const Grid* __restrict__ gp, const int*
     const int cb = cell_start[cell], ce = cell_start[cell + 1];
     if (ce == cb) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (snc) {
+        // partial evaluation (one rank's slab of central atoms): a cell without a central atom needs no candidates at
+        // all - its rows are empty.  7/8 of the cells at world size 8.
+        bool any = false;
+        for (int i = cb + (int)threadIdx.x; i < ce; i += P1_THREADS) any |= snc[i] == 0;
+        if (!__syncthreads_or(any)) {
+            for (int i = cb + (int)threadIdx.x; i < ce; i += P1_THREADS) { cnt[i] = 0; if (SKIN) cand_cnt[i] = 0; }
+            return;
+        }
+    }
 
     // candidate segments: one per non-empty stencil cell (warp 0: lane <-> stencil cell, ballot-compacted)
     if (warp == 0) {
