@@ -34,11 +34,13 @@
 
 #define NSP 7            /* H C N O S F Cl */
 #define NR 16            /* radial shifts                          */
-#define NA 8             /* angular radial shifts                  */
-#define NZ 4             /* angular sections                       */
+#define NAZ 32           /* entries of one angular sub-AEV = n_a radial shifts x n_z sections: 8 x 4 for the ANI-2x shape
+                            (BASELINE.json configs[0]), 4 x 8 for the ANI-1x shape (reading R4) */
+#define NAMAX 8
+#define NZMAX 8
 #define NPAIR (NSP * (NSP + 1) / 2)
 #define AEV_RAD (NSP * NR)                    /* 112 */
-#define AEV_DIM (AEV_RAD + NPAIR * NA * NZ)   /* 1008  (N radial + N(N+1)/2 angular sub-AEVs) */
+#define AEV_DIM (AEV_RAD + NPAIR * NAZ)       /* 1008  (N radial + N(N+1)/2 angular sub-AEVs) */
 #define L0 AEV_DIM
 #define L1 256
 #define L2 192
@@ -47,7 +49,8 @@
 
 typedef struct {
     double rcr, rca, eta_r, eta_a, zeta, alpha;
-    double shf_r[NR], shf_a[NA], shf_z[NZ];
+    double shf_r[NR], shf_a[NAMAX], shf_z[NZMAX];
+    int n_a, n_z;            /* n_a * n_z == NAZ; layout of a sub-AEV: [a][z], index n_z * a + z */
 } ora_params;
 
 static const double ORA_PI = 3.14159265358979323846;
@@ -181,7 +184,8 @@ static void aev_of(const ora_params *P, const nbr_t *nb, int64_t m, double *G)
             double cz = uj[0] * uk[1] - uj[1] * uk[0];
             double s = sqrt(cx * cx + cy * cy + cz * cz);            /* sin(theta) >= 0 */
             double fj = fcut(nb[a].R, P->rca), fk = fcut(nb[b].R, P->rca);
-            double *blk = G + AEV_RAD + NA * NZ * pairidx(nb[a].sp, nb[b].sp);
+            double *blk = G + AEV_RAD + NAZ * pairidx(nb[a].sp, nb[b].sp);
+            const int NA = P->n_a, NZ = P->n_z;
             for (int q = 0; q < NA; ++q) {
                 double mm = 0.5 * (nb[a].R + nb[b].R) - P->shf_a[q];
                 double B = exp(-P->eta_a * mm * mm);
@@ -323,7 +327,8 @@ static void centre_forces(const ora_params *P, int64_t i, const nbr_t *nb, int64
             }
             double fj = fcut(Rj, P->rca), fk = fcut(Rk, P->rca);
             double dfj = dfcut(Rj, P->rca), dfk = dfcut(Rk, P->rca);
-            const double *gb = g + AEV_RAD + NA * NZ * pairidx(nb[a].sp, nb[b].sp);
+            const double *gb = g + AEV_RAD + NAZ * pairidx(nb[a].sp, nb[b].sp);
+            const int NA = P->n_a, NZ = P->n_z;
             double gj[3] = {0, 0, 0}, gk[3] = {0, 0, 0};   /* sum over (a,z) of g * grad_j, g * grad_k */
             for (int q = 0; q < NA; ++q) {
                 double mm = 0.5 * (Rj + Rk) - P->shf_a[q];

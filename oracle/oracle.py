@@ -13,13 +13,14 @@ import numpy as np
 
 from . import build as _build
 
-_NR, _NA, _NZ = 16, 8, 4
+_NR, _NAMAX, _NZMAX = 16, 8, 8
 
 
 class _Params(C.Structure):
     _fields_ = [("rcr", C.c_double), ("rca", C.c_double), ("eta_r", C.c_double), ("eta_a", C.c_double),
                 ("zeta", C.c_double), ("alpha", C.c_double),
-                ("shf_r", C.c_double * _NR), ("shf_a", C.c_double * _NA), ("shf_z", C.c_double * _NZ)]
+                ("shf_r", C.c_double * _NR), ("shf_a", C.c_double * _NAMAX), ("shf_z", C.c_double * _NZMAX),
+                ("n_a", C.c_int), ("n_z", C.c_int)]
 
 
 _lib = None
@@ -64,9 +65,11 @@ def _params(p) -> _Params:
     q.zeta, q.alpha = float(np.float32(p.zeta)), float(np.float32(p.celu_alpha))
     for i in range(_NR):
         q.shf_r[i] = float(np.float32(p.shf_r[i]))
-    for i in range(_NA):
+    q.n_a, q.n_z = len(p.shf_a), len(p.shf_z)
+    assert q.n_a * q.n_z == 32 and q.n_a <= _NAMAX and q.n_z <= _NZMAX
+    for i in range(q.n_a):
         q.shf_a[i] = float(np.float32(p.shf_a[i]))
-    for i in range(_NZ):
+    for i in range(q.n_z):
         q.shf_z[i] = float(np.float32(p.shf_z[i]))
     return q
 

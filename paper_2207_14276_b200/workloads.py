@@ -68,6 +68,88 @@ def default_params() -> AniParams:
                      shf_r=shf_r, shf_a=shf_a, shf_z=shf_z)
 
 
+def ani1x_params() -> AniParams:
+    """ANI-1x / ANI-1ccx-shaped AEV parameters ("ANI-1x ... H, C, N, and O"; L73: "R_c ... fixed to 5.2 Å").
+    The paper prints no other value; eta / shift values are those of the published ANI-1x model (Smith et al., ANI-1x
+    data set / TorchANI `ani-1x_8x` parameter file; DESIGN.md reading R4): 16 radial shifts 0.9 + 0.26875 m, EtaR 16;
+    angular grid 4 ShfA (0.9 + 0.65 a) x 8 ShfZ ((2k+1) pi/16), EtaA 8, Zeta 32; Rca 3.5 Å.  Species H, C, N, O = 0..3 of
+    the library's species order, so the 384-entry ANI-1x AEV is a sub-vector of the 1008-entry layout."""
+    shf_r = (0.9 + 0.26875 * np.arange(N_RAD_SHIFTS, dtype=np.float64)).astype(np.float32)
+    shf_a = (0.9 + 0.65 * np.arange(4, dtype=np.float64)).astype(np.float32)
+    shf_z = ((2.0 * np.arange(8, dtype=np.float64) + 1.0) * math.pi / 16.0).astype(np.float32)
+    return AniParams(rcr=np.float32(5.2), rca=np.float32(3.5), eta_r=np.float32(16.0), eta_a=np.float32(8.0),
+                     zeta=np.float32(32.0), celu_alpha=np.float32(0.1), shf_r=shf_r, shf_a=shf_a, shf_z=shf_z)
+
+
+# ANI-1x network shape (reading R4: the published model's hydrogen network, used here for all four elements):
+ANI1X_SPECIES = 4
+ANI1X_AEV_DIM = ANI1X_SPECIES * N_RAD_SHIFTS + (ANI1X_SPECIES * (ANI1X_SPECIES + 1) // 2) * 32     # 64 + 320 = 384
+ANI1X_LAYERS = (ANI1X_AEV_DIM, 160, 128, 96, 1)
+ANI1X_PARAMS_PER_NET = sum(ANI1X_LAYERS[i] * ANI1X_LAYERS[i + 1] + ANI1X_LAYERS[i + 1] for i in range(4))
+
+
+def make_weights_ani1x(n_models: int, seed: int = WEIGHT_SEED + 1) -> np.ndarray:
+    """Flat fp32 blob of the NATIVE ANI-1x shape: for e: for s in H,C,N,O: W1[160][384], b1, W2[128][160], b2,
+    W3[96][128], b3, W4[1][96], b4 (same initialisation rule as `make_weights`)."""
+    rng = np.random.default_rng(seed)
+    out = np.empty(n_models * ANI1X_SPECIES * ANI1X_PARAMS_PER_NET, dtype=np.float32)
+    p = 0
+    for _e in range(n_models):
+        for _s in range(ANI1X_SPECIES):
+            for l in range(4):
+                fan_in, fan_out = ANI1X_LAYERS[l], ANI1X_LAYERS[l + 1]
+                w = rng.standard_normal(fan_in * fan_out) * (1.0 / math.sqrt(fan_in))
+                out[p:p + w.size] = w.astype(np.float32); p += w.size
+                b = rng.standard_normal(fan_out) * 0.1
+                out[p:p + b.size] = b.astype(np.float32); p += b.size
+    assert p == out.size
+    return out
+
+
+def split_net_ani1x(blob: np.ndarray, e: int, s: int):
+    p = (e * ANI1X_SPECIES + s) * ANI1X_PARAMS_PER_NET
+    out = []
+    for l in range(4):
+        fan_in, fan_out = ANI1X_LAYERS[l], ANI1X_LAYERS[l + 1]
+        out.append(blob[p:p + fan_in * fan_out].reshape(fan_out, fan_in)); p += fan_in * fan_out
+        out.append(blob[p:p + fan_out]); p += fan_out
+    return tuple(out)
+
+
+def ani1x_feature_map() -> np.ndarray:
+    """Position of each of the 384 ANI-1x features (radial [s_j][m], then angular [pair(u<=v) of 4][a][z]) inside the
+    1008-entry layout of the library (radial [s_j of 7][m], angular [pairidx of 7][32]).  Index arithmetic only."""
+    idx = []
+    for sj in range(ANI1X_SPECIES):
+        idx += [N_RAD_SHIFTS * sj + m for m in range(N_RAD_SHIFTS)]
+    for u in range(ANI1X_SPECIES):
+        for v in range(u, ANI1X_SPECIES):
+            p7 = N_SPECIES * u - u * (u - 1) // 2 + (v - u)
+            idx += [AEV_RADIAL + 32 * p7 + q for q in range(32)]
+    return np.asarray(idx, dtype=np.int64)
+
+
+def embed_ani1x(blob1x: np.ndarray, n_models: int) -> np.ndarray:
+    """An ANI-1x-shaped ensemble as a blob of the library's fixed layout (7 species, 1008 -> 256 -> 192 -> 160 -> 1):
+    each small matrix sits in the top-left corner of its big one (W1's columns scattered by `ani1x_feature_map`),
+    everything else - including all parameters of S, F, Cl - is zero.  Padding units see z = 0, CELU(0) = 0, and feed zero
+    weights, so the embedded network computes exactly the native one and its input gradient.  Marshalling only."""
+    fmap = ani1x_feature_map()
+    out = np.zeros(n_models * N_SPECIES * PARAMS_PER_NET, dtype=np.float32)
+    for e in range(n_models):
+        for s in range(ANI1X_SPECIES):
+            small = split_net_ani1x(blob1x, e, s)
+            big = split_net(out, e, s)
+            W1s, W1b = small[0], big[0]
+            W1b[:W1s.shape[0], fmap] = W1s
+            big[1][:small[1].size] = small[1]
+            for l in (1, 2, 3):
+                Ws, Wb = small[2 * l], big[2 * l]
+                Wb[:Ws.shape[0], :Ws.shape[1]] = Ws
+                big[2 * l + 1][:small[2 * l + 1].size] = small[2 * l + 1]
+    return out
+
+
 @dataclasses.dataclass
 class System:
     """One synthetic input: fp32 positions [N,3], int32 species [N], optional cubic box edge,
@@ -310,7 +392,7 @@ def make_system(config: int) -> System:
             4: biosystem_98k, 5: replicas_1024x30}[config]()
 
 
-def small_periodic_mix(n_atoms: int = 600, L: float = 18.3, seed: int = 77, n_models: int = 2) -> System:
+def small_periodic_mix(n_atoms: int = 600, L: float = 18.3, seed: int = 77, n_models: int = 2, hcno_only: bool = False) -> System:
     """A small periodic 5-species box at the density of configs[2] (~0.098 Å^-3), used by parity
     tests that need several cells/tiles and a ragged tail at a size the oracle finishes in seconds."""
     rng = np.random.default_rng(seed)
@@ -321,6 +403,8 @@ def small_periodic_mix(n_atoms: int = 600, L: float = 18.3, seed: int = 77, n_mo
     pts = _rsa_fill(rng, L, np.empty((0, 3)), n_atoms, propose, 1)
     species = rng.choice(np.array([H, C, N, O, S], dtype=np.int32), size=n_atoms,
                          p=[0.50, 0.31, 0.09, 0.095, 0.005]).astype(np.int32)
+    if hcno_only:                                  # ANI-1x covers H, C, N, O: the few S become O
+        species[species == S] = O
     return System(f"mix{n_atoms}", pts.astype(np.float32), species,
                   np.array([L, L, L], dtype=np.float32), None, n_models=n_models)
 
