@@ -182,6 +182,9 @@ def main():
     ap.add_argument("--impl", default="dhp", choices=["dhp", "reference"])
     ap.add_argument("--config", type=int, default=4, help="1-based BASELINE.json config (default 4 = configs[3], 98k atoms)")
     ap.add_argument("--mlp", default="auto", choices=["auto", "simt", "tensor", "fp16"])
+    ap.add_argument("--model", default="ani2x", choices=["ani2x", "ani1x"],
+                    help="ani1x: the ANI-1x / ANI-1ccx shape of PAPER.md L87 / L159 on the same geometry (species H, C, N, O - the few S "
+                         "become O; Rcr 5.2 Å, 4 x 8 angular grid, 384 features, 384-160-128-96-1 networks loaded zero-padded)")
     ap.add_argument("--shard", default="replicas", choices=["replicas", "slab"],
                     help="N > 1: 'replicas' = one independent system per GPU (weak scaling, the default the contract asks for); "
                          "'slab' = ONE system, central atoms partitioned into spatial slabs, partial E / F summed over NCCL (strong scaling)")
@@ -200,6 +203,12 @@ def main():
     params = W.default_params()
     system = W.make_system(args.config)
     blob = W.make_weights(system.n_models)
+    if args.model == "ani1x":
+        params = W.ani1x_params()
+        sp1 = system.species.copy()
+        sp1[sp1 > W.O] = W.O                                   # S, F, Cl -> O: ANI-1x covers H, C, N, O
+        system = W.System(system.name + "+ani1x", system.pos, sp1, system.box, system.mol_offsets, system.n_models)
+        blob = W.embed_ani1x(W.make_weights_ani1x(system.n_models), system.n_models)
     if args.impl == "reference":
         run_reference(args, system, params, blob)
         return

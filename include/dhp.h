@@ -19,9 +19,12 @@
  *     no allocation, no host synchronisation.  Data-dependent faults (species outside 0..6, neighbour
  *     capacity overflow) set a device-side status word that stays set until dhp_status() reads it.
  *   - Units are the caller's: Å in, Hartree and Hartree/Å out (F = -dE/dr); no conversion inside.
- *   - Species index 0..6 = H, C, N, O, S, F, Cl.  The shape is fixed at compile time:
- *     16 radial shifts, 8 x 4 angular shifts, AEV length 7*16 + 28*32 = 1008,
- *     networks 1008 -> 256 -> 192 -> 160 -> 1 with CELU (BASELINE.json configs[0]).
+ *   - Species index 0..6 = H, C, N, O, S, F, Cl.  The layout is fixed at compile time:
+ *     16 radial shifts, 32 angular entries per species pair, AEV length 7*16 + 28*32 = 1008,
+ *     networks 1008 -> 256 -> 192 -> 160 -> 1 with CELU (BASELINE.json configs[0]).  The angular grid is 8 x 4
+ *     (ANI-2x) or 4 x 8 (ANI-1x / ANI-1ccx: species H, C, N, O = 0..3; its 384-entry AEV is the
+ *     sub-vector of the 1008 layout that those four species span, and its narrower 384 -> 160 -> 128 -> 96 -> 1
+ *     networks are loaded zero-padded into the fixed layout - same results, the cost of the wide shape).
  */
 #ifndef DHP_H
 #define DHP_H
@@ -34,8 +37,10 @@ extern "C" {
 
 #define DHP_N_SPECIES 7
 #define DHP_N_SHF_R 16
-#define DHP_N_SHF_A 8
+#define DHP_N_SHF_A 8    /* the ANI-2x angular grid: 8 radial shifts x 4 sections ... */
 #define DHP_N_SHF_Z 4
+#define DHP_MAX_SHF_A 8  /* ... capacity of the parameter arrays (ANI-1x grid: 4 x 8)  */
+#define DHP_MAX_SHF_Z 8
 #define DHP_AEV_DIM 1008
 #define DHP_NET_PARAMS 338689 /* 1008*256+256 + 256*192+192 + 192*160+160 + 160+1 */
 
@@ -60,9 +65,11 @@ typedef struct dhp_params {
     float eta_a;      /* eta of Eq. 5, Å^-2                                    */
     float zeta;       /* xi of Eq. 5                                           */
     float celu_alpha; /* CELU(x) = x (x>0), alpha (exp(x/alpha) - 1) otherwise */
-    float shf_r[DHP_N_SHF_R]; /* R_s of Eq. 4, Å   */
-    float shf_a[DHP_N_SHF_A]; /* R_s of Eq. 5, Å   */
-    float shf_z[DHP_N_SHF_Z]; /* theta_s of Eq. 5  */
+    float shf_r[DHP_N_SHF_R];   /* R_s of Eq. 4, Å                                              */
+    float shf_a[DHP_MAX_SHF_A]; /* R_s of Eq. 5, Å: the first n_shf_a entries                   */
+    float shf_z[DHP_MAX_SHF_Z]; /* theta_s of Eq. 5: the first n_shf_z entries                  */
+    int32_t n_shf_a;  /* angular grid of Eq. 5: 8 x 4 (ANI-2x shape, BASELINE.json configs[0]) or 4 x 8 (ANI-1x / ANI-1ccx shape, */
+    int32_t n_shf_z;  /* PAPER.md L87); n_shf_a * n_shf_z = 32 entries per species pair, laid out [a][z]                           */
 } dhp_params;
 
 typedef struct dhp_ctx dhp_ctx;         /* workspace sized for max_atoms, bound to one CUDA stream */

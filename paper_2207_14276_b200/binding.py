@@ -62,7 +62,7 @@ SYMBOLS = {
 
 class DhpParams(C.Structure):
     _fields_ = [("rcr", _f32), ("rca", _f32), ("eta_r", _f32), ("eta_a", _f32), ("zeta", _f32), ("celu_alpha", _f32),
-                ("shf_r", _f32 * 16), ("shf_a", _f32 * 8), ("shf_z", _f32 * 4)]
+                ("shf_r", _f32 * 16), ("shf_a", _f32 * 8), ("shf_z", _f32 * 8), ("n_shf_a", C.c_int32), ("n_shf_z", C.c_int32)]
 
 
 class DhpError(RuntimeError):
@@ -139,9 +139,10 @@ def make_params(p) -> DhpParams:
     q.zeta, q.celu_alpha = float(p.zeta), float(p.celu_alpha)
     for i in range(16):
         q.shf_r[i] = float(p.shf_r[i])
-    for i in range(8):
+    q.n_shf_a, q.n_shf_z = len(p.shf_a), len(p.shf_z)          # 8 x 4 (ANI-2x shape) or 4 x 8 (ANI-1x shape)
+    for i in range(q.n_shf_a):
         q.shf_a[i] = float(p.shf_a[i])
-    for i in range(4):
+    for i in range(q.n_shf_z):
         q.shf_z[i] = float(p.shf_z[i])
     return q
 

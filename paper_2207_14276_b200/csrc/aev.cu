@@ -81,7 +81,7 @@ struct __align__(16) WarpSmemFwd {
     float fca[MAX_ANG];          // f_c(R; Rca)
     union {                      // the radial part is finished before the first angular round is staged: same bytes
         float2 rr[MAX_RAD];      // all neighbours: R, f_c(R; Rcr)
-        struct { float tA[NZ][TP]; float tB[NA][TP]; } st;
+        float st[12][TP];        // staged factor rows of one round: n_z angular rows, then n_a radial rows (8 + 4 or 4 + 8)
     };
     int4 tab[NPAIR + 1];         // non-empty species pairs in slot order: first slot, j0 | k0 << 8 | nk << 16 | same << 24,
                                  // triplets, angular block; terminated by {total slots, ...}
@@ -97,7 +97,7 @@ __device__ __forceinline__ void put_feature(float v, float* __restrict__ row_f32
     row_hi[plane_stride + colidx] = __float2half_rn(v - __half2float(hi));
 }
 
-template <bool PLANES>
+template <bool PLANES, int NAg, int NZg>     // NAg x NZg: the angular grid of Eq. 5, 8 x 4 (ANI-2x shape) or 4 x 8 (ANI-1x shape)
 __global__ void __launch_bounds__(AEV_WARPS * 32, 5)
 k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, const int* __restrict__ col,
           const unsigned short* __restrict__ seg_cnt, const int* __restrict__ rowmap, const unsigned* __restrict__ tile_mask,
@@ -199,13 +199,17 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
 
     __syncwarp();                                        // rr is dead from here on: its bytes become the staging rows
     // ---- angular (Eq. 5) ------------------------------------------------------------------------------
-    const int za = lane & 3, aa = lane >> 2;
+    static_assert(NAg * NZg == 32 && NAg + NZg == 12, "angular grid");
+    const int za = lane % NZg, aa = lane / NZg;          // this lane's feature (a, z) of a pair block, index NZg a + z
     float facc = 0.f;                                    // running sum of feature (aa, za) of the current pair
     int e = 0;                                           // table entry of this lane's slot (monotonic over the rounds)
     for (int T0 = 0; T0 < T_pad; T0 += 32) {
         const int t = T0 + lane;
-        float A[NZ] = {0.f, 0.f, 0.f, 0.f};
-        float B[NA] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        float A[NZg], B[NAg];
+#pragma unroll
+        for (int z = 0; z < NZg; ++z) A[z] = 0.f;
+#pragma unroll
+        for (int a = 0; a < NAg; ++a) B[a] = 0.f;
         int my_blk = 0;                                  // angular block of this lane's slot
         bool my_end = false;                             // this slot is the last one of its species pair
         if (t < T_pad) {
@@ -232,29 +236,29 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
                 const float f2 = 2.0f * S.fca[j] * S.fca[k];
                 const float Rm = 0.5f * (qj.w + qk.w);
 #pragma unroll
-                for (int z = 0; z < NZ; ++z) {
+                for (int z = 0; z < NZg; ++z) {
                     const float uu = fmaxf(fmaf(0.5f * K.sin_z[z], sn, fmaf(0.5f * K.cos_z[z], c, 0.5f)), 0.f);
                     A[z] = f2 * fast_exp2(K.zeta * fast_log2(uu));    // 2 ((1+cos(theta-theta_z))/2)^zeta f_j f_k
                 }
 #pragma unroll
-                for (int a = 0; a < NA; ++a) {
+                for (int a = 0; a < NAg; ++a) {
                     const float mm = Rm - K.shf_a[a];
                     B[a] = fast_exp2(-K.eta_a_l2e * mm * mm);
                 }
             }
         }
 #pragma unroll
-        for (int z = 0; z < NZ; ++z) S.st.tA[z][lane] = A[z];
+        for (int z = 0; z < NZg; ++z) S.st[z][lane] = A[z];
 #pragma unroll
-        for (int a = 0; a < NA; ++a) S.st.tB[a][lane] = B[a];
+        for (int a = 0; a < NAg; ++a) S.st[NZg + a][lane] = B[a];
         __syncwarp();
         // phase 2: the 8 quads of the round in order (pairs are padded to whole quads, so a pair ends at a quad end);
         // the branch is warp-uniform
         const unsigned endmask = __ballot_sync(FULL, my_end);
 #pragma unroll
         for (int qd = 0; qd < 8; ++qd) {
-            const float4 a4 = *reinterpret_cast<const float4*>(&S.st.tA[za][4 * qd]);
-            const float4 b4 = *reinterpret_cast<const float4*>(&S.st.tB[aa][4 * qd]);
+            const float4 a4 = *reinterpret_cast<const float4*>(&S.st[za][4 * qd]);
+            const float4 b4 = *reinterpret_cast<const float4*>(&S.st[NZg + aa][4 * qd]);
             facc = fmaf(a4.x, b4.x, facc); facc = fmaf(a4.y, b4.y, facc);
             facc = fmaf(a4.z, b4.z, facc); facc = fmaf(a4.w, b4.w, facc);
             if ((endmask >> (4 * qd + 3)) & 1u) {             // pair complete: its 32 features go out, 64 (128) contiguous bytes
@@ -313,6 +317,7 @@ struct __align__(16) WarpSmemBwd {
     int sp[MAX_ANG];
 };
 
+template <int NAg, int NZg>
 __global__ void __launch_bounds__(BWD_WARPS * 32, 4)
 k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, const int* __restrict__ col,
           const unsigned short* __restrict__ seg_cnt, const int* __restrict__ rowmap, const Grid* __restrict__ gp,
@@ -440,9 +445,9 @@ k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
             const float sn = fast_sqrt(cx * cx + cy * cy + cz * cz);
             const float Rm = 0.5f * (qj.w + qk.w);
             const float4* gb = reinterpret_cast<const float4*>(grow + 32 * ipair(S.sp[j], S.sp[k]));
-            float Az[NZ], dAz[NZ];
+            float Az[NZg], dAz[NZg];
 #pragma unroll
-            for (int z = 0; z < NZ; ++z) {
+            for (int z = 0; z < NZg; ++z) {
                 const float u = fmaxf(fmaf(0.5f * K.sin_z[z], sn, fmaf(0.5f * K.cos_z[z], c, 0.5f)), 0.f);
                 const float wz = fast_exp2((K.zeta - 1.0f) * fast_log2(u));       // u^(zeta-1)
                 Az[z] = 2.0f * u * wz;                                             // A = 2 u^zeta
@@ -450,13 +455,17 @@ k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
             }
             float S0 = 0.f, Sm = 0.f, St = 0.f;
 #pragma unroll
-            for (int a = 0; a < NA; ++a) {
-                const float4 g4 = __ldg(gb + a);
+            for (int a = 0; a < NAg; ++a) {
                 const float mm = Rm - K.shf_a[a];
                 const float B = fast_exp2(-K.eta_a_l2e * mm * mm);
                 const float dB = -K.eta_a * mm * B;                                // dB/dR_ij = dB/dR_ik
-                const float ua = g4.x * Az[0] + g4.y * Az[1] + g4.z * Az[2] + g4.w * Az[3];
-                const float va = g4.x * dAz[0] + g4.y * dAz[1] + g4.z * dAz[2] + g4.w * dAz[3];
+                float ua = 0.f, va = 0.f;                                          // entries (a, z) of the pair block: [a][z]
+#pragma unroll
+                for (int z4 = 0; z4 < NZg / 4; ++z4) {
+                    const float4 g4 = __ldg(gb + a * (NZg / 4) + z4);
+                    ua += g4.x * Az[4 * z4] + g4.y * Az[4 * z4 + 1] + g4.z * Az[4 * z4 + 2] + g4.w * Az[4 * z4 + 3];
+                    va += g4.x * dAz[4 * z4] + g4.y * dAz[4 * z4 + 1] + g4.z * dAz[4 * z4 + 2] + g4.w * dAz[4 * z4 + 3];
+                }
                 S0 = fmaf(B, ua, S0); Sm = fmaf(dB, ua, Sm); St = fmaf(B, va, St);
             }
             const float dth = St * fj.x * fk.x;                                    // sum g dT/dtheta
@@ -556,9 +565,13 @@ int aev_init(Ctx* ctx) {
     for (int hi = 0, p = 0; hi < NSP; ++hi)            // the literal table above must match prio_sp()
         for (int lo = 0; lo <= hi; ++lo, ++p)
             if ((prio_sp(lo) | (prio_sp(hi) << 4)) != (int)h_pair_sp[p]) return DHP_E_BADARG;
-    DHP_CUDA(ctx, cudaFuncSetAttribute(k_aev_fwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(WarpSmemFwd) * AEV_WARPS)));
-    DHP_CUDA(ctx, cudaFuncSetAttribute(k_aev_fwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(WarpSmemFwd) * AEV_WARPS)));
-    DHP_CUDA(ctx, cudaFuncSetAttribute(k_aev_bwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(WarpSmemBwd) * BWD_WARPS)));
+    const int fs = (int)(sizeof(WarpSmemFwd) * AEV_WARPS), bs = (int)(sizeof(WarpSmemBwd) * BWD_WARPS);
+    DHP_CUDA(ctx, cudaFuncSetAttribute((k_aev_fwd<false, 8, 4>), cudaFuncAttributeMaxDynamicSharedMemorySize, fs));
+    DHP_CUDA(ctx, cudaFuncSetAttribute((k_aev_fwd<true, 8, 4>), cudaFuncAttributeMaxDynamicSharedMemorySize, fs));
+    DHP_CUDA(ctx, cudaFuncSetAttribute((k_aev_fwd<false, 4, 8>), cudaFuncAttributeMaxDynamicSharedMemorySize, fs));
+    DHP_CUDA(ctx, cudaFuncSetAttribute((k_aev_fwd<true, 4, 8>), cudaFuncAttributeMaxDynamicSharedMemorySize, fs));
+    DHP_CUDA(ctx, cudaFuncSetAttribute((k_aev_bwd<8, 4>), cudaFuncAttributeMaxDynamicSharedMemorySize, bs));
+    DHP_CUDA(ctx, cudaFuncSetAttribute((k_aev_bwd<4, 8>), cudaFuncAttributeMaxDynamicSharedMemorySize, bs));
     return DHP_OK;
 }
 
@@ -574,12 +587,13 @@ int aev_forward(Ctx* ctx, bool planes) {
     const int nw = ctx->partial ? (int)std::min<int64_t>(ctx->max_rows, (int64_t)n + NSP * ROW_ALIGN) : n;
     const int blocks = (nw + AEV_WARPS - 1) / AEV_WARPS;
     const size_t plane_stride = (size_t)ctx->max_rows * AEV_LD;
-    if (planes)
-        DHP_LAUNCH(ctx, k_aev_fwd<true>, blocks, AEV_WARPS * 32, smem, ctx->spos, ctx->row_ptr, ctx->col, ctx->seg_cnt, ctx->rowmap,
-                   ctx->tile_mask, ctx->grid, ctx->aevc, nw, ctx->aev, ctx->aev_planes, plane_stride, ctx->status, row_slot);
-    else
-        DHP_LAUNCH(ctx, k_aev_fwd<false>, blocks, AEV_WARPS * 32, smem, ctx->spos, ctx->row_ptr, ctx->col, ctx->seg_cnt, ctx->rowmap,
-                   ctx->tile_mask, ctx->grid, ctx->aevc, nw, ctx->aev, ctx->aev_planes, plane_stride, ctx->status, row_slot);
+#define DHP_AEV_FWD(P, A, Z)                                                                                                    \
+    DHP_LAUNCH(ctx, (k_aev_fwd<P, A, Z>), blocks, AEV_WARPS * 32, smem, ctx->spos, ctx->row_ptr, ctx->col, ctx->seg_cnt, ctx->rowmap, \
+               ctx->tile_mask, ctx->grid, ctx->aevc, nw, ctx->aev, ctx->aev_planes, plane_stride, ctx->status, row_slot)
+    const bool g84 = ctx->aevc.n_a == 8;                 // 8 x 4 (ANI-2x shape) or 4 x 8 (ANI-1x shape) angular grid
+    if (planes) { if (g84) DHP_AEV_FWD(true, 8, 4); else DHP_AEV_FWD(true, 4, 8); }
+    else        { if (g84) DHP_AEV_FWD(false, 8, 4); else DHP_AEV_FWD(false, 4, 8); }
+#undef DHP_AEV_FWD
     DHP_CUDA(ctx, cudaGetLastError());
     return DHP_OK;
 }
@@ -591,8 +605,12 @@ int aev_backward(Ctx* ctx, float* F_out) {
     // fsorted was zeroed with the rest of the per-call arena at the start of the call (nlist_build)
     const int* row_slot = ctx->partial ? ctx->row_slot : nullptr;
     const int nw = ctx->partial ? (int)std::min<int64_t>(ctx->max_rows, (int64_t)n + NSP * ROW_ALIGN) : n;
-    DHP_LAUNCH(ctx, k_aev_bwd, (nw + BWD_WARPS - 1) / BWD_WARPS, BWD_WARPS * 32, smem, ctx->spos, ctx->row_ptr, ctx->col,
-               ctx->seg_cnt, ctx->rowmap, ctx->grid, ctx->aevc, nw, ctx->grad, ctx->fsorted, row_slot);
+    if (ctx->aevc.n_a == 8)
+        DHP_LAUNCH(ctx, (k_aev_bwd<8, 4>), (nw + BWD_WARPS - 1) / BWD_WARPS, BWD_WARPS * 32, smem, ctx->spos, ctx->row_ptr, ctx->col,
+                   ctx->seg_cnt, ctx->rowmap, ctx->grid, ctx->aevc, nw, ctx->grad, ctx->fsorted, row_slot);
+    else
+        DHP_LAUNCH(ctx, (k_aev_bwd<4, 8>), (nw + BWD_WARPS - 1) / BWD_WARPS, BWD_WARPS * 32, smem, ctx->spos, ctx->row_ptr, ctx->col,
+                   ctx->seg_cnt, ctx->rowmap, ctx->grid, ctx->aevc, nw, ctx->grad, ctx->fsorted, row_slot);
     DHP_LAUNCH(ctx, k_unsort_forces, (n + 255) / 256, 256, 0, ctx->fsorted, ctx->perm, n, F_out);
     DHP_CUDA(ctx, cudaGetLastError());
     return DHP_OK;

@@ -20,6 +20,8 @@ static void default_params(dhp_params* p) {
     for (int m = 0; m < NR; ++m) p->shf_r[m] = (float)(0.8 + 0.2625 * m);
     for (int a = 0; a < NA; ++a) p->shf_a[a] = (float)(0.8 + 0.3375 * a);
     for (int z = 0; z < NZ; ++z) p->shf_z[z] = (float)((2.0 * z + 1.0) * 3.14159265358979323846 / 8.0);
+    for (int z = NZ; z < DHP_MAX_SHF_Z; ++z) p->shf_z[z] = 0.f;
+    p->n_shf_a = NA; p->n_shf_z = NZ;
 }
 
 static void make_aev_const(const dhp_params& p, AevConst* k) {
@@ -29,8 +31,12 @@ static void make_aev_const(const dhp_params& p, AevConst* k) {
     k->eta_r_l2e = (float)((double)p.eta_r * l2e); k->eta_a_l2e = (float)((double)p.eta_a * l2e);
     k->eta_r = p.eta_r; k->eta_a = p.eta_a; k->zeta = p.zeta;
     for (int m = 0; m < NR; ++m) k->shf_r[m] = p.shf_r[m];
-    for (int a = 0; a < NA; ++a) k->shf_a[a] = p.shf_a[a];
-    for (int z = 0; z < NZ; ++z) { k->cos_z[z] = (float)cos((double)p.shf_z[z]); k->sin_z[z] = (float)sin((double)p.shf_z[z]); }
+    k->n_a = p.n_shf_a; k->n_z = p.n_shf_z;
+    for (int a = 0; a < DHP_MAX_SHF_A; ++a) k->shf_a[a] = a < p.n_shf_a ? p.shf_a[a] : 0.f;
+    for (int z = 0; z < DHP_MAX_SHF_Z; ++z) {
+        k->cos_z[z] = z < p.n_shf_z ? (float)cos((double)p.shf_z[z]) : 0.f;
+        k->sin_z[z] = z < p.n_shf_z ? (float)sin((double)p.shf_z[z]) : 0.f;
+    }
 }
 
 template <typename T>
@@ -175,6 +181,7 @@ int dhp_create(dhp_ctx** out, const dhp_params* params, int64_t max_atoms, int64
     c->stream = (cudaStream_t)cuda_stream;
     if (params) c->params = *params; else default_params(&c->params);
     if (!(c->params.rca > 0.f) || !(c->params.rcr >= c->params.rca) || !(c->params.celu_alpha > 0.f)) { delete h; return DHP_E_BADARG; }
+    if (!((c->params.n_shf_a == 8 && c->params.n_shf_z == 4) || (c->params.n_shf_a == 4 && c->params.n_shf_z == 8))) { delete h; return DHP_E_BADARG; }
     make_aev_const(c->params, &c->aevc);
     int dev = 0;
     cudaDeviceProp prop;

@@ -63,8 +63,9 @@ struct AevConst {
     float eta_r_l2e;            // eta_r * log2(e)
     float eta_a_l2e;
     float eta_r, eta_a, zeta;
-    float shf_r[NR], shf_a[NA];
-    float cos_z[NZ], sin_z[NZ];
+    float shf_r[NR], shf_a[DHP_MAX_SHF_A];
+    float cos_z[DHP_MAX_SHF_Z], sin_z[DHP_MAX_SHF_Z];
+    int n_a, n_z;               // angular grid: 8 x 4 (ANI-2x shape) or 4 x 8 (ANI-1x shape); n_a * n_z = 32
 };
 
 struct Weights {

@@ -31,7 +31,12 @@ def test_library_builds_loads_and_exports_everything():
 
 def test_params_struct_matches_header():
     import ctypes
-    assert ctypes.sizeof(binding.DhpParams) == 4 * (6 + 16 + 8 + 4)
+    # 6 scalars, shf_r[16], shf_a[8], shf_z[8], n_shf_a, n_shf_z (include/dhp.h: dhp_params)
+    assert ctypes.sizeof(binding.DhpParams) == 4 * (6 + 16 + 8 + 8 + 2)
+    from paper_2207_14276_b200 import workloads as W
+    for p, grid in ((W.default_params(), (8, 4)), (W.ani1x_params(), (4, 8))):
+        q = binding.make_params(p)
+        assert (q.n_shf_a, q.n_shf_z) == grid and abs(q.shf_z[grid[1] - 1] - float(p.shf_z[-1])) < 1e-7
 
 
 def test_no_cpu_fallback_without_gpu():

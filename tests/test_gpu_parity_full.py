@@ -229,3 +229,48 @@ def test_collinear_cusp_sensitivity_is_bounded(torch, B, params, blob8):
     assert err[3:].max() <= F_TOL                              # atoms not on the line are unaffected
     assert np.abs(F.sum(0)).max() < 1e-5                       # Newton's third law survives the cusp
     d.close()
+
+
+# ------------------------------------------------------------------------------------------- ANI-1x shape (row f3)
+@pytest.mark.parametrize("mode", [1, 2])
+def test_ani1x_shape_four_species_box(torch, B, blob8, mode):
+    """SURVEY.md §8(f3), PAPER.md L87 / L159: the ANI-1x / ANI-1ccx shape - species H, C, N, O, Rcr = 5.2 Å (L73),
+    4 x 8 angular grid, 384 features, networks 384 -> 160 -> 128 -> 96 -> 1 (reading R4) - through the same
+    library: `dhp_params` selects the grid, the narrow networks are loaded zero-padded (workloads.embed_ani1x).  Lists
+    bit-exact at the 5.2 Å cutoff, AEV / dE/dG rows, E and F against the oracle, SIMT and tensor paths."""
+    p1x = W.ani1x_params()
+    s = W.small_periodic_mix(900, 21.0, seed=31, n_models=2, hcno_only=True)
+    blob = W.embed_ani1x(W.make_weights_ani1x(2), 2)
+    d = B.Dhp(s.n_atoms, params=p1x)
+    if mode == 2 and not d.dhp_tensor_path_available():
+        d.close()
+        pytest.skip("tensor path not available in this build")
+    d.dhp_set_mlp_mode(mode)
+    w = d.dhp_weights_load(blob, 2)
+    pos, sp, mol = B.to_device(s)
+    E, F = d.dhp_ani_energy_forces(pos, s.box, sp, w)
+    torch.cuda.synchronize()
+    assert d.dhp_status() == 0
+    Ea, Fo, go = oracle.energy_forces(s.pos, s.species, s.box, p1x, blob, 2, want_dEdG=True)
+    assert abs(E.item() - Ea.sum()) / s.n_atoms <= E_TOL_PER_ATOM
+    assert np.max(np.abs(F.cpu().numpy() - Fo)) <= F_TOL
+    G = d.dhp_debug_aev().cpu().numpy()
+    Go = oracle.aev(s.pos, s.species, s.box, p1x)
+    assert np.max(np.abs(G - Go)) <= AEV_TOL
+    fmap = W.ani1x_feature_map()
+    off = np.ones(1008, bool)
+    off[fmap] = False
+    assert np.all(G[:, off] == 0.0)                              # only the 384 ANI-1x features exist
+    g = d.dhp_debug_grad().cpu().numpy()
+    close = np.abs(g - go) <= GRAD_TOL
+    assert np.all(close | ((g == 0) & (Go == 0))) and np.all(close[Go != 0])
+    lists_equal(B, d, s, p1x)
+    d.close()
+
+
+def test_ani1x_params_are_validated(torch, B):
+    import dataclasses
+    p = W.ani1x_params()
+    bad = dataclasses.replace(p, shf_z=p.shf_z[:4])              # 4 x 4: not one of the two grids
+    with pytest.raises(B.DhpError):
+        B.Dhp(16, params=bad)
