@@ -189,6 +189,7 @@ int dhp_create(dhp_ctx** out, const dhp_params* params, int64_t max_atoms, int64
     c->sm_count = prop.multiProcessorCount;
     { const char* e = getenv("DHP_NO_SMALL_PATH"); c->no_small_path = e && e[0] == '1'; }
     { const char* e = getenv("DHP_TC_PAIRS"); c->tc_pairs = (e && e[0] >= '0' && e[0] <= '3') ? e[0] - '0' : 0; }   // cta_group::2 kernels
+    { const char* e = getenv("DHP_TC_TWO"); c->tc_two = (e && e[0] >= '0' && e[0] <= '3') ? e[0] - '0' : 2; }   // two row tiles per CTA: B1 by default
     c->cc_major = prop.major;
     c->max_atoms = max_atoms;
     c->max_mols = max_mols;

@@ -577,6 +577,282 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
 }
 
 // ======================================================================================================
+// G1 and B1 with TWO row tiles per CTA.  Experiments (profiles/r2b_*.md) show the one-tile kernel above bound by the
+// chip-wide L2 -> SM throughput (about 50 B/clk/SM with all 148 SMs streaming): one 64-wide K block of one 128-row tile
+// brings 96 KB (A 32 KB, W 64 KB) for 1 536 MMA cycles.  Here the two row tiles of a pair (same species, same feature-
+// block mask: nlist.cu keeps both pair-uniform) share every weight K block: W is fetched once, the MMAs of tile 0
+// accumulate into TMEM columns [0, 256) and those of tile 1 into [256, 512).  Per K block: 128 KB for 3 072 MMA cycles
+// (42 B/clk) in G1, and for a 3-block column tile of B1 112 KB for 2 304 cycles (49 B/clk, was 71).  The price: both
+// accumulator stages belong to the item in flight, so the epilogue of an item overlaps only the first K blocks of the
+// next one (tile 0's accumulator is released first) - small against B1's 32 K blocks, visible in G1.
+//   smem: W ring 2 x 64 KB (hi plane, lo plane), A ring 3 x 32 KB (hi, lo); roles as in k_gemm_tc.
+// ======================================================================================================
+constexpr int T2_WSLOTS = 2, T2_ASLOTS = 3;
+constexpr int T2_W_BYTES = 2 * B_SLOT_BYTES;          // 64 KB
+constexpr int T2_A_BYTES = 2 * A_PLANE_BYTES;         // 32 KB
+constexpr int T2_SMEM = T2_WSLOTS * T2_W_BYTES + T2_ASLOTS * T2_A_BYTES + 1024 /*align*/ + 256 /*barriers, TMEM word, ring*/;
+
+template <int EPI, int CMP>
+__global__ void __launch_bounds__(TC_THREADS, 1)
+k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const TcArgs p) {
+    static_assert((EPI == EPI_CELU && CMP == CMP_K) || (EPI == EPI_GRAD && CMP == CMP_N), "two-tile kernel: G1 and B1 only");
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t raw = smem_u32(smem_raw);
+    const uint32_t base = (raw + 1023u) & ~1023u;
+    uint8_t* base_ptr = smem_raw + (base - raw);
+    const uint32_t wring = base, aring = base + T2_WSLOTS * T2_W_BYTES;
+    constexpr int DATA = T2_WSLOTS * T2_W_BYTES + T2_ASLOTS * T2_A_BYTES;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(base_ptr + DATA);
+    const uint32_t bar0 = base + DATA;
+    // barriers: wfull[2], wempty[2], afull[3], aempty[3], tfull[2], tempty[2], sfull[RING], sempty[RING]
+    constexpr int NBARS = 2 * T2_WSLOTS + 2 * T2_ASLOTS + 4 + 2 * RING;
+    auto wfull_bar = [&](int s) { return bar0 + 8u * s; };
+    auto wempty_bar = [&](int s) { return bar0 + 8u * (T2_WSLOTS + s); };
+    auto afull_bar = [&](int s) { return bar0 + 8u * (2 * T2_WSLOTS + s); };
+    auto aempty_bar = [&](int s) { return bar0 + 8u * (2 * T2_WSLOTS + T2_ASLOTS + s); };
+    auto tfull_bar = [&](int s) { return bar0 + 8u * (2 * T2_WSLOTS + 2 * T2_ASLOTS + s); };
+    auto tempty_bar = [&](int s) { return bar0 + 8u * (2 * T2_WSLOTS + 2 * T2_ASLOTS + 2 + s); };
+    auto sfull_bar = [&](int s) { return bar0 + 8u * (2 * T2_WSLOTS + 2 * T2_ASLOTS + 4 + s); };
+    auto sempty_bar = [&](int s) { return bar0 + 8u * (2 * T2_WSLOTS + 2 * T2_ASLOTS + 4 + RING + s); };
+    volatile uint32_t* tmem_word = reinterpret_cast<volatile uint32_t*>(bars + NBARS);
+    volatile int* ring = reinterpret_cast<volatile int*>(bars + NBARS + 1);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n_pairs = p.sp_start[NSP] / (2 * BM);            // species groups are aligned to 256 rows
+    const int total_items = n_pairs * p.n_tiles;
+    const int KB = (p.K + BK - 1) / BK;
+    const unsigned all_k = KB >= 32 ? 0xffffffffu : ((1u << KB) - 1u);
+
+    if (warp == EPI_WARPS && lane == 0) {
+        for (int s = 0; s < T2_WSLOTS; ++s) { mbar_init(wfull_bar(s), 1); mbar_init(wempty_bar(s), 1); }
+        for (int s = 0; s < T2_ASLOTS; ++s) { mbar_init(afull_bar(s), 1); mbar_init(aempty_bar(s), 1); }
+        for (int s = 0; s < 2; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), EPI_WARPS); }
+        for (int s = 0; s < RING; ++s) { mbar_init(sfull_bar(s), 1); mbar_init(sempty_bar(s), 1 + EPI_WARPS); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        prefetch_tmap(&tmA);
+        prefetch_tmap(&tmB);
+    }
+    if (warp == EPI_WARPS + 1) tmem_alloc(smem_u32((const void*)tmem_word), TMEM_COLS);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_word;
+
+    // tile masks are pair-uniform (nlist.cu): the first tile's mask speaks for both
+    auto k_mask = [&](int pr) -> unsigned {
+        if (CMP != CMP_K) return all_k;
+        const unsigned m = p.tile_mask[2 * pr];
+        return m ? m : (1u << 14);                             // an all-zero pair still runs one block of zeros
+    };
+
+    if (warp == EPI_WARPS) {
+        // ===== item scheduler + producer =====
+        if (elect_one()) {
+            int ws = 0; uint32_t wphase = 0;
+            int as = 0; uint32_t aphase = 0;
+            int slot = 0; uint32_t sphase = 0;
+            for (;;) {
+                int item, pr = 0, nt = 0;
+                for (;;) {
+                    int t = atomicAdd(p.sched, 1);
+                    if (CMP == CMP_N) {
+                        // B1: an item's cost is its number of feature blocks (1..4) x all of K, and there are only a few
+                        // items per SM: hand them out LONGEST FIRST (four passes over the items: 4, 3, 2, 1 blocks), so that
+                        // the tail of the launch is made of short items
+                        if (t >= 4 * total_items) { item = -1; break; }
+                        const int pass = t / total_items;
+                        item = t - pass * total_items;
+                        pr = item / p.n_tiles; nt = item - pr * p.n_tiles;
+                        if (min(4, __popc(p.tile_mask[2 * pr]) - 4 * nt) == 4 - pass) break;
+                    } else {
+                        item = t;
+                        if (item >= total_items) { item = -1; break; }
+                        pr = item / p.n_tiles; nt = item - pr * p.n_tiles;
+                        break;
+                    }
+                }
+                mbar_wait(sempty_bar(slot), sphase ^ 1u);
+                ring[slot] = item;
+                mbar_arrive(sfull_bar(slot));
+                if (++slot == RING) { slot = 0; sphase ^= 1u; }
+                if (item < 0) break;
+                const int s = max(p.row_species[2 * pr * BM], 0);
+                int brow = (2 * s) * p.b_rows_per_species;
+                int sel[4] = {0, 0, 0, 0};
+                int nb = 0;
+                uint32_t wtx;
+                if (CMP == CMP_N) {
+                    nb = select_blocks(p.tile_mask[2 * pr], nt, sel);
+                    wtx = 2u * (uint32_t)nb * NB_BLOCK_BYTES;
+                } else {
+                    brow += nt * p.b_rows_per_tile;
+                    wtx = 2u * (uint32_t)p.BN * BK * 2u;
+                }
+                for (unsigned km = k_mask(pr); km; km &= km - 1u) {
+                    const int kb = __ffs(km) - 1;
+                    // the weight K block, once for both row tiles
+                    mbar_wait(wempty_bar(ws), wphase ^ 1u);
+                    const uint32_t sb = wring + ws * T2_W_BYTES;
+                    mbar_expect_tx(wfull_bar(ws), wtx);
+                    if (CMP == CMP_N) {
+#pragma unroll
+                        for (int j = 0; j < 4; ++j)
+                            if (j < nb) {
+                                tma_load_2d(sb + j * NB_BLOCK_BYTES, &tmB, kb * BK, brow + sel[j] * KBLK, wfull_bar(ws));
+                                tma_load_2d(sb + B_SLOT_BYTES + j * NB_BLOCK_BYTES, &tmB, kb * BK,
+                                            brow + p.b_rows_per_species + sel[j] * KBLK, wfull_bar(ws));
+                            }
+                    } else {
+                        tma_load_2d(sb, &tmB, kb * BK, brow, wfull_bar(ws));
+                        tma_load_2d(sb + B_SLOT_BYTES, &tmB, kb * BK, brow + p.b_rows_per_species, wfull_bar(ws));
+                    }
+                    if (++ws == T2_WSLOTS) { ws = 0; wphase ^= 1u; }
+                    // the A tiles of the two rows tiles
+#pragma unroll
+                    for (int r = 0; r < 2; ++r) {
+                        const int rt = 2 * pr + r;
+                        mbar_wait(aempty_bar(as), aphase ^ 1u);
+                        const uint32_t sa = aring + as * T2_A_BYTES;
+                        mbar_expect_tx(afull_bar(as), (uint32_t)T2_A_BYTES);
+                        if (p.a_tiled) {
+                            const int kba = p.a_kb_per_tile * nt + kb;
+                            bulk_load(sa, p.a_tiled + tile_off(p.plane_tiles, p.a_kblocks, 0, rt, kba), A_PLANE_BYTES, afull_bar(as));
+                            bulk_load(sa + A_PLANE_BYTES, p.a_tiled + tile_off(p.plane_tiles, p.a_kblocks, 1, rt, kba), A_PLANE_BYTES,
+                                      afull_bar(as));
+                        } else {
+                            const int ka = p.a_k_off_per_tile * nt + kb * BK;
+                            tma_load_2d(sa, &tmA, ka, rt * BM, afull_bar(as));
+                            tma_load_2d(sa + A_PLANE_BYTES, &tmA, ka, p.a_plane_rows + rt * BM, afull_bar(as));
+                        }
+                        if (++as == T2_ASLOTS) { as = 0; aphase ^= 1u; }
+                    }
+                }
+            }
+        }
+    } else if (warp == EPI_WARPS + 1) {
+        // ===== MMA issuer =====
+        if (elect_one()) {
+            int ws = 0; uint32_t wphase = 0;
+            int as = 0; uint32_t aphase = 0;
+            uint32_t acc_phase = 0;
+            int slot = 0; uint32_t sphase = 0;
+            for (;;) {
+                mbar_wait(sfull_bar(slot), sphase);
+                const int item = ring[slot];
+                mbar_arrive(sempty_bar(slot));
+                if (++slot == RING) { slot = 0; sphase ^= 1u; }
+                if (item < 0) break;
+                const int pr = item / p.n_tiles, nt = item - pr * p.n_tiles;
+                int bn = p.BN;
+                if (CMP == CMP_N) bn = KBLK * min(4, __popc(p.tile_mask[2 * pr]) - 4 * nt);
+                const uint32_t idesc = make_idesc(bn);
+                uint32_t accumulate = 0u;
+                const bool tiled = p.a_tiled != nullptr;
+                const uint64_t a_step = tiled ? (uint64_t)(4096 >> 4) : 2u;
+                for (unsigned km = k_mask(pr); km; km &= km - 1u) {
+                    const int kb = __ffs(km) - 1;
+                    mbar_wait(wfull_bar(ws), wphase);
+                    const uint32_t sb = wring + ws * T2_W_BYTES;
+                    const uint64_t b_hi = make_smem_desc(sb), b_lo = make_smem_desc(sb + B_SLOT_BYTES);
+                    const int ksteps = min(BK / 16, (p.K - kb * BK) / 16);
+#pragma unroll
+                    for (int r = 0; r < 2; ++r) {
+                        if (accumulate == 0u) {                       // first K block of the item: the accumulator must be drained
+                            mbar_wait(tempty_bar(r), acc_phase ^ 1u);
+                        }
+                        mbar_wait(afull_bar(as), aphase);
+                        tc_fence_after();
+                        const uint32_t sa = aring + as * T2_A_BYTES;
+                        const uint64_t a_hi = tiled ? make_smem_desc_tiled(sa) : make_smem_desc(sa);
+                        const uint64_t a_lo = tiled ? make_smem_desc_tiled(sa + A_PLANE_BYTES) : make_smem_desc(sa + A_PLANE_BYTES);
+                        const uint32_t d_tmem = tmem_base + (uint32_t)(r * ACC_STRIDE);
+                        for (int k = 0; k < ksteps; ++k) {
+                            const uint64_t adv = (uint64_t)(k * 2), a_adv = (uint64_t)k * a_step;
+                            umma_f16(d_tmem, a_hi + a_adv, b_hi + adv, idesc, (accumulate | (uint32_t)(k > 0)));
+                            if (!p.single) {
+                                umma_f16(d_tmem, a_hi + a_adv, b_lo + adv, idesc, 1u);
+                                umma_f16(d_tmem, a_lo + a_adv, b_hi + adv, idesc, 1u);
+                            }
+                        }
+                        umma_commit(aempty_bar(as));
+                        if (++as == T2_ASLOTS) { as = 0; aphase ^= 1u; }
+                    }
+                    accumulate = 1u;
+                    umma_commit(wempty_bar(ws));
+                    if (++ws == T2_WSLOTS) { ws = 0; wphase ^= 1u; }
+                }
+                umma_commit(tfull_bar(0));                             // both accumulators complete -> epilogue
+                umma_commit(tfull_bar(1));
+                acc_phase ^= 1u;
+            }
+        }
+    } else {
+        // ===== epilogue (warps 0..7): tile 0's accumulator first, so that the next item's MMAs can start on it =====
+        const int q = warp & 3, half = warp >> 2;
+        uint32_t acc_phase = 0;
+        int slot = 0; uint32_t sphase = 0;
+        const float kexp = 1.4426950408889634f / p.alpha;
+        for (;;) {
+            mbar_wait(sfull_bar(slot), sphase);
+            const int item = ring[slot];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(sempty_bar(slot));
+            if (++slot == RING) { slot = 0; sphase ^= 1u; }
+            if (item < 0) break;
+            const int pr = item / p.n_tiles, nt = item - pr * p.n_tiles;
+            const int s = max(p.row_species[2 * pr * BM], 0);
+            const int ncols = p.n_tiles * p.BN;
+            const int r_in = q * 32 + lane;
+            int sel[4] = {0, 0, 0, 0};
+            int bn = p.BN;
+            if (CMP == CMP_N) bn = KBLK * select_blocks(p.tile_mask[2 * pr], nt, sel);
+#pragma unroll 1
+            for (int r = 0; r < 2; ++r) {
+                const int rt = 2 * pr + r;
+                const int row = rt * BM + r_in;
+                mbar_wait(tfull_bar(r), acc_phase);
+                tc_fence_after();
+                const uint32_t t_row = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(r * ACC_STRIDE);
+                for (int c0 = half * 32; c0 < bn; c0 += 64) {
+                    const int col = nt * p.BN + c0;
+                    uint32_t v[32];
+                    tmem_ld32_issue(t_row + (uint32_t)c0, v);
+                    if (EPI == EPI_CELU) {
+                        float x[32], aux[32];
+                        load32(p.bias + (size_t)s * ncols + col, aux);
+                        const int ocol = nt * p.out_cols_per_tile + c0;
+                        const size_t in_tile = (size_t)(((ocol & 63) >> 3) * BM + r_in) * 8;
+                        const size_t o_hi = tile_off(p.plane_tiles, p.out_kblocks, 0, rt, ocol >> 6) + in_tile;
+                        const size_t o_lo = tile_off(p.plane_tiles, p.out_kblocks, 1, rt, ocol >> 6) + in_tile;
+                        tmem_ld_wait();
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) x[i] = celu_f(fmaf(__uint_as_float(v[i]), p.acc_scale, aux[i]), p.alpha, kexp);
+                        store_split32_tiled(x, p.out_planes + o_hi, p.out_planes + o_lo);
+                    } else {   // EPI_GRAD: chunk c0 belongs to the (c0/64)-th selected block
+                        const int j = c0 >> 6;
+                        const int blk = j == 0 ? sel[0] : j == 1 ? sel[1] : j == 2 ? sel[2] : sel[3];
+                        const int gcol = blk * KBLK + (c0 & 63);
+                        float4* dst = reinterpret_cast<float4*>(p.out_f32 + (size_t)row * p.out_ld + gcol);
+                        tmem_ld_wait();
+#pragma unroll
+                        for (int i = 0; i < 8; ++i)
+                            dst[i] = make_float4(__uint_as_float(v[4 * i]) * p.acc_scale, __uint_as_float(v[4 * i + 1]) * p.acc_scale,
+                                                 __uint_as_float(v[4 * i + 2]) * p.acc_scale, __uint_as_float(v[4 * i + 3]) * p.acc_scale);
+                    }
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(tempty_bar(r));
+            }
+            acc_phase ^= 1u;
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == EPI_WARPS + 1) tmem_dealloc(tmem_base, TMEM_COLS);
+}
+
+// ======================================================================================================
 // G1 and B1 on CTA PAIRS (tcgen05 cta_group::2).  profiles/r1e + the single-pass experiment show
 // the one-CTA kernel above at the point where the L2 -> shared-memory fill (96 KB per 64-wide K block of one 128-row
 // tile, 1 536 MMA cycles) and the tensor pipe are both near their limits.  Here two CTAs of a cluster take two
@@ -1645,6 +1921,12 @@ int launch_gemm(Ctx* ctx, const CUtensorMap& a, const CUtensorMap& b, const TcAr
 }
 
 template <int EPI, int CMP>
+int launch_gemm2(Ctx* ctx, const CUtensorMap& a, const CUtensorMap& b, const TcArgs& args) {
+    DHP_LAUNCH(ctx, (k_gemm_tc2<EPI, CMP>), ctx->sm_count, TC_THREADS, T2_SMEM, a, b, args);
+    return DHP_OK;
+}
+
+template <int EPI, int CMP>
 int launch_pair(Ctx* ctx, const CUtensorMap& a, const CUtensorMap& b, const TcArgs& args) {
     DHP_LAUNCH(ctx, (k_gemm_pair<EPI, CMP>), ctx->sm_count & ~1, TC_THREADS, P_SMEM_BYTES, a, b, args);
     return DHP_OK;
@@ -1670,6 +1952,8 @@ int mlp_tc_alloc(Ctx* ctx) {
     DHP_CUDA(ctx, cudaFuncSetAttribute((k_gemm_pair<EPI_CELU, CMP_K>), cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM_BYTES));
     DHP_CUDA(ctx, cudaFuncSetAttribute((k_gemm_pair<EPI_GRAD, CMP_N>), cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM_BYTES));
     DHP_CUDA(ctx, cudaFuncSetAttribute(k_mlp_mid, cudaFuncAttributeMaxDynamicSharedMemorySize, MID_SMEM));
+    DHP_CUDA(ctx, cudaFuncSetAttribute((k_gemm_tc2<EPI_CELU, CMP_K>), cudaFuncAttributeMaxDynamicSharedMemorySize, T2_SMEM));
+    DHP_CUDA(ctx, cudaFuncSetAttribute((k_gemm_tc2<EPI_GRAD, CMP_N>), cudaFuncAttributeMaxDynamicSharedMemorySize, T2_SMEM));
     TcWorkspace* w = new (std::nothrow) TcWorkspace();
     if (!w) return DHP_E_NOMEM;
     memset((void*)w, 0, sizeof(*w));
@@ -1769,7 +2053,13 @@ int mlp_tc(Ctx* ctx, const Weights* wt, bool forward_only) {
         DHP_LAUNCH(ctx, k_pair_schedule, 1, 1024, 0, ctx->tile_mask, ctx->sp_start, M, ncl, ws->pair_scratch, ws->pair_sched);
         a.pair_start = ws->pair_sched;
     }
+    // two row tiles per CTA (k_gemm_tc2) pay when there are enough tile pairs to keep every SM busy for several items
+    const int64_t n_pairs_bound = (ctx->n_atoms + 2 * ROW_TILE - 1) / (2 * ROW_TILE);
+    const bool big = n_pairs_bound * M >= 12 * (int64_t)ctx->sm_count;
+    const bool two_g1 = fusedp && !pairs && ((ctx->tc_two & 1) != 0) && big;
+    const bool two_b1 = fusedp && !pairs_b1 && ((ctx->tc_two & 2) != 0) && big;
     if (pairs) rc = launch_pair<EPI_CELU, CMP_K>(ctx, ws->m_aev, t->m_w1f_half, a);
+    else if (two_g1) rc = launch_gemm2<EPI_CELU, CMP_K>(ctx, ws->m_aev, t->m_w1f, a);
     else rc = launch_gemm<EPI_CELU, CMP_K>(ctx, ws->m_aev, t->m_w1f, a);
     if (rc != DHP_OK) return rc;
     prof_mark(ctx, DHP_PHASE_MLP_MID);
@@ -1821,13 +2111,14 @@ int mlp_tc(Ctx* ctx, const Weights* wt, bool forward_only) {
         const int KBt = (M * H1) / BK;                                                       // 4 K blocks per network
         int ks = 1;
         while (ks * 2 <= KBt && KBt % (ks * 2) == 0 && tiles_bound * ks * 2 <= ctx->sm_count) ks *= 2;
-        a.ksplit = pairs_b1 ? 1 : ks;
+        a.ksplit = (pairs_b1 || two_b1) ? 1 : ks;
         if (a.ksplit > 1)
             DHP_CUDA(ctx, cudaMemsetAsync(ctx->grad, 0, sizeof(float) * (size_t)std::min<int64_t>(tiles_bound * ROW_TILE, ctx->max_rows) * AEV_LD,
                                           ctx->stream));
     }
     a.pair_start = ws->pair_sched + (ncl + 1);
     if (pairs_b1) rc = launch_pair<EPI_GRAD, CMP_N>(ctx, ws->m_aev, t->m_w1b_half, a);
+    else if (two_b1) rc = launch_gemm2<EPI_GRAD, CMP_N>(ctx, ws->m_aev, t->m_w1b, a);
     else rc = launch_gemm<EPI_GRAD, CMP_N>(ctx, ws->m_aev, t->m_w1b, a);
     if (rc != DHP_OK) return rc;
     DHP_CUDA(ctx, cudaGetLastError());
