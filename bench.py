@@ -270,9 +270,8 @@ def main():
     if rank == 0:
         sampler.start()
         time.sleep(0.3)
-    d.dhp_profile_enable(True)
-    d.dhp_profile_reset()
     l0 = d.dhp_launch_count()
+    g0 = d.dhp_graph_replays()
     stream = torch.cuda.current_stream()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
@@ -283,6 +282,13 @@ def main():
     barrier()
     ms_total = ev0.elapsed_time(ev1)
     launches = d.dhp_launch_count() - l0
+    graph_replays = d.dhp_graph_replays() - g0
+    # per-phase CUDA events in a second pass over the same K steps: the events sit between the kernels, so small systems
+    # (whose call is otherwise replayed as one CUDA graph) take the plain enqueue path while they are on
+    d.dhp_profile_enable(True)
+    d.dhp_profile_reset()
+    for k in range(args.steps):
+        step(k)
     phase_ms, calls = d.dhp_profile_read()
     d.dhp_profile_enable(False)
     n_row_tiles, n_active_blocks = d.dhp_debug_tile_blocks()
@@ -521,7 +527,7 @@ def main():
             "ns_per_day_at_0.5fs": value / atoms_all * NS_PER_DAY_PER_EVAL_PER_S,   # per replica
             "evals_per_s_per_gpu": value / atoms_all,
             "phase_ms": ph,
-            "gpu_launches": int(launches),
+            "gpu_launches": int(launches), "graph_replays": int(graph_replays),
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "ms_per_step": e2e_ms / args.steps},

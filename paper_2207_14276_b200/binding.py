@@ -54,6 +54,7 @@ SYMBOLS = {
     "dhp_profile_reset": (C.c_int, [_vp]),
     "dhp_profile_read": (C.c_int, [_vp, C.POINTER(C.c_double), C.POINTER(_i64)]),
     "dhp_launch_count": (_i64, [_vp]),
+    "dhp_graph_replays": (_i64, [_vp]),
     "dhp_strerror": (C.c_char_p, [_i32]),
     "dhp_last_cuda_error": (C.c_char_p, [_vp]),
     "dhp_version": (C.c_char_p, []),
@@ -392,6 +393,9 @@ class Dhp:
 
     def dhp_launch_count(self) -> int:
         return int(self.lib.dhp_launch_count(self.ctx))
+
+    def dhp_graph_replays(self) -> int:
+        return int(self.lib.dhp_graph_replays(self.ctx))
 
 
 def to_device(system, device="cuda:0"):

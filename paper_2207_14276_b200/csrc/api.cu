@@ -45,7 +45,10 @@ static bool dalloc(T** p, size_t count) {
     return cudaMalloc((void**)p, sizeof(T) * (count ? count : 1)) == cudaSuccess;
 }
 
+static void graphs_invalidate(Ctx* ctx);
 static void free_all(Ctx* c) {
+    graphs_invalidate(c);
+    if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     void* ptrs[] = {c->sticky, c->cand_bad, c->grid, c->zero_arena, c->ff_arena, c->bbox, c->cell_of, c->perm_tmp, c->cell_start, c->perm,
                     c->inv_perm, c->spos, c->smol, c->snc, c->n_rad, c->n_ang, c->row_ptr, c->col, c->sp_count, c->sp_start,
                     c->rowmap, c->blk_hist, c->key_start, c->amask, c->col2feat, c->aev, c->grad,
@@ -88,9 +91,9 @@ static void prof_drain(Ctx* ctx) {
     p.n_pending = 0;
 }
 
-static int run_energy_forces(Ctx* ctx, const float* pos, const float* box, const int32_t* species, int64_t n,
-                             const int32_t* mol_offsets, int64_t n_mol, const Weights* w, double* E, float* F,
-                             const uint8_t* central = nullptr) {
+static int enqueue_energy_forces(Ctx* ctx, const float* pos, const float* box, const int32_t* species, int64_t n,
+                                 const int32_t* mol_offsets, int64_t n_mol, const Weights* w, double* E, float* F,
+                                 const uint8_t* central = nullptr) {
     ctx->prof.cur_slot = -1;
     if (ctx->prof.on) {
         if (ctx->prof.n_pending == 64) prof_drain(ctx);
@@ -120,6 +123,76 @@ static int run_energy_forces(Ctx* ctx, const float* pos, const float* box, const
     prof_mark(ctx, DHP_N_PHASES);
     ctx->prof.cur_slot = -1;
     ctx->n_models = w->n_models;
+    return DHP_OK;
+}
+
+static void graphs_invalidate(Ctx* ctx) {
+    for (GraphEntry& g : ctx->graphs) {
+        if (g.used && g.exec) cudaGraphExecDestroy(g.exec);
+        g.used = false; g.exec = nullptr;
+    }
+}
+
+// The hot call.  Large systems: enqueue the kernels.  Small systems (n <= SMALL_N: the solute of the hybrid scheme, PAPER.md
+// L112-118, L200-208 - the call RESPA's outer step makes): the same enqueue is captured ONCE per argument set into a CUDA
+// graph on the library's own stream and replayed on the caller's stream afterwards - same kernels, same arithmetic, no
+// per-launch host work and no gaps between a dozen dependent 15-40 us launches.  A changed pointer, size, box or mode is a
+// new graph (4 are kept, least recently used first out).
+static int run_energy_forces(Ctx* ctx, const float* pos, const float* box, const int32_t* species, int64_t n,
+                             const int32_t* mol_offsets, int64_t n_mol, const Weights* w, double* E, float* F,
+                             const uint8_t* central = nullptr) {
+    const bool small = ctx->graph_on && n > 0 && n <= SMALL_N && !(ctx->skin > 0.f) && !ctx->prof.on;
+    if (!small) return enqueue_energy_forces(ctx, pos, box, species, n, mol_offsets, n_mol, w, E, F, central);
+    float bx[4] = {0.f, 0.f, 0.f, box ? 1.f : 0.f};
+    if (box) for (int c = 0; c < 3; ++c) bx[c] = box[c];
+    GraphEntry* hit = nullptr;
+    GraphEntry* victim = &ctx->graphs[0];
+    for (GraphEntry& g : ctx->graphs) {
+        if (g.used && g.pos == pos && g.species == species && g.mol == mol_offsets && g.central == central && g.weights == w && g.E == E &&
+            g.F == F && g.n == n && g.n_mol == n_mol && g.mlp_mode == ctx->mlp_mode && memcmp(g.box, bx, sizeof(bx)) == 0) { hit = &g; break; }
+        if (!g.used || (victim->used && g.stamp < victim->stamp)) victim = &g;
+    }
+    if (!hit) {
+        if (victim->used && victim->exec) cudaGraphExecDestroy(victim->exec);
+        victim->used = false; victim->exec = nullptr;
+        cudaStream_t user = ctx->stream;
+        if (cudaStreamBeginCapture(ctx->cap_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+            cudaGetLastError();
+            ctx->graph_on = false;                      // capture is not possible here: plain enqueue from now on
+            return enqueue_energy_forces(ctx, pos, box, species, n, mol_offsets, n_mol, w, E, F, central);
+        }
+        ctx->stream = ctx->cap_stream;
+        const int64_t l0 = ctx->launches;
+        const int rc = enqueue_energy_forces(ctx, pos, box, species, n, mol_offsets, n_mol, w, E, F, central);
+        ctx->stream = user;
+        cudaGraph_t graph = nullptr;
+        const cudaError_t e1 = cudaStreamEndCapture(ctx->cap_stream, &graph);
+        if (rc != DHP_OK) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return rc; }
+        cudaGraphExec_t exec = nullptr;
+        const cudaError_t e2 = e1 == cudaSuccess ? cudaGraphInstantiate(&exec, graph, 0) : e1;
+        if (graph) cudaGraphDestroy(graph);
+        if (e2 != cudaSuccess) {                          // could not build the graph: run the call the plain way
+            cudaGetLastError();
+            ctx->graph_on = false;
+            ctx->launches = l0;
+            return enqueue_energy_forces(ctx, pos, box, species, n, mol_offsets, n_mol, w, E, F, central);
+        }
+        hit = victim;
+        hit->used = true; hit->exec = exec;
+        hit->pos = pos; hit->species = species; hit->mol = mol_offsets; hit->central = central; hit->weights = w; hit->E = E; hit->F = F;
+        hit->n = n; hit->n_mol = n_mol; hit->mlp_mode = ctx->mlp_mode; memcpy(hit->box, bx, sizeof(bx));
+        hit->launches = ctx->launches - l0;
+        hit->s_n_mol = ctx->n_mol; hit->s_periodic = ctx->periodic; hit->s_partial = ctx->partial; hit->s_planes = ctx->aev_in_planes;
+        hit->s_models = ctx->n_models;
+        ctx->launches = l0;                               // counted per replay below
+    }
+    // the host-side state a plain enqueue would have left behind
+    ctx->n_atoms = n; ctx->n_mol = hit->s_n_mol; ctx->periodic = hit->s_periodic; ctx->partial = hit->s_partial;
+    ctx->aev_in_planes = hit->s_planes; ctx->n_models = hit->s_models; ctx->cand_valid = false;
+    hit->stamp = ++ctx->graph_clock;
+    DHP_CUDA(ctx, cudaGraphLaunch(hit->exec, ctx->stream));
+    ctx->launches += hit->launches;
+    ctx->graph_replays++;
     return DHP_OK;
 }
 
@@ -188,6 +261,8 @@ int dhp_create(dhp_ctx** out, const dhp_params* params, int64_t max_atoms, int64
     if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) { delete h; return DHP_E_CUDA; }
     c->sm_count = prop.multiProcessorCount;
     { const char* e = getenv("DHP_NO_SMALL_PATH"); c->no_small_path = e && e[0] == '1'; }
+    { const char* e = getenv("DHP_NO_GRAPH"); c->graph_on = !(e && e[0] == '1'); }
+    if (c->graph_on && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); c->graph_on = false; c->cap_stream = nullptr; }
     { const char* e = getenv("DHP_TC_PAIRS"); c->tc_pairs = (e && e[0] >= '0' && e[0] <= '3') ? e[0] - '0' : 0; }   // cta_group::2 kernels
     { const char* e = getenv("DHP_TC_TWO"); c->tc_two = (e && e[0] >= '0' && e[0] <= '3') ? e[0] - '0' : 2; }   // two row tiles per CTA: B1 by default
     c->cc_major = prop.major;
@@ -280,6 +355,7 @@ int dhp_weights_load(dhp_ctx* h, const float* blob, int64_t n_floats, int n_mode
 int dhp_weights_free(dhp_ctx* h, dhp_weights* w) {
     if (!h || !w) return DHP_E_BADARG;
     cudaStreamSynchronize(h->c.stream);
+    graphs_invalidate(&h->c);                      // captured calls hold this handle's device pointers
     mlp_tc_weights_free(&h->c, &w->w);
     if (w->w.blob) cudaFree(w->w.blob);
     delete w;
@@ -405,7 +481,7 @@ int dhp_set_mlp_mode(dhp_ctx* h, int mode) {
     if (!h || mode < DHP_MLP_AUTO || mode > DHP_MLP_TENSOR_FP16) return DHP_E_BADARG;
     if (mode >= DHP_MLP_TENSOR && !mlp_tc_available(&h->c)) return DHP_E_NOTIMPL;
     h->c.mlp_mode = mode;
-    return DHP_OK;
+    return DHP_OK;     // (captured graphs are keyed on the mode)
 }
 
 int dhp_set_skin(dhp_ctx* h, float skin) {
@@ -513,6 +589,7 @@ int dhp_profile_read(dhp_ctx* h, double* ms, int64_t* n_calls) {
 }
 
 int64_t dhp_launch_count(dhp_ctx* h) { return h ? h->c.launches : 0; }
+int64_t dhp_graph_replays(dhp_ctx* h) { return h ? h->c.graph_replays : 0; }
 
 const char* dhp_strerror(int code) {
     switch (code) {

@@ -37,6 +37,8 @@ constexpr int ROW_ALIGN = 2 * ROW_TILE;         // species groups start at multi
                                                 // kept equal within such a pair
 constexpr int KBLK = 64;                        // feature-block width: the unit in which zero columns are skipped
 constexpr int N_KBLK = AEV_LD / KBLK;           // 16 blocks: 14 angular (2 species pairs each) + 2 radial
+constexpr int SMALL_N = 320;                      // systems up to this size take the single-block list build (above ~300 atoms one SM is
+                                                // slower than the thirteen small launches of the general path) and CUDA-graph replay
 constexpr int MAX_MODELS = DHP_MAX_MODELS;
 constexpr int MAX_ANG = DHP_MAX_ANG;                    // angular neighbours staged per centre (status CAPACITY beyond)
 
@@ -83,6 +85,21 @@ struct Profile {
     int64_t calls;
 };
 
+// One captured hot call of a small system (api.cu): the kernels of such a call are 15-40 us each and the gaps between a dozen
+// dependent launches are a sixth of the call, so the call is captured once per argument set and replayed as a CUDA graph.
+struct GraphEntry {
+    bool used;
+    const void *pos, *species, *mol, *central, *weights, *E, *F;
+    int64_t n, n_mol;
+    float box[4];              // edges, [3] = 1 if periodic
+    int mlp_mode;
+    cudaGraphExec_t exec;
+    int64_t launches;          // kernels in the graph (dhp_launch_count)
+    int64_t s_n_mol; bool s_periodic, s_partial, s_planes; int s_models;   // host-side state the enqueue leaves behind
+    uint64_t stamp;
+};
+constexpr int N_GRAPHS = 4;
+
 struct Ctx {
     cudaStream_t stream;
     dhp_params params;
@@ -96,6 +113,11 @@ struct Ctx {
     int tc_two;            // bit 0: G1, bit 1: B1 run with two row tiles per CTA sharing each weight K block (k_gemm_tc2) on large
                            // systems; DHP_TC_TWO=<bits> in the environment at dhp_create overrides the default (2: B1 only)
     int64_t launches;
+    bool graph_on;         // small systems replay a captured graph (DHP_NO_GRAPH=1 at dhp_create turns it off)
+    cudaStream_t cap_stream;   // the library's own stream for capture (the caller's may be the legacy default stream, which cannot capture)
+    GraphEntry graphs[N_GRAPHS];
+    uint64_t graph_clock;
+    int64_t graph_replays;
     char cuda_err[256];
     Profile prof;
 

@@ -892,7 +892,6 @@ k_refilter(const float4* __restrict__ spos, const __grid_constant__ BoxArg bx, c
 // list is the same bit-exact list), rows are ordered by order_row() and the species-grouped, class-ordered row
 // assignment is a stable count over at most SMALL_N keys in shared memory.
 // ---------------------------------------------------------------------------------------------
-constexpr int SMALL_N = 320;      // above ~300 atoms one SM is slower than the thirteen small launches of the general path
 constexpr int SMALL_THREADS = 1024;
 
 __global__ void __launch_bounds__(SMALL_THREADS)
@@ -1105,8 +1104,10 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
         DHP_LAUNCH(ctx, k_reset_rows, 2 * ctx->sm_count, 256, 0, ctx->row_slot, ctx->row_species, (int)ctx->max_rows, gate);
     }
     if (!periodic && !by_mol) {
-        static const unsigned init[6] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0u, 0u, 0u};
-        DHP_CUDA(ctx, cudaMemcpyAsync(ctx->bbox, init, sizeof(init), cudaMemcpyHostToDevice, st));
+        // ordered-uint min / max accumulators: {0xffffffff x 3, 0 x 3} (two memsets: a copy from pageable host memory could
+        // not be captured into a CUDA graph)
+        DHP_CUDA(ctx, cudaMemsetAsync(ctx->bbox, 0xFF, 3 * sizeof(unsigned), st));
+        DHP_CUDA(ctx, cudaMemsetAsync(ctx->bbox + 3, 0, 3 * sizeof(unsigned), st));
         int blocks = (int)std::min<int64_t>((n + 255) / 256, 4 * ctx->sm_count);
         DHP_LAUNCH(ctx, k_bbox, blocks, 256, 0, pos, n, ctx->bbox, gate);
     }

@@ -472,3 +472,59 @@ def test_capacity_fault_in_the_middle_of_an_md_run_is_reported(torch, B, params,
     assert d.dhp_status() == 0
     d.dhp_md_destroy(md)
     d.close()
+
+
+@pytest.mark.parametrize("name", ["ligand50", "water96", "replicas8"])
+def test_small_systems_replay_a_captured_graph(torch, B, params, blob8, name):
+    """Small systems (the hybrid scheme's per-step call) are captured into a CUDA graph on the first
+    call with a given argument set and replayed afterwards.  The replays must give the oracle's answer for the CURRENT
+    contents of the buffers (positions are rewritten in place between calls), count as replays, and a different buffer
+    must not be served by a stale graph."""
+    s = W.replicas_1024x30(n_mol=8) if name == "replicas8" else SYSTEMS[name]()     # 240 atoms in 8 molecules: still "small"
+    blob = blob8[: s.n_models * 7 * W.PARAMS_PER_NET]
+    d = make_ctx(B, s, params)
+    w = d.dhp_weights_load(blob, s.n_models)
+    pos, sp, mol = B.to_device(s)
+    n_mol = max(1, s.n_mol)
+    E = torch.empty(n_mol, dtype=torch.float64, device="cuda")
+    F = torch.empty((s.n_atoms, 3), dtype=torch.float32, device="cuda")
+    per = s.n_atoms if s.mol_offsets is None else np.diff(s.mol_offsets)
+    rng = np.random.default_rng(3)
+    q = s.pos.copy()
+    r0 = d.dhp_graph_replays()
+    for it in range(4):
+        pos.copy_(torch.from_numpy(q).cuda())                 # same buffer, new contents
+        d.dhp_ani_energy_forces(pos, s.box, sp, w, mol, E=E, F=F)
+        torch.cuda.synchronize()
+        assert d.dhp_status() == 0
+        s2 = W.System(s.name, q, s.species, s.box, s.mol_offsets, s.n_models)
+        Eo, Fo = oracle.total_energy_forces(s2, params, blob)
+        assert np.max(np.abs(E.cpu().numpy() - Eo) / per) <= E_TOL_PER_ATOM
+        assert np.max(np.abs(F.cpu().numpy() - Fo)) <= F_TOL
+        q = (q.astype(np.float64) + rng.normal(0, 0.02, q.shape)).astype(np.float32)
+    assert d.dhp_graph_replays() - r0 == 4                    # the capture call is served by the new graph too
+    l0 = d.dhp_launch_count()
+    d.dhp_ani_energy_forces(pos, s.box, sp, w, mol, E=E, F=F)
+    assert d.dhp_launch_count() - l0 >= 6                     # replayed kernels are counted
+    # a different position buffer is a different graph, not a stale replay
+    pos2 = torch.from_numpy(s.pos).cuda()
+    E2, F2 = d.dhp_ani_energy_forces(pos2, s.box, sp, w, mol)
+    torch.cuda.synchronize()
+    Eo, Fo = oracle.total_energy_forces(s, params, blob)
+    assert np.max(np.abs(E2.cpu().numpy() - Eo) / per) <= E_TOL_PER_ATOM and np.max(np.abs(F2.cpu().numpy() - Fo)) <= F_TOL
+    # energy-only and masked calls go through the same mechanism
+    Ee = d.dhp_ani_energy(pos2, s.box, sp, w, mol)
+    Ee = d.dhp_ani_energy(pos2, s.box, sp, w, mol, E=Ee)
+    torch.cuda.synchronize()
+    assert np.max(np.abs(Ee.cpu().numpy() - Eo) / per) <= E_TOL_PER_ATOM
+    d.close()
+
+
+def test_graph_replay_can_be_switched_off(torch, B, params, blob8, monkeypatch):
+    monkeypatch.setenv("DHP_NO_GRAPH", "1")
+    s = SYSTEMS["ligand50"]()
+    d, E, F = run_gpu(B, torch, s, params, blob8)
+    assert d.dhp_graph_replays() == 0
+    Eo, Fo = oracle.total_energy_forces(s, params, blob8[: s.n_models * 7 * W.PARAMS_PER_NET])
+    assert abs(E[0] - Eo[0]) / s.n_atoms <= E_TOL_PER_ATOM and np.max(np.abs(F - Fo)) <= F_TOL
+    d.close()
