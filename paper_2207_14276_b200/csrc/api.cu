@@ -141,6 +141,10 @@ static void graphs_invalidate(Ctx* ctx) {
 static int run_energy_forces(Ctx* ctx, const float* pos, const float* box, const int32_t* species, int64_t n,
                              const int32_t* mol_offsets, int64_t n_mol, const Weights* w, double* E, float* F,
                              const uint8_t* central = nullptr) {
+    {   // the SIMT scaffold's buffers exist from the first time it is going to run (never inside a graph capture)
+        const bool tensor = ctx->mlp_mode >= DHP_MLP_TENSOR || (ctx->mlp_mode == DHP_MLP_AUTO && w->tc != nullptr);
+        if (!tensor) { const int rc = mlp_simt_ensure(ctx, w->n_models); if (rc != DHP_OK) return rc; }
+    }
     const bool small = ctx->graph_on && n > 0 && n <= SMALL_N && !(ctx->skin > 0.f) && !ctx->prof.on;
     if (!small) return enqueue_energy_forces(ctx, pos, box, species, n, mol_offsets, n_mol, w, E, F, central);
     float bx[4] = {0.f, 0.f, 0.f, box ? 1.f : 0.f};
@@ -307,7 +311,6 @@ int dhp_create(dhp_ctx** out, const dhp_params* params, int64_t max_atoms, int64
     }
     ok &= dalloc(&c->st_pos, 3 * N) && dalloc(&c->st_species, N) && dalloc(&c->st_mol, NM + 1) && dalloc(&c->st_E, NM) && dalloc(&c->st_F, 3 * N);
     if (ok) ok = aev_init(c) == DHP_OK;
-    if (ok) ok = mlp_simt_alloc(c) == DHP_OK;
     if (ok && mlp_tc_available(c)) ok = mlp_tc_alloc(c) == DHP_OK;
     if (ok) {
         for (auto& row : c->prof.ev) for (auto& e : row) ok &= cudaEventCreate(&e) == cudaSuccess;
@@ -344,6 +347,16 @@ int dhp_weights_load(dhp_ctx* h, const float* blob, int64_t n_floats, int n_mode
     cudaError_t e = cudaMemcpyAsync(w->w.blob, blob, sizeof(float) * (size_t)n_floats, cudaMemcpyDefault, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) { cudaFree(w->w.blob); delete w; return cuda_fail(c, e, "weights upload"); }
+    // activation workspaces are sized by the ensembles actually loaded (setup time; not by DHP_MAX_MODELS)
+    if (n_models > c->max_models_seen) c->max_models_seen = n_models;
+    {
+        int rc = DHP_OK;
+        const bool simt = c->mlp_mode == DHP_MLP_SIMT || !mlp_tc_available(c);
+        if (simt) rc = mlp_simt_ensure(c, c->max_models_seen);
+        if (rc == DHP_OK && mlp_tc_available(c)) rc = mlp_tc_ensure(c, c->max_models_seen, c->mlp_mode == DHP_MLP_TENSOR_LAYERWISE);
+        if (rc != DHP_OK) { cudaFree(w->w.blob); delete w; return rc; }
+        graphs_invalidate(c);                      // captured calls may hold the old buffers
+    }
     if (mlp_tc_available(c)) {
         int rc = mlp_tc_weights(c, &w->w);
         if (rc != DHP_OK) { mlp_tc_weights_free(c, &w->w); cudaFree(w->w.blob); delete w; return rc; }
@@ -481,6 +494,13 @@ int dhp_set_mlp_mode(dhp_ctx* h, int mode) {
     if (!h || mode < DHP_MLP_AUTO || mode > DHP_MLP_TENSOR_FP16) return DHP_E_BADARG;
     if (mode >= DHP_MLP_TENSOR && !mlp_tc_available(&h->c)) return DHP_E_NOTIMPL;
     h->c.mlp_mode = mode;
+    if (h->c.max_models_seen > 0) {               // the workspaces of the newly selected path (setup call: may allocate)
+        int rc = DHP_OK;
+        if (mode == DHP_MLP_SIMT) rc = mlp_simt_ensure(&h->c, h->c.max_models_seen);
+        else rc = mlp_tc_ensure(&h->c, h->c.max_models_seen, mode == DHP_MLP_TENSOR_LAYERWISE);
+        if (rc != DHP_OK) return rc;
+        graphs_invalidate(&h->c);
+    }
     return DHP_OK;     // (captured graphs are keyed on the mode)
 }
 

@@ -185,7 +185,9 @@ struct Ctx {
     float* aev;            // [max_rows][AEV_LD]  internal column order, see col2feat()
     float* grad;           // [max_rows][AEV_LD]  dE/dAEV
     float* e_atom;         // [max_rows]
-    float* act[6];         // SIMT path intermediates: h1,h2,h3(delta3),delta2,delta1 ; see mlp_simt.cu
+    float* act[6];         // SIMT path intermediates: h1,h2,h3(delta3),delta2,delta1 ; see mlp_simt.cu (allocated on demand)
+    int simt_models;       // networks per row those buffers hold (0 = not allocated)
+    int max_models_seen;   // largest ensemble loaded on this context so far
     float* fsorted;        // [N][3] forces in sorted order
     double* e_out_tmp;     // [max(1,max_mols)]
     int* export_tmp;       // [N+1]
@@ -219,13 +221,14 @@ int aev_init(Ctx* ctx);                    // per-device kernel attributes
 int aev_forward(Ctx* ctx, bool planes);   // planes: write the tensor path's fp16 hi/lo planes instead of fp32 rows
 int aev_backward(Ctx* ctx, float* F_out);
 int mlp_simt(Ctx* ctx, const Weights* w, bool forward_only);
-int mlp_simt_alloc(Ctx* ctx);
+int mlp_simt_ensure(Ctx* ctx, int n_models);   // setup-time (or first-use) sizing of the SIMT activations
 void mlp_simt_free(Ctx* ctx);
 int energy_reduce(Ctx* ctx, double* E_out);
 
 // tensor path (mlp_tc.cu)
 bool mlp_tc_available(Ctx* ctx);
 int mlp_tc_alloc(Ctx* ctx);
+int mlp_tc_ensure(Ctx* ctx, int n_models, bool layerwise);   // setup-time sizing of the tensor path's activation planes
 void mlp_tc_free(Ctx* ctx);
 int mlp_tc_weights(Ctx* ctx, Weights* w);
 void mlp_tc_weights_free(Ctx* ctx, Weights* w);

@@ -134,11 +134,18 @@ __global__ void k_out_layer(const float* __restrict__ h3, const float* __restric
     if (lane == 0) e_atom[row] = esum * inv_m;
 }
 
-int mlp_simt_alloc(Ctx* ctx) {
+// The fp32 scaffold keeps every activation in HBM (39 KB per row at 8 networks): its buffers exist only once the SIMT path is
+// actually going to run, sized by the ensemble in use (setup time, or the first SIMT call).  Grows, never shrinks.
+int mlp_simt_ensure(Ctx* ctx, int n_models) {
+    if (n_models <= ctx->simt_models) return DHP_OK;
     const size_t R = (size_t)ctx->max_rows;
     const size_t widths[6] = {H1, H2, H3, H3, H2, H1};   // h1 h2 h3 d3 d2 d1
-    for (int b = 0; b < 6; ++b)
-        if (cudaMalloc(&ctx->act[b], sizeof(float) * R * MAX_MODELS * widths[b]) != cudaSuccess) return DHP_E_NOMEM;
+    cudaStreamSynchronize(ctx->stream);
+    for (int b = 0; b < 6; ++b) {
+        if (ctx->act[b]) { cudaFree(ctx->act[b]); ctx->act[b] = nullptr; }
+        if (cudaMalloc(&ctx->act[b], sizeof(float) * R * n_models * widths[b]) != cudaSuccess) { cudaGetLastError(); ctx->simt_models = 0; return DHP_E_NOMEM; }
+    }
+    ctx->simt_models = n_models;
     return DHP_OK;
 }
 void mlp_simt_free(Ctx* ctx) {

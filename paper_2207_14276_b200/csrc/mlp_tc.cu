@@ -1902,6 +1902,8 @@ bool make_map(CUtensorMap* m, const void* ptr, uint64_t rows, uint64_t cols, uin
 struct TcWorkspace {                  // per context
     __half* aev;                                   // [2][max_rows][AEV_LD] row-major hi / lo planes (A of G1, via TMA)
     __half *h1, *h2, *d3, *d2, *d1;                // tiled activation planes (see the header); d3 is padded to 192 per model
+    int act_models;                                // h1 / d1 hold this many networks per row (grown by mlp_tc_ensure)
+    int lw_models;                                 // h2 / d3 / d2 (layer-by-layer mode only) likewise; 0 = not allocated
     CUtensorMap m_aev;
     int* pair_sched;                               // [2][n_clusters + 1] item ranges of the pair kernels (G1, B1)
     int* pair_scratch;                             // [max_rows / 256 * MAX_MODELS] cost prefix scratch of k_pair_schedule
@@ -1958,17 +1960,40 @@ int mlp_tc_alloc(Ctx* ctx) {
     if (!w) return DHP_E_NOMEM;
     memset((void*)w, 0, sizeof(*w));
     ctx->tc_ws = w;
-    const size_t R = (size_t)ctx->max_rows, M = MAX_MODELS;
-    struct { __half** p; size_t width; } bufs[] = {{&w->aev, (size_t)AEV_LD}, {&w->h1, M * H1}, {&w->h2, M * H2},
-                                                    {&w->d3, M * H2},          {&w->d2, M * H2}, {&w->d1, M * H1}};
-    for (auto& b : bufs) {
-        if (cudaMalloc((void**)b.p, 2 * R * b.width * sizeof(__half)) != cudaSuccess) return DHP_E_NOMEM;
-        if (cudaMemset(*b.p, 0, 2 * R * b.width * sizeof(__half)) != cudaSuccess) return DHP_E_CUDA;
-    }
+    const size_t R = (size_t)ctx->max_rows;
+    // the activation planes are sized by the ensemble that is actually loaded (mlp_tc_ensure, from dhp_weights_load)
+    if (cudaMalloc((void**)&w->aev, 2 * R * AEV_LD * sizeof(__half)) != cudaSuccess) return DHP_E_NOMEM;
+    if (cudaMemset(w->aev, 0, 2 * R * AEV_LD * sizeof(__half)) != cudaSuccess) return DHP_E_CUDA;
     if (cudaMalloc((void**)&w->pair_sched, sizeof(int) * 2 * (ctx->sm_count / 2 + 1)) != cudaSuccess) return DHP_E_NOMEM;
     if (cudaMalloc((void**)&w->pair_scratch, sizeof(int) * (R / (2 * BM) * MAX_MODELS + 1)) != cudaSuccess) return DHP_E_NOMEM;
     if (!make_map(&w->m_aev, w->aev, 2 * R, AEV_LD, BM)) return DHP_E_CUDA;
     ctx->aev_planes = w->aev;
+    return DHP_OK;
+}
+
+// Setup-time sizing of the activation planes (4 B per element as fp16 hi / lo): h1 and d1 for `n_models` networks per
+// row (16 KB per row at 8 networks), and - only if the layer-by-layer comparison mode is in use - h2, d3, d2.  Grows, never
+// shrinks; the planes are zeroed so that padding rows stay finite.  Not a hot call: allocates and synchronises.
+int mlp_tc_ensure(Ctx* ctx, int n_models, bool layerwise) {
+    TcWorkspace* w = (TcWorkspace*)ctx->tc_ws;
+    if (!w) return DHP_OK;
+    const size_t R = (size_t)ctx->max_rows;
+    auto grow = [&](__half** p, size_t width) -> int {
+        if (*p) { cudaStreamSynchronize(ctx->stream); cudaFree(*p); *p = nullptr; }
+        if (cudaMalloc((void**)p, 2 * R * width * sizeof(__half)) != cudaSuccess) { cudaGetLastError(); return DHP_E_NOMEM; }
+        if (cudaMemset(*p, 0, 2 * R * width * sizeof(__half)) != cudaSuccess) return DHP_E_CUDA;
+        return DHP_OK;
+    };
+    int rc;
+    if (n_models > w->act_models) {
+        if ((rc = grow(&w->h1, (size_t)n_models * H1)) != DHP_OK || (rc = grow(&w->d1, (size_t)n_models * H1)) != DHP_OK) { w->act_models = 0; return rc; }
+        w->act_models = n_models;
+    }
+    if (layerwise && n_models > w->lw_models) {
+        if ((rc = grow(&w->h2, (size_t)n_models * H2)) != DHP_OK || (rc = grow(&w->d3, (size_t)n_models * H2)) != DHP_OK ||
+            (rc = grow(&w->d2, (size_t)n_models * H2)) != DHP_OK) { w->lw_models = 0; return rc; }
+        w->lw_models = n_models;
+    }
     return DHP_OK;
 }
 
@@ -2031,6 +2056,7 @@ int mlp_tc(Ctx* ctx, const Weights* wt, bool forward_only) {
     const int M = wt->n_models;
     const int R = (int)ctx->max_rows;
     int rc;
+    if (M > ws->act_models || (ctx->mlp_mode == DHP_MLP_TENSOR_LAYERWISE && M > ws->lw_models)) return DHP_E_NOTIMPL;   // mlp_tc_ensure not run
     // e_atom and the tile schedulers were zeroed with the rest of the per-call arena at the start of the call (nlist_build)
     if (!ctx->aev_in_planes)     // rows came from a forward pass in fp32 (debug / mixed use): split them here
         DHP_LAUNCH(ctx, k_split_rows, 4 * ctx->sm_count, 256, 0, ctx->aev, AEV_LD, ctx->sp_start, AEV_LD, ws->aev, R);
