@@ -886,34 +886,28 @@ k_refilter(const float4* __restrict__ spos, const __grid_constant__ BoxArg bx, c
 }
 
 // ---------------------------------------------------------------------------------------------
-// Small systems (n <= SMALL_N; the hybrid scheme's solute, BASELINE.json configs[0]-[1]): the whole of a1 in ONE block.
-// Thirteen launches with 3-15 us floors cost ~90 us for 50 atoms; here the atoms stay in the caller's order (perm =
-// identity), every pair is tested (fp32 with the error margin of k_refilter, the canonical fp64 predicate inside it: the
-// list is the same bit-exact list), rows are ordered by order_row() and the species-grouped, class-ordered row
-// assignment is a stable count over at most SMALL_N keys in shared memory.
+// Small systems (n <= SMALL_N; the hybrid scheme's solute, BASELINE.json configs[0]-[1]).  The thirteen launches of the
+// general path cost 3-15 us each, far more than their work; here a1 is three launches whose work is one warp per atom
+// (round 1 did all of it in ONE block: 9 atoms per warp in sequence, each with several dependent global round trips -
+// 61 us for 288 atoms; spread over n warps it is a few microseconds, and the launches cost nothing inside the replayed
+// graph of the small-system call).  The atoms stay in the caller's order (perm = identity); every pair is tested (fp32
+// with the error margin of k_refilter, the canonical fp64 predicate inside it: the list is the same bit-exact list):
+//   k_small_pairs   warp <-> atom: all pairs of the row -> unordered entries (pass-1 format), counts; sorted copies
+//   k_small_rows    warp <-> atom: CSR offset (prefix over at most 320 counts), order_row(): runs, masks
+//   k_small_assign  one block: species-grouped, class-ordered row assignment (stable count over <= 320 keys), tile masks
 // ---------------------------------------------------------------------------------------------
-constexpr int SMALL_THREADS = 1024;
+constexpr int SMALL_WARPS = 8;
 
-__global__ void __launch_bounds__(SMALL_THREADS)
-k_nlist_small(const float* __restrict__ pos, const int* __restrict__ species, int n, const int* __restrict__ mol_offsets, int n_mol,
+__global__ void __launch_bounds__(SMALL_WARPS * 32)
+k_small_pairs(const float* __restrict__ pos, const int* __restrict__ species, int n, const int* __restrict__ mol_offsets, int n_mol,
               const uint8_t* __restrict__ central, int periodic, double Lx, double Ly, double Lz, double rcr2, double rca2, int stride,
-              int64_t pair_cap, Grid* __restrict__ grid, int* __restrict__ status, int* __restrict__ perm, int* __restrict__ inv_perm,
+              Grid* __restrict__ grid, int* __restrict__ status, int* __restrict__ perm, int* __restrict__ inv_perm,
               float4* __restrict__ spos, int* __restrict__ smol, unsigned char* __restrict__ snc, unsigned* __restrict__ tmp,
-              int* __restrict__ n_rad, int* __restrict__ n_ang, int* __restrict__ row_ptr, int* __restrict__ col,
-              unsigned short* __restrict__ seg_cnt, unsigned* __restrict__ amask, int* __restrict__ sp_count, int* __restrict__ sp_start,
-              int* __restrict__ rowmap, int* __restrict__ row_species, int* __restrict__ row_slot, unsigned* __restrict__ tile_mask) {
+              int* __restrict__ n_rad) {
     __shared__ Grid g;
-    __shared__ float4 sp4[SMALL_N];
-    __shared__ int mol_s[SMALL_N];
-    __shared__ short key_s[SMALL_N];
-    __shared__ unsigned char nc_s[SMALL_N];
-    __shared__ int segs[SMALL_THREADS / 32][16];
-    __shared__ int tot_s[NKEY], kstart_s[NKEY];
-    __shared__ int ovf_s;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const bool by_mol = mol_offsets != nullptr && n_mol > 0;
-    // ---- phase 0: grid description (what the AEV kernels read), atoms in the caller's order
-    if (tid == 0) {
+    if (tid == 0) {                                          // grid description (what the AEV kernels read)
         const double L[3] = {Lx, Ly, Lz};
         g.periodic = periodic; g.by_molecule = by_mol ? 1 : 0; g.ncell = 1;
         for (int c = 0; c < 3; ++c) {
@@ -921,89 +915,99 @@ k_nlist_small(const float* __restrict__ pos, const int* __restrict__ species, in
             g.inv_L[c] = periodic ? 1.0 / L[c] : 0.0; g.wrap[c] = periodic ? 1 : 0;
             g.Lf[c] = (float)L[c]; g.inv_Lf[c] = periodic ? (float)(1.0 / L[c]) : 0.f;
         }
-        *grid = g;
-        ovf_s = 0;
-    }
-    for (int k = tid; k < NKEY; k += SMALL_THREADS) tot_s[k] = 0;
-    if (tid < n) {
-        int s = species[tid];
-        if (s < 0 || s >= NSP) atomicExch(status, DHP_E_SPECIES);
-        s = min(max(s, 0), NSP - 1);
-        const float4 p4 = make_float4(pos[3 * tid], pos[3 * tid + 1], pos[3 * tid + 2], __int_as_float(s));
-        int m = 0;
-        if (by_mol) {
-            int lo = 0, hi = n_mol;            // largest m with mol_offsets[m] <= tid
-            while (hi - lo > 1) {
-                const int mid = (lo + hi) >> 1;
-                if (mol_offsets[mid] <= tid) lo = mid; else hi = mid;
-            }
-            m = lo;
-        }
-        const unsigned char nc = central ? (central[tid] ? 0 : 1) : 0;
-        sp4[tid] = p4; mol_s[tid] = m; nc_s[tid] = nc;
-        spos[tid] = p4; smol[tid] = m; snc[tid] = nc; perm[tid] = tid; inv_perm[tid] = tid;
+        if (blockIdx.x == 0) *grid = g;
     }
     __syncthreads();
-    // ---- phase 1: all pairs of a row by one warp -> unordered entries (pass-1 format), counts
-    {
+    const int i = blockIdx.x * SMALL_WARPS + warp;
+    if (i >= n) return;
+    auto mol_of = [&](int a) -> int {                        // largest m with mol_offsets[m] <= a
+        if (!by_mol) return 0;
+        int lo = 0, hi = n_mol;
+        while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (mol_offsets[mid] <= a) lo = mid; else hi = mid; }
+        return lo;
+    };
+    int si = species[i];
+    if (lane == 0 && (si < 0 || si >= NSP)) atomicExch(status, DHP_E_SPECIES);
+    si = min(max(si, 0), NSP - 1);
+    const float4 pi = make_float4(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], __int_as_float(si));
+    const int mi = mol_of(i);
+    const unsigned char nci = central ? (central[i] ? 0 : 1) : 0;
+    if (lane == 0) { spos[i] = pi; smol[i] = mi; snc[i] = nci; perm[i] = i; inv_perm[i] = i; }
+    int base = 0;
+    if (!nci) {
         const float rcr2f = (float)rcr2, rca2f = (float)rca2;
         const float rcr = sqrtf(rcr2f), rca = sqrtf(rca2f);
         const float kr = 2.0f * 2.0f * rcr * 3.0f * 5.9604645e-08f, ka = 2.0f * 2.0f * rca * 3.0f * 5.9604645e-08f;
         const float mr0 = 2.0f * rcr2f * 2.3841858e-07f, ma0 = 2.0f * rca2f * 2.3841858e-07f;
         const float Lfx = g.Lf[0], Lfy = g.Lf[1], Lfz = g.Lf[2], iLx = g.inv_Lf[0], iLy = g.inv_Lf[1], iLz = g.inv_Lf[2];
         const unsigned lt = (1u << lane) - 1u;
-        for (int i = warp; i < n; i += SMALL_THREADS / 32) {
-            int base = 0;
-            if (!nc_s[i]) {
-                const float4 pi = sp4[i];
-                const int mi = mol_s[i];
-                for (int c0 = 0; c0 < n; c0 += 32) {
-                    const int j = c0 + lane;
-                    const bool have = j < n && j != i && mol_s[min(j, n - 1)] == mi;
-                    const float4 pj = sp4[min(j, n - 1)];
-                    float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
-                    const float dm = fmaxf(fabsf(dx), fmaxf(fabsf(dy), fabsf(dz)));
-                    if (periodic) { dx -= Lfx * rintf(dx * iLx); dy -= Lfy * rintf(dy * iLy); dz -= Lfz * rintf(dz * iLz); }
-                    const float r2 = dx * dx + dy * dy + dz * dz;
-                    bool in_r = have && r2 <= rcr2f;
-                    bool in_a = have && r2 <= rca2f;
-                    if (have && (fabsf(r2 - rcr2f) <= fmaf(kr, dm, mr0) || fabsf(r2 - rca2f) <= fmaf(ka, dm, ma0))) {
-                        const double r2d = pair_r2(pi, pj, g);
-                        in_r = r2d <= rcr2;
-                        in_a = r2d <= rca2;
-                    }
-                    const unsigned m = __ballot_sync(0xffffffffu, in_r);
-                    if (in_r) {
-                        const int o = base + __popc(m & lt);
-                        if (o < stride) tmp[(size_t)i * stride + o] = (unsigned)j | ((unsigned)__float_as_int(pj.w) << 28) | (in_a ? 0u : ENT_RADIAL_ONLY);
-                    }
-                    base += __popc(m);
-                }
+        for (int c0 = 0; c0 < n; c0 += 32) {
+            const int j = c0 + lane, jc = min(j, n - 1);
+            const int sj = min(max(species[jc], 0), NSP - 1);
+            const float4 pj = make_float4(pos[3 * jc], pos[3 * jc + 1], pos[3 * jc + 2], __int_as_float(sj));
+            const bool have = j < n && j != i && (!by_mol || mol_of(jc) == mi);
+            float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+            const float dm = fmaxf(fabsf(dx), fmaxf(fabsf(dy), fabsf(dz)));
+            if (periodic) { dx -= Lfx * rintf(dx * iLx); dy -= Lfy * rintf(dy * iLy); dz -= Lfz * rintf(dz * iLz); }
+            const float r2 = dx * dx + dy * dy + dz * dz;
+            bool in_r = have && r2 <= rcr2f;
+            bool in_a = have && r2 <= rca2f;
+            if (have && (fabsf(r2 - rcr2f) <= fmaf(kr, dm, mr0) || fabsf(r2 - rca2f) <= fmaf(ka, dm, ma0))) {
+                const double r2d = pair_r2(pi, pj, g);
+                in_r = r2d <= rcr2;
+                in_a = r2d <= rca2;
             }
-            if (lane == 0) {
-                if (base > stride) { atomicExch(status, DHP_E_CAPACITY); base = stride; }
-                n_rad[i] = base;
+            const unsigned m = __ballot_sync(0xffffffffu, in_r);
+            if (in_r) {
+                const int o = base + __popc(m & lt);
+                if (o < stride) tmp[(size_t)i * stride + o] = (unsigned)j | ((unsigned)sj << 28) | (in_a ? 0u : ENT_RADIAL_ONLY);
             }
+            base += __popc(m);
         }
     }
-    __syncthreads();
-    // ---- phase 2: CSR offsets
-    block_scan_excl(n_rad, row_ptr, n);
-    __syncthreads();
-    if (tid == 0 && (row_ptr[n] < 0 || (int64_t)row_ptr[n] > pair_cap)) { atomicExch(status, DHP_E_CAPACITY); ovf_s = 1; }
-    __syncthreads();
-    if (ovf_s) {                                            // neighbour storage overflow: an empty list, as in the general path
-        for (int a = tid; a <= n; a += SMALL_THREADS) { row_ptr[a] = 0; if (a < n) n_rad[a] = 0; }
-        __syncthreads();
+    if (lane == 0) {
+        if (base > stride) { atomicExch(status, DHP_E_CAPACITY); base = stride; }
+        n_rad[i] = base;
     }
-    // ---- phase 3: order every row, run lengths, feature-block masks
-    for (int i = warp; i < n; i += SMALL_THREADS / 32)
-        order_row(tmp + (size_t)i * stride, n_rad[i], row_ptr[i], i, lane, segs[warp], col, n_ang, seg_cnt, amask, false, nullptr, nullptr);
-    __syncthreads();
-    // ---- phase 4: species-grouped, class-ordered rows (stable in atom order), tile masks
+}
+
+__global__ void __launch_bounds__(SMALL_WARPS * 32)
+k_small_rows(const unsigned* __restrict__ tmp, int stride, const int* __restrict__ n_rad_in, int n, int64_t pair_cap,
+             int* __restrict__ status, int* __restrict__ row_ptr, int* __restrict__ col, int* __restrict__ n_ang,
+             unsigned short* __restrict__ seg_cnt, unsigned* __restrict__ amask) {
+    __shared__ int segs[SMALL_WARPS][16];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int i = blockIdx.x * SMALL_WARPS + warp;
+    if (i >= n) return;
+    // CSR offset of row i and the total, from the (at most SMALL_N) counts: no separate scan launch
+    int before = 0, total = 0;
+    for (int a = lane; a < n; a += 32) { const int c = n_rad_in[a]; total += c; if (a < i) before += c; }
+    for (int o = 16; o; o >>= 1) { before += __shfl_xor_sync(0xffffffffu, before, o); total += __shfl_xor_sync(0xffffffffu, total, o); }
+    int ni = n_rad_in[i];
+    if ((int64_t)total > pair_cap) {                         // neighbour storage overflow: an empty list, as in the general path
+        if (lane == 0 && i == 0) atomicExch(status, DHP_E_CAPACITY);
+        before = 0; total = 0; ni = 0;
+    }
+    __syncwarp();
+    if (lane == 0) { row_ptr[i] = before; if (i == n - 1) row_ptr[n] = total; }
+    order_row(tmp + (size_t)i * stride, ni, before, i, lane, segs[warp], col, n_ang, seg_cnt, amask, false, nullptr, nullptr);
+}
+
+constexpr int SMALL_THREADS = 320;
+static_assert(SMALL_THREADS >= SMALL_N, "one thread per atom in k_small_assign");
+
+__global__ void __launch_bounds__(SMALL_THREADS)
+k_small_assign(const float4* __restrict__ spos, const unsigned char* __restrict__ snc, const unsigned* __restrict__ amask, int n,
+               const int* __restrict__ row_ptr, int* __restrict__ n_rad, int* __restrict__ sp_count, int* __restrict__ sp_start, int* __restrict__ rowmap, int* __restrict__ row_species,
+               int* __restrict__ row_slot, unsigned* __restrict__ tile_mask) {
+    __shared__ short key_s[SMALL_N];
+    __shared__ int tot_s[NKEY], kstart_s[NKEY];
+    const int tid = threadIdx.x;
+    for (int k = tid; k < NKEY; k += SMALL_THREADS) tot_s[k] = 0;
+    if (tid < n && row_ptr[n] == 0) n_rad[tid] = 0;          // an emptied (overflowed) list: the counts the export reads say so too
     int key = -1, sp = 0;
     unsigned am = 0;
-    if (tid < n && !nc_s[tid]) { sp = __float_as_int(sp4[tid].w); am = amask[tid]; key = row_key(sp, am); }
+    if (tid < n && !snc[tid]) { sp = __float_as_int(spos[tid].w); am = amask[tid]; key = row_key(sp, am); }
     if (tid < n) key_s[tid] = (short)key;
     __syncthreads();
     int rank = 0;
@@ -1077,10 +1081,14 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
     double L[3] = {0, 0, 0};
     if (periodic) for (int c = 0; c < 3; ++c) L[c] = (double)box_host[c];
     if (!skin && n <= SMALL_N && !ctx->no_small_path) {          // small systems: the whole of a1 in one block
-        DHP_LAUNCH(ctx, k_nlist_small, 1, SMALL_THREADS, 0, pos, species, n, mol_offsets, by_mol ? n_mol : 0, central, periodic ? 1 : 0,
-                   L[0], L[1], L[2], rcr * rcr, rca * rca, ctx->tmp_stride, ctx->pair_cap, ctx->grid, ctx->status, ctx->perm, ctx->inv_perm,
-                   ctx->spos, ctx->smol, ctx->snc, ctx->tmp_col, ctx->n_rad, ctx->n_ang, ctx->row_ptr, ctx->col, ctx->seg_cnt, ctx->amask,
-                   ctx->sp_count, ctx->sp_start, ctx->rowmap, ctx->row_species, ctx->row_slot, ctx->tile_mask);
+        const int sb = (n + SMALL_WARPS - 1) / SMALL_WARPS;
+        DHP_LAUNCH(ctx, k_small_pairs, sb, SMALL_WARPS * 32, 0, pos, species, n, mol_offsets, by_mol ? n_mol : 0, central, periodic ? 1 : 0,
+                   L[0], L[1], L[2], rcr * rcr, rca * rca, ctx->tmp_stride, ctx->grid, ctx->status, ctx->perm, ctx->inv_perm, ctx->spos,
+                   ctx->smol, ctx->snc, ctx->tmp_col, ctx->n_rad);
+        DHP_LAUNCH(ctx, k_small_rows, sb, SMALL_WARPS * 32, 0, ctx->tmp_col, ctx->tmp_stride, ctx->n_rad, n, ctx->pair_cap, ctx->status,
+                   ctx->row_ptr, ctx->col, ctx->n_ang, ctx->seg_cnt, ctx->amask);
+        DHP_LAUNCH(ctx, k_small_assign, 1, SMALL_THREADS, 0, ctx->spos, ctx->snc, ctx->amask, n, ctx->row_ptr, ctx->n_rad, ctx->sp_count, ctx->sp_start, ctx->rowmap,
+                   ctx->row_species, ctx->row_slot, ctx->tile_mask);
         DHP_CUDA(ctx, cudaGetLastError());
         return DHP_OK;
     }
