@@ -428,6 +428,11 @@ __device__ __forceinline__ double pair_r2(const float4& pi, const float4& pj, co
     return __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
 }
 
+// predicated 4-byte global store (keeps the hot loop of k_pairs free of branches)
+__device__ __forceinline__ void st_if(bool p, unsigned* a, unsigned v) {
+    asm volatile("{ .reg .pred q; setp.ne.u32 q, %0, 0; @q st.global.u32 [%1], %2; }" ::"r"((unsigned)p), "l"(a), "r"(v) : "memory");
+}
+
 constexpr int P1_THREADS = 128;
 constexpr int ROWS_PER_BLK = 64;        // granularity of the block-sum scan that yields the CSR offsets
 constexpr int CAND_TILE = 1024;        // candidates staged per tile (16 KB)
@@ -552,8 +557,16 @@ k_pairs(const float4* __restrict__ spos, const Grid* __restrict__ gp, const int*
                 for (int d = 0; d < 3; ++d) ri[d] -= g.L[d] * rint(ri[d] * g.inv_L[d]);
             }
             const float pix = (float)ri[0], piy = (float)ri[1], piz = (float)ri[2];
-            int base = t0 ? cnt[i] : 0;
-            int cbase = (SKIN && t0) ? cand_cnt[i] : 0;
+            const int base0 = t0 ? cnt[i] : 0;
+            const int cbase0 = (SKIN && t0) ? cand_cnt[i] : 0;
+            int base = base0, cbase = cbase0;
+            unsigned* trow = tmp + (size_t)i * stride;
+            unsigned* crow = SKIN ? cand_out + (size_t)i * cstride : nullptr;
+            asm volatile("" : "+l"(trow), "+l"(crow));      // keep the row pointers in registers
+            // fast pass: fp32 alone decides and only remembers whether any candidate fell inside a margin; such a row
+            // (about one in 2000) is then redone by the exact pass, which overwrites the same entries
+            float amb_min = 1.0f;                          // min over candidates of (distance to a threshold - margin)
+#pragma unroll 2
             for (int c0 = 0; c0 < tn; c0 += 32) {
                 const float4 c = cand[c0 + lane];          // the tile is padded with far-away dummies
                 const int jj = __float_as_int(c.w);
@@ -565,30 +578,46 @@ k_pairs(const float4* __restrict__ spos, const Grid* __restrict__ gp, const int*
                 }
                 const float r2 = dx * dx + dy * dy + dz * dz;
                 const bool other = (jj & 0x0fffffff) != i && (!WRAP || c0 + lane < tn);
-                bool in_r = other && r2 <= rcr2f;
-                bool in_a = other && r2 <= rca2f;
-                const bool amb = other && (fabsf(r2 - rcr2f) <= mr || fabsf(r2 - rca2f) <= ma);
-                if (__any_sync(0xffffffffu, amb)) {
-                    if (amb) {
+                const bool in_r = other & (r2 <= rcr2f);
+                // self and dummies may trip this too: that only sends the row to the exact pass
+                amb_min = fminf(amb_min, fminf(fabsf(r2 - rcr2f) - mr, fabsf(r2 - rca2f) - ma));
+                const unsigned m = __ballot_sync(0xffffffffu, in_r);
+                const unsigned pos = (unsigned)(base + __popc(m & lt));
+                st_if(in_r & (pos < (unsigned)stride), trow + pos, (unsigned)jj | (r2 <= rca2f ? 0u : ENT_RADIAL_ONLY));
+                base += __popc(m);
+                if (SKIN) {
+                    const bool in_c = other & (r2 <= rs2_incl);
+                    const unsigned mc = __ballot_sync(0xffffffffu, in_c);
+                    const unsigned cpos = (unsigned)(cbase + __popc(mc & lt));
+                    st_if(in_c & (cpos < (unsigned)cstride), crow + cpos, (unsigned)jj);
+                    cbase += __popc(mc);
+                }
+            }
+            const bool amb_seen = amb_min <= 0.f;
+            if (__any_sync(0xffffffffu, amb_seen)) {
+                base = base0;
+                for (int c0 = 0; c0 < tn; c0 += 32) {
+                    const float4 c = cand[c0 + lane];
+                    const int jj = __float_as_int(c.w);
+                    float dx = c.x - pix, dy = c.y - piy, dz = c.z - piz;
+                    if (WRAP) {
+                        if (wrapx) dx -= Lx * rintf(dx * iLx);
+                        if (wrapy) dy -= Ly * rintf(dy * iLy);
+                        if (wrapz) dz -= Lz * rintf(dz * iLz);
+                    }
+                    const float r2 = dx * dx + dy * dy + dz * dz;
+                    const bool other = (jj & 0x0fffffff) != i && (!WRAP || c0 + lane < tn);
+                    bool in_r = other && r2 <= rcr2f;
+                    bool in_a = other && r2 <= rca2f;
+                    if (other && (fabsf(r2 - rcr2f) <= mr || fabsf(r2 - rca2f) <= ma)) {
                         const double r2d = pair_r2(pio, spos[jj & 0x0fffffff], g);
                         in_r = r2d <= rcr2;
                         in_a = r2d <= rca2;
                     }
-                }
-                const unsigned m = __ballot_sync(0xffffffffu, in_r);
-                if (in_r) {
+                    const unsigned m = __ballot_sync(0xffffffffu, in_r);
                     const int pos = base + __popc(m & lt);
-                    if (pos < stride) tmp[(size_t)i * stride + pos] = (unsigned)jj | (in_a ? 0u : ENT_RADIAL_ONLY);
-                }
-                base += __popc(m);
-                if (SKIN) {
-                    const bool in_c = other && r2 <= rs2_incl;
-                    const unsigned mc = __ballot_sync(0xffffffffu, in_c);
-                    if (in_c) {
-                        const int pos = cbase + __popc(mc & lt);
-                        if (pos < cstride) cand_out[(size_t)i * cstride + pos] = (unsigned)jj;
-                    }
-                    cbase += __popc(mc);
+                    if (in_r && pos < stride) trow[pos] = (unsigned)jj | (in_a ? 0u : ENT_RADIAL_ONLY);
+                    base += __popc(m);
                 }
             }
             if (lane == 0) {
