@@ -515,9 +515,9 @@ k_pairs(const float4* __restrict__ spos, const Grid* __restrict__ gp, const int*
         const int tn = min(CAND_TILE, ncand - t0);
         // ---- stage the tile -------------------------------------------------------------------
         float bmax = 0.f;
+        int sg = 0;                                    // f only grows along a thread's walk: so does its segment
         for (int t = threadIdx.x; t < tn; t += P1_THREADS) {
             const int f = t0 + t;
-            int sg = 0;
             while (sg + 1 < nseg && seg_off[sg + 1] <= f) ++sg;
             const int j = seg_cell_b[sg] + (f - seg_off[sg]);
             const float4 pj = spos[j];
@@ -565,35 +565,41 @@ k_pairs(const float4* __restrict__ spos, const Grid* __restrict__ gp, const int*
             asm volatile("" : "+l"(trow), "+l"(crow));      // keep the row pointers in registers
             // fast pass: fp32 alone decides and only remembers whether any candidate fell inside a margin; such a row
             // (about one in 2000) is then redone by the exact pass, which overwrites the same entries
-            float amb_min = 1.0f;                          // min over candidates of (distance to a threshold - margin)
-#pragma unroll 2
-            for (int c0 = 0; c0 < tn; c0 += 32) {
-                const float4 c = cand[c0 + lane];          // the tile is padded with far-away dummies
-                const int jj = __float_as_int(c.w);
-                float dx = c.x - pix, dy = c.y - piy, dz = c.z - piz;
-                if (WRAP) {
-                    if (wrapx) dx -= Lx * rintf(dx * iLx);
-                    if (wrapy) dy -= Ly * rintf(dy * iLy);
-                    if (wrapz) dz -= Lz * rintf(dz * iLz);
-                }
-                const float r2 = dx * dx + dy * dy + dz * dz;
-                const bool other = (jj & 0x0fffffff) != i && (!WRAP || c0 + lane < tn);
-                const bool in_r = other & (r2 <= rcr2f);
-                // self and dummies may trip this too: that only sends the row to the exact pass
-                amb_min = fminf(amb_min, fminf(fabsf(r2 - rcr2f) - mr, fabsf(r2 - rca2f) - ma));
-                const unsigned m = __ballot_sync(0xffffffffu, in_r);
-                const unsigned pos = (unsigned)(base + __popc(m & lt));
-                st_if(in_r & (pos < (unsigned)stride), trow + pos, (unsigned)jj | (r2 <= rca2f ? 0u : ENT_RADIAL_ONLY));
-                base += __popc(m);
-                if (SKIN) {
-                    const bool in_c = other & (r2 <= rs2_incl);
-                    const unsigned mc = __ballot_sync(0xffffffffu, in_c);
-                    const unsigned cpos = (unsigned)(cbase + __popc(mc & lt));
-                    st_if(in_c & (cpos < (unsigned)cstride), crow + cpos, (unsigned)jj);
-                    cbase += __popc(mc);
+            // distance of R^2 to either threshold, minimum over the candidates (self and dummies included: harmless)
+            float near_r = 1.0e30f, near_a = 1.0e30f;
+            {
+                const float4* cp = cand + lane;
+                int lin = lane;
+#pragma unroll 4
+                for (int c0 = 0; c0 < tn; c0 += 32, cp += 32, lin += 32) {      // warp-uniform trip count (ballots inside)
+                    const float4 c = *cp;                  // the tile is padded with far-away dummies
+                    const unsigned jj = __float_as_uint(c.w);
+                    float dx = c.x - pix, dy = c.y - piy, dz = c.z - piz;
+                    if (WRAP) {
+                        if (wrapx) dx -= Lx * rintf(dx * iLx);
+                        if (wrapy) dy -= Ly * rintf(dy * iLy);
+                        if (wrapz) dz -= Lz * rintf(dz * iLz);
+                    }
+                    const float r2 = dx * dx + dy * dy + dz * dz;
+                    const bool other = (jj & 0x0fffffffu) != (unsigned)i && (!WRAP || lin < tn);
+                    const float ur = rcr2f - r2, ua = rca2f - r2;       // sign bit of ua: beyond the angular cutoff
+                    const bool in_r = other & (ur >= 0.f);
+                    near_r = fminf(near_r, fabsf(ur));
+                    near_a = fminf(near_a, fabsf(ua));
+                    const unsigned m = __ballot_sync(0xffffffffu, in_r);
+                    const unsigned pos = (unsigned)base + __popc(m & lt);
+                    st_if(in_r & (pos < (unsigned)stride), trow + pos, jj | (__float_as_uint(ua) & ENT_RADIAL_ONLY));
+                    base += __popc(m);
+                    if (SKIN) {
+                        const bool in_c = other & (r2 <= rs2_incl);
+                        const unsigned mc = __ballot_sync(0xffffffffu, in_c);
+                        const unsigned cpos = (unsigned)cbase + __popc(mc & lt);
+                        st_if(in_c & (cpos < (unsigned)cstride), crow + cpos, jj);
+                        cbase += __popc(mc);
+                    }
                 }
             }
-            const bool amb_seen = amb_min <= 0.f;
+            const bool amb_seen = near_r <= mr || near_a <= ma;
             if (__any_sync(0xffffffffu, amb_seen)) {
                 base = base0;
                 for (int c0 = 0; c0 < tn; c0 += 32) {
@@ -656,7 +662,15 @@ constexpr int MAX_STRIDE_CHUNKS = 6;    // tmp_stride <= 192
 // then radial-only) x neighbour species into col[row_start ..), the 14 run lengths, the angular count and the
 // feature-block mask of the atom are stored; with reuse_rows the tile mask of the atom's (kept) row is refreshed too.
 // sg: 16 ints of shared memory private to the warp.
-__device__ __forceinline__ void order_row(const unsigned* __restrict__ src, int ni, int row_start, int i, int lane, int* sg,
+// species of the two members of internal pair `lane` (lo | hi << 4): depends on the lane only, so callers compute it once
+__device__ __forceinline__ int lane_pair_species(int lane) {
+    if (lane >= NPAIR) return 0;
+    int hi = 0;
+    while ((hi + 1) * (hi + 2) / 2 <= lane) ++hi;
+    return prio_sp(lane - hi * (hi + 1) / 2) | (prio_sp(hi) << 4);
+}
+
+__device__ __forceinline__ void order_row(const unsigned* __restrict__ src, int ni, int row_start, int i, int lane, int lane_pair, int* sg,
                                           int* __restrict__ col, int* __restrict__ n_ang, unsigned short* __restrict__ seg_cnt,
                                           unsigned* __restrict__ amask, bool reuse_rows, const int* __restrict__ rowmap,
                                           unsigned* __restrict__ tile_mask) {
@@ -684,9 +698,7 @@ __device__ __forceinline__ void order_row(const unsigned* __restrict__ src, int 
         const unsigned am = has1 & 0x7fu, am2 = has2 & 0x7fu, rm = (am | (has1 >> 8)) & 0x7fu;
         bool pp = false;
         if (lane < NPAIR) {                                   // lane = internal pair index
-            int hi = 0;
-            while ((hi + 1) * (hi + 2) / 2 <= lane) ++hi;
-            const int sa = prio_sp(lane - hi * (hi + 1) / 2), sb = prio_sp(hi);
+            const int sa = lane_pair & 15, sb = lane_pair >> 4;
             pp = (sa == sb) ? ((am2 >> sa) & 1u) != 0 : (((am >> sa) & (am >> sb)) & 1u) != 0;
         }
         const unsigned pm = __ballot_sync(0xffffffffu, pp);
@@ -777,10 +789,11 @@ k_rows(const unsigned* __restrict__ tmp, int stride, const int* __restrict__ cnt
     __syncthreads();
 
     int* sg = segs[warp];
+    const int lane_pair = lane_pair_species(lane);
     for (int q = warp; q < ROWS_PER_BLK; q += P2_THREADS / 32) {
         const int i = i0 + q;
         if (i >= n) break;
-        order_row(tmp + (size_t)i * stride, rcnt[q], rstart[q], i, lane, sg, col, n_ang, seg_cnt, amask, reuse_rows, rowmap, tile_mask);
+        order_row(tmp + (size_t)i * stride, rcnt[q], rstart[q], i, lane, lane_pair, sg, col, n_ang, seg_cnt, amask, reuse_rows, rowmap, tile_mask);
     }
 }
 
@@ -1019,7 +1032,7 @@ k_small_rows(const unsigned* __restrict__ tmp, int stride, const int* __restrict
     }
     __syncwarp();
     if (lane == 0) { row_ptr[i] = before; if (i == n - 1) row_ptr[n] = total; }
-    order_row(tmp + (size_t)i * stride, ni, before, i, lane, segs[warp], col, n_ang, seg_cnt, amask, false, nullptr, nullptr);
+    order_row(tmp + (size_t)i * stride, ni, before, i, lane, lane_pair_species(lane), segs[warp], col, n_ang, seg_cnt, amask, false, nullptr, nullptr);
 }
 
 constexpr int SMALL_THREADS = 320;
