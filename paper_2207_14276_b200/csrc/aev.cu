@@ -88,13 +88,16 @@ struct __align__(16) WarpSmemFwd {
 };
 
 // one feature value of this lane -> the row, either fp32 or as the two-term fp16 split in the hi / lo planes
+// (planes: tiled operand layout, aev_tiled_off(); row_hi points at (row, column 0) of the hi plane, so a column adds
+//  its 64-column block, its 8-column group and its position in the group)
 template <bool PLANES>
 __device__ __forceinline__ void put_feature(float v, float* __restrict__ row_f32, __half* __restrict__ row_hi,
                                             size_t plane_stride, int colidx) {
     if (!PLANES) { row_f32[colidx] = v; return; }
     const __half hi = __float2half_rn(fminf(fmaxf(v, -65000.f), 65000.f));
-    row_hi[colidx] = hi;
-    row_hi[plane_stride + colidx] = __float2half_rn(v - __half2float(hi));
+    const int o = (colidx >> 6) * (ROW_TILE * KBLK) + ((colidx & 63) >> 3) * (ROW_TILE * 8) + (colidx & 7);
+    row_hi[o] = hi;
+    row_hi[plane_stride + o] = __float2half_rn(v - __half2float(hi));
 }
 
 template <bool PLANES, int NAg, int NZg>     // NAg x NZg: the angular grid of Eq. 5, 8 x 4 (ANI-2x shape) or 4 x 8 (ANI-1x shape)
@@ -140,7 +143,7 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
     const int row = rowmap[i];
     if (row < 0) return;                               // not a central atom of this call (partial evaluation)
     float* row_f32 = aev + (size_t)row * AEV_LD;
-    __half* row_hi = planes + (size_t)row * AEV_LD;
+    __half* row_hi = planes + aev_tiled_off(row, 0);
 
     // ---- stage all neighbours -------------------------------------------------------------------------
     for (int a = lane; a < nst; a += 32) {
@@ -305,6 +308,9 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
 //   scatter      one global atomic triple per neighbour and one for the centre.
 // -------------------------------------------------------------------------------------------------
 constexpr int BWD_WARPS = 8;
+#ifndef BWD_MINB
+#define BWD_MINB 4
+#endif
 
 constexpr int OWN = 3;   // neighbour slots per lane that can be angular (MAX_ANG = 96 = 3 x 32)
 static_assert(MAX_ANG <= OWN * 32, "angular neighbours must fit the per-lane force registers");
@@ -320,7 +326,7 @@ struct __align__(16) WarpSmemBwd {
 // SPLIT (small systems): one block of 8 warps per atom - warp 0 does the neighbour pass, the angular rounds are dealt out to the
 // 8 warps (one warp per atom is latency-bound: ~4 k dependent instructions, 36 us for a 50-atom solute whatever its size)
 template <int NAg, int NZg, bool SPLIT>
-__global__ void __launch_bounds__(BWD_WARPS * 32, 4)
+__global__ void __launch_bounds__(BWD_WARPS * 32, BWD_MINB)
 k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, const int* __restrict__ col,
           const unsigned short* __restrict__ seg_cnt, const int* __restrict__ rowmap, const Grid* __restrict__ gp,
           const __grid_constant__ AevConst K, int n, const float* __restrict__ grad, float* __restrict__ fsorted,

@@ -233,11 +233,11 @@ __global__ void k_gather_planes(const __half* __restrict__ planes, size_t plane_
         for (int c = threadIdx.x; c < AEV_DIM; c += blockDim.x) dst[(size_t)a * AEV_DIM + c] = 0.f;
         return;
     }
-    const __half* hi = planes + (size_t)row * AEV_LD;
-    const __half* lo = hi + plane_stride;
     const unsigned mask = tile_mask[row / ROW_TILE];
-    for (int c = threadIdx.x; c < AEV_DIM; c += blockDim.x)
-        dst[(size_t)a * AEV_DIM + col2feat[c]] = ((mask >> (c / KBLK)) & 1u) ? __half2float(hi[c]) + __half2float(lo[c]) : 0.f;
+    for (int c = threadIdx.x; c < AEV_DIM; c += blockDim.x) {
+        const size_t o = aev_tiled_off(row, c);
+        dst[(size_t)a * AEV_DIM + col2feat[c]] = ((mask >> (c / KBLK)) & 1u) ? __half2float(planes[o]) + __half2float(planes[plane_stride + o]) : 0.f;
+    }
 }
 
 }  // namespace dhp

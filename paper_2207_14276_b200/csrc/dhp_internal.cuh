@@ -37,6 +37,13 @@ constexpr int ROW_ALIGN = 2 * ROW_TILE;         // species groups start at multi
                                                 // kept equal within such a pair
 constexpr int KBLK = 64;                        // feature-block width: the unit in which zero columns are skipped
 constexpr int N_KBLK = AEV_LD / KBLK;           // 16 blocks: 14 angular (2 species pairs each) + 2 radial
+// The fp16 hi / lo planes of the AEV rows are stored in the tiled operand layout of the tensor path (mlp_tc.cu): the image
+// of the no-swizzle K-major UMMA A tile, [plane][row tile][64-column block][8-column group][row in tile][8 halves], so that
+// one 16-wide K step of a row tile is 4 KB of contiguous bytes per plane.  Offset in halves inside one plane:
+__host__ __device__ __forceinline__ size_t aev_tiled_off(int row, int col) {
+    return ((size_t)(row / ROW_TILE) * N_KBLK + (size_t)(col / KBLK)) * (size_t)(ROW_TILE * KBLK) +
+           (size_t)((((col % KBLK) >> 3) * ROW_TILE + (row % ROW_TILE)) * 8 + (col & 7));
+}
 constexpr int SMALL_N = 320;                      // systems up to this size take the single-block list build (above ~300 atoms one SM is
                                                 // slower than the thirteen small launches of the general path) and CUDA-graph replay
 constexpr int MAX_MODELS = DHP_MAX_MODELS;
@@ -194,7 +201,7 @@ struct Ctx {
     // host-call staging
     float* st_pos; int* st_species; int* st_mol; double* st_E; float* st_F;
     void* tc_ws;           // tensor-path workspace (mlp_tc.cu)
-    __half* aev_planes;    // [2][max_rows][AEV_LD] fp16 hi / lo planes of the AEV rows (owned by tc_ws), or null
+    __half* aev_planes;    // [2][max_rows * AEV_LD] fp16 hi / lo planes of the AEV rows in the tiled layout of aev_tiled_off() (owned by tc_ws), or null
     bool aev_in_planes;    // the last forward pass wrote aev_planes (active blocks only) instead of aev
 };
 

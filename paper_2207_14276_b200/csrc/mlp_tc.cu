@@ -1246,8 +1246,9 @@ k_gemm_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
 // Every reuse is ordered by the data dependencies themselves (see the hazard notes at the barriers).
 // ======================================================================================================
 #ifndef MID_DBG
-#define MID_DBG 0      // timing experiments only: 1 = epilogues without work, 2 = no MMAs issued, 4 = no d1 stores
+#define MID_DBG 0      // timing experiments only: 1 = epilogues without work, 2 = no MMAs issued, 4 = no d1 stores, 8 = half the weight bytes
 #endif
+#define MID_WB(x) ((MID_DBG & 8) ? (x) / 2u : (x))
 #ifndef MID_TRACE
 #define MID_TRACE 0    // timing experiments only: CTA 0 records clock64() per role for a few items and prints them at the end
 #endif
@@ -1465,8 +1466,8 @@ k_mlp_mid(const MidArgs p) {
                     // the ring's slots free up while the previous item's B2 runs; once they are refilled, wait for that B2
                     if (j == MID_SLOTS && prev_rt >= 0) load_h1_for_b2();
                     const uint32_t sa = next_slot();
-                    mbar_expect_tx(full_bar(slot), 64u * H2 * 2u + 16384u);
-                    bulk_load(sa, w + MID_W_G2 + (size_t)j * 64 * H2, 64u * H2 * 2u, full_bar(slot));
+                    mbar_expect_tx(full_bar(slot), MID_WB(64u * H2 * 2u) + 16384u);
+                    bulk_load(sa, w + MID_W_G2 + (size_t)j * 64 * H2, MID_WB(64u * H2 * 2u), full_bar(slot));
                     const size_t goff = (size_t)((j & 1) * 4) * BM * 8;
                     bulk_load(sa + MID_A_OFF, p.h1 + tile_off(p.plane_tiles, M * 4, 0, rt, e * 4 + (j >> 1)) + goff, 8192u, full_bar(slot));
                     bulk_load(sa + MID_A_OFF + 8192, p.h1 + tile_off(p.plane_tiles, M * 4, 1, rt, e * 4 + (j >> 1)) + goff, 8192u,
@@ -1475,21 +1476,21 @@ k_mlp_mid(const MidArgs p) {
                 }
                 for (int j = 0; j < H2 / 32; ++j) {                       // G3
                     const uint32_t sa = next_slot();
-                    mbar_expect_tx(full_bar(slot), 64u * H3 * 2u);
-                    bulk_load(sa, w + MID_W_G3 + (size_t)j * 64 * H3, 64u * H3 * 2u, full_bar(slot));
+                    mbar_expect_tx(full_bar(slot), MID_WB(64u * H3 * 2u));
+                    bulk_load(sa, w + MID_W_G3 + (size_t)j * 64 * H3, MID_WB(64u * H3 * 2u), full_bar(slot));
                     advance();
                 }
                 if (p.forward_only) continue;
                 for (int j = 0; j < H3 / 32; ++j) {                       // B3
                     const uint32_t sa = next_slot();
-                    mbar_expect_tx(full_bar(slot), 64u * H2 * 2u);
-                    bulk_load(sa, w + MID_W_B3 + (size_t)j * 64 * H2, 64u * H2 * 2u, full_bar(slot));
+                    mbar_expect_tx(full_bar(slot), MID_WB(64u * H2 * 2u));
+                    bulk_load(sa, w + MID_W_B3 + (size_t)j * 64 * H2, MID_WB(64u * H2 * 2u), full_bar(slot));
                     advance();
                 }
                 for (int j = 0; j < H2 / 32; ++j) {                       // B2
                     const uint32_t sa = next_slot();
-                    mbar_expect_tx(full_bar(slot), 64u * H1 * 2u);
-                    bulk_load(sa, w + MID_W_B2 + (size_t)j * 64 * H1, 64u * H1 * 2u, full_bar(slot));
+                    mbar_expect_tx(full_bar(slot), MID_WB(64u * H1 * 2u));
+                    bulk_load(sa, w + MID_W_B2 + (size_t)j * 64 * H1, MID_WB(64u * H1 * 2u), full_bar(slot));
                     advance();
                 }
                 prev_rt = rt; prev_e = e;
@@ -1816,8 +1817,9 @@ __global__ void k_split_rows(const float* __restrict__ src, int ld_src, const in
         const float4 v = *reinterpret_cast<const float4*>(src + (size_t)r * ld_src + c);
         __half h[4], l[4];
         split_half(v.x, h[0], l[0]); split_half(v.y, h[1], l[1]); split_half(v.z, h[2], l[2]); split_half(v.w, h[3], l[3]);
-        *reinterpret_cast<uint2*>(dst + (size_t)r * ncol + c) = *reinterpret_cast<uint2*>(h);
-        *reinterpret_cast<uint2*>(dst + ((size_t)plane_rows + r) * ncol + c) = *reinterpret_cast<uint2*>(l);
+        // the tiled operand layout of the AEV planes (ncol = AEV_LD): 4 consecutive columns stay inside one 8-column group
+        *reinterpret_cast<uint2*>(dst + aev_tiled_off(r, c)) = *reinterpret_cast<uint2*>(h);
+        *reinterpret_cast<uint2*>(dst + (size_t)plane_rows * ncol + aev_tiled_off(r, c)) = *reinterpret_cast<uint2*>(l);
     }
 }
 
@@ -1951,7 +1953,6 @@ int mlp_tc_alloc(Ctx* ctx) {
         (rc = set_smem_tc<EPI_OUT, CMP_NONE>(ctx)) != DHP_OK || (rc = set_smem_tc<EPI_DCELU, CMP_NONE>(ctx)) != DHP_OK ||
         (rc = set_smem_tc<EPI_GRAD, CMP_N>(ctx)) != DHP_OK)
         return rc;
-    DHP_CUDA(ctx, cudaFuncSetAttribute((k_gemm_pair<EPI_CELU, CMP_K>), cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM_BYTES));
     DHP_CUDA(ctx, cudaFuncSetAttribute((k_gemm_pair<EPI_GRAD, CMP_N>), cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM_BYTES));
     DHP_CUDA(ctx, cudaFuncSetAttribute(k_mlp_mid, cudaFuncAttributeMaxDynamicSharedMemorySize, MID_SMEM));
     DHP_CUDA(ctx, cudaFuncSetAttribute((k_gemm_tc2<EPI_CELU, CMP_K>), cudaFuncAttributeMaxDynamicSharedMemorySize, T2_SMEM));
@@ -2070,10 +2071,14 @@ int mlp_tc(Ctx* ctx, const Weights* wt, bool forward_only) {
     // G1: AEV rows (row-major, TMA) -> h1
     a.K = AEV_LD; a.BN = H1; a.n_tiles = M; a.a_k_off_per_tile = 0; a.b_rows_per_species = M * H1; a.b_rows_per_tile = H1;
     a.acc_scale = 1.0f / W_SCALE; a.bias = t->b1;
-    a.a_tiled = nullptr; a.out_planes = ws->h1; a.out_kblocks = M * KB1; a.out_cols_per_tile = H1;
+    a.a_tiled = ws->aev; a.a_kblocks = N_KBLK; a.a_kb_per_tile = 0;      // the AEV planes are in the tiled operand layout: plain bulk copies
+    a.out_planes = ws->h1; a.out_kblocks = M * KB1; a.out_cols_per_tile = H1;
     a.sched = ctx->tc_sched + 0;
     const bool fusedp = ctx->mlp_mode != DHP_MLP_TENSOR_LAYERWISE;
-    const bool pairs = (ctx->tc_pairs & 1) && fusedp, pairs_b1 = (ctx->tc_pairs & 2) && fusedp;    // G1 / B1 on CTA pairs (cta_group::2)
+    // B1 on CTA pairs (cta_group::2).  The pair kernel's G1 instantiation fetched row-major AEV planes with tensor TMA; the planes
+    // are now in the tiled operand layout and that experiment (measured equal to the one-CTA kernel) is retired:
+    // bit 0 of DHP_TC_PAIRS is ignored
+    const bool pairs = false, pairs_b1 = (ctx->tc_pairs & 2) && fusedp;
     const int ncl = ctx->sm_count / 2;
     if (pairs || pairs_b1) {
         DHP_LAUNCH(ctx, k_pair_schedule, 1, 1024, 0, ctx->tile_mask, ctx->sp_start, M, ncl, ws->pair_scratch, ws->pair_sched);
@@ -2084,8 +2089,7 @@ int mlp_tc(Ctx* ctx, const Weights* wt, bool forward_only) {
     const bool big = n_pairs_bound * M >= 12 * (int64_t)ctx->sm_count;
     const bool two_g1 = fusedp && !pairs && ((ctx->tc_two & 1) != 0) && big;
     const bool two_b1 = fusedp && !pairs_b1 && ((ctx->tc_two & 2) != 0) && big;
-    if (pairs) rc = launch_pair<EPI_CELU, CMP_K>(ctx, ws->m_aev, t->m_w1f_half, a);
-    else if (two_g1) rc = launch_gemm2<EPI_CELU, CMP_K>(ctx, ws->m_aev, t->m_w1f, a);
+    if (two_g1) rc = launch_gemm2<EPI_CELU, CMP_K>(ctx, ws->m_aev, t->m_w1f, a);
     else rc = launch_gemm<EPI_CELU, CMP_K>(ctx, ws->m_aev, t->m_w1f, a);
     if (rc != DHP_OK) return rc;
     prof_mark(ctx, DHP_PHASE_MLP_MID);
