@@ -1775,6 +1775,538 @@ k_mlp_mid(const MidArgs p) {
 }
 
 
+// ======================================================================================================
+// G1 fused into the front of the middle chain: one work item = (row tile, network) runs
+//     AEV rows -> h1 -> h2 -> (E_i, d3) -> d2 -> d1
+// inside one CTA, so h1 never goes to HBM as an operand (profiles/r2b: writing h1, 754 MB per step, is what G1 waited
+// for, and reading it back was most of k_mlp_mid's first phase).  Differences from k_mlp_mid:
+//   * G1 accumulates z1 (256 columns) in tensor memory; its epilogue writes h1 = CELU(z1 + b1) in 64-column blocks into X
+//     as the A operand of G2 (the fourth block takes the place of the first once G2's first K block has been read), so G2
+//     starts under G1's epilogue exactly as G3 starts under G2's.  The same thread also stores its h1 values to a per-CTA
+//     scratch tile (128 KB, rewritten by every item: it stays in L2) from which B2's epilogue gets CELU'(z1) back.
+//   * operands of G1 stream through the ring one 16-wide K step per slot: the W1 image of the step (16 KB, pre-tiled like
+//     the other weights) and the AEV planes' 2 x 4 KB (tiled operand layout, aev_tiled_off()); only the feature blocks of the
+//     row tile's mask are visited.
+//   * tensor memory is used in a ping-pong map, offset O = 256 (item parity): z1 [O, O+256); G2 accumulator [O+256, O+448);
+//     G3 accumulator [O, O+160); d3 [O+160, O+320) (hi 80 columns, lo 80 columns); B3 accumulator [O+320, O+512); B2
+//     accumulator [O, O+256) - all modulo 512.  The next item's G1 (z1 at [O+256, ...)) therefore runs under this item's B2
+//     epilogue, which is where the tensor pipe idled in k_mlp_mid while d1 was stored.
+// ======================================================================================================
+constexpr int FU_SLOTS = 5;
+constexpr int FU_SLOT_BYTES = 24576;             // G1: W1 image of one K step (16 KB) + AEV hi (4 KB) + lo (4 KB); G2 / G3 / B3: two K steps; B2: one
+constexpr int FU_A_OFF = 16384;
+constexpr int FU_CONST_FLOATS = H1 + H2 + H3 + H3;   // b1 | b2 | b3 | w4
+constexpr int FU_CONST_BYTES = FU_CONST_FLOATS * 4;
+constexpr int FU_SMEM = MID_X_BYTES + FU_SLOTS * FU_SLOT_BYTES + 2 * FU_CONST_BYTES + 1024 /*align*/ + 512 /*barriers, TMEM word, ring*/;
+static_assert(FU_SMEM <= 232448, "shared memory of k_mlp_fused");
+constexpr int FU_W1_STEP = 32 * H1;              // halves of the W1 image of one K step: [plane][8-column group (2)][n][8]
+constexpr int FU_SCRATCH = 2 * H1 * BM;          // halves of one CTA's h1 scratch tile: [plane][64-column block (4)][group][row][8]
+
+struct FusedArgs {
+    int single, forward_only, n_models, plane_tiles;
+    const int* row_species;
+    const int* sp_start;
+    const unsigned* tile_mask;
+    const __half* aev;        // AEV planes, tiled operand layout
+    const __half* w1img;      // [species][network][64 K steps][FU_W1_STEP]
+    const __half* wimg;       // [species][network][MID_W_TOTAL] (G2, G3, B3, B2)
+    __half* scratch;          // [gridDim.x][FU_SCRATCH]
+    __half* d1;
+    const float *b1, *b2, *b3, *w4, *b4;
+    float inv_models, alpha;
+    float* e_atom;
+    int* sched;
+};
+
+__device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
+
+__global__ void __launch_bounds__(MID_THREADS, 1)
+k_mlp_fused(const FusedArgs p) {
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t raw = smem_u32(smem_raw);
+    const uint32_t base = (raw + 1023u) & ~1023u;
+    uint8_t* x_ptr = smem_raw + (base - raw);
+    const uint32_t xs = base;
+    const uint32_t slots = base + MID_X_BYTES;
+    const uint32_t cst_s = slots + FU_SLOTS * FU_SLOT_BYTES;
+    const float* cst_ptr = reinterpret_cast<const float*>(x_ptr + MID_X_BYTES + FU_SLOTS * FU_SLOT_BYTES);
+    const uint32_t bar0 = cst_s + 2 * FU_CONST_BYTES;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(x_ptr + MID_X_BYTES + FU_SLOTS * FU_SLOT_BYTES + 2 * FU_CONST_BYTES);
+    // barriers: full[SLOTS], empty[SLOTS], then 17 single ones (below), sfull[RING], sempty[RING]; then the TMEM word and the item ring
+    constexpr int NB1 = 17;
+    constexpr int NBARS = 2 * FU_SLOTS + NB1 + 2 * RING;
+    auto full_bar = [&](int s) { return bar0 + 8u * s; };
+    auto empty_bar = [&](int s) { return bar0 + 8u * (FU_SLOTS + s); };
+    const uint32_t b1s = bar0 + 8u * (2 * FU_SLOTS);
+    const uint32_t acc1_bar = b1s, accp_bar = b1s + 8u, accq_bar = b1s + 16u;
+    auto xr_bar = [&](int k) { return b1s + 24u + 8u * k; };            // k = 0..3: 64-column block k of an epilogue's output is ready
+    const uint32_t x0free_bar = b1s + 56u;                              // G2 has read h1 block 0: its place in X may take block 3
+    const uint32_t xfree_bar = b1s + 64u;                               // B2's MMAs have completed: X (d2) is dead
+    const uint32_t hsaved_bar = b1s + 72u;                              // the item's h1 is in the scratch tile (visible to the async proxy)
+    auto hfull_bar = [&](int k) { return b1s + 80u + 8u * k; };         // k = 0..2: h1 block k is back in X (for CELU'(z1))
+    auto cfull_bar = [&](int b) { return b1s + 104u + 8u * b; };
+    auto cempty_bar = [&](int b) { return b1s + 120u + 8u * b; };
+    auto sfull_bar = [&](int s) { return bar0 + 8u * (2 * FU_SLOTS + NB1 + s); };
+    auto sempty_bar = [&](int s) { return bar0 + 8u * (2 * FU_SLOTS + NB1 + RING + s); };
+    volatile uint32_t* tmem_word = reinterpret_cast<volatile uint32_t*>(bars + NBARS);
+    volatile int* ring = reinterpret_cast<volatile int*>(bars + NBARS + 1);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int M = p.n_models;
+    const int total_items = (p.sp_start[NSP] / BM) * M;
+    __half* scratch = p.scratch + (size_t)blockIdx.x * FU_SCRATCH;
+
+    if (warp == MID_EPI_WARPS && lane == 0) {
+        for (int s = 0; s < FU_SLOTS; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+        mbar_init(acc1_bar, 1); mbar_init(accp_bar, 1); mbar_init(accq_bar, 1);
+        for (int k = 0; k < 4; ++k) mbar_init(xr_bar(k), MID_EPI_WARPS);
+        mbar_init(x0free_bar, 1); mbar_init(xfree_bar, 1); mbar_init(hsaved_bar, MID_EPI_WARPS);
+        for (int k = 0; k < 3; ++k) mbar_init(hfull_bar(k), 1);
+        for (int b = 0; b < 2; ++b) { mbar_init(cfull_bar(b), 1); mbar_init(cempty_bar(b), MID_EPI_WARPS); }
+        for (int s = 0; s < RING; ++s) { mbar_init(sfull_bar(s), 1); mbar_init(sempty_bar(s), 1 + MID_EPI_WARPS); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == MID_EPI_WARPS + 1) tmem_alloc(smem_u32((const void*)tmem_word), TMEM_COLS);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_word;
+
+    auto g1_mask = [&](int rt) -> unsigned { const unsigned m = p.tile_mask[rt]; return m ? m : (1u << 14); };   // an all-zero tile runs one block of zeros
+
+    if (warp == MID_EPI_WARPS) {
+        // ===== item scheduler + producer =====
+        if (elect_one()) {
+            int slot = 0; uint32_t phase = 0;
+            int rs = 0; uint32_t rphase = 0;
+            int cb = 0; uint32_t cphase = 0;
+            uint32_t hphase = 0;
+            bool have_prev = false;
+            auto next_slot = [&]() -> uint32_t {
+                mbar_wait(empty_bar(slot), phase ^ 1u);
+                return slots + (uint32_t)slot * FU_SLOT_BYTES;
+            };
+            auto advance = [&]() { if (++slot == FU_SLOTS) { slot = 0; phase ^= 1u; } };
+            // h1 of the PREVIOUS item: scratch -> X once its B2 MMAs (the last readers of d2 in X) have completed; three 64-column
+            // blocks (hi plane then lo plane) for CELU'(z1) in B2's epilogue, the fourth comes by plain loads there
+            auto reload_h1 = [&]() {
+                mbar_wait(hsaved_bar, hphase);
+                mbar_wait(xfree_bar, hphase); hphase ^= 1u;
+                for (int k = 0; k < 3; ++k) {
+                    mbar_expect_tx(hfull_bar(k), (uint32_t)MID_H_ROUND);
+                    bulk_load(xs + (uint32_t)(k * MID_H_ROUND), scratch + (size_t)k * (BM * BK), 16384u, hfull_bar(k));
+                    bulk_load(xs + (uint32_t)(k * MID_H_ROUND) + 16384u, scratch + (size_t)(4 + k) * (BM * BK), 16384u, hfull_bar(k));
+                }
+            };
+            for (;;) {
+                int item = atomicAdd(p.sched, 1);
+                if (item >= total_items) item = -1;
+                mbar_wait(sempty_bar(rs), rphase ^ 1u);
+                ring[rs] = item;
+                mbar_arrive(sfull_bar(rs));
+                if (++rs == RING) { rs = 0; rphase ^= 1u; }
+                if (item < 0) break;
+                const int rt = item / M, e = item - rt * M;
+                const int s = max(p.row_species[rt * BM], 0);
+                const int se = s * M + e;
+                const __half* w = p.wimg + (size_t)se * MID_W_TOTAL;
+                const __half* w1 = p.w1img + (size_t)se * (AEV_LD / 16) * FU_W1_STEP;
+                {   // b1 | b2 | b3 | w4 of this network
+                    mbar_wait(cempty_bar(cb), cphase ^ 1u);
+                    const uint32_t dst = cst_s + (uint32_t)(cb * FU_CONST_BYTES);
+                    mbar_expect_tx(cfull_bar(cb), (uint32_t)FU_CONST_BYTES);
+                    bulk_load(dst, p.b1 + (size_t)se * H1, H1 * 4u, cfull_bar(cb));
+                    bulk_load(dst + H1 * 4u, p.b2 + (size_t)se * H2, H2 * 4u, cfull_bar(cb));
+                    bulk_load(dst + (H1 + H2) * 4u, p.b3 + (size_t)se * H3, H3 * 4u, cfull_bar(cb));
+                    bulk_load(dst + (H1 + H2 + H3) * 4u, p.w4 + (size_t)se * H3, H3 * 4u, cfull_bar(cb));
+                    if (++cb == 2) { cb = 0; cphase ^= 1u; }
+                }
+                // G1: the K steps of the active feature blocks.  The ring refills while the previous item's B2 runs; once it is
+                // full, wait for that B2 and bring the previous item's h1 back for its epilogue
+                bool reloaded = !have_prev || p.forward_only;
+                int issued = 0;
+                for (unsigned km = g1_mask(rt); km; km &= km - 1u) {
+                    const int kb = __ffs(km) - 1;
+                    const __half* a_hi = p.aev + tile_off(p.plane_tiles, N_KBLK, 0, rt, kb);
+                    const __half* a_lo = p.aev + tile_off(p.plane_tiles, N_KBLK, 1, rt, kb);
+                    for (int ks = 0; ks < 4; ++ks) {
+                        if (issued == FU_SLOTS && !reloaded) { reload_h1(); reloaded = true; }
+                        const uint32_t sa = next_slot();
+                        mbar_expect_tx(full_bar(slot), (uint32_t)FU_SLOT_BYTES);
+                        bulk_load(sa, w1 + (size_t)(kb * 4 + ks) * FU_W1_STEP, 16384u, full_bar(slot));
+                        bulk_load(sa + FU_A_OFF, a_hi + ks * (2 * BM * 8), 4096u, full_bar(slot));
+                        bulk_load(sa + FU_A_OFF + 4096u, a_lo + ks * (2 * BM * 8), 4096u, full_bar(slot));
+                        advance();
+                        ++issued;
+                    }
+                }
+                if (!reloaded) reload_h1();
+                for (int j = 0; j < H1 / 32; ++j) {                       // G2: W2 K steps 2j, 2j+1 (A = h1 in X)
+                    const uint32_t sa = next_slot();
+                    mbar_expect_tx(full_bar(slot), 64u * H2 * 2u);
+                    bulk_load(sa, w + MID_W_G2 + (size_t)j * 64 * H2, 64u * H2 * 2u, full_bar(slot));
+                    advance();
+                }
+                for (int j = 0; j < H2 / 32; ++j) {                       // G3
+                    const uint32_t sa = next_slot();
+                    mbar_expect_tx(full_bar(slot), 64u * H3 * 2u);
+                    bulk_load(sa, w + MID_W_G3 + (size_t)j * 64 * H3, 64u * H3 * 2u, full_bar(slot));
+                    advance();
+                }
+                have_prev = true;
+                if (p.forward_only) continue;
+                for (int j = 0; j < H3 / 32; ++j) {                       // B3
+                    const uint32_t sa = next_slot();
+                    mbar_expect_tx(full_bar(slot), 64u * H2 * 2u);
+                    bulk_load(sa, w + MID_W_B3 + (size_t)j * 64 * H2, 64u * H2 * 2u, full_bar(slot));
+                    advance();
+                }
+                for (int j = 0; j < H2 / 16; ++j) {                       // B2: one K step per slot (16 KB)
+                    const uint32_t sa = next_slot();
+                    mbar_expect_tx(full_bar(slot), 32u * H1 * 2u);
+                    bulk_load(sa, w + MID_W_B2 + (size_t)j * 32 * H1, 32u * H1 * 2u, full_bar(slot));
+                    advance();
+                }
+            }
+            if (have_prev && !p.forward_only) reload_h1();               // the last item of this CTA
+        }
+    } else if (warp == MID_EPI_WARPS + 1) {
+        // ===== MMA issuer =====
+        if (elect_one()) {
+            int slot = 0; uint32_t phase = 0;
+            int rs = 0; uint32_t rphase = 0;
+            uint32_t xphase = 0;                                   // bit k: parity of xr[k]
+            int nit = 0;
+            auto wait_xr = [&](int kb) {
+                mbar_wait(xr_bar(kb), (xphase >> kb) & 1u);
+                xphase ^= 1u << kb;
+                tc_fence_after();
+            };
+            auto wait_slot = [&]() -> uint32_t {
+                mbar_wait(full_bar(slot), phase);
+                tc_fence_after();
+                return slots + (uint32_t)slot * FU_SLOT_BYTES;
+            };
+            auto release_slot = [&]() {
+                umma_commit(empty_bar(slot));
+                if (++slot == FU_SLOTS) { slot = 0; phase ^= 1u; }
+            };
+            auto mma3 = [&](uint32_t d, uint64_t a_hi, uint64_t a_lo, uint64_t b_hi, uint64_t b_lo, uint32_t idesc, uint32_t acc) {
+                umma_f16(d, a_hi, b_hi, idesc, acc);
+                if (!p.single) { umma_f16(d, a_hi, b_lo, idesc, 1u); umma_f16(d, a_lo, b_hi, idesc, 1u); }
+            };
+            auto mma3_ts = [&](uint32_t d, uint32_t a_hi, uint32_t a_lo, uint64_t b_hi, uint64_t b_lo, uint32_t idesc, uint32_t acc) {
+                umma_f16_ts(d, a_hi, b_hi, idesc, acc);
+                if (!p.single) { umma_f16_ts(d, a_hi, b_lo, idesc, 1u); umma_f16_ts(d, a_lo, b_hi, idesc, 1u); }
+            };
+            for (;;) {
+                mbar_wait(sfull_bar(rs), rphase);
+                const int item = ring[rs];
+                mbar_arrive(sempty_bar(rs));
+                if (++rs == RING) { rs = 0; rphase ^= 1u; }
+                if (item < 0) break;
+                const int rt = item / M;
+                const uint32_t O = (nit & 1) ? 256u : 0u;
+                ++nit;
+                {   // G1: AEV W1^T -> z1 at [O, O + 256)
+                    const uint32_t idesc = make_idesc(H1);
+                    const int nsteps = 4 * __popc(g1_mask(rt));
+                    uint32_t accumulate = 0u;
+                    for (int j = 0; j < nsteps; ++j) {
+                        const uint32_t sa = wait_slot();
+                        mma3(tmem_base + O, make_desc_ns(sa + FU_A_OFF, 2048u), make_desc_ns(sa + FU_A_OFF + 4096u, 2048u),
+                             make_desc_ns(sa, H1 * 16u), make_desc_ns(sa + 2u * H1 * 16u, H1 * 16u), idesc, accumulate);
+                        accumulate = 1u;
+                        release_slot();
+                    }
+                    umma_commit(acc1_bar);
+                }
+                {   // G2: h1 W2^T -> [O + 256, O + 448); h1 block kb is K steps 4 kb .. 4 kb + 3, block 3 sits in block 0's place
+                    const uint32_t idesc = make_idesc(H2), lbo = H2 * 16u, d = tmem_base + (O ^ 256u);
+                    uint32_t accumulate = 0u;
+                    for (int sl = 0; sl < H1 / 32; ++sl) {
+                        if ((sl & 1) == 0) wait_xr(sl >> 1);
+                        const uint32_t sa = wait_slot();
+#pragma unroll
+                        for (int t = 0; t < 2; ++t) {
+                            const int j = 2 * sl + t;
+                            const uint32_t sb = sa + (uint32_t)t * 4u * lbo;
+                            const uint32_t a0 = xs + (uint32_t)((2 * j) % 24) * 2048u;
+                            mma3(d, make_desc_ns(a0, 2048u), make_desc_ns(a0 + (uint32_t)MID_X_PLANE, 2048u), make_desc_ns(sb, lbo),
+                                 make_desc_ns(sb + 2u * lbo, lbo), idesc, accumulate);
+                            accumulate = 1u;
+                        }
+                        release_slot();
+                        if (sl == 1) umma_commit(x0free_bar);
+                    }
+                    umma_commit(accp_bar);
+                }
+                {   // G3: h2 W3^T -> [O, O + 160)
+                    const uint32_t idesc = make_idesc(H3), lbo = H3 * 16u, d = tmem_base + O;
+                    uint32_t accumulate = 0u;
+                    for (int sl = 0; sl < H2 / 32; ++sl) {
+                        if ((sl & 1) == 0) wait_xr(sl >> 1);
+                        const uint32_t sa = wait_slot();
+#pragma unroll
+                        for (int t = 0; t < 2; ++t) {
+                            const int j = 2 * sl + t;
+                            const uint32_t sb = sa + (uint32_t)t * 4u * lbo;
+                            const uint32_t a0 = xs + (uint32_t)j * 4096u;
+                            mma3(d, make_desc_ns(a0, 2048u), make_desc_ns(a0 + (uint32_t)MID_X_PLANE, 2048u), make_desc_ns(sb, lbo),
+                                 make_desc_ns(sb + 2u * lbo, lbo), idesc, accumulate);
+                            accumulate = 1u;
+                        }
+                        release_slot();
+                    }
+                    umma_commit(accq_bar);
+                }
+                if (p.forward_only) continue;
+                {   // B3: d3 W3 -> [O + 320, O + 512); A = d3 in tensor memory, K step j at hi (O + 160 + 8 j), lo (O + 240 + 8 j) mod 512
+                    const uint32_t idesc = make_idesc(H2), lbo = H2 * 16u, d = tmem_base + ((O + 320u) & 511u);
+                    uint32_t accumulate = 0u;
+                    for (int sl = 0; sl < H3 / 32; ++sl) {
+                        if ((sl & 1) == 0) wait_xr(sl >> 1);
+                        const uint32_t sa = wait_slot();
+#pragma unroll
+                        for (int t = 0; t < 2; ++t) {
+                            const uint32_t j = (uint32_t)(2 * sl + t);
+                            const uint32_t sb = sa + (uint32_t)t * 4u * lbo;
+                            mma3_ts(d, tmem_base + ((O + 160u + 8u * j) & 511u), tmem_base + ((O + 240u + 8u * j) & 511u), make_desc_ns(sb, lbo),
+                                    make_desc_ns(sb + 2u * lbo, lbo), idesc, accumulate);
+                            accumulate = 1u;
+                        }
+                        release_slot();
+                    }
+                    umma_commit(accp_bar);
+                }
+                {   // B2: d2 W2 -> [O, O + 256); one K step per slot
+                    const uint32_t idesc = make_idesc(H1), lbo = H1 * 16u, d = tmem_base + O;
+                    uint32_t accumulate = 0u;
+                    for (int j = 0; j < H2 / 16; ++j) {
+                        if ((j & 3) == 0) wait_xr(j >> 2);
+                        const uint32_t sa = wait_slot();
+                        const uint32_t a0 = xs + (uint32_t)j * 4096u;
+                        mma3(d, make_desc_ns(a0, 2048u), make_desc_ns(a0 + (uint32_t)MID_X_PLANE, 2048u), make_desc_ns(sa, lbo),
+                             make_desc_ns(sa + 2u * lbo, lbo), idesc, accumulate);
+                        accumulate = 1u;
+                        release_slot();
+                    }
+                    umma_commit(accq_bar);
+                    umma_commit(xfree_bar);                               // ... and X is free for the h1 reload (producer)
+                }
+            }
+        }
+    } else {
+        // ===== epilogue warps: a warp may touch only TMEM lanes 32 (warp % 4) .. + 31; the four warps of a lane
+        //       quadrant take every fourth 16-column chunk, so round k of an epilogue covers columns 64 k .. 64 k + 63 =====
+        const int q = warp & 3, cg = warp >> 2;
+        const int r_in = q * 32 + lane;
+        const uint32_t lane_base = tmem_base + ((uint32_t)(q * 32) << 16);
+        int rs = 0; uint32_t rphase = 0;
+        uint32_t a1phase = 0, pphase = 0, qphase = 0, hph = 0, x0ph = 0;
+        int cb = 0; uint32_t cphase = 0;
+        int nit = 0;
+        const float kexp = 1.4426950408889634f / p.alpha, inv_alpha = 1.0f / p.alpha;
+        const float sc = 1.0f / W_SCALE;
+        auto signal_x = [&](int k) {
+            fence_proxy_async_smem();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(xr_bar(k));
+        };
+        auto signal_t = [&](int k) {
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(xr_bar(k));
+        };
+        auto lds16 = [&](const float* src, float (&x)[16]) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const float4 t4 = *reinterpret_cast<const float4*>(src + 4 * i);
+                x[4 * i] = t4.x; x[4 * i + 1] = t4.y; x[4 * i + 2] = t4.z; x[4 * i + 3] = t4.w;
+            }
+        };
+        // this thread's 16 columns c0.. of the scratch tile / of d1's item: offsets inside one plane of 4 blocks
+        auto tile_in = [&](int c0) -> size_t { return (size_t)(c0 >> 6) * (BM * BK) + (size_t)(((c0 & 63) >> 3) * BM + r_in) * 8; };
+        for (;;) {
+            mbar_wait(sfull_bar(rs), rphase);
+            const int item = ring[rs];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(sempty_bar(rs));
+            if (++rs == RING) { rs = 0; rphase ^= 1u; }
+            if (item < 0) break;
+            const int rt = item / M, e = item - rt * M;
+            const int s = max(p.row_species[rt * BM], 0);
+            const int row = rt * BM + r_in;
+            const int se = s * M + e;
+            const uint32_t O = (nit & 1) ? 256u : 0u;
+            ++nit;
+            uint32_t v[16];
+            float x[16], aux[16];
+            mbar_wait(cfull_bar(cb), cphase);
+            const float* cst = cst_ptr + cb * FU_CONST_FLOATS;
+            // ---- G1 (z1): h1 = CELU(acc / 64 + b1) -> X (A of G2) and, for CELU'(z1) later, the scratch tile
+            mbar_wait(acc1_bar, a1phase); a1phase ^= 1u;
+            tc_fence_after();
+#pragma unroll 1
+            for (int k = 0; k < 4; ++k) {
+                const int c0 = 64 * k + 16 * cg;
+                tmem_ld16_issue(lane_base + O + (uint32_t)c0, v);
+                lds16(cst + c0, aux);
+                if (k == 3) { mbar_wait(x0free_bar, x0ph); x0ph ^= 1u; }      // G2 is done with block 0: block 3 takes its place
+                tmem_ld_wait();
+#pragma unroll
+                for (int i = 0; i < 16; ++i) x[i] = celu_f(fmaf(__uint_as_float(v[i]), sc, aux[i]), p.alpha, kexp);
+                store_split16_x(x, x_ptr, k < 3 ? c0 : c0 - 192, r_in);
+                if (!p.forward_only) store_split16_tiled(x, scratch + tile_in(c0), scratch + (size_t)4 * (BM * BK) + tile_in(c0));
+                signal_x(k);
+            }
+            if (!p.forward_only) {           // the scratch stores of this warp are ordered before the producer's bulk reads
+                fence_proxy_async_all();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(hsaved_bar);
+            }
+            // ---- G2: h2 = CELU(acc / 64 + b2) -> X, block by block
+            mbar_wait(accp_bar, pphase); pphase ^= 1u;
+            tc_fence_after();
+#pragma unroll 1
+            for (int k = 0; k < 3; ++k) {
+                const int c0 = 64 * k + 16 * cg;
+                tmem_ld16_issue(lane_base + (O ^ 256u) + (uint32_t)c0, v);
+                lds16(cst + H1 + c0, aux);
+                tmem_ld_wait();
+#pragma unroll
+                for (int i = 0; i < 16; ++i) x[i] = celu_f(fmaf(__uint_as_float(v[i]), sc, aux[i]), p.alpha, kexp);
+                store_split16_x(x, x_ptr, c0, r_in);
+                signal_x(k);
+            }
+            // ---- G3: h3 = CELU(acc / 64 + b3); E_i += (w4.h3 + b4)/M; d3 = w4 CELU'(z3) 2^10 / M -> tensor memory (A of B3)
+            float w4v[16];
+            mbar_wait(accq_bar, qphase); qphase ^= 1u;
+            tc_fence_after();
+            float e_acc = 0.f;
+            const float dsc = p.inv_models * D_SCALE;
+#pragma unroll 1
+            for (int k = 0; k < 3; ++k) {
+                const int c0 = 64 * k + 16 * cg;
+                if (c0 < H3) {
+                    tmem_ld16_issue(lane_base + O + (uint32_t)c0, v);
+                    lds16(cst + H1 + H2 + c0, aux);
+                    lds16(cst + H1 + H2 + H3 + c0, w4v);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) {
+                        const float h = celu_f(fmaf(__uint_as_float(v[i]), sc, aux[i]), p.alpha, kexp);
+                        e_acc = fmaf(w4v[i], h, e_acc);
+                        x[i] = w4v[i] * dsc * dcelu_from_h(h, inv_alpha);
+                    }
+                    if (!p.forward_only) {
+                        uint32_t ph[8], pl[8];
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) split_pair(x[2 * i], x[2 * i + 1], ph[i], pl[i]);   // K even -> low half
+                        tmem_st8(lane_base + ((O + 160u + (uint32_t)(c0 >> 1)) & 511u), ph);
+                        tmem_st8(lane_base + ((O + 240u + (uint32_t)(c0 >> 1)) & 511u), pl);
+                        tmem_st_wait();
+                    }
+                }
+                if (!p.forward_only) signal_t(k);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(cempty_bar(cb));
+            if (++cb == 2) { cb = 0; cphase ^= 1u; }
+            atomicAdd(&p.e_atom[row], (e_acc + (cg == 0 ? p.b4[se] : 0.f)) * p.inv_models);
+            if (p.forward_only) { tc_fence_before(); continue; }
+            // ---- B3: d2 = (acc / 64) CELU'(z2), CELU' from this thread's own h2 in X, d2 written over it
+            mbar_wait(accp_bar, pphase); pphase ^= 1u;
+            tc_fence_after();
+#pragma unroll 1
+            for (int k = 0; k < 3; ++k) {
+                const int c0 = 64 * k + 16 * cg;
+                tmem_ld16_issue(lane_base + ((O + 320u) & 511u) + (uint32_t)c0, v);
+                uint4 hh[2], hl[2];
+#pragma unroll
+                for (int i = 0; i < 2; ++i) {
+                    const uint8_t* src = x_ptr + (size_t)(((c0 >> 3) + i) * BM + r_in) * 16;
+                    hh[i] = *reinterpret_cast<const uint4*>(src);
+                    hl[i] = *reinterpret_cast<const uint4*>(src + MID_X_PLANE);
+                }
+                join16(hh, hl, aux);
+                tmem_ld_wait();
+#pragma unroll
+                for (int i = 0; i < 16; ++i) x[i] = __uint_as_float(v[i]) * sc * dcelu_from_h(aux[i], inv_alpha);
+                store_split16_x(x, x_ptr, c0, r_in);
+                signal_x(k);
+            }
+            // ---- B2: d1 = (acc / 64) CELU'(z1) -> global (tiled planes).  h1 blocks 0..2 come back into X by bulk copy (producer),
+            //      block 3 by plain loads of what this very thread stored (issued here, their latency runs under the first rounds)
+            uint4 gh[2], gl[2], lh[2], ll[2];
+            {
+                const __half* s_hi = scratch + tile_in(192 + cg * 16);
+                const __half* s_lo = s_hi + (size_t)4 * (BM * BK);
+#pragma unroll
+                for (int i = 0; i < 2; ++i) {
+                    lh[i] = *reinterpret_cast<const uint4*>(s_hi + i * (BM * 8));
+                    ll[i] = *reinterpret_cast<const uint4*>(s_lo + i * (BM * 8));
+                }
+            }
+            mbar_wait(accq_bar, qphase); qphase ^= 1u;
+            tc_fence_after();
+            __half* d_hi = p.d1 + tile_off(p.plane_tiles, M * 4, 0, rt, e * 4);
+            __half* d_lo = p.d1 + tile_off(p.plane_tiles, M * 4, 1, rt, e * 4);
+#pragma unroll 1
+            for (int k = 0; k < 4; ++k) {
+                const int c0 = 64 * k + 16 * cg;
+                tmem_ld16_issue(lane_base + O + (uint32_t)c0, v);
+                if (k < 3) {
+                    mbar_wait(hfull_bar(k), hph);
+                    const uint8_t* src = x_ptr + (size_t)k * MID_H_ROUND + (size_t)((2 * cg) * BM + r_in) * 16;
+#pragma unroll
+                    for (int i = 0; i < 2; ++i) {
+                        gh[i] = *reinterpret_cast<const uint4*>(src + i * (BM * 16));
+                        gl[i] = *reinterpret_cast<const uint4*>(src + 16384 + i * (BM * 16));
+                    }
+                    join16(gh, gl, aux);
+                } else {
+                    join16(lh, ll, aux);
+                }
+                tmem_ld_wait();
+#pragma unroll
+                for (int i = 0; i < 16; ++i) x[i] = __uint_as_float(v[i]) * sc * dcelu_from_h(aux[i], inv_alpha);
+                store_split16_tiled(x, d_hi + tile_in(c0), d_lo + tile_in(c0));
+            }
+            hph ^= 1u;
+            tc_fence_before();
+            // every epilogue warp has read its h1 out of X before any of them writes the next item's h1 into it
+            asm volatile("bar.sync 1, %0;" ::"n"(32 * MID_EPI_WARPS) : "memory");
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == MID_EPI_WARPS + 1) tmem_dealloc(tmem_base, TMEM_COLS);
+}
+
+// W1 images for k_mlp_fused: img[(s*M + e)][K step (64)][plane][8-column group (2)][n (256)][8], columns in the internal AEV order
+__global__ void k_prep_w1img(const float* __restrict__ blob, int n_models, __half* __restrict__ img) {
+    const int se = blockIdx.y;
+    const int s = se / n_models, e = se - s * n_models;
+    const float* net = blob + (size_t)(e * NSP + s) * NET_PARAMS;
+    const int total = (AEV_LD / 16) * FU_W1_STEP;
+    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += gridDim.x * blockDim.x) {
+        const int step = idx / FU_W1_STEP;
+        int rem = idx - step * FU_W1_STEP;
+        const int plane = rem / (16 * H1);
+        rem -= plane * 16 * H1;
+        const int g = rem / (8 * H1);
+        rem -= g * 8 * H1;
+        const int n = rem >> 3, c = 16 * step + 8 * g + (rem & 7);
+        const int k = col2feat(c);
+        const float v = k >= 0 ? net[OFF_W1 + (size_t)n * AEV_DIM + k] : 0.f;
+        __half hi, lo;
+        split_half(v * W_SCALE, hi, lo);
+        img[(size_t)se * total + idx] = plane ? lo : hi;
+    }
+}
+
 // weight images for k_mlp_mid: img[(s*M + e)][MID_W_TOTAL], see the layout above
 __global__ void k_prep_mid(const float* __restrict__ blob, int n_models, __half* __restrict__ img) {
     const int se = blockIdx.y;                      // s * n_models + e
@@ -1909,10 +2441,12 @@ struct TcWorkspace {                  // per context
     CUtensorMap m_aev;
     int* pair_sched;                               // [2][n_clusters + 1] item ranges of the pair kernels (G1, B1)
     int* pair_scratch;                             // [max_rows / 256 * MAX_MODELS] cost prefix scratch of k_pair_schedule
+    __half* fscratch;                              // [SMs][FU_SCRATCH] h1 scratch tiles of k_mlp_fused (L2-resident)
 };
 struct TcWeights {                    // per weight handle
     __half *w1f, *w2f, *w3f, *w3b, *w2b, *w1b;
     __half* wmid;                                   // k_mlp_mid weight images [species][network][MID_W_TOTAL]
+    __half* w1img;                                  // k_mlp_fused W1 images [species][network][64 K steps][FU_W1_STEP]
     float *b1, *b2, *b3, *w4, *b4;
     CUtensorMap m_w1f, m_w2f, m_w3f, m_w3b, m_w2b, m_w1b;
     CUtensorMap m_w1f_half, m_w1b_half;             // the pair kernels' boxes: 128 rows of W1 (G1), 32 rows of W1^T (B1)
@@ -1955,6 +2489,7 @@ int mlp_tc_alloc(Ctx* ctx) {
         return rc;
     DHP_CUDA(ctx, cudaFuncSetAttribute((k_gemm_pair<EPI_GRAD, CMP_N>), cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM_BYTES));
     DHP_CUDA(ctx, cudaFuncSetAttribute(k_mlp_mid, cudaFuncAttributeMaxDynamicSharedMemorySize, MID_SMEM));
+    DHP_CUDA(ctx, cudaFuncSetAttribute(k_mlp_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, FU_SMEM));
     DHP_CUDA(ctx, cudaFuncSetAttribute((k_gemm_tc2<EPI_CELU, CMP_K>), cudaFuncAttributeMaxDynamicSharedMemorySize, T2_SMEM));
     DHP_CUDA(ctx, cudaFuncSetAttribute((k_gemm_tc2<EPI_GRAD, CMP_N>), cudaFuncAttributeMaxDynamicSharedMemorySize, T2_SMEM));
     TcWorkspace* w = new (std::nothrow) TcWorkspace();
@@ -1967,6 +2502,8 @@ int mlp_tc_alloc(Ctx* ctx) {
     if (cudaMemset(w->aev, 0, 2 * R * AEV_LD * sizeof(__half)) != cudaSuccess) return DHP_E_CUDA;
     if (cudaMalloc((void**)&w->pair_sched, sizeof(int) * 2 * (ctx->sm_count / 2 + 1)) != cudaSuccess) return DHP_E_NOMEM;
     if (cudaMalloc((void**)&w->pair_scratch, sizeof(int) * (R / (2 * BM) * MAX_MODELS + 1)) != cudaSuccess) return DHP_E_NOMEM;
+    if (cudaMalloc((void**)&w->fscratch, (size_t)ctx->sm_count * FU_SCRATCH * sizeof(__half)) != cudaSuccess) return DHP_E_NOMEM;
+    if (cudaMemset(w->fscratch, 0, (size_t)ctx->sm_count * FU_SCRATCH * sizeof(__half)) != cudaSuccess) return DHP_E_CUDA;
     if (!make_map(&w->m_aev, w->aev, 2 * R, AEV_LD, BM)) return DHP_E_CUDA;
     ctx->aev_planes = w->aev;
     return DHP_OK;
@@ -2005,6 +2542,7 @@ void mlp_tc_free(Ctx* ctx) {
     for (__half* p : ptrs) if (p) cudaFree(p);
     if (w->pair_sched) cudaFree(w->pair_sched);
     if (w->pair_scratch) cudaFree(w->pair_scratch);
+    if (w->fscratch) cudaFree(w->fscratch);
     delete w;
     ctx->tc_ws = nullptr;
     ctx->aev_planes = nullptr;
@@ -2030,6 +2568,8 @@ int mlp_tc_weights(Ctx* ctx, Weights* wt) {
     if (!make_map(&t->m_w1b_half, t->w1b, (uint64_t)2 * NSP * AEV_LD, (uint64_t)M * H1, (uint32_t)(KBLK / 2))) return DHP_E_CUDA;
     if (cudaMalloc((void**)&t->wmid, (size_t)NSP * M * MID_W_TOTAL * sizeof(__half)) != cudaSuccess) return DHP_E_NOMEM;
     DHP_LAUNCH(ctx, k_prep_mid, dim3(64, NSP * M), 256, 0, wt->blob, M, t->wmid);
+    if (cudaMalloc((void**)&t->w1img, (size_t)NSP * M * (AEV_LD / 16) * FU_W1_STEP * sizeof(__half)) != cudaSuccess) return DHP_E_NOMEM;
+    DHP_LAUNCH(ctx, k_prep_w1img, dim3(128, NSP * M), 256, 0, wt->blob, M, t->w1img);
     float** smalls[] = {&t->b1, &t->b2, &t->b3, &t->w4, &t->b4};
     const size_t sizes[] = {(size_t)NSP * M * H1, (size_t)NSP * M * H2, (size_t)NSP * M * H3, (size_t)NSP * M * H3, (size_t)NSP * M};
     for (int i = 0; i < 5; ++i)
@@ -2043,7 +2583,7 @@ int mlp_tc_weights(Ctx* ctx, Weights* wt) {
 void mlp_tc_weights_free(Ctx*, Weights* wt) {
     TcWeights* t = (TcWeights*)wt->tc;
     if (!t) return;
-    void* ptrs[] = {t->w1f, t->w2f, t->w3f, t->w3b, t->w2b, t->w1b, t->wmid, t->b1, t->b2, t->b3, t->w4, t->b4};
+    void* ptrs[] = {t->w1f, t->w2f, t->w3f, t->w3b, t->w2b, t->w1b, t->wmid, t->w1img, t->b1, t->b2, t->b3, t->w4, t->b4};
     for (void* p : ptrs) if (p) cudaFree(p);
     delete t;
     wt->tc = nullptr;
@@ -2089,11 +2629,22 @@ int mlp_tc(Ctx* ctx, const Weights* wt, bool forward_only) {
     const bool big = n_pairs_bound * M >= 12 * (int64_t)ctx->sm_count;
     const bool two_g1 = fusedp && !pairs && ((ctx->tc_two & 1) != 0) && big;
     const bool two_b1 = fusedp && !pairs_b1 && ((ctx->tc_two & 2) != 0) && big;
-    if (two_g1) rc = launch_gemm2<EPI_CELU, CMP_K>(ctx, ws->m_aev, t->m_w1f, a);
+    // G1 fused into the front of the middle chain (k_mlp_fused): no G1 launch, h1 never becomes an HBM operand
+    const bool fuse1 = fusedp && ctx->tc_fuse != 0;
+    if (fuse1) rc = DHP_OK;
+    else if (two_g1) rc = launch_gemm2<EPI_CELU, CMP_K>(ctx, ws->m_aev, t->m_w1f, a);
     else rc = launch_gemm<EPI_CELU, CMP_K>(ctx, ws->m_aev, t->m_w1f, a);
     if (rc != DHP_OK) return rc;
     prof_mark(ctx, DHP_PHASE_MLP_MID);
-    if (ctx->mlp_mode != DHP_MLP_TENSOR_LAYERWISE) {
+    if (fuse1) {
+        FusedArgs m{};
+        m.single = a.single; m.forward_only = forward_only ? 1 : 0; m.n_models = M; m.plane_tiles = R / BM;
+        m.row_species = ctx->row_species; m.sp_start = ctx->sp_start; m.tile_mask = ctx->tile_mask;
+        m.aev = ws->aev; m.w1img = t->w1img; m.wimg = t->wmid; m.scratch = ws->fscratch; m.d1 = ws->d1;
+        m.b1 = t->b1; m.b2 = t->b2; m.b3 = t->b3; m.w4 = t->w4; m.b4 = t->b4;
+        m.inv_models = 1.0f / (float)M; m.alpha = ctx->params.celu_alpha; m.e_atom = ctx->e_atom; m.sched = ctx->tc_sched + 1;
+        DHP_LAUNCH(ctx, k_mlp_fused, ctx->sm_count, MID_THREADS, FU_SMEM, m);
+    } else if (ctx->mlp_mode != DHP_MLP_TENSOR_LAYERWISE) {
         // G2 .. B2 fused: h1 -> d1 with h2, d3, d2 kept on chip
         MidArgs m{};
         m.single = a.single;
