@@ -1249,6 +1249,12 @@ k_gemm_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
 #define MID_DBG 0      // timing experiments only: 1 = epilogues without work, 2 = no MMAs issued, 4 = no d1 stores, 8 = half the weight bytes
 #endif
 #define MID_WB(x) ((MID_DBG & 8) ? (x) / 2u : (x))
+#ifndef FU_BULK_H1
+#define FU_BULK_H1 0   // k_mlp_fused: h1 blocks 0..2 reach the scratch tile as bulk copies out of X (1) or as plain stores of the epilogue threads (0)
+#endif
+#ifndef FU_BULK_D1
+#define FU_BULK_D1 1   // k_mlp_fused: d1 blocks 0..2 are written over h1 in X and leave as bulk copies (1), or plain stores (0)
+#endif
 #ifndef MID_TRACE
 #define MID_TRACE 0    // timing experiments only: CTA 0 records clock64() per role for a few items and prints them at the end
 #endif
@@ -1833,19 +1839,18 @@ k_mlp_fused(const FusedArgs p) {
     const uint32_t bar0 = cst_s + 2 * FU_CONST_BYTES;
     uint64_t* bars = reinterpret_cast<uint64_t*>(x_ptr + MID_X_BYTES + FU_SLOTS * FU_SLOT_BYTES + 2 * FU_CONST_BYTES);
     // barriers: full[SLOTS], empty[SLOTS], then 17 single ones (below), sfull[RING], sempty[RING]; then the TMEM word and the item ring
-    constexpr int NB1 = 17;
+    constexpr int NB1 = 18;   // acc1, accp, accq, xr[4], xfree[3], hfull[3], cfull[2], cempty[2], hsaved
     constexpr int NBARS = 2 * FU_SLOTS + NB1 + 2 * RING;
     auto full_bar = [&](int s) { return bar0 + 8u * s; };
     auto empty_bar = [&](int s) { return bar0 + 8u * (FU_SLOTS + s); };
     const uint32_t b1s = bar0 + 8u * (2 * FU_SLOTS);
     const uint32_t acc1_bar = b1s, accp_bar = b1s + 8u, accq_bar = b1s + 16u;
     auto xr_bar = [&](int k) { return b1s + 24u + 8u * k; };            // k = 0..3: 64-column block k of an epilogue's output is ready
-    const uint32_t x0free_bar = b1s + 56u;                              // G2 has read h1 block 0: its place in X may take block 3
-    const uint32_t xfree_bar = b1s + 64u;                               // B2's MMAs have completed: X (d2) is dead
-    const uint32_t hsaved_bar = b1s + 72u;                              // the item's h1 is in the scratch tile (visible to the async proxy)
+    auto xfree_bar = [&](int k) { return b1s + 56u + 8u * k; };         // k = 0..2: B2 has read d2 block k: its place in X may take h1 block k back
     auto hfull_bar = [&](int k) { return b1s + 80u + 8u * k; };         // k = 0..2: h1 block k is back in X (for CELU'(z1))
     auto cfull_bar = [&](int b) { return b1s + 104u + 8u * b; };
     auto cempty_bar = [&](int b) { return b1s + 120u + 8u * b; };
+    const uint32_t hsaved_bar = b1s + 136u;                             // plain-store variant: the item's h1 is in the scratch tile, visible to the async proxy
     auto sfull_bar = [&](int s) { return bar0 + 8u * (2 * FU_SLOTS + NB1 + s); };
     auto sempty_bar = [&](int s) { return bar0 + 8u * (2 * FU_SLOTS + NB1 + RING + s); };
     volatile uint32_t* tmem_word = reinterpret_cast<volatile uint32_t*>(bars + NBARS);
@@ -1860,8 +1865,8 @@ k_mlp_fused(const FusedArgs p) {
         for (int s = 0; s < FU_SLOTS; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
         mbar_init(acc1_bar, 1); mbar_init(accp_bar, 1); mbar_init(accq_bar, 1);
         for (int k = 0; k < 4; ++k) mbar_init(xr_bar(k), MID_EPI_WARPS);
-        mbar_init(x0free_bar, 1); mbar_init(xfree_bar, 1); mbar_init(hsaved_bar, MID_EPI_WARPS);
-        for (int k = 0; k < 3; ++k) mbar_init(hfull_bar(k), 1);
+        for (int k = 0; k < 3; ++k) { mbar_init(xfree_bar(k), 1); mbar_init(hfull_bar(k), 1); }
+        mbar_init(hsaved_bar, MID_EPI_WARPS);
         for (int b = 0; b < 2; ++b) { mbar_init(cfull_bar(b), 1); mbar_init(cempty_bar(b), MID_EPI_WARPS); }
         for (int s = 0; s < RING; ++s) { mbar_init(sfull_bar(s), 1); mbar_init(sempty_bar(s), 1 + MID_EPI_WARPS); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -1887,16 +1892,17 @@ k_mlp_fused(const FusedArgs p) {
                 return slots + (uint32_t)slot * FU_SLOT_BYTES;
             };
             auto advance = [&]() { if (++slot == FU_SLOTS) { slot = 0; phase ^= 1u; } };
-            // h1 of the PREVIOUS item: scratch -> X once its B2 MMAs (the last readers of d2 in X) have completed; three 64-column
-            // blocks (hi plane then lo plane) for CELU'(z1) in B2's epilogue, the fourth comes by plain loads there
-            auto reload_h1 = [&]() {
-                mbar_wait(hsaved_bar, hphase);
-                mbar_wait(xfree_bar, hphase); hphase ^= 1u;
-                for (int k = 0; k < 3; ++k) {
-                    mbar_expect_tx(hfull_bar(k), (uint32_t)MID_H_ROUND);
-                    bulk_load(xs + (uint32_t)(k * MID_H_ROUND), scratch + (size_t)k * (BM * BK), 16384u, hfull_bar(k));
-                    bulk_load(xs + (uint32_t)(k * MID_H_ROUND) + 16384u, scratch + (size_t)(4 + k) * (BM * BK), 16384u, hfull_bar(k));
-                }
+            // h1 of the PREVIOUS item: scratch -> X, block k as soon as that item's B2 has read d2 block k out of X (its K steps 4 k ..
+            // 4 k + 3 have completed); three 64-column blocks (hi plane then lo plane) for CELU'(z1) in B2's epilogue, the fourth comes
+            // by plain loads there.  The ring paces this thread by B2's progress (a G1 slot frees when a B2 step retires), so block 0
+            // can go before the first G1 slot, block 1 after it and block 2 once the ring has been refilled: none of the waits blocks
+            auto reload_h1 = [&](int k) {
+                if (!FU_BULK_H1 && k == 0) mbar_wait(hsaved_bar, hphase);
+                mbar_wait(xfree_bar(k), hphase);
+                mbar_expect_tx(hfull_bar(k), (uint32_t)MID_H_ROUND);
+                // (block k goes where d2's block k was: hi plane at 16 k KB, lo plane 48 KB further - nothing B2 still reads)
+                bulk_load(xs + (uint32_t)k * 16384u, scratch + (size_t)k * (BM * BK), 16384u, hfull_bar(k));
+                bulk_load(xs + (uint32_t)MID_X_PLANE + (uint32_t)k * 16384u, scratch + (size_t)(4 + k) * (BM * BK), 16384u, hfull_bar(k));
             };
             for (;;) {
                 int item = atomicAdd(p.sched, 1);
@@ -1923,14 +1929,14 @@ k_mlp_fused(const FusedArgs p) {
                 }
                 // G1: the K steps of the active feature blocks.  The ring refills while the previous item's B2 runs; once it is
                 // full, wait for that B2 and bring the previous item's h1 back for its epilogue
-                bool reloaded = !have_prev || p.forward_only;
+                int next_reload = (!have_prev || p.forward_only) ? 3 : 0;
                 int issued = 0;
                 for (unsigned km = g1_mask(rt); km; km &= km - 1u) {
                     const int kb = __ffs(km) - 1;
                     const __half* a_hi = p.aev + tile_off(p.plane_tiles, N_KBLK, 0, rt, kb);
                     const __half* a_lo = p.aev + tile_off(p.plane_tiles, N_KBLK, 1, rt, kb);
                     for (int ks = 0; ks < 4; ++ks) {
-                        if (issued == FU_SLOTS && !reloaded) { reload_h1(); reloaded = true; }
+                        if (next_reload < 3 && (issued == 0 || issued == 1 || issued == FU_SLOTS)) reload_h1(next_reload++);
                         const uint32_t sa = next_slot();
                         mbar_expect_tx(full_bar(slot), (uint32_t)FU_SLOT_BYTES);
                         bulk_load(sa, w1 + (size_t)(kb * 4 + ks) * FU_W1_STEP, 16384u, full_bar(slot));
@@ -1940,7 +1946,8 @@ k_mlp_fused(const FusedArgs p) {
                         ++issued;
                     }
                 }
-                if (!reloaded) reload_h1();
+                while (next_reload < 3) reload_h1(next_reload++);
+                if (have_prev && !p.forward_only) hphase ^= 1u;
                 for (int j = 0; j < H1 / 32; ++j) {                       // G2: W2 K steps 2j, 2j+1 (A = h1 in X)
                     const uint32_t sa = next_slot();
                     mbar_expect_tx(full_bar(slot), 64u * H2 * 2u);
@@ -1968,7 +1975,7 @@ k_mlp_fused(const FusedArgs p) {
                     advance();
                 }
             }
-            if (have_prev && !p.forward_only) reload_h1();               // the last item of this CTA
+            if (have_prev && !p.forward_only) for (int k = 0; k < 3; ++k) reload_h1(k);   // the last item of this CTA
         }
     } else if (warp == MID_EPI_WARPS + 1) {
         // ===== MMA issuer =====
@@ -2007,10 +2014,13 @@ k_mlp_fused(const FusedArgs p) {
                 if (item < 0) break;
                 const int rt = item / M;
                 const uint32_t O = (nit & 1) ? 256u : 0u;
-                ++nit;
+                TR(0, nit, 0);
                 {   // G1: AEV W1^T -> z1 at [O, O + 256)
                     const uint32_t idesc = make_idesc(H1);
                     const int nsteps = 4 * __popc(g1_mask(rt));
+#if MID_TRACE
+                    if (blockIdx.x == 0 && nit >= 8 && nit < 16) g_tr[2][nit - 8][0] = nsteps;
+#endif
                     uint32_t accumulate = 0u;
                     for (int j = 0; j < nsteps; ++j) {
                         const uint32_t sa = wait_slot();
@@ -2021,26 +2031,41 @@ k_mlp_fused(const FusedArgs p) {
                     }
                     umma_commit(acc1_bar);
                 }
-                {   // G2: h1 W2^T -> [O + 256, O + 448); h1 block kb is K steps 4 kb .. 4 kb + 3, block 3 sits in block 0's place
+                TR(0, nit, 1);
+                {   // G2: h1 W2^T -> [O + 256, O + 448); h1 block kb is K steps 4 kb .. 4 kb + 3: blocks 0..2 in X, block 3 in tensor memory
                     const uint32_t idesc = make_idesc(H2), lbo = H2 * 16u, d = tmem_base + (O ^ 256u);
                     uint32_t accumulate = 0u;
                     for (int sl = 0; sl < H1 / 32; ++sl) {
-                        if ((sl & 1) == 0) wait_xr(sl >> 1);
+                        if ((sl & 1) == 0) {
+                            const int kb = sl >> 1;
+                            wait_xr(kb);
+                            if (FU_BULK_H1 && kb < 3 && !p.forward_only) {      // h1 block kb (every epilogue warp has fenced its part) -> scratch tile
+                                bulk_store(scratch + (size_t)kb * (BM * BK), xs + (uint32_t)kb * 16384u, 16384u);
+                                bulk_store(scratch + (size_t)(4 + kb) * (BM * BK), xs + (uint32_t)MID_X_PLANE + (uint32_t)kb * 16384u, 16384u);
+                                bulk_commit();
+                            }
+                        }
                         const uint32_t sa = wait_slot();
 #pragma unroll
                         for (int t = 0; t < 2; ++t) {
                             const int j = 2 * sl + t;
                             const uint32_t sb = sa + (uint32_t)t * 4u * lbo;
-                            const uint32_t a0 = xs + (uint32_t)((2 * j) % 24) * 2048u;
-                            mma3(d, make_desc_ns(a0, 2048u), make_desc_ns(a0 + (uint32_t)MID_X_PLANE, 2048u), make_desc_ns(sb, lbo),
-                                 make_desc_ns(sb + 2u * lbo, lbo), idesc, accumulate);
+                            if (j < 12) {
+                                const uint32_t a0 = xs + (uint32_t)j * 4096u;
+                                mma3(d, make_desc_ns(a0, 2048u), make_desc_ns(a0 + (uint32_t)MID_X_PLANE, 2048u), make_desc_ns(sb, lbo),
+                                     make_desc_ns(sb + 2u * lbo, lbo), idesc, accumulate);
+                            } else {                                      // block 3 of h1 is in tensor memory: hi [O + 448, + 32), lo [O + 480, + 32)
+                                const uint32_t a_hi = tmem_base + ((O + 448u + 8u * (uint32_t)(j - 12)) & 511u);
+                                mma3_ts(d, a_hi, a_hi + 32u, make_desc_ns(sb, lbo), make_desc_ns(sb + 2u * lbo, lbo), idesc, accumulate);
+                            }
                             accumulate = 1u;
                         }
                         release_slot();
-                        if (sl == 1) umma_commit(x0free_bar);
                     }
+                    if (FU_BULK_H1) bulk_wait_all();                      // blocks 0..2 have left X (G2's epilogue overwrites them) and are in the scratch tile
                     umma_commit(accp_bar);
                 }
+                TR(0, nit, 2);
                 {   // G3: h2 W3^T -> [O, O + 160)
                     const uint32_t idesc = make_idesc(H3), lbo = H3 * 16u, d = tmem_base + O;
                     uint32_t accumulate = 0u;
@@ -2060,7 +2085,8 @@ k_mlp_fused(const FusedArgs p) {
                     }
                     umma_commit(accq_bar);
                 }
-                if (p.forward_only) continue;
+                TR(0, nit, 3);
+                if (p.forward_only) { ++nit; continue; }
                 {   // B3: d3 W3 -> [O + 320, O + 512); A = d3 in tensor memory, K step j at hi (O + 160 + 8 j), lo (O + 240 + 8 j) mod 512
                     const uint32_t idesc = make_idesc(H2), lbo = H2 * 16u, d = tmem_base + ((O + 320u) & 511u);
                     uint32_t accumulate = 0u;
@@ -2079,6 +2105,7 @@ k_mlp_fused(const FusedArgs p) {
                     }
                     umma_commit(accp_bar);
                 }
+                TR(0, nit, 4);
                 {   // B2: d2 W2 -> [O, O + 256); one K step per slot
                     const uint32_t idesc = make_idesc(H1), lbo = H1 * 16u, d = tmem_base + O;
                     uint32_t accumulate = 0u;
@@ -2090,10 +2117,12 @@ k_mlp_fused(const FusedArgs p) {
                              make_desc_ns(sa + 2u * lbo, lbo), idesc, accumulate);
                         accumulate = 1u;
                         release_slot();
+                        if ((j & 3) == 3) umma_commit(xfree_bar(j >> 2)); // d2 block j / 4 has been read: its place is free for the h1 reload (producer)
                     }
                     umma_commit(accq_bar);
-                    umma_commit(xfree_bar);                               // ... and X is free for the h1 reload (producer)
                 }
+                TR(0, nit, 5);
+                ++nit;
             }
         }
     } else {
@@ -2103,7 +2132,7 @@ k_mlp_fused(const FusedArgs p) {
         const int r_in = q * 32 + lane;
         const uint32_t lane_base = tmem_base + ((uint32_t)(q * 32) << 16);
         int rs = 0; uint32_t rphase = 0;
-        uint32_t a1phase = 0, pphase = 0, qphase = 0, hph = 0, x0ph = 0;
+        uint32_t a1phase = 0, pphase = 0, qphase = 0, hph = 0;
         int cb = 0; uint32_t cphase = 0;
         int nit = 0;
         const float kexp = 1.4426950408889634f / p.alpha, inv_alpha = 1.0f / p.alpha;
@@ -2140,28 +2169,45 @@ k_mlp_fused(const FusedArgs p) {
             const int row = rt * BM + r_in;
             const int se = s * M + e;
             const uint32_t O = (nit & 1) ? 256u : 0u;
-            ++nit;
+            const bool trw = warp == 0 && lane == 0; (void)trw;
             uint32_t v[16];
             float x[16], aux[16];
             mbar_wait(cfull_bar(cb), cphase);
             const float* cst = cst_ptr + cb * FU_CONST_FLOATS;
             // ---- G1 (z1): h1 = CELU(acc / 64 + b1) -> X (A of G2) and, for CELU'(z1) later, the scratch tile
+            if (trw) TR(1, nit, 0);
             mbar_wait(acc1_bar, a1phase); a1phase ^= 1u;
             tc_fence_after();
+            if (trw) TR(1, nit, 1);
 #pragma unroll 1
             for (int k = 0; k < 4; ++k) {
                 const int c0 = 64 * k + 16 * cg;
                 tmem_ld16_issue(lane_base + O + (uint32_t)c0, v);
                 lds16(cst + c0, aux);
-                if (k == 3) { mbar_wait(x0free_bar, x0ph); x0ph ^= 1u; }      // G2 is done with block 0: block 3 takes its place
                 tmem_ld_wait();
 #pragma unroll
                 for (int i = 0; i < 16; ++i) x[i] = celu_f(fmaf(__uint_as_float(v[i]), sc, aux[i]), p.alpha, kexp);
-                store_split16_x(x, x_ptr, k < 3 ? c0 : c0 - 192, r_in);
-                if (!p.forward_only) store_split16_tiled(x, scratch + tile_in(c0), scratch + (size_t)4 * (BM * BK) + tile_in(c0));
-                signal_x(k);
+                if (k < 3) {
+                    store_split16_x(x, x_ptr, c0, r_in);
+                    signal_x(k);
+                    if (!FU_BULK_H1 && !p.forward_only) {      // ... and to the scratch tile, after the signal: G2 does not wait for these stores
+                        store_split16_tiled(x, scratch + tile_in(c0), scratch + (size_t)4 * (BM * BK) + tile_in(c0));
+                    }
+                } else {                     // X holds three blocks: the fourth is G2's A operand from tensor memory (the 64 columns no accumulator uses)
+                    uint32_t ph[8], pl[8];
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) split_pair(x[2 * i], x[2 * i + 1], ph[i], pl[i]);   // K even -> low half
+                    tmem_st8(lane_base + ((O + 448u + 8u * (uint32_t)cg) & 511u), ph);
+                    tmem_st8(lane_base + ((O + 480u + 8u * (uint32_t)cg) & 511u), pl);
+                    tmem_st_wait();
+                    signal_t(k);
+                }
+                // blocks 0..2 go to the scratch tile as bulk copies out of X (MMA issuer); block 3, which B2's epilogue reads back with
+                // plain loads, is stored by the thread that will read it
+                if (k == 3 && !p.forward_only) store_split16_tiled(x, scratch + tile_in(c0), scratch + (size_t)4 * (BM * BK) + tile_in(c0));
+                if (trw) TR(1, nit, 2 + k);
             }
-            if (!p.forward_only) {           // the scratch stores of this warp are ordered before the producer's bulk reads
+            if (!FU_BULK_H1 && !p.forward_only) {       // this warp's scratch stores are ordered before the producer's bulk reads
                 fence_proxy_async_all();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(hsaved_bar);
@@ -2169,6 +2215,7 @@ k_mlp_fused(const FusedArgs p) {
             // ---- G2: h2 = CELU(acc / 64 + b2) -> X, block by block
             mbar_wait(accp_bar, pphase); pphase ^= 1u;
             tc_fence_after();
+            if (trw) TR(1, nit, 6);
 #pragma unroll 1
             for (int k = 0; k < 3; ++k) {
                 const int c0 = 64 * k + 16 * cg;
@@ -2179,11 +2226,13 @@ k_mlp_fused(const FusedArgs p) {
                 for (int i = 0; i < 16; ++i) x[i] = celu_f(fmaf(__uint_as_float(v[i]), sc, aux[i]), p.alpha, kexp);
                 store_split16_x(x, x_ptr, c0, r_in);
                 signal_x(k);
+                if (trw) TR(1, nit, 7 + k);
             }
             // ---- G3: h3 = CELU(acc / 64 + b3); E_i += (w4.h3 + b4)/M; d3 = w4 CELU'(z3) 2^10 / M -> tensor memory (A of B3)
             float w4v[16];
             mbar_wait(accq_bar, qphase); qphase ^= 1u;
             tc_fence_after();
+            if (trw) TR(1, nit, 10);
             float e_acc = 0.f;
             const float dsc = p.inv_models * D_SCALE;
 #pragma unroll 1
@@ -2210,15 +2259,17 @@ k_mlp_fused(const FusedArgs p) {
                     }
                 }
                 if (!p.forward_only) signal_t(k);
+                if (trw) TR(1, nit, 11 + k);
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(cempty_bar(cb));
             if (++cb == 2) { cb = 0; cphase ^= 1u; }
             atomicAdd(&p.e_atom[row], (e_acc + (cg == 0 ? p.b4[se] : 0.f)) * p.inv_models);
-            if (p.forward_only) { tc_fence_before(); continue; }
+            if (p.forward_only) { tc_fence_before(); ++nit; continue; }
             // ---- B3: d2 = (acc / 64) CELU'(z2), CELU' from this thread's own h2 in X, d2 written over it
             mbar_wait(accp_bar, pphase); pphase ^= 1u;
             tc_fence_after();
+            if (trw) TR(1, nit, 14);
 #pragma unroll 1
             for (int k = 0; k < 3; ++k) {
                 const int c0 = 64 * k + 16 * cg;
@@ -2236,6 +2287,7 @@ k_mlp_fused(const FusedArgs p) {
                 for (int i = 0; i < 16; ++i) x[i] = __uint_as_float(v[i]) * sc * dcelu_from_h(aux[i], inv_alpha);
                 store_split16_x(x, x_ptr, c0, r_in);
                 signal_x(k);
+                if (trw) TR(1, nit, 15 + k);
             }
             // ---- B2: d1 = (acc / 64) CELU'(z1) -> global (tiled planes).  h1 blocks 0..2 come back into X by bulk copy (producer),
             //      block 3 by plain loads of what this very thread stored (issued here, their latency runs under the first rounds)
@@ -2251,6 +2303,7 @@ k_mlp_fused(const FusedArgs p) {
             }
             mbar_wait(accq_bar, qphase); qphase ^= 1u;
             tc_fence_after();
+            if (trw) TR(1, nit, 18);
             __half* d_hi = p.d1 + tile_off(p.plane_tiles, M * 4, 0, rt, e * 4);
             __half* d_lo = p.d1 + tile_off(p.plane_tiles, M * 4, 1, rt, e * 4);
 #pragma unroll 1
@@ -2259,11 +2312,11 @@ k_mlp_fused(const FusedArgs p) {
                 tmem_ld16_issue(lane_base + O + (uint32_t)c0, v);
                 if (k < 3) {
                     mbar_wait(hfull_bar(k), hph);
-                    const uint8_t* src = x_ptr + (size_t)k * MID_H_ROUND + (size_t)((2 * cg) * BM + r_in) * 16;
+                    const uint8_t* src = x_ptr + (size_t)k * 16384 + (size_t)((2 * cg) * BM + r_in) * 16;
 #pragma unroll
                     for (int i = 0; i < 2; ++i) {
                         gh[i] = *reinterpret_cast<const uint4*>(src + i * (BM * 16));
-                        gl[i] = *reinterpret_cast<const uint4*>(src + 16384 + i * (BM * 16));
+                        gl[i] = *reinterpret_cast<const uint4*>(src + MID_X_PLANE + i * (BM * 16));
                     }
                     join16(gh, gl, aux);
                 } else {
@@ -2272,17 +2325,55 @@ k_mlp_fused(const FusedArgs p) {
                 tmem_ld_wait();
 #pragma unroll
                 for (int i = 0; i < 16; ++i) x[i] = __uint_as_float(v[i]) * sc * dcelu_from_h(aux[i], inv_alpha);
-                store_split16_tiled(x, d_hi + tile_in(c0), d_lo + tile_in(c0));
+                if (FU_BULK_D1 && k < 3) {
+                    // d1 over this thread's own h1 in X (already the global tiled layout of the block), then the block leaves as two
+                    // bulk copies: 3/4 of d1 never passes through the LSU store path
+                    uint8_t* dst = x_ptr + (size_t)k * 16384 + (size_t)((2 * cg) * BM + r_in) * 16;
+                    uint32_t ph[8], pl[8];
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) split_pair(x[2 * i], x[2 * i + 1], ph[i], pl[i]);
+#pragma unroll
+                    for (int i = 0; i < 2; ++i) {
+                        *reinterpret_cast<uint4*>(dst + i * (BM * 16)) = make_uint4(ph[4 * i], ph[4 * i + 1], ph[4 * i + 2], ph[4 * i + 3]);
+                        *reinterpret_cast<uint4*>(dst + MID_X_PLANE + i * (BM * 16)) = make_uint4(pl[4 * i], pl[4 * i + 1], pl[4 * i + 2], pl[4 * i + 3]);
+                    }
+                    fence_proxy_async_smem();
+                    asm volatile("bar.sync 2, %0;" ::"n"(32 * MID_EPI_WARPS) : "memory");
+                    if (warp == 0 && lane == 0) {
+                        bulk_store(d_hi + (size_t)k * (BM * BK), xs + (uint32_t)k * 16384u, 16384u);
+                        bulk_store(d_lo + (size_t)k * (BM * BK), xs + (uint32_t)MID_X_PLANE + (uint32_t)k * 16384u, 16384u);
+                        bulk_commit();
+                    }
+                } else {
+                    store_split16_tiled(x, d_hi + tile_in(c0), d_lo + tile_in(c0));
+                }
+                if (trw) TR(1, nit, 19 + k);
             }
             hph ^= 1u;
+            if (FU_BULK_D1 && warp == 0 && lane == 0) bulk_wait_read<0>();       // d1's blocks have left X
             tc_fence_before();
             // every epilogue warp has read its h1 out of X before any of them writes the next item's h1 into it
             asm volatile("bar.sync 1, %0;" ::"n"(32 * MID_EPI_WARPS) : "memory");
+            if (trw) TR(1, nit, 23);
+            ++nit;
         }
     }
+    if (threadIdx.x == 0) bulk_wait_all();
     tc_fence_before();
     __syncthreads();
     if (warp == MID_EPI_WARPS + 1) tmem_dealloc(tmem_base, TMEM_COLS);
+#if MID_TRACE
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        const long long t0 = g_tr[0][0][0];
+        for (int it = 0; it < 8; ++it) {
+            printf("FMMA item %d (%lld G1 steps):", it, g_tr[2][it][0]);
+            for (int e = 0; e < 6; ++e) printf(" %lld", g_tr[0][it][e] - t0);
+            printf("\nFEPI item %d:", it);
+            for (int e = 0; e < 24; ++e) printf(" %lld", g_tr[1][it][e] - t0);
+            printf("\n");
+        }
+    }
+#endif
 }
 
 // W1 images for k_mlp_fused: img[(s*M + e)][K step (64)][plane][8-column group (2)][n (256)][8], columns in the internal AEV order
