@@ -26,6 +26,13 @@ __device__ __forceinline__ float fast_log2(float x) { float y; asm("lg2.approx.f
 __device__ __forceinline__ float fast_sqrt(float x) { float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float fast_rcp(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
+// Blackwell's packed fp32 pipe: one FFMA2 does two fp32 FMAs (the AEV kernels are bound by instruction issue, not by a pipe).
+// A pair is a 64-bit register; when both halves of an operand are the same value ptxas uses the scalar-broadcast form.
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float a, float b) { f32x2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
+__device__ __forceinline__ void unpack2(f32x2 v, float& a, float& b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+
 struct NbrGeom {
     float ux, uy, uz, R;
     int sp;
@@ -65,7 +72,10 @@ __device__ __forceinline__ float dfcut(float R, float inv_rc, float pi_over_rc) 
 //                       pair ends, then stored once to the row buffer (no read-modify-write, no atomics).
 // Output: PLANES = false, full fp32 rows (SIMT MLP path); PLANES = true, the two-term fp16 split of the
 // feature blocks that are active for the row's tile (what G1 reads), written straight into the tensor path's planes.
-constexpr int AEV_WARPS = 8;
+#ifndef FWD_W
+#define FWD_W 8
+#endif
+constexpr int AEV_WARPS = FWD_W;
 constexpr int MAX_RAD = DHP_MAX_RAD;    // radial neighbours staged per centre (= the pair list's per-row capacity)
 
 // internal pair p = hi (hi + 1) / 2 + lo over priority positions -> species(lo) | species(hi) << 4 (prio_sp(), dhp_internal.cuh);
@@ -101,7 +111,7 @@ __device__ __forceinline__ void put_feature(float v, float* __restrict__ row_f32
 }
 
 template <bool PLANES, int NAg, int NZg>     // NAg x NZg: the angular grid of Eq. 5, 8 x 4 (ANI-2x shape) or 4 x 8 (ANI-1x shape)
-__global__ void __launch_bounds__(AEV_WARPS * 32, 5)
+__global__ void __launch_bounds__(AEV_WARPS * 32, 40 / AEV_WARPS)
 k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, const int* __restrict__ col,
           const unsigned short* __restrict__ seg_cnt, const int* __restrict__ rowmap, const unsigned* __restrict__ tile_mask,
           const Grid* __restrict__ gp, const __grid_constant__ AevConst K, int n, float* __restrict__ aev,
@@ -307,9 +317,12 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
 //                indices, so there are no atomics and no read-modify-write in shared memory.
 //   scatter      one global atomic triple per neighbour and one for the centre.
 // -------------------------------------------------------------------------------------------------
-constexpr int BWD_WARPS = 8;
+#ifndef BWD_W
+#define BWD_W 8
+#endif
+constexpr int BWD_WARPS = BWD_W;
 #ifndef BWD_MINB
-#define BWD_MINB 4
+#define BWD_MINB (32 / BWD_W)
 #endif
 
 constexpr int OWN = 3;   // neighbour slots per lane that can be angular (MAX_ANG = 96 = 3 x 32)
@@ -443,6 +456,10 @@ k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
     // ---- angular (Eq. 5) -----------------------------------------------------------------------------------
     const int npairs = na * (na - 1) / 2;
     const float inv_na = na > 0 ? fast_rcp((float)na) : 0.f;
+    // distance of the round's first and last slot, carried from round to round (T0 = d0 na + r0; an integer division per round
+    // was 6 % of the kernel's instructions)
+    int d0 = 0, r0 = 32 * sw;
+    while (na > 0 && r0 >= na) { r0 -= na; ++d0; }
     for (int T0 = 32 * sw; T0 < npairs; T0 += 32 * NWARP) {
         const int t = T0 + lane;
         if (t < npairs) {
@@ -458,29 +475,37 @@ k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
             const float sn = fast_sqrt(cx * cx + cy * cy + cz * cz);
             const float Rm = 0.5f * (qj.w + qk.w);
             const float4* gb = reinterpret_cast<const float4*>(grow + 32 * ipair(S.sp[j], S.sp[k]));
-            float Az[NZg], dAz[NZg];
+            f32x2 AdA[NZg];                                                        // (A_z, dA_z/dtheta) as packed pairs
 #pragma unroll
             for (int z = 0; z < NZg; ++z) {
                 const float u = fmaxf(fmaf(0.5f * K.sin_z[z], sn, fmaf(0.5f * K.cos_z[z], c, 0.5f)), 0.f);
                 const float wz = fast_exp2((K.zeta - 1.0f) * fast_log2(u));       // u^(zeta-1)
-                Az[z] = 2.0f * u * wz;                                             // A = 2 u^zeta
-                dAz[z] = -K.zeta * wz * (sn * K.cos_z[z] - c * K.sin_z[z]);        // dA/dtheta
+                AdA[z] = pack2(2.0f * u * wz,                                      // A = 2 u^zeta
+                               -K.zeta * wz * (sn * K.cos_z[z] - c * K.sin_z[z])); // dA/dtheta
             }
-            float S0 = 0.f, Sm = 0.f, St = 0.f;
+            f32x2 S0t = pack2(0.f, 0.f);                                           // (S0, St)
+            float Sm = 0.f;
 #pragma unroll
             for (int a = 0; a < NAg; ++a) {
                 const float mm = Rm - K.shf_a[a];
                 const float B = fast_exp2(-K.eta_a_l2e * mm * mm);
                 const float dB = -K.eta_a * mm * B;                                // dB/dR_ij = dB/dR_ik
-                float ua = 0.f, va = 0.f;                                          // entries (a, z) of the pair block: [a][z]
+                f32x2 uv = pack2(0.f, 0.f);                                        // (ua, va) over the entries (a, z) of the pair block: [a][z]
 #pragma unroll
                 for (int z4 = 0; z4 < NZg / 4; ++z4) {
                     const float4 g4 = __ldg(gb + a * (NZg / 4) + z4);
-                    ua += g4.x * Az[4 * z4] + g4.y * Az[4 * z4 + 1] + g4.z * Az[4 * z4 + 2] + g4.w * Az[4 * z4 + 3];
-                    va += g4.x * dAz[4 * z4] + g4.y * dAz[4 * z4 + 1] + g4.z * dAz[4 * z4 + 2] + g4.w * dAz[4 * z4 + 3];
+                    uv = fma2(pack2(g4.x, g4.x), AdA[4 * z4], uv);
+                    uv = fma2(pack2(g4.y, g4.y), AdA[4 * z4 + 1], uv);
+                    uv = fma2(pack2(g4.z, g4.z), AdA[4 * z4 + 2], uv);
+                    uv = fma2(pack2(g4.w, g4.w), AdA[4 * z4 + 3], uv);
                 }
-                S0 = fmaf(B, ua, S0); Sm = fmaf(dB, ua, Sm); St = fmaf(B, va, St);
+                S0t = fma2(pack2(B, B), uv, S0t);
+                float ua, va;
+                unpack2(uv, ua, va);
+                Sm = fmaf(dB, ua, Sm);
             }
+            float S0, St;
+            unpack2(S0t, S0, St);
             const float dth = St * fj.x * fk.x;                                    // sum g dT/dtheta
             const float dRj = (Sm * fj.x + S0 * fj.y) * fk.x;                      // sum g dT/dR_ij
             const float dRk = (Sm * fk.x + S0 * fk.y) * fj.x;
@@ -497,7 +522,9 @@ k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
         __syncwarp();
         // gather: neighbour nn is j of slot d na + nn and k of slot d na + (nn - d - 1 mod na), for every d in the round
         const int cntr = min(32, npairs - T0);
-        const int d_lo = T0 / na, d_hi = (T0 + cntr - 1) / na;
+        const int d_lo = d0;
+        int d_hi = d0, rl = r0 + cntr - 1;
+        while (rl >= na) { rl -= na; ++d_hi; }
 #pragma unroll
         for (int q = 0; q < OWN; ++q) {
             const int nn = lane + 32 * q;
@@ -512,6 +539,8 @@ k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
                 }
             }
         }
+        r0 += 32 * NWARP;
+        while (r0 >= na) { r0 -= na; ++d0; }
         __syncwarp();
     }
 

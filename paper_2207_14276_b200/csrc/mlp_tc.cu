@@ -222,6 +222,16 @@ __device__ __forceinline__ float celu_f(float v, float alpha, float k) {
 // CELU'(z) from h = CELU(z): 1 for h > 0, h / alpha + 1 (<= 1) otherwise
 __device__ __forceinline__ float dcelu_from_h(float h, float inv_alpha) { return fminf(fmaf(h, inv_alpha, 1.0f), 1.0f); }
 
+// Blackwell's packed fp32 instructions (FFMA2 / FMUL2 / FADD2: two fp32 results per issue slot); the epilogues are bound by
+// instruction issue (4 epilogue warps per scheduler, ~175 instructions per 16 columns), and rounding is that of the scalar forms
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float a, float b) { f32x2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
+__device__ __forceinline__ void unpack2(f32x2 v, float& a, float& b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+
 // two floats -> packed fp16 pair, round-to-nearest, saturating to the largest finite fp16 (first argument -> low half)
 __device__ __forceinline__ uint32_t cvt_pack(float lo_half, float hi_half) {
     uint32_t r;
@@ -232,7 +242,9 @@ __device__ __forceinline__ uint32_t cvt_pack(float lo_half, float hi_half) {
 __device__ __forceinline__ void split_pair(float x0, float x1, uint32_t& hi, uint32_t& lo) {
     hi = cvt_pack(x0, x1);
     const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&hi));
-    lo = cvt_pack(x0 - f.x, x1 - f.y);
+    float d0, d1;
+    unpack2(sub2(pack2(x0, x1), pack2(f.x, f.y)), d0, d1);
+    lo = cvt_pack(d0, d1);
 }
 __device__ __forceinline__ void split_half(float x, __half& hi, __half& lo) {
     x = fminf(fmaxf(x, -65000.f), 65000.f);
@@ -247,8 +259,30 @@ __device__ __forceinline__ uint32_t pack_half2(__half a, __half b) {
 __device__ __forceinline__ void unpack_add(uint32_t h, uint32_t l, float& a, float& b) {
     const float2 fh = __half22float2(*reinterpret_cast<__half2*>(&h));
     const float2 fl = __half22float2(*reinterpret_cast<__half2*>(&l));
-    a = fh.x + fl.x;
-    b = fh.y + fl.y;
+    unpack2(add2(pack2(fh.x, fh.y), pack2(fl.x, fl.y)), a, b);
+}
+// 16 accumulator columns -> CELU(acc * sc + bias): the multiply-adds as packed pairs (same roundings as celu_f)
+__device__ __forceinline__ void celu16(const uint32_t (&v)[16], const float (&b)[16], float sc, float alpha, float kexp, float (&x)[16]) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const f32x2 z = fma2(pack2(__uint_as_float(v[2 * i]), __uint_as_float(v[2 * i + 1])), pack2(sc, sc), pack2(b[2 * i], b[2 * i + 1]));
+        float t0, t1, z0, z1, e0, e1;
+        unpack2(mul2(z, pack2(kexp, kexp)), t0, t1);
+        unpack2(fma2(pack2(fast_ex2(t0), fast_ex2(t1)), pack2(alpha, alpha), pack2(-alpha, -alpha)), e0, e1);
+        unpack2(z, z0, z1);
+        x[2 * i] = fmaxf(z0, fminf(e0, 0.f));
+        x[2 * i + 1] = fmaxf(z1, fminf(e1, 0.f));
+    }
+}
+// 16 accumulator columns -> (acc * sc) * CELU'(z) with CELU' recovered from the stored activation h (dcelu_from_h)
+__device__ __forceinline__ void dcelu16(const uint32_t (&v)[16], const float (&h)[16], float sc, float inv_alpha, float (&x)[16]) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        float g0, g1;
+        unpack2(fma2(pack2(h[2 * i], h[2 * i + 1]), pack2(inv_alpha, inv_alpha), pack2(1.0f, 1.0f)), g0, g1);
+        const f32x2 a = mul2(pack2(__uint_as_float(v[2 * i]), __uint_as_float(v[2 * i + 1])), pack2(sc, sc));
+        unpack2(mul2(a, pack2(fminf(g0, 1.0f), fminf(g1, 1.0f))), x[2 * i], x[2 * i + 1]);
+    }
 }
 // tiled activation layout: element offset of (row tile rt, 64-column block kb) and, inside it, of (8-column group g, row r)
 __device__ __forceinline__ size_t tile_off(int plane_tiles, int kblocks, int plane, int rt, int kb) {
@@ -2185,8 +2219,7 @@ k_mlp_fused(const FusedArgs p) {
                 tmem_ld16_issue(lane_base + O + (uint32_t)c0, v);
                 lds16(cst + c0, aux);
                 tmem_ld_wait();
-#pragma unroll
-                for (int i = 0; i < 16; ++i) x[i] = celu_f(fmaf(__uint_as_float(v[i]), sc, aux[i]), p.alpha, kexp);
+                celu16(v, aux, sc, p.alpha, kexp, x);
                 if (k < 3) {
                     store_split16_x(x, x_ptr, c0, r_in);
                     signal_x(k);
@@ -2222,8 +2255,7 @@ k_mlp_fused(const FusedArgs p) {
                 tmem_ld16_issue(lane_base + (O ^ 256u) + (uint32_t)c0, v);
                 lds16(cst + H1 + c0, aux);
                 tmem_ld_wait();
-#pragma unroll
-                for (int i = 0; i < 16; ++i) x[i] = celu_f(fmaf(__uint_as_float(v[i]), sc, aux[i]), p.alpha, kexp);
+                celu16(v, aux, sc, p.alpha, kexp, x);
                 store_split16_x(x, x_ptr, c0, r_in);
                 signal_x(k);
                 if (trw) TR(1, nit, 7 + k);
@@ -2243,11 +2275,15 @@ k_mlp_fused(const FusedArgs p) {
                     lds16(cst + H1 + H2 + c0, aux);
                     lds16(cst + H1 + H2 + H3 + c0, w4v);
                     tmem_ld_wait();
+                    float h3[16];
+                    celu16(v, aux, sc, p.alpha, kexp, h3);
 #pragma unroll
-                    for (int i = 0; i < 16; ++i) {
-                        const float h = celu_f(fmaf(__uint_as_float(v[i]), sc, aux[i]), p.alpha, kexp);
-                        e_acc = fmaf(w4v[i], h, e_acc);
-                        x[i] = w4v[i] * dsc * dcelu_from_h(h, inv_alpha);
+                    for (int i = 0; i < 8; ++i) {
+                        float g0, g1;
+                        e_acc = fmaf(w4v[2 * i], h3[2 * i], e_acc);
+                        e_acc = fmaf(w4v[2 * i + 1], h3[2 * i + 1], e_acc);
+                        unpack2(fma2(pack2(h3[2 * i], h3[2 * i + 1]), pack2(inv_alpha, inv_alpha), pack2(1.0f, 1.0f)), g0, g1);
+                        unpack2(mul2(mul2(pack2(w4v[2 * i], w4v[2 * i + 1]), pack2(dsc, dsc)), pack2(fminf(g0, 1.0f), fminf(g1, 1.0f))), x[2 * i], x[2 * i + 1]);
                     }
                     if (!p.forward_only) {
                         uint32_t ph[8], pl[8];
@@ -2283,8 +2319,7 @@ k_mlp_fused(const FusedArgs p) {
                 }
                 join16(hh, hl, aux);
                 tmem_ld_wait();
-#pragma unroll
-                for (int i = 0; i < 16; ++i) x[i] = __uint_as_float(v[i]) * sc * dcelu_from_h(aux[i], inv_alpha);
+                dcelu16(v, aux, sc, inv_alpha, x);
                 store_split16_x(x, x_ptr, c0, r_in);
                 signal_x(k);
                 if (trw) TR(1, nit, 15 + k);
@@ -2323,8 +2358,7 @@ k_mlp_fused(const FusedArgs p) {
                     join16(lh, ll, aux);
                 }
                 tmem_ld_wait();
-#pragma unroll
-                for (int i = 0; i < 16; ++i) x[i] = __uint_as_float(v[i]) * sc * dcelu_from_h(aux[i], inv_alpha);
+                dcelu16(v, aux, sc, inv_alpha, x);
                 if (FU_BULK_D1 && k < 3) {
                     // d1 over this thread's own h1 in X (already the global tiled layout of the block), then the block leaves as two
                     // bulk copies: 3/4 of d1 never passes through the LSU store path
