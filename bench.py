@@ -9,7 +9,7 @@ configs[3], the 98 000-atom biosystem the north_star targets are quoted on.  Pri
 
   value   atoms*evals/s, inputs resident in HBM, CUDA events over exactly K steps, max over ranks
   e2e     same metric through dhp_ani_energy_forces_host: pinned host buffers, H2D + D2H inside
-  roofline  the dominant kernel (k_mlp_mid, tensor-bound): algorithmic FLOPs / device time of the timed (burst) loop vs the
+  roofline  the dominant kernel (k_mlp_fused, tensor-bound): algorithmic FLOPs / device time of the timed (burst) loop vs the
             measured BURST bf16 peak; `frac` counts a product once, `issued_frac` the 3 MMAs issued per product
   roofline_mlp_phase / roofline_kernels   the same for the whole MLP phase and for every kernel group (HBM-bound ones vs copy bandwidth)
   cpu_baseline  the fp64 oracle, as it stands, on a bounded sample of the same workload (rank 0, N=1)
@@ -483,7 +483,15 @@ def main():
         tr = traffic_98k() if (args.config == 4 and tensor_path) else {}
         scale_n = N / 98000.0
         kernels = []
-        if tensor_path:
+        # default: G1 runs inside the fused chain kernel (k_mlp_fused; DHP_TC_FUSE=0 keeps G1 and k_mlp_mid as two launches)
+        fused_g1 = tensor_path and os.environ.get("DHP_TC_FUSE", "1") != "0" and args.mlp != "simt"
+        n_mlp_kernels = 2 if fused_g1 else 3
+        if tensor_path and fused_g1:
+            kernels += [tensor_entry("k_mlp_fused (G1+G2+G3+out+B3+B2 in one kernel: AEV planes -> E_i, d1)", ph["mlp_g1"] + ph["mlp_mid"],
+                                     (f_g1 + f_mid) * M * N, i_g1 + i_mid, tr.get("fused"), (f_g1_dense + f_mid) * M * N),
+                        tensor_entry("k_gemm_tc2<GRAD,N-skip> (B1: d1 -> dE/dAEV) + energy reduction", ph["mlp_b1"], f_g1 * M * N, i_g1, tr.get("b1"),
+                                     f_g1_dense * M * N)]
+        elif tensor_path:
             kernels += [tensor_entry("k_gemm_tc<CELU,K-skip> (G1: AEV -> h1)", ph["mlp_g1"], f_g1 * M * N, i_g1, tr.get("g1"), f_g1_dense * M * N),
                         tensor_entry("k_mlp_mid (G2+G3+out+B3+B2 fused: h1 -> E_i, d1)", ph["mlp_mid"], f_mid * M * N, i_mid, tr.get("mid")),
                         tensor_entry("k_gemm_tc<GRAD,N-skip> (B1: d1 -> dE/dAEV) + energy reduction", ph["mlp_b1"], f_g1 * M * N, i_g1, tr.get("b1"),
@@ -495,18 +503,22 @@ def main():
                     hbm_entry("k_aev_fwd (a2)", ph["aev_fwd"], 4256.0, tr.get("aev_fwd"), "issue-bound; the floor that binds is MUFU, not HBM", 69.0 * scale_n),
                     hbm_entry("k_aev_bwd + k_unsort_forces (a5)", ph["aev_bwd"], 4268.0, tr.get("aev_bwd"), "issue-bound", 140.0 * scale_n)]
         if tensor_path:
-            roof = dict(max(kernels[:3], key=lambda k: k["ms_per_launch"]))          # the dominant kernel of the step
+            roof = dict(max(kernels[:n_mlp_kernels], key=lambda k: k["ms_per_launch"]))          # the dominant kernel of the step
             roof["peak_source"] = f"{pk['source']} {peak_kind} bf16 peak (fp16 operands, same rate); the timed loop is a burst"
             roof["arithmetic"] = ("fp16 operands, 1 tcgen05 MMA per product, fp32 accumulate (opt-in mixed precision, outside the parity bar)"
                                   if args.mlp == "fp16" else "fp16 two-term split, 3 tcgen05 MMAs per product, fp32 accumulate: `frac` counts one "
                                   "product once (ceiling 1/3), `issued_frac` counts the MMAs issued")
-            tsum = (tr["g1"] + tr["mid"] + tr["b1"]) if {"g1", "mid", "b1"} <= set(tr) else None
-            mlp_phase = tensor_entry("MLP phase (G1 + k_mlp_mid + B1)", ph["mlp"], (2 * f_g1 + f_mid) * M * N, 2 * i_g1 + i_mid, tsum,
+            if fused_g1:
+                tsum = (tr["fused"] + tr["b1"]) if {"fused", "b1"} <= set(tr) else None
+            else:
+                tsum = (tr["g1"] + tr["mid"] + tr["b1"]) if {"g1", "mid", "b1"} <= set(tr) else None
+            mlp_phase = tensor_entry("MLP phase (k_mlp_fused + B1)" if fused_g1 else "MLP phase (G1 + k_mlp_mid + B1)", ph["mlp"], (2 * f_g1 + f_mid) * M * N, 2 * i_g1 + i_mid, tsum,
                                      (2 * f_g1_dense + f_mid) * M * N)
             mlp_phase.update({"row_tiles": n_row_tiles, "active_feature_blocks_per_tile": act})
             if sustained is not None and sustained.get("phase_ms"):
                 sp = sustained["phase_ms"]
-                sustained["roofline"] = tensor_entry(roof["kernel"], sp["mlp_mid"] if "k_mlp_mid" in roof["kernel"] else sp["mlp_g1"],
+                sustained["roofline"] = tensor_entry(roof["kernel"], sp["mlp_g1"] + sp["mlp_mid"] if "k_mlp_fused" in roof["kernel"] else
+                                                     sp["mlp_mid"] if "k_mlp_mid" in roof["kernel"] else sp["mlp_b1"] if "B1" in roof["kernel"] else sp["mlp_g1"],
                                                      roof["algorithmic_flop_per_launch"],
                                                      roof["issued_tflops"] * roof["ms_per_launch"] * 1e9, roof["traffic"],
                                                      peak=pk["bf16_tflops_sustained"], kind="sustained")
