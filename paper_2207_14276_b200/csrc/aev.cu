@@ -98,17 +98,22 @@ struct __align__(16) WarpSmemFwd {
 };
 
 // one feature value of this lane -> the row, either fp32 or as the two-term fp16 split in the hi / lo planes
-// (planes: tiled operand layout, aev_tiled_off(); row_hi points at (row, column 0) of the hi plane, so a column adds
-//  its 64-column block, its 8-column group and its position in the group)
+// Planes (tiled operand layout, aev_tiled_off()): `row_hi` points at (row, column 0) of the hi plane and `lane_off` is the lane's
+// fixed part of the offset, so that a 32-column angular block blk costs one shift (its 64-column block and 8-column group
+// fold into blk * 4096 halves) and a 16-column radial slot q one more (14 * 8192 + q * 2048).  AEV entries are sums of at
+// most MAX_ANG^2 / 2 terms of at most 2: far inside the fp16 range, no clamp.
 template <bool PLANES>
-__device__ __forceinline__ void put_feature(float v, float* __restrict__ row_f32, __half* __restrict__ row_hi,
-                                            size_t plane_stride, int colidx) {
+__device__ __forceinline__ void put_value(float v, float* __restrict__ row_f32, __half* __restrict__ row_hi, size_t plane_stride,
+                                          int colidx, int tiled) {
     if (!PLANES) { row_f32[colidx] = v; return; }
-    const __half hi = __float2half_rn(fminf(fmaxf(v, -65000.f), 65000.f));
-    const int o = (colidx >> 6) * (ROW_TILE * KBLK) + ((colidx & 63) >> 3) * (ROW_TILE * 8) + (colidx & 7);
-    row_hi[o] = hi;
-    row_hi[plane_stride + o] = __float2half_rn(v - __half2float(hi));
+    const __half hi = __float2half_rn(v);
+    row_hi[tiled] = hi;
+    row_hi[plane_stride + tiled] = __float2half_rn(v - __half2float(hi));
 }
+// angular block blk, column 32 blk + lane; lane_off = (lane >> 3) * 1024 + (lane & 7)
+#define PUT_ANG(v, blk) put_value<PLANES>(v, row_f32, row_hi, plane_stride, 32 * (blk) + lane, ((blk) << 12) + lane_off)
+// radial slot q (priority order), column AEV_ANG + 16 q + lane for lane < 16
+#define PUT_RAD(v, q) put_value<PLANES>(v, row_f32, row_hi, plane_stride, AEV_ANG + 16 * (q) + lane, 14 * (ROW_TILE * KBLK) + ((q) << 11) + lane_off)
 
 template <bool PLANES, int NAg, int NZg>     // NAg x NZg: the angular grid of Eq. 5, 8 x 4 (ANI-2x shape) or 4 x 8 (ANI-1x shape)
 __global__ void __launch_bounds__(AEV_WARPS * 32, 40 / AEV_WARPS)
@@ -154,6 +159,7 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
     if (row < 0) return;                               // not a central atom of this call (partial evaluation)
     float* row_f32 = aev + (size_t)row * AEV_LD;
     __half* row_hi = planes + aev_tiled_off(row, 0);
+    const int lane_off = (lane >> 3) * (ROW_TILE * 8) + (lane & 7);
 
     // ---- stage all neighbours -------------------------------------------------------------------------
     for (int a = lane; a < nst; a += 32) {
@@ -206,7 +212,7 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
                 acc = fmaf(fast_exp2(-K.eta_r_l2e * dr * dr), q.y, acc);
             }
             acc += __shfl_xor_sync(FULL, acc, 16);
-            if (lane < 16) put_feature<PLANES>(acc, row_f32, row_hi, plane_stride, rad_col(s) + m);
+            if (lane < 16) PUT_RAD(acc, (rad_col(s) - AEV_ANG) >> 4);
         }
     }
 
@@ -276,7 +282,7 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
             facc = fmaf(a4.z, b4.z, facc); facc = fmaf(a4.w, b4.w, facc);
             if ((endmask >> (4 * qd + 3)) & 1u) {             // pair complete: its 32 features go out, 64 (128) contiguous bytes
                 const int blk = __shfl_sync(FULL, my_blk, 4 * qd + 3);
-                put_feature<PLANES>(facc, row_f32, row_hi, plane_stride, 32 * blk + lane);
+                PUT_ANG(facc, blk);
                 facc = 0.f;
             }
         }
@@ -290,7 +296,7 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
     if (PLANES) { mask = tile_mask[row / ROW_TILE]; if (mask == 0) mask = 1u << 14; }   // G1 runs one zero block for an all-zero tile
     // lane p < 28: angular block p is read (its 64-wide block is active) but this atom has no such pair
     unsigned zm = __ballot_sync(FULL, lane < NPAIR && ((mask >> (lane >> 1)) & 1u) && !((nz_pairs >> lane) & 1u));
-    for (; zm; zm &= zm - 1u) put_feature<PLANES>(0.f, row_f32, row_hi, plane_stride, 32 * (__ffs(zm) - 1) + lane);
+    for (; zm; zm &= zm - 1u) PUT_ANG(0.f, __ffs(zm) - 1);
     // lane q < 8: radial slot q (priority order; slot 7 is the 16 padding columns) likewise
     bool rz = false;
     if (lane < 8) {
@@ -303,7 +309,7 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
     }
     unsigned rm = __ballot_sync(FULL, rz);
     for (; rm; rm &= rm - 1u)
-        if (lane < 16) put_feature<PLANES>(0.f, row_f32, row_hi, plane_stride, AEV_ANG + 16 * (__ffs(rm) - 1) + lane);
+        if (lane < 16) PUT_RAD(0.f, __ffs(rm) - 1);
 }
 
 // -------------------------------------------------------------------------------------------------
