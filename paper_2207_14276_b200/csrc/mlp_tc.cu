@@ -2561,7 +2561,8 @@ bool make_map(CUtensorMap* m, const void* ptr, uint64_t rows, uint64_t cols, uin
 struct TcWorkspace {                  // per context
     __half* aev;                                   // [2][max_rows][AEV_LD] row-major hi / lo planes (A of G1, via TMA)
     __half *h1, *h2, *d3, *d2, *d1;                // tiled activation planes (see the header); d3 is padded to 192 per model
-    int act_models;                                // h1 / d1 hold this many networks per row (grown by mlp_tc_ensure)
+    int act_models;                                // d1 holds this many networks per row (grown by mlp_tc_ensure)
+    int h1_models;                                 // h1 likewise (allocated only where it is an HBM operand); 0 = not allocated
     int lw_models;                                 // h2 / d3 / d2 (layer-by-layer mode only) likewise; 0 = not allocated
     CUtensorMap m_aev;
     int* pair_sched;                               // [2][n_clusters + 1] item ranges of the pair kernels (G1, B1)
@@ -2649,8 +2650,14 @@ int mlp_tc_ensure(Ctx* ctx, int n_models, bool layerwise) {
     };
     int rc;
     if (n_models > w->act_models) {
-        if ((rc = grow(&w->h1, (size_t)n_models * H1)) != DHP_OK || (rc = grow(&w->d1, (size_t)n_models * H1)) != DHP_OK) { w->act_models = 0; return rc; }
+        if ((rc = grow(&w->d1, (size_t)n_models * H1)) != DHP_OK) { w->act_models = 0; return rc; }
         w->act_models = n_models;
+    }
+    // h1 is an HBM operand only on the two-launch path (DHP_TC_FUSE=0) and in the layer-by-layer mode: the fused chain kernel
+    // keeps it on chip (8 KB per row and 8 networks less: 0.8 GB at 98 000 atoms)
+    if ((!ctx->tc_fuse || layerwise) && n_models > w->h1_models) {
+        if ((rc = grow(&w->h1, (size_t)n_models * H1)) != DHP_OK) { w->h1_models = 0; return rc; }
+        w->h1_models = n_models;
     }
     if (layerwise && n_models > w->lw_models) {
         if ((rc = grow(&w->h2, (size_t)n_models * H2)) != DHP_OK || (rc = grow(&w->d3, (size_t)n_models * H2)) != DHP_OK ||
@@ -2723,6 +2730,7 @@ int mlp_tc(Ctx* ctx, const Weights* wt, bool forward_only) {
     const int R = (int)ctx->max_rows;
     int rc;
     if (M > ws->act_models || (ctx->mlp_mode == DHP_MLP_TENSOR_LAYERWISE && M > ws->lw_models)) return DHP_E_NOTIMPL;   // mlp_tc_ensure not run
+    if ((!ctx->tc_fuse || ctx->mlp_mode == DHP_MLP_TENSOR_LAYERWISE) && M > ws->h1_models) return DHP_E_NOTIMPL;
     // e_atom and the tile schedulers were zeroed with the rest of the per-call arena at the start of the call (nlist_build)
     if (!ctx->aev_in_planes)     // rows came from a forward pass in fp32 (debug / mixed use): split them here
         DHP_LAUNCH(ctx, k_split_rows, 4 * ctx->sm_count, 256, 0, ctx->aev, AEV_LD, ctx->sp_start, AEV_LD, ws->aev, R);
