@@ -133,10 +133,12 @@ static void graphs_invalidate(Ctx* ctx) {
     }
 }
 
-// The hot call.  Large systems: enqueue the kernels.  Small systems (n <= SMALL_N: the solute of the hybrid scheme, PAPER.md
-// L112-118, L200-208 - the call RESPA's outer step makes): the same enqueue is captured ONCE per argument set into a CUDA
-// graph on the library's own stream and replayed on the caller's stream afterwards - same kernels, same arithmetic, no
-// per-launch host work and no gaps between a dozen dependent 15-40 us launches.  A changed pointer, size, box or mode is a
+// The hot call.  The enqueue of the kernels is captured ONCE per argument set into a CUDA graph on the library's own stream and
+// replayed on the caller's stream afterwards - same kernels, same arithmetic, no per-launch host work and no gaps between
+// dependent launches.  It matters most for small systems (n <= SMALL_N: the solute of the hybrid scheme, PAPER.md L112-118,
+// L200-208 - the call RESPA's outer step makes: a dozen dependent 15-40 us launches); above SMALL_N it saves the ~1 % of the step
+// that the nine short list kernels spend waiting for their launches, and switches itself off for a caller whose argument
+// sets never repeat.  A changed pointer, size, box or mode is a
 // new graph (4 are kept, least recently used first out).
 static int run_energy_forces(Ctx* ctx, const float* pos, const float* box, const int32_t* species, int64_t n,
                              const int32_t* mol_offsets, int64_t n_mol, const Weights* w, double* E, float* F,
@@ -145,7 +147,8 @@ static int run_energy_forces(Ctx* ctx, const float* pos, const float* box, const
         const bool tensor = ctx->mlp_mode >= DHP_MLP_TENSOR || (ctx->mlp_mode == DHP_MLP_AUTO && w->tc != nullptr);
         if (!tensor) { const int rc = mlp_simt_ensure(ctx, w->n_models); if (rc != DHP_OK) return rc; }
     }
-    const bool small = ctx->graph_on && n > 0 && n <= SMALL_N && !(ctx->skin > 0.f) && !ctx->prof.on;
+    const bool large = n > SMALL_N;
+    const bool small = ctx->graph_on && n > 0 && (!large || ctx->graph_large) && !(ctx->skin > 0.f) && !ctx->prof.on;
     if (!small) return enqueue_energy_forces(ctx, pos, box, species, n, mol_offsets, n_mol, w, E, F, central);
     float bx[4] = {0.f, 0.f, 0.f, box ? 1.f : 0.f};
     if (box) for (int c = 0; c < 3; ++c) bx[c] = box[c];
@@ -155,6 +158,13 @@ static int run_energy_forces(Ctx* ctx, const float* pos, const float* box, const
         if (g.used && g.pos == pos && g.species == species && g.mol == mol_offsets && g.central == central && g.weights == w && g.E == E &&
             g.F == F && g.n == n && g.n_mol == n_mol && g.mlp_mode == ctx->mlp_mode && memcmp(g.box, bx, sizeof(bx)) == 0) { hit = &g; break; }
         if (!g.used || (victim->used && g.stamp < victim->stamp)) victim = &g;
+    }
+    if (large) {                                      // a caller whose arguments change every call (a new box per step) gains nothing
+        if (hit) ctx->gl_hit++;
+        else if (++ctx->gl_miss > 16 && ctx->gl_miss > ctx->gl_hit) {
+            ctx->graph_large = false;
+            return enqueue_energy_forces(ctx, pos, box, species, n, mol_offsets, n_mol, w, E, F, central);
+        }
     }
     if (!hit) {
         if (victim->used && victim->exec) cudaGraphExecDestroy(victim->exec);
@@ -266,6 +276,7 @@ int dhp_create(dhp_ctx** out, const dhp_params* params, int64_t max_atoms, int64
     c->sm_count = prop.multiProcessorCount;
     { const char* e = getenv("DHP_NO_SMALL_PATH"); c->no_small_path = e && e[0] == '1'; }
     { const char* e = getenv("DHP_NO_GRAPH"); c->graph_on = !(e && e[0] == '1'); }
+    { const char* e = getenv("DHP_GRAPH_ALL"); c->graph_large = !(e && e[0] == '0'); c->gl_miss = c->gl_hit = 0; }
     if (c->graph_on && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); c->graph_on = false; c->cap_stream = nullptr; }
     { const char* e = getenv("DHP_TC_FUSE"); c->tc_fuse = (e && e[0] == '0') ? 0 : 1; }
     { const char* e = getenv("DHP_TC_PAIRS"); c->tc_pairs = (e && e[0] >= '0' && e[0] <= '3') ? e[0] - '0' : 0; }   // cta_group::2 kernels

@@ -126,6 +126,8 @@ struct Ctx {
     GraphEntry graphs[N_GRAPHS];
     uint64_t graph_clock;
     int64_t graph_replays;
+    bool graph_large;      // systems above SMALL_N replay too (DHP_GRAPH_ALL=0 turns it off); switched off by itself when the argument
+    int64_t gl_miss, gl_hit;   // sets keep changing (a new box every step): more captures than replays
     char cuda_err[256];
     Profile prof;
 

@@ -541,6 +541,43 @@ def test_small_systems_replay_a_captured_graph(torch, B, params, blob8, name):
     d.close()
 
 
+def test_graph_replay_of_a_large_system_and_its_switch_off_under_changing_arguments(torch, B, params, blob8):
+    """Systems above the small-system limit are replayed too (the cell-list path's 17 kernels as one graph).  Replays must
+    give the oracle's answer for the current buffer contents; a caller whose argument set changes every call (here: the box)
+    makes the library fall back to plain enqueues by itself - results unchanged either way."""
+    s = SYSTEMS["mix600"]()
+    blob = blob8[: s.n_models * 7 * W.PARAMS_PER_NET]
+    d = make_ctx(B, s, params)
+    w = d.dhp_weights_load(blob, s.n_models)
+    pos, sp, mol = B.to_device(s)
+    E = torch.empty(1, dtype=torch.float64, device="cuda")
+    F = torch.empty((s.n_atoms, 3), dtype=torch.float32, device="cuda")
+    rng = np.random.default_rng(11)
+    q = s.pos.copy()
+    r0 = d.dhp_graph_replays()
+    for it in range(3):
+        pos.copy_(torch.from_numpy(q).cuda())
+        d.dhp_ani_energy_forces(pos, s.box, sp, w, mol, E=E, F=F)
+        torch.cuda.synchronize()
+        assert d.dhp_status() == 0
+        Eo, Fo = oracle.total_energy_forces(W.System(s.name, q, s.species, s.box, s.mol_offsets, s.n_models), params, blob)
+        assert abs(E.item() - Eo[0]) / s.n_atoms <= E_TOL_PER_ATOM and np.max(np.abs(F.cpu().numpy() - Fo)) <= F_TOL
+        q = (q.astype(np.float64) + rng.normal(0, 0.02, q.shape)).astype(np.float32)
+    assert d.dhp_graph_replays() - r0 == 3
+    # a new box on every call: a new graph each time, until the library stops capturing
+    r1 = d.dhp_graph_replays()
+    box = np.array(s.box, dtype=np.float64)
+    for it in range(40):
+        b = (box * (1.0 + 1e-4 * (it + 1))).astype(np.float32)
+        d.dhp_ani_energy_forces(pos, b, sp, w, mol, E=E, F=F)
+    torch.cuda.synchronize()
+    assert d.dhp_status() == 0
+    assert d.dhp_graph_replays() - r1 < 40                    # it gave up replaying
+    Eo, Fo = oracle.total_energy_forces(W.System(s.name, pos.cpu().numpy(), s.species, b, s.mol_offsets, s.n_models), params, blob)
+    assert abs(E.item() - Eo[0]) / s.n_atoms <= E_TOL_PER_ATOM and np.max(np.abs(F.cpu().numpy() - Fo)) <= F_TOL
+    d.close()
+
+
 def test_graph_replay_can_be_switched_off(torch, B, params, blob8, monkeypatch):
     monkeypatch.setenv("DHP_NO_GRAPH", "1")
     s = SYSTEMS["ligand50"]()
