@@ -14,9 +14,13 @@
 // so that the 32 lanes of a warp write (and, for CELU', read back) 512 contiguous bytes per instruction, and the
 // next GEMM fetches its A operand as one contiguous 16 KB cp.async.bulk per plane and K block (descriptor:
 // SWIZZLE_NONE, leading byte offset 2048 = next 8-column group, stride byte offset 128 = next 8 rows).
-// AEV rows (A of G1) and all weights (B) stay row-major and come in through TMA tensor maps with SWIZZLE_128B.
+// The AEV planes (A of G1) are written in the same tiled layout by the AEV kernel (aev_tiled_off()); the weights (B) of
+// k_gemm_tc / k_gemm_tc2 / k_gemm_pair stay row-major and come in through TMA tensor maps with SWIZZLE_128B, those of the
+// chain kernels (k_mlp_fused, k_mlp_mid) are pre-tiled images fetched with plain bulk copies.
 //
-// One persistent, warp-specialised kernel template does all six GEMMs of the path:
+// Default path (two launches): k_mlp_fused = G1 + G2 + G3 + output layer + B3 + B2 for one (row tile, network) per work item,
+// every intermediate on chip (further down), then B1 = k_gemm_tc2.  The persistent, warp-specialised template below runs any
+// one of the six GEMMs as its own launch: B1, the two-launch path (DHP_TC_FUSE=0: G1, then k_mlp_mid), the layer-by-layer mode:
 //   warps 0..7  epilogue       (tcgen05.ld 32x32b -> bias / CELU / CELU' / split -> global), overlapped with the
 //                               next tile's MMAs through two TMEM accumulator stages (2 x 256 columns)
 //   warp 8      TMA producer   (cp.async.bulk.tensor.2d, SWIZZLE_128B, 64-wide K blocks, mbarrier ring)
