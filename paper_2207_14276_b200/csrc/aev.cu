@@ -32,6 +32,8 @@ typedef unsigned long long f32x2;
 __device__ __forceinline__ f32x2 pack2(float a, float b) { f32x2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
 __device__ __forceinline__ void unpack2(f32x2 v, float& a, float& b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
 __device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 
 struct NbrGeom {
     float ux, uy, uz, R;
@@ -196,23 +198,41 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
     }
     __syncwarp();
 
-    // ---- radial (Eq. 4): lane = (shift m, parity h), one register sum per neighbour species ----------------
+    // ---- radial (Eq. 4): lane = (shift pair m2, neighbour phase h); the two Gaussians of a lane as one packed fp32 pair,
+    //      one register sum per neighbour species; the 16 sums of a species leave as 8 packed stores per plane -------------
     {
-        const int m = lane & 15, h = lane >> 4;
-        const float shf = K.shf_r[m];
+        const int m2 = lane & 7, h = lane >> 3;
+        const f32x2 nshf = pack2(-K.shf_r[2 * m2], -K.shf_r[2 * m2 + 1]);
+        const f32x2 neta = pack2(-K.eta_r_l2e, -K.eta_r_l2e);
         for (int s = 0; s < NSP; ++s) {
             const int ca = __shfl_sync(FULL, cnt, s), sa = __shfl_sync(FULL, start, s);
             const int cr = __shfl_sync(FULL, cnt, 8 + s), sr = __shfl_sync(FULL, start, 8 + s) - ca;
             if (ca + cr == 0) continue;
-            float acc = 0.f;
+            f32x2 acc = pack2(0.f, 0.f);
 #pragma unroll 2
-            for (int x = h; x < ca + cr; x += 2) {
+            for (int x = h; x < ca + cr; x += 4) {
                 const float2 q = S.rr[x < ca ? sa + x : sr + x];
-                const float dr = q.x - shf;
-                acc = fmaf(fast_exp2(-K.eta_r_l2e * dr * dr), q.y, acc);
+                const f32x2 dr = add2(pack2(q.x, q.x), nshf);
+                float a0, a1;
+                unpack2(mul2(mul2(dr, neta), dr), a0, a1);
+                acc = fma2(pack2(fast_exp2(a0), fast_exp2(a1)), pack2(q.y, q.y), acc);
             }
-            acc += __shfl_xor_sync(FULL, acc, 16);
-            if (lane < 16) PUT_RAD(acc, (rad_col(s) - AEV_ANG) >> 4);
+            float v0, v1;
+            unpack2(acc, v0, v1);
+            v0 += __shfl_xor_sync(FULL, v0, 8);  v1 += __shfl_xor_sync(FULL, v1, 8);
+            v0 += __shfl_xor_sync(FULL, v0, 16); v1 += __shfl_xor_sync(FULL, v1, 16);
+            if (lane < 8) {
+                const int q = (rad_col(s) - AEV_ANG) >> 4;                 // radial slot (priority order), columns AEV_ANG + 16 q + 2 m2, + 1
+                if (!PLANES) {
+                    *reinterpret_cast<float2*>(row_f32 + AEV_ANG + 16 * q + 2 * m2) = make_float2(v0, v1);
+                } else {
+                    const int o = 14 * (ROW_TILE * KBLK) + (q << 11) + (m2 >> 2) * (ROW_TILE * 8) + 2 * (m2 & 3);
+                    const __half2 hi = __floats2half2_rn(v0, v1);
+                    const float2 hf = __half22float2(hi);
+                    *reinterpret_cast<__half2*>(row_hi + o) = hi;
+                    *reinterpret_cast<__half2*>(row_hi + plane_stride + o) = __floats2half2_rn(v0 - hf.x, v1 - hf.y);
+                }
+            }
         }
     }
 
