@@ -74,6 +74,9 @@ __device__ __forceinline__ float dfcut(float R, float inv_rc, float pi_over_rc) 
 //                       pair ends, then stored once to the row buffer (no read-modify-write, no atomics).
 // Output: PLANES = false, full fp32 rows (SIMT MLP path); PLANES = true, the two-term fp16 split of the
 // feature blocks that are active for the row's tile (what G1 reads), written straight into the tensor path's planes.
+#ifndef AEV_ABL
+#define AEV_ABL 0      // timing experiments only (wrong results): 1 = no radial loop, 2 = no phase-2 accumulation, 4 = no MUFU in the angular factors
+#endif
 #ifndef FWD_W
 #define FWD_W 8
 #endif
@@ -210,7 +213,7 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
             if (ca + cr == 0) continue;
             f32x2 acc = pack2(0.f, 0.f);
 #pragma unroll 2
-            for (int x = h; x < ca + cr; x += 4) {
+            for (int x = h; x < ((AEV_ABL & 1) ? 0 : ca + cr); x += 4) {
                 const float2 q = S.rr[x < ca ? sa + x : sr + x];
                 const f32x2 dr = add2(pack2(q.x, q.x), nshf);
                 float a0, a1;
@@ -277,12 +280,12 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
 #pragma unroll
                 for (int z = 0; z < NZg; ++z) {
                     const float uu = fmaxf(fmaf(0.5f * K.sin_z[z], sn, fmaf(0.5f * K.cos_z[z], c, 0.5f)), 0.f);
-                    A[z] = f2 * fast_exp2(K.zeta * fast_log2(uu));    // 2 ((1+cos(theta-theta_z))/2)^zeta f_j f_k
+                    A[z] = (AEV_ABL & 4) ? f2 * uu : f2 * fast_exp2(K.zeta * fast_log2(uu));    // 2 ((1+cos(theta-theta_z))/2)^zeta f_j f_k
                 }
 #pragma unroll
                 for (int a = 0; a < NAg; ++a) {
                     const float mm = Rm - K.shf_a[a];
-                    B[a] = fast_exp2(-K.eta_a_l2e * mm * mm);
+                    B[a] = (AEV_ABL & 4) ? mm : fast_exp2(-K.eta_a_l2e * mm * mm);
                 }
             }
         }
@@ -295,7 +298,7 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
         // the branch is warp-uniform
         const unsigned endmask = __ballot_sync(FULL, my_end);
 #pragma unroll
-        for (int qd = 0; qd < 8; ++qd) {
+        for (int qd = 0; qd < ((AEV_ABL & 2) ? 0 : 8); ++qd) {
             const float4 a4 = *reinterpret_cast<const float4*>(&S.st[za][4 * qd]);
             const float4 b4 = *reinterpret_cast<const float4*>(&S.st[NZg + aa][4 * qd]);
             facc = fmaf(a4.x, b4.x, facc); facc = fmaf(a4.y, b4.y, facc);
