@@ -75,7 +75,8 @@ __device__ __forceinline__ float dfcut(float R, float inv_rc, float pi_over_rc) 
 // Output: PLANES = false, full fp32 rows (SIMT MLP path); PLANES = true, the two-term fp16 split of the
 // feature blocks that are active for the row's tile (what G1 reads), written straight into the tensor path's planes.
 #ifndef AEV_ABL
-#define AEV_ABL 0      // timing experiments only (wrong results): 1 = no radial loop, 2 = no phase-2 accumulation, 4 = no MUFU in the angular factors
+#define AEV_ABL 0      // timing experiments only (wrong results): 1 = no radial loop, 2 = no phase-2 accumulation, 4 = no MUFU in the angular factors;
+                       // backward: 16 = no radial derivative, 32 = no contraction with the dE/dG block, 64 = no gather, 128 = no angular rounds
 #endif
 #ifndef FWD_W
 #define FWD_W 8
@@ -455,7 +456,7 @@ k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
             const float4* gr = reinterpret_cast<const float4*>(&S.g_rad[NR * nbq.sp]);
             float coef = 0.f;
 #pragma unroll
-            for (int m4 = 0; m4 < NR / 4; ++m4) {
+            for (int m4 = 0; m4 < ((AEV_ABL & 16) ? 0 : NR / 4); ++m4) {
                 const float4 g4 = gr[m4];
                 const float gm[4] = {g4.x, g4.y, g4.z, g4.w};
 #pragma unroll
@@ -489,7 +490,7 @@ k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
     // was 6 % of the kernel's instructions)
     int d0 = 0, r0 = 32 * sw;
     while (na > 0 && r0 >= na) { r0 -= na; ++d0; }
-    for (int T0 = 32 * sw; T0 < npairs; T0 += 32 * NWARP) {
+    for (int T0 = 32 * sw; T0 < ((AEV_ABL & 128) ? 0 : npairs); T0 += 32 * NWARP) {
         const int t = T0 + lane;
         if (t < npairs) {
             int d = (int)(((float)t + 0.5f) * inv_na);
@@ -515,7 +516,7 @@ k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
             f32x2 S0t = pack2(0.f, 0.f);                                           // (S0, St)
             float Sm = 0.f;
 #pragma unroll
-            for (int a = 0; a < NAg; ++a) {
+            for (int a = 0; a < ((AEV_ABL & 32) ? 0 : NAg); ++a) {
                 const float mm = Rm - K.shf_a[a];
                 const float B = fast_exp2(-K.eta_a_l2e * mm * mm);
                 const float dB = -K.eta_a * mm * B;                                // dB/dR_ij = dB/dR_ik
@@ -557,7 +558,7 @@ k_aev_bwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
 #pragma unroll
         for (int q = 0; q < OWN; ++q) {
             const int nn = lane + 32 * q;
-            if (32 * q < na && nn < na) {
+            if (32 * q < na && nn < na && !(AEV_ABL & 64)) {
                 for (int d = d_lo; d <= d_hi; ++d) {
                     const int tj = d * na + nn - T0;
                     if ((unsigned)tj < (unsigned)cntr) { Fx[q] -= Sw.st[0][tj]; Fy[q] -= Sw.st[1][tj]; Fz[q] -= Sw.st[2][tj]; }
