@@ -274,3 +274,32 @@ def test_ani1x_params_are_validated(torch, B):
     bad = dataclasses.replace(p, shf_z=p.shf_z[:4])              # 4 x 4: not one of the two grids
     with pytest.raises(B.DhpError):
         B.Dhp(16, params=bad)
+
+
+def test_random_systems_sizes_and_ensembles(torch, B, params, blob8):
+    """Seeded sweep over system size (40 .. 3 500 atoms: the single-block list path, a handful of row tiles, tens of tiles
+    with ragged tails for every species) and ensemble size (1 .. 8): every call - repeated three times on the same context,
+    so that replayed graphs, the chain kernel's ping-pong tensor-memory maps and its per-SM scratch tiles are reused - and
+    the energy-only call must land inside the north_star bars."""
+    rng = np.random.default_rng(123)
+    for it in range(16):
+        n = int(rng.integers(40, 3500))
+        n_models = int(rng.integers(1, 9))
+        edge = max((n / 0.1) ** (1.0 / 3.0), 10.5)
+        s = W.small_periodic_mix(n, float(edge), seed=int(rng.integers(1, 10**6)), n_models=n_models)
+        blob = blob8[: n_models * 7 * W.PARAMS_PER_NET]
+        d = B.Dhp(s.n_atoms, params=params)
+        w = d.dhp_weights_load(blob, n_models)
+        pos, sp, mol = B.to_device(s)
+        E = torch.empty(1, dtype=torch.float64, device="cuda")
+        F = torch.empty((n, 3), dtype=torch.float32, device="cuda")
+        for _ in range(3):
+            d.dhp_ani_energy_forces(pos, s.box, sp, w, mol, E=E, F=F)
+        Ee = d.dhp_ani_energy(pos, s.box, sp, w, mol)
+        torch.cuda.synchronize()
+        assert d.dhp_status() == 0
+        Eo, Fo = oracle.total_energy_forces(s, params, blob)
+        assert abs(E.item() - Eo[0]) / n <= E_TOL_PER_ATOM, (it, n, n_models)
+        assert abs(Ee.item() - Eo[0]) / n <= E_TOL_PER_ATOM, (it, n, n_models)
+        assert np.max(np.abs(F.cpu().numpy() - Fo)) <= F_TOL, (it, n, n_models)
+        d.close()
