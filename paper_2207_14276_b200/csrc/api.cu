@@ -148,7 +148,12 @@ static int run_energy_forces(Ctx* ctx, const float* pos, const float* box, const
         if (!tensor) { const int rc = mlp_simt_ensure(ctx, w->n_models); if (rc != DHP_OK) return rc; }
     }
     const bool large = n > SMALL_N;
-    const bool small = ctx->graph_on && n > 0 && (!large || ctx->graph_large) && !(ctx->skin > 0.f) && !ctx->prof.on;
+    const bool small = ctx->graph_on && n > 0 && (!large || ctx->graph_large) && !ctx->prof.on;
+    // list reuse: the enqueue is one of two fixed sequences (device-side reuse check, or forced rebuild when the problem changed),
+    // each with its own graph; the kernels of the path not taken are gated on the device as in a plain enqueue
+    const bool skin_on = ctx->skin > 0.f && ctx->cand != nullptr && n > 0;
+    const bool reuse_same = skin_on && nlist_reuse_same(ctx, n, box, mol_offsets, n_mol, central);
+    const float skin_key = skin_on ? ctx->skin : 0.f;
     if (!small) return enqueue_energy_forces(ctx, pos, box, species, n, mol_offsets, n_mol, w, E, F, central);
     float bx[4] = {0.f, 0.f, 0.f, box ? 1.f : 0.f};
     if (box) for (int c = 0; c < 3; ++c) bx[c] = box[c];
@@ -156,7 +161,8 @@ static int run_energy_forces(Ctx* ctx, const float* pos, const float* box, const
     GraphEntry* victim = &ctx->graphs[0];
     for (GraphEntry& g : ctx->graphs) {
         if (g.used && g.pos == pos && g.species == species && g.mol == mol_offsets && g.central == central && g.weights == w && g.E == E &&
-            g.F == F && g.n == n && g.n_mol == n_mol && g.mlp_mode == ctx->mlp_mode && memcmp(g.box, bx, sizeof(bx)) == 0) { hit = &g; break; }
+            g.F == F && g.n == n && g.n_mol == n_mol && g.mlp_mode == ctx->mlp_mode && g.skin == skin_key && g.reuse_same == reuse_same &&
+            memcmp(g.box, bx, sizeof(bx)) == 0) { hit = &g; break; }
         if (!g.used || (victim->used && g.stamp < victim->stamp)) victim = &g;
     }
     if (large) {                                      // a caller whose arguments change every call (a new box per step) gains nothing
@@ -195,6 +201,7 @@ static int run_energy_forces(Ctx* ctx, const float* pos, const float* box, const
         hit->used = true; hit->exec = exec;
         hit->pos = pos; hit->species = species; hit->mol = mol_offsets; hit->central = central; hit->weights = w; hit->E = E; hit->F = F;
         hit->n = n; hit->n_mol = n_mol; hit->mlp_mode = ctx->mlp_mode; memcpy(hit->box, bx, sizeof(bx));
+        hit->skin = skin_key; hit->reuse_same = reuse_same;
         hit->launches = ctx->launches - l0;
         hit->s_n_mol = ctx->n_mol; hit->s_periodic = ctx->periodic; hit->s_partial = ctx->partial; hit->s_planes = ctx->aev_in_planes;
         hit->s_models = ctx->n_models;
@@ -202,7 +209,8 @@ static int run_energy_forces(Ctx* ctx, const float* pos, const float* box, const
     }
     // the host-side state a plain enqueue would have left behind
     ctx->n_atoms = n; ctx->n_mol = hit->s_n_mol; ctx->periodic = hit->s_periodic; ctx->partial = hit->s_partial;
-    ctx->aev_in_planes = hit->s_planes; ctx->n_models = hit->s_models; ctx->cand_valid = false;
+    ctx->aev_in_planes = hit->s_planes; ctx->n_models = hit->s_models;
+    if (skin_on) nlist_reuse_mark(ctx, n, box, mol_offsets, n_mol, central); else ctx->cand_valid = false;
     hit->stamp = ++ctx->graph_clock;
     DHP_CUDA(ctx, cudaGraphLaunch(hit->exec, ctx->stream));
     ctx->launches += hit->launches;
@@ -520,6 +528,7 @@ int dhp_set_skin(dhp_ctx* h, float skin) {
     if (!h || !(skin >= 0.f) || skin > 4.0f) return DHP_E_BADARG;
     Ctx* c = &h->c;
     cudaStreamSynchronize(c->stream);
+    graphs_invalidate(c);                          // captured calls hold the candidate buffers of the old skin (or none)
     for (void* p : {(void*)c->cand, (void*)c->cand_cnt, (void*)c->pos_ref, (void*)c->rebuild, (void*)c->rebuild_count}) if (p) cudaFree(p);
     c->cand = nullptr; c->cand_cnt = nullptr; c->pos_ref = nullptr; c->rebuild = nullptr; c->rebuild_count = nullptr;
     c->skin = 0.f; c->cand_valid = false; c->cand_stride = 0;

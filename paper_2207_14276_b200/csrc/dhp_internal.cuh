@@ -100,6 +100,8 @@ struct GraphEntry {
     int64_t n, n_mol;
     float box[4];              // edges, [3] = 1 if periodic
     int mlp_mode;
+    float skin;                // list reuse: the skin in force and which enqueue was captured (reuse check / forced rebuild)
+    bool reuse_same;
     cudaGraphExec_t exec;
     int64_t launches;          // kernels in the graph (dhp_launch_count)
     int64_t s_n_mol; bool s_periodic, s_partial, s_planes; int s_models;   // host-side state the enqueue leaves behind
@@ -224,6 +226,8 @@ void prof_mark(Ctx* ctx, int boundary);   // records event `boundary` (start of 
     } while (0)
 
 // ---- phases (each enqueues kernels on ctx->stream) ------------------------------------------------
+bool nlist_reuse_same(const Ctx* ctx, int64_t n, const float* box_host, const int32_t* mol_offsets, int64_t n_mol, const uint8_t* central);
+void nlist_reuse_mark(Ctx* ctx, int64_t n, const float* box_host, const int32_t* mol_offsets, int64_t n_mol, const uint8_t* central);
 int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t* species, int64_t n,
                 const int32_t* mol_offsets, int64_t n_mol, const uint8_t* central = nullptr);
 int nlist_export(Ctx* ctx, int32_t* row_ptr, int32_t* col, bool angular);

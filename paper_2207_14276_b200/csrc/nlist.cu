@@ -1089,6 +1089,30 @@ k_small_assign(const float4* __restrict__ spos, const unsigned char* __restrict_
 // ---------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------
+// List reuse (dhp_set_skin): is this call the same problem as the one the candidate list was built for (size, box, molecule
+// table, masked or not)?  Whether the atoms have stayed within skin / 2 is decided on the device.  Shared with the graph replay
+// of the hot call (api.cu), which must pick the graph of the right enqueue (reuse check, or forced rebuild) and leave the same
+// host-side record behind as a plain enqueue.
+static void reuse_box(const float* box_host, float (&bx)[4]) {
+    const bool periodic = box_host != nullptr;
+    for (int c = 0; c < 3; ++c) bx[c] = periodic ? (float)(double)box_host[c] : 0.f;
+    bx[3] = periodic ? 1.f : 0.f;
+}
+bool nlist_reuse_same(const Ctx* ctx, int64_t n, const float* box_host, const int32_t* mol_offsets, int64_t n_mol, const uint8_t* central) {
+    const bool by_mol = mol_offsets != nullptr && n_mol > 0;
+    float bx[4];
+    reuse_box(box_host, bx);
+    return ctx->cand_valid && ctx->cand_n == n && ctx->cand_nmol == (by_mol ? n_mol : 0) && ctx->cand_mol == (const void*)mol_offsets &&
+           ctx->cand_central == (central != nullptr) && memcmp(bx, ctx->cand_box, sizeof(bx)) == 0;
+}
+void nlist_reuse_mark(Ctx* ctx, int64_t n, const float* box_host, const int32_t* mol_offsets, int64_t n_mol, const uint8_t* central) {
+    const bool by_mol = mol_offsets != nullptr && n_mol > 0;
+    float bx[4];
+    reuse_box(box_host, bx);
+    ctx->cand_valid = true; ctx->cand_n = n; ctx->cand_nmol = by_mol ? n_mol : 0; ctx->cand_mol = (const void*)mol_offsets;
+    ctx->cand_central = central != nullptr; memcpy(ctx->cand_box, bx, sizeof(bx));
+}
+
 int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t* species, int64_t n64,
                 const int32_t* mol_offsets, int64_t n_mol64, const uint8_t* central) {
     const int n = (int)n64, n_mol = (int)n_mol64;
@@ -1139,8 +1163,7 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
         // reuse is possible only for the same problem (size, box, molecule table, masked or not); whether the atoms
         // have stayed within skin / 2 of the last full build is decided on the device
         const float bx[4] = {(float)L[0], (float)L[1], (float)L[2], periodic ? 1.f : 0.f};
-        const bool same = ctx->cand_valid && ctx->cand_n == n && ctx->cand_nmol == (by_mol ? n_mol : 0) && ctx->cand_mol == (const void*)mol_offsets &&
-                          ctx->cand_central == (central != nullptr) && memcmp(bx, ctx->cand_box, sizeof(bx)) == 0;
+        const bool same = nlist_reuse_same(ctx, n, box_host, mol_offsets, n_mol, central);
         if (same) {
             DHP_CUDA(ctx, cudaMemsetAsync(ctx->rebuild, 0, sizeof(int), st));
             const float h = 0.5f * ctx->skin;
@@ -1149,8 +1172,8 @@ int nlist_build(Ctx* ctx, const float* pos, const float* box_host, const int32_t
         } else {
             DHP_LAUNCH(ctx, k_set_flag, 1, 1, 0, ctx->rebuild, 1);
         }
-        ctx->cand_valid = true; ctx->cand_n = n; ctx->cand_nmol = by_mol ? n_mol : 0; ctx->cand_mol = (const void*)mol_offsets;
-        ctx->cand_central = central != nullptr; memcpy(ctx->cand_box, bx, sizeof(bx));
+        (void)bx;
+        nlist_reuse_mark(ctx, n, box_host, mol_offsets, n_mol, central);
         DHP_LAUNCH(ctx, k_reset_rows, 2 * ctx->sm_count, 256, 0, ctx->row_slot, ctx->row_species, (int)ctx->max_rows, gate);
     }
     if (!periodic && !by_mol) {
