@@ -14,6 +14,7 @@
 // are distinct and all k are distinct and the per-neighbour force accumulators in shared memory are
 // updated without atomics; one global atomic triple per neighbour at the end.
 #include <algorithm>
+#include <cstdlib>
 
 #include "dhp_internal.cuh"
 
@@ -121,8 +122,12 @@ __device__ __forceinline__ void put_value(float v, float* __restrict__ row_f32, 
 // radial slot q (priority order), column AEV_ANG + 16 q + lane for lane < 16
 #define PUT_RAD(v, q) put_value<PLANES>(v, row_f32, row_hi, plane_stride, AEV_ANG + 16 * (q) + lane, 14 * (ROW_TILE * KBLK) + ((q) << 11) + lane_off)
 
-template <bool PLANES, int NAg, int NZg>     // NAg x NZg: the angular grid of Eq. 5, 8 x 4 (ANI-2x shape) or 4 x 8 (ANI-1x shape)
-__global__ void __launch_bounds__(AEV_WARPS * 32, 40 / AEV_WARPS)
+// SPLIT (small systems, n <= SMALL_N): one block of AEV_WARPS warps per atom, as in the backward kernel - warp 0 stages the neighbours
+// and does the radial part, the angular rounds are dealt out to the warps (one warp per atom is latency-bound: ~3 k dependent
+// instructions whatever the system size); each warp sums its rounds' pair blocks into a private shared row, the rows are added
+// and written at the end.
+template <bool PLANES, int NAg, int NZg, bool SPLIT>     // NAg x NZg: the angular grid of Eq. 5, 8 x 4 (ANI-2x shape) or 4 x 8 (ANI-1x shape)
+__global__ void __launch_bounds__(AEV_WARPS * 32, SPLIT ? 1 : 40 / AEV_WARPS)
 k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, const int* __restrict__ col,
           const unsigned short* __restrict__ seg_cnt, const int* __restrict__ rowmap, const unsigned* __restrict__ tile_mask,
           const Grid* __restrict__ gp, const __grid_constant__ AevConst K, int n, float* __restrict__ aev,
@@ -135,10 +140,14 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
     // full evaluation: warp <-> atom in sorted (cell) order, so that the warps of a block share neighbours; partial
     // evaluation (row_slot != null, n = an upper bound of the rows): warp <-> row, so that no warp is spent on the atoms
     // that are not central in this call
-    int i = blockIdx.x * AEV_WARPS + w;
+    int i = SPLIT ? (int)blockIdx.x : blockIdx.x * AEV_WARPS + w;
     if (i >= n) return;
     if (row_slot) { i = row_slot[i]; if (i < 0) return; }
-    WarpSmemFwd& S = reinterpret_cast<WarpSmemFwd*>(smem_raw)[w];
+    WarpSmemFwd& S = reinterpret_cast<WarpSmemFwd*>(smem_raw)[SPLIT ? 0 : w];       // geometry and pair table of the atom
+    WarpSmemFwd& Sw = reinterpret_cast<WarpSmemFwd*>(smem_raw)[w];                   // this warp's staging rows
+    float* part = reinterpret_cast<float*>(smem_raw + sizeof(WarpSmemFwd) * AEV_WARPS) + (size_t)w * (NPAIR * 32);   // SPLIT: this warp's pair-block sums
+    const int sw = SPLIT ? w : 0;
+    constexpr int NWARP = SPLIT ? AEV_WARPS : 1;
     const unsigned FULL = 0xffffffffu;
     const unsigned lt = (1u << lane) - 1u;
 
@@ -167,8 +176,12 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
     __half* row_hi = planes + aev_tiled_off(row, 0);
     const int lane_off = (lane >> 3) * (ROW_TILE * 8) + (lane & 7);
 
+    if (SPLIT) {
+#pragma unroll
+        for (int p = 0; p < NPAIR; ++p) part[p * 32 + lane] = 0.f;
+    }
     // ---- stage all neighbours -------------------------------------------------------------------------
-    for (int a = lane; a < nst; a += 32) {
+    for (int a = lane; a < (sw == 0 ? nst : 0); a += 32) {
         const NbrGeom q = neighbour_geom(pi, spos[col[rb + a]], g);
         S.rr[a] = make_float2(q.R, fcut(q.R, inv_rcr));
         if (a < na) {
@@ -197,8 +210,8 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
         pstart -= padded;
         const unsigned nz = __ballot_sync(FULL, pcount > 0);
         nz_pairs = nz;
-        if (pcount > 0) S.tab[__popc(nz & lt)] = make_int4(pstart, ja0 | (kb0 << 8) | (cb << 16) | ((psa == psb) << 24), pcount, lane);
-        if (lane == 0) S.tab[__popc(nz)] = make_int4(T_pad, 0, 0, 0);
+        if (pcount > 0 && sw == 0) S.tab[__popc(nz & lt)] = make_int4(pstart, ja0 | (kb0 << 8) | (cb << 16) | ((psa == psb) << 24), pcount, lane);
+        if (lane == 0 && sw == 0) S.tab[__popc(nz)] = make_int4(T_pad, 0, 0, 0);
     }
     __syncwarp();
 
@@ -208,7 +221,7 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
         const int m2 = lane & 7, h = lane >> 3;
         const f32x2 nshf = pack2(-K.shf_r[2 * m2], -K.shf_r[2 * m2 + 1]);
         const f32x2 neta = pack2(-K.eta_r_l2e, -K.eta_r_l2e);
-        for (int s = 0; s < NSP; ++s) {
+        for (int s = 0; s < (sw == 0 ? NSP : 0); ++s) {
             const int ca = __shfl_sync(FULL, cnt, s), sa = __shfl_sync(FULL, start, s);
             const int cr = __shfl_sync(FULL, cnt, 8 + s), sr = __shfl_sync(FULL, start, 8 + s) - ca;
             if (ca + cr == 0) continue;
@@ -240,13 +253,13 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
         }
     }
 
-    __syncwarp();                                        // rr is dead from here on: its bytes become the staging rows
+    if (SPLIT) __syncthreads(); else __syncwarp();       // rr is dead from here on: its bytes become the staging rows
     // ---- angular (Eq. 5) ------------------------------------------------------------------------------
     static_assert(NAg * NZg == 32 && NAg + NZg == 12, "angular grid");
     const int za = lane % NZg, aa = lane / NZg;          // this lane's feature (a, z) of a pair block, index NZg a + z
     float facc = 0.f;                                    // running sum of feature (aa, za) of the current pair
     int e = 0;                                           // table entry of this lane's slot (monotonic over the rounds)
-    for (int T0 = 0; T0 < T_pad; T0 += 32) {
+    for (int T0 = 32 * sw; T0 < T_pad; T0 += 32 * NWARP) {
         const int t = T0 + lane;
         float A[NZg], B[NAg];
 #pragma unroll
@@ -291,28 +304,45 @@ k_aev_fwd(const float4* __restrict__ spos, const int* __restrict__ row_ptr, cons
             }
         }
 #pragma unroll
-        for (int z = 0; z < NZg; ++z) S.st[z][lane] = A[z];
+        for (int z = 0; z < NZg; ++z) Sw.st[z][lane] = A[z];
 #pragma unroll
-        for (int a = 0; a < NAg; ++a) S.st[NZg + a][lane] = B[a];
+        for (int a = 0; a < NAg; ++a) Sw.st[NZg + a][lane] = B[a];
         __syncwarp();
         // phase 2: the 8 quads of the round in order (pairs are padded to whole quads, so a pair ends at a quad end);
         // the branch is warp-uniform
         const unsigned endmask = __ballot_sync(FULL, my_end);
 #pragma unroll
         for (int qd = 0; qd < ((AEV_ABL & 2) ? 0 : 8); ++qd) {
-            const float4 a4 = *reinterpret_cast<const float4*>(&S.st[za][4 * qd]);
-            const float4 b4 = *reinterpret_cast<const float4*>(&S.st[NZg + aa][4 * qd]);
+            const float4 a4 = *reinterpret_cast<const float4*>(&Sw.st[za][4 * qd]);
+            const float4 b4 = *reinterpret_cast<const float4*>(&Sw.st[NZg + aa][4 * qd]);
             facc = fmaf(a4.x, b4.x, facc); facc = fmaf(a4.y, b4.y, facc);
             facc = fmaf(a4.z, b4.z, facc); facc = fmaf(a4.w, b4.w, facc);
             if ((endmask >> (4 * qd + 3)) & 1u) {             // pair complete: its 32 features go out, 64 (128) contiguous bytes
                 const int blk = __shfl_sync(FULL, my_blk, 4 * qd + 3);
-                PUT_ANG(facc, blk);
+                if (SPLIT) part[blk * 32 + lane] += facc; else PUT_ANG(facc, blk);
                 facc = 0.f;
             }
+        }
+        if (SPLIT) {                                         // this warp's next round is NWARP rounds away: bank the open pair's partial sum
+            const int blk = __shfl_sync(FULL, my_blk, 31);
+            part[blk * 32 + lane] += facc;
+            facc = 0.f;
         }
         __syncwarp();
     }
     __syncwarp();
+    if (SPLIT) {
+        __syncthreads();
+        const float* all = reinterpret_cast<const float*>(smem_raw + sizeof(WarpSmemFwd) * AEV_WARPS);
+        for (int p = w; p < NPAIR; p += AEV_WARPS) {
+            if (!((nz_pairs >> p) & 1u)) continue;
+            float v = 0.f;
+#pragma unroll
+            for (int q = 0; q < AEV_WARPS; ++q) v += all[(size_t)q * (NPAIR * 32) + p * 32 + lane];
+            PUT_ANG(v, p);
+        }
+        if (w != 0) return;                                  // the zeros below are warp 0's
+    }
 
     // ---- zeros for what this atom lacks but a reader will touch -------------------------------------------
     // (tensor path: the feature blocks that are active for the row's tile; fp32 rows: everything)
@@ -638,10 +668,15 @@ int aev_init(Ctx* ctx) {
         for (int lo = 0; lo <= hi; ++lo, ++p)
             if ((prio_sp(lo) | (prio_sp(hi) << 4)) != (int)h_pair_sp[p]) return DHP_E_BADARG;
     const int fs = (int)(sizeof(WarpSmemFwd) * AEV_WARPS), bs = (int)(sizeof(WarpSmemBwd) * BWD_WARPS);
-    DHP_CUDA(ctx, cudaFuncSetAttribute((k_aev_fwd<false, 8, 4>), cudaFuncAttributeMaxDynamicSharedMemorySize, fs));
-    DHP_CUDA(ctx, cudaFuncSetAttribute((k_aev_fwd<true, 8, 4>), cudaFuncAttributeMaxDynamicSharedMemorySize, fs));
-    DHP_CUDA(ctx, cudaFuncSetAttribute((k_aev_fwd<false, 4, 8>), cudaFuncAttributeMaxDynamicSharedMemorySize, fs));
-    DHP_CUDA(ctx, cudaFuncSetAttribute((k_aev_fwd<true, 4, 8>), cudaFuncAttributeMaxDynamicSharedMemorySize, fs));
+    const int fss = fs + (int)(sizeof(float) * AEV_WARPS * NPAIR * 32);      // SPLIT: + the warps' pair-block sums
+    DHP_CUDA(ctx, cudaFuncSetAttribute((k_aev_fwd<false, 8, 4, false>), cudaFuncAttributeMaxDynamicSharedMemorySize, fs));
+    DHP_CUDA(ctx, cudaFuncSetAttribute((k_aev_fwd<true, 8, 4, false>), cudaFuncAttributeMaxDynamicSharedMemorySize, fs));
+    DHP_CUDA(ctx, cudaFuncSetAttribute((k_aev_fwd<false, 4, 8, false>), cudaFuncAttributeMaxDynamicSharedMemorySize, fs));
+    DHP_CUDA(ctx, cudaFuncSetAttribute((k_aev_fwd<true, 4, 8, false>), cudaFuncAttributeMaxDynamicSharedMemorySize, fs));
+    DHP_CUDA(ctx, cudaFuncSetAttribute((k_aev_fwd<false, 8, 4, true>), cudaFuncAttributeMaxDynamicSharedMemorySize, fss));
+    DHP_CUDA(ctx, cudaFuncSetAttribute((k_aev_fwd<true, 8, 4, true>), cudaFuncAttributeMaxDynamicSharedMemorySize, fss));
+    DHP_CUDA(ctx, cudaFuncSetAttribute((k_aev_fwd<false, 4, 8, true>), cudaFuncAttributeMaxDynamicSharedMemorySize, fss));
+    DHP_CUDA(ctx, cudaFuncSetAttribute((k_aev_fwd<true, 4, 8, true>), cudaFuncAttributeMaxDynamicSharedMemorySize, fss));
     DHP_CUDA(ctx, cudaFuncSetAttribute((k_aev_bwd<8, 4, false>), cudaFuncAttributeMaxDynamicSharedMemorySize, bs));
     DHP_CUDA(ctx, cudaFuncSetAttribute((k_aev_bwd<4, 8, false>), cudaFuncAttributeMaxDynamicSharedMemorySize, bs));
     DHP_CUDA(ctx, cudaFuncSetAttribute((k_aev_bwd<8, 4, true>), cudaFuncAttributeMaxDynamicSharedMemorySize, bs));
@@ -659,14 +694,22 @@ int aev_forward(Ctx* ctx, bool planes) {
     // call's atom count instead, and rows beyond the last group hold -1
     const int* row_slot = ctx->partial ? ctx->row_slot : nullptr;
     const int nw = ctx->partial ? (int)std::min<int64_t>(ctx->max_rows, (int64_t)n + NSP * ROW_ALIGN) : n;
-    const int blocks = (nw + AEV_WARPS - 1) / AEV_WARPS;
+    // small systems: a block of 8 warps per atom (SPLIT), else a warp per atom
+    const bool split = n <= SMALL_N && !ctx->no_fwd_split;      // measured: 50 atoms 26.7 -> 14.6 us, 288 atoms 15.1 -> 12.6 us
+    const int blocks = split ? nw : (nw + AEV_WARPS - 1) / AEV_WARPS;
+    const size_t smem_l = smem + (split ? sizeof(float) * AEV_WARPS * NPAIR * 32 : 0);
     const size_t plane_stride = (size_t)ctx->max_rows * AEV_LD;
-#define DHP_AEV_FWD(P, A, Z)                                                                                                    \
-    DHP_LAUNCH(ctx, (k_aev_fwd<P, A, Z>), blocks, AEV_WARPS * 32, smem, ctx->spos, ctx->row_ptr, ctx->col, ctx->seg_cnt, ctx->rowmap, \
+#define DHP_AEV_FWD(P, A, Z, S)                                                                                                 \
+    DHP_LAUNCH(ctx, (k_aev_fwd<P, A, Z, S>), blocks, AEV_WARPS * 32, smem_l, ctx->spos, ctx->row_ptr, ctx->col, ctx->seg_cnt, ctx->rowmap, \
                ctx->tile_mask, ctx->grid, ctx->aevc, nw, ctx->aev, ctx->aev_planes, plane_stride, ctx->status, row_slot)
     const bool g84 = ctx->aevc.n_a == 8;                 // 8 x 4 (ANI-2x shape) or 4 x 8 (ANI-1x shape) angular grid
-    if (planes) { if (g84) DHP_AEV_FWD(true, 8, 4); else DHP_AEV_FWD(true, 4, 8); }
-    else        { if (g84) DHP_AEV_FWD(false, 8, 4); else DHP_AEV_FWD(false, 4, 8); }
+    if (split) {
+        if (planes) { if (g84) DHP_AEV_FWD(true, 8, 4, true); else DHP_AEV_FWD(true, 4, 8, true); }
+        else        { if (g84) DHP_AEV_FWD(false, 8, 4, true); else DHP_AEV_FWD(false, 4, 8, true); }
+    } else {
+        if (planes) { if (g84) DHP_AEV_FWD(true, 8, 4, false); else DHP_AEV_FWD(true, 4, 8, false); }
+        else        { if (g84) DHP_AEV_FWD(false, 8, 4, false); else DHP_AEV_FWD(false, 4, 8, false); }
+    }
 #undef DHP_AEV_FWD
     DHP_CUDA(ctx, cudaGetLastError());
     return DHP_OK;
