@@ -888,6 +888,9 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
     tc_fence_before();
     __syncthreads();
     if (warp == EPI_WARPS + 1) tmem_dealloc(tmem_base, TMEM_COLS);
+#ifdef T2_TRACE
+    if (EPI == EPI_GRAD && threadIdx.x == 0) { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); printf("T2END %d %llu\n", (int)blockIdx.x, t); }
+#endif
 }
 
 // ======================================================================================================
