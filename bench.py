@@ -174,7 +174,18 @@ def workload_name(cfg: int, system) -> str:
     return f"BASELINE.json configs[{cfg - 1}]: {system.name}, {system.n_atoms} atoms, {system.n_models}-network ensemble"
 
 
+def _ensure_built():
+    """The libraries are built in-tree and git-ignored: a checkout without them builds them once (no CPU fallback exists)."""
+    from paper_2207_14276_b200 import build as cuda_build
+    from oracle import build as oracle_build
+    if not os.path.exists(cuda_build.LIB):
+        cuda_build.build(force=True)
+    if not os.path.exists(oracle_build.LIB):
+        oracle_build.build(force=True)
+
+
 def main():
+    _ensure_built()
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
