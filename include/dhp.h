@@ -268,11 +268,13 @@ int dhp_profile_read(dhp_ctx* ctx, double* ms, int64_t* n_calls);
 
 /* Number of kernels this library has launched on the context since dhp_create (kernels of replayed graphs included). */
 int64_t dhp_launch_count(dhp_ctx* ctx);
-/* Small systems (n_atoms <= 320: the solute of the hybrid scheme, the call RESPA's outer step makes,
- * L200-208) are latency-bound: their hot call is captured once per argument set (pointers, sizes, box, mode) into a CUDA
- * graph and replayed on later calls with the same arguments - same kernels, same results, no per-launch host work.
- * Returns the number of hot calls served by a replay so far.  DHP_NO_GRAPH=1 in the environment at dhp_create turns
- * the mechanism off; it is also off while list reuse (dhp_set_skin) or phase profiling is on. */
+/* The hot call is captured once per argument set (pointers, sizes, box, mode, list-reuse state) into a CUDA graph and replayed
+ * on later calls with the same arguments - same kernels, same results, no per-launch host work.  It matters most for small
+ * systems (n_atoms <= 320: the solute of the hybrid scheme, the call RESPA's outer step makes, L200-208),
+ * which are latency-bound; larger systems are replayed too (DHP_GRAPH_ALL=0 in the environment turns that off, and the library
+ * stops by itself when a caller's argument set changes on every call, e.g. a new box each step).  Four graphs are kept per
+ * context (least recently used first out).  Returns the number of hot calls served by a replay so far.  DHP_NO_GRAPH=1 in the
+ * environment at dhp_create turns the mechanism off; it is also off while phase profiling is on. */
 int64_t dhp_graph_replays(dhp_ctx* ctx);
 
 const char* dhp_strerror(int code);
