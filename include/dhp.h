@@ -225,6 +225,41 @@ int dhp_md_open(dhp_ctx* ctx, dhp_md* md, float* pos, float* vel, const float* b
                 int n_inner, int64_t lo, int64_t hi);
 int dhp_md_close(dhp_ctx* ctx, dhp_md* md, float* vel, const float* F_slow, float dt, int n_inner, int64_t lo, int64_t hi);
 
+/* Kinetic energy for callers that cannot allocate device memory.
+ *
+ * Who that is: a plug-in of an MD engine that claimed the whole GPU at start-up and hands out only the buffers it
+ * registered (the set-up this library is written for: the engine is the master and reserves its memory once, PAPER.md
+ * L128-134) - there a cudaMalloc may simply fail, and the engine's rules usually forbid it anyway; a per-step diagnostic
+ * inside a running MD loop, where cudaMalloc / cudaFree would stall every stream of the device while they run; a process
+ * whose framework allocator owns the device memory, so a raw cudaMalloc competes with it.  Every other call of this library
+ * needs a dhp_ctx (dhp_create allocates the workspace) and, for the kinetic energy, a dhp_md handle (dhp_md_create
+ * allocates the accumulators); this one needs neither and calls no cudaMalloc, cudaFree or allocating library routine,
+ * on its first call or on any later one.
+ *
+ *   vel       dev fp32 [n_atoms][3], Å/fs
+ *   inv_mass  dev fp32 [n_atoms], as in dhp_md_create: 0.2625499639 / (mass in amu)
+ *   n_atoms   0 .. DHP_KINETIC_STATIC_MAX_ATOMS; more is refused with DHP_E_CAPACITY before anything is enqueued
+ *             (n_atoms = 0 writes E_kin = 0)
+ *   E_kin     dev fp64 [1], written (not added to): sum_i 1/2 |v_i|^2 / inv_mass_i, Hartree - the value dhp_md_run
+ *             reports in E_out[2], up to the order of the fp64 additions (here fixed: block partials added in block order,
+ *             so two calls on the same data give the same bits)
+ *   cuda_stream  a cudaStream_t (NULL = legacy default stream) of the device that is CURRENT in the calling thread; the
+ *             pointers must belong to that device.  Asynchronous: a memset of 256 bytes and one kernel are enqueued.
+ *
+ * Where the working memory lives instead: a fixed 33 KB array inside libdhp.so's device image (one partial sum per block of
+ * 256 atoms, which is what sets the size limit, plus an arrival counter).  Every GPU that loads the library holds that array
+ * until the process exits, whether this function is ever called or not.  Consequences a caller has to know:
+ *   - there is ONE array per GPU, shared by every call from every thread and stream.  It keeps what the last call left; the
+ *     function clears the counter itself at the start of each call.  Two calls that can run on the same GPU at the same
+ *     time (different streams, or different host threads without ordering between their streams) race on it and both
+ *     results are then undefined - order such calls yourself (same stream, or an event between the streams);
+ *   - the first call on each device looks up the array's device address (cudaGetSymbolAddress, once per device, kept for
+ *     later calls); that is set-up work, so make this first call before you start capturing any stream;
+ * Errors: DHP_E_BADARG (null pointer with n_atoms > 0, null E_kin, n_atoms < 0), DHP_E_CAPACITY (n_atoms above the limit),
+ * DHP_E_CUDA (the address lookup, the memset or the launch failed). */
+#define DHP_KINETIC_STATIC_MAX_ATOMS 1048576
+int dhp_kinetic_energy_static(const float* vel, const float* inv_mass, int64_t n_atoms, double* E_kin, void* cuda_stream);
+
 /* Same computation with HOST buffers (pos, species, mol_offsets, E, F all host; pinned memory makes
  * the copies asynchronous): host->device copies, the kernels, device->host copies and one stream
  * synchronisation all happen inside the call.  This is the end-to-end entry point bench.py times. */

@@ -43,6 +43,7 @@ SYMBOLS = {
     "dhp_md_run": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _i32, _f32, _i32, _i32, _vp]),
     "dhp_md_open": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _f32, _i32, _i64, _i64]),
     "dhp_md_close": (C.c_int, [_vp, _vp, _vp, _vp, _f32, _i32, _i64, _i64]),
+    "dhp_kinetic_energy_static": (C.c_int, [_vp, _vp, _i64, _vp, _vp]),
     "dhp_status": (C.c_int, [_vp]),
     "dhp_set_mlp_mode": (C.c_int, [_vp, _i32]),
     "dhp_tensor_path_available": (C.c_int, [_vp]),
@@ -131,6 +132,39 @@ def _check_inputs(torch, device, pos, species, mol_offsets=None, host: bool = Fa
             raise DhpError("mol_offsets needs n_mol + 1 >= 2 entries")
         if host and (int(mol_offsets[0]) != 0 or int(mol_offsets[-1]) != n):     # values of device tables are not read here:
             raise DhpError("mol_offsets must start at 0 and end at n_atoms")      # that would synchronise the hot call
+
+
+KINETIC_STATIC_MAX_ATOMS = 1048576      # DHP_KINETIC_STATIC_MAX_ATOMS of include/dhp.h
+
+
+def dhp_kinetic_energy_static(vel, inv_mass, E_kin, stream=None):
+    """Kinetic energy sum_i 1/2 |v_i|^2 / inv_mass_i (Hartree) of cuda tensors vel fp32 [N, 3] and inv_mass fp32 [N], written
+    into the caller's cuda tensor E_kin (fp64, one element) - the entry point for code that must not allocate device memory
+    (an MD engine's plug-in working inside the engine's own reservation, a diagnostic inside a running loop where a
+    cudaMalloc would stall the device, a process whose allocator owns the GPU).  Neither the library nor this wrapper
+    allocates: no context, no handle, the result goes where the caller says, and the working memory is a fixed array
+    inside libdhp.so - which is why N is limited to KINETIC_STATIC_MAX_ATOMS and why calls that could overlap on one GPU
+    must be ordered by the caller (they share that array).  `stream`: a torch.cuda.Stream, or None for torch's current
+    stream; the tensors' device is made current for the call.  Asynchronous.  Make the first call on a device outside any
+    stream capture: it looks up the array's address.  See include/dhp.h."""
+    import torch
+    lib = load_library()
+    for name, a, dt, shape in (("vel", vel, torch.float32, (int(inv_mass.shape[0]), 3)), ("inv_mass", inv_mass, torch.float32, None),
+                               ("E_kin", E_kin, torch.float64, None)):
+        if not (a.is_cuda and a.dtype == dt and a.is_contiguous() and a.device == vel.device):
+            raise DhpError(f"{name} must be a contiguous {dt} cuda tensor on {vel.device}")
+        if shape is not None and tuple(a.shape) != shape:
+            raise DhpError(f"{name} must have shape {list(shape)}")
+    n = int(inv_mass.shape[0])
+    if inv_mass.dim() != 1 or E_kin.numel() < 1:
+        raise DhpError("inv_mass must be [N] and E_kin must hold one fp64")
+    if n > KINETIC_STATIC_MAX_ATOMS:
+        raise DhpError(f"dhp_kinetic_energy_static handles at most {KINETIC_STATIC_MAX_ATOMS} atoms (its working memory is a "
+                       f"fixed array inside the library), got {n}")
+    with torch.cuda.device(vel.device):
+        st = torch.cuda.current_stream() if stream is None else stream
+        _check(lib.dhp_kinetic_energy_static(_vp(_dptr(vel)), _vp(_dptr(inv_mass)), n, _vp(_dptr(E_kin)), _vp(st.cuda_stream)))
+    return E_kin
 
 
 def make_params(p) -> DhpParams:

@@ -9,6 +9,7 @@
 // context's stream; there is no host synchronisation inside a run, and with dhp_set_skin the neighbour list of
 // the ANI call is reused between outer steps ("atomic positions do not move much between two time-steps", L134).
 #include <initializer_list>
+#include <mutex>
 #include <new>
 #include <string.h>
 
@@ -224,6 +225,104 @@ int dhp_md_close(dhp_ctx* h, dhp_md* md, float* vel, const float* F_slow, float 
     DHP_LAUNCH(c, k_md_kick_drift, nb, 256, 0, (float*)nullptr, vel, m->inv_mass, F_slow, 0.5f * dt, ff, 0.5f * d, 0.f, t1, t0);
     DHP_CUDA(c, cudaGetLastError());
     return DHP_OK;
+}
+
+
+}  // extern "C"
+
+// ---- kinetic energy for callers that may not allocate (include/dhp.h: dhp_kinetic_energy_static) ------------------------
+// Same sum as k_md_kinetic, E_kin = sum_i 1/2 |v_i|^2 / inv_mass_i in fp64, but nothing here comes from cudaMalloc.
+// k_md_kinetic adds into an accumulator that dhp_md_create allocated; this variant keeps its working memory - one partial
+// sum per block and an arrival counter - in a fixed array that is part of the library image, so the entry point needs no
+// context, no handle and no allocator.  The price is a size limit and a single shared copy per GPU (see the header).
+namespace dhp {
+
+constexpr int KIN_THREADS = 256;
+constexpr int KIN_MAX_BLOCKS = DHP_KINETIC_STATIC_MAX_ATOMS / KIN_THREADS;   // one block per 256 atoms, one partial per block
+constexpr int KIN_HEAD = 32;                                                 // doubles in front of the partials: 256 bytes for the counter
+static_assert(DHP_KINETIC_STATIC_MAX_ATOMS % KIN_THREADS == 0, "whole blocks");
+
+// [0] (as unsigned): number of blocks of the running call that have stored their partial; [KIN_HEAD + b]: partial sum of block b.
+// 33 KB, resident on every GPU that has loaded libdhp.so for as long as the process lives.  On the host this name is only a
+// handle for cudaGetSymbolAddress - it is NOT the device address and must never be handed to a kernel as it stands.
+static __device__ __align__(256) double g_kin_scratch[KIN_HEAD + KIN_MAX_BLOCKS];
+
+__global__ void __launch_bounds__(KIN_THREADS)
+k_md_kinetic_static(const float* __restrict__ vel, const float* __restrict__ inv_mass, int n, double* __restrict__ scratch,
+                    double* __restrict__ E_kin) {
+    __shared__ double wsum[KIN_THREADS / 32];
+    __shared__ bool last;
+    const int tid = threadIdx.x, i = blockIdx.x * KIN_THREADS + tid;
+    double e = 0.0;
+    if (i < n) {
+        const double vx = vel[3 * i], vy = vel[3 * i + 1], vz = vel[3 * i + 2];
+        e = 0.5 * (vx * vx + vy * vy + vz * vz) / (double)inv_mass[i];
+    }
+    for (int o = 16; o; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
+    if ((tid & 31) == 0) wsum[tid >> 5] = e;
+    __syncthreads();
+    if (tid == 0) {
+        double b = 0.0;
+        for (int w = 0; w < KIN_THREADS / 32; ++w) b += wsum[w];
+        scratch[KIN_HEAD + blockIdx.x] = b;
+        __threadfence();                                                     // the partial is visible before the arrival is counted
+        last = atomicAdd((unsigned*)scratch, 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (!last) return;
+    // the block that arrives last adds the partials in block order: the result does not depend on which block that was
+    __threadfence();
+    double t = 0.0;
+    for (int b = tid; b < (int)gridDim.x; b += KIN_THREADS) t += __ldcg(&scratch[KIN_HEAD + b]);
+    for (int o = 16; o; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    if ((tid & 31) == 0) wsum[tid >> 5] = t;
+    __syncthreads();
+    if (tid == 0) {
+        double tot = 0.0;
+        for (int w = 0; w < KIN_THREADS / 32; ++w) tot += wsum[w];
+        *E_kin = tot;
+        *(unsigned*)scratch = 0u;                                            // leave the counter as the next call expects it
+    }
+}
+
+// Device address of g_kin_scratch per device ordinal, looked up once per device with that device current.
+constexpr int KIN_MAX_DEVICES = 64;
+static std::mutex g_kin_mu;
+static double* g_kin_addr[KIN_MAX_DEVICES];
+
+static cudaError_t kin_scratch_address(double** out) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const bool cached = dev >= 0 && dev < KIN_MAX_DEVICES;
+    std::lock_guard<std::mutex> lock(g_kin_mu);
+    if (cached && g_kin_addr[dev]) { *out = g_kin_addr[dev]; return cudaSuccess; }
+    double* p = nullptr;
+    e = cudaGetSymbolAddress((void**)&p, g_kin_scratch);                     // the address on the CURRENT device
+    if (e != cudaSuccess) return e;
+    if (!p) return cudaErrorInvalidSymbol;
+    if (cached) g_kin_addr[dev] = p;
+    *out = p;
+    return cudaSuccess;
+}
+
+}  // namespace dhp
+
+extern "C" {
+
+int dhp_kinetic_energy_static(const float* vel, const float* inv_mass, int64_t n_atoms, double* E_kin, void* cuda_stream) {
+    if (!E_kin || n_atoms < 0 || (n_atoms > 0 && (!vel || !inv_mass))) return DHP_E_BADARG;
+    if (n_atoms > DHP_KINETIC_STATIC_MAX_ATOMS) return DHP_E_CAPACITY;       // more blocks than the fixed array has partials for
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (n_atoms == 0) return cudaMemsetAsync(E_kin, 0, sizeof(double), st) == cudaSuccess ? DHP_OK : DHP_E_CUDA;
+    double* scratch = nullptr;
+    if (kin_scratch_address(&scratch) != cudaSuccess) { cudaGetLastError(); return DHP_E_CUDA; }
+    // the array keeps whatever the previous call left: the counter has to read zero when the first block arrives, also after
+    // a call that was cut short; the partials need no clearing, every block of this call overwrites its own before it is read
+    if (cudaMemsetAsync(scratch, 0, sizeof(double) * KIN_HEAD, st) != cudaSuccess) { cudaGetLastError(); return DHP_E_CUDA; }
+    const int blocks = (int)((n_atoms + KIN_THREADS - 1) / KIN_THREADS);
+    k_md_kinetic_static<<<blocks, KIN_THREADS, 0, st>>>(vel, inv_mass, (int)n_atoms, scratch, E_kin);
+    return cudaGetLastError() == cudaSuccess ? DHP_OK : DHP_E_CUDA;
 }
 
 }  // extern "C"
