@@ -150,6 +150,67 @@ def kd_pairs(pos, box, rc):
     return set(map(tuple, pr)) | set(map(tuple, pr[:, ::-1]))
 
 
+def kd_pairs_ortho(pos, box, rc):
+    """Periodic k-d tree with one edge PER AXIS (scipy's own minimum image): the independent statement of the oracle's
+    orthorhombic branch (pair_r2: d -= L_axis * rint(d / L_axis))."""
+    from scipy.spatial import cKDTree
+    L = np.asarray(box, dtype=np.float64)
+    p = pos.astype(np.float64)
+    p = p - L * np.floor(p / L)
+    p = np.where(p >= L, p - L, p)
+    pr = cKDTree(p, boxsize=L).query_pairs(rc, output_type="ndarray")
+    return set(map(tuple, pr)) | set(map(tuple, pr[:, ::-1]))
+
+
+@pytest.mark.parametrize("n,box", [(900, (17.3, 21.9, 24.6)), (300, (10.3, 13.0, 22.5)), (400, (22.5, 10.3, 13.0))])
+@pytest.mark.parametrize("rc", [5.1, 3.5])
+def test_pairs_orthorhombic_box_match_kdtree(params, n, box, rc):
+    """every other pin uses a cubic box, so `L = box[0]` for all three axes in pair_r2 passed them all.  Three
+    different edges, the short one on different axes (10.3 Å is barely 2 Rcr: most pairs along it cross the boundary)."""
+    s = W.small_periodic_ortho(n, box, seed=78 + n)
+    shift = np.array([0.0, 2.0, -1.0], np.float32) * s.box            # whole-box shifts per axis: atoms outside [0, L)
+    pos = s.pos.copy()
+    pos[::5] += shift
+    rp, col = oracle.pairs(pos, s.box, rc)
+    mine = {(i, int(j)) for i in range(s.n_atoms) for j in col[rp[i]:rp[i + 1]]}
+    assert mine == kd_pairs_ortho(pos, s.box, float(np.float32(rc)))
+    # a cubic box with the first edge is a different list: the test distinguishes the two
+    assert mine != kd_pairs(pos, s.box, float(np.float32(rc)))
+
+
+def test_energy_forces_follow_an_axis_permutation_of_an_orthorhombic_box(params):
+    """Relabelling the axes (x, y, z) -> (z, x, y) of positions AND box is a symmetry of Eqs. 2-5 with per-axis minimum image:
+    same energies, forces with permuted components.  A per-axis mix-up anywhere (pairs, AEV displacements, force
+    back-substitution) breaks it because the three edges differ."""
+    s = W.small_periodic_ortho(240, (10.3, 13.0, 18.1), seed=91, n_models=1)
+    blob = W.make_weights(1)
+    Ea, Fa, _ = oracle.energy_forces(s.pos, s.species, s.box, params, blob, 1)
+    perm = [2, 0, 1]
+    Eb, Fb, _ = oracle.energy_forces(np.ascontiguousarray(s.pos[:, perm]), s.species, np.ascontiguousarray(s.box[perm]), params, blob, 1)
+    assert np.max(np.abs(Ea - Eb)) <= 1e-12
+    assert np.max(np.abs(Fa[:, perm] - Fb)) <= 1e-11
+    assert np.abs(Fa).max() > 1e-3                                     # not a trivially empty system
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+@pytest.mark.parametrize("periodic", [False, True])
+def test_pair_at_exactly_the_cutoff_is_in_the_list_one_ulp_beyond_is_not(params, axis, periodic):
+    """Eq. 3 is "R <= Rc" (reading Q2): the tie is inclusive, at both cutoffs, in the oracle itself (the GPU half
+    of this statement lives in test_gpu_parity_full.py).  Separations are exact in fp32: 1.0 + float32(rc) is representable."""
+    box = np.array([23.0, 26.0, 29.0], np.float32) if periodic else None
+    for rc in (params.rcr, params.rca):
+        rcf = np.float32(rc)
+        e = np.zeros(3, np.float32); e[axis] = 1.0
+        at, beyond = np.float32(1.0) + rcf, np.nextafter(np.float32(1.0) + rcf, np.float32(100.0))
+        assert np.float64(at) - 1.0 == np.float64(rcf) and np.float64(beyond) - 1.0 > np.float64(rcf)
+        base = np.ones(3, np.float32)
+        pos = np.stack([base, base + (at - 1) * e, base - (beyond - 1) * e]).astype(np.float32)
+        assert np.float64(pos[1, axis]) - 1.0 == np.float64(rcf) and 1.0 - np.float64(pos[2, axis]) > np.float64(rcf)
+        rp, col = oracle.pairs(pos, box, float(rc))
+        assert list(col[rp[0]:rp[1]]) == [1]                           # the tie is kept, one ulp beyond is not
+        assert list(col[rp[1]:rp[2]]) == [0] and rp[3] == rp[2]
+
+
 @pytest.mark.parametrize("cfg,rc", [(1, 5.1), (1, 3.5), (2, 5.1), (2, 3.5)])
 def test_pairs_match_kdtree(params, cfg, rc):
     s = W.make_system(cfg)
