@@ -214,10 +214,15 @@ int dhp_md_run(dhp_ctx* ctx, dhp_md* md, float* pos, float* vel, const float* bo
 
 /* One outer step of the same scheme, split at the slow-force evaluation and restricted to the atoms [lo, hi) that a rank
  * OWNS - the building blocks of the multi-GPU MD loop (domain decomposition):
- *   dhp_md_open   v += (dt/2) a_slow ; [ v += (d/2) a_fast ; x += d v ; v += (d/2) a_fast ]^n_inner   for atoms [lo, hi)
+ *   dhp_md_open   v += (dt/2) a_slow ; [ v += (d/2) a_fast ; x += d v ; v += (d/2) a_fast ]^n_inner, WITHOUT the last fast
+ *                 half kick                                                                          for atoms [lo, hi)
  *   ... the caller all-gathers the new positions, evaluates its partial slow force with
  *       dhp_ani_energy_forces_partial and reduce-scatters it (paper_2207_14276_b200/shard.py) ...
- *   dhp_md_close  v += (dt/2) a_slow                                                               for atoms [lo, hi)
+ *   dhp_md_close  v += (d/2) a_fast (the pending one, fast force at the final positions) + (dt/2) a_slow   for atoms [lo, hi)
+ * After the pair the state is that of one full outer step.  BETWEEN the two calls the velocities lack that last fast half
+ * kick (the two kicks are one kernel in dhp_md_close): do not read them there.  dhp_md_close must be given the dt and n_inner
+ * of the dhp_md_open it completes, and there must be one - anything else is DHP_E_BADARG (an empty range [lo, lo) is a
+ * no-op in both calls).
  * F_slow: dev fp32 [n_atoms][3], the TOTAL slow force; only rows [lo, hi) are read.  The md handle must have been
  * created with the bonds whose two atoms both lie in [lo, hi) (ranges are cut at molecule boundaries).  pos / vel are
  * the full [n_atoms][3] arrays; only rows [lo, hi) are written.  Asynchronous.  Errors: BADARG. */
@@ -272,7 +277,8 @@ int dhp_ani_energy_forces_host(dhp_ctx* ctx, const float* pos, const float* box,
  * own status into it on the device, so a fault at an intermediate call of an unsynchronised sequence (dhp_md_run
  * enqueues n_steps calls) is not lost; reading clears it.  After DHP_E_CAPACITY the results of the faulting call are
  * those of a truncated list (or of an empty one if the total pair storage overflowed); with list reuse the candidate
- * list is discarded and the next call rebuilds. */
+ * list is discarded and the next call rebuilds.  Within ONE call a capacity fault takes precedence over a species fault
+ * (the word then reads DHP_E_CAPACITY whichever came first); across calls the first faulting call is the one reported. */
 int dhp_status(dhp_ctx* ctx);
 
 int dhp_set_mlp_mode(dhp_ctx* ctx, int mode);
@@ -306,10 +312,13 @@ int64_t dhp_launch_count(dhp_ctx* ctx);
 /* The hot call is captured once per argument set (pointers, sizes, box, mode, list-reuse state) into a CUDA graph and replayed
  * on later calls with the same arguments - same kernels, same results, no per-launch host work.  It matters most for small
  * systems (n_atoms <= 320: the solute of the hybrid scheme, the call RESPA's outer step makes, L200-208),
- * which are latency-bound; larger systems are replayed too (DHP_GRAPH_ALL=0 in the environment turns that off, and the library
- * stops by itself when a caller's argument set changes on every call, e.g. a new box each step).  Four graphs are kept per
- * context (least recently used first out).  Returns the number of hot calls served by a replay so far.  DHP_NO_GRAPH=1 in the
- * environment at dhp_create turns the mechanism off; it is also off while phase profiling is on. */
+ * which are latency-bound; larger systems are replayed too (DHP_GRAPH_ALL=0 in the environment turns that off).  The graph is
+ * built when an argument set is seen for the SECOND time; the first call with it runs as a plain enqueue, so a caller whose
+ * arguments never repeat (new output buffers on every call, a new box each step) pays nothing for the mechanism.  Eight argument
+ * sets are remembered per context (least recently used first out): rotate at most eight buffer sets, and pass the same E / F.
+ * If graphs keep being built and then serve fewer than two calls each, the library stops building them for that size class.
+ * Returns the number of hot calls served by a replay so far.  DHP_NO_GRAPH=1 in the environment at dhp_create turns the
+ * mechanism off; it is also off while phase profiling is on. */
 int64_t dhp_graph_replays(dhp_ctx* ctx);
 
 const char* dhp_strerror(int code);

@@ -86,6 +86,10 @@ def load_library() -> C.CDLL:
             fn = getattr(lib, name)          # AttributeError if the symbol is not exported
             fn.restype = res
             fn.argtypes = args
+        version = lib.dhp_version().decode()
+        if "[extra flags:" in version and os.environ.get("DHP_ALLOW_EXPERIMENT") != "1":
+            raise DhpError(f"{LIB_PATH} is an experiment build ({version}): some of those macros give wrong results by design. "
+                           "Rebuild without DHP_NVCC_EXTRA (python -m paper_2207_14276_b200.build), or set DHP_ALLOW_EXPERIMENT=1")
         _lib = lib
     return _lib
 
@@ -372,14 +376,28 @@ class Dhp:
         self._n = int(pos.shape[0])
         return E_out
 
+    def _check_rows3(self, **arrays):
+        """fp32 [N, 3] cuda tensors of this context's device, contiguous, all with the same N (the C ABI reads raw addresses)."""
+        t, n = self.torch, None
+        for name, a in arrays.items():
+            ok = (hasattr(a, "is_cuda") and a.device == self.device and a.dtype == t.float32 and a.is_contiguous()
+                  and a.dim() == 2 and int(a.shape[1]) == 3 and (n is None or int(a.shape[0]) == n))
+            if not ok:
+                raise DhpError(f"{name} must be a contiguous float32 tensor of shape [N, 3] on {self.device}")
+            n = int(a.shape[0])
+
     def dhp_md_open(self, md, pos, vel, box, F_slow, dt: float, n_inner: int, lo: int, hi: int):
-        """First half kick + inner loop for the owned atoms [lo, hi) (in place on the cuda tensors pos, vel)."""
+        """First half kick + inner loop (all but its last fast half kick, see include/dhp.h) for the owned atoms [lo, hi),
+        in place on the cuda tensors pos, vel."""
+        self._check_rows3(pos=pos, vel=vel, F_slow=F_slow)
         boxh = None if box is None else np.ascontiguousarray(box, dtype=np.float32)
         _check(self.lib.dhp_md_open(self.ctx, md, _vp(_dptr(pos)), _vp(_dptr(vel)), _vp(_dptr(boxh)), _vp(_dptr(F_slow)),
                                     C.c_float(float(dt)), int(n_inner), int(lo), int(hi)), self.ctx)
 
     def dhp_md_close(self, md, vel, F_slow, dt: float, n_inner: int, lo: int, hi: int):
-        """Second half kick for the owned atoms [lo, hi)."""
+        """The pending fast half kick and the second slow half kick for the owned atoms [lo, hi); dt and n_inner must be those
+        of the dhp_md_open this call completes."""
+        self._check_rows3(vel=vel, F_slow=F_slow)
         _check(self.lib.dhp_md_close(self.ctx, md, _vp(_dptr(vel)), _vp(_dptr(F_slow)), C.c_float(float(dt)), int(n_inner),
                                      int(lo), int(hi)), self.ctx)
 

@@ -7,6 +7,14 @@
 #include <string.h>
 
 #include "dhp_internal.cuh"
+#if defined(__has_include)
+#if __has_include("dhp_build_flags.h")
+#include "dhp_build_flags.h"          // written by build.py: the extra compiler flags of this build
+#endif
+#endif
+#ifndef DHP_EXTRA_FLAGS
+#define DHP_EXTRA_FLAGS ""
+#endif
 
 namespace dhp {
 
@@ -133,13 +141,13 @@ static void graphs_invalidate(Ctx* ctx) {
     }
 }
 
-// The hot call.  The enqueue of the kernels is captured ONCE per argument set into a CUDA graph on the library's own stream and
-// replayed on the caller's stream afterwards - same kernels, same arithmetic, no per-launch host work and no gaps between
+// The hot call.  The enqueue of the kernels is captured ONCE per argument set (when that set is seen for the second time) into a
+// CUDA graph on the library's own stream and replayed on the caller's stream afterwards - same kernels, same arithmetic, no per-launch host work and no gaps between
 // dependent launches.  It matters most for small systems (n <= SMALL_N: the solute of the hybrid scheme, PAPER.md L112-118,
 // L200-208 - the call RESPA's outer step makes: a dozen dependent 15-40 us launches); above SMALL_N it saves the ~1 % of the step
 // that the nine short list kernels spend waiting for their launches, and switches itself off for a caller whose argument
 // sets never repeat.  A changed pointer, size, box or mode is a
-// new graph (4 are kept, least recently used first out).
+// new graph (8 keys are kept, least recently used first out).
 static int run_energy_forces(Ctx* ctx, const float* pos, const float* box, const int32_t* species, int64_t n,
                              const int32_t* mol_offsets, int64_t n_mol, const Weights* w, double* E, float* F,
                              const uint8_t* central = nullptr) {
@@ -148,7 +156,7 @@ static int run_energy_forces(Ctx* ctx, const float* pos, const float* box, const
         if (!tensor) { const int rc = mlp_simt_ensure(ctx, w->n_models); if (rc != DHP_OK) return rc; }
     }
     const bool large = n > SMALL_N;
-    const bool small = ctx->graph_on && n > 0 && (!large || ctx->graph_large) && !ctx->prof.on;
+    const bool small = ctx->graph_on && n > 0 && (large ? ctx->graph_large : ctx->graph_small) && !ctx->prof.on;
     // list reuse: the enqueue is one of two fixed sequences (device-side reuse check, or forced rebuild when the problem changed),
     // each with its own graph; the kernels of the path not taken are gated on the device as in a plain enqueue
     const bool skin_on = ctx->skin > 0.f && ctx->cand != nullptr && n > 0;
@@ -165,16 +173,28 @@ static int run_energy_forces(Ctx* ctx, const float* pos, const float* box, const
             memcmp(g.box, bx, sizeof(bx)) == 0) { hit = &g; break; }
         if (!g.used || (victim->used && g.stamp < victim->stamp)) victim = &g;
     }
-    if (large) {                                      // a caller whose arguments change every call (a new box per step) gains nothing
-        if (hit) ctx->gl_hit++;
-        else if (++ctx->gl_miss > 16 && ctx->gl_miss > ctx->gl_hit) {
-            ctx->graph_large = false;
-            return enqueue_energy_forces(ctx, pos, box, species, n, mol_offsets, n_mol, w, E, F, central);
-        }
-    }
+    // A graph is built on the SECOND sighting of an argument set; the first sighting only records the key and runs as a plain
+    // enqueue.  A caller whose arguments never repeat (fresh E / F buffers on every call, a new box per step, more rotating
+    // position buffers than the table has entries) therefore never pays for a capture, at any system size.
     if (!hit) {
         if (victim->used && victim->exec) cudaGraphExecDestroy(victim->exec);
-        victim->used = false; victim->exec = nullptr;
+        victim->used = true; victim->exec = nullptr;
+        victim->pos = pos; victim->species = species; victim->mol = mol_offsets; victim->central = central; victim->weights = w;
+        victim->E = E; victim->F = F; victim->n = n; victim->n_mol = n_mol; victim->mlp_mode = ctx->mlp_mode;
+        memcpy(victim->box, bx, sizeof(bx)); victim->skin = skin_key; victim->reuse_same = reuse_same;
+        victim->stamp = ++ctx->graph_clock;
+        return enqueue_energy_forces(ctx, pos, box, species, n, mol_offsets, n_mol, w, E, F, central);
+    }
+    if (!hit->exec) {
+        // what is left to guard against is an argument set that comes back once or twice and then changes for good: when, after
+        // 16 captures of a size class, the graphs have served fewer than two calls each on average, that class stops capturing
+        int64_t& caps = ctx->g_captures[large ? 1 : 0];
+        int64_t& reps = ctx->g_replays[large ? 1 : 0];
+        if (caps >= 16 && reps < 2 * caps) {
+            if (large) ctx->graph_large = false; else ctx->graph_small = false;
+            return enqueue_energy_forces(ctx, pos, box, species, n, mol_offsets, n_mol, w, E, F, central);
+        }
+        ++caps;
         cudaStream_t user = ctx->stream;
         if (cudaStreamBeginCapture(ctx->cap_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
             cudaGetLastError();
@@ -197,11 +217,7 @@ static int run_energy_forces(Ctx* ctx, const float* pos, const float* box, const
             ctx->launches = l0;
             return enqueue_energy_forces(ctx, pos, box, species, n, mol_offsets, n_mol, w, E, F, central);
         }
-        hit = victim;
-        hit->used = true; hit->exec = exec;
-        hit->pos = pos; hit->species = species; hit->mol = mol_offsets; hit->central = central; hit->weights = w; hit->E = E; hit->F = F;
-        hit->n = n; hit->n_mol = n_mol; hit->mlp_mode = ctx->mlp_mode; memcpy(hit->box, bx, sizeof(bx));
-        hit->skin = skin_key; hit->reuse_same = reuse_same;
+        hit->exec = exec;
         hit->launches = ctx->launches - l0;
         hit->s_n_mol = ctx->n_mol; hit->s_periodic = ctx->periodic; hit->s_partial = ctx->partial; hit->s_planes = ctx->aev_in_planes;
         hit->s_models = ctx->n_models;
@@ -215,6 +231,7 @@ static int run_energy_forces(Ctx* ctx, const float* pos, const float* box, const
     DHP_CUDA(ctx, cudaGraphLaunch(hit->exec, ctx->stream));
     ctx->launches += hit->launches;
     ctx->graph_replays++;
+    ctx->g_replays[large ? 1 : 0]++;
     return DHP_OK;
 }
 
@@ -284,7 +301,7 @@ int dhp_create(dhp_ctx** out, const dhp_params* params, int64_t max_atoms, int64
     c->sm_count = prop.multiProcessorCount;
     { const char* e = getenv("DHP_NO_SMALL_PATH"); c->no_small_path = e && e[0] == '1'; }
     { const char* e = getenv("DHP_NO_GRAPH"); c->graph_on = !(e && e[0] == '1'); }
-    { const char* e = getenv("DHP_GRAPH_ALL"); c->graph_large = !(e && e[0] == '0'); c->gl_miss = c->gl_hit = 0; }
+    { const char* e = getenv("DHP_GRAPH_ALL"); c->graph_large = !(e && e[0] == '0'); c->graph_small = true; c->g_captures[0] = c->g_captures[1] = c->g_replays[0] = c->g_replays[1] = 0; }
     if (c->graph_on && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); c->graph_on = false; c->cap_stream = nullptr; }
     { const char* e = getenv("DHP_NO_FWD_SPLIT"); c->no_fwd_split = e && e[0] == '1'; }
     { const char* e = getenv("DHP_TC_FUSE"); c->tc_fuse = (e && e[0] == '0') ? 0 : 1; }
@@ -506,6 +523,7 @@ int dhp_status(dhp_ctx* h) {
     cudaError_t e = cudaMemcpyAsync(&s, c->status, sizeof(int), cudaMemcpyDeviceToHost, c->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(&sticky, c->sticky, sizeof(int), cudaMemcpyDeviceToHost, c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->sticky, 0, sizeof(int), c->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->status, 0, sizeof(int), c->stream);   // reading clears both words: a fault of the LAST call is reported once
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e, "status");
     return sticky != 0 ? sticky : s;
@@ -647,6 +665,8 @@ const char* dhp_strerror(int code) {
     }
 }
 const char* dhp_last_cuda_error(dhp_ctx* h) { return h ? h->c.cuda_err : ""; }
-const char* dhp_version(void) { return "dhp 0.1 (sm_100a)"; }
+// "dhp 0.1 (sm_100a)" for a default build; a build with extra compiler flags (DHP_NVCC_EXTRA: the timing-experiment macros, some of
+// which give wrong results by design) says so: "dhp 0.1 (sm_100a) [extra flags: ...]" - binding.load_library() refuses such a library
+const char* dhp_version(void) { return sizeof(DHP_EXTRA_FLAGS) > 1 ? "dhp 0.1 (sm_100a) [extra flags: " DHP_EXTRA_FLAGS "]" : "dhp 0.1 (sm_100a)"; }
 
 }  // extern "C"

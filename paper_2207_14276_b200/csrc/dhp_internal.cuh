@@ -102,12 +102,12 @@ struct GraphEntry {
     int mlp_mode;
     float skin;                // list reuse: the skin in force and which enqueue was captured (reuse check / forced rebuild)
     bool reuse_same;
-    cudaGraphExec_t exec;
+    cudaGraphExec_t exec;      // null while the key has been seen only once (no graph yet)
     int64_t launches;          // kernels in the graph (dhp_launch_count)
     int64_t s_n_mol; bool s_periodic, s_partial, s_planes; int s_models;   // host-side state the enqueue leaves behind
     uint64_t stamp;
 };
-constexpr int N_GRAPHS = 4;
+constexpr int N_GRAPHS = 8;
 
 struct Ctx {
     cudaStream_t stream;
@@ -129,8 +129,10 @@ struct Ctx {
     GraphEntry graphs[N_GRAPHS];
     uint64_t graph_clock;
     int64_t graph_replays;
-    bool graph_large;      // systems above SMALL_N replay too (DHP_GRAPH_ALL=0 turns it off); switched off by itself when the argument
-    int64_t gl_miss, gl_hit;   // sets keep changing (a new box every step): more captures than replays
+    bool graph_large;      // systems above SMALL_N replay too (DHP_GRAPH_ALL=0 turns it off)
+    bool graph_small;      // systems up to SMALL_N replay
+    int64_t g_captures[2], g_replays[2];   // per size class (0 small, 1 large): graphs built and calls they served; a class whose
+                           // graphs serve fewer than two calls each on average switches itself off (run_energy_forces)
     char cuda_err[256];
     Profile prof;
 

@@ -27,6 +27,8 @@ struct Md {
     float* f_fast;     // [N][3]
     double* e;         // [3] E_slow, E_fast, E_kin
     bool primed;       // f_slow / f_fast hold the forces at the current positions
+    float open_dt;     // dhp_md_open .. dhp_md_close: the step in flight (0 = none): close must finish the step open began
+    int open_n_inner;
 };
 
 // v += inv_m (ca Fa + cb Fb); optionally x += delta v
@@ -208,6 +210,7 @@ int dhp_md_open(dhp_ctx* h, dhp_md* md, float* pos, float* vel, const float* box
                    k == 0 ? 0.5f * d : d, d, t1, t0);
         if ((rc = fast_forces(c, m, pos, box)) != DHP_OK) return rc;
     }
+    m->open_dt = dt; m->open_n_inner = n_inner;           // the last fast half kick is dhp_md_close's: it needs the same d
     DHP_CUDA(c, cudaGetLastError());
     return DHP_OK;
 }
@@ -221,6 +224,9 @@ int dhp_md_close(dhp_ctx* h, dhp_md* md, float* vel, const float* F_slow, float 
     const int t0 = (int)(3 * lo), t1 = (int)(3 * hi), nb = (t1 - t0 + 255) / 256;
     const float* ff = m->n_bonds > 0 ? m->f_fast : nullptr;
     if (m->n_bonds == 0) n_inner = 1;
+    // close finishes the step open began: another dt or n_inner would apply the pending fast half kick with the wrong length
+    if (m->open_dt == 0.f || m->open_dt != dt || m->open_n_inner != n_inner) return DHP_E_BADARG;
+    m->open_dt = 0.f;
     const float d = dt / (float)n_inner;
     DHP_LAUNCH(c, k_md_kick_drift, nb, 256, 0, (float*)nullptr, vel, m->inv_mass, F_slow, 0.5f * dt, ff, 0.5f * d, 0.f, t1, t0);
     DHP_CUDA(c, cudaGetLastError());

@@ -177,7 +177,7 @@ __global__ void k_assign_cells(const float* __restrict__ pos, const int* __restr
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     int s = species[i];
-    if (s < 0 || s >= NSP) atomicExch(status, DHP_E_SPECIES);
+    if (s < 0 || s >= NSP) atomicCAS(status, 0, DHP_E_SPECIES);   // never over a CAPACITY fault: k_scan_blocks derives cand_bad from the word
     int cell;
     if (g->by_molecule) {
         int lo = 0, hi = n_mol;            // largest m with mol_offsets[m] <= i
@@ -969,7 +969,7 @@ k_small_pairs(const float* __restrict__ pos, const int* __restrict__ species, in
         return lo;
     };
     int si = species[i];
-    if (lane == 0 && (si < 0 || si >= NSP)) atomicExch(status, DHP_E_SPECIES);
+    if (lane == 0 && (si < 0 || si >= NSP)) atomicCAS(status, 0, DHP_E_SPECIES);
     si = min(max(si, 0), NSP - 1);
     const float4 pi = make_float4(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], __int_as_float(si));
     const int mi = mol_of(i);

@@ -149,7 +149,11 @@ def owner_bounds(n_atoms: int, world: int, unit: int = 1, first_unit_atom: int =
 
 class Exchange:
     """Padded layout for collectives with equal chunks: rank r's atoms [bounds[r], bounds[r+1]) occupy rows
-    [r * chunk, r * chunk + len_r) of a [world * chunk, 3] buffer.  Index arithmetic and torch.distributed calls only."""
+    [r * chunk, r * chunk + len_r) of a [world * chunk, 3] buffer.  Index arithmetic and torch.distributed calls only.
+    The collectives run whenever a process group of `world` ranks exists - also a group of ONE rank, where they are the
+    identity: that is the only way the NCCL branch (reduce_scatter_tensor / all_gather_into_tensor on CUDA tensors) can be
+    executed on a one-GPU box.  Without a process group (world must then be 1) the calls are plain copies.  The padded
+    buffers are allocated on first use and kept, so that a step allocates nothing."""
 
     def __init__(self, bounds, device, group=None):
         import torch
@@ -159,10 +163,14 @@ class Exchange:
         self.world = int(self.bounds.size - 1)
         self.n = int(self.bounds[-1])
         self.chunk = int(max(1, np.diff(self.bounds).max()))
-        self.rank = dist.get_rank(group) if (dist.is_available() and dist.is_initialized()) else 0
-        live = self.world > 1 and dist.is_available() and dist.is_initialized()
-        self.live = live
-        self.backend = dist.get_backend(group) if live else None
+        have_pg = dist.is_available() and dist.is_initialized()
+        if have_pg and dist.get_world_size(group) != self.world:
+            raise ValueError(f"bounds describe {self.world} ranks, the process group has {dist.get_world_size(group)}")
+        if not have_pg and self.world != 1:
+            raise ValueError("more than one rank needs an initialised process group")
+        self.rank = dist.get_rank(group) if have_pg else 0
+        self.live = have_pg
+        self.backend = dist.get_backend(group) if have_pg else None
         to_pad = np.full(self.world * self.chunk, self.n, dtype=np.int64)          # padding rows read the extra zero row
         to_atom = np.empty(self.n, dtype=np.int64)
         for r in range(self.world):
@@ -172,6 +180,17 @@ class Exchange:
         self.to_pad = torch.from_numpy(to_pad).to(device)
         self.to_atom = torch.from_numpy(to_atom).to(device)
         self.lo, self.hi = int(self.bounds[self.rank]), int(self.bounds[self.rank + 1])
+        self._buf = {}
+
+    def _buffers(self, like):
+        """(padded [world*chunk, 3], chunk [chunk, 3], extended [n + 1, 3] with a zero last row) for like's dtype / device."""
+        key = (like.dtype, like.device)
+        if key not in self._buf:
+            t = self.torch
+            self._buf[key] = (t.empty((self.world * self.chunk, 3), dtype=like.dtype, device=like.device),
+                              t.zeros((self.chunk, 3), dtype=like.dtype, device=like.device),
+                              t.zeros((self.n + 1, 3), dtype=like.dtype, device=like.device))
+        return self._buf[key]
 
     def reduce_scatter_forces(self, F_partial, F_total):
         """F_total[lo:hi] = sum over ranks of F_partial[lo:hi] (the rows this rank owns); other rows are left alone.
@@ -181,13 +200,14 @@ class Exchange:
         if not self.live:
             F_total[self.lo:self.hi] = F_partial[self.lo:self.hi]
             return F_total
-        src = t.cat([F_partial, t.zeros((1, 3), dtype=F_partial.dtype, device=F_partial.device)])[self.to_pad]
+        padded, out, ext = self._buffers(F_partial)
+        ext[: self.n] = F_partial                                                   # the last row stays zero
+        t.index_select(ext, 0, self.to_pad, out=padded)
         if self.backend == "nccl":
-            out = t.empty((self.chunk, 3), dtype=F_partial.dtype, device=F_partial.device)
-            self.dist.reduce_scatter_tensor(out, src, op=self.dist.ReduceOp.SUM, group=self.group)
+            self.dist.reduce_scatter_tensor(out, padded, op=self.dist.ReduceOp.SUM, group=self.group)
         else:
-            self.dist.all_reduce(src, op=self.dist.ReduceOp.SUM, group=self.group)
-            out = src[self.rank * self.chunk:(self.rank + 1) * self.chunk]
+            self.dist.all_reduce(padded, op=self.dist.ReduceOp.SUM, group=self.group)
+            out = padded[self.rank * self.chunk:(self.rank + 1) * self.chunk]
         F_total[self.lo:self.hi] = out[: self.hi - self.lo]
         return F_total
 
@@ -196,11 +216,11 @@ class Exchange:
         t = self.torch
         if not self.live:
             return pos
-        mine = t.zeros((self.chunk, 3), dtype=pos.dtype, device=pos.device)
-        mine[: self.hi - self.lo] = pos[self.lo:self.hi]
-        full = t.empty((self.world * self.chunk, 3), dtype=pos.dtype, device=pos.device)
+        full, mine, ext = self._buffers(pos)
+        mine[: self.hi - self.lo] = pos[self.lo:self.hi]                            # rows beyond the own count stay zero
         self.dist.all_gather_into_tensor(full, mine, group=self.group)
-        pos.copy_(full[self.to_atom])
+        t.index_select(full, 0, self.to_atom, out=ext[: self.n])
+        pos.copy_(ext[: self.n])
         return pos
 
     def all_reduce_energy(self, E):
@@ -240,17 +260,24 @@ class ShardedMd:
                                     bond_r0 if bonds is not None and len(bonds) else None)
         self.mask_every, self.steps_since_mask, self.mask = int(mask_every), 0, None
         self.F_total = torch.zeros((self.ex.n, 3), dtype=dtype or torch.float32, device=species.device)
-        self.E = None
+        # outputs of the partial call and the mask live in buffers that are allocated once: the library replays a captured graph
+        # only when a call's pointers repeat (include/dhp.h: dhp_graph_replays), and a step should not allocate anyway
+        self.F_part = torch.zeros((self.ex.n, 3), dtype=dtype or torch.float32, device=species.device)
+        self.E = torch.zeros(1, dtype=torch.float64, device=species.device)
         self.primed = False
 
     def _slow(self, pos):
         if self.mask is None or self.steps_since_mask >= self.mask_every:
-            self.mask = slab_mask_device(pos, self.box, self.ex.world, self.ex.rank)
+            m = slab_mask_device(pos, self.box, self.ex.world, self.ex.rank)
+            if self.mask is None:
+                self.mask = m
+            else:
+                self.mask.copy_(m)                       # same address: the argument set of the partial call does not change
             self.steps_since_mask = 0
         self.steps_since_mask += 1
-        E, F = self.dhp.dhp_ani_energy_forces_partial(pos, self.box, self.species, self.weights, self.mask)
-        self.ex.reduce_scatter_forces(F, self.F_total)
-        self.E = self.ex.all_reduce_energy(E)
+        self.dhp.dhp_ani_energy_forces_partial(pos, self.box, self.species, self.weights, self.mask, E=self.E, F=self.F_part)
+        self.ex.reduce_scatter_forces(self.F_part, self.F_total)
+        self.ex.all_reduce_energy(self.E)
 
     def run(self, pos, vel, dt: float, n_inner: int, n_steps: int):
         """`n_steps` outer steps in place on pos / vel [N, 3] (all rows of pos are current on every rank on return; only

@@ -55,3 +55,17 @@ def test_product_path_does_not_import_the_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 src = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in src and "from oracle" not in src and "liboracle" not in src, f
+
+
+def test_experiment_builds_cannot_pass_for_the_default_library(monkeypatch):
+    """DHP_NVCC_EXTRA injects timing-experiment macros, some of which give wrong results by design.  The flags are
+    compiled into dhp_version() and kept in a stamp beside the library: a library built with other flags than the current ones
+    is stale (rebuilt by build()), and the default build says nothing about extra flags (binding.load_library refuses one
+    that does unless DHP_ALLOW_EXPERIMENT=1)."""
+    from paper_2207_14276_b200 import build
+    build.build()
+    assert not build._stale()
+    assert b"extra flags" not in binding.load_library().dhp_version()
+    assert open(build.STAMP).read() == ""
+    monkeypatch.setattr(build, "EXTRA", ["-DMID_TRACE=1"])
+    assert build._stale()

@@ -196,7 +196,13 @@ def test_sharded_driver_on_one_rank_equals_the_oracle_trajectory(torch, B, param
     h = d.dhp_md_create(md.inv_mass)
     F = torch.from_numpy(np.random.default_rng(5).normal(size=(s.n_atoms, 3)).astype(np.float32)).cuda()
     d.dhp_md_open(h, pos2, vel2, s.box, F, 0.5, 1, 30, 90)
+    with pytest.raises(B.DhpError):                         # close completes the step open began: same dt, same n_inner
+        d.dhp_md_close(h, vel2, F, 0.25, 1, 30, 90)
     d.dhp_md_close(h, vel2, F, 0.5, 1, 30, 90)
+    with pytest.raises(B.DhpError):                         # nothing is open any more
+        d.dhp_md_close(h, vel2, F, 0.5, 1, 30, 90)
+    with pytest.raises(B.DhpError):                         # buffers the C ABI would misread
+        d.dhp_md_open(h, pos2.double(), vel2, s.box, F, 0.5, 1, 30, 90)
     torch.cuda.synchronize()
     moved = np.nonzero(np.abs(pos2.cpu().numpy() - s.pos).sum(1))[0]
     assert moved.min() == 30 and moved.max() == 89
@@ -207,3 +213,58 @@ def test_sharded_driver_on_one_rank_equals_the_oracle_trajectory(torch, B, param
         d.dhp_md_open(h, pos2, vel2, s.box, F, 0.5, 1, 90, 30)
     d.dhp_md_destroy(h)
     d.close()
+
+
+def test_sharded_driver_on_a_one_rank_nccl_group(torch, B, params):
+    """The NCCL branch of shard.Exchange - reduce_scatter_tensor and all_gather_into_tensor on CUDA tensors, on the stream the
+    kernels run on - executed on the one GPU there is: on a process group of ONE rank both collectives are legal and are the
+    identity.  First the exchange alone, then shard.ShardedMd on that group with list reuse on (partial call + Verlet skin +
+    graph replay together, what every step of a sharded run does) against the oracle trajectory."""
+    import socket
+    import torch.distributed as dist
+    from paper_2207_14276_b200 import shard
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    assert not dist.is_initialized()
+    torch.cuda.set_device(0)
+    dist.init_process_group("nccl", init_method=f"tcp://127.0.0.1:{port}", rank=0, world_size=1)
+    try:
+        s = W.make_system(1)
+        md = W.md_inputs(s)
+        blob = W.make_weights(1)
+        bounds = shard.owner_bounds(s.n_atoms, 1, unit=3)
+        ex = shard.Exchange(bounds, torch.device("cuda:0"))
+        assert ex.live and ex.backend == "nccl" and ex.chunk == s.n_atoms
+        rng = np.random.default_rng(8)
+        part = torch.from_numpy(rng.normal(size=(s.n_atoms, 3)).astype(np.float32)).cuda()
+        tot = torch.zeros_like(part)
+        for _ in range(2):                                    # second call: the kept buffers
+            ex.reduce_scatter_forces(part, tot)
+            assert torch.equal(tot, part)
+        x = torch.from_numpy(rng.normal(size=(s.n_atoms, 3)).astype(np.float32)).cuda()
+        x0 = x.clone()
+        ex.all_gather_positions(x)
+        assert torch.equal(x, x0)
+        e = torch.tensor([1.25], dtype=torch.float64, device="cuda")
+        assert ex.all_reduce_energy(e).item() == 1.25
+        # the driver on the same group
+        d = B.Dhp(s.n_atoms, params=params)
+        d.dhp_set_skin(1.0)
+        w = d.dhp_weights_load(blob, 1)
+        pos = torch.from_numpy(s.pos.copy()).cuda()
+        vel = torch.from_numpy(md.vel.copy()).cuda()
+        sp = torch.from_numpy(s.species).cuda()
+        drv = shard.ShardedMd(d, w, sp, s.box, bounds, md.inv_mass, md.bonds, md.bond_k, md.bond_r0, mask_every=2)
+        r0 = d.dhp_graph_replays()
+        E = drv.run(pos, vel, 0.5, 2, 5)
+        torch.cuda.synchronize()
+        assert d.dhp_status() == 0
+        assert d.dhp_graph_replays() - r0 >= 3                # same E / F / mask addresses every step: the call is replayed
+        assert 1 <= d.dhp_nlist_rebuild_count() < 6           # the list was reused on some steps at least
+        xo, vo, (Es, _, _) = oracle_run(s, md, params, blob, 0.5, 2, 5)
+        assert np.max(np.abs(pos.cpu().numpy() - xo)) <= X_TOL and np.max(np.abs(vel.cpu().numpy() - vo)) <= V_TOL
+        assert abs(E.item() - Es) / s.n_atoms <= 1e-6
+        d.close()
+    finally:
+        dist.destroy_process_group()

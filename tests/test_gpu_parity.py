@@ -495,10 +495,47 @@ def test_capacity_fault_in_the_middle_of_an_md_run_is_reported(torch, B, params,
     d.close()
 
 
+@pytest.mark.parametrize("n_atoms", [300, 420])
+def test_capacity_and_species_fault_in_the_same_call(torch, B, params, blob8, n_atoms):
+    """a species fault must not hide a capacity fault of the same call (the library derives "the candidate list was
+    truncated" from the word reading CAPACITY), and a fault raised by the LAST call is reported once, not on every read.
+    A ball at ~12 x liquid density overflows every list row; one atom carries species 9.  Both list paths (<= 320 atoms: the
+    three-launch path; above: cell list), with list reuse on."""
+    rng = np.random.default_rng(31)
+    pts = np.empty((0, 3))
+    while pts.shape[0] < n_atoms:
+        c = rng.uniform(-4.4, 4.4, 3)
+        if np.linalg.norm(c) <= 4.4 and (pts.shape[0] == 0 or np.linalg.norm(pts - c, axis=1).min() >= 0.5):
+            pts = np.concatenate([pts, c[None]])
+    sp = rng.integers(0, 4, n_atoms).astype(np.int32)
+    bad = sp.copy()
+    bad[n_atoms // 2] = 9
+    d = B.Dhp(n_atoms, params=params)
+    d.dhp_set_skin(1.0)
+    w = d.dhp_weights_load(blob8[: 7 * W.PARAMS_PER_NET], 1)
+    pos = torch.from_numpy(pts.astype(np.float32)).cuda()
+    d.dhp_ani_energy_forces(pos, None, torch.from_numpy(bad).cuda(), w)
+    assert d.dhp_status() == -2                           # capacity, although the species fault is raised first (binning)
+    assert d.dhp_status() == 0                            # read once
+    d.dhp_ani_energy_forces(pos, None, torch.from_numpy(sp).cuda(), w)
+    assert d.dhp_status() == -2                           # still too dense, species fine
+    assert d.dhp_status() == 0
+    # dilute again (x 2.3: liquid density): a clean call with the canonical list
+    pos2 = (pos * 2.3).contiguous()
+    spd = torch.from_numpy(sp).cuda()
+    d.dhp_ani_energy_forces(pos2, None, spd, w)
+    assert d.dhp_status() == 0
+    d.dhp_nlist_build(pos2, None, spd)
+    rp, col, _, _ = d.dhp_nlist_export()
+    rpo, colo = oracle.pairs(pos2.cpu().numpy(), None, params.rcr)
+    assert csr_equal(rp, col, rpo, colo)
+    d.close()
+
+
 @pytest.mark.parametrize("name", ["ligand50", "water96", "replicas8"])
 def test_small_systems_replay_a_captured_graph(torch, B, params, blob8, name):
-    """Small systems (the hybrid scheme's per-step call) are captured into a CUDA graph on the first
-    call with a given argument set and replayed afterwards.  The replays must give the oracle's answer for the CURRENT
+    """Small systems (the hybrid scheme's per-step call) are captured into a CUDA graph on the second
+    call with a given argument set (the first only records the set and runs as a plain enqueue) and replayed afterwards.  The replays must give the oracle's answer for the CURRENT
     contents of the buffers (positions are rewritten in place between calls), count as replays, and a different buffer
     must not be served by a stale graph."""
     s = W.replicas_1024x30(n_mol=8) if name == "replicas8" else SYSTEMS[name]()     # 240 atoms in 8 molecules: still "small"
@@ -523,7 +560,7 @@ def test_small_systems_replay_a_captured_graph(torch, B, params, blob8, name):
         assert np.max(np.abs(E.cpu().numpy() - Eo) / per) <= E_TOL_PER_ATOM
         assert np.max(np.abs(F.cpu().numpy() - Fo)) <= F_TOL
         q = (q.astype(np.float64) + rng.normal(0, 0.02, q.shape)).astype(np.float32)
-    assert d.dhp_graph_replays() - r0 == 4                    # the capture call is served by the new graph too
+    assert d.dhp_graph_replays() - r0 == 3                    # first call plain; the capture call is served by the new graph too
     l0 = d.dhp_launch_count()
     d.dhp_ani_energy_forces(pos, s.box, sp, w, mol, E=E, F=F)
     assert d.dhp_launch_count() - l0 >= 6                     # replayed kernels are counted
@@ -563,8 +600,8 @@ def test_graph_replay_of_a_large_system_and_its_switch_off_under_changing_argume
         Eo, Fo = oracle.total_energy_forces(W.System(s.name, q, s.species, s.box, s.mol_offsets, s.n_models), params, blob)
         assert abs(E.item() - Eo[0]) / s.n_atoms <= E_TOL_PER_ATOM and np.max(np.abs(F.cpu().numpy() - Fo)) <= F_TOL
         q = (q.astype(np.float64) + rng.normal(0, 0.02, q.shape)).astype(np.float32)
-    assert d.dhp_graph_replays() - r0 == 3
-    # a new box on every call: a new graph each time, until the library stops capturing
+    assert d.dhp_graph_replays() - r0 == 2                    # first call plain, second captures and replays
+    # a new box on every call: no argument set is ever seen twice, so nothing is captured or replayed
     r1 = d.dhp_graph_replays()
     box = np.array(s.box, dtype=np.float64)
     for it in range(40):
@@ -572,8 +609,38 @@ def test_graph_replay_of_a_large_system_and_its_switch_off_under_changing_argume
         d.dhp_ani_energy_forces(pos, b, sp, w, mol, E=E, F=F)
     torch.cuda.synchronize()
     assert d.dhp_status() == 0
-    assert d.dhp_graph_replays() - r1 < 40                    # it gave up replaying
+    assert d.dhp_graph_replays() - r1 == 0
     Eo, Fo = oracle.total_energy_forces(W.System(s.name, pos.cpu().numpy(), s.species, b, s.mol_offsets, s.n_models), params, blob)
+    assert abs(E.item() - Eo[0]) / s.n_atoms <= E_TOL_PER_ATOM and np.max(np.abs(F.cpu().numpy() - Fo)) <= F_TOL
+    d.close()
+
+
+def test_graph_table_does_not_thrash_under_rotating_buffers(torch, B, params, blob8):
+    """A caller that rotates more position buffers than the table has keys (8), or that gets fresh E / F buffers on every
+    call, never sees the same argument set twice in the table: every call is a plain enqueue, no graph is built and thrown
+    away.  Six rotating buffers fit: from the second round on every call is a replay.  Results are the oracle's either way."""
+    s = SYSTEMS["ligand50"]()
+    blob = blob8[: s.n_models * 7 * W.PARAMS_PER_NET]
+    Eo, Fo = oracle.total_energy_forces(s, params, blob)
+    d = make_ctx(B, s, params)
+    w = d.dhp_weights_load(blob, s.n_models)
+    _, sp, mol = B.to_device(s)
+    E = torch.empty(1, dtype=torch.float64, device="cuda")
+    F = torch.empty((s.n_atoms, 3), dtype=torch.float32, device="cuda")
+    bufs = [torch.from_numpy(s.pos).cuda() for _ in range(10)]
+    r0 = d.dhp_graph_replays()
+    for it in range(30):
+        d.dhp_ani_energy_forces(bufs[it % 10], s.box, sp, w, mol, E=E, F=F)
+    assert d.dhp_graph_replays() - r0 == 0
+    keep = []
+    for it in range(12):                                      # new E / F every call (kept alive: no address comes back)
+        keep.append(d.dhp_ani_energy_forces(bufs[0], s.box, sp, w, mol))
+    assert d.dhp_graph_replays() - r0 == 0
+    for it in range(18):
+        d.dhp_ani_energy_forces(bufs[it % 6], s.box, sp, w, mol, E=E, F=F)
+    torch.cuda.synchronize()
+    assert d.dhp_graph_replays() - r0 == 12
+    assert d.dhp_status() == 0
     assert abs(E.item() - Eo[0]) / s.n_atoms <= E_TOL_PER_ATOM and np.max(np.abs(F.cpu().numpy() - Fo)) <= F_TOL
     d.close()
 

@@ -162,12 +162,16 @@ class _OracleDhp:
             return np.zeros_like(x)
         return M.bond_energy_forces(x, box, md["bonds"], md["k"], md["r0"])[1]
 
-    def dhp_ani_energy_forces_partial(self, pos, box, species, weights, central, mol_offsets=None):
+    def dhp_ani_energy_forces_partial(self, pos, box, species, weights, central, mol_offsets=None, E=None, F=None):
         import torch
         import oracle
         c = np.nonzero(central.numpy())[0].astype(np.int32)
         Ec, Fc, _ = oracle.energy_forces(pos.numpy(), species.numpy(), box, self.params, self.blob, self.n_models, centres=c)
-        return torch.tensor([Ec.sum()], dtype=torch.float64), torch.from_numpy(Fc.copy())
+        Eo, Fo = torch.tensor([Ec.sum()], dtype=torch.float64), torch.from_numpy(Fc.copy())
+        if E is None or F is None:
+            return Eo, Fo
+        E.copy_(Eo); F.copy_(Fo)                            # the caller's buffers, as binding.Dhp fills them
+        return E, F
 
     def dhp_md_open(self, md, pos, vel, box, F_slow, dt, n_inner, lo, hi):
         x, v, w = pos.numpy(), vel.numpy(), md["w"]
