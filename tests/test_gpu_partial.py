@@ -130,3 +130,54 @@ def test_sharded_call_on_a_one_rank_nccl_group(torch, B, params):
         d.close()
     finally:
         dist.destroy_process_group()
+
+
+def test_config4_slab_partial_call_at_full_size(torch, B, params):
+    """The launch configuration a rank of an 8-GPU run executes: configs[3], 98 000 atoms, 8 networks, with
+    the central-atom mask of ONE of 8 spatial slabs - k_pairs skips 7/8 of the cells, the AEV / MLP kernels walk the row
+    tiles of a ragged 12 250-atom subset.  Slabs 0 and 5: E, every force component and the lists of the central atoms
+    against the oracle restricted to the same centres.  Then the same call as shard.ShardedMd issues it on every step:
+    list reuse on, positions rewritten in place, mask kept - third call (reused list, replayed graph) against the oracle."""
+    s = W.make_system(4)
+    blob = W.make_weights(8)
+    d = B.Dhp(s.n_atoms, params=params)
+    w = d.dhp_weights_load(blob, 8)
+    pos, sp, _ = B.to_device(s)
+    d.dhp_nlist_build(pos, s.box, sp)                          # the list handle is a token of the context (include/dhp.h)
+    rows = {rc: oracle.pairs(s.pos, s.box, rc) for rc in (params.rcr, params.rca)}
+    E = torch.empty(1, dtype=torch.float64, device="cuda")
+    F = torch.empty((s.n_atoms, 3), dtype=torch.float32, device="cuda")
+    for r in (0, 5):
+        mask = shard.slab_mask_device(pos, s.box, 8, r)
+        centres = shard.slab_centres(s.pos, s.box, 8, r)
+        assert len(centres) == 12250 and np.array_equal(np.nonzero(mask.cpu().numpy())[0], centres)
+        d.dhp_ani_energy_forces_partial(pos, s.box, sp, w, mask, E=E, F=F)
+        torch.cuda.synchronize()
+        assert d.dhp_status() == 0
+        Ea, Fo, _ = oracle.energy_forces(s.pos, s.species, s.box, params, blob, 8, centres=centres)
+        assert abs(E.item() - Ea.sum()) / len(centres) <= E_TOL_PER_ATOM
+        assert np.max(np.abs(F.cpu().numpy() - Fo)) <= F_TOL
+        # lists of the call: the canonical rows for the central atoms, nothing for the others
+        rp, col, rpa, cola = (a.cpu().numpy() for a in d.dhp_nlist_export())
+        central = np.zeros(s.n_atoms, bool)
+        central[centres] = True
+        for got_rp, got_col, rc in ((rp, col, params.rcr), (rpa, cola, params.rca)):
+            rpo, colo = rows[rc]
+            cnt = np.where(central, np.diff(rpo), 0)
+            assert np.array_equal(np.diff(got_rp.astype(np.int64)), cnt)
+            keep = np.repeat(central, np.diff(rpo))
+            assert np.array_equal(got_col, colo[keep])
+    # list reuse + graph replay + mask together (slab 5's mask, as between two mask refreshes of ShardedMd)
+    d.dhp_set_skin(1.0)
+    r0, g0 = d.dhp_nlist_rebuild_count(), d.dhp_graph_replays()
+    for k in range(3):
+        q = W.jitter(s, 0.01, 900 + k)
+        pos.copy_(torch.from_numpy(q).cuda())
+        d.dhp_ani_energy_forces_partial(pos, s.box, sp, w, mask, E=E, F=F)
+    torch.cuda.synchronize()
+    assert d.dhp_status() == 0
+    assert d.dhp_nlist_rebuild_count() - r0 == 1 and d.dhp_graph_replays() - g0 >= 1
+    Ea, Fo, _ = oracle.energy_forces(q, s.species, s.box, params, blob, 8, centres=centres)
+    assert abs(E.item() - Ea.sum()) / len(centres) <= E_TOL_PER_ATOM
+    assert np.max(np.abs(F.cpu().numpy() - Fo)) <= F_TOL
+    d.close()
