@@ -492,11 +492,21 @@ def main():
                 e["dense_k_tflops"] = dense_flop / (ms * 1e-3) / 1e12     # counts the skipped zero blocks: NOT a utilisation
             return e
 
-        def hbm_entry(name, ms, bytes_per_atom, traffic, note, floor_us=None):
+        def hbm_entry(name, ms, bytes_per_atom, traffic, note, floor_us=None, compact_bytes_per_atom=None):
+            # `frac` divides the survey's per-atom figure (§8(d): fp32 rows with every feature column, 4 x 1008 B + the list
+            # reads) by the kernel time.  The kernel moves less than that: fp16 hi / lo planes of the ACTIVE feature blocks
+            # only (`traffic` is what DRAM saw).  `frac_compacted` uses the survey's second figure, the row without the columns
+            # of absent species.  Neither says how busy the kernel is - these kernels are bound on chip - which is what
+            # `time_over_arithmetic_floor` is for.
             ach = bytes_per_atom * N / (ms * 1e-3) / 1e9
             e = {"kernel": name, "bound": "hbm", "achieved": ach, "peak": pk["hbm_gbs"], "unit": "GB/s",
                  "frac": ach / pk["hbm_gbs"], "traffic": traffic, "ms_per_launch": ms,
-                 "algorithmic_bytes_per_launch": bytes_per_atom * N, "note": note}
+                 "algorithmic_bytes_per_launch": bytes_per_atom * N,
+                 "note": note + "; `frac` counts the survey's dense fp32 row bytes, not the bytes the kernel moves (see `traffic`); "
+                                "the number that says how far the kernel is from its limit is `time_over_arithmetic_floor`"}
+            if compact_bytes_per_atom is not None:
+                e["compacted_bytes_per_launch"] = compact_bytes_per_atom * N
+                e["frac_compacted"] = compact_bytes_per_atom * N / (ms * 1e-3) / 1e9 / pk["hbm_gbs"]
             if floor_us is not None:                                      # the kernel's real floor is arithmetic, not bytes
                 e["arithmetic_floor_us"] = floor_us
                 e["time_over_arithmetic_floor"] = ms * 1e3 / floor_us
@@ -522,8 +532,9 @@ def main():
         # ops per atom at 16 / clk / SM; a5 about twice a2's arithmetic
         kernels += [hbm_entry("nlist (a1: all kernels)", ph["nlist"], 264.0, tr.get("nlist"), "working set is L2-resident; instruction-bound",
                               11.0 * scale_n),
-                    hbm_entry("k_aev_fwd (a2)", ph["aev_fwd"], 4256.0, tr.get("aev_fwd"), "issue-bound; the floor that binds is MUFU, not HBM", 69.0 * scale_n),
-                    hbm_entry("k_aev_bwd + k_unsort_forces (a5)", ph["aev_bwd"], 4268.0, tr.get("aev_bwd"), "issue-bound", 140.0 * scale_n)]
+                    hbm_entry("k_aev_fwd (a2)", ph["aev_fwd"], 4256.0, tr.get("aev_fwd"), "L1 / shared-memory pipe and issue-bound; the floor that binds is MUFU, not HBM", 69.0 * scale_n,
+                              2464.0),
+                    hbm_entry("k_aev_bwd + k_unsort_forces (a5)", ph["aev_bwd"], 4268.0, tr.get("aev_bwd"), "L1 / shared-memory pipe bound", 140.0 * scale_n, 2476.0)]
         if tensor_path:
             roof = dict(max(kernels[:n_mlp_kernels], key=lambda k: k["ms_per_launch"]))          # the dominant kernel of the step
             roof["peak_source"] = f"{pk['source']} {peak_kind} bf16 peak (fp16 operands, same rate); the timed loop is a burst"

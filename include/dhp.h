@@ -21,7 +21,7 @@
  *   - Units are the caller's: Å in, Hartree and Hartree/Å out (F = -dE/dr); no conversion inside.
  *   - Species index 0..6 = H, C, N, O, S, F, Cl.  The layout is fixed at compile time:
  *     16 radial shifts, 32 angular entries per species pair, AEV length 7*16 + 28*32 = 1008,
- *     networks 1008 -> 256 -> 192 -> 160 -> 1 with CELU (BASELINE.json configs[0]).  The angular grid is 8 x 4
+ *     networks 1008 -> 256 -> 192 -> 160 -> 1 with CELU (the published ANI-2x shape).  The angular grid is 8 x 4
  *     (ANI-2x) or 4 x 8 (ANI-1x / ANI-1ccx: species H, C, N, O = 0..3; its 384-entry AEV is the
  *     sub-vector of the 1008 layout that those four species span, and its narrower 384 -> 160 -> 128 -> 96 -> 1
  *     networks are loaded zero-padded into the fixed layout - same results, the cost of the wide shape).
@@ -56,7 +56,7 @@ enum {
 };
 
 /* AEV hyper-parameters (Eqs. 3-5).  NULL in dhp_create = values of
- * BASELINE.json configs[0]: Rcr 5.1, Rca 3.5, EtaR 19.7, EtaA 12.5, Zeta 14.1, CELU alpha 0.1,
+ * the published ANI-2x model: Rcr 5.1, Rca 3.5, EtaR 19.7, EtaA 12.5, Zeta 14.1, CELU alpha 0.1,
  * ShfR = 0.8 + 0.2625 m, ShfA = 0.8 + 0.3375 a, ShfZ = (2k+1) pi/8. */
 typedef struct dhp_params {
     float rcr;        /* radial cutoff R_c of Eq. 3 used in Eq. 4, Å          */
@@ -68,7 +68,7 @@ typedef struct dhp_params {
     float shf_r[DHP_N_SHF_R];   /* R_s of Eq. 4, Å                                              */
     float shf_a[DHP_MAX_SHF_A]; /* R_s of Eq. 5, Å: the first n_shf_a entries                   */
     float shf_z[DHP_MAX_SHF_Z]; /* theta_s of Eq. 5: the first n_shf_z entries                  */
-    int32_t n_shf_a;  /* angular grid of Eq. 5: 8 x 4 (ANI-2x shape, BASELINE.json configs[0]) or 4 x 8 (ANI-1x / ANI-1ccx shape, */
+    int32_t n_shf_a;  /* angular grid of Eq. 5: 8 x 4 (ANI-2x shape) or 4 x 8 (ANI-1x / ANI-1ccx shape,                           */
     int32_t n_shf_z;  /* PAPER.md L87); n_shf_a * n_shf_z = 32 entries per species pair, laid out [a][z]                           */
 } dhp_params;
 
@@ -77,16 +77,20 @@ typedef struct dhp_nlist dhp_nlist;     /* device-resident CSR pair list, owned 
 typedef struct dhp_weights dhp_weights; /* device-resident network parameters, owned by the context */
 
 /* MLP arithmetic, dhp_set_mlp_mode().  AUTO, SIMT, TENSOR and TENSOR_LAYERWISE meet the parity tolerances against the
- * fp64 oracle; TENSOR_FP16 is the opt-in mixed-precision trade of PAPER.md L161 and does not. */
+ * fp64 reference (energy within 1e-6 Hartree/atom, forces within 5e-5 Hartree/Å); TENSOR_FP16 is the opt-in
+ * mixed-precision trade of PAPER.md L161 and does not. */
 enum {
     DHP_MLP_AUTO = 0,   /* tensor path when available, else SIMT                                   */
     DHP_MLP_SIMT = 1,   /* fp32 FFMA GEMMs                                                          */
-    DHP_MLP_TENSOR = 2, /* tcgen05 / TMEM GEMMs, fp16 two-term split operands, fp32 accumulate; the four
-                           middle GEMMs of the chain fused into one kernel (activations stay on chip)   */
+    DHP_MLP_TENSOR = 2, /* tcgen05 / TMEM GEMMs, fp16 two-term split operands (3 MMAs per product), fp32 accumulate.
+                           One fused chain kernel runs every layer forward and the back-propagation down to the
+                           first-layer deltas (AEV planes in, E_i and d1 out; h1, h2, h3 never leave the SM);
+                           one more GEMM turns d1 into dE/dAEV                                                 */
     DHP_MLP_TENSOR_LAYERWISE = 3, /* same arithmetic, one launch per GEMM (bring-up / comparison path)  */
     DHP_MLP_TENSOR_FP16 = 4 /* the fused tensor path with ONE fp16 MMA per product (operands rounded to fp16, fp32
-                               accumulate): the "mixed precision" option of PAPER.md L161.  About 2x faster MLP; force
-                               errors ~1e-3 Hartree/Å, i.e. outside the 5e-5 bar - never selected by AUTO             */
+                               accumulate): the "mixed precision" option of PAPER.md L161.  Measured at 98 000 atoms with
+                               8 networks: MLP phase 1.41 -> 1.16 ms; force errors 3-4e-4 Hartree/Å, i.e. outside the
+                               5e-5 bar - never selected by AUTO                                                      */
 };
 
 /* Phases timed by dhp_profile_* (CUDA events on the context stream). */
@@ -150,8 +154,8 @@ int dhp_set_skin(dhp_ctx* ctx, float skin);
 int64_t dhp_nlist_rebuild_count(dhp_ctx* ctx);
 
 /* Number of directed pairs in the radial (<= rcr) and angular (<= rca) lists.  Synchronises.
- * (SURVEY.md §8(b) proposed these counts as outputs of dhp_nlist_export; they are a call of their own because the
- * caller needs them BEFORE it can allocate the col / col_ang buffers that dhp_nlist_export fills.)
+ * (The counts are a call of their own because the caller needs them BEFORE it can allocate the col / col_ang buffers
+ * that dhp_nlist_export fills.)
  * A dhp_nlist handle is a token of the context that built it: passing it to another context is DHP_E_BADARG. */
 int dhp_nlist_sizes(dhp_ctx* ctx, const dhp_nlist* nl, int64_t* nnz, int64_t* nnz_ang);
 
@@ -213,7 +217,7 @@ int dhp_md_run(dhp_ctx* ctx, dhp_md* md, float* pos, float* vel, const float* bo
                const dhp_weights* weights, int n_models, float dt, int n_inner, int n_steps, double* E_out);
 
 /* One outer step of the same scheme, split at the slow-force evaluation and restricted to the atoms [lo, hi) that a rank
- * OWNS - the building blocks of the multi-GPU MD loop (domain decomposition, PAPER.md L134, L194; SURVEY.md §8(e)):
+ * OWNS - the building blocks of the multi-GPU MD loop (domain decomposition, PAPER.md L134, L194):
  *   dhp_md_open   v += (dt/2) a_slow ; [ v += (d/2) a_fast ; x += d v ; v += (d/2) a_fast ]^n_inner, WITHOUT the last fast
  *                 half kick                                                                          for atoms [lo, hi)
  *   ... the caller all-gathers the new positions, evaluates its partial slow force with

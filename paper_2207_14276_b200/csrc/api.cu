@@ -305,7 +305,6 @@ int dhp_create(dhp_ctx** out, const dhp_params* params, int64_t max_atoms, int64
     if (c->graph_on && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); c->graph_on = false; c->cap_stream = nullptr; }
     { const char* e = getenv("DHP_NO_FWD_SPLIT"); c->no_fwd_split = e && e[0] == '1'; }
     { const char* e = getenv("DHP_TC_FUSE"); c->tc_fuse = (e && e[0] == '0') ? 0 : 1; }
-    { const char* e = getenv("DHP_TC_PAIRS"); c->tc_pairs = (e && e[0] >= '0' && e[0] <= '3') ? e[0] - '0' : 0; }   // cta_group::2 kernels
     { const char* e = getenv("DHP_TC_TWO"); c->tc_two = (e && e[0] >= '0' && e[0] <= '3') ? e[0] - '0' : 2; }   // two row tiles per CTA: B1 by default
     c->cc_major = prop.major;
     c->max_atoms = max_atoms;

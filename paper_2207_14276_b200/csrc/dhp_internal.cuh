@@ -119,8 +119,6 @@ struct Ctx {
     bool no_small_path;    // DHP_NO_SMALL_PATH=1 at dhp_create: small systems also take the general (cell list) path (tests)
     bool no_fwd_split;     // DHP_NO_FWD_SPLIT=1: small systems keep one warp per atom in the AEV forward pass (comparison)
     int tc_fuse;           // 1 (default): G1 runs inside the fused chain kernel (k_mlp_fused); DHP_TC_FUSE=0 keeps G1 + k_mlp_mid as two launches
-    int tc_pairs;          // bit 0: G1, bit 1: B1 run on CTA pairs (tcgen05 cta_group::2); DHP_TC_PAIRS=<bits> in the environment
-                           // at dhp_create overrides the default
     int tc_two;            // bit 0: G1, bit 1: B1 run with two row tiles per CTA sharing each weight K block (k_gemm_tc2) on large
                            // systems; DHP_TC_TWO=<bits> in the environment at dhp_create overrides the default (2: B1 only)
     int64_t launches;

@@ -15,7 +15,7 @@
 // next GEMM fetches its A operand as one contiguous 16 KB cp.async.bulk per plane and K block (descriptor:
 // SWIZZLE_NONE, leading byte offset 2048 = next 8-column group, stride byte offset 128 = next 8 rows).
 // The AEV planes (A of G1) are written in the same tiled layout by the AEV kernel (aev_tiled_off()); the weights (B) of
-// k_gemm_tc / k_gemm_tc2 / k_gemm_pair stay row-major and come in through TMA tensor maps with SWIZZLE_128B, those of the
+// k_gemm_tc / k_gemm_tc2 stay row-major and come in through TMA tensor maps with SWIZZLE_128B, those of the
 // chain kernels (k_mlp_fused, k_mlp_mid) are pre-tiled images fetched with plain bulk copies.
 //
 // Default path (two launches): k_mlp_fused = G1 + G2 + G3 + output layer + B3 + B2 for one (row tile, network) per work item,
@@ -97,7 +97,6 @@ struct TcArgs {
     int out_cols_per_tile;    // output column pitch per column tile (BN, or 192 for the 160-wide d3)
     const unsigned* tile_mask;  // [row tiles] active 64-wide feature blocks (G1: K blocks to visit, B1: N blocks to produce)
     int* sched;               // dynamic tile counter of this launch (zeroed by the host)
-    const int* pair_start;    // pair kernels: [n_clusters + 1] item range of every cluster (k_pair_schedule)
     int ksplit;               // EPI_GRAD only: the K blocks of a tile are split over this many work items (power of two
                               // <= KB) which add their partial results into out_f32 (zeroed by the host) - small systems,
                               // where one tile's 32 sequential K blocks would leave most SMs idle
@@ -894,378 +893,9 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
 }
 
 // ======================================================================================================
-// G1 and B1 on CTA PAIRS (tcgen05 cta_group::2).  profiles/r1e + the single-pass experiment show
-// the one-CTA kernel above at the point where the L2 -> shared-memory fill (96 KB per 64-wide K block of one 128-row
-// tile, 1 536 MMA cycles) and the tensor pipe are both near their limits.  Here two CTAs of a cluster take two
-// adjacent row tiles (same species: groups are aligned to 256 rows, and tile masks are pair-uniform, nlist.cu) and
-// ONE tcgen05.mma.cta_group::2 of M = 256 multiplies both: each CTA stages its own 128 rows of A and only HALF of
-// the weight tile (N/2 rows), so a K block costs 64 KB per SM instead of 96 KB and a third pipeline stage fits.
-//   roles per CTA   warp 0: TMA producer (own A rows, own half of W) -> local full barrier
-//                   warp 1: leader CTA - MMA issuer for the pair; peer CTA - relay: local full barrier -> remote arrive
-//                           on the leader's peer-full barrier (plain bulk copies cannot signal another CTA's barrier)
-//                   warps 2..9: epilogue of the CTA's own 128 rows (own TMEM lanes)
-//   barriers        empty[stage], tfull[acc]: tcgen05.commit multicast to both CTAs; tempty[acc] lives in the leader and
-//                   counts the epilogue warps of both CTAs (the peer's arrive remotely)
-//   schedule        static and cost-balanced (k_pair_schedule): cluster c takes a contiguous range of items; G1 orders them
-//                   pair-major (a pair's AEV tile is reused by its 8 networks out of L2), B1 column-tile-major
-// B1's column tile = up to 4 selected 64-wide feature blocks; the N split gives CTA r the r-th 32-row half of every
-// selected block, so accumulator columns [0, 32 nb) are the first halves and [32 nb, 64 nb) the second halves.
-// ======================================================================================================
-constexpr int P_STAGES = 3;
-constexpr int P_BHALF_BYTES = 128 * BK * 2;                              // 16 KB: half of a 256-row W tile, one plane
-constexpr int P_STAGE_BYTES = 2 * A_PLANE_BYTES + 2 * P_BHALF_BYTES;     // 64 KB
-constexpr int P_MAX_PAIRS = 3072;                                       // pairs whose mask / species are cached in shared memory
-constexpr int P_SMEM_BYTES = P_STAGES * P_STAGE_BYTES + 1024 + 256 + P_MAX_PAIRS * 5;
-
-__device__ __forceinline__ uint32_t cluster_ctarank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
-__device__ __forceinline__ uint32_t cluster_id_x() { uint32_t r; asm volatile("mov.u32 %0, %%clusterid.x;" : "=r"(r)); return r; }
-__device__ __forceinline__ uint32_t n_clusters_x() { uint32_t r; asm volatile("mov.u32 %0, %%nclusterid.x;" : "=r"(r)); return r; }
-__device__ __forceinline__ void cluster_sync_all() {
-    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void mbar_arrive_remote(uint32_t bar, uint32_t cta) {
-    asm volatile("{\n\t.reg .b32 ra;\n\tmapa.shared::cluster.u32 ra, %0, %1;\n\t"
-                 "mbarrier.arrive.shared::cluster.b64 _, [ra];\n\t}" ::"r"(bar), "r"(cta) : "memory");
-}
-// tensor load of a CTA pair: the bytes land in THIS CTA's shared memory, the completion is signalled on the barrier at
-// the same offset in the LEADER CTA (rank 0) - the MMA issuer waits on one barrier for both halves
-__device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar) {
-    asm volatile("{\n\t.reg .b32 rb;\n\tmapa.shared::cluster.u32 rb, %4, 0;\n\t"
-                 "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [rb];\n\t}"
-                 ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar) : "memory");
-}
-// (barriers that receive remote arrivals are waited on with the plain mbar_wait: polling with .acquire.cluster cost
-// 0.05 ms per kernel)
-__device__ __forceinline__ void tmem_alloc2(uint32_t smem_dst, uint32_t cols) {
-    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(cols) : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void tmem_dealloc2(uint32_t taddr, uint32_t cols) {
-    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(cols) : "memory");
-}
-__device__ __forceinline__ void umma2_f16(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "setp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-        ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
-}
-__device__ __forceinline__ void umma2_commit(uint32_t bar) {      // arrives on `bar` in BOTH CTAs of the pair
-    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
-                 ::"r"(bar), "h"((uint16_t)3) : "memory");
-}
-// instruction descriptor of the pair MMA: M = 256 (128 rows per CTA), N = bn
-__device__ __forceinline__ uint32_t make_idesc2(int bn) {
-    return (1u << 4) | ((uint32_t)(bn >> 3) << 17) | ((uint32_t)(256 >> 4) << 24);
-}
-
-// Static, cost-balanced schedule of the pair kernels: items are ordered column tile (major) x row-tile pair, cluster c
-// takes the CONTIGUOUS item range [start[c], start[c+1]) and the boundaries split the total cost evenly.  The cost of an
-// item is known before the launch from the pair's feature-block mask: G1 runs popc(mask) K blocks (same for every
-// network nt), B1 produces min(4, popc - 4 nt) N blocks.  One block; out = [2][ncl + 1] (G1 then B1); scratch holds the
-// running cost prefix of the items.
-__device__ __forceinline__ int pair_item_cost(unsigned mask, int nt, int which) {
-    const int pc = __popc(mask);
-    if (which == 0) return 2 * max(pc, 1) + 1;                           // G1: K blocks + per-item overhead
-    const int nb = min(4, max(pc - 4 * nt, 0));
-    return nb ? 8 * nb + 1 : 0;                                          // B1: N blocks over all of K; skipped items cost nothing
-}
-__global__ void __launch_bounds__(1024)
-k_pair_schedule(const unsigned* __restrict__ tile_mask, const int* __restrict__ sp_start, int n_tiles_g1, int ncl,
-                int* __restrict__ scratch, int* __restrict__ out) {
-    __shared__ int wsum[32];
-    __shared__ int carry_s;
-    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    const int n_pairs = sp_start[NSP] / (2 * BM);
-    for (int which = 0; which < 2; ++which) {
-        const int n_tiles = which == 0 ? n_tiles_g1 : AEV_LD / 256;
-        const int n_items = n_pairs * n_tiles;
-        if (tid == 0) carry_s = 0;
-        __syncthreads();
-        for (int b = 0; b < n_items; b += 1024) {                         // inclusive prefix of the item costs -> scratch
-            const int i = b + tid;
-            int v = 0;
-            if (i < n_items) {                          // G1: pair-major (the 8 networks of a pair back to back: its AEV tile
-                int nt, pr;                             // stays in L2); B1: column-tile-major
-                if (which == 0) { pr = i / n_tiles; nt = i - pr * n_tiles; } else { nt = i / n_pairs; pr = i - nt * n_pairs; }
-                v = pair_item_cost(tile_mask[2 * pr], nt, which);
-            }
-            int x = v;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
-            if (lane == 31) wsum[wid] = x;
-            __syncthreads();
-            if (wid == 0) {
-                int w = wsum[lane];
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(0xffffffffu, w, o); if (lane >= o) w += y; }
-                wsum[lane] = w;
-            }
-            __syncthreads();
-            const int incl = carry_s + (wid ? wsum[wid - 1] : 0) + x;
-            if (i < n_items) scratch[i] = incl;
-            __syncthreads();
-            if (tid == 1023) carry_s = incl;
-            __syncthreads();
-        }
-        const long long total = carry_s;
-        for (int c = tid; c <= ncl; c += 1024) {                          // first item whose prefix reaches the c-th share
-            int lo = 0, hi = n_items;
-            if (c < ncl) {
-                const long long target = total * c / ncl;
-                while (lo < hi) { const int mid = (lo + hi) >> 1; if (scratch[mid] <= target) lo = mid + 1; else hi = mid; }
-                if (c == 0) lo = 0;
-            } else lo = n_items;
-            out[which * (ncl + 1) + c] = lo;
-        }
-        __syncthreads();
-    }
-}
-
-template <int EPI, int CMP>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(TC_THREADS, 1)
-k_gemm_pair(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const TcArgs p) {
-    static_assert((EPI == EPI_CELU && CMP == CMP_K) || (EPI == EPI_GRAD && CMP == CMP_N), "pair kernel: G1 and B1 only");
-    extern __shared__ uint8_t smem_raw[];
-    const uint32_t raw = smem_u32(smem_raw);
-    const uint32_t base = (raw + 1023u) & ~1023u;
-    uint8_t* base_ptr = smem_raw + (base - raw);
-    uint64_t* bars = reinterpret_cast<uint64_t*>(base_ptr + P_STAGES * P_STAGE_BYTES);
-    const uint32_t bar0 = base + P_STAGES * P_STAGE_BYTES;
-    // barrier layout: full[S], empty[S], pfull[S] (leader: the peer's stage is full), tfull[2], tempty[2], then the TMEM word
-    constexpr int NBARS = 3 * P_STAGES + 4;
-    auto full_bar = [&](int s) { return bar0 + 8u * s; };
-    auto empty_bar = [&](int s) { return bar0 + 8u * (P_STAGES + s); };
-    auto pfull_bar = [&](int s) { return bar0 + 8u * (2 * P_STAGES + s); };
-    auto tfull_bar = [&](int s) { return bar0 + 8u * (3 * P_STAGES + s); };
-    auto tempty_bar = [&](int s) { return bar0 + 8u * (3 * P_STAGES + 2 + s); };
-    volatile uint32_t* tmem_word = reinterpret_cast<volatile uint32_t*>(bars + NBARS);
-    // per-pair metadata, read once: the role loops below must not pay a global-memory latency per item (the shared-
-    // memory stages drain in ~2 us, less than two dependent loads)
-    unsigned* s_mask = reinterpret_cast<unsigned*>(base_ptr + P_STAGES * P_STAGE_BYTES + 256);
-    signed char* s_sp = reinterpret_cast<signed char*>(s_mask + P_MAX_PAIRS);
-
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int rank = (int)cluster_ctarank();
-    const int cid = (int)cluster_id_x();
-    const int n_pairs = p.sp_start[NSP] / (2 * BM);          // species groups are aligned to 256 rows
-    const int item_lo = p.pair_start[cid], item_hi = p.pair_start[cid + 1];   // cost-balanced contiguous range (k_pair_schedule)
-    // G1: every operand arrives by a tensor load, which a CTA pair can complete on the leader's barrier directly;
-    // B1's A operand comes by plain bulk copies, which signal only their own CTA: the peer relays (warp 1)
-    constexpr bool DIRECT = CMP == CMP_K;
-    const int KB = (p.K + BK - 1) / BK;
-    const unsigned all_k = KB >= 32 ? 0xffffffffu : ((1u << KB) - 1u);
-
-    if (warp == EPI_WARPS && lane == 0) {
-        for (int s = 0; s < P_STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); mbar_init(pfull_bar(s), 1); }
-        for (int s = 0; s < 2; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), 2 * EPI_WARPS); }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        prefetch_tmap(&tmA);
-        prefetch_tmap(&tmB);
-    }
-    if (warp == EPI_WARPS + 1) tmem_alloc2(smem_u32((const void*)tmem_word), TMEM_COLS);
-    for (int i = threadIdx.x; i < min(n_pairs, P_MAX_PAIRS); i += TC_THREADS) {
-        s_mask[i] = p.tile_mask[2 * i];
-        s_sp[i] = (signed char)max(p.row_species[2 * i * BM], 0);
-    }
-    tc_fence_before();
-    __syncthreads();
-    cluster_sync_all();                                        // both CTAs' barriers exist before anyone signals them
-    tc_fence_after();
-    const uint32_t tmem_base = *tmem_word;
-
-    // tile masks are pair-uniform (nlist.cu), so both CTAs derive the same K blocks / N blocks from the first tile's mask
-    auto pair_mask = [&](int pr) -> unsigned { return pr < P_MAX_PAIRS ? s_mask[pr] : p.tile_mask[2 * pr]; };
-    auto pair_species = [&](int pr) -> int { return pr < P_MAX_PAIRS ? (int)s_sp[pr] : max(p.row_species[2 * pr * BM], 0); };
-    auto k_mask = [&](int pr) -> unsigned {
-        if (CMP != CMP_K) return all_k;
-        const unsigned m = pair_mask(pr);
-        return m ? m : (1u << 14);
-    };
-    auto has_work = [&](int pr, int nt) -> bool { return CMP != CMP_N || 4 * nt < __popc(pair_mask(pr)); };
-
-    if (warp == EPI_WARPS) {
-        // ===== TMA producer: own 128 rows of A, own half of the weight tile =====
-        if (elect_one()) {
-            int stage = 0; uint32_t phase = 0;
-            for (int item = item_lo; item < item_hi; ++item) {
-                const int nt = CMP == CMP_K ? item % p.n_tiles : item / n_pairs, pr = CMP == CMP_K ? item / p.n_tiles : item - nt * n_pairs;
-                if (!has_work(pr, nt)) continue;
-                const int rt = 2 * pr + rank, row0 = rt * BM;
-                const int s = pair_species(pr);
-                int brow = (2 * s) * p.b_rows_per_species;
-                int sel[4] = {0, 0, 0, 0};
-                int nb = 0;
-                uint32_t tx;
-                if (CMP == CMP_N) {
-                    nb = select_blocks(pair_mask(pr), nt, sel);
-                    brow += rank * (KBLK / 2);
-                    tx = 2u * A_PLANE_BYTES + 2u * (uint32_t)nb * (NB_BLOCK_BYTES / 2);
-                } else {
-                    brow += nt * p.b_rows_per_tile + rank * (p.BN / 2);
-                    tx = 2u * A_PLANE_BYTES + 2u * (uint32_t)(p.BN / 2) * BK * 2u;
-                }
-                for (unsigned km = k_mask(pr); km; km &= km - 1u) {
-                    const int kb = __ffs(km) - 1;
-                    mbar_wait(empty_bar(stage), phase ^ 1u);
-                    const uint32_t sa = base + stage * P_STAGE_BYTES;
-                    const uint32_t sb = sa + 2 * A_PLANE_BYTES;
-                    if (DIRECT) {
-                        // all four loads are tensor loads: both CTAs signal the leader's barrier, which expects the bytes of both
-                        if (rank == 0) mbar_expect_tx(full_bar(stage), 2u * tx);
-                        const int ka = p.a_k_off_per_tile * nt + kb * BK;
-                        tma_load_2d_pair(sa, &tmA, ka, row0, full_bar(stage));
-                        tma_load_2d_pair(sa + A_PLANE_BYTES, &tmA, ka, p.a_plane_rows + row0, full_bar(stage));
-                        tma_load_2d_pair(sb, &tmB, kb * BK, brow, full_bar(stage));
-                        tma_load_2d_pair(sb + P_BHALF_BYTES, &tmB, kb * BK, brow + p.b_rows_per_species, full_bar(stage));
-                        if (++stage == P_STAGES) { stage = 0; phase ^= 1u; }
-                        continue;
-                    }
-                    mbar_expect_tx(full_bar(stage), tx);
-                    if (p.a_tiled) {
-                        const int kba = p.a_kb_per_tile * nt + kb;
-                        bulk_load(sa, p.a_tiled + tile_off(p.plane_tiles, p.a_kblocks, 0, rt, kba), A_PLANE_BYTES, full_bar(stage));
-                        bulk_load(sa + A_PLANE_BYTES, p.a_tiled + tile_off(p.plane_tiles, p.a_kblocks, 1, rt, kba), A_PLANE_BYTES,
-                                  full_bar(stage));
-                    } else {
-                        const int ka = p.a_k_off_per_tile * nt + kb * BK;
-                        tma_load_2d(sa, &tmA, ka, row0, full_bar(stage));
-                        tma_load_2d(sa + A_PLANE_BYTES, &tmA, ka, p.a_plane_rows + row0, full_bar(stage));
-                    }
-                    if (CMP == CMP_N) {
-#pragma unroll
-                        for (int j = 0; j < 4; ++j)
-                            if (j < nb) {
-                                tma_load_2d(sb + j * (NB_BLOCK_BYTES / 2), &tmB, kb * BK, brow + sel[j] * KBLK, full_bar(stage));
-                                tma_load_2d(sb + P_BHALF_BYTES + j * (NB_BLOCK_BYTES / 2), &tmB, kb * BK,
-                                            brow + p.b_rows_per_species + sel[j] * KBLK, full_bar(stage));
-                            }
-                    } else {
-                        tma_load_2d(sb, &tmB, kb * BK, brow, full_bar(stage));
-                        tma_load_2d(sb + P_BHALF_BYTES, &tmB, kb * BK, brow + p.b_rows_per_species, full_bar(stage));
-                    }
-                    if (++stage == P_STAGES) { stage = 0; phase ^= 1u; }
-                }
-            }
-        }
-    } else if (warp == EPI_WARPS + 1) {
-        if (elect_one()) {
-            int stage = 0; uint32_t phase = 0;
-            if (rank == 0) {
-                // ===== MMA issuer of the pair =====
-                int acc = 0; uint32_t acc_phase = 0;
-                for (int item = item_lo; item < item_hi; ++item) {
-                    const int nt = CMP == CMP_K ? item % p.n_tiles : item / n_pairs, pr = CMP == CMP_K ? item / p.n_tiles : item - nt * n_pairs;
-                    if (!has_work(pr, nt)) continue;
-                    int bn = p.BN;
-                    if (CMP == CMP_N) bn = KBLK * min(4, __popc(pair_mask(pr)) - 4 * nt);
-                    const uint32_t idesc = make_idesc2(bn);
-                    mbar_wait(tempty_bar(acc), acc_phase ^ 1u);
-                    tc_fence_after();
-                    const uint32_t d_tmem = tmem_base + (uint32_t)(acc * ACC_STRIDE);
-                    uint32_t accumulate = 0u;
-                    for (unsigned km = k_mask(pr); km; km &= km - 1u) {
-                        const int kb = __ffs(km) - 1;
-                        mbar_wait(full_bar(stage), phase);
-                        if (!DIRECT) mbar_wait(pfull_bar(stage), phase);
-                        tc_fence_after();
-                        const uint32_t sa = base + stage * P_STAGE_BYTES;
-                        const bool tiled = p.a_tiled != nullptr;
-                        const uint64_t a_hi = tiled ? make_smem_desc_tiled(sa) : make_smem_desc(sa);
-                        const uint64_t a_lo = tiled ? make_smem_desc_tiled(sa + A_PLANE_BYTES) : make_smem_desc(sa + A_PLANE_BYTES);
-                        const uint64_t b_hi = make_smem_desc(sa + 2 * A_PLANE_BYTES);
-                        const uint64_t b_lo = make_smem_desc(sa + 2 * A_PLANE_BYTES + P_BHALF_BYTES);
-                        const uint64_t a_step = tiled ? (uint64_t)(4096 >> 4) : 2u;
-                        const int ksteps = min(BK / 16, (p.K - kb * BK) / 16);
-                        for (int k = 0; k < ksteps; ++k) {
-                            const uint64_t adv = (uint64_t)(k * 2), a_adv = (uint64_t)k * a_step;
-                            umma2_f16(d_tmem, a_hi + a_adv, b_hi + adv, idesc, accumulate);
-                            if (!p.single) {
-                                umma2_f16(d_tmem, a_hi + a_adv, b_lo + adv, idesc, 1u);
-                                umma2_f16(d_tmem, a_lo + a_adv, b_hi + adv, idesc, 1u);
-                            }
-                            accumulate = 1u;
-                        }
-                        umma2_commit(empty_bar(stage));                // frees the stage in both CTAs when the MMAs retire
-                        if (++stage == P_STAGES) { stage = 0; phase ^= 1u; }
-                    }
-                    umma2_commit(tfull_bar(acc));                      // accumulator complete -> both epilogues
-                    if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
-                }
-            } else if (!DIRECT) {
-                // ===== relay: this CTA's stage is full -> tell the leader's MMA issuer =====
-                for (int item = item_lo; item < item_hi; ++item) {
-                    const int nt = CMP == CMP_K ? item % p.n_tiles : item / n_pairs, pr = CMP == CMP_K ? item / p.n_tiles : item - nt * n_pairs;
-                    if (!has_work(pr, nt)) continue;
-                    for (unsigned km = k_mask(pr); km; km &= km - 1u) {
-                        mbar_wait(full_bar(stage), phase);
-                        mbar_arrive_remote(pfull_bar(stage), 0u);
-                        if (++stage == P_STAGES) { stage = 0; phase ^= 1u; }
-                    }
-                }
-            }
-        }
-    } else {
-        // ===== epilogue of this CTA's 128 rows (own TMEM lanes) =====
-        const int q = warp & 3, half = warp >> 2;
-        int acc = 0; uint32_t acc_phase = 0;
-        const float kexp = 1.4426950408889634f / p.alpha;
-        for (int item = item_lo; item < item_hi; ++item) {
-            const int nt = CMP == CMP_K ? item % p.n_tiles : item / n_pairs, pr = CMP == CMP_K ? item / p.n_tiles : item - nt * n_pairs;
-            if (!has_work(pr, nt)) continue;
-            const int rt = 2 * pr + rank;
-            const int row = rt * BM + q * 32 + lane;
-            const int s = pair_species(pr);
-            const int ncols = p.n_tiles * p.BN;
-            const int r_in = q * 32 + lane;
-            int sel[4] = {0, 0, 0, 0};
-            int bn = p.BN, nb = 0;
-            if (CMP == CMP_N) { nb = select_blocks(pair_mask(pr), nt, sel); bn = KBLK * nb; }
-            mbar_wait(tfull_bar(acc), acc_phase);
-            tc_fence_after();
-            const uint32_t t_row = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * ACC_STRIDE);
-            for (int c0 = half * 32; c0 < bn; c0 += 64) {
-                uint32_t v[32];
-                tmem_ld32_issue(t_row + (uint32_t)c0, v);
-                if (EPI == EPI_CELU) {
-                    const int col = nt * p.BN + c0;
-                    float x[32], aux[32];
-                    load32(p.bias + (size_t)s * ncols + col, aux);
-                    const int ocol = nt * p.out_cols_per_tile + c0;
-                    const size_t in_tile = (size_t)(((ocol & 63) >> 3) * BM + r_in) * 8;
-                    const size_t o_hi = tile_off(p.plane_tiles, p.out_kblocks, 0, rt, ocol >> 6) + in_tile;
-                    const size_t o_lo = tile_off(p.plane_tiles, p.out_kblocks, 1, rt, ocol >> 6) + in_tile;
-                    tmem_ld_wait();
-#pragma unroll
-                    for (int i = 0; i < 32; ++i) x[i] = celu_f(fmaf(__uint_as_float(v[i]), p.acc_scale, aux[i]), p.alpha, kexp);
-                    store_split32_tiled(x, p.out_planes + o_hi, p.out_planes + o_lo);
-                } else {   // EPI_GRAD: chunk cc < nb is the first half of selected block cc, chunk nb + j the second half of block j
-                    const int cc = c0 >> 5;
-                    const int j = cc < nb ? cc : cc - nb;
-                    const int blk = j == 0 ? sel[0] : j == 1 ? sel[1] : j == 2 ? sel[2] : sel[3];
-                    const int gcol = blk * KBLK + (cc < nb ? 0 : KBLK / 2);
-                    float4* dst = reinterpret_cast<float4*>(p.out_f32 + (size_t)row * p.out_ld + gcol);
-                    tmem_ld_wait();
-#pragma unroll
-                    for (int i = 0; i < 8; ++i)
-                        dst[i] = make_float4(__uint_as_float(v[4 * i]) * p.acc_scale, __uint_as_float(v[4 * i + 1]) * p.acc_scale,
-                                             __uint_as_float(v[4 * i + 2]) * p.acc_scale, __uint_as_float(v[4 * i + 3]) * p.acc_scale);
-                }
-            }
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) {
-                if (rank == 0) mbar_arrive(tempty_bar(acc));
-                else mbar_arrive_remote(tempty_bar(acc), 0u);
-            }
-            if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
-        }
-    }
-    tc_fence_before();
-    __syncthreads();
-    cluster_sync_all();                                        // nobody leaves while the peer may still signal or read
-    if (warp == EPI_WARPS + 1) tmem_dealloc2(tmem_base, TMEM_COLS);
-}
+// (A cta_group::2 variant of G1 / B1 - k_gemm_pair: two row tiles per MMA, half of the weight tile per CTA, cost-balanced
+// static schedule - lived here in rounds 1-2.  Measured twice, never faster than k_gemm_tc2: removed in round 3; the
+// measurements are in DESIGN.md §6.3.)
 
 // ======================================================================================================
 // Fused middle of the chain.  G2, G3, B3 and B2 are small GEMMs whose split-fp16 activations (4 B per element)
@@ -2572,8 +2202,6 @@ struct TcWorkspace {                  // per context
     int h1_models;                                 // h1 likewise (allocated only where it is an HBM operand); 0 = not allocated
     int lw_models;                                 // h2 / d3 / d2 (layer-by-layer mode only) likewise; 0 = not allocated
     CUtensorMap m_aev;
-    int* pair_sched;                               // [2][n_clusters + 1] item ranges of the pair kernels (G1, B1)
-    int* pair_scratch;                             // [max_rows / 256 * MAX_MODELS] cost prefix scratch of k_pair_schedule
     __half* fscratch;                              // [SMs][FU_SCRATCH] h1 scratch tiles of k_mlp_fused (L2-resident)
 };
 struct TcWeights {                    // per weight handle
@@ -2582,7 +2210,6 @@ struct TcWeights {                    // per weight handle
     __half* w1img;                                  // k_mlp_fused W1 images [species][network][64 K steps][FU_W1_STEP]
     float *b1, *b2, *b3, *w4, *b4;
     CUtensorMap m_w1f, m_w2f, m_w3f, m_w3b, m_w2b, m_w1b;
-    CUtensorMap m_w1f_half, m_w1b_half;             // the pair kernels' boxes: 128 rows of W1 (G1), 32 rows of W1^T (B1)
 };
 
 template <int EPI, int CMP>
@@ -2594,12 +2221,6 @@ int launch_gemm(Ctx* ctx, const CUtensorMap& a, const CUtensorMap& b, const TcAr
 template <int EPI, int CMP>
 int launch_gemm2(Ctx* ctx, const CUtensorMap& a, const CUtensorMap& b, const TcArgs& args) {
     DHP_LAUNCH(ctx, (k_gemm_tc2<EPI, CMP>), ctx->sm_count, TC_THREADS, T2_SMEM, a, b, args);
-    return DHP_OK;
-}
-
-template <int EPI, int CMP>
-int launch_pair(Ctx* ctx, const CUtensorMap& a, const CUtensorMap& b, const TcArgs& args) {
-    DHP_LAUNCH(ctx, (k_gemm_pair<EPI, CMP>), ctx->sm_count & ~1, TC_THREADS, P_SMEM_BYTES, a, b, args);
     return DHP_OK;
 }
 
@@ -2620,7 +2241,6 @@ int mlp_tc_alloc(Ctx* ctx) {
         (rc = set_smem_tc<EPI_OUT, CMP_NONE>(ctx)) != DHP_OK || (rc = set_smem_tc<EPI_DCELU, CMP_NONE>(ctx)) != DHP_OK ||
         (rc = set_smem_tc<EPI_GRAD, CMP_N>(ctx)) != DHP_OK)
         return rc;
-    DHP_CUDA(ctx, cudaFuncSetAttribute((k_gemm_pair<EPI_GRAD, CMP_N>), cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM_BYTES));
     DHP_CUDA(ctx, cudaFuncSetAttribute(k_mlp_mid, cudaFuncAttributeMaxDynamicSharedMemorySize, MID_SMEM));
     DHP_CUDA(ctx, cudaFuncSetAttribute(k_mlp_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, FU_SMEM));
     DHP_CUDA(ctx, cudaFuncSetAttribute((k_gemm_tc2<EPI_CELU, CMP_K>), cudaFuncAttributeMaxDynamicSharedMemorySize, T2_SMEM));
@@ -2633,8 +2253,6 @@ int mlp_tc_alloc(Ctx* ctx) {
     // the activation planes are sized by the ensemble that is actually loaded (mlp_tc_ensure, from dhp_weights_load)
     if (cudaMalloc((void**)&w->aev, 2 * R * AEV_LD * sizeof(__half)) != cudaSuccess) return DHP_E_NOMEM;
     if (cudaMemset(w->aev, 0, 2 * R * AEV_LD * sizeof(__half)) != cudaSuccess) return DHP_E_CUDA;
-    if (cudaMalloc((void**)&w->pair_sched, sizeof(int) * 2 * (ctx->sm_count / 2 + 1)) != cudaSuccess) return DHP_E_NOMEM;
-    if (cudaMalloc((void**)&w->pair_scratch, sizeof(int) * (R / (2 * BM) * MAX_MODELS + 1)) != cudaSuccess) return DHP_E_NOMEM;
     if (cudaMalloc((void**)&w->fscratch, (size_t)ctx->sm_count * FU_SCRATCH * sizeof(__half)) != cudaSuccess) return DHP_E_NOMEM;
     if (cudaMemset(w->fscratch, 0, (size_t)ctx->sm_count * FU_SCRATCH * sizeof(__half)) != cudaSuccess) return DHP_E_CUDA;
     if (!make_map(&w->m_aev, w->aev, 2 * R, AEV_LD, BM)) return DHP_E_CUDA;
@@ -2679,8 +2297,6 @@ void mlp_tc_free(Ctx* ctx) {
     if (!w) return;
     __half* ptrs[] = {w->aev, w->h1, w->h2, w->d3, w->d2, w->d1};
     for (__half* p : ptrs) if (p) cudaFree(p);
-    if (w->pair_sched) cudaFree(w->pair_sched);
-    if (w->pair_scratch) cudaFree(w->pair_scratch);
     if (w->fscratch) cudaFree(w->fscratch);
     delete w;
     ctx->tc_ws = nullptr;
@@ -2703,8 +2319,6 @@ int mlp_tc_weights(Ctx* ctx, Weights* wt) {
         DHP_LAUNCH(ctx, k_prep_weights, dim3(256, NSP), 256, 0, wt->blob, M, m.mode, m.rows, m.cols, *m.p);
         if (!make_map(m.m, *m.p, (uint64_t)2 * NSP * m.rows, m.cols, m.box_rows)) return DHP_E_CUDA;
     }
-    if (!make_map(&t->m_w1f_half, t->w1f, (uint64_t)2 * NSP * M * H1, AEV_LD, 128u)) return DHP_E_CUDA;
-    if (!make_map(&t->m_w1b_half, t->w1b, (uint64_t)2 * NSP * AEV_LD, (uint64_t)M * H1, (uint32_t)(KBLK / 2))) return DHP_E_CUDA;
     if (cudaMalloc((void**)&t->wmid, (size_t)NSP * M * MID_W_TOTAL * sizeof(__half)) != cudaSuccess) return DHP_E_NOMEM;
     DHP_LAUNCH(ctx, k_prep_mid, dim3(64, NSP * M), 256, 0, wt->blob, M, t->wmid);
     if (cudaMalloc((void**)&t->w1img, (size_t)NSP * M * (AEV_LD / 16) * FU_W1_STEP * sizeof(__half)) != cudaSuccess) return DHP_E_NOMEM;
@@ -2755,20 +2369,11 @@ int mlp_tc(Ctx* ctx, const Weights* wt, bool forward_only) {
     a.out_planes = ws->h1; a.out_kblocks = M * KB1; a.out_cols_per_tile = H1;
     a.sched = ctx->tc_sched + 0;
     const bool fusedp = ctx->mlp_mode != DHP_MLP_TENSOR_LAYERWISE;
-    // B1 on CTA pairs (cta_group::2).  The pair kernel's G1 instantiation fetched row-major AEV planes with tensor TMA; the planes
-    // are now in the tiled operand layout and that experiment (measured equal to the one-CTA kernel) is retired:
-    // bit 0 of DHP_TC_PAIRS is ignored
-    const bool pairs = false, pairs_b1 = (ctx->tc_pairs & 2) && fusedp;
-    const int ncl = ctx->sm_count / 2;
-    if (pairs || pairs_b1) {
-        DHP_LAUNCH(ctx, k_pair_schedule, 1, 1024, 0, ctx->tile_mask, ctx->sp_start, M, ncl, ws->pair_scratch, ws->pair_sched);
-        a.pair_start = ws->pair_sched;
-    }
     // two row tiles per CTA (k_gemm_tc2) pay when there are enough tile pairs to keep every SM busy for several items
     const int64_t n_pairs_bound = (ctx->n_atoms + 2 * ROW_TILE - 1) / (2 * ROW_TILE);
     const bool big = n_pairs_bound * M >= 12 * (int64_t)ctx->sm_count;
-    const bool two_g1 = fusedp && !pairs && ((ctx->tc_two & 1) != 0) && big;
-    const bool two_b1 = fusedp && !pairs_b1 && ((ctx->tc_two & 2) != 0) && big;
+    const bool two_g1 = fusedp && ((ctx->tc_two & 1) != 0) && big;
+    const bool two_b1 = fusedp && ((ctx->tc_two & 2) != 0) && big;
     // G1 fused into the front of the middle chain (k_mlp_fused): no G1 launch, h1 never becomes an HBM operand
     const bool fuse1 = fusedp && ctx->tc_fuse != 0;
     if (fuse1) rc = DHP_OK;
@@ -2832,14 +2437,12 @@ int mlp_tc(Ctx* ctx, const Weights* wt, bool forward_only) {
         const int KBt = (M * H1) / BK;                                                       // 4 K blocks per network
         int ks = 1;
         while (ks * 2 <= KBt && KBt % (ks * 2) == 0 && tiles_bound * ks * 2 <= ctx->sm_count) ks *= 2;
-        a.ksplit = (pairs_b1 || two_b1) ? 1 : ks;
+        a.ksplit = two_b1 ? 1 : ks;
         if (a.ksplit > 1)
             DHP_CUDA(ctx, cudaMemsetAsync(ctx->grad, 0, sizeof(float) * (size_t)std::min<int64_t>(tiles_bound * ROW_TILE, ctx->max_rows) * AEV_LD,
                                           ctx->stream));
     }
-    a.pair_start = ws->pair_sched + (ncl + 1);
-    if (pairs_b1) rc = launch_pair<EPI_GRAD, CMP_N>(ctx, ws->m_aev, t->m_w1b_half, a);
-    else if (two_b1) rc = launch_gemm2<EPI_GRAD, CMP_N>(ctx, ws->m_aev, t->m_w1b, a);
+    if (two_b1) rc = launch_gemm2<EPI_GRAD, CMP_N>(ctx, ws->m_aev, t->m_w1b, a);
     else rc = launch_gemm<EPI_GRAD, CMP_N>(ctx, ws->m_aev, t->m_w1b, a);
     if (rc != DHP_OK) return rc;
     DHP_CUDA(ctx, cudaGetLastError());

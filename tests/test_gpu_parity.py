@@ -280,26 +280,6 @@ def test_mixed_precision_mode_error_is_bounded_and_documented(torch, B, params, 
 
 
 @pytest.mark.parametrize("name", ["water96", "mix600", "replicas16"])
-def test_cta_pair_kernels_opt_in(torch, B, params, blob8, name, monkeypatch):
-    """DHP_TC_PAIRS bit 1 runs B1 as a tcgen05 cta_group::2 kernel (two row tiles per MMA, half of the weight tile per
-    CTA, cost-balanced static schedule); bit 0 (G1 on pairs) is retired and ignored.  Same arithmetic as the default kernels,
-    so the same bars apply."""
-    monkeypatch.setenv("DHP_TC_PAIRS", "3")
-    s = SYSTEMS[name]()
-    probe = make_ctx(B, s, params)
-    ok = probe.dhp_tensor_path_available()
-    probe.close()
-    if not ok:
-        pytest.skip("tensor path not available in this build")
-    d, E, F = run_gpu(B, torch, s, params, blob8, B.MLP_TENSOR)
-    Eo, Fo = oracle.total_energy_forces(s, params, blob8[: s.n_models * 7 * W.PARAMS_PER_NET])
-    per = s.n_atoms if s.mol_offsets is None else np.diff(s.mol_offsets)
-    assert np.max(np.abs(E - Eo) / per) <= E_TOL_PER_ATOM
-    assert np.max(np.abs(F - Fo)) <= F_TOL
-    d.close()
-
-
-@pytest.mark.parametrize("name", ["water96", "mix600", "replicas16"])
 def test_two_launch_g1_and_middle_kernels(torch, B, params, blob8, name, monkeypatch):
     """The default tensor path runs G1 inside the fused chain kernel (k_mlp_fused: h1 never becomes an HBM operand).
     DHP_TC_FUSE=0 keeps the earlier pair of launches (G1 = k_gemm_tc with the AEV planes in the tiled operand layout, then
