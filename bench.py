@@ -40,12 +40,12 @@ from paper_2207_14276_b200 import workloads as W  # noqa: E402
 METRIC = "ani_energy_forces_atoms_evals_per_s"
 UNIT = "atoms*evals/s"
 NS_PER_DAY_PER_EVAL_PER_S = 0.5e-6 * 86400.0      # 0.5 fs step
-TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r2_traffic_98k.csv")
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r3_traffic_98k.csv")
 
 
 def traffic_98k():
     """DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per launch at configs[3], read from the committed summary of
-    the `ncu --set full` capture of this same command (profiles/r2_traffic_98k.csv; the README beside it names the command
+    the `ncu --set full` capture of this same command (profiles/r3_traffic_98k.csv; profiles/r3_README.md names the command
     and the commit it was taken at).  Returns {} when the file is missing: `traffic` is then null, never a stale constant."""
     out = {}
     try:
